@@ -1,0 +1,256 @@
+"""CPU oracle for the linear-tree h-adaptation cycle -- TEST INFRASTRUCTURE ONLY.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  The product
+(``paper_2306_06744_b200``) never does, and the two share no code.
+
+The arithmetic lives in ``oracle/lto.cpp`` (plain sequential C++17, pointer tree);
+this file only compiles it with g++ and marshals numpy arrays through ctypes.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "lto.cpp")
+_LIB = os.path.join(_HERE, "liblto.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile oracle/lto.cpp -> oracle/liblto.so (g++, no CUDA)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp.%d" % os.getpid()
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-shared", "-fPIC", _SRC, "-o", tmp])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _p(a, t):
+    return a.ctypes.data_as(C.POINTER(t))
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        L.lto_encode.restype = C.c_uint64
+        L.lto_encode.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_uint32)]
+        L.lto_raw_id.restype = C.c_uint64
+        L.lto_raw_id.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_uint32)]
+        L.lto_decode.restype = None
+        L.lto_decode.argtypes = [C.c_int, C.c_int, C.c_uint64, C.POINTER(C.c_int), C.POINTER(C.c_uint32)]
+        L.lto_sort_linearise.restype = C.c_int64
+        L.lto_sort_linearise.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_uint64), C.c_int64]
+        L.lto_build.restype = C.c_void_p
+        L.lto_build.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int)]
+        L.lto_build_from_keys.restype = C.c_void_p
+        L.lto_build_from_keys.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int),
+                                          C.POINTER(C.c_uint64), C.c_int64]
+        L.lto_free.restype = None
+        L.lto_free.argtypes = [C.c_void_p]
+        L.lto_num_leaves.restype = C.c_int64
+        L.lto_num_leaves.argtypes = [C.c_void_p]
+        L.lto_keys.restype = None
+        L.lto_keys.argtypes = [C.c_void_p, C.POINTER(C.c_uint64)]
+        L.lto_leaf_boxes.restype = None
+        L.lto_leaf_boxes.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_uint32)]
+        L.lto_dfs_is_sorted.restype = C.c_int
+        L.lto_dfs_is_sorted.argtypes = [C.c_void_p]
+        L.lto_adapt.restype = None
+        L.lto_adapt.argtypes = [C.c_void_p, C.POINTER(C.c_int8)]
+        L.lto_balance.restype = C.c_int
+        L.lto_balance.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
+        L.lto_connect.restype = C.c_int
+        L.lto_connect.argtypes = [C.c_void_p, C.c_int]
+        L.lto_face_counts.restype = None
+        L.lto_face_counts.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
+        L.lto_faces.restype = None
+        L.lto_faces.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_uint8),
+                                C.POINTER(C.c_int32), C.POINTER(C.c_uint8),
+                                C.POINTER(C.c_int32), C.POINTER(C.c_uint8),
+                                C.POINTER(C.c_int32), C.POINTER(C.c_uint8)]
+        L.lto_build_map.restype = C.c_int
+        L.lto_build_map.argtypes = [C.c_void_p]
+        L.lto_map.restype = None
+        L.lto_map.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_uint8)]
+        L.lto_num_old_leaves.restype = C.c_int64
+        L.lto_num_old_leaves.argtypes = [C.c_void_p]
+        L.lto_old_keys.restype = None
+        L.lto_old_keys.argtypes = [C.c_void_p, C.POINTER(C.c_uint64)]
+        L.lto_transfer_rows.restype = C.c_int
+        L.lto_transfer_rows.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                        C.c_int, C.c_int, C.c_int64, C.c_int64]
+        L.lto_drop_snapshot.restype = None
+        L.lto_drop_snapshot.argtypes = [C.c_void_p]
+        L.lto_operators.restype = C.c_int
+        L.lto_operators.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_double)]
+        L.lto_gauss_legendre.restype = None
+        L.lto_gauss_legendre.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        _lib = L
+    return _lib
+
+
+# ------------------------------------------------------------------ free functions
+def encode(dim, maxl, level, x):
+    xx = np.zeros(3, np.uint32)
+    xx[:dim] = x[:dim]
+    return int(lib().lto_encode(dim, maxl, level, _p(xx, C.c_uint32)))
+
+
+def raw_id(dim, maxl, level, x):
+    xx = np.zeros(3, np.uint32)
+    xx[:dim] = x[:dim]
+    return int(lib().lto_raw_id(dim, maxl, level, _p(xx, C.c_uint32)))
+
+
+def decode(dim, maxl, key):
+    lvl = C.c_int(0)
+    xx = np.zeros(3, np.uint32)
+    lib().lto_decode(dim, maxl, C.c_uint64(int(key)), C.byref(lvl), _p(xx, C.c_uint32))
+    return lvl.value, tuple(int(v) for v in xx[:dim])
+
+
+def sort_linearise(dim, maxl, keys):
+    k = np.ascontiguousarray(keys, dtype=np.uint64).copy()
+    m = lib().lto_sort_linearise(dim, maxl, _p(k, C.c_uint64), k.size)
+    return k[:m].copy()
+
+
+def gauss_legendre(n):
+    z = np.zeros(n)
+    w = np.zeros(n)
+    lib().lto_gauss_legendre(n, _p(z, C.c_double), _p(w, C.c_double))
+    return z, w
+
+
+def operators(dim, p):
+    """Dense transfer operators: dict(interp[nc,N,N], proj[nc,N,N], mass[N,N], S[nc,N,N])."""
+    nc, N = 1 << dim, (p + 1) ** dim
+    out = {}
+    for which, name, shape in ((0, "interp", (nc, N, N)), (1, "proj", (nc, N, N)),
+                               (2, "mass", (N, N)), (3, "S", (nc, N, N))):
+        a = np.zeros(shape)
+        rc = lib().lto_operators(dim, p, which, _p(a, C.c_double))
+        assert rc == 0
+        out[name] = a
+    return out
+
+
+class OracleError(RuntimeError):
+    pass
+
+
+class Tree:
+    """Pointer-based linear-tree oracle.  Same verbs as the product's C ABI."""
+
+    def __init__(self, dim, base_level, max_level, periodic=None, keys=None):
+        self.dim, self.base, self.maxl = dim, base_level, max_level
+        self.nc, self.nf = 1 << dim, 2 * dim
+        per = np.zeros(3, np.int32)
+        if periodic is not None:
+            per[:dim] = np.asarray(periodic, np.int32)[:dim]
+        if keys is None:
+            self._h = lib().lto_build(dim, base_level, max_level, _p(per, C.c_int))
+        else:
+            k = np.ascontiguousarray(keys, dtype=np.uint64)
+            self._h = lib().lto_build_from_keys(dim, base_level, max_level, _p(per, C.c_int),
+                                                _p(k, C.c_uint64), k.size)
+        if not self._h:
+            raise OracleError("oracle: bad arguments or incomplete key set")
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            lib().lto_free(self._h)
+            self._h = None
+
+    # -- state
+    def num_leaves(self):
+        return int(lib().lto_num_leaves(self._h))
+
+    def keys(self):
+        k = np.zeros(self.num_leaves(), np.uint64)
+        lib().lto_keys(self._h, _p(k, C.c_uint64))
+        return k
+
+    def leaf_boxes(self):
+        """(level[M] int32, xyz[M,3] uint32 integer anchors in finest-cell units)."""
+        M = self.num_leaves()
+        lvl = np.zeros(M, np.int32)
+        xyz = np.zeros((M, 3), np.uint32)
+        lib().lto_leaf_boxes(self._h, _p(lvl, C.c_int32), _p(xyz, C.c_uint32))
+        return lvl, xyz
+
+    def dfs_is_sorted(self):
+        return bool(lib().lto_dfs_is_sorted(self._h))
+
+    # -- the cycle
+    def adapt(self, flags):
+        f = np.ascontiguousarray(flags, dtype=np.int8)
+        assert f.size == self.num_leaves()
+        lib().lto_adapt(self._h, _p(f, C.c_int8))
+
+    def balance(self):
+        ns = C.c_int64(0)
+        it = lib().lto_balance(self._h, C.byref(ns))
+        self.last_balance_splits = ns.value
+        return int(it)
+
+    def connect(self, method=0):
+        rc = lib().lto_connect(self._h, method)
+        if rc != 0:
+            raise OracleError("oracle connect: rc=%d (unbalanced or incomplete tree)" % rc)
+        cnt = np.zeros(3, np.int64)
+        lib().lto_face_counts(self._h, _p(cnt, C.c_int64))
+        M, nf = self.num_leaves(), self.nf
+        F = dict(
+            nbr=np.zeros(M * nf, np.int32), kind=np.zeros(M * nf, np.uint8),
+            conf=np.zeros((int(cnt[0]), 2), np.int32), conf_axis=np.zeros(int(cnt[0]), np.uint8),
+            hang=np.zeros((int(cnt[1]), 2), np.int32), hang_info=np.zeros(int(cnt[1]), np.uint8),
+            bnd=np.zeros(int(cnt[2]), np.int32), bnd_face=np.zeros(int(cnt[2]), np.uint8),
+        )
+        lib().lto_faces(self._h, _p(F["nbr"], C.c_int32), _p(F["kind"], C.c_uint8),
+                        _p(F["conf"], C.c_int32), _p(F["conf_axis"], C.c_uint8),
+                        _p(F["hang"], C.c_int32), _p(F["hang_info"], C.c_uint8),
+                        _p(F["bnd"], C.c_int32), _p(F["bnd_face"], C.c_uint8))
+        F["n_conf"], F["n_hang"], F["n_bnd"] = (int(c) for c in cnt)
+        return F
+
+    def build_map(self):
+        rc = lib().lto_build_map(self._h)
+        if rc != 0:
+            raise OracleError("oracle map: a new leaf is more than one level from the old tree")
+        M = self.num_leaves()
+        src = np.zeros(M, np.int32)
+        kind = np.zeros(M, np.uint8)
+        lib().lto_map(self._h, _p(src, C.c_int32), _p(kind, C.c_uint8))
+        return src, kind
+
+    def old_keys(self):
+        k = np.zeros(int(lib().lto_num_old_leaves(self._h)), np.uint64)
+        lib().lto_old_keys(self._h, _p(k, C.c_uint64))
+        return k
+
+    def transfer_rows(self, u_old, p, nvars, j0, j1):
+        """Rows [j0, j1) of u_new (requires build_map())."""
+        N = (p + 1) ** self.dim
+        u_old = np.ascontiguousarray(u_old, dtype=np.float64)
+        out = np.zeros((j1 - j0, nvars, N))
+        rc = lib().lto_transfer_rows(self._h, _p(u_old, C.c_double), _p(out, C.c_double), p, nvars, j0, j1)
+        if rc != 0:
+            raise OracleError("oracle transfer: rc=%d" % rc)
+        return out
+
+    def transfer(self, u_old, p, nvars):
+        """Alg. 7 map + copy / interpolate / project; consumes the snapshot."""
+        self.build_map()
+        out = self.transfer_rows(u_old, p, nvars, 0, self.num_leaves())
+        lib().lto_drop_snapshot(self._h)
+        return out
+
+    def drop_snapshot(self):
+        lib().lto_drop_snapshot(self._h)

@@ -1,0 +1,927 @@
+// oracle/lto.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// Plain, slow, sequential CPU oracle for the h-adaptation cycle of
+// "An efficient GPU-based h-adaptation framework via linear trees for the flux
+// reconstruction method" (arxiv 2306.06744; citations are PAPER.md:<line>).
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+// reference leg may load this.  It shares no code, header, table or constant
+// generator with the CUDA library (paper_2306_06744_b200/csrc, include/lt.h).
+//
+// Form (BASELINE.json north_star): a pointer-based tree, std::sort, brute-force
+// O(N^2) face adjacency for tiny meshes, point-location descent for large ones,
+// dense mass / projection matrices built by over-integrated Gauss quadrature
+// and solved by Gaussian elimination.  Every function cites the passage it
+// follows; readings of silent/garbled passages are the ones listed in
+// DESIGN.md (section "Readings").
+//
+// Pins (tests/test_oracle_*.py, -m "not gpu"): see DESIGN.md section "Oracle
+// pins".  No function here is "parity unpinned".
+//
+// Build: g++ -O2 -std=c++17 -shared -fPIC oracle/lto.cpp -o oracle/liblto.so
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+constexpr int kLevelBits = 5;  // reading A-2: m_b fixed at 5
+
+struct Node {
+  int level = 0;
+  uint32_t x[3] = {0, 0, 0};  // integer anchor in units of the finest cell
+  Node* child[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  Node* parent = nullptr;
+  int64_t idx = -1;   // position in the sorted leaf array (leaves only)
+  bool mark = false;  // scratch
+  bool is_leaf() const { return child[0] == nullptr; }
+};
+
+struct Faces {
+  std::vector<int32_t> nbr;
+  std::vector<uint8_t> kind;
+  std::vector<int32_t> conf;
+  std::vector<uint8_t> conf_axis;
+  std::vector<int32_t> hang;
+  std::vector<uint8_t> hang_info;
+  std::vector<int32_t> bnd;
+  std::vector<uint8_t> bnd_face;
+};
+
+struct Ops {  // dense transfer operators for one (dim, p)
+  int dim = 0, p = -1, N = 0;
+  std::vector<double> interp;  // [nc][N][N]  child c value n = sum_m interp[c][n][m] * parent m   (Eq. 8)
+  std::vector<double> proj;    // [nc][N][N]  parent n = sum_c sum_m proj[c][n][m] * child c m     (Eq. 12)
+  std::vector<double> mass;    // [N][N]   M   (Eq. 13)
+  std::vector<double> S;       // [nc][N][N] S_c (Eq. 13)
+};
+
+struct Tree {
+  int dim = 2, base = 0, maxl = 0, nc = 4, nf = 4;
+  int periodic[3] = {0, 0, 0};
+  Node* root = nullptr;
+  std::vector<Node*> leaves;   // sorted by Morton ID
+  std::vector<uint64_t> keys;  // their IDs
+  // snapshot of the tree before the last adapt (T_o of Alg. 7)
+  Node* old_root = nullptr;
+  std::vector<Node*> old_leaves;
+  std::vector<uint64_t> old_keys;
+  bool have_old = false;
+  std::vector<int32_t> map_src;
+  std::vector<uint8_t> map_kind;
+  Faces faces;
+  Ops ops;
+};
+
+// ---------------------------------------------------------------- Alg. 1
+// Morton encoding, PAPER.md:92-97 (Alg. 1) with readings A-1..A-3:
+//  step 2: integer coordinates at the octant's own depth, xi = x >> (Dmax - D)
+//  step 3: interleave, digit k = (z_k y_k x_k), x lowest                (:96)
+//  step 4: pad dim*(Dmax - D) zero bits                                  (:97, garbled)
+//  step 5: append the depth in m_b = 5 low bits                          (:97, :142)
+uint64_t raw_id(int dim, int level, const uint32_t* xi_at_level) {
+  uint64_t r = 0;
+  for (int k = 0; k < level; ++k)
+    for (int a = 0; a < dim; ++a)
+      r |= (uint64_t)((xi_at_level[a] >> k) & 1u) << (dim * k + a);
+  return r;  // "raw Morton ID": no padding, no depth
+}
+
+uint64_t encode(int dim, int maxl, int level, const uint32_t* x_finest) {
+  uint32_t xi[3] = {0, 0, 0};
+  for (int a = 0; a < dim; ++a) xi[a] = level == 0 ? 0u : (x_finest[a] >> (maxl - level));
+  uint64_t r = raw_id(dim, level, xi);
+  uint64_t padded = (maxl == level) ? r : (r << (dim * (maxl - level)));
+  return (padded << kLevelBits) | (uint64_t)level;
+}
+
+void decode(int dim, int maxl, uint64_t key, int* level, uint32_t* x_finest) {
+  *level = (int)(key & ((1u << kLevelBits) - 1));
+  uint64_t r = key >> kLevelBits;
+  for (int a = 0; a < 3; ++a) x_finest[a] = 0;
+  for (int k = 0; k < maxl; ++k)
+    for (int a = 0; a < dim; ++a)
+      x_finest[a] |= (uint32_t)((r >> (dim * k + a)) & 1u) << k;
+}
+
+uint64_t key_of(const Tree* t, const Node* n) { return encode(t->dim, t->maxl, n->level, n->x); }
+
+// a is a strict ancestor of b (integer boxes; PAPER.md:84 half-open regions)
+bool contains_strict(int dim, int maxl, int la, const uint32_t* xa, int lb, const uint32_t* xb) {
+  if (la >= lb) return false;
+  uint32_t wa = 1u << (maxl - la);
+  for (int a = 0; a < dim; ++a)
+    if (xb[a] < xa[a] || xb[a] >= xa[a] + wa) return false;
+  return true;
+}
+
+// ---------------------------------------------------------------- tree basics
+void free_subtree(Node* n) {
+  if (!n) return;
+  for (int c = 0; c < 8; ++c) free_subtree(n->child[c]);
+  delete n;
+}
+
+// split: child k has anchor x0 + i*Delta/2, i = bits of k, x lowest (reading A-6)
+void split(Tree* t, Node* n) {
+  uint32_t h = 1u << (t->maxl - n->level - 1);
+  for (int c = 0; c < t->nc; ++c) {
+    Node* ch = new Node();
+    ch->level = n->level + 1;
+    for (int a = 0; a < t->dim; ++a) ch->x[a] = n->x[a] + (((c >> a) & 1) ? h : 0u);
+    ch->parent = n;
+    n->child[c] = ch;
+  }
+}
+
+void merge(Tree* t, Node* n) {
+  for (int c = 0; c < t->nc; ++c) {
+    free_subtree(n->child[c]);
+    n->child[c] = nullptr;
+  }
+}
+
+Node* clone(const Node* n, Node* parent) {
+  Node* m = new Node(*n);
+  m->parent = parent;
+  for (int c = 0; c < 8; ++c)
+    if (n->child[c]) m->child[c] = clone(n->child[c], m);
+  return m;
+}
+
+void dfs_leaves(Tree* t, Node* n, std::vector<Node*>& out) {
+  if (n->is_leaf()) {
+    out.push_back(n);
+    return;
+  }
+  for (int c = 0; c < t->nc; ++c) dfs_leaves(t, n->child[c], out);
+}
+
+// list leaves by depth-first traversal, then std::sort on the 64-bit ID
+void relist(Tree* t) {
+  t->leaves.clear();
+  dfs_leaves(t, t->root, t->leaves);
+  std::vector<std::pair<uint64_t, Node*>> kv;
+  kv.reserve(t->leaves.size());
+  for (Node* n : t->leaves) kv.emplace_back(key_of(t, n), n);
+  std::sort(kv.begin(), kv.end(), [](const auto& a, const auto& b) { return a.first < b.first; });
+  t->keys.resize(kv.size());
+  for (size_t i = 0; i < kv.size(); ++i) {
+    t->keys[i] = kv[i].first;
+    t->leaves[i] = kv[i].second;
+    kv[i].second->idx = (int64_t)i;
+  }
+}
+
+void list_into(Tree* t, Node* root, std::vector<Node*>& lv, std::vector<uint64_t>& ks) {
+  lv.clear();
+  dfs_leaves(t, root, lv);
+  std::sort(lv.begin(), lv.end(), [t](Node* a, Node* b) { return key_of(t, a) < key_of(t, b); });
+  ks.resize(lv.size());
+  for (size_t i = 0; i < lv.size(); ++i) {
+    ks[i] = key_of(t, lv[i]);
+    lv[i]->idx = (int64_t)i;
+  }
+}
+
+// point location: descend from the root towards integer point x, stop at a leaf
+// or at depth `limit`
+Node* locate(Tree* t, Node* root, const uint32_t* x, int limit) {
+  Node* n = root;
+  while (!n->is_leaf() && n->level < limit) {
+    int sh = t->maxl - n->level - 1;
+    int c = 0;
+    for (int a = 0; a < t->dim; ++a) c |= (int)((x[a] >> sh) & 1u) << a;
+    n = n->child[c];
+  }
+  return n;
+}
+
+// same-level face neighbour anchor of `n` across local face f (reading D-1:
+// 0=-x 1=+x 2=-y 3=+y 4=-z 5=+z), periodic wrap of integer coordinates
+// (PAPER.md:267).  Returns false when the face is on a non-periodic boundary.
+bool neighbour_anchor(const Tree* t, const Node* n, int f, uint32_t* nx) {
+  int a = f >> 1;
+  int64_t w = (int64_t)1 << (t->maxl - n->level);
+  int64_t L = (int64_t)1 << t->maxl;
+  for (int b = 0; b < 3; ++b) nx[b] = n->x[b];
+  int64_t v = (int64_t)n->x[a] + ((f & 1) ? w : -w);
+  if (v < 0 || v >= L) {
+    if (!t->periodic[a]) return false;
+    v = (v + L) % L;
+  }
+  nx[a] = (uint32_t)v;
+  return true;
+}
+
+// ---------------------------------------------------------------- Alg. 6
+// Adaptation; readings B-1..B-4.
+//  flags > 0 : refine (ignored at level == max_level)
+//  flags < 0 : coarsen; honoured only when all 2^dim siblings are leaves and all
+//              carry a coarsen flag (steps 3-4) and level > base_level
+//  one level per call.
+void adapt(Tree* t, const int8_t* flags) {
+  // snapshot T_o for Alg. 7
+  free_subtree(t->old_root);
+  t->old_root = clone(t->root, nullptr);
+  list_into(t, t->old_root, t->old_leaves, t->old_keys);
+  t->have_old = true;
+
+  std::vector<Node*> to_refine, to_merge;
+  const int64_t M = (int64_t)t->leaves.size();
+  for (int64_t i = 0; i < M; ++i) {
+    Node* n = t->leaves[i];
+    if (flags[i] > 0 && n->level < t->maxl) to_refine.push_back(n);
+  }
+  for (int64_t i = 0; i < M; ++i) {
+    Node* n = t->leaves[i];
+    Node* p = n->parent;
+    if (!p || p->child[0] != n) continue;  // visit each sibling group once
+    if (n->level <= t->base) continue;
+    bool all = true;
+    for (int c = 0; c < t->nc; ++c) {
+      Node* s = p->child[c];
+      if (!s->is_leaf() || !(flags[s->idx] < 0)) {
+        all = false;
+        break;
+      }
+    }
+    if (all) to_merge.push_back(p);
+  }
+  for (Node* n : to_refine) split(t, n);
+  for (Node* p : to_merge) merge(t, p);
+  relist(t);
+}
+
+// ---------------------------------------------------------------- 2:1 balance
+// PAPER.md:130-147, Alg. 4 (:153-161).  Face balance (reading C-1).  The result
+// is the unique coarsest refinement in which face-adjacent leaves differ by at
+// most one level (reading C-2); it is computed by Jacobi ripple sweeps (reading
+// C-3): in one sweep every leaf L is examined against the tree as it stood at
+// the start of the sweep; every face-neighbour leaf with level < level(L) - 1
+// is marked; all marked leaves are split once.  Returns the number of sweeps
+// that split at least one leaf.
+int balance(Tree* t, int64_t* n_split_total) {
+  int iters = 0;
+  int64_t total = 0;
+  for (;;) {
+    std::vector<Node*> marked;
+    for (Node* L : t->leaves) {
+      for (int f = 0; f < t->nf; ++f) {
+        uint32_t nx[3];
+        if (!neighbour_anchor(t, L, f, nx)) continue;
+        Node* N = locate(t, t->root, nx, L->level);
+        if (N->is_leaf() && N->level < L->level - 1 && !N->mark) {
+          N->mark = true;
+          marked.push_back(N);
+        }
+      }
+    }
+    if (marked.empty()) break;
+    for (Node* N : marked) {
+      N->mark = false;
+      split(t, N);
+    }
+    total += (int64_t)marked.size();
+    ++iters;
+    relist(t);
+  }
+  if (n_split_total) *n_split_total = total;
+  return iters;
+}
+
+// ---------------------------------------------------------------- Alg. 5
+// Face connectivity.  Per (element, face) slot (reading D-2):
+//   kind 0 boundary (nbr -1); 1 conforming; 2 | slot<<4 neighbour coarser;
+//   3 neighbour finer (nbr = the slot-0 fine neighbour).
+// slot (reading D-3) = position of the fine face inside the coarse face,
+// tangential axes ascending, smaller coordinate first.
+// Returns 0, or -1 if a level jump > 1 is met (reading D-5).
+int slot_of(const Tree* t, const Node* fine, const Node* coarse, int axis) {
+  uint32_t wf = 1u << (t->maxl - fine->level);
+  int s = 0, bit = 0;
+  for (int a = 0; a < t->dim; ++a) {
+    if (a == axis) continue;
+    uint32_t rel = (fine->x[a] - coarse->x[a]) / wf;  // 0 or 1: geometric position
+    s |= (int)(rel & 1u) << bit;
+    ++bit;
+  }
+  return s;
+}
+
+int connect_descent(Tree* t, std::vector<int32_t>& nbr, std::vector<uint8_t>& kind) {
+  const int64_t M = (int64_t)t->leaves.size();
+  nbr.assign((size_t)M * t->nf, -1);
+  kind.assign((size_t)M * t->nf, 0);
+  for (int64_t e = 0; e < M; ++e) {
+    Node* L = t->leaves[e];
+    for (int f = 0; f < t->nf; ++f) {
+      uint32_t nx[3];
+      size_t s = (size_t)e * t->nf + f;
+      if (!neighbour_anchor(t, L, f, nx)) continue;  // boundary
+      Node* N = locate(t, t->root, nx, L->level);
+      if (N->is_leaf()) {
+        if (N->level == L->level) {
+          kind[s] = 1;
+          nbr[s] = (int32_t)N->idx;
+        } else if (N->level == L->level - 1) {
+          kind[s] = (uint8_t)(2 | (slot_of(t, L, N, f >> 1) << 4));
+          nbr[s] = (int32_t)N->idx;
+        } else {
+          return -1;
+        }
+      } else {
+        // finer neighbours: the child of N that touches the face and has
+        // tangential bits 0 (reading D-2)
+        int c = (f & 1) ? 0 : (1 << (f >> 1));
+        Node* F = N->child[c];
+        if (!F->is_leaf()) return -1;
+        kind[s] = 3;
+        nbr[s] = (int32_t)F->idx;
+      }
+    }
+  }
+  return 0;
+}
+
+// Brute force over all pairs (tiny meshes): two leaves are face neighbours
+// across axis a iff their integer boxes abut along a (mod domain width if
+// periodic) and overlap with positive (dim-1)-measure in the other axes.
+int connect_bruteforce(Tree* t, std::vector<int32_t>& nbr, std::vector<uint8_t>& kind) {
+  const int64_t M = (int64_t)t->leaves.size();
+  const int64_t Lw = (int64_t)1 << t->maxl;
+  nbr.assign((size_t)M * t->nf, -1);
+  kind.assign((size_t)M * t->nf, 0);
+  for (int64_t e = 0; e < M; ++e) {
+    Node* A = t->leaves[e];
+    int64_t wa = (int64_t)1 << (t->maxl - A->level);
+    for (int f = 0; f < t->nf; ++f) {
+      int ax = f >> 1;
+      size_t s = (size_t)e * t->nf + f;
+      // plane coordinate the neighbour must start/end at
+      int64_t plane = (f & 1) ? (int64_t)A->x[ax] + wa : (int64_t)A->x[ax];
+      bool wrapped = false;
+      if (f & 1) {
+        if (plane == Lw) { plane = 0; wrapped = true; }
+      } else {
+        if (plane == 0) { plane = Lw; wrapped = true; }
+      }
+      if (wrapped && !t->periodic[ax]) continue;  // boundary
+      std::vector<Node*> touching;
+      for (int64_t g = 0; g < M; ++g) {
+        Node* B = t->leaves[g];
+        int64_t wb = (int64_t)1 << (t->maxl - B->level);
+        int64_t bface = (f & 1) ? (int64_t)B->x[ax] : (int64_t)B->x[ax] + wb;
+        if (bface != plane) continue;
+        bool overlap = true;
+        for (int a = 0; a < t->dim; ++a) {
+          if (a == ax) continue;
+          int64_t lo = std::max<int64_t>(A->x[a], B->x[a]);
+          int64_t hi = std::min<int64_t>((int64_t)A->x[a] + wa, (int64_t)B->x[a] + wb);
+          if (hi <= lo) overlap = false;
+        }
+        if (overlap) touching.push_back(B);
+      }
+      if (touching.empty()) return -2;  // incomplete tree
+      if (touching.size() == 1) {
+        Node* B = touching[0];
+        if (B->level == A->level) {
+          kind[s] = 1;
+          nbr[s] = (int32_t)B->idx;
+        } else if (B->level == A->level - 1) {
+          kind[s] = (uint8_t)(2 | (slot_of(t, A, B, ax) << 4));
+          nbr[s] = (int32_t)B->idx;
+        } else {
+          return -1;
+        }
+      } else {
+        if ((int)touching.size() != (1 << (t->dim - 1))) return -1;
+        Node* first = nullptr;
+        for (Node* B : touching) {
+          if (B->level != A->level + 1) return -1;
+          bool is_first = true;  // smallest tangential coordinates
+          for (int a = 0; a < t->dim; ++a)
+            if (a != ax && B->x[a] != A->x[a]) is_first = false;
+          if (is_first) first = B;
+        }
+        if (!first) return -1;
+        kind[s] = 3;
+        nbr[s] = (int32_t)first->idx;
+      }
+    }
+  }
+  return 0;
+}
+
+// Face tables in canonical order (reading D-4): leaves in array order, local
+// faces 0..nf-1; a conforming face is emitted by the element on its minus side
+// (local face odd) as (e, nbr), axis = f>>1; a hanging face by the fine element
+// as (e_fine, e_coarse), info = f | slot<<3; a boundary face by its element.
+void face_tables(Tree* t) {
+  Faces& F = t->faces;
+  F.conf.clear(); F.conf_axis.clear(); F.hang.clear(); F.hang_info.clear();
+  F.bnd.clear(); F.bnd_face.clear();
+  const int64_t M = (int64_t)t->leaves.size();
+  for (int64_t e = 0; e < M; ++e)
+    for (int f = 0; f < t->nf; ++f) {
+      size_t s = (size_t)e * t->nf + f;
+      int k = F.kind[s] & 0xF;
+      if (k == 0) {
+        F.bnd.push_back((int32_t)e);
+        F.bnd_face.push_back((uint8_t)f);
+      } else if (k == 1) {
+        if (f & 1) {
+          F.conf.push_back((int32_t)e);
+          F.conf.push_back(F.nbr[s]);
+          F.conf_axis.push_back((uint8_t)(f >> 1));
+        }
+      } else if (k == 2) {
+        F.hang.push_back((int32_t)e);
+        F.hang.push_back(F.nbr[s]);
+        F.hang_info.push_back((uint8_t)(f | ((F.kind[s] >> 4) << 3)));
+      }
+    }
+}
+
+// ---------------------------------------------------------------- Alg. 7
+// Old/new mapping, computed on the integer boxes: for each
+// new leaf descend the OLD tree towards its anchor:
+//   old leaf, same level      -> kind 0 copy,    src = old index
+//   old leaf, one level above -> kind 1 | child<<4 refine, src = old index
+//   old interior node at the new leaf's level whose children are all leaves
+//                             -> kind 2 coarsen, src = old index of first child
+// anything else -> error (reading: LT_ERR_MAPPING).
+int build_map(Tree* t) {
+  const int64_t M = (int64_t)t->leaves.size();
+  t->map_src.assign((size_t)M, -1);
+  t->map_kind.assign((size_t)M, 0);
+  if (!t->have_old) {  // identity (state rule)
+    for (int64_t j = 0; j < M; ++j) t->map_src[j] = (int32_t)j;
+    return 0;
+  }
+  for (int64_t j = 0; j < M; ++j) {
+    Node* L = t->leaves[j];
+    Node* O = locate(t, t->old_root, L->x, L->level);
+    if (O->is_leaf()) {
+      if (O->level == L->level) {
+        t->map_kind[j] = 0;
+        t->map_src[j] = (int32_t)O->idx;
+      } else if (O->level == L->level - 1) {
+        int sh = t->maxl - L->level;
+        int c = 0;
+        for (int a = 0; a < t->dim; ++a) c |= (int)((L->x[a] >> sh) & 1u) << a;
+        t->map_kind[j] = (uint8_t)(1 | (c << 4));
+        t->map_src[j] = (int32_t)O->idx;
+      } else {
+        return -1;
+      }
+    } else {
+      for (int c = 0; c < t->nc; ++c)
+        if (!O->child[c]->is_leaf()) return -1;
+      for (int c = 1; c < t->nc; ++c)
+        if (O->child[c]->idx != O->child[0]->idx + c) return -1;
+      t->map_kind[j] = 2;
+      t->map_src[j] = (int32_t)O->child[0]->idx;
+    }
+  }
+  return 0;
+}
+
+// ---------------------------------------------------------------- quadrature
+// n-point Gauss-Legendre rule on [-1,1]: Newton iteration on P_n via the
+// three-term recurrence.  Pinned in tests against closed forms (n = 1,2,3),
+// sum of weights and monomial exactness.
+void gauss_legendre(int n, std::vector<double>& z, std::vector<double>& w) {
+  z.assign(n, 0.0);
+  w.assign(n, 0.0);
+  for (int i = 0; i < n; ++i) {
+    double x = -std::cos(M_PI * (i + 0.75) / (n + 0.5));
+    for (int it = 0; it < 100; ++it) {
+      double p0 = 1.0, p1 = x;
+      for (int k = 2; k <= n; ++k) {
+        double pk = ((2.0 * k - 1.0) * x * p1 - (k - 1.0) * p0) / k;
+        p0 = p1;
+        p1 = pk;
+      }
+      if (n == 1) { p0 = 1.0; p1 = x; }
+      double dp = n * (x * p1 - p0) / (x * x - 1.0);
+      double dx = p1 / dp;
+      x -= dx;
+      if (std::fabs(dx) < 1e-16) break;
+    }
+    double p0 = 1.0, p1 = x;
+    for (int k = 2; k <= n; ++k) {
+      double pk = ((2.0 * k - 1.0) * x * p1 - (k - 1.0) * p0) / k;
+      p0 = p1;
+      p1 = pk;
+    }
+    double dp = n * (x * p1 - p0) / (x * x - 1.0);
+    z[i] = x;
+    w[i] = 2.0 / ((1.0 - x * x) * dp * dp);
+  }
+  for (int i = 0; i < n / 2; ++i) {  // symmetrise
+    double s = 0.5 * (z[n - 1 - i] - z[i]);
+    z[i] = -s;
+    z[n - 1 - i] = s;
+    double ww = 0.5 * (w[i] + w[n - 1 - i]);
+    w[i] = w[n - 1 - i] = ww;
+  }
+  if (n % 2) z[n / 2] = 0.0;
+}
+
+// 1-D Lagrange polynomial l_i through nodes z (Eq. 3) at x
+double lagrange(const std::vector<double>& z, int i, double x) {
+  double v = 1.0;
+  for (size_t k = 0; k < z.size(); ++k)
+    if ((int)k != i) v *= (x - z[k]) / (z[i] - z[k]);
+  return v;
+}
+
+// tensor-product Lagrange basis function n (x fastest; reading E-5) at xi
+double tensor_lagrange(const std::vector<double>& z, int dim, int n, const double* xi) {
+  int P1 = (int)z.size();
+  double v = 1.0;
+  for (int a = 0; a < dim; ++a) {
+    v *= lagrange(z, n % P1, xi[a]);
+    n /= P1;
+  }
+  return v;
+}
+
+// Solve A X = B in place (A: n x n, B: n x m, row major), partial pivoting
+void solve_dense(std::vector<double> A, int n, std::vector<double>& B, int m) {
+  for (int k = 0; k < n; ++k) {
+    int piv = k;
+    for (int r = k + 1; r < n; ++r)
+      if (std::fabs(A[(size_t)r * n + k]) > std::fabs(A[(size_t)piv * n + k])) piv = r;
+    if (piv != k) {
+      for (int c = 0; c < n; ++c) std::swap(A[(size_t)k * n + c], A[(size_t)piv * n + c]);
+      for (int c = 0; c < m; ++c) std::swap(B[(size_t)k * m + c], B[(size_t)piv * m + c]);
+    }
+    double d = A[(size_t)k * n + k];
+    for (int r = k + 1; r < n; ++r) {
+      double f = A[(size_t)r * n + k] / d;
+      if (f == 0.0) continue;
+      for (int c = k; c < n; ++c) A[(size_t)r * n + c] -= f * A[(size_t)k * n + c];
+      for (int c = 0; c < m; ++c) B[(size_t)r * m + c] -= f * B[(size_t)k * m + c];
+    }
+  }
+  for (int k = n - 1; k >= 0; --k) {
+    for (int c = 0; c < m; ++c) {
+      double s = B[(size_t)k * m + c];
+      for (int j = k + 1; j < n; ++j) s -= A[(size_t)k * n + j] * B[(size_t)j * m + c];
+      B[(size_t)k * m + c] = s / A[(size_t)k * n + k];
+    }
+  }
+}
+
+// Transfer operators, PAPER.md:204-255 (section 4.2), readings E-1..E-4.
+//  solution points: p+1 Gauss-Legendre points per direction (E-1)
+//  interp[c] : Eq. 8 evaluated at child c's solution points; child c occupies
+//              xi_a in [b_a - 1, b_a] with b_a = (c>>a)&1, i.e.
+//              xi = (z + 2b - 1)/2                                     (:210, :230)
+//  M, S_c    : Eq. 13 by (p+6)-point tensor Gauss quadrature, S_c integrated over
+//              child c's region (reading E-3)
+//  proj[c]   = M^{-1} S_c by dense Gaussian elimination               (Eq. 12)
+void build_ops(Tree* t, int p) {
+  Ops& o = t->ops;
+  if (o.p == p && o.dim == t->dim) return;
+  const int dim = t->dim, nc = t->nc, P1 = p + 1;
+  int N = 1;
+  for (int a = 0; a < dim; ++a) N *= P1;
+  o.dim = dim; o.p = p; o.N = N;
+  std::vector<double> z, w, qz, qw;
+  gauss_legendre(P1, z, w);
+  gauss_legendre(p + 6, qz, qw);
+  const int Q = p + 6;
+  int NQ = 1;
+  for (int a = 0; a < dim; ++a) NQ *= Q;
+
+  o.interp.assign((size_t)nc * N * N, 0.0);
+  for (int c = 0; c < nc; ++c)
+    for (int n = 0; n < N; ++n) {
+      double xi[3];
+      int r = n;
+      for (int a = 0; a < dim; ++a) {
+        int b = (c >> a) & 1;
+        xi[a] = 0.5 * (z[r % P1] + 2.0 * b - 1.0);
+        r /= P1;
+      }
+      for (int m = 0; m < N; ++m)
+        o.interp[((size_t)c * N + n) * N + m] = tensor_lagrange(z, dim, m, xi);
+    }
+
+  // mass matrix over the parent, in parent reference coordinates
+  o.mass.assign((size_t)N * N, 0.0);
+  for (int q = 0; q < NQ; ++q) {
+    double xi[3], wq = 1.0;
+    int r = q;
+    for (int a = 0; a < dim; ++a) {
+      xi[a] = qz[r % Q];
+      wq *= qw[r % Q];
+      r /= Q;
+    }
+    std::vector<double> l(N);
+    for (int n = 0; n < N; ++n) l[n] = tensor_lagrange(z, dim, n, xi);
+    for (int j = 0; j < N; ++j)
+      for (int i = 0; i < N; ++i) o.mass[(size_t)j * N + i] += wq * l[j] * l[i];
+  }
+  // S_c over child c: xi = (zeta + 2b - 1)/2, d xi = 2^-dim d zeta
+  o.S.assign((size_t)nc * N * N, 0.0);
+  const double jac = std::ldexp(1.0, -dim);
+  for (int c = 0; c < nc; ++c)
+    for (int q = 0; q < NQ; ++q) {
+      double zeta[3], xi[3], wq = jac;
+      int r = q;
+      for (int a = 0; a < dim; ++a) {
+        int b = (c >> a) & 1;
+        zeta[a] = qz[r % Q];
+        xi[a] = 0.5 * (zeta[a] + 2.0 * b - 1.0);
+        wq *= qw[r % Q];
+        r /= Q;
+      }
+      std::vector<double> lp(N), lc(N);
+      for (int n = 0; n < N; ++n) {
+        lp[n] = tensor_lagrange(z, dim, n, xi);
+        lc[n] = tensor_lagrange(z, dim, n, zeta);
+      }
+      for (int j = 0; j < N; ++j)
+        for (int i = 0; i < N; ++i) o.S[((size_t)c * N + j) * N + i] += wq * lp[j] * lc[i];
+    }
+  o.proj.assign((size_t)nc * N * N, 0.0);
+  for (int c = 0; c < nc; ++c) {
+    std::vector<double> B(o.S.begin() + (size_t)c * N * N, o.S.begin() + (size_t)(c + 1) * N * N);
+    solve_dense(o.mass, N, B, N);
+    std::copy(B.begin(), B.end(), o.proj.begin() + (size_t)c * N * N);
+  }
+}
+
+// u[e][v][n] (reading E-5).  Rows [j0, j1) of the new tree are produced.
+void transfer_rows(Tree* t, const double* u_old, double* u_new_rows, int nvars, int64_t j0, int64_t j1) {
+  const Ops& o = t->ops;
+  const int N = o.N, nc = t->nc;
+  const size_t E = (size_t)nvars * N;
+  for (int64_t j = j0; j < j1; ++j) {
+    double* dst = u_new_rows + (size_t)(j - j0) * E;
+    int kind = t->map_kind[j] & 0xF;
+    int64_t src = t->map_src[j];
+    if (kind == 0) {
+      std::memcpy(dst, u_old + (size_t)src * E, E * sizeof(double));
+    } else if (kind == 1) {
+      int c = t->map_kind[j] >> 4;
+      const double* I = &o.interp[(size_t)c * N * N];
+      for (int v = 0; v < nvars; ++v) {
+        const double* up = u_old + (size_t)src * E + (size_t)v * N;
+        for (int n = 0; n < N; ++n) {
+          double s = 0.0;
+          for (int m = 0; m < N; ++m) s += I[(size_t)n * N + m] * up[m];
+          dst[(size_t)v * N + n] = s;
+        }
+      }
+    } else {
+      for (int v = 0; v < nvars; ++v)
+        for (int n = 0; n < N; ++n) {
+          double s = 0.0;
+          for (int c = 0; c < nc; ++c) {
+            const double* R = &o.proj[(size_t)c * N * N];
+            const double* uc = u_old + (size_t)(src + c) * E + (size_t)v * N;
+            for (int m = 0; m < N; ++m) s += R[(size_t)n * N + m] * uc[m];
+          }
+          dst[(size_t)v * N + n] = s;
+        }
+    }
+  }
+}
+
+// ---------------------------------------------------------------- Alg. 3
+// Linearisation: reverse, std::unique with the binary
+// predicate "two consecutive Morton IDs are overlapping", reverse back.
+bool overlapping(int dim, int maxl, uint64_t a, uint64_t b) {
+  int la, lb;
+  uint32_t xa[3], xb[3];
+  decode(dim, maxl, a, &la, xa);
+  decode(dim, maxl, b, &lb, xb);
+  if (a == b) return true;
+  return contains_strict(dim, maxl, la, xa, lb, xb) || contains_strict(dim, maxl, lb, xb, la, xa);
+}
+
+int64_t sort_linearise(int dim, int maxl, uint64_t* keys, int64_t n) {
+  std::sort(keys, keys + n);
+  std::reverse(keys, keys + n);
+  uint64_t* e = std::unique(keys, keys + n,
+                            [=](uint64_t a, uint64_t b) { return overlapping(dim, maxl, a, b); });
+  int64_t m = e - keys;
+  std::reverse(keys, keys + m);
+  return m;
+}
+
+bool complete_subtree(const Tree* t, const Node* n) {
+  if (n->is_leaf()) return true;
+  for (int c = 0; c < t->nc; ++c) {
+    if (!n->child[c]) return false;
+    if (!complete_subtree(t, n->child[c])) return false;
+  }
+  return true;
+}
+
+Tree* new_tree(int dim, int base, int maxl, const int* periodic) {
+  if (dim != 2 && dim != 3) return nullptr;
+  if (base < 0 || base > maxl) return nullptr;
+  if (dim * maxl + kLevelBits > 63 || maxl > 31) return nullptr;
+  Tree* t = new Tree();
+  t->dim = dim; t->base = base; t->maxl = maxl;
+  t->nc = 1 << dim; t->nf = 2 * dim;
+  for (int a = 0; a < dim; ++a) t->periodic[a] = periodic ? periodic[a] : 0;
+  t->root = new Node();
+  return t;
+}
+
+void refine_uniform(Tree* t, Node* n, int to_level) {
+  if (n->level >= to_level) return;
+  split(t, n);
+  for (int c = 0; c < t->nc; ++c) refine_uniform(t, n->child[c], to_level);
+}
+
+}  // namespace
+
+// ======================================================================= C ABI
+extern "C" {
+
+typedef struct Tree lto_tree;
+
+uint64_t lto_encode(int dim, int maxl, int level, const uint32_t* x) { return encode(dim, maxl, level, x); }
+uint64_t lto_raw_id(int dim, int maxl, int level, const uint32_t* x) {
+  uint32_t xi[3] = {0, 0, 0};
+  for (int a = 0; a < dim; ++a) xi[a] = level == 0 ? 0u : (x[a] >> (maxl - level));
+  return raw_id(dim, level, xi);
+}
+void lto_decode(int dim, int maxl, uint64_t key, int* level, uint32_t* x) { decode(dim, maxl, key, level, x); }
+
+int64_t lto_sort_linearise(int dim, int maxl, uint64_t* keys, int64_t n) {
+  return sort_linearise(dim, maxl, keys, n);
+}
+
+void* lto_build(int dim, int base, int maxl, const int* periodic) {
+  Tree* t = new_tree(dim, base, maxl, periodic);
+  if (!t) return nullptr;
+  refine_uniform(t, t->root, base);
+  relist(t);
+  return t;
+}
+
+// unsorted keys -> sort + linearise (Alg. 3) -> pointer tree.  Returns NULL if
+// the linearised set does not tile the domain.
+void* lto_build_from_keys(int dim, int base, int maxl, const int* periodic, const uint64_t* keys, int64_t n) {
+  Tree* t = new_tree(dim, base, maxl, periodic);
+  if (!t) return nullptr;
+  std::vector<uint64_t> k(keys, keys + n);
+  int64_t m = sort_linearise(dim, maxl, k.data(), n);
+  for (int64_t i = 0; i < m; ++i) {
+    int lvl;
+    uint32_t x[3];
+    decode(dim, maxl, k[i], &lvl, x);
+    Node* nd = t->root;
+    while (nd->level < lvl) {
+      if (nd->is_leaf()) split(t, nd);
+      int sh = maxl - nd->level - 1;
+      int c = 0;
+      for (int a = 0; a < dim; ++a) c |= (int)((x[a] >> sh) & 1u) << a;
+      nd = nd->child[c];
+    }
+    nd->mark = true;  // a stored leaf
+  }
+  // completeness: every leaf of the pointer tree must be a stored key
+  std::vector<Node*> lv;
+  dfs_leaves(t, t->root, lv);
+  bool ok = (int64_t)lv.size() == m;
+  for (Node* q : lv) {
+    if (!q->mark) ok = false;
+    q->mark = false;
+  }
+  if (!ok) {
+    free_subtree(t->root);
+    delete t;
+    return nullptr;
+  }
+  relist(t);
+  return t;
+}
+
+void lto_free(void* h) {
+  Tree* t = (Tree*)h;
+  if (!t) return;
+  free_subtree(t->root);
+  free_subtree(t->old_root);
+  delete t;
+}
+
+int64_t lto_num_leaves(void* h) { return (int64_t)((Tree*)h)->leaves.size(); }
+void lto_keys(void* h, uint64_t* out) {
+  Tree* t = (Tree*)h;
+  std::memcpy(out, t->keys.data(), t->keys.size() * sizeof(uint64_t));
+}
+// integer anchors (finest units, [M][3]) and levels of the leaves, array order
+void lto_leaf_boxes(void* h, int32_t* level, uint32_t* xyz) {
+  Tree* t = (Tree*)h;
+  for (size_t i = 0; i < t->leaves.size(); ++i) {
+    level[i] = t->leaves[i]->level;
+    for (int a = 0; a < 3; ++a) xyz[3 * i + a] = t->leaves[i]->x[a];
+  }
+}
+// 1 if the DFS order of the pointer tree equals the std::sort order of the IDs
+int lto_dfs_is_sorted(void* h) {
+  Tree* t = (Tree*)h;
+  std::vector<Node*> lv;
+  dfs_leaves(t, t->root, lv);
+  if (lv.size() != t->leaves.size()) return 0;
+  for (size_t i = 0; i < lv.size(); ++i)
+    if (lv[i] != t->leaves[i]) return 0;
+  return 1;
+}
+
+void lto_adapt(void* h, const int8_t* flags) { adapt((Tree*)h, flags); }
+int lto_balance(void* h, int64_t* n_split) { return balance((Tree*)h, n_split); }
+
+// method: 0 = point-location descent, 1 = brute force O(N^2)
+int lto_connect(void* h, int method) {
+  Tree* t = (Tree*)h;
+  int rc = method == 1 ? connect_bruteforce(t, t->faces.nbr, t->faces.kind)
+                       : connect_descent(t, t->faces.nbr, t->faces.kind);
+  if (rc != 0) return rc;
+  face_tables(t);
+  return 0;
+}
+void lto_face_counts(void* h, int64_t* out3) {
+  Tree* t = (Tree*)h;
+  out3[0] = (int64_t)t->faces.conf_axis.size();
+  out3[1] = (int64_t)t->faces.hang_info.size();
+  out3[2] = (int64_t)t->faces.bnd.size();
+}
+void lto_faces(void* h, int32_t* nbr, uint8_t* kind, int32_t* conf, uint8_t* conf_axis, int32_t* hang,
+               uint8_t* hang_info, int32_t* bnd, uint8_t* bnd_face) {
+  Faces& F = ((Tree*)h)->faces;
+  auto cp = [](auto* dst, const auto& v) {
+    if (dst && !v.empty()) std::memcpy(dst, v.data(), v.size() * sizeof(v[0]));
+  };
+  cp(nbr, F.nbr); cp(kind, F.kind); cp(conf, F.conf); cp(conf_axis, F.conf_axis);
+  cp(hang, F.hang); cp(hang_info, F.hang_info); cp(bnd, F.bnd); cp(bnd_face, F.bnd_face);
+}
+
+// Alg. 7.  Returns 0 or -1 (a new leaf more than one level from T_o).
+int lto_build_map(void* h) { return build_map((Tree*)h); }
+void lto_map(void* h, int32_t* src, uint8_t* kind) {
+  Tree* t = (Tree*)h;
+  std::memcpy(src, t->map_src.data(), t->map_src.size() * sizeof(int32_t));
+  std::memcpy(kind, t->map_kind.data(), t->map_kind.size());
+}
+int64_t lto_num_old_leaves(void* h) { return (int64_t)((Tree*)h)->old_keys.size(); }
+void lto_old_keys(void* h, uint64_t* out) {
+  Tree* t = (Tree*)h;
+  std::memcpy(out, t->old_keys.data(), t->old_keys.size() * sizeof(uint64_t));
+}
+
+// Transfer rows [j0, j1) of the new tree (slab-wise so config 5 fits the host).
+// Requires lto_build_map first.  u_old is the whole old array.
+int lto_transfer_rows(void* h, const double* u_old, double* u_new_rows, int p, int nvars, int64_t j0, int64_t j1) {
+  Tree* t = (Tree*)h;
+  if (p < 0 || p > 7 || nvars < 1) return -1;
+  if (t->map_src.size() != t->leaves.size()) return -1;
+  build_ops(t, p);
+  transfer_rows(t, u_old, u_new_rows, nvars, j0, j1);
+  return 0;
+}
+// drop the snapshot (state rule: lt_transfer consumes it)
+void lto_drop_snapshot(void* h) {
+  Tree* t = (Tree*)h;
+  free_subtree(t->old_root);
+  t->old_root = nullptr;
+  t->old_leaves.clear();
+  t->old_keys.clear();
+  t->have_old = false;
+}
+
+// operator access for pins: which = 0 interp[nc][N][N], 1 proj[nc][N][N], 2 mass[N][N], 3 S[nc][N][N]
+int lto_operators(int dim, int p, int which, double* out) {
+  int per[3] = {0, 0, 0};
+  Tree* t = new_tree(dim, 0, 1, per);
+  if (!t) return -1;
+  build_ops(t, p);
+  const std::vector<double>* v = which == 0 ? &t->ops.interp : which == 1 ? &t->ops.proj
+                                 : which == 2 ? &t->ops.mass : &t->ops.S;
+  std::memcpy(out, v->data(), v->size() * sizeof(double));
+  free_subtree(t->root);
+  delete t;
+  return 0;
+}
+void lto_gauss_legendre(int n, double* z, double* w) {
+  std::vector<double> zz, ww;
+  gauss_legendre(n, zz, ww);
+  std::memcpy(z, zz.data(), n * sizeof(double));
+  std::memcpy(w, ww.data(), n * sizeof(double));
+}
+
+}  // extern "C"

@@ -1,0 +1,139 @@
+"""Set-based brute-force model of the tree operations, for pinning the oracle on tiny inputs.
+
+Independent of oracle/lto.cpp in form: no pointer tree, no Morton IDs, no descent.  A mesh
+is a Python set of cells ``(level, ix, iy[, iz])`` with integer coordinates in units of the
+cell's OWN level; neighbours are found by testing set membership of a cell and its
+ancestors; balance is the Jacobi ripple of SURVEY 8(c) written on sets.  Only usable for a
+few thousand cells.
+"""
+from itertools import product
+
+
+def uniform(dim, level):
+    return {(level,) + c for c in product(range(1 << level), repeat=dim)}
+
+
+def children(cell):
+    l, c = cell[0], cell[1:]
+    return [(l + 1,) + tuple(2 * ci + b for ci, b in zip(c, bits))
+            for bits in product((0, 1), repeat=len(c))]
+
+
+def parent(cell):
+    return (cell[0] - 1,) + tuple(ci >> 1 for ci in cell[1:])
+
+
+def containing_leaf(mesh, cell):
+    """The leaf equal to `cell` or an ancestor of it, else None (cell is refined or outside)."""
+    while cell[0] >= 0:
+        if cell in mesh:
+            return cell
+        if cell[0] == 0:
+            return None
+        cell = parent(cell)
+    return None
+
+
+def face_neighbour(cell, axis, sign, periodic):
+    l, c = cell[0], list(cell[1:])
+    c[axis] += sign
+    n = 1 << l
+    if c[axis] < 0 or c[axis] >= n:
+        if not periodic[axis]:
+            return None
+        c[axis] %= n
+    return (l,) + tuple(c)
+
+
+def adapt(mesh, flag_of, base, maxl):
+    """flag_of: dict cell -> -1/0/+1.  One level per call (Alg. 6)."""
+    out = set(mesh)
+    for cell in mesh:
+        if flag_of.get(cell, 0) > 0 and cell[0] < maxl:
+            out.discard(cell)
+            out.update(children(cell))
+    seen = set()
+    for cell in mesh:
+        if cell[0] <= base:
+            continue
+        par = parent(cell)
+        if par in seen:
+            continue
+        seen.add(par)
+        sib = children(par)
+        if all(s in mesh and flag_of.get(s, 0) < 0 for s in sib):
+            for s in sib:
+                out.discard(s)
+            out.add(par)
+    return out
+
+
+def balance(mesh, periodic):
+    """Jacobi ripple; returns (mesh, iters, splits)."""
+    mesh = set(mesh)
+    dim = len(next(iter(mesh))) - 1
+    iters = splits = 0
+    while True:
+        marked = set()
+        for cell in mesh:
+            for axis in range(dim):
+                for sign in (-1, 1):
+                    nb = face_neighbour(cell, axis, sign, periodic)
+                    if nb is None:
+                        continue
+                    leaf = containing_leaf(mesh, nb)
+                    if leaf is not None and leaf[0] < cell[0] - 1:
+                        marked.add(leaf)
+        if not marked:
+            return mesh, iters, splits
+        for m in marked:
+            mesh.discard(m)
+            mesh.update(children(m))
+        iters += 1
+        splits += len(marked)
+
+
+def is_balanced(mesh, periodic):
+    dim = len(next(iter(mesh))) - 1
+    for cell in mesh:
+        for axis in range(dim):
+            for sign in (-1, 1):
+                nb = face_neighbour(cell, axis, sign, periodic)
+                if nb is None:
+                    continue
+                leaf = containing_leaf(mesh, nb)
+                if leaf is not None and leaf[0] < cell[0] - 1:
+                    return False
+    return True
+
+
+def face_census(mesh, periodic):
+    """(n_conf, n_hang, n_bnd) counted from every cell's own faces."""
+    dim = len(next(iter(mesh))) - 1
+    conf2 = hang = bnd = 0
+    for cell in mesh:
+        for axis in range(dim):
+            for sign in (-1, 1):
+                nb = face_neighbour(cell, axis, sign, periodic)
+                if nb is None:
+                    bnd += 1
+                    continue
+                leaf = containing_leaf(mesh, nb)
+                if leaf is None:
+                    continue  # finer neighbours: counted from their side
+                if leaf[0] == cell[0]:
+                    conf2 += 1
+                else:
+                    hang += 1
+    assert conf2 % 2 == 0
+    return conf2 // 2, hang, bnd
+
+
+def volume(mesh, maxl):
+    dim = len(next(iter(mesh))) - 1
+    return sum(1 << (dim * (maxl - c[0])) for c in mesh)
+
+
+def to_cells(level, xyz, dim, maxl):
+    """oracle/GPU leaf boxes (anchor in finest units) -> list of set-model cells, array order."""
+    return [(int(l),) + tuple(int(x) >> (maxl - int(l)) for x in X[:dim]) for l, X in zip(level, xyz)]
