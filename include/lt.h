@@ -1,0 +1,208 @@
+/* lt.h -- C ABI of liblt: the single-GPU h-adaptation cycle over a linear quadtree /
+ * octree (arxiv 2306.06744, "An efficient GPU-based h-adaptation framework via linear
+ * trees for the flux reconstruction method").  Citations are PAPER.md:<line>.
+ *
+ * One adaptation cycle:
+ *     lt_adapt -> lt_balance -> lt_connect -> lt_transfer
+ * on a tree created by lt_build (uniform base tree) or lt_build_from_keys (unsorted,
+ * possibly overlapping keys -> radix sort + linearise, Alg. 3).
+ *
+ * Conventions
+ *   - "device" pointers are CUDA device memory of the GPU that was current when the
+ *     tree was built; "host" pointers are ordinary host memory.
+ *   - Every call enqueues on the CUDA stream given at build time.  Calls that return a
+ *     count or a status detected on the device synchronise that stream (stated per call).
+ *   - Every int-returning call returns LT_OK (0) or a negative lt_status.  No exceptions,
+ *     no aborts, no CPU fallback: without a CUDA device every call fails with LT_ERR_CUDA.
+ *   - The tree owns every device array it hands out (keys, map, face arrays).  Such
+ *     pointers stay valid until the next mutating call on the same tree (lt_adapt,
+ *     lt_balance, lt_connect, lt_transfer, lt_reserve, lt_free).
+ *
+ * Key format (Alg. 1; readings A-1..A-3 of DESIGN.md)
+ *     key = (interleave(x, y[, z]) << 5) | level
+ *   x_a in [0, 2^max_level): integer anchor (minimum corner) in units of the
+ *   finest cell, a multiple of 2^(max_level - level); bit k of axis a sits at interleaved
+ *   position dim*k + a (x lowest); the depth occupies the 5 low bits, so the
+ *   first child of a key is key + 1 (Eq. 7 case 3).  Leaves are stored in
+ *   ascending uint64 order.
+ *
+ * Local face numbering (reading D-1): 0 = -x, 1 = +x, 2 = -y, 3 = +y,
+ * 4 = -z, 5 = +z; the opposite face of f is f ^ 1.
+ */
+#ifndef LT_H_
+#define LT_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lt_tree lt_tree; /* opaque */
+
+typedef enum {
+  LT_OK = 0,
+  LT_ERR_ARG = -1,        /* bad argument (dim, levels, p, nvars, NULL pointer, n too large)       */
+  LT_ERR_CUDA = -2,       /* a CUDA runtime call failed (lt_last_cuda_error gives the code)        */
+  LT_ERR_OOM = -3,        /* device allocation failed                                              */
+  LT_ERR_CAPACITY = -4,   /* a device buffer would overflow and could not be grown                 */
+  LT_ERR_UNBALANCED = -5, /* lt_connect met face neighbours more than one level apart (D-5)        */
+  LT_ERR_MAPPING = -6,    /* lt_transfer met a new leaf more than one level from T_old (Alg. 7)    */
+  LT_ERR_INCOMPLETE = -7  /* lt_build_from_keys: the linearised keys do not tile the domain        */
+} lt_status;
+
+/* Face connectivity (Alg. 5; format = readings D-2..D-4).
+ * All pointers are device memory owned by the tree.  nf = 2*dim.
+ *   nbr[e*nf+f], kind[e*nf+f]  -- the paper's face array F plus a type byte:
+ *     kind & 15 == 0  boundary           nbr = -1
+ *     kind & 15 == 1  conforming         nbr = the same-level neighbour
+ *     kind & 15 == 2  neighbour coarser  nbr = the coarse neighbour; kind >> 4 = slot of
+ *                     this fine face inside the coarse face: the leaf's child-id bits on
+ *                     the tangential axes, ascending axis order, smaller coordinate first
+ *
+ *     kind & 15 == 3  neighbour finer    nbr = the slot-0 fine neighbour
+ *   conf[i] = (e_minus, e_plus), conf_axis[i] in 0..dim-1: one row per conforming face,
+ *     emitted by the element on its minus side (local face odd)
+ *   hang[i] = (e_fine, e_coarse), hang_info[i] = f_fine | slot << 3: one row per fine face
+ *     of a hanging face, emitted by the fine element ("search from the fine side",
+ *     PAPER.md:188)
+ *   bnd[i] = element, bnd_face[i] = local face: one row per boundary face.
+ * Each list is in emission order: leaves in array order, local faces 0..nf-1. */
+typedef struct {
+  int64_t n_leaves, n_conf, n_hang, n_bnd;
+  const int32_t* nbr;
+  const uint8_t* kind;
+  const int32_t* conf;
+  const uint8_t* conf_axis;
+  const int32_t* hang;
+  const uint8_t* hang_info;
+  const int32_t* bnd;
+  const uint8_t* bnd_face;
+} lt_faces;
+
+/* ---- construction ------------------------------------------------------------------ */
+
+/* Uniform tree of 2^(dim*base_level) leaves at depth base_level, written directly in
+ * Morton order (Alg. 1).  dim in {2,3}; 0 <= base_level <= max_level; max_level <= 29
+ * (2-D) / 19 (3-D) so that dim*max_level + 5 <= 63 bits.  base_level is D_min (leaves are
+ * never coarsened above it), max_level is D_max.
+ *   domain   host [2*dim]: lo_x.., hi_x.. -- stored for the caller (lt_domain); the tree
+ *            works on integer coordinates only ("perfect cubes").  May be NULL.
+ *   periodic host [dim]: non-zero = wrap neighbour coordinates on that axis.
+ *            May be NULL (no periodic axis).
+ *   cuda_stream  a cudaStream_t (NULL = the legacy default stream).
+ * Asynchronous. */
+int lt_build(int dim, int base_level, int max_level, const double* domain, const int* periodic,
+             void* cuda_stream, lt_tree** out);
+
+/* Tree from n unsorted device keys (any levels >= base_level; duplicates and ancestors
+ * allowed): LSD radix sort over the used key bits, then linearisation (Alg. 3,
+ * drop duplicates and every key that is an ancestor of its successor).
+ * Fails with LT_ERR_INCOMPLETE if the result does not tile the domain.  Synchronises. */
+int lt_build_from_keys(int dim, int base_level, int max_level, const double* domain,
+                       const int* periodic, void* cuda_stream, const uint64_t* d_keys, int64_t n,
+                       lt_tree** out);
+
+void lt_free(lt_tree*);
+
+/* Make room for `n_leaves` leaves in every tree-owned buffer (buffers also grow on
+ * demand).  Synchronises when it has to reallocate. */
+int lt_reserve(lt_tree*, int64_t n_leaves);
+
+/* ---- the cycle --------------------------------------------------------------------- */
+
+/* Alg. 6: d_flags device int8 [lt_num_leaves], > 0 refine
+ * (ignored at max_level), < 0 coarsen (honoured only for complete sibling groups whose
+ * 2^dim members are all leaves, all flagged < 0, level > base_level).  One level per
+ * call.  Snapshots the pre-adapt keys as T_old (replacing any earlier snapshot).
+ * The new leaves are written in Morton order by an order-preserving expansion (a leaf's
+ * children occupy its Morton interval), so no sort is needed; set
+ * lt_set_option(t, LT_OPT_ADAPT_SORT, 1) to realise it as the paper does (append, radix
+ * sort, linearise) -- same result.  Synchronises once (reads the new leaf count to size
+ * buffers). */
+int lt_adapt(lt_tree*, const int8_t* d_flags);
+
+/* 2:1 face balance (Alg. 4; readings C-1..C-7): the unique coarsest
+ * refinement in which leaves sharing a (dim-1)-face (periodic images included) differ by
+ * at most one level, by Jacobi ripple sweeps run in ONE cooperative kernel (no host round
+ * trip per sweep).  *iters (host, may be NULL) = number of sweeps that split >= 1 leaf.
+ * Synchronises at the end (reads leaf count / status).  On LT_ERR_CAPACITY (growth
+ * impossible) the tree is a valid, partially balanced refinement of the input. */
+int lt_balance(lt_tree*, int* iters);
+
+/* Alg. 5: fills *out (host struct; device arrays inside).
+ * LT_ERR_UNBALANCED if a level jump > 1 is met.  Synchronises. */
+int lt_connect(lt_tree*, lt_faces* out);
+
+/* Alg. 7 + section 4.2: maps T_old -> current tree and moves the
+ * solution: copy (same ID), interpolation of the parent's Lagrange expansion at the
+ * child's solution points (Eq. 8), L2 projection of the 2^dim children (Eq. 9-13).
+ *   d_u_old device [n_old][nvars][N] fp64, d_u_new device [lt_num_leaves][nvars][N] fp64,
+ *   N = (p+1)^dim Gauss-Legendre solution points, x fastest (readings E-1, E-5).
+ *   The arrays must not overlap.  1 <= p+1 <= 8 (p = 0..7), nvars >= 1.
+ * Without a snapshot this is a plain copy.  Drops the snapshot.  Asynchronous; a mapping
+ * error is sticky and is returned by this call only if detected before it returns --
+ * lt_sync reports it otherwise. */
+int lt_transfer(lt_tree*, const double* d_u_old, double* d_u_new, int p, int nvars);
+
+/* Same as lt_transfer with HOST arrays: copies h_u_old in, runs the transfer, copies
+ * h_u_new out (device staging buffers owned by the tree).  Synchronises. */
+int lt_transfer_host(lt_tree*, const double* h_u_old, double* h_u_new, int p, int nvars);
+
+/* ---- accessors --------------------------------------------------------------------- */
+
+int64_t lt_num_leaves(lt_tree*);       /* synchronises only if the count is not cached   */
+int64_t lt_num_old_leaves(lt_tree*);   /* leaves of the snapshot T_old (0 if none)        */
+const uint64_t* lt_keys(lt_tree*);     /* device, sorted                                  */
+const uint64_t* lt_old_keys(lt_tree*); /* device, snapshot (NULL if none)                 */
+
+/* Alg. 7's mapping arrays, valid after lt_transfer until the next mutating call:
+ *   src[j]  old index of the leaf (copy / refined-from) or of the first child (fused-from)
+ *   kind[j] 0 copy; 1 | child_id << 4 refine; 2 coarsen. */
+int lt_map(lt_tree*, const int32_t** d_src, const uint8_t** d_kind);
+
+/* Decode: d_level device int32 [n], d_xyz device uint32 [n][3]
+ * (integer anchors in finest-cell units; unused axes 0).  Asynchronous. */
+int lt_leaf_boxes(lt_tree*, int32_t* d_level, uint32_t* d_xyz);
+
+/* Batch key codec on device arrays (Alg. 1).  d_xyz uint32 [n][3], d_level int32 [n]. */
+int lt_encode(int dim, int max_level, const uint32_t* d_xyz, const int32_t* d_level, int64_t n,
+              uint64_t* d_keys, void* cuda_stream);
+int lt_decode(int dim, int max_level, const uint64_t* d_keys, int64_t n, int32_t* d_level,
+              uint32_t* d_xyz, void* cuda_stream);
+
+/* Ascending LSD radix sort of n device keys in place (8-bit digits over bits
+ * [0, key_bits)), then, if linearise != 0, Alg. 3.  *n_out (host) = resulting count.
+ * Synchronises. */
+int lt_sort_keys(int dim, int max_level, uint64_t* d_keys, int64_t n, int linearise,
+                 int64_t* n_out, void* cuda_stream);
+
+int lt_domain(lt_tree*, double* lo_hi /* host [2*dim] */);
+int lt_info(lt_tree*, int* dim, int* base_level, int* max_level, int* periodic /* host [3] */);
+
+/* Wait for the tree's stream and return (and clear) the sticky device status. */
+int lt_sync(lt_tree*);
+
+typedef enum {
+  LT_OPT_ADAPT_SORT = 1, /* 0 (default): ordered expansion; 1: append + sort + linearise */
+  LT_OPT_BALANCE_FULL_SWEEPS = 2, /* 1: every sweep examines every leaf (debug)         */
+  LT_OPT_DEBUG_BALANCE_SLACK = 3  /* v > 0: lt_balance pretends its buffers hold only n + v
+                                     leaves, to exercise the LT_ERR_CAPACITY retry (tests) */
+} lt_option;
+int lt_set_option(lt_tree*, int option, int value);
+
+/* Per-call device times of the last cycle in milliseconds (CUDA events on the tree's
+ * stream): out[0..3] = adapt, balance, connect, transfer; 0 where not run.
+ * Synchronises. */
+int lt_timings(lt_tree*, float* out4);
+/* Number of kernels liblt launched on this tree since it was built. */
+int64_t lt_launch_count(lt_tree*);
+
+const char* lt_strerror(int status);
+int lt_last_cuda_error(void); /* cudaError_t of the last failing runtime call (this thread) */
+int lt_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LT_H_ */

@@ -1,0 +1,592 @@
+// lt_api.cu -- the C ABI of liblt (include/lt.h): argument checks, buffer management and
+// the sequence of kernel launches behind each call.  Product code; no CPU fallback: every
+// step of the path runs in the kernels of lt_tree.cu / lt_connect.cu / lt_transfer.cu /
+// lt_sort.cu.
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "lt_internal.h"
+
+namespace lt {
+
+thread_local int g_last_cuda_error = 0;
+
+static void free_dev(void* p) {
+  if (p) cudaFree(p);
+}
+
+template <typename T>
+static int alloc_dev(T** p, int64_t count) {
+  *p = nullptr;
+  if (count <= 0) count = 1;
+  LT_CUDA(cudaMalloc((void**)p, (size_t)count * sizeof(T)));
+  return LT_OK;
+}
+
+static int64_t round_cap(int64_t n) { return (n + 1023) / 1024 * 1024; }
+
+// (Re)allocate every per-leaf buffer for `need` leaves, preserving the current keys, the
+// snapshot and both bucket indices.
+static int grow(Tree* t, int64_t need) {
+  if (need <= t->cap) return LT_OK;
+  if (need >= (1ll << 31) - 1024) return LT_ERR_CAPACITY;
+  int64_t cap = round_cap(need + need / 4);
+  if (cap >= (1ll << 31) - 1024) cap = round_cap(need);
+  LT_CUDA(cudaStreamSynchronize(t->stream));
+  const int nf = 2 * t->g.dim;
+  uint64_t* nk[3] = {nullptr, nullptr, nullptr};
+  uint8_t* mark = nullptr;
+  int* fr[2] = {nullptr, nullptr};
+  int32_t* nbr = nullptr;
+  uint8_t* kind = nullptr;
+  int32_t* msrc = nullptr;
+  uint8_t* mkind = nullptr;
+  int rc = LT_OK;
+  for (int b = 0; b < 3 && rc == LT_OK; ++b) rc = alloc_dev(&nk[b], cap);
+  if (rc == LT_OK) rc = alloc_dev(&mark, cap);
+  if (rc == LT_OK) rc = alloc_dev(&fr[0], cap);
+  if (rc == LT_OK) rc = alloc_dev(&fr[1], cap);
+  if (rc == LT_OK) rc = alloc_dev(&nbr, cap * nf);
+  if (rc == LT_OK) rc = alloc_dev(&kind, cap * nf);
+  if (rc == LT_OK) rc = alloc_dev(&msrc, cap);
+  if (rc == LT_OK) rc = alloc_dev(&mkind, cap);
+  if (rc != LT_OK) {
+    for (int b = 0; b < 3; ++b) free_dev(nk[b]);
+    free_dev(mark); free_dev(fr[0]); free_dev(fr[1]); free_dev(nbr); free_dev(kind); free_dev(msrc); free_dev(mkind);
+    return rc;
+  }
+  if (t->keys[t->cur] && t->n_valid && t->n > 0)
+    LT_CUDA(cudaMemcpyAsync(nk[t->cur], t->keys[t->cur], (size_t)t->n * 8, cudaMemcpyDeviceToDevice, t->stream));
+  if (t->keys[t->old] && t->have_old && t->n_old > 0)
+    LT_CUDA(cudaMemcpyAsync(nk[t->old], t->keys[t->old], (size_t)t->n_old * 8, cudaMemcpyDeviceToDevice, t->stream));
+  LT_CUDA(cudaMemsetAsync(mark, 0, (size_t)cap, t->stream));
+  LT_CUDA(cudaStreamSynchronize(t->stream));
+  for (int b = 0; b < 3; ++b) {
+    free_dev(t->keys[b]);
+    t->keys[b] = nk[b];
+  }
+  free_dev(t->mark); t->mark = mark;
+  free_dev(t->frontier[0]); t->frontier[0] = fr[0];
+  free_dev(t->frontier[1]); t->frontier[1] = fr[1];
+  free_dev(t->nbr); t->nbr = nbr;
+  free_dev(t->kind); t->kind = kind;
+  free_dev(t->map_src); t->map_src = msrc;
+  free_dev(t->map_kind); t->map_kind = mkind;
+  t->map_valid = false;
+  t->cap = cap;
+  return LT_OK;
+}
+
+// a face table (rows of `width` int32) and its byte column, grown together
+static int grow_pair(int32_t** rows, uint8_t** bytes, int64_t* cap, int64_t need, int width) {
+  if (need <= *cap && *rows && *bytes) return LT_OK;
+  free_dev(*rows);
+  free_dev(*bytes);
+  *rows = nullptr;
+  *bytes = nullptr;
+  *cap = 0;
+  const int64_t c = round_cap(need + need / 8);
+  int rc = alloc_dev(rows, c * width);
+  if (rc == LT_OK) rc = alloc_dev(bytes, c);
+  if (rc == LT_OK) *cap = c;
+  return rc;
+}
+
+// copy the device scalars to the pinned mirror and wait
+static int fetch_scalars(Tree* t) {
+  LT_CUDA(cudaMemcpyAsync(t->h_s, t->d_s, sizeof(DevScalars), cudaMemcpyDeviceToHost, t->stream));
+  LT_CUDA(cudaStreamSynchronize(t->stream));
+  t->n = t->h_s->n;
+  t->n_valid = true;
+  return LT_OK;
+}
+
+static int take_status(Tree* t) {
+  int st = t->h_s->status;
+  if (st != 0) {
+    cudaMemsetAsync(&t->d_s->status, 0, sizeof(int), t->stream);
+    t->h_s->status = 0;
+  }
+  return st;
+}
+
+static void tic(Tree* t, int which) { cudaEventRecord(t->ev[2 * which], t->stream); }
+static void toc(Tree* t, int which) {
+  cudaEventRecord(t->ev[2 * which + 1], t->stream);
+  t->ev_set[which] = true;
+}
+
+static int new_tree(int dim, int base, int maxl, const double* domain, const int* periodic, void* stream,
+                    Tree** out) {
+  if (!out) return LT_ERR_ARG;
+  *out = nullptr;
+  if (dim != 2 && dim != 3) return LT_ERR_ARG;
+  if (base < 0 || maxl < base) return LT_ERR_ARG;
+  if (dim * maxl + kLevelBits > 63 || maxl > 29) return LT_ERR_ARG;
+  if ((int64_t)dim * base > 30) return LT_ERR_ARG;  // 2^(dim*base) leaves must fit an int32 index
+  int dev = 0;
+  LT_CUDA(cudaGetDevice(&dev));
+  lt_tree* t = new (std::nothrow) lt_tree();
+  if (!t) return LT_ERR_OOM;
+  memset((void*)t, 0, sizeof(lt_tree));
+  t->device = dev;
+  t->stream = (cudaStream_t)stream;
+  cudaError_t e = cudaDeviceGetAttribute(&t->num_sms, cudaDevAttrMultiProcessorCount, dev);
+  if (e != cudaSuccess) {
+    g_last_cuda_error = (int)e;
+    delete t;
+    return LT_ERR_CUDA;
+  }
+  Geo& g = t->g;
+  g.dim = dim;
+  g.base = base;
+  g.maxl = maxl;
+  g.ilevel = base;
+  while (dim * g.ilevel > 24) --g.ilevel;  // bucket index of at most 2^24 cells
+  g.ishift = dim * (maxl - g.ilevel);
+  g.nbuckets = 1 << (dim * g.ilevel);
+  g.periodic = 0;
+  for (int a = 0; a < dim; ++a)
+    if (periodic && periodic[a]) g.periodic |= 1 << a;
+  g.total = (1ull << (dim * maxl)) - 1;
+  for (int a = 0; a < dim; ++a) {
+    t->domain[a] = domain ? domain[a] : 0.0;
+    t->domain[dim + a] = domain ? domain[dim + a] : 1.0;
+  }
+  t->cur = 0;
+  t->old = 1;
+  t->tmp = 2;
+  t->ops_p = -1;
+  int rc = LT_OK;
+  auto fail = [&](int code) {
+    lt_free(t);
+    return code;
+  };
+  for (int b = 0; b < 3; ++b)
+    if ((rc = alloc_dev(&t->first[b], (int64_t)g.nbuckets + 1)) != LT_OK) return fail(rc);
+  if ((rc = alloc_dev(&t->d_s, 1)) != LT_OK) return fail(rc);
+  if ((rc = alloc_dev(&t->d_sums, kMaxGrid)) != LT_OK) return fail(rc);
+  if ((rc = alloc_dev(&t->d_sums3, 3 * kMaxGrid)) != LT_OK) return fail(rc);
+  if (cudaMallocHost((void**)&t->h_s, sizeof(DevScalars)) != cudaSuccess) return fail(LT_ERR_OOM);
+  if (cudaMallocHost((void**)&t->h_sums, (3 * kMaxGrid + 16) * sizeof(unsigned long long)) != cudaSuccess)
+    return fail(LT_ERR_OOM);
+  memset(t->h_s, 0, sizeof(DevScalars));
+  if (cudaMemsetAsync(t->d_s, 0, sizeof(DevScalars), t->stream) != cudaSuccess) return fail(LT_ERR_CUDA);
+  for (int i = 0; i < 8; ++i)
+    if (cudaEventCreate(&t->ev[i]) != cudaSuccess) return fail(LT_ERR_CUDA);
+  *out = t;
+  return LT_OK;
+}
+
+}  // namespace lt
+
+using namespace lt;
+
+extern "C" {
+
+int lt_version(void) { return 100; }
+int lt_last_cuda_error(void) { return g_last_cuda_error; }
+
+const char* lt_strerror(int status) {
+  switch (status) {
+    case LT_OK: return "ok";
+    case LT_ERR_ARG: return "bad argument";
+    case LT_ERR_CUDA: return "CUDA runtime error (no device, or a launch failed)";
+    case LT_ERR_OOM: return "out of device memory";
+    case LT_ERR_CAPACITY: return "device buffer capacity exceeded";
+    case LT_ERR_UNBALANCED: return "tree is not 2:1 face balanced";
+    case LT_ERR_MAPPING: return "a new leaf is more than one level from the old tree";
+    case LT_ERR_INCOMPLETE: return "keys do not tile the domain";
+  }
+  return "unknown status";
+}
+
+void lt_free(lt_tree* t) {
+  if (!t) return;
+  cudaStreamSynchronize(t->stream);
+  for (int b = 0; b < 3; ++b) {
+    free_dev(t->keys[b]);
+    free_dev(t->first[b]);
+  }
+  free_dev(t->d_s); free_dev(t->d_sums); free_dev(t->d_sums3);
+  if (t->h_s) cudaFreeHost(t->h_s);
+  if (t->h_sums) cudaFreeHost(t->h_sums);
+  free_dev(t->mark); free_dev(t->frontier[0]); free_dev(t->frontier[1]);
+  free_dev(t->nbr); free_dev(t->kind);
+  free_dev(t->conf); free_dev(t->conf_axis); free_dev(t->hang); free_dev(t->hang_info);
+  free_dev(t->bnd); free_dev(t->bnd_face);
+  free_dev(t->map_src); free_dev(t->map_kind); free_dev(t->d_ops);
+  free_dev(t->stage_old); free_dev(t->stage_new);
+  free_dev(t->sort_tmp); free_dev(t->sort_hist); free_dev(t->sort_status);
+  for (int i = 0; i < 8; ++i)
+    if (t->ev[i]) cudaEventDestroy(t->ev[i]);
+  delete t;
+}
+
+int lt_build(int dim, int base_level, int max_level, const double* domain, const int* periodic,
+             void* cuda_stream, lt_tree** out) {
+  Tree* t = nullptr;
+  int rc = new_tree(dim, base_level, max_level, domain, periodic, cuda_stream, &t);
+  if (rc != LT_OK) return rc;
+  const int64_t nb = 1ll << (dim * base_level);
+  if ((rc = grow(t, nb * 2)) != LT_OK) {
+    lt_free((lt_tree*)t);
+    return rc;
+  }
+  if ((rc = launch_build_uniform(t)) != LT_OK) {
+    lt_free((lt_tree*)t);
+    return rc;
+  }
+  t->n = nb;
+  t->n_valid = true;
+  *out = (lt_tree*)t;
+  return LT_OK;
+}
+
+int lt_reserve(lt_tree* t, int64_t n_leaves) {
+  if (!t || n_leaves < 0) return LT_ERR_ARG;
+  if (!t->n_valid) {
+    int rc = fetch_scalars(t);
+    if (rc != LT_OK) return rc;
+  }
+  return grow(t, n_leaves);
+}
+
+int64_t lt_num_leaves(lt_tree* t) {
+  if (!t) return LT_ERR_ARG;
+  if (!t->n_valid) {
+    int rc = fetch_scalars(t);
+    if (rc != LT_OK) return rc;
+  }
+  return t->n;
+}
+int64_t lt_num_old_leaves(lt_tree* t) { return t && t->have_old ? t->n_old : 0; }
+const uint64_t* lt_keys(lt_tree* t) { return t ? t->keys[t->cur] : nullptr; }
+const uint64_t* lt_old_keys(lt_tree* t) { return t && t->have_old ? t->keys[t->old] : nullptr; }
+
+int lt_domain(lt_tree* t, double* lo_hi) {
+  if (!t || !lo_hi) return LT_ERR_ARG;
+  for (int a = 0; a < 2 * t->g.dim; ++a) lo_hi[a] = t->domain[a];
+  return LT_OK;
+}
+int lt_info(lt_tree* t, int* dim, int* base_level, int* max_level, int* periodic) {
+  if (!t) return LT_ERR_ARG;
+  if (dim) *dim = t->g.dim;
+  if (base_level) *base_level = t->g.base;
+  if (max_level) *max_level = t->g.maxl;
+  if (periodic)
+    for (int a = 0; a < 3; ++a) periodic[a] = (t->g.periodic >> a) & 1;
+  return LT_OK;
+}
+
+int lt_set_option(lt_tree* t, int option, int value) {
+  if (!t) return LT_ERR_ARG;
+  if (option == LT_OPT_ADAPT_SORT) t->opt_adapt_sort = value != 0;
+  else if (option == LT_OPT_BALANCE_FULL_SWEEPS) t->opt_full_sweeps = value != 0;
+  else if (option == LT_OPT_DEBUG_BALANCE_SLACK) t->opt_debug_slack = value > 0 ? value : 0;
+  else return LT_ERR_ARG;
+  return LT_OK;
+}
+
+int lt_sync(lt_tree* t) {
+  if (!t) return LT_ERR_ARG;
+  int rc = fetch_scalars(t);
+  if (rc != LT_OK) return rc;
+  return take_status(t);
+}
+
+int lt_timings(lt_tree* t, float* out4) {
+  if (!t || !out4) return LT_ERR_ARG;
+  LT_CUDA(cudaStreamSynchronize(t->stream));
+  for (int i = 0; i < 4; ++i) {
+    out4[i] = 0.f;
+    if (t->ev_set[i]) LT_CUDA(cudaEventElapsedTime(&out4[i], t->ev[2 * i], t->ev[2 * i + 1]));
+  }
+  return LT_OK;
+}
+int64_t lt_launch_count(lt_tree* t) { return t ? t->launches : 0; }
+
+int lt_leaf_boxes(lt_tree* t, int32_t* d_level, uint32_t* d_xyz) {
+  if (!t) return LT_ERR_ARG;
+  return launch_leaf_boxes(t, d_level, d_xyz);
+}
+
+int lt_encode(int dim, int max_level, const uint32_t* d_xyz, const int32_t* d_level, int64_t n,
+              uint64_t* d_keys, void* cuda_stream) {
+  if ((dim != 2 && dim != 3) || n < 0 || !d_xyz || !d_level || !d_keys) return LT_ERR_ARG;
+  if (dim * max_level + kLevelBits > 63 || max_level > 29 || max_level < 0) return LT_ERR_ARG;
+  return launch_encode(dim, max_level, d_xyz, d_level, n, d_keys, (cudaStream_t)cuda_stream);
+}
+int lt_decode(int dim, int max_level, const uint64_t* d_keys, int64_t n, int32_t* d_level, uint32_t* d_xyz,
+              void* cuda_stream) {
+  if ((dim != 2 && dim != 3) || n < 0 || !d_keys) return LT_ERR_ARG;
+  return launch_decode(dim, max_level, d_keys, n, d_level, d_xyz, (cudaStream_t)cuda_stream);
+}
+
+// ---------------------------------------------------------------------------- adapt
+int lt_adapt(lt_tree* t, const int8_t* d_flags) {
+  if (!t || !d_flags) return LT_ERR_ARG;
+  int rc;
+  if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
+  tic(t, 0);
+  const int G = grid_for(t, 8);
+  if ((rc = launch_adapt_count(t, d_flags, G)) != LT_OK) return rc;
+  // the new size is needed on the host to size buffers: one small read-back
+  LT_CUDA(cudaMemcpyAsync(t->h_sums, t->d_sums, (size_t)G * sizeof(unsigned long long), cudaMemcpyDeviceToHost,
+                          t->stream));
+  LT_CUDA(cudaStreamSynchronize(t->stream));
+  int64_t n_b = 0, n_kept = 0;
+  const unsigned long long* hs = (const unsigned long long*)t->h_sums;
+  for (int b = 0; b < G; ++b) {
+    n_b += (int64_t)(hs[b] & 0xffffffffull);
+    n_kept += (int64_t)(hs[b] >> 32);
+  }
+  const int64_t n_in = t->n;
+  const int64_t need = t->opt_adapt_sort ? n_kept + n_b : n_b;
+  if ((rc = grow(t, need)) != LT_OK) return rc;
+  if (!t->opt_adapt_sort) {
+    // path B: ordered expansion cur -> tmp
+    if ((rc = launch_adapt_scatter(t, d_flags, G, 0)) != LT_OK) return rc;
+    const int o = t->old;
+    t->old = t->cur;
+    t->cur = t->tmp;
+    t->tmp = o;
+    t->n = n_b;
+  } else {
+    // path A (Alg. 6 as printed): append -> radix sort -> linearise
+    LT_CUDA(cudaMemsetAsync(&t->d_s->aux, 0, sizeof(int), t->stream));
+    if ((rc = launch_adapt_scatter(t, d_flags, G, 1)) != LT_OK) return rc;
+    if ((rc = fetch_scalars(t)) != LT_OK) return rc;
+    t->n = n_in;  // fetch_scalars read the (unchanged) device count
+    const int64_t n_app = n_kept + t->h_s->aux;
+    SortScratch sc = {t->sort_tmp, t->sort_cap, t->sort_hist, t->sort_status, t->sort_status_cap, nullptr};
+    rc = sort_keys(t->keys[t->tmp], n_app, t->g.dim * t->g.maxl + kLevelBits, &sc, t->stream, &t->launches);
+    t->sort_tmp = sc.tmp; t->sort_cap = sc.cap; t->sort_hist = sc.hist; t->sort_status = sc.status;
+    t->sort_status_cap = sc.status_cap;
+    if (rc != LT_OK) return rc;
+    int64_t n_lin = 0;
+    // the previous snapshot buffer receives the result (the snapshot is being replaced)
+    rc = linearise_keys(t->g.dim, t->g.maxl, t->keys[t->tmp], t->keys[t->old], n_app, &n_lin, t->d_sums,
+                        &t->d_s->aux, (int*)t->h_sums, G, t->stream, &t->launches);
+    if (rc != LT_OK) return rc;
+    const int o = t->old;
+    t->old = t->cur;
+    t->cur = o;
+    t->n = n_lin;
+    int nn = (int)n_lin;
+    LT_CUDA(cudaMemcpyAsync(&t->d_s->n, &nn, sizeof(int), cudaMemcpyHostToDevice, t->stream));
+    LT_CUDA(cudaStreamSynchronize(t->stream));
+    if ((rc = launch_build_index(t, t->cur)) != LT_OK) return rc;
+  }
+  t->have_old = true;
+  t->n_old = n_in;
+  t->n_valid = true;
+  t->map_valid = false;
+  toc(t, 0);
+  return LT_OK;
+}
+
+// ---------------------------------------------------------------------------- balance
+int lt_balance(lt_tree* t, int* iters) {
+  if (!t) return LT_ERR_ARG;
+  int rc;
+  if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
+  tic(t, 1);
+  int total_iters = 0;
+  int64_t slack = t->opt_debug_slack;
+  for (int attempt = 0;; ++attempt) {
+    // (testing aid: pretend the buffers hold only n + slack leaves, to exercise the retry)
+    const int64_t cap_told = slack > 0 && t->n + slack < t->cap ? t->n + slack : t->cap;
+    if ((rc = launch_balance(t, cap_told)) != LT_OK) return rc;
+    if ((rc = fetch_scalars(t)) != LT_OK) return rc;
+    if (t->h_s->parity) {
+      const int c = t->cur;
+      t->cur = t->tmp;
+      t->tmp = c;
+    }
+    total_iters += t->h_s->iters;
+    const int st = take_status(t);
+    if (st == LT_OK) break;
+    if (st != LT_ERR_CAPACITY || attempt >= 40) return st;
+    // the analogue of the paper's "perform the balance algorithm again" when the
+    // allocated cap is exceeded: grow and continue from the valid,
+    // partially balanced tree
+    LT_CUDA(cudaMemsetAsync(t->mark, 0, (size_t)t->cap, t->stream));
+    if (cap_told < t->cap) {
+      slack *= 2;
+      continue;
+    }
+    if ((rc = grow(t, t->cap * 2)) != LT_OK) return rc == LT_ERR_OOM ? LT_ERR_CAPACITY : rc;
+  }
+  if (iters) *iters = total_iters;
+  t->map_valid = false;
+  toc(t, 1);
+  return LT_OK;
+}
+
+// ---------------------------------------------------------------------------- connect
+int lt_connect(lt_tree* t, lt_faces* out) {
+  if (!t || !out) return LT_ERR_ARG;
+  int rc;
+  if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
+  tic(t, 2);
+  const int G = grid_for(t, 8);
+  if ((rc = launch_connect_search(t, G)) != LT_OK) return rc;
+  LT_CUDA(cudaMemcpyAsync(t->h_sums, t->d_sums3, (size_t)3 * G * sizeof(int), cudaMemcpyDeviceToHost, t->stream));
+  if ((rc = fetch_scalars(t)) != LT_OK) return rc;
+  const int st = take_status(t);
+  if (st != LT_OK) return st;
+  int64_t nc = 0, nh = 0, nb = 0;
+  for (int b = 0; b < G; ++b) {
+    nc += t->h_sums[3 * b];
+    nh += t->h_sums[3 * b + 1];
+    nb += t->h_sums[3 * b + 2];
+  }
+  if ((rc = grow_pair(&t->conf, &t->conf_axis, &t->cap_conf, nc, 2)) != LT_OK) return rc;
+  if ((rc = grow_pair(&t->hang, &t->hang_info, &t->cap_hang, nh, 2)) != LT_OK) return rc;
+  if ((rc = grow_pair(&t->bnd, &t->bnd_face, &t->cap_bnd, nb, 1)) != LT_OK) return rc;
+  if ((rc = launch_connect_tables(t, G)) != LT_OK) return rc;
+  out->n_leaves = t->n;
+  out->n_conf = nc;
+  out->n_hang = nh;
+  out->n_bnd = nb;
+  out->nbr = t->nbr;
+  out->kind = t->kind;
+  out->conf = t->conf;
+  out->conf_axis = t->conf_axis;
+  out->hang = t->hang;
+  out->hang_info = t->hang_info;
+  out->bnd = t->bnd;
+  out->bnd_face = t->bnd_face;
+  toc(t, 2);
+  return LT_OK;
+}
+
+// ---------------------------------------------------------------------------- transfer
+int lt_transfer(lt_tree* t, const double* d_u_old, double* d_u_new, int p, int nvars) {
+  if (!t || !d_u_old || !d_u_new || p < 0 || p > 7 || nvars < 1) return LT_ERR_ARG;
+  int rc;
+  if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
+  if ((rc = build_operators(t, p)) != LT_OK) return rc;
+  tic(t, 3);
+  if ((rc = launch_map(t)) != LT_OK) return rc;
+  if ((rc = launch_transfer(t, d_u_old, d_u_new, p, nvars)) != LT_OK) return rc;
+  t->have_old = false;
+  t->n_old = 0;
+  t->map_valid = true;
+  toc(t, 3);
+  return LT_OK;
+}
+
+int lt_map(lt_tree* t, const int32_t** d_src, const uint8_t** d_kind) {
+  if (!t || !t->map_valid) return LT_ERR_ARG;
+  if (d_src) *d_src = t->map_src;
+  if (d_kind) *d_kind = t->map_kind;
+  return LT_OK;
+}
+
+int lt_transfer_host(lt_tree* t, const double* h_u_old, double* h_u_new, int p, int nvars) {
+  if (!t || !h_u_old || !h_u_new || p < 0 || p > 7 || nvars < 1) return LT_ERR_ARG;
+  int rc;
+  if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
+  int64_t E = nvars;
+  for (int a = 0; a < t->g.dim; ++a) E *= (p + 1);
+  const int64_t n_old = t->have_old ? t->n_old : t->n, n_new = t->n;
+  if (t->stage_old_cap < n_old * E) {
+    free_dev(t->stage_old);
+    t->stage_old_cap = 0;
+    if ((rc = alloc_dev(&t->stage_old, n_old * E)) != LT_OK) return rc;
+    t->stage_old_cap = n_old * E;
+  }
+  if (t->stage_new_cap < n_new * E) {
+    free_dev(t->stage_new);
+    t->stage_new_cap = 0;
+    if ((rc = alloc_dev(&t->stage_new, n_new * E)) != LT_OK) return rc;
+    t->stage_new_cap = n_new * E;
+  }
+  LT_CUDA(cudaMemcpyAsync(t->stage_old, h_u_old, (size_t)n_old * E * 8, cudaMemcpyHostToDevice, t->stream));
+  if ((rc = lt_transfer(t, t->stage_old, t->stage_new, p, nvars)) != LT_OK) return rc;
+  LT_CUDA(cudaMemcpyAsync(h_u_new, t->stage_new, (size_t)n_new * E * 8, cudaMemcpyDeviceToHost, t->stream));
+  rc = fetch_scalars(t);
+  if (rc != LT_OK) return rc;
+  return take_status(t);
+}
+
+// ---------------------------------------------------------------------------- sort / build from keys
+int lt_sort_keys(int dim, int max_level, uint64_t* d_keys, int64_t n, int linearise, int64_t* n_out,
+                 void* cuda_stream) {
+  if ((dim != 2 && dim != 3) || n < 0 || (n > 0 && !d_keys)) return LT_ERR_ARG;
+  if (dim * max_level + kLevelBits > 63 || max_level < 0) return LT_ERR_ARG;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  SortScratch sc = {nullptr, 0, nullptr, nullptr, 0, nullptr};
+  int64_t launches = 0;
+  int rc = sort_keys(d_keys, n, dim * max_level + kLevelBits, &sc, s, &launches);
+  int64_t m = n;
+  if (rc == LT_OK && linearise && n > 0) {
+    unsigned long long* d_sums = nullptr;
+    int* d_total = nullptr;
+    int* h_total = nullptr;
+    uint64_t* d_out = nullptr;
+    const int G = 148 * 4;
+    if (cudaMalloc(&d_sums, G * sizeof(unsigned long long)) != cudaSuccess ||
+        cudaMalloc(&d_total, sizeof(int)) != cudaSuccess || cudaMalloc(&d_out, (size_t)n * 8) != cudaSuccess ||
+        cudaMallocHost((void**)&h_total, sizeof(int)) != cudaSuccess) {
+      rc = LT_ERR_OOM;
+    } else {
+      rc = linearise_keys(dim, max_level, d_keys, d_out, n, &m, d_sums, d_total, h_total, G, s, &launches);
+      if (rc == LT_OK && cudaMemcpyAsync(d_keys, d_out, (size_t)m * 8, cudaMemcpyDeviceToDevice, s) != cudaSuccess)
+        rc = LT_ERR_CUDA;
+    }
+    cudaStreamSynchronize(s);
+    free_dev(d_sums); free_dev(d_total); free_dev(d_out);
+    if (h_total) cudaFreeHost(h_total);
+  }
+  if (cudaStreamSynchronize(s) != cudaSuccess && rc == LT_OK) rc = LT_ERR_CUDA;
+  free_dev(sc.tmp); free_dev(sc.hist); free_dev(sc.status);
+  if (n_out) *n_out = m;
+  return rc;
+}
+
+int lt_build_from_keys(int dim, int base_level, int max_level, const double* domain, const int* periodic,
+                       void* cuda_stream, const uint64_t* d_keys, int64_t n, lt_tree** out) {
+  if (!d_keys || n < 1 || n >= (1ll << 30)) return LT_ERR_ARG;
+  Tree* t = nullptr;
+  int rc = new_tree(dim, base_level, max_level, domain, periodic, cuda_stream, &t);
+  if (rc != LT_OK) return rc;
+  auto fail = [&](int code) {
+    lt_free((lt_tree*)t);
+    return code;
+  };
+  if ((rc = grow(t, n)) != LT_OK) return fail(rc);
+  if (cudaMemcpyAsync(t->keys[t->tmp], d_keys, (size_t)n * 8, cudaMemcpyDeviceToDevice, t->stream) != cudaSuccess)
+    return fail(LT_ERR_CUDA);
+  SortScratch sc = {nullptr, 0, nullptr, nullptr, 0, nullptr};
+  rc = sort_keys(t->keys[t->tmp], n, dim * max_level + kLevelBits, &sc, t->stream, &t->launches);
+  t->sort_tmp = sc.tmp; t->sort_cap = sc.cap; t->sort_hist = sc.hist; t->sort_status = sc.status;
+  t->sort_status_cap = sc.status_cap;
+  if (rc != LT_OK) return fail(rc);
+  int64_t m = 0;
+  rc = linearise_keys(dim, max_level, t->keys[t->tmp], t->keys[t->cur], n, &m, t->d_sums, &t->d_s->aux,
+                      (int*)t->h_sums, grid_for(t, 4), t->stream, &t->launches);
+  if (rc != LT_OK) return fail(rc);
+  int nn = (int)m;
+  if (cudaMemcpyAsync(&t->d_s->n, &nn, sizeof(int), cudaMemcpyHostToDevice, t->stream) != cudaSuccess)
+    return fail(LT_ERR_CUDA);
+  if (cudaStreamSynchronize(t->stream) != cudaSuccess) return fail(LT_ERR_CUDA);
+  t->n = m;
+  t->n_valid = true;
+  if ((rc = launch_check_tiling(t)) != LT_OK) return fail(rc);
+  if ((rc = fetch_scalars(t)) != LT_OK) return fail(rc);
+  t->n = m;
+  int st = take_status(t);
+  if (st != LT_OK) return fail(st);
+  if (t->h_s->volume != (1ull << (dim * max_level))) return fail(LT_ERR_INCOMPLETE);
+  if ((rc = launch_build_index(t, t->cur)) != LT_OK) return fail(rc);
+  *out = (lt_tree*)t;
+  return LT_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,231 @@
+// lt_dev.cuh -- device-side helpers of liblt (key algebra, bucketed point location,
+// block scans).  Product code: shares nothing with oracle/.
+//
+// Key format (include/lt.h; Alg. 1):  key = (morton << 5) | level,
+// morton = bit-interleaved integer anchor in finest-cell units, x lowest.
+#pragma once
+#include <cooperative_groups.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace lt {
+
+constexpr int kLevelBits = 5;
+constexpr uint64_t kLevelMask = 31;
+
+// Static description of a tree, passed by value to every kernel.
+struct Geo {
+  int dim, base, maxl;
+  int ilevel;       // level of the bucket index (<= base), see locate()
+  int ishift;       // dim * (maxl - ilevel): morton >> ishift = bucket
+  int nbuckets;     // 2^(dim*ilevel)
+  int periodic;     // bit a set = axis a periodic
+  uint64_t total;   // (1 << dim*maxl) - 1 : all morton bits in use
+};
+
+template <int DIM> struct Dim;
+template <> struct Dim<2> {
+  static constexpr int NC = 4, NF = 4;
+  static constexpr uint64_t kAxis0 = 0x5555555555555555ull;  // bits 0,2,4,..
+};
+template <> struct Dim<3> {
+  static constexpr int NC = 8, NF = 6;
+  static constexpr uint64_t kAxis0 = 0x1249249249249249ull;  // bits 0,3,6,..
+};
+
+__host__ __device__ __forceinline__ int key_level(uint64_t k) { return (int)(k & kLevelMask); }
+__host__ __device__ __forceinline__ uint64_t key_morton(uint64_t k) { return k >> kLevelBits; }
+__host__ __device__ __forceinline__ uint64_t make_key(uint64_t m, int l) {
+  return (m << kLevelBits) | (uint64_t)l;
+}
+
+// ---- bit interleave ("magic number approach") ---------------------------
+__host__ __device__ __forceinline__ uint64_t dilate2(uint32_t v) {
+  uint64_t x = v;
+  x = (x | (x << 16)) & 0x0000FFFF0000FFFFull;
+  x = (x | (x << 8)) & 0x00FF00FF00FF00FFull;
+  x = (x | (x << 4)) & 0x0F0F0F0F0F0F0F0Full;
+  x = (x | (x << 2)) & 0x3333333333333333ull;
+  x = (x | (x << 1)) & 0x5555555555555555ull;
+  return x;
+}
+__host__ __device__ __forceinline__ uint32_t compact2(uint64_t x) {
+  x &= 0x5555555555555555ull;
+  x = (x | (x >> 1)) & 0x3333333333333333ull;
+  x = (x | (x >> 2)) & 0x0F0F0F0F0F0F0F0Full;
+  x = (x | (x >> 4)) & 0x00FF00FF00FF00FFull;
+  x = (x | (x >> 8)) & 0x0000FFFF0000FFFFull;
+  x = (x | (x >> 16)) & 0x00000000FFFFFFFFull;
+  return (uint32_t)x;
+}
+__host__ __device__ __forceinline__ uint64_t dilate3(uint32_t v) {
+  uint64_t x = v & 0x1FFFFFu;
+  x = (x | (x << 32)) & 0x001F00000000FFFFull;
+  x = (x | (x << 16)) & 0x001F0000FF0000FFull;
+  x = (x | (x << 8)) & 0x100F00F00F00F00Full;
+  x = (x | (x << 4)) & 0x10C30C30C30C30C3ull;
+  x = (x | (x << 2)) & 0x1249249249249249ull;
+  return x;
+}
+__host__ __device__ __forceinline__ uint32_t compact3(uint64_t x) {
+  x &= 0x1249249249249249ull;
+  x = (x | (x >> 2)) & 0x10C30C30C30C30C3ull;
+  x = (x | (x >> 4)) & 0x100F00F00F00F00Full;
+  x = (x | (x >> 8)) & 0x001F0000FF0000FFull;
+  x = (x | (x >> 16)) & 0x001F00000000FFFFull;
+  x = (x | (x >> 32)) & 0x00000000001FFFFFull;
+  return (uint32_t)x;
+}
+template <int DIM>
+__host__ __device__ __forceinline__ uint64_t interleave(const uint32_t* x) {
+  if (DIM == 2) return dilate2(x[0]) | (dilate2(x[1]) << 1);
+  return dilate3(x[0]) | (dilate3(x[1]) << 1) | (dilate3(x[2]) << 2);
+}
+template <int DIM>
+__host__ __device__ __forceinline__ void deinterleave(uint64_t m, uint32_t* x) {
+  if (DIM == 2) {
+    x[0] = compact2(m);
+    x[1] = compact2(m >> 1);
+    x[2] = 0;
+  } else {
+    x[0] = compact3(m);
+    x[1] = compact3(m >> 1);
+    x[2] = compact3(m >> 2);
+  }
+}
+
+// child id of a leaf = digit (level-1) of its path = low DIM bits of the raw ID
+// (PAPER.md:173); 0 for the root.
+template <int DIM>
+__device__ __forceinline__ int child_id(const Geo& g, uint64_t m, int l) {
+  return (int)((m >> (DIM * (g.maxl - l))) & (uint64_t)(Dim<DIM>::NC - 1));
+}
+
+// a (level la) is a strict ancestor of b (level lb)
+template <int DIM>
+__device__ __forceinline__ bool is_ancestor(const Geo& g, uint64_t ka, uint64_t kb) {
+  int la = key_level(ka), lb = key_level(kb);
+  if (la >= lb) return false;
+  int sh = DIM * (g.maxl - la);
+  return (key_morton(ka) >> sh) == (key_morton(kb) >> sh);
+}
+
+// Same-level face neighbour of the cell (m, l) across local face f (0=-x 1=+x 2=-y ...),
+// computed on the dilated integer: add / subtract the cell width on one axis with the
+// carry rippling over the other axes' bit positions.  Coordinates wrap mod 2^maxl
+// (periodic treatment).  Returns false when the face lies on the domain
+// boundary of a non-periodic axis; *wrapped tells whether the wrap was used.
+template <int DIM>
+__device__ __forceinline__ bool face_neighbour(const Geo& g, uint64_t m, int l, int f, uint64_t* mn) {
+  const int a = f >> 1;
+  const int sh = DIM * (g.maxl - l) + a;
+  const uint64_t wbit = 1ull << sh;
+  const uint64_t maskA = (Dim<DIM>::kAxis0 << a) & g.total;
+  const uint64_t hiA = maskA & ~(wbit - 1);
+  bool edge;
+  uint64_t na;
+  if (f & 1) {
+    edge = (m & hiA) == hiA;
+    na = ((m | ~maskA) + wbit) & maskA;
+  } else {
+    edge = (m & hiA) == 0;
+    na = ((m & maskA) - wbit) & maskA;
+  }
+  *mn = (m & ~maskA) | na;
+  return !(edge && !((g.periodic >> a) & 1));
+}
+
+// Point location (the lower-bound search of PAPER.md:134-143, Eq. 7, in one form):
+// index of the leaf whose cell contains the finest-level point with morton code `mn`,
+// i.e. the last j with morton(keys[j]) <= mn.  `first` is the bucket index: first[b] =
+// index of the first leaf inside cell b of the uniform level-`ilevel` grid (every leaf
+// has level >= ilevel, so every bucket starts with a leaf whose anchor is the bucket's).
+__device__ __forceinline__ int locate(const Geo& g, const uint64_t* __restrict__ keys,
+                                      const int* __restrict__ first, uint64_t mn) {
+  const uint32_t b = (uint32_t)(mn >> g.ishift);
+  int lo = first[b], hi = first[b + 1];
+  const uint64_t bound = (mn << kLevelBits) | kLevelMask;  // keys <= bound  <=>  morton <= mn
+  while (hi - lo > 1) {
+    int mid = (lo + hi) >> 1;
+    if (keys[mid] <= bound) lo = mid; else hi = mid;
+  }
+  return lo;
+}
+
+// ---- block-wide exclusive scan (blockDim.x multiple of 32, <= 1024) ------------------
+template <typename T>
+__device__ __forceinline__ T warp_incl_scan(T v) {
+  const int lane = threadIdx.x & 31;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    T o = __shfl_up_sync(0xffffffffu, v, d);
+    if (lane >= d) v += o;
+  }
+  return v;
+}
+// returns the exclusive prefix of v within the block; *total = block sum.
+// `sm` must hold 33 T's.  Ends with a barrier, so sm may be reused immediately.
+template <typename T>
+__device__ __forceinline__ T block_excl_scan(T v, T* sm, T* total) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  T inc = warp_incl_scan(v);
+  if (lane == 31) sm[w] = inc;
+  __syncthreads();
+  if (w == 0) {
+    T s = lane < nw ? sm[lane] : T(0);
+    T si = warp_incl_scan(s);
+    sm[lane] = si - s;
+    if (lane == 31) sm[32] = si;
+  }
+  __syncthreads();
+  T res = sm[w] + inc - v;
+  *total = sm[32];
+  __syncthreads();
+  return res;
+}
+template <typename T>
+__device__ __forceinline__ T block_sum(T v, T* sm) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+  if (lane == 0) sm[w] = v;
+  __syncthreads();
+  T s = T(0);
+  if (w == 0) {
+    s = lane < nw ? sm[lane] : T(0);
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+    if (lane == 0) sm[32] = s;
+  }
+  __syncthreads();
+  s = sm[32];
+  __syncthreads();
+  return s;
+}
+
+// Contiguous chunk of [0, n) owned by block b of G: multiples of `tile` items.
+__device__ __forceinline__ void block_chunk(int64_t n, int G, int b, int tile, int64_t* lo, int64_t* hi) {
+  int64_t per = (n + G - 1) / G;
+  per = (per + tile - 1) / tile * tile;
+  int64_t l = (int64_t)b * per, h = l + per;
+  *lo = l < n ? l : n;
+  *hi = h < n ? h : n;
+}
+
+// sum of sums[0..b) and of all G entries; every thread of the block gets both.
+template <typename T>
+__device__ __forceinline__ void chunk_offsets(const T* __restrict__ sums, int G, int b, T* sm, T* before, T* total) {
+  T mine = T(0), all = T(0);
+  for (int i = threadIdx.x; i < G; i += blockDim.x) {
+    T s = sums[i];
+    all += s;
+    if (i < b) mine += s;
+  }
+  *before = block_sum(mine, sm);
+  *total = block_sum(all, sm);
+}
+
+// sticky device status word: first error wins
+__device__ __forceinline__ void set_status(int* status, int code) { atomicCAS(status, 0, code); }
+
+}  // namespace lt

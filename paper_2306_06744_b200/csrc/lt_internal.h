@@ -1,0 +1,123 @@
+// lt_internal.h -- host-side state of a tree and the launcher prototypes shared by the
+// translation units of liblt.  Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/lt.h"
+#include "lt_dev.cuh"
+
+namespace lt {
+
+// Device-resident scalars of a tree (one allocation).
+struct DevScalars {
+  int n;                 // current leaf count
+  int status;            // sticky lt_status detected on the device (0 = ok)
+  int iters;             // balance: sweeps that split >= 1 leaf
+  int parity;            // balance: 0 = result in the buffer it started in, 1 = in the other
+  int n_face[3];         // connect: n_conf, n_hang, n_bnd
+  int aux;               // scratch counter (path-A append cursor, sort tickets)
+  unsigned long long volume;  // build_from_keys: sum of leaf volumes
+  int splits;            // balance: leaves split in total
+  int pad;
+};
+
+constexpr int kMaxGrid = 4096;  // upper bound on persistent grid sizes (chunk-sum arrays)
+
+struct Tree {
+  Geo g;
+  double domain[6];
+  cudaStream_t stream;
+  int device, num_sms;
+
+  int64_t cap;            // leaf capacity of every per-leaf buffer
+  uint64_t* keys[3];      // cur / old (snapshot) / tmp rotate through these
+  int* first[3];          // bucket index per key buffer, nbuckets + 1 entries
+  int cur, old, tmp;
+  bool have_old;
+  int64_t n_old;
+  int64_t n;              // host copy of the leaf count
+  bool n_valid;
+
+  DevScalars* d_s;
+  DevScalars* h_s;        // pinned mirror
+  unsigned long long* d_sums;  // [kMaxGrid] chunk sums (packed pairs)
+  int* d_sums3;           // [3*kMaxGrid] connect chunk sums
+  int* h_sums;            // pinned [3*kMaxGrid + ..]
+
+  uint8_t* mark;          // [cap] balance marks: bit0 split, bit1 re-examine
+  int* frontier[2];       // [cap] leaves to examine in the next sweep
+
+  // connectivity
+  int32_t* nbr;
+  uint8_t* kind;
+  int64_t cap_conf, cap_hang, cap_bnd;
+  int32_t* conf; uint8_t* conf_axis;
+  int32_t* hang; uint8_t* hang_info;
+  int32_t* bnd;  uint8_t* bnd_face;
+
+  // Alg. 7 map
+  int32_t* map_src;
+  uint8_t* map_kind;
+  bool map_valid;
+
+  // transfer operators on the device for (dim, p): I^0,I^1,R^0,R^1, each [P1][P1]
+  double* d_ops;
+  int ops_p;
+
+  // host staging for lt_transfer_host
+  double* stage_old; double* stage_new; int64_t stage_old_cap, stage_new_cap;
+
+  // sort scratch
+  uint64_t* sort_tmp; int64_t sort_cap; unsigned* sort_hist; unsigned* sort_status; int64_t sort_status_cap;
+
+  int opt_adapt_sort, opt_full_sweeps, opt_debug_slack;
+  cudaEvent_t ev[8];
+  bool ev_set[4];
+  int64_t launches;
+};
+
+extern thread_local int g_last_cuda_error;
+#define LT_CUDA(call)                                   \
+  do {                                                  \
+    cudaError_t e_ = (call);                            \
+    if (e_ != cudaSuccess) {                            \
+      lt::g_last_cuda_error = (int)e_;                  \
+      cudaGetLastError();                               \
+      return e_ == cudaErrorMemoryAllocation ? LT_ERR_OOM : LT_ERR_CUDA; \
+    }                                                   \
+  } while (0)
+
+int grid_for(const Tree* t, int blocks_per_sm);
+
+// ---- lt_tree.cu
+int launch_build_uniform(Tree* t);
+int launch_build_index(Tree* t, int buf);
+int launch_adapt_count(Tree* t, const int8_t* d_flags, int G);
+int launch_adapt_scatter(Tree* t, const int8_t* d_flags, int G, int path_a);
+int launch_balance(Tree* t, int64_t cap_told);
+int launch_leaf_boxes(Tree* t, int32_t* d_level, uint32_t* d_xyz);
+int launch_encode(int dim, int maxl, const uint32_t* d_xyz, const int32_t* d_level, int64_t n, uint64_t* d_keys, cudaStream_t s);
+int launch_decode(int dim, int maxl, const uint64_t* d_keys, int64_t n, int32_t* d_level, uint32_t* d_xyz, cudaStream_t s);
+int launch_check_tiling(Tree* t);
+
+// ---- lt_connect.cu
+int launch_connect_search(Tree* t, int G);
+int launch_connect_tables(Tree* t, int G);
+
+// ---- lt_transfer.cu
+int launch_map(Tree* t);
+int launch_transfer(Tree* t, const double* d_u_old, double* d_u_new, int p, int nvars);
+int build_operators(Tree* t, int p);
+
+// ---- lt_sort.cu
+struct SortScratch {
+  uint64_t* tmp; int64_t cap; unsigned* hist; unsigned* status; int64_t status_cap; int* counter;
+};
+int sort_keys(uint64_t* d_keys, int64_t n, int key_bits, SortScratch* sc, cudaStream_t s, int64_t* launches);
+int linearise_keys(int dim, int maxl, const uint64_t* d_in, uint64_t* d_out, int64_t n, int64_t* n_out,
+                   unsigned long long* d_sums, int* d_total, int* h_total, int G, cudaStream_t s, int64_t* launches);
+
+}  // namespace lt
+
+struct lt_tree : lt::Tree {};

@@ -1,0 +1,545 @@
+// lt_tree.cu -- key codec (Alg. 1), uniform build, adaptation (Alg. 6) and the 2:1 balance
+// ripple (Alg. 4 re-expressed) for sm_100a.  Product code.
+//
+// Every kernel here is a persistent grid (a multiple of the SM count) that reads the leaf
+// count from device memory, so no launch depends on a host round trip.
+#include <cooperative_groups.h>
+
+#include "lt_internal.h"
+
+namespace cg = cooperative_groups;
+
+namespace lt {
+
+constexpr int BT = 256;  // threads per block of the tree kernels
+
+enum { ACT_KEEP = 0, ACT_REFINE = 1, ACT_PARENT = 2, ACT_DROP = 3 };
+
+// ------------------------------------------------------------------------ Alg. 1 (batch)
+template <int DIM>
+__global__ void k_encode(int maxl, const uint32_t* __restrict__ xyz, const int32_t* __restrict__ level,
+                         int64_t n, uint64_t* __restrict__ keys) {
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    uint32_t x[3] = {xyz[3 * i], xyz[3 * i + 1], xyz[3 * i + 2]};
+    int l = level[i];
+    // steps 2-4: coordinates at the finest resolution with the low (maxl-l) bits cleared
+    // are the level-l path digits followed by the zero padding
+    uint32_t clr = l >= maxl ? 0xFFFFFFFFu : ~((1u << (maxl - l)) - 1u);
+    for (int a = 0; a < 3; ++a) x[a] &= clr;
+    keys[i] = make_key(interleave<DIM>(x), l);
+  }
+}
+
+template <int DIM>
+__global__ void k_decode(const uint64_t* __restrict__ keys, int64_t n, int32_t* __restrict__ level,
+                         uint32_t* __restrict__ xyz) {
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    uint64_t k = keys[i];
+    uint32_t x[3];
+    deinterleave<DIM>(key_morton(k), x);
+    if (level) level[i] = key_level(k);
+    if (xyz) {
+      xyz[3 * i] = x[0];
+      xyz[3 * i + 1] = x[1];
+      xyz[3 * i + 2] = x[2];
+    }
+  }
+}
+
+template <int DIM>
+__global__ void k_decode_n(const uint64_t* __restrict__ keys, const DevScalars* __restrict__ s,
+                           int32_t* __restrict__ level, uint32_t* __restrict__ xyz) {
+  const int64_t n = s->n;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    uint64_t k = keys[i];
+    uint32_t x[3];
+    deinterleave<DIM>(key_morton(k), x);
+    if (level) level[i] = key_level(k);
+    if (xyz) {
+      xyz[3 * i] = x[0];
+      xyz[3 * i + 1] = x[1];
+      xyz[3 * i + 2] = x[2];
+    }
+  }
+}
+
+// ------------------------------------------------------------------------ uniform build
+// Leaf i of the uniform level-`base` tree has raw ID i (Morton order), key =
+// (i << dim*(maxl-base)) << 5 | base (Alg. 1 with the padding of step 4).
+template <int DIM>
+__global__ void k_build_uniform(Geo g, uint64_t* __restrict__ keys, int* __restrict__ first, DevScalars* s) {
+  const int64_t nb = 1ll << (DIM * g.base);
+  const int pad = DIM * (g.maxl - g.base);
+  const int sub = DIM * (g.base - g.ilevel);
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < nb; i += (int64_t)gridDim.x * blockDim.x) {
+    keys[i] = make_key((uint64_t)i << pad, g.base);
+    if ((i & ((1ll << sub) - 1)) == 0) first[i >> sub] = (int)i;
+    if (i == 0) {
+      first[g.nbuckets] = (int)nb;
+      s->n = (int)nb;
+    }
+  }
+}
+
+template <int DIM>
+__global__ void k_build_index(Geo g, const uint64_t* __restrict__ keys, const DevScalars* __restrict__ s,
+                              int* __restrict__ first) {
+  const int64_t n = s->n;
+  const uint64_t bmask = (1ull << g.ishift) - 1;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    uint64_t m = key_morton(keys[i]);
+    if ((m & bmask) == 0) first[m >> g.ishift] = (int)i;
+    if (i == 0) first[g.nbuckets] = (int)n;
+  }
+}
+
+// volume sum + level >= base check (lt_build_from_keys completeness)
+template <int DIM>
+__global__ void k_check_tiling(Geo g, const uint64_t* __restrict__ keys, DevScalars* s) {
+  __shared__ unsigned long long sm[33];
+  const int64_t n = s->n;
+  unsigned long long v = 0;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    uint64_t k = keys[i];
+    int l = key_level(k);
+    if (l < g.base || l > g.maxl) {
+      set_status(&s->status, LT_ERR_INCOMPLETE);
+    } else {
+      v += 1ull << (DIM * (g.maxl - l));
+      // anchor must be aligned to the cell width
+      if (key_morton(k) & ((1ull << (DIM * (g.maxl - l))) - 1)) set_status(&s->status, LT_ERR_INCOMPLETE);
+    }
+  }
+  v = block_sum(v, sm);
+  if (threadIdx.x == 0 && v) atomicAdd(&s->volume, v);
+}
+
+// ------------------------------------------------------------------------ Alg. 6
+// What happens to leaf i (readings B-1..B-4):
+//   a complete sibling group (2^dim consecutive entries) whose members all
+//   carry a coarsen flag and sit above the base level is replaced by its parent (emitted
+//   in place of child 0, the others are dropped); otherwise a refine flag below max_level
+//   replaces the leaf by its 2^dim children; otherwise the leaf is kept.
+template <int DIM>
+__device__ __forceinline__ int adapt_action(const Geo& g, const uint64_t* __restrict__ keys,
+                                            const int8_t* __restrict__ flags, int64_t i, int64_t n,
+                                            uint64_t key) {
+  constexpr int NC = Dim<DIM>::NC;
+  const int l = key_level(key);
+  const int8_t fl = flags[i];
+  if (fl < 0 && l > g.base) {
+    const uint64_t m = key_morton(key);
+    const int sh = DIM * (g.maxl - l);
+    const int cid = (int)((m >> sh) & (uint64_t)(NC - 1));
+    const int64_t g0 = i - cid;
+    if (g0 >= 0 && g0 + NC <= n) {
+      const uint64_t pm = m & ~((uint64_t)(NC - 1) << sh);
+      // first and last sibling present as leaves => the NC-2 entries between them are
+      // exactly the other siblings (completeness)
+      if (keys[g0] == make_key(pm, l) && keys[g0 + NC - 1] == make_key(pm | ((uint64_t)(NC - 1) << sh), l)) {
+        bool all = true;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) all = all && (flags[g0 + c] < 0);
+        if (all) return cid == 0 ? ACT_PARENT : ACT_DROP;
+      }
+    }
+  }
+  if (fl > 0 && l < g.maxl) return ACT_REFINE;
+  return ACT_KEEP;
+}
+
+// pass 1: per-chunk output counts.  sums[b] = (kept << 32) | count_B   (see lt_adapt)
+template <int DIM>
+__global__ void __launch_bounds__(BT) k_adapt_count(Geo g, const uint64_t* __restrict__ keys,
+                                                    const int8_t* __restrict__ flags,
+                                                    const DevScalars* __restrict__ s,
+                                                    unsigned long long* __restrict__ sums) {
+  constexpr int NC = Dim<DIM>::NC;
+  __shared__ unsigned long long sm[33];
+  const int64_t n = s->n;
+  int64_t lo, hi;
+  block_chunk(n, gridDim.x, blockIdx.x, BT, &lo, &hi);
+  unsigned long long acc = 0;
+  for (int64_t i = lo + threadIdx.x; i < hi; i += BT) {
+    int act = adapt_action<DIM>(g, keys, flags, i, n, keys[i]);
+    unsigned long long c = act == ACT_REFINE ? NC : (act == ACT_DROP ? 0 : 1);
+    unsigned long long kept = (act == ACT_KEEP || act == ACT_REFINE) ? 1 : 0;
+    acc += c | (kept << 32);
+  }
+  acc = block_sum(acc, sm);
+  if (threadIdx.x == 0) sums[blockIdx.x] = acc;
+}
+
+// pass 2 (path B, ordered expansion): children / parent are written in place of the
+// source entries, which keeps the array sorted because a leaf's children occupy exactly
+// its Morton interval (reading B-5).  Also rebuilds the bucket index.
+template <int DIM>
+__global__ void __launch_bounds__(BT) k_adapt_scatter(Geo g, const uint64_t* __restrict__ keys,
+                                                      const int8_t* __restrict__ flags, DevScalars* s,
+                                                      const unsigned long long* __restrict__ sums,
+                                                      uint64_t* __restrict__ out, int* __restrict__ first_out,
+                                                      int64_t cap) {
+  constexpr int NC = Dim<DIM>::NC;
+  __shared__ unsigned long long sm[33];
+  const int64_t n = s->n;
+  unsigned long long before, total;
+  chunk_offsets(sums, gridDim.x, blockIdx.x, sm, &before, &total);
+  const int64_t n_out = (int64_t)(total & 0xffffffffull);
+  if (n_out > cap) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) set_status(&s->status, LT_ERR_CAPACITY);
+    return;
+  }
+  int64_t lo, hi;
+  block_chunk(n, gridDim.x, blockIdx.x, BT, &lo, &hi);
+  int64_t run = (int64_t)(before & 0xffffffffull);
+  const uint64_t bmask = (1ull << g.ishift) - 1;
+  for (int64_t t0 = lo; t0 < hi; t0 += BT) {
+    const int64_t i = t0 + threadIdx.x;
+    int act = ACT_DROP;
+    uint64_t key = 0;
+    if (i < hi) {
+      key = keys[i];
+      act = adapt_action<DIM>(g, keys, flags, i, n, key);
+    }
+    int c = act == ACT_REFINE ? NC : (act == ACT_DROP ? 0 : 1);
+    unsigned long long tile_total;
+    unsigned long long ex = block_excl_scan<unsigned long long>((unsigned long long)c, sm, &tile_total);
+    int64_t pos = run + (int64_t)ex;
+    run += (int64_t)tile_total;
+    if (c == 0) continue;
+    const int l = key_level(key);
+    const uint64_t m = key_morton(key);
+    if ((m & bmask) == 0) first_out[m >> g.ishift] = (int)pos;
+    if (act == ACT_KEEP) {
+      out[pos] = key;
+    } else if (act == ACT_PARENT) {
+      out[pos] = make_key(m, l - 1);  // child 0 has the parent's anchor
+    } else {
+      const int sh = DIM * (g.maxl - l - 1);
+#pragma unroll
+      for (int k = 0; k < NC; ++k) out[pos + k] = make_key(m | ((uint64_t)k << sh), l + 1);  // reading A-6
+    }
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    first_out[g.nbuckets] = (int)n_out;
+    s->n = (int)n_out;
+  }
+}
+
+// pass 2 (path A, as the paper does it): kept entries stay (a refined octant is removed
+// later by the linearisation), children and parents are appended through
+// an atomic cursor in no particular order; sort + linearise follow (Alg. 6 step 6).
+template <int DIM>
+__global__ void __launch_bounds__(BT) k_adapt_append(Geo g, const uint64_t* __restrict__ keys,
+                                                     const int8_t* __restrict__ flags, DevScalars* s,
+                                                     const unsigned long long* __restrict__ sums,
+                                                     uint64_t* __restrict__ out, int64_t cap) {
+  constexpr int NC = Dim<DIM>::NC;
+  __shared__ unsigned long long sm[33];
+  const int64_t n = s->n;
+  unsigned long long before, total;
+  chunk_offsets(sums, gridDim.x, blockIdx.x, sm, &before, &total);
+  const int64_t n_kept = (int64_t)(total >> 32);
+  if (n_kept + (int64_t)(total & 0xffffffffull) > cap) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) set_status(&s->status, LT_ERR_CAPACITY);
+    return;
+  }
+  int64_t lo, hi;
+  block_chunk(n, gridDim.x, blockIdx.x, BT, &lo, &hi);
+  int64_t run = (int64_t)(before >> 32);
+  for (int64_t t0 = lo; t0 < hi; t0 += BT) {
+    const int64_t i = t0 + threadIdx.x;
+    int act = ACT_DROP;
+    uint64_t key = 0;
+    if (i < hi) {
+      key = keys[i];
+      act = adapt_action<DIM>(g, keys, flags, i, n, key);
+    }
+    int kept = (act == ACT_KEEP || act == ACT_REFINE) ? 1 : 0;
+    unsigned long long tile_total;
+    unsigned long long ex = block_excl_scan<unsigned long long>((unsigned long long)kept, sm, &tile_total);
+    int64_t pos = run + (int64_t)ex;
+    run += (int64_t)tile_total;
+    const int l = key_level(key);
+    const uint64_t m = key_morton(key);
+    if (kept) out[pos] = key;
+    if (act == ACT_REFINE) {
+      int64_t at = n_kept + atomicAdd(&s->aux, NC);
+      const int sh = DIM * (g.maxl - l - 1);
+      for (int k = 0; k < NC; ++k) out[at + k] = make_key(m | ((uint64_t)k << sh), l + 1);
+    } else if (act == ACT_PARENT) {
+      int64_t at = n_kept + atomicAdd(&s->aux, 1);
+      out[at] = make_key(m, l - 1);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------ 2:1 balance
+// PAPER.md:130-161 (Alg. 4), face balance (reading C-1), Jacobi ripple (readings C-2,
+// C-3): a sweep examines leaves against the tree as it stood at the start of the sweep;
+// every face neighbour found >= 2 levels coarser is marked; marked leaves split once.
+// All sweeps run inside this one cooperative kernel.
+//
+// After the first (full) sweep only a frontier is examined: the children created by the
+// previous sweep, plus every leaf that saw a neighbour >= 3 levels coarser (its
+// neighbour's children will still be too coarse).  DESIGN.md proves that this marks the
+// same set as a full sweep.
+struct BalanceArgs {
+  Geo g;
+  uint64_t* keys[2];
+  int* first[2];
+  uint8_t* mark;
+  int* frontier[2];
+  unsigned long long* sums;
+  DevScalars* s;
+  int64_t cap;
+  int full_sweeps;
+};
+
+template <int DIM>
+__device__ __forceinline__ void balance_examine(const Geo& g, const uint64_t* __restrict__ keys,
+                                                const int* __restrict__ first, uint8_t* mark, int i, int f) {
+  const uint64_t key = keys[i];
+  const int l = key_level(key);
+  if (l < g.base + 2) return;  // no leaf is coarser than the base level
+  uint64_t mn;
+  if (!face_neighbour<DIM>(g, key_morton(key), l, f, &mn)) return;
+  const int j = locate(g, keys, first, mn);
+  const int lj = key_level(keys[j]);
+  if (lj < l - 1) {
+    atomicOr((unsigned*)(mark + (j & ~3)), 1u << (8 * (j & 3)));
+    if (lj < l - 2) atomicOr((unsigned*)(mark + (i & ~3)), 2u << (8 * (i & 3)));
+  }
+}
+
+template <int DIM>
+__global__ void __launch_bounds__(BT) k_balance(BalanceArgs a) {
+  constexpr int NC = Dim<DIM>::NC, NF = Dim<DIM>::NF;
+  __shared__ unsigned long long sm[33];
+  cg::grid_group grid = cg::this_grid();
+  const Geo g = a.g;
+  const int64_t gtid = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  const int64_t gsize = (int64_t)gridDim.x * blockDim.x;
+  const uint64_t bmask = (1ull << g.ishift) - 1;
+  int64_t n = a.s->n;
+  int par = 0, iters = 0, fpar = 0;
+  int64_t nfront = -1;  // -1: full sweep
+  int64_t splits = 0;
+  int err = 0;
+  for (;;) {
+    const uint64_t* keys = a.keys[par];
+    const int* first = a.first[par];
+    // ---- sweep
+    if (nfront < 0) {
+      for (int64_t sidx = gtid; sidx < n * NF; sidx += gsize)
+        balance_examine<DIM>(g, keys, first, a.mark, (int)(sidx / NF), (int)(sidx % NF));
+    } else {
+      const int* fr = a.frontier[fpar];
+      for (int64_t sidx = gtid; sidx < nfront * NF; sidx += gsize)
+        balance_examine<DIM>(g, keys, first, a.mark, fr[sidx / NF], (int)(sidx % NF));
+    }
+    grid.sync();
+    // ---- count: low 32 = leaves out, high 32 = frontier entries out
+    int64_t lo, hi;
+    block_chunk(n, gridDim.x, blockIdx.x, BT, &lo, &hi);
+    unsigned long long acc = 0;
+    for (int64_t i = lo + threadIdx.x; i < hi; i += BT) {
+      const unsigned mk = a.mark[i];
+      unsigned long long c = (mk & 1) ? NC : 1;
+      unsigned long long fc = (mk & 1) ? NC : ((mk & 2) ? 1 : 0);
+      acc += c | (fc << 32);
+    }
+    acc = block_sum(acc, sm);
+    if (threadIdx.x == 0) a.sums[blockIdx.x] = acc;
+    grid.sync();
+    unsigned long long before, total;
+    chunk_offsets(a.sums, gridDim.x, blockIdx.x, sm, &before, &total);
+    const int64_t n_new = (int64_t)(total & 0xffffffffull);
+    if (n_new == n) break;  // no leaf was marked: balanced
+    if (n_new > a.cap) {
+      err = LT_ERR_CAPACITY;
+      break;
+    }
+    // ---- split marked leaves (order-preserving), rebuild index, emit next frontier
+    uint64_t* out = a.keys[par ^ 1];
+    int* first_out = a.first[par ^ 1];
+    int* fr_out = a.frontier[fpar ^ 1];
+    int64_t run = (int64_t)(before & 0xffffffffull), frun = (int64_t)(before >> 32);
+    for (int64_t t0 = lo; t0 < hi; t0 += BT) {
+      const int64_t i = t0 + threadIdx.x;
+      unsigned mk = 0;
+      uint64_t key = 0;
+      unsigned long long c = 0;
+      if (i < hi) {
+        key = keys[i];
+        mk = a.mark[i];
+        if (mk) a.mark[i] = 0;
+        c = ((mk & 1) ? NC : 1) | ((unsigned long long)((mk & 1) ? NC : ((mk & 2) ? 1 : 0)) << 32);
+      }
+      unsigned long long tile_total;
+      unsigned long long ex = block_excl_scan<unsigned long long>(c, sm, &tile_total);
+      const int64_t pos = run + (int64_t)(ex & 0xffffffffull);
+      const int64_t fpos = frun + (int64_t)(ex >> 32);
+      run += (int64_t)(tile_total & 0xffffffffull);
+      frun += (int64_t)(tile_total >> 32);
+      if (i >= hi) continue;
+      const int l = key_level(key);
+      const uint64_t m = key_morton(key);
+      if ((m & bmask) == 0) first_out[m >> g.ishift] = (int)pos;
+      if (mk & 1) {
+        const int sh = DIM * (g.maxl - l - 1);
+#pragma unroll
+        for (int k = 0; k < NC; ++k) {
+          out[pos + k] = make_key(m | ((uint64_t)k << sh), l + 1);
+          fr_out[fpos + k] = (int)(pos + k);
+        }
+      } else {
+        out[pos] = key;
+        if (mk & 2) fr_out[fpos] = (int)pos;
+      }
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) first_out[g.nbuckets] = (int)n_new;
+    splits += (n_new - n) / (NC - 1);
+    n = n_new;
+    nfront = a.full_sweeps ? -1 : (int64_t)(total >> 32);
+    par ^= 1;
+    fpar ^= 1;
+    ++iters;
+    grid.sync();
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    a.s->n = (int)n;
+    a.s->iters = iters;
+    a.s->parity = par;
+    a.s->splits = (int)splits;
+    if (err) set_status(&a.s->status, err);
+  }
+}
+
+// ------------------------------------------------------------------------ launchers
+int grid_for(const Tree* t, int blocks_per_sm) {
+  int G = t->num_sms * blocks_per_sm;
+  return G > kMaxGrid ? kMaxGrid : G;
+}
+
+#define LT_DISPATCH_DIM(t, expr2, expr3) \
+  do {                                   \
+    if ((t)->g.dim == 2) { expr2; } else { expr3; } \
+  } while (0)
+
+int launch_build_uniform(Tree* t) {
+  int G = grid_for(t, 4);
+  LT_DISPATCH_DIM(t, (k_build_uniform<2><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s)),
+                  (k_build_uniform<3><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s)));
+  t->launches++;
+  LT_CUDA(cudaGetLastError());
+  return LT_OK;
+}
+
+int launch_build_index(Tree* t, int buf) {
+  int G = grid_for(t, 4);
+  LT_DISPATCH_DIM(t, (k_build_index<2><<<G, BT, 0, t->stream>>>(t->g, t->keys[buf], t->d_s, t->first[buf])),
+                  (k_build_index<3><<<G, BT, 0, t->stream>>>(t->g, t->keys[buf], t->d_s, t->first[buf])));
+  t->launches++;
+  LT_CUDA(cudaGetLastError());
+  return LT_OK;
+}
+
+int launch_check_tiling(Tree* t) {
+  int G = grid_for(t, 4);
+  LT_DISPATCH_DIM(t, (k_check_tiling<2><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], t->d_s)),
+                  (k_check_tiling<3><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], t->d_s)));
+  t->launches++;
+  LT_CUDA(cudaGetLastError());
+  return LT_OK;
+}
+
+int launch_adapt_count(Tree* t, const int8_t* d_flags, int G) {
+  LT_DISPATCH_DIM(t, (k_adapt_count<2><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], d_flags, t->d_s, t->d_sums)),
+                  (k_adapt_count<3><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], d_flags, t->d_s, t->d_sums)));
+  t->launches++;
+  LT_CUDA(cudaGetLastError());
+  return LT_OK;
+}
+
+int launch_adapt_scatter(Tree* t, const int8_t* d_flags, int G, int path_a) {
+  if (path_a) {
+    LT_DISPATCH_DIM(t,
+                    (k_adapt_append<2><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], d_flags, t->d_s, t->d_sums,
+                                                                t->keys[t->tmp], t->cap)),
+                    (k_adapt_append<3><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], d_flags, t->d_s, t->d_sums,
+                                                                t->keys[t->tmp], t->cap)));
+  } else {
+    LT_DISPATCH_DIM(t,
+                    (k_adapt_scatter<2><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], d_flags, t->d_s, t->d_sums,
+                                                                 t->keys[t->tmp], t->first[t->tmp], t->cap)),
+                    (k_adapt_scatter<3><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], d_flags, t->d_s, t->d_sums,
+                                                                 t->keys[t->tmp], t->first[t->tmp], t->cap)));
+  }
+  t->launches++;
+  LT_CUDA(cudaGetLastError());
+  return LT_OK;
+}
+
+int launch_balance(Tree* t, int64_t cap_told) {
+  BalanceArgs a;
+  a.g = t->g;
+  a.keys[0] = t->keys[t->cur];
+  a.keys[1] = t->keys[t->tmp];
+  a.first[0] = t->first[t->cur];
+  a.first[1] = t->first[t->tmp];
+  a.mark = t->mark;
+  a.frontier[0] = t->frontier[0];
+  a.frontier[1] = t->frontier[1];
+  a.sums = t->d_sums;
+  a.s = t->d_s;
+  a.cap = cap_told;
+  a.full_sweeps = t->opt_full_sweeps;
+  void* fn = t->g.dim == 2 ? (void*)k_balance<2> : (void*)k_balance<3>;
+  int per_sm = 0;
+  LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, BT, 0));
+  if (per_sm < 1) return LT_ERR_CUDA;
+  int G = t->num_sms * per_sm;
+  if (G > kMaxGrid) G = kMaxGrid;
+  void* args[] = {&a};
+  LT_CUDA(cudaLaunchCooperativeKernel(fn, dim3(G), dim3(BT), args, 0, t->stream));
+  t->launches++;
+  return LT_OK;
+}
+
+int launch_leaf_boxes(Tree* t, int32_t* d_level, uint32_t* d_xyz) {
+  int G = grid_for(t, 8);
+  LT_DISPATCH_DIM(t, (k_decode_n<2><<<G, BT, 0, t->stream>>>(t->keys[t->cur], t->d_s, d_level, d_xyz)),
+                  (k_decode_n<3><<<G, BT, 0, t->stream>>>(t->keys[t->cur], t->d_s, d_level, d_xyz)));
+  t->launches++;
+  LT_CUDA(cudaGetLastError());
+  return LT_OK;
+}
+
+static int grid_for_n(int64_t n) {
+  int64_t G = (n + BT - 1) / BT;
+  if (G < 1) G = 1;
+  if (G > 148 * 16) G = 148 * 16;
+  return (int)G;
+}
+
+int launch_encode(int dim, int maxl, const uint32_t* d_xyz, const int32_t* d_level, int64_t n, uint64_t* d_keys,
+                  cudaStream_t s) {
+  if (n == 0) return LT_OK;
+  if (dim == 2) k_encode<2><<<grid_for_n(n), BT, 0, s>>>(maxl, d_xyz, d_level, n, d_keys);
+  else k_encode<3><<<grid_for_n(n), BT, 0, s>>>(maxl, d_xyz, d_level, n, d_keys);
+  LT_CUDA(cudaGetLastError());
+  return LT_OK;
+}
+
+int launch_decode(int dim, int maxl, const uint64_t* d_keys, int64_t n, int32_t* d_level, uint32_t* d_xyz,
+                  cudaStream_t s) {
+  (void)maxl;
+  if (n == 0) return LT_OK;
+  if (dim == 2) k_decode<2><<<grid_for_n(n), BT, 0, s>>>(d_keys, n, d_level, d_xyz);
+  else k_decode<3><<<grid_for_n(n), BT, 0, s>>>(d_keys, n, d_level, d_xyz);
+  LT_CUDA(cudaGetLastError());
+  return LT_OK;
+}
+
+}  // namespace lt
