@@ -191,10 +191,12 @@ typedef enum {
 } lt_option;
 int lt_set_option(lt_tree*, int option, int value);
 
-/* Per-call device times of the last cycle in milliseconds (CUDA events on the tree's
- * stream): out[0..3] = adapt, balance, connect, transfer; 0 where not run.
+/* Device times of the last cycle in milliseconds (CUDA events on the tree's stream):
+ * out[0..3] = the calls lt_adapt, lt_balance, lt_connect, lt_transfer; out[4] = the Alg. 7
+ * map kernel alone, out[5] = the solution-transfer kernel alone, out[6] = the connectivity
+ * search kernel alone, out[7] = the face-table kernel alone; 0 where not run.
  * Synchronises. */
-int lt_timings(lt_tree*, float* out4);
+int lt_timings(lt_tree*, float* out8);
 /* Number of kernels liblt launched on this tree since it was built. */
 int64_t lt_launch_count(lt_tree*);
 

@@ -164,8 +164,11 @@ class Tree:
             raise OracleError("oracle: bad arguments or incomplete key set")
 
     def __del__(self):
-        if getattr(self, "_h", None):
-            lib().lto_free(self._h)
+        if getattr(self, "_h", None) and _lib is not None:
+            try:
+                _lib.lto_free(self._h)
+            except Exception:  # interpreter shutdown
+                pass
             self._h = None
 
     # -- state

@@ -175,7 +175,7 @@ static int new_tree(int dim, int base, int maxl, const double* domain, const int
     return fail(LT_ERR_OOM);
   memset(t->h_s, 0, sizeof(DevScalars));
   if (cudaMemsetAsync(t->d_s, 0, sizeof(DevScalars), t->stream) != cudaSuccess) return fail(LT_ERR_CUDA);
-  for (int i = 0; i < 8; ++i)
+  for (int i = 0; i < 16; ++i)
     if (cudaEventCreate(&t->ev[i]) != cudaSuccess) return fail(LT_ERR_CUDA);
   *out = t;
   return LT_OK;
@@ -221,7 +221,7 @@ void lt_free(lt_tree* t) {
   free_dev(t->map_src); free_dev(t->map_kind); free_dev(t->d_ops);
   free_dev(t->stage_old); free_dev(t->stage_new);
   free_dev(t->sort_tmp); free_dev(t->sort_hist); free_dev(t->sort_status);
-  for (int i = 0; i < 8; ++i)
+  for (int i = 0; i < 16; ++i)
     if (t->ev[i]) cudaEventDestroy(t->ev[i]);
   delete t;
 }
@@ -298,12 +298,12 @@ int lt_sync(lt_tree* t) {
   return take_status(t);
 }
 
-int lt_timings(lt_tree* t, float* out4) {
-  if (!t || !out4) return LT_ERR_ARG;
+int lt_timings(lt_tree* t, float* out8) {
+  if (!t || !out8) return LT_ERR_ARG;
   LT_CUDA(cudaStreamSynchronize(t->stream));
-  for (int i = 0; i < 4; ++i) {
-    out4[i] = 0.f;
-    if (t->ev_set[i]) LT_CUDA(cudaEventElapsedTime(&out4[i], t->ev[2 * i], t->ev[2 * i + 1]));
+  for (int i = 0; i < 8; ++i) {
+    out8[i] = 0.f;
+    if (t->ev_set[i]) LT_CUDA(cudaEventElapsedTime(&out8[i], t->ev[2 * i], t->ev[2 * i + 1]));
   }
   return LT_OK;
 }
@@ -434,7 +434,9 @@ int lt_connect(lt_tree* t, lt_faces* out) {
   if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
   tic(t, 2);
   const int G = grid_for(t, 8);
+  tic(t, 6);
   if ((rc = launch_connect_search(t, G)) != LT_OK) return rc;
+  toc(t, 6);
   LT_CUDA(cudaMemcpyAsync(t->h_sums, t->d_sums3, (size_t)3 * G * sizeof(int), cudaMemcpyDeviceToHost, t->stream));
   if ((rc = fetch_scalars(t)) != LT_OK) return rc;
   const int st = take_status(t);
@@ -448,7 +450,9 @@ int lt_connect(lt_tree* t, lt_faces* out) {
   if ((rc = grow_pair(&t->conf, &t->conf_axis, &t->cap_conf, nc, 2)) != LT_OK) return rc;
   if ((rc = grow_pair(&t->hang, &t->hang_info, &t->cap_hang, nh, 2)) != LT_OK) return rc;
   if ((rc = grow_pair(&t->bnd, &t->bnd_face, &t->cap_bnd, nb, 1)) != LT_OK) return rc;
+  tic(t, 7);
   if ((rc = launch_connect_tables(t, G)) != LT_OK) return rc;
+  toc(t, 7);
   out->n_leaves = t->n;
   out->n_conf = nc;
   out->n_hang = nh;
@@ -472,8 +476,12 @@ int lt_transfer(lt_tree* t, const double* d_u_old, double* d_u_new, int p, int n
   if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
   if ((rc = build_operators(t, p)) != LT_OK) return rc;
   tic(t, 3);
+  tic(t, 4);
   if ((rc = launch_map(t)) != LT_OK) return rc;
+  toc(t, 4);
+  tic(t, 5);
   if ((rc = launch_transfer(t, d_u_old, d_u_new, p, nvars)) != LT_OK) return rc;
+  toc(t, 5);
   t->have_old = false;
   t->n_old = 0;
   t->map_valid = true;

@@ -72,8 +72,8 @@ struct Tree {
   uint64_t* sort_tmp; int64_t sort_cap; unsigned* sort_hist; unsigned* sort_status; int64_t sort_status_cap;
 
   int opt_adapt_sort, opt_full_sweeps, opt_debug_slack;
-  cudaEvent_t ev[8];
-  bool ev_set[4];
+  cudaEvent_t ev[16];
+  bool ev_set[8];
   int64_t launches;
 };
 

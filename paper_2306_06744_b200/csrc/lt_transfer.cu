@@ -65,91 +65,298 @@ __global__ void k_map_identity(const DevScalars* __restrict__ s, int32_t* __rest
 }
 
 // ------------------------------------------------------------------------ transfer
-// One warp per new element.  The three cases are warp-uniform branches.
-//   u[e][v][n], n = ix + P1*(iy + P1*iz) (reading E-5); E = nvars * N doubles per element.
-// A 1-D operator is applied along axis d to the flattened [v][n] block:
-//   out[k] = sum_i op[q][i] * in[k + (i - q) * P1^d],  q = (k / P1^d) % P1.
-template <int P1, int STRIDE>
-__device__ __forceinline__ double apply_1d(const double* __restrict__ op, const double* __restrict__ in, int k) {
-  const int q = (k / STRIDE) % P1;
-  const double* row = op + q * P1;
-  const double* col = in + (k - q * STRIDE);
-  double acc = 0.0;
-#pragma unroll
-  for (int i = 0; i < P1; ++i) acc = fma(row[i], col[i * STRIDE], acc);
-  return acc;
-}
+// One warp per unit of work, found by walking the new leaves (warp-uniform branches):
+//   copy     one new leaf: a streaming 128-bit copy of its E = nvars*N doubles;
+//   refine   one PARENT (the warp that meets child 0 does all 2^dim children, the warps
+//            that meet children 1.. skip): the parent is read once and the 1-D operators
+//            are applied one direction at a time with the intermediate results shared by
+//            the children (sum factorisation: 2N + 4N + 8N outputs of P1 FMAs each in 3-D
+//            instead of 8 * 3N);
+//   coarsen  one new parent: the mirror image, children pairs are fused direction by
+//            direction (4N + 2N + N outputs of 2*P1 FMAs).
+// Every stage works on "pencils": a lane loads the P1 values along the contraction
+// direction into registers and produces all outputs that depend on them, with the operator
+// entries coming straight from constant memory (compile-time indices -> immediate c[][]
+// operands of DFMA, no shared-memory or register traffic for coefficients).
+//   u[e][v][n], n = ix + P1*(iy + P1*iz) (reading E-5).
+//
+// c_ops[P1-1][which][row][col]: which 0,1 = I^0, I^1 (Eq. 8); 2,3 = R^0, R^1 (Eq. 12).
+__constant__ double c_ops[8][4][8][8];
+
+template <int P1> struct Pad {  // z-plane stride in shared memory (doubles): de-conflicts banks
+  static constexpr int PP = P1 * P1;
+  static constexpr int ZS = (PP % 16 == 0) ? PP + 4 : PP;
+};
 
 template <int DIM, int P1>
-__global__ void __launch_bounds__(256) k_transfer(const DevScalars* __restrict__ s,
+struct Xfer {
+  static constexpr int PP = P1 * P1;
+  static constexpr int N = DIM == 2 ? PP : PP * P1;
+  static constexpr int NC = 1 << DIM;
+  static constexpr int ZS = Pad<P1>::ZS;
+  static constexpr int NP = DIM == 2 ? PP : ZS * P1;     // padded size of one N-block
+  static constexpr int ROWS = N / P1;                     // x-pencils per variable
+  static constexpr int SMEM_DOUBLES = DIM == 2 ? 2 * NP : 6 * NP;  // per warp
+
+  // padded offset of node n (3-D only pads between z planes)
+  __device__ static __forceinline__ int off(int n) { return DIM == 2 ? n : (n / PP) * ZS + (n % PP); }
+
+  // ---- parent -> 2^dim children (Eq. 8)
+  __device__ static __forceinline__ void refine(const double* __restrict__ up, double* __restrict__ dst, int nvars,
+                                                size_t E, double* sm, int lane) {
+    double* t1 = sm;            // [2][NP]   after x
+    double* t2 = sm + 2 * NP;   // [4][NP]   after y (3-D)
+    for (int v = 0; v < nvars; ++v) {
+      const double* u = up + (size_t)v * N;
+      // stage x: lane = (bx, row); both halves of a row are produced by two lanes
+      for (int q = lane; q < 2 * ROWS; q += 32) {
+        const int bx = q / ROWS, r = q % ROWS;
+        double in[P1];
+        if (P1 % 2 == 0) {
+          const double2* u2 = reinterpret_cast<const double2*>(u + r * P1);
+#pragma unroll
+          for (int i = 0; i < P1 / 2; ++i) {
+            double2 t = __ldcs(u2 + i);
+            in[2 * i] = t.x;
+            in[2 * i + 1] = t.y;
+          }
+        } else {
+#pragma unroll
+          for (int i = 0; i < P1; ++i) in[i] = __ldcs(u + r * P1 + i);
+        }
+        double* o = t1 + bx * NP + off(r * P1);
+#pragma unroll
+        for (int m = 0; m < P1; ++m) {
+          double a0 = 0.0, a1 = 0.0;
+#pragma unroll
+          for (int i = 0; i < P1; ++i) {
+            a0 = fma(c_ops[P1 - 1][0][m][i], in[i], a0);
+            a1 = fma(c_ops[P1 - 1][1][m][i], in[i], a1);
+          }
+          o[m] = bx ? a1 : a0;
+        }
+      }
+      __syncwarp();
+      if (DIM == 2) {
+        // stage y: pencil (bx, x'); outputs go to children (bx, by)
+        for (int q = lane; q < 2 * P1; q += 32) {
+          const int bx = q / P1, x = q % P1;
+          double in[P1];
+#pragma unroll
+          for (int i = 0; i < P1; ++i) in[i] = t1[bx * NP + i * P1 + x];
+#pragma unroll
+          for (int by = 0; by < 2; ++by) {
+            double* d = dst + (size_t)(bx + 2 * by) * E + (size_t)v * N + x;
+#pragma unroll
+            for (int m = 0; m < P1; ++m) {
+              double a = 0.0;
+#pragma unroll
+              for (int i = 0; i < P1; ++i) a = fma(c_ops[P1 - 1][by][m][i], in[i], a);
+              __stcs(d + m * P1, a);
+            }
+          }
+        }
+      } else {
+        // stage y: pencil (bx, z, x')
+        for (int q = lane; q < 2 * PP; q += 32) {
+          const int bx = q / PP, z = (q % PP) / P1, x = q % P1;
+          double in[P1];
+#pragma unroll
+          for (int i = 0; i < P1; ++i) in[i] = t1[bx * NP + z * ZS + i * P1 + x];
+#pragma unroll
+          for (int by = 0; by < 2; ++by) {
+            double* o = t2 + (by * 2 + bx) * NP + z * ZS + x;
+#pragma unroll
+            for (int m = 0; m < P1; ++m) {
+              double a = 0.0;
+#pragma unroll
+              for (int i = 0; i < P1; ++i) a = fma(c_ops[P1 - 1][by][m][i], in[i], a);
+              o[m * P1] = a;
+            }
+          }
+        }
+        __syncwarp();
+        // stage z: pencil (cxy = bx + 2 by, rem = x' + P1 y'); outputs go to children cxy + 4 bz
+        for (int q = lane; q < 4 * PP; q += 32) {
+          const int cxy = q / PP, rem = q % PP;
+          double in[P1];
+#pragma unroll
+          for (int i = 0; i < P1; ++i) in[i] = t2[cxy * NP + i * ZS + rem];
+#pragma unroll
+          for (int bz = 0; bz < 2; ++bz) {
+            double* d = dst + (size_t)(cxy + 4 * bz) * E + (size_t)v * N + rem;
+#pragma unroll
+            for (int m = 0; m < P1; ++m) {
+              double a = 0.0;
+#pragma unroll
+              for (int i = 0; i < P1; ++i) a = fma(c_ops[P1 - 1][bz][m][i], in[i], a);
+              __stcs(d + m * PP, a);
+            }
+          }
+        }
+      }
+      __syncwarp();
+    }
+  }
+
+  // ---- 2^dim children -> parent (Eq. 9-13): u_P = sum_c (R^{bz} x R^{by} x R^{bx}) u_c
+  __device__ static __forceinline__ void coarsen(const double* __restrict__ uc, double* __restrict__ dst, int nvars,
+                                                 size_t E, double* sm, int lane) {
+    double* s1 = sm;            // [NC/2][NP]  after x (index: by + 2 bz)
+    double* s2 = sm + 4 * NP;   // [2][NP]     after y (3-D, index bz)
+    for (int v = 0; v < nvars; ++v) {
+      // stage x: pencil (cyz, row): fuse the children bx = 0, 1
+      for (int q = lane; q < (NC / 2) * ROWS; q += 32) {
+        const int cyz = q / ROWS, r = q % ROWS;
+        const double* a = uc + (size_t)(2 * cyz) * E + (size_t)v * N + r * P1;
+        const double* b = a + E;
+        double ia[P1], ib[P1];
+        if (P1 % 2 == 0) {
+#pragma unroll
+          for (int i = 0; i < P1 / 2; ++i) {
+            double2 t = __ldcs(reinterpret_cast<const double2*>(a) + i);
+            ia[2 * i] = t.x;
+            ia[2 * i + 1] = t.y;
+            t = __ldcs(reinterpret_cast<const double2*>(b) + i);
+            ib[2 * i] = t.x;
+            ib[2 * i + 1] = t.y;
+          }
+        } else {
+#pragma unroll
+          for (int i = 0; i < P1; ++i) {
+            ia[i] = __ldcs(a + i);
+            ib[i] = __ldcs(b + i);
+          }
+        }
+        double* o = s1 + cyz * NP + off(r * P1);
+#pragma unroll
+        for (int m = 0; m < P1; ++m) {
+          double acc = 0.0;
+#pragma unroll
+          for (int i = 0; i < P1; ++i) {
+            acc = fma(c_ops[P1 - 1][2][m][i], ia[i], acc);
+            acc = fma(c_ops[P1 - 1][3][m][i], ib[i], acc);
+          }
+          o[m] = acc;
+        }
+      }
+      __syncwarp();
+      if (DIM == 2) {
+        // stage y: pencil x'
+        for (int x = lane; x < P1; x += 32) {
+          double ia[P1], ib[P1];
+#pragma unroll
+          for (int i = 0; i < P1; ++i) {
+            ia[i] = s1[i * P1 + x];
+            ib[i] = s1[NP + i * P1 + x];
+          }
+          double* d = dst + (size_t)v * N + x;
+#pragma unroll
+          for (int m = 0; m < P1; ++m) {
+            double acc = 0.0;
+#pragma unroll
+            for (int i = 0; i < P1; ++i) {
+              acc = fma(c_ops[P1 - 1][2][m][i], ia[i], acc);
+              acc = fma(c_ops[P1 - 1][3][m][i], ib[i], acc);
+            }
+            __stcs(d + m * P1, acc);
+          }
+        }
+      } else {
+        // stage y: pencil (bz, z, x'): fuse by = 0, 1
+        for (int q = lane; q < 2 * PP; q += 32) {
+          const int bz = q / PP, z = (q % PP) / P1, x = q % P1;
+          double ia[P1], ib[P1];
+#pragma unroll
+          for (int i = 0; i < P1; ++i) {
+            ia[i] = s1[(2 * bz) * NP + z * ZS + i * P1 + x];
+            ib[i] = s1[(2 * bz + 1) * NP + z * ZS + i * P1 + x];
+          }
+          double* o = s2 + bz * NP + z * ZS + x;
+#pragma unroll
+          for (int m = 0; m < P1; ++m) {
+            double acc = 0.0;
+#pragma unroll
+            for (int i = 0; i < P1; ++i) {
+              acc = fma(c_ops[P1 - 1][2][m][i], ia[i], acc);
+              acc = fma(c_ops[P1 - 1][3][m][i], ib[i], acc);
+            }
+            o[m * P1] = acc;
+          }
+        }
+        __syncwarp();
+        // stage z: pencil rem = (y', x'): fuse bz = 0, 1
+        for (int rem = lane; rem < PP; rem += 32) {
+          double ia[P1], ib[P1];
+#pragma unroll
+          for (int i = 0; i < P1; ++i) {
+            ia[i] = s2[i * ZS + rem];
+            ib[i] = s2[NP + i * ZS + rem];
+          }
+          double* d = dst + (size_t)v * N + rem;
+#pragma unroll
+          for (int m = 0; m < P1; ++m) {
+            double acc = 0.0;
+#pragma unroll
+            for (int i = 0; i < P1; ++i) {
+              acc = fma(c_ops[P1 - 1][2][m][i], ia[i], acc);
+              acc = fma(c_ops[P1 - 1][3][m][i], ib[i], acc);
+            }
+            __stcs(d + m * PP, acc);
+          }
+        }
+      }
+      __syncwarp();
+    }
+  }
+};
+
+template <int DIM, int P1>
+__global__ void __launch_bounds__(256, 4) k_transfer(const DevScalars* __restrict__ s,
                                                   const int32_t* __restrict__ map_src,
                                                   const uint8_t* __restrict__ map_kind,
                                                   const double* __restrict__ u_old, double* __restrict__ u_new,
-                                                  int E, const double* __restrict__ ops_g, int vec2) {
-  constexpr int NC = Dim<DIM>::NC;
-  constexpr int PP = P1 * P1;
+                                                  int nvars, int vec2) {
+  using X = Xfer<DIM, P1>;
   extern __shared__ double smem[];
-  double* ops = smem;  // I^0, I^1, R^0, R^1
-  for (int i = threadIdx.x; i < 4 * PP; i += blockDim.x) ops[i] = ops_g[i];
-  __syncthreads();
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
-  double* b0 = smem + 4 * PP + (size_t)w * 3 * E;
-  double* b1 = b0 + E;
-  double* b2 = b1 + E;
+  double* wsm = smem + (size_t)w * X::SMEM_DOUBLES;
+  const size_t E = (size_t)nvars * X::N;
   const int64_t n = s->n;
   for (int64_t j = (int64_t)blockIdx.x * nw + w; j < n; j += (int64_t)gridDim.x * nw) {
     const int kd = map_kind[j];
     const int64_t so = map_src[j];
     double* dst = u_new + (size_t)j * E;
+    const double* sp = u_old + (size_t)so * E;
     if ((kd & 15) == 0) {  // direct copy
-      const double* sp = u_old + (size_t)so * E;
       if (vec2) {
         const double2* s2 = reinterpret_cast<const double2*>(sp);
         double2* d2 = reinterpret_cast<double2*>(dst);
-        for (int k = lane; k < E / 2; k += 32) __stcs(d2 + k, __ldcs(s2 + k));
+        const int T = (int)(E / 2);
+        for (int k = lane; k < T; k += 32 * 4) {
+          double2 r[4];
+#pragma unroll
+          for (int q = 0; q < 4; ++q)
+            if (k + 32 * q < T) r[q] = __ldcs(s2 + k + 32 * q);
+#pragma unroll
+          for (int q = 0; q < 4; ++q)
+            if (k + 32 * q < T) __stcs(d2 + k + 32 * q, r[q]);
+        }
       } else {
-        for (int k = lane; k < E; k += 32) __stcs(dst + k, __ldcs(sp + k));
+        for (int k = lane; k < (int)E; k += 32 * 4) {
+          double r[4];
+#pragma unroll
+          for (int q = 0; q < 4; ++q)
+            if (k + 32 * q < (int)E) r[q] = __ldcs(sp + k + 32 * q);
+#pragma unroll
+          for (int q = 0; q < 4; ++q)
+            if (k + 32 * q < (int)E) __stcs(dst + k + 32 * q, r[q]);
+        }
       }
     } else if ((kd & 15) == 1) {  // interpolation, Eq. 8
-      const int cid = kd >> 4;
-      const double* sp = u_old + (size_t)so * E;
-      for (int k = lane; k < E; k += 32) b0[k] = sp[k];
-      __syncwarp();
-      const double* ox = ops + ((cid >> 0) & 1) * PP;
-      const double* oy = ops + ((cid >> 1) & 1) * PP;
-      for (int k = lane; k < E; k += 32) b1[k] = apply_1d<P1, 1>(ox, b0, k);
-      __syncwarp();
-      if (DIM == 2) {
-        for (int k = lane; k < E; k += 32) __stcs(dst + k, apply_1d<P1, P1>(oy, b1, k));
-      } else {
-        const double* oz = ops + ((cid >> 2) & 1) * PP;
-        for (int k = lane; k < E; k += 32) b0[k] = apply_1d<P1, P1>(oy, b1, k);
-        __syncwarp();
-        for (int k = lane; k < E; k += 32) __stcs(dst + k, apply_1d<P1, PP>(oz, b0, k));
-      }
-      __syncwarp();
-    } else {  // L2 projection of the NC children, Eq. 9-13
-      for (int k = lane; k < E; k += 32) b2[k] = 0.0;
-      for (int c = 0; c < NC; ++c) {
-        const double* sp = u_old + (size_t)(so + c) * E;
-        for (int k = lane; k < E; k += 32) b0[k] = __ldcs(sp + k);
-        __syncwarp();
-        const double* ox = ops + (2 + ((c >> 0) & 1)) * PP;
-        const double* oy = ops + (2 + ((c >> 1) & 1)) * PP;
-        for (int k = lane; k < E; k += 32) b1[k] = apply_1d<P1, 1>(ox, b0, k);
-        __syncwarp();
-        if (DIM == 2) {
-          for (int k = lane; k < E; k += 32) b2[k] += apply_1d<P1, P1>(oy, b1, k);
-        } else {
-          const double* oz = ops + (2 + ((c >> 2) & 1)) * PP;
-          for (int k = lane; k < E; k += 32) b0[k] = apply_1d<P1, P1>(oy, b1, k);
-          __syncwarp();
-          for (int k = lane; k < E; k += 32) b2[k] += apply_1d<P1, PP>(oz, b0, k);
-        }
-        __syncwarp();
-      }
-      for (int k = lane; k < E; k += 32) __stcs(dst + k, b2[k]);
-      __syncwarp();
+      if ((kd >> 4) == 0) X::refine(sp, dst, nvars, E, wsm, lane);  // children 1.. are written with child 0
+    } else {  // L2 projection of the 2^dim children, Eq. 9-13
+      X::coarsen(sp, dst, nvars, E, wsm, lane);
     }
   }
 }
@@ -192,11 +399,13 @@ static void gl_rule(int n, std::vector<long double>& z, std::vector<long double>
 }
 
 int build_operators(Tree* t, int p) {
-  if (t->ops_p == p && t->d_ops) return LT_OK;
-  const int P1 = p + 1, PP = P1 * P1;
+  static bool uploaded[64][8];  // per device, per P1
+  const int dev = t->device & 63;
+  if (uploaded[dev][p]) return LT_OK;
+  const int P1 = p + 1;
   std::vector<long double> z, w;
   gl_rule(P1, z, w);
-  std::vector<double> h(4 * PP);
+  std::vector<double> h(4 * 64, 0.0);
   for (int b = 0; b < 2; ++b)
     for (int m = 0; m < P1; ++m) {
       const long double xi = 0.5L * (z[m] + 2 * b - 1);
@@ -204,14 +413,13 @@ int build_operators(Tree* t, int p) {
         long double v = 1.0L;
         for (int k = 0; k < P1; ++k)
           if (k != i) v *= (xi - z[k]) / (z[i] - z[k]);
-        h[b * PP + m * P1 + i] = (double)v;                                  // I^b[m][i]
-        h[(2 + b) * PP + i * P1 + m] = (double)(0.5L * (w[m] / w[i]) * v);   // R^b[i][m]
+        h[b * 64 + m * 8 + i] = (double)v;                                // I^b[m][i]
+        h[(2 + b) * 64 + i * 8 + m] = (double)(0.5L * (w[m] / w[i]) * v);  // R^b[i][m]
       }
     }
-  if (!t->d_ops) LT_CUDA(cudaMalloc(&t->d_ops, 4 * 64 * sizeof(double)));
-  LT_CUDA(cudaMemcpyAsync(t->d_ops, h.data(), 4 * PP * sizeof(double), cudaMemcpyHostToDevice, t->stream));
-  LT_CUDA(cudaStreamSynchronize(t->stream));  // h goes out of scope
-  t->ops_p = p;
+  LT_CUDA(cudaMemcpyToSymbol(c_ops, h.data(), 4 * 64 * sizeof(double), (size_t)p * 4 * 64 * sizeof(double),
+                             cudaMemcpyHostToDevice));
+  uploaded[dev][p] = true;
   return LT_OK;
 }
 
@@ -232,37 +440,35 @@ int launch_map(Tree* t) {
 }
 
 template <int DIM, int P1>
-static int launch_transfer_t(Tree* t, const double* u_old, double* u_new, int E, int vec2) {
-  const int PP = P1 * P1;
+static int launch_transfer_t(Tree* t, const double* u_old, double* u_new, int nvars, int vec2) {
+  using X = Xfer<DIM, P1>;
   int warps = 8;
-  size_t per_warp = (size_t)3 * E * sizeof(double);
-  const size_t budget = 200 * 1024 - 4 * PP * sizeof(double);
-  while (warps > 1 && warps * per_warp > budget) warps >>= 1;
-  if (warps * per_warp > budget) return LT_ERR_ARG;
-  size_t smem = 4 * PP * sizeof(double) + warps * per_warp;
+  const size_t per_warp = (size_t)X::SMEM_DOUBLES * sizeof(double);
+  while (warps > 1 && warps * per_warp > 96 * 1024) warps >>= 1;
+  const size_t smem = warps * per_warp;
   auto fn = k_transfer<DIM, P1>;
   LT_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int per_sm = 0;
   LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, warps * 32, smem));
   if (per_sm < 1) per_sm = 1;
-  int G = t->num_sms * per_sm;
-  fn<<<G, warps * 32, smem, t->stream>>>(t->d_s, t->map_src, t->map_kind, u_old, u_new, E, t->d_ops, vec2);
+  const int G = t->num_sms * per_sm;
+  fn<<<G, warps * 32, smem, t->stream>>>(t->d_s, t->map_src, t->map_kind, u_old, u_new, nvars, vec2);
   t->launches++;
   LT_CUDA(cudaGetLastError());
   return LT_OK;
 }
 
 template <int DIM>
-static int launch_transfer_d(Tree* t, const double* u_old, double* u_new, int p, int E, int vec2) {
+static int launch_transfer_d(Tree* t, const double* u_old, double* u_new, int p, int nvars, int vec2) {
   switch (p) {
-    case 0: return launch_transfer_t<DIM, 1>(t, u_old, u_new, E, vec2);
-    case 1: return launch_transfer_t<DIM, 2>(t, u_old, u_new, E, vec2);
-    case 2: return launch_transfer_t<DIM, 3>(t, u_old, u_new, E, vec2);
-    case 3: return launch_transfer_t<DIM, 4>(t, u_old, u_new, E, vec2);
-    case 4: return launch_transfer_t<DIM, 5>(t, u_old, u_new, E, vec2);
-    case 5: return launch_transfer_t<DIM, 6>(t, u_old, u_new, E, vec2);
-    case 6: return launch_transfer_t<DIM, 7>(t, u_old, u_new, E, vec2);
-    case 7: return launch_transfer_t<DIM, 8>(t, u_old, u_new, E, vec2);
+    case 0: return launch_transfer_t<DIM, 1>(t, u_old, u_new, nvars, vec2);
+    case 1: return launch_transfer_t<DIM, 2>(t, u_old, u_new, nvars, vec2);
+    case 2: return launch_transfer_t<DIM, 3>(t, u_old, u_new, nvars, vec2);
+    case 3: return launch_transfer_t<DIM, 4>(t, u_old, u_new, nvars, vec2);
+    case 4: return launch_transfer_t<DIM, 5>(t, u_old, u_new, nvars, vec2);
+    case 5: return launch_transfer_t<DIM, 6>(t, u_old, u_new, nvars, vec2);
+    case 6: return launch_transfer_t<DIM, 7>(t, u_old, u_new, nvars, vec2);
+    case 7: return launch_transfer_t<DIM, 8>(t, u_old, u_new, nvars, vec2);
   }
   return LT_ERR_ARG;
 }
@@ -272,8 +478,8 @@ int launch_transfer(Tree* t, const double* d_u_old, double* d_u_new, int p, int 
   for (int a = 0; a < t->g.dim; ++a) N *= (p + 1);
   const int E = nvars * N;
   const int vec2 = (E % 2 == 0) && (((uintptr_t)d_u_old & 15) == 0) && (((uintptr_t)d_u_new & 15) == 0);
-  return t->g.dim == 2 ? launch_transfer_d<2>(t, d_u_old, d_u_new, p, E, vec2)
-                       : launch_transfer_d<3>(t, d_u_old, d_u_new, p, E, vec2);
+  return t->g.dim == 2 ? launch_transfer_d<2>(t, d_u_old, d_u_new, p, nvars, vec2)
+                       : launch_transfer_d<3>(t, d_u_old, d_u_new, p, nvars, vec2);
 }
 
 }  // namespace lt

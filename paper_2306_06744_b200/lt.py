@@ -147,8 +147,11 @@ class Tree:
 
     def free(self):
         h = getattr(self, "_h", None)
-        if h:
-            lib().lt_free(h)
+        if h and _lib is not None:
+            try:
+                _lib.lt_free(h)
+            except Exception:  # interpreter shutdown
+                pass
             self._h = None
 
     # ---- the cycle
@@ -239,9 +242,10 @@ class Tree:
         _check(lib().lt_set_option(self._h, option, value), "lt_set_option")
 
     def timings(self):
-        out = (C.c_float * 4)()
+        out = (C.c_float * 8)()
         _check(lib().lt_timings(self._h, out), "lt_timings")
-        return dict(adapt=out[0], balance=out[1], connect=out[2], transfer=out[3])
+        return dict(adapt=out[0], balance=out[1], connect=out[2], transfer=out[3], k_map=out[4], k_transfer=out[5],
+                    k_connect_search=out[6], k_connect_tables=out[7])
 
     def launch_count(self) -> int:
         return int(lib().lt_launch_count(self._h))
