@@ -30,7 +30,7 @@ if ROOT not in sys.path:
 METRIC = "leaves/s per full adapt+2:1 balance+connectivity+transfer cycle"
 UNIT = "leaves/s"
 PREP_CYCLES = 3           # config-5 cycles 0..2 run untimed to develop the tree
-PERIOD = (3, 4, 5)        # config-5 cycles a step runs
+PERIOD = (3, 4, 5)        # config-5 cycles a step runs (--cycles a,b,.. overrides: profiling aid)
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 
 
@@ -196,6 +196,23 @@ class Runner:
         return M
 
 
+def max_over_ranks(ms, world, device):
+    """Timing rule for N > 1: the slowest rank's device time (all-reduce MAX)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    tt = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
+def whole_job_value(leaves_per_rank, world, ms):
+    """Replicas only: every rank runs the same independent workload,
+    so the job processed world * leaves in the slowest rank's time."""
+    return world * leaves_per_rank / (ms * 1e-3)
+
+
 def algorithmic_bytes(dim, M0, Ma, M1, n_faces3, Bu):
     """SURVEY.md 8(d) minimal bytes of the kernels actually run (path B), per cycle."""
     nf = 2 * dim
@@ -306,14 +323,10 @@ def run_ours(args):
     t_wall = time.perf_counter() - t_wall0
     clocks = sampler.stop()
 
-    tot_ms = sum(s["ms"] for s in steps)
-    if world > 1:
-        tt = torch.tensor([tot_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        tot_ms = float(tt.item())
+    tot_ms = max_over_ranks(sum(s["ms"] for s in steps), world, dev)
     leaves = sum(s["M1"] for s in steps)
     faces = sum(sum(s["faces"]) for s in steps)
-    value = world * leaves / (tot_ms * 1e-3)
+    value = whole_job_value(leaves, world, tot_ms)
 
     # ---- roofline of the dominant kernel (k_transfer): algorithmic bytes / measured kernel time
     peak, peak_src = hbm_peak()
@@ -354,11 +367,8 @@ def run_ours(args):
         R.tree = None
         torch.cuda.empty_cache()
         e2e = run_e2e(R, args, world, dev)
-        if world > 1:
-            tt = torch.tensor([e2e["ms"]], dtype=torch.float64, device=dev)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            e2e["ms"] = float(tt.item())
-        e2e["value"] = world * e2e["leaves"] / (e2e["ms"] * 1e-3)
+        e2e["ms"] = max_over_ranks(e2e["ms"], world, dev)
+        e2e["value"] = whole_job_value(e2e["leaves"], world, e2e["ms"])
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -375,7 +385,7 @@ def run_ours(args):
                                    "max level +3, vortex-tube flags + 10% random refine / 10% random group coarsen "
                                    "(seed 2), p=3 (64 solution points), 5 fp64 vars",
                        "step": "one adaptation cycle; steps run config-5 cycles %s after an untimed tree-only "
-                               "replay of cycles 0-2" % (list(PERIOD),),
+                               "replay of cycles 0-%d" % (list(PERIOD), PREP_CYCLES - 1),
                        "leaves_out_per_step": [s["M1"] for s in steps], "leaves_in_per_step": [s["M0"] for s in steps],
                        "balance_iters": [s["iters"] for s in steps],
                        "l2": "inputs larger than L2 (u_old + u_new are 57-115 GB per step)",
@@ -461,7 +471,15 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cycles", default=None,
+                    help="consecutive config-5 cycles a step cycles through (default 3,4,5 = the bench "
+                         "workload; smaller ones, e.g. 2, keep an ncu --set full capture short)")
     args = ap.parse_args()
+    if args.cycles:
+        global PERIOD, PREP_CYCLES
+        PERIOD = tuple(int(c) for c in args.cycles.split(","))
+        assert all(b == a + 1 for a, b in zip(PERIOD, PERIOD[1:])), "--cycles must be consecutive"
+        PREP_CYCLES = PERIOD[0]
     if args.steps < 1:
         args.steps = 1
     if args.impl == "reference":

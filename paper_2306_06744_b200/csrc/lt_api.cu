@@ -44,6 +44,8 @@ static int grow(Tree* t, int64_t need) {
   uint8_t* kind = nullptr;
   int32_t* msrc = nullptr;
   uint8_t* mkind = nullptr;
+  int32_t* frows = nullptr;
+  uint8_t* fbytes = nullptr;
   int rc = LT_OK;
   for (int b = 0; b < 3 && rc == LT_OK; ++b) rc = alloc_dev(&nk[b], cap);
   if (rc == LT_OK) rc = alloc_dev(&mark, cap);
@@ -53,9 +55,14 @@ static int grow(Tree* t, int64_t need) {
   if (rc == LT_OK) rc = alloc_dev(&kind, cap * nf);
   if (rc == LT_OK) rc = alloc_dev(&msrc, cap);
   if (rc == LT_OK) rc = alloc_dev(&mkind, cap);
+  // face-table pool: every (leaf, face) slot emits at most one row into exactly one of the
+  // three tables, so nf*cap rows (of at most 2 int32 + 1 byte) hold all of them
+  if (rc == LT_OK) rc = alloc_dev(&frows, cap * nf * 2);
+  if (rc == LT_OK) rc = alloc_dev(&fbytes, cap * nf);
   if (rc != LT_OK) {
     for (int b = 0; b < 3; ++b) free_dev(nk[b]);
     free_dev(mark); free_dev(fr[0]); free_dev(fr[1]); free_dev(nbr); free_dev(kind); free_dev(msrc); free_dev(mkind);
+    free_dev(frows); free_dev(fbytes);
     return rc;
   }
   if (t->keys[t->cur] && t->n_valid && t->n > 0)
@@ -75,24 +82,11 @@ static int grow(Tree* t, int64_t need) {
   free_dev(t->kind); t->kind = kind;
   free_dev(t->map_src); t->map_src = msrc;
   free_dev(t->map_kind); t->map_kind = mkind;
+  free_dev(t->face_rows); t->face_rows = frows;
+  free_dev(t->face_bytes); t->face_bytes = fbytes;
   t->map_valid = false;
   t->cap = cap;
   return LT_OK;
-}
-
-// a face table (rows of `width` int32) and its byte column, grown together
-static int grow_pair(int32_t** rows, uint8_t** bytes, int64_t* cap, int64_t need, int width) {
-  if (need <= *cap && *rows && *bytes) return LT_OK;
-  free_dev(*rows);
-  free_dev(*bytes);
-  *rows = nullptr;
-  *bytes = nullptr;
-  *cap = 0;
-  const int64_t c = round_cap(need + need / 8);
-  int rc = alloc_dev(rows, c * width);
-  if (rc == LT_OK) rc = alloc_dev(bytes, c);
-  if (rc == LT_OK) *cap = c;
-  return rc;
 }
 
 // copy the device scalars to the pinned mirror and wait
@@ -216,8 +210,7 @@ void lt_free(lt_tree* t) {
   if (t->h_sums) cudaFreeHost(t->h_sums);
   free_dev(t->mark); free_dev(t->frontier[0]); free_dev(t->frontier[1]);
   free_dev(t->nbr); free_dev(t->kind);
-  free_dev(t->conf); free_dev(t->conf_axis); free_dev(t->hang); free_dev(t->hang_info);
-  free_dev(t->bnd); free_dev(t->bnd_face);
+  free_dev(t->face_rows); free_dev(t->face_bytes);
   free_dev(t->map_src); free_dev(t->map_kind); free_dev(t->d_ops);
   free_dev(t->stage_old); free_dev(t->stage_new);
   free_dev(t->sort_tmp); free_dev(t->sort_hist); free_dev(t->sort_status);
@@ -437,34 +430,27 @@ int lt_connect(lt_tree* t, lt_faces* out) {
   tic(t, 6);
   if ((rc = launch_connect_search(t, G)) != LT_OK) return rc;
   toc(t, 6);
-  LT_CUDA(cudaMemcpyAsync(t->h_sums, t->d_sums3, (size_t)3 * G * sizeof(int), cudaMemcpyDeviceToHost, t->stream));
-  if ((rc = fetch_scalars(t)) != LT_OK) return rc;
-  const int st = take_status(t);
-  if (st != LT_OK) return st;
-  int64_t nc = 0, nh = 0, nb = 0;
-  for (int b = 0; b < G; ++b) {
-    nc += t->h_sums[3 * b];
-    nh += t->h_sums[3 * b + 1];
-    nb += t->h_sums[3 * b + 2];
-  }
-  if ((rc = grow_pair(&t->conf, &t->conf_axis, &t->cap_conf, nc, 2)) != LT_OK) return rc;
-  if ((rc = grow_pair(&t->hang, &t->hang_info, &t->cap_hang, nh, 2)) != LT_OK) return rc;
-  if ((rc = grow_pair(&t->bnd, &t->bnd_face, &t->cap_bnd, nb, 1)) != LT_OK) return rc;
+  // the table kernel places the three tables back to back in the pool from the chunk sums it
+  // reads itself, so it is enqueued before the counts travel to the host
   tic(t, 7);
   if ((rc = launch_connect_tables(t, G)) != LT_OK) return rc;
   toc(t, 7);
+  if ((rc = fetch_scalars(t)) != LT_OK) return rc;
+  const int st = take_status(t);
+  if (st != LT_OK) return st;
+  const int64_t nc = t->h_s->n_face[0], nh = t->h_s->n_face[1], nb = t->h_s->n_face[2];
   out->n_leaves = t->n;
   out->n_conf = nc;
   out->n_hang = nh;
   out->n_bnd = nb;
   out->nbr = t->nbr;
   out->kind = t->kind;
-  out->conf = t->conf;
-  out->conf_axis = t->conf_axis;
-  out->hang = t->hang;
-  out->hang_info = t->hang_info;
-  out->bnd = t->bnd;
-  out->bnd_face = t->bnd_face;
+  out->conf = t->face_rows;
+  out->conf_axis = t->face_bytes;
+  out->hang = t->face_rows + 2 * nc;
+  out->hang_info = t->face_bytes + nc;
+  out->bnd = t->face_rows + 2 * (nc + nh);
+  out->bnd_face = t->face_bytes + nc + nh;
   toc(t, 2);
   return LT_OK;
 }

@@ -80,27 +80,47 @@ __global__ void __launch_bounds__(CT) k_connect_search(Geo g, const uint64_t* __
   }
 }
 
+// The three tables live back to back in one pool of nf*cap rows (every slot emits at most
+// one row): conf rows [0, n_conf), hang rows [n_conf, n_conf + n_hang), then bnd.  The
+// region offsets come from the chunk sums, so no host round trip separates the passes.
 template <int DIM>
-__global__ void __launch_bounds__(CT) k_connect_tables(const DevScalars* __restrict__ s,
+__global__ void __launch_bounds__(CT) k_connect_tables(DevScalars* __restrict__ s,
                                                        const int32_t* __restrict__ nbr,
                                                        const uint8_t* __restrict__ kind,
-                                                       const int* __restrict__ sums3, int32_t* __restrict__ conf,
-                                                       uint8_t* __restrict__ conf_axis, int32_t* __restrict__ hang,
-                                                       uint8_t* __restrict__ hang_info, int32_t* __restrict__ bnd,
-                                                       uint8_t* __restrict__ bnd_face) {
+                                                       const int* __restrict__ sums3, int32_t* __restrict__ rows,
+                                                       uint8_t* __restrict__ bytes) {
   constexpr int NF = Dim<DIM>::NF;
   __shared__ unsigned long long sm[33];
   const int64_t nslots = (int64_t)s->n * NF;
-  // prefix of the three counters over the chunks before this one
-  unsigned long long b0 = 0, b1 = 0, b2 = 0;
-  for (int i = threadIdx.x; i < (int)blockIdx.x; i += CT) {
-    b0 += sums3[3 * i];
-    b1 += sums3[3 * i + 1];
-    b2 += sums3[3 * i + 2];
+  // prefix of the three counters over the chunks before this one, and their totals
+  unsigned long long b0 = 0, b1 = 0, b2 = 0, a0 = 0, a1 = 0, a2 = 0;
+  for (int i = threadIdx.x; i < (int)gridDim.x; i += CT) {
+    const unsigned long long c0 = sums3[3 * i], c1 = sums3[3 * i + 1], c2 = sums3[3 * i + 2];
+    a0 += c0;
+    a1 += c1;
+    a2 += c2;
+    if (i < (int)blockIdx.x) {
+      b0 += c0;
+      b1 += c1;
+      b2 += c2;
+    }
   }
   int64_t r_conf = (int64_t)block_sum(b0, sm);
   int64_t r_hang = (int64_t)block_sum(b1, sm);
   int64_t r_bnd = (int64_t)block_sum(b2, sm);
+  const int64_t n_conf = (int64_t)block_sum(a0, sm), n_hang = (int64_t)block_sum(a1, sm);
+  const int64_t n_bnd = (int64_t)block_sum(a2, sm);
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    s->n_face[0] = (int)n_conf;
+    s->n_face[1] = (int)n_hang;
+    s->n_face[2] = (int)n_bnd;
+  }
+  int32_t* __restrict__ conf = rows;
+  int32_t* __restrict__ hang = rows + 2 * n_conf;
+  int32_t* __restrict__ bnd = rows + 2 * (n_conf + n_hang);
+  uint8_t* __restrict__ conf_axis = bytes;
+  uint8_t* __restrict__ hang_info = bytes + n_conf;
+  uint8_t* __restrict__ bnd_face = bytes + n_conf + n_hang;
   int64_t lo, hi;
   block_chunk(nslots, gridDim.x, blockIdx.x, CT, &lo, &hi);
   for (int64_t t0 = lo; t0 < hi; t0 += CT) {
@@ -152,11 +172,9 @@ int launch_connect_search(Tree* t, int G) {
 
 int launch_connect_tables(Tree* t, int G) {
   if (t->g.dim == 2)
-    k_connect_tables<2><<<G, CT, 0, t->stream>>>(t->d_s, t->nbr, t->kind, t->d_sums3, t->conf, t->conf_axis, t->hang,
-                                                 t->hang_info, t->bnd, t->bnd_face);
+    k_connect_tables<2><<<G, CT, 0, t->stream>>>(t->d_s, t->nbr, t->kind, t->d_sums3, t->face_rows, t->face_bytes);
   else
-    k_connect_tables<3><<<G, CT, 0, t->stream>>>(t->d_s, t->nbr, t->kind, t->d_sums3, t->conf, t->conf_axis, t->hang,
-                                                 t->hang_info, t->bnd, t->bnd_face);
+    k_connect_tables<3><<<G, CT, 0, t->stream>>>(t->d_s, t->nbr, t->kind, t->d_sums3, t->face_rows, t->face_bytes);
   t->launches++;
   LT_CUDA(cudaGetLastError());
   return LT_OK;

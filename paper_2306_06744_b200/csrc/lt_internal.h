@@ -51,10 +51,9 @@ struct Tree {
   // connectivity
   int32_t* nbr;
   uint8_t* kind;
-  int64_t cap_conf, cap_hang, cap_bnd;
-  int32_t* conf; uint8_t* conf_axis;
-  int32_t* hang; uint8_t* hang_info;
-  int32_t* bnd;  uint8_t* bnd_face;
+  // face-table pool [cap*nf] rows: conf | hang | bnd back to back (lt_connect)
+  int32_t* face_rows;     // [cap*nf*2]
+  uint8_t* face_bytes;    // [cap*nf]
 
   // Alg. 7 map
   int32_t* map_src;
