@@ -19,7 +19,7 @@ struct DevScalars {
   int aux;               // scratch counter (path-A append cursor, sort tickets)
   unsigned long long volume;  // build_from_keys: sum of leaf volumes
   int splits;            // balance: leaves split in total
-  int pad;
+  unsigned ticket;       // tile ticket of the persistent kernels (zeroed before each launch)
 };
 
 constexpr int kMaxGrid = 4096;  // upper bound on persistent grid sizes (chunk-sum arrays)
