@@ -139,7 +139,8 @@ int lt_connect(lt_tree*, lt_faces* out);
  * child's solution points (Eq. 8), L2 projection of the 2^dim children (Eq. 9-13).
  *   d_u_old device [n_old][nvars][N] fp64, d_u_new device [lt_num_leaves][nvars][N] fp64,
  *   N = (p+1)^dim Gauss-Legendre solution points, x fastest (readings E-1, E-5).
- *   The arrays must not overlap.  1 <= p+1 <= 8 (p = 0..7), nvars >= 1.
+ *   The arrays must not overlap and must be 16-byte aligned (cudaMalloc / torch allocations
+ *   are).  1 <= p+1 <= 8 (p = 0..7), nvars >= 1.
  * Without a snapshot this is a plain copy.  Drops the snapshot.  Asynchronous; a mapping
  * error is sticky and is returned by this call only if detected before it returns --
  * lt_sync reports it otherwise. */
@@ -194,7 +195,7 @@ int lt_set_option(lt_tree*, int option, int value);
 /* Device times of the last cycle in milliseconds (CUDA events on the tree's stream):
  * out[0..3] = the calls lt_adapt, lt_balance, lt_connect, lt_transfer; out[4] = the Alg. 7
  * map kernel alone, out[5] = the solution-transfer kernel alone, out[6] = the connectivity
- * search kernel alone, out[7] = the face-table kernel alone; 0 where not run.
+ * kernel alone, out[7] = reserved (0); 0 where not run.
  * Synchronises. */
 int lt_timings(lt_tree*, float* out8);
 /* Number of kernels liblt launched on this tree since it was built. */

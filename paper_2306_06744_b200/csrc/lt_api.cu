@@ -36,7 +36,7 @@ static int grow(Tree* t, int64_t need) {
   int64_t cap = round_cap(need + need / 4);
   if (cap >= (1ll << 31) - 1024) cap = round_cap(need);
   LT_CUDA(cudaStreamSynchronize(t->stream));
-  const int nf = 2 * t->g.dim;
+  const int dim = t->g.dim, nf = 2 * dim;
   uint64_t* nk[3] = {nullptr, nullptr, nullptr};
   uint8_t* mark = nullptr;
   int* fr[2] = {nullptr, nullptr};
@@ -46,6 +46,7 @@ static int grow(Tree* t, int64_t need) {
   uint8_t* mkind = nullptr;
   int32_t* frows = nullptr;
   uint8_t* fbytes = nullptr;
+  unsigned long long* tstate = nullptr;
   int rc = LT_OK;
   for (int b = 0; b < 3 && rc == LT_OK; ++b) rc = alloc_dev(&nk[b], cap);
   if (rc == LT_OK) rc = alloc_dev(&mark, cap);
@@ -55,14 +56,15 @@ static int grow(Tree* t, int64_t need) {
   if (rc == LT_OK) rc = alloc_dev(&kind, cap * nf);
   if (rc == LT_OK) rc = alloc_dev(&msrc, cap);
   if (rc == LT_OK) rc = alloc_dev(&mkind, cap);
-  // face-table pool: every (leaf, face) slot emits at most one row into exactly one of the
-  // three tables, so nf*cap rows (of at most 2 int32 + 1 byte) hold all of them
-  if (rc == LT_OK) rc = alloc_dev(&frows, cap * nf * 2);
-  if (rc == LT_OK) rc = alloc_dev(&fbytes, cap * nf);
+  // face-table pool with fixed regions (lt_connect.cu face_regions): n_conf, n_hang <= dim*M
+  // rows of 2 int32, n_bnd <= nf*M rows of 1 int32, one byte per row
+  if (rc == LT_OK) rc = alloc_dev(&frows, cap * (4 * dim + nf));
+  if (rc == LT_OK) rc = alloc_dev(&fbytes, cap * (2 * dim + nf));
+  if (rc == LT_OK) rc = alloc_dev(&tstate, 2 * (cap / 256 + 2));
   if (rc != LT_OK) {
     for (int b = 0; b < 3; ++b) free_dev(nk[b]);
     free_dev(mark); free_dev(fr[0]); free_dev(fr[1]); free_dev(nbr); free_dev(kind); free_dev(msrc); free_dev(mkind);
-    free_dev(frows); free_dev(fbytes);
+    free_dev(frows); free_dev(fbytes); free_dev(tstate);
     return rc;
   }
   if (t->keys[t->cur] && t->n_valid && t->n > 0)
@@ -84,6 +86,7 @@ static int grow(Tree* t, int64_t need) {
   free_dev(t->map_kind); t->map_kind = mkind;
   free_dev(t->face_rows); t->face_rows = frows;
   free_dev(t->face_bytes); t->face_bytes = fbytes;
+  free_dev(t->tile_state); t->tile_state = tstate;
   t->map_valid = false;
   t->cap = cap;
   return LT_OK;
@@ -210,7 +213,7 @@ void lt_free(lt_tree* t) {
   if (t->h_sums) cudaFreeHost(t->h_sums);
   free_dev(t->mark); free_dev(t->frontier[0]); free_dev(t->frontier[1]);
   free_dev(t->nbr); free_dev(t->kind);
-  free_dev(t->face_rows); free_dev(t->face_bytes);
+  free_dev(t->face_rows); free_dev(t->face_bytes); free_dev(t->tile_state);
   free_dev(t->map_src); free_dev(t->map_kind); free_dev(t->d_ops);
   free_dev(t->stage_old); free_dev(t->stage_new);
   free_dev(t->sort_tmp); free_dev(t->sort_hist); free_dev(t->sort_status);
@@ -426,15 +429,9 @@ int lt_connect(lt_tree* t, lt_faces* out) {
   int rc;
   if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
   tic(t, 2);
-  const int G = grid_for(t, 8);
   tic(t, 6);
-  if ((rc = launch_connect_search(t, G)) != LT_OK) return rc;
+  if ((rc = launch_connect(t)) != LT_OK) return rc;
   toc(t, 6);
-  // the table kernel places the three tables back to back in the pool from the chunk sums it
-  // reads itself, so it is enqueued before the counts travel to the host
-  tic(t, 7);
-  if ((rc = launch_connect_tables(t, G)) != LT_OK) return rc;
-  toc(t, 7);
   if ((rc = fetch_scalars(t)) != LT_OK) return rc;
   const int st = take_status(t);
   if (st != LT_OK) return st;
@@ -445,12 +442,17 @@ int lt_connect(lt_tree* t, lt_faces* out) {
   out->n_bnd = nb;
   out->nbr = t->nbr;
   out->kind = t->kind;
-  out->conf = t->face_rows;
-  out->conf_axis = t->face_bytes;
-  out->hang = t->face_rows + 2 * nc;
-  out->hang_info = t->face_bytes + nc;
-  out->bnd = t->face_rows + 2 * (nc + nh);
-  out->bnd_face = t->face_bytes + nc + nh;
+  {
+    int32_t *conf, *hang, *bnd;
+    uint8_t *conf_axis, *hang_info, *bnd_face;
+    face_regions(t, &conf, &conf_axis, &hang, &hang_info, &bnd, &bnd_face);
+    out->conf = conf;
+    out->conf_axis = conf_axis;
+    out->hang = hang;
+    out->hang_info = hang_info;
+    out->bnd = bnd;
+    out->bnd_face = bnd_face;
+  }
   toc(t, 2);
   return LT_OK;
 }
@@ -458,6 +460,8 @@ int lt_connect(lt_tree* t, lt_faces* out) {
 // ---------------------------------------------------------------------------- transfer
 int lt_transfer(lt_tree* t, const double* d_u_old, double* d_u_new, int p, int nvars) {
   if (!t || !d_u_old || !d_u_new || p < 0 || p > 7 || nvars < 1) return LT_ERR_ARG;
+  // the kernels move x-pencils of an even number of doubles with 128-bit accesses
+  if ((p + 1) % 2 == 0 && ((((uintptr_t)d_u_old) | ((uintptr_t)d_u_new)) & 15)) return LT_ERR_ARG;
   int rc;
   if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
   if ((rc = build_operators(t, p)) != LT_OK) return rc;

@@ -1,13 +1,19 @@
-// lt_connect.cu -- face connectivity (Alg. 5) for sm_100a: one thread per
-// (leaf, local face) slot builds the same-level search key, locates it in the sorted leaf
-// array (Eq. 7) and classifies the face; a second pass compacts the three face tables in
-// emission order (reading D-4) through a scan -- no atomics, deterministic output.
+// lt_connect.cu -- face connectivity (Alg. 5) for sm_100a, ONE kernel, one
+// pass over the leaves:
+//   - a tile of 256 consecutive leaves is claimed through a ticket; one thread per (leaf,
+//     local face) slot builds the same-level search key, finds it (sibling shortcut or
+//     bucketed lower bound, Eq. 7) and classifies the face into shared memory;
+//   - nbr / kind (the paper's face array F) leave in slot order, coalesced;
+//   - one thread per leaf counts its rows, a packed block scan orders them inside the tile,
+//     a decoupled look-back over the earlier tiles orders the tiles, and the three face
+//     tables are written in emission order (reading D-4) -- no atomics on the data, the
+//     output is deterministic.
 // Product code.
 #include "lt_internal.h"
 
 namespace lt {
 
-constexpr int CT = 256;
+constexpr int CT = 256;  // threads per block = leaves per tile
 
 // slot of a fine face inside the coarse face: the fine leaf's child-id bits on the
 // tangential axes, ascending axis order ("the first contributor along one
@@ -20,161 +26,223 @@ __device__ __forceinline__ int face_slot(int cid, int axis) {
   return cid & 3;
 }
 
+// Classify face f of leaf i.  Returns kind; *nb_out = neighbour index (or -1).
 template <int DIM>
-__global__ void __launch_bounds__(CT) k_connect_search(Geo g, const uint64_t* __restrict__ keys,
-                                                       const int* __restrict__ first, DevScalars* s,
-                                                       int32_t* __restrict__ nbr, uint8_t* __restrict__ kind,
-                                                       int* __restrict__ sums3) {
-  constexpr int NF = Dim<DIM>::NF;
-  __shared__ unsigned long long sm[33];
-  const int64_t nslots = (int64_t)s->n * NF;
-  int64_t lo, hi;
-  block_chunk(nslots, gridDim.x, blockIdx.x, CT, &lo, &hi);
-  unsigned long long acc = 0;  // three 21-bit fields would overflow per chunk: use 3 x 20 bits per tile, flush per tile
-  int c_conf = 0, c_hang = 0, c_bnd = 0;
-  for (int64_t sidx = lo + threadIdx.x; sidx < hi; sidx += CT) {
-    const int i = (int)(sidx / NF), f = (int)(sidx % NF);
-    const uint64_t key = keys[i];
-    const int l = key_level(key);
-    const uint64_t m = key_morton(key);
-    int kd = 0, nb = -1;
-    uint64_t mn;
-    if (face_neighbour<DIM>(g, m, l, f, &mn)) {
-      const int j = locate(g, keys, first, mn);
-      const int lj = key_level(keys[j]);
-      if (lj == l) {  // Eq. 7 case 1: the search key is in the tree -> conforming
-        kd = 1;
-        nb = j;
-      } else if (lj == l - 1) {  // Eq. 7 case 2: the entry to the left is the parent
-        kd = 2 | (face_slot<DIM>(child_id<DIM>(g, m, l), f >> 1) << 4);
-        nb = j;
-      } else if (lj < l - 1) {
-        set_status(&s->status, LT_ERR_UNBALANCED);  // reading D-5
-      } else {
-        // Eq. 7 case 3: the search key is subdivided.  Record the slot-0 fine neighbour:
-        // the child of the search key touching this face with tangential bits 0 (D-2).
-        int j2 = j;
-        if (!(f & 1)) {
-          const uint64_t mn2 = mn | (1ull << (DIM * (g.maxl - l - 1) + (f >> 1)));
-          j2 = locate(g, keys, first, mn2);
-        }
-        if (key_level(keys[j2]) != l + 1) set_status(&s->status, LT_ERR_UNBALANCED);
-        kd = 3;
-        nb = j2;
+__device__ __forceinline__ int connect_face(const Geo& g, const uint64_t* __restrict__ keys,
+                                            const int* __restrict__ first, int n, int i, int f, int* status,
+                                            int* nb_out) {
+  constexpr int NC = Dim<DIM>::NC;
+  const uint64_t key = keys[i];
+  const int l = key_level(key);
+  const uint64_t m = key_morton(key);
+  const int a = f >> 1;
+  *nb_out = -1;
+  if (l > 0) {
+    // A face interior to the parent looks at a sibling.  If that sibling is a leaf and every
+    // sibling between the two is a leaf too, it sits exactly (cid' - cid) entries away
+    // (PAPER.md:200): one key comparison decides, no search.
+    const int sh = DIM * (g.maxl - l);
+    const int cid = (int)((m >> sh) & (uint64_t)(NC - 1));
+    if (((cid >> a) & 1) != (f & 1)) {
+      const int j = i + ((cid ^ (1 << a)) - cid);
+      if (j >= 0 && j < n && keys[j] == make_key(m ^ (1ull << (sh + a)), l)) {
+        *nb_out = j;
+        return 1;
       }
     }
-    nbr[sidx] = nb;
-    kind[sidx] = (uint8_t)kd;
-    c_conf += (kd == 1) & (f & 1);
-    c_hang += ((kd & 15) == 2);
-    c_bnd += (kd == 0);
   }
-  (void)acc;
-  int t_conf = (int)block_sum<unsigned long long>(c_conf, sm);
-  int t_hang = (int)block_sum<unsigned long long>(c_hang, sm);
-  int t_bnd = (int)block_sum<unsigned long long>(c_bnd, sm);
-  if (threadIdx.x == 0) {
-    sums3[3 * blockIdx.x + 0] = t_conf;
-    sums3[3 * blockIdx.x + 1] = t_hang;
-    sums3[3 * blockIdx.x + 2] = t_bnd;
+  uint64_t mn;
+  if (!face_neighbour<DIM>(g, m, l, f, &mn)) return 0;  // domain boundary
+  const int j = locate(g, keys, first, mn);
+  const int lj = key_level(keys[j]);
+  if (lj == l) {  // Eq. 7 case 1: the search key is in the tree -> conforming
+    *nb_out = j;
+    return 1;
   }
+  if (lj == l - 1) {  // Eq. 7 case 2: the entry to the left is the parent -> hanging, fine side
+    *nb_out = j;
+    return 2 | (face_slot<DIM>(child_id<DIM>(g, m, l), a) << 4);
+  }
+  if (lj < l - 1) {
+    set_status(status, LT_ERR_UNBALANCED);  // reading D-5
+    return 0;
+  }
+  // Eq. 7 case 3: the search key is subdivided.  Record the slot-0 fine neighbour: the child
+  // of the search key touching this face with tangential bits 0 (reading D-2).
+  int j2 = j;
+  if (!(f & 1)) {
+    const uint64_t mn2 = mn | (1ull << (DIM * (g.maxl - l - 1) + a));
+    j2 = locate(g, keys, first, mn2);
+  }
+  if (key_level(keys[j2]) != l + 1) set_status(status, LT_ERR_UNBALANCED);
+  *nb_out = j2;
+  return 3;
 }
 
-// The three tables live back to back in one pool of nf*cap rows (every slot emits at most
-// one row): conf rows [0, n_conf), hang rows [n_conf, n_conf + n_hang), then bnd.  The
-// region offsets come from the chunk sums, so no host round trip separates the passes.
+// Tile status words of the decoupled look-back, two independent channels per tile:
+//   st[2t]   = flag << 62 | n_conf << 31 | n_hang        st[2t+1] = flag << 62 | n_bnd
+// flag 1 = the tile's own counts, 2 = inclusive prefix over tiles 0..t.  No field carries
+// into its neighbour because every partial sum is bounded by a final total < 2^31.
+constexpr unsigned long long kFlagAgg = 1ull << 62, kFlagInc = 2ull << 62, kValMask = (1ull << 62) - 1;
+
+// (one warp) exclusive prefix of channel ch over the tiles before `tile`, 32 predecessors per
+// step; publishes the tile's inclusive prefix.
+__device__ __forceinline__ unsigned long long lookback_warp(volatile unsigned long long* st, int tile, int ch,
+                                                            unsigned long long own, int lane) {
+  unsigned long long excl = 0;
+  for (int t = tile - 1; t >= 0; t -= 32) {
+    const int idx = t - lane;
+    unsigned long long v = kFlagInc;  // before tile 0: an inclusive prefix of zero
+    if (idx >= 0) {
+      do { v = st[2 * (size_t)idx + ch]; } while ((v >> 62) == 0);
+    }
+    const unsigned inc = __ballot_sync(0xffffffffu, (v >> 62) == 2);
+    const int stop = inc ? __ffs(inc) - 1 : 31;  // nearest predecessor that is already inclusive
+    unsigned long long c = lane <= stop ? (v & kValMask) : 0ull;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xffffffffu, c, d);
+    excl += c;
+    if (inc) break;
+  }
+  if (lane == 0) st[2 * (size_t)tile + ch] = kFlagInc | (excl + own);
+  return excl;
+}
+
 template <int DIM>
-__global__ void __launch_bounds__(CT) k_connect_tables(DevScalars* __restrict__ s,
-                                                       const int32_t* __restrict__ nbr,
-                                                       const uint8_t* __restrict__ kind,
-                                                       const int* __restrict__ sums3, int32_t* __restrict__ rows,
-                                                       uint8_t* __restrict__ bytes) {
+__global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restrict__ keys,
+                                                const int* __restrict__ first, DevScalars* s,
+                                                int32_t* __restrict__ nbr, uint8_t* __restrict__ kind,
+                                                int32_t* __restrict__ conf, uint8_t* __restrict__ conf_axis,
+                                                int32_t* __restrict__ hang, uint8_t* __restrict__ hang_info,
+                                                int32_t* __restrict__ bnd, uint8_t* __restrict__ bnd_face,
+                                                unsigned long long* st, unsigned* ticket) {
   constexpr int NF = Dim<DIM>::NF;
+  __shared__ int s_nb[CT * NF];
+  __shared__ uint8_t s_kd[CT * NF];
   __shared__ unsigned long long sm[33];
-  const int64_t nslots = (int64_t)s->n * NF;
-  // prefix of the three counters over the chunks before this one, and their totals
-  unsigned long long b0 = 0, b1 = 0, b2 = 0, a0 = 0, a1 = 0, a2 = 0;
-  for (int i = threadIdx.x; i < (int)gridDim.x; i += CT) {
-    const unsigned long long c0 = sums3[3 * i], c1 = sums3[3 * i + 1], c2 = sums3[3 * i + 2];
-    a0 += c0;
-    a1 += c1;
-    a2 += c2;
-    if (i < (int)blockIdx.x) {
-      b0 += c0;
-      b1 += c1;
-      b2 += c2;
+  __shared__ unsigned long long s_excl[2];
+  __shared__ int s_tile;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int n = s->n;
+  const int ntiles = (n + CT - 1) / CT;
+  for (;;) {
+    if (threadIdx.x == 0) s_tile = (int)atomicAdd(ticket, 1u);
+    __syncthreads();
+    const int tile = s_tile;
+    if (tile >= ntiles) break;
+    const int e0 = tile * CT;
+    const int ne = min(CT, n - e0);
+    // ---- search: one thread per slot, NF rounds; F leaves in slot order, coalesced
+#pragma unroll 1
+    for (int r = 0; r < NF; ++r) {
+      const int sl = r * CT + threadIdx.x;
+      const int le = sl / NF, f = sl - le * NF;
+      if (le < ne) {
+        int nb;
+        const int kd = connect_face<DIM>(g, keys, first, n, e0 + le, f, &s->status, &nb);
+        s_nb[sl] = nb;
+        s_kd[sl] = (uint8_t)kd;
+        const size_t gs = (size_t)e0 * NF + sl;
+        nbr[gs] = nb;
+        kind[gs] = (uint8_t)kd;
+      }
     }
-  }
-  int64_t r_conf = (int64_t)block_sum(b0, sm);
-  int64_t r_hang = (int64_t)block_sum(b1, sm);
-  int64_t r_bnd = (int64_t)block_sum(b2, sm);
-  const int64_t n_conf = (int64_t)block_sum(a0, sm), n_hang = (int64_t)block_sum(a1, sm);
-  const int64_t n_bnd = (int64_t)block_sum(a2, sm);
-  if (blockIdx.x == 0 && threadIdx.x == 0) {
-    s->n_face[0] = (int)n_conf;
-    s->n_face[1] = (int)n_hang;
-    s->n_face[2] = (int)n_bnd;
-  }
-  int32_t* __restrict__ conf = rows;
-  int32_t* __restrict__ hang = rows + 2 * n_conf;
-  int32_t* __restrict__ bnd = rows + 2 * (n_conf + n_hang);
-  uint8_t* __restrict__ conf_axis = bytes;
-  uint8_t* __restrict__ hang_info = bytes + n_conf;
-  uint8_t* __restrict__ bnd_face = bytes + n_conf + n_hang;
-  int64_t lo, hi;
-  block_chunk(nslots, gridDim.x, blockIdx.x, CT, &lo, &hi);
-  for (int64_t t0 = lo; t0 < hi; t0 += CT) {
-    const int64_t sidx = t0 + threadIdx.x;
-    int kd = 255, nb = 0, f = 0;
-    if (sidx < hi) {
-      kd = kind[sidx];
-      nb = nbr[sidx];
-      f = (int)(sidx % NF);
+    __syncthreads();
+    // ---- rows of this thread's leaf: conf | hang << 21 | bnd << 42
+    unsigned long long cnt = 0;
+    if ((int)threadIdx.x < ne) {
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        const int kd = s_kd[threadIdx.x * NF + f];
+        cnt += (unsigned long long)((kd == 1) & (f & 1)) | ((unsigned long long)((kd & 15) == 2) << 21) |
+               ((unsigned long long)(kd == 0) << 42);
+      }
     }
-    const bool is_conf = (kd == 1) && (f & 1), is_hang = (kd & 15) == 2 && kd != 255, is_bnd = kd == 0;
-    unsigned long long v = (unsigned long long)is_conf | ((unsigned long long)is_hang << 21) |
-                           ((unsigned long long)is_bnd << 42);
     unsigned long long tot;
-    unsigned long long ex = block_excl_scan<unsigned long long>(v, sm, &tot);
-    const int e = (int)(sidx / NF);
-    if (is_conf) {
-      int64_t p = r_conf + (int64_t)(ex & 0x1fffff);
-      conf[2 * p] = e;
-      conf[2 * p + 1] = nb;
-      conf_axis[p] = (uint8_t)(f >> 1);
-    } else if (is_hang) {
-      int64_t p = r_hang + (int64_t)((ex >> 21) & 0x1fffff);
-      hang[2 * p] = e;
-      hang[2 * p + 1] = nb;
-      hang_info[p] = (uint8_t)(f | ((kd >> 4) << 3));
-    } else if (is_bnd) {
-      int64_t p = r_bnd + (int64_t)((ex >> 42) & 0x1fffff);
-      bnd[p] = e;
-      bnd_face[p] = (uint8_t)f;
+    const unsigned long long ex = block_excl_scan<unsigned long long>(cnt, sm, &tot);
+    const unsigned long long t_conf = tot & 0x1fffff, t_hang = (tot >> 21) & 0x1fffff, t_bnd = (tot >> 42) & 0x1fffff;
+    // ---- order the tiles: publish the tile's own counts, then look back (warp 0: conf and
+    // hang, warp 1: bnd)
+    if (w < 2) {
+      const unsigned long long own = w == 0 ? ((t_conf << 31) | t_hang) : t_bnd;
+      volatile unsigned long long* vst = st;
+      if (lane == 0 && tile > 0) vst[2 * (size_t)tile + w] = kFlagAgg | own;
+      const unsigned long long excl = lookback_warp(vst, tile, w, own, lane);
+      if (lane == 0) s_excl[w] = excl;
     }
-    r_conf += (int64_t)(tot & 0x1fffff);
-    r_hang += (int64_t)((tot >> 21) & 0x1fffff);
-    r_bnd += (int64_t)((tot >> 42) & 0x1fffff);
+    __syncthreads();
+    const unsigned long long x0 = s_excl[0], x1 = s_excl[1];
+    int64_t p_conf = (int64_t)(x0 >> 31) + (int64_t)(ex & 0x1fffff);
+    int64_t p_hang = (int64_t)(x0 & 0x7fffffffull) + (int64_t)((ex >> 21) & 0x1fffff);
+    int64_t p_bnd = (int64_t)x1 + (int64_t)((ex >> 42) & 0x1fffff);
+    if (tile == ntiles - 1 && threadIdx.x == 0) {
+      s->n_face[0] = (int)((x0 >> 31) + t_conf);
+      s->n_face[1] = (int)((x0 & 0x7fffffffull) + t_hang);
+      s->n_face[2] = (int)(x1 + t_bnd);
+    }
+    // ---- emit (leaf order, local faces 0..NF-1: reading D-4)
+    if ((int)threadIdx.x < ne) {
+      const int e = e0 + threadIdx.x;
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        const int kd = s_kd[threadIdx.x * NF + f];
+        const int nb = s_nb[threadIdx.x * NF + f];
+        if (kd == 1) {
+          if (f & 1) {  // a conforming face is emitted by the element on its minus side
+            reinterpret_cast<int2*>(conf)[p_conf] = make_int2(e, nb);
+            conf_axis[p_conf] = (uint8_t)(f >> 1);
+            ++p_conf;
+          }
+        } else if ((kd & 15) == 2) {  // hanging: emitted by the fine element
+          reinterpret_cast<int2*>(hang)[p_hang] = make_int2(e, nb);
+          hang_info[p_hang] = (uint8_t)(f | ((kd >> 4) << 3));
+          ++p_hang;
+        } else if (kd == 0) {
+          bnd[p_bnd] = e;
+          bnd_face[p_bnd] = (uint8_t)f;
+          ++p_bnd;
+        }
+      }
+    }
+    __syncthreads();  // s_kd / s_nb / s_tile / s_excl are reused by the next tile
   }
 }
 
-int launch_connect_search(Tree* t, int G) {
-  if (t->g.dim == 2)
-    k_connect_search<2><<<G, CT, 0, t->stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->nbr, t->kind,
-                                                 t->d_sums3);
-  else
-    k_connect_search<3><<<G, CT, 0, t->stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->nbr, t->kind,
-                                                 t->d_sums3);
-  t->launches++;
-  LT_CUDA(cudaGetLastError());
-  return LT_OK;
+// The three tables have fixed regions in the pool.  Each face slot emits at most one row; only
+// a face exterior to the parent can see a coarser neighbour (an interior face looks at a
+// sibling's cell, tiled by leaves at least as fine) and only odd faces emit conforming rows:
+//   n_conf <= dim*M,  n_hang <= dim*M,  n_bnd <= nf*M.
+void face_regions(const Tree* t, int32_t** conf, uint8_t** conf_axis, int32_t** hang, uint8_t** hang_info,
+                  int32_t** bnd, uint8_t** bnd_face) {
+  const size_t dc = (size_t)t->g.dim * (size_t)t->cap;
+  *conf = t->face_rows;
+  *hang = t->face_rows + 2 * dc;
+  *bnd = t->face_rows + 4 * dc;
+  *conf_axis = t->face_bytes;
+  *hang_info = t->face_bytes + dc;
+  *bnd_face = t->face_bytes + 2 * dc;
 }
 
-int launch_connect_tables(Tree* t, int G) {
+int launch_connect(Tree* t) {
+  int32_t *conf, *hang, *bnd;
+  uint8_t *conf_axis, *hang_info, *bnd_face;
+  face_regions(t, &conf, &conf_axis, &hang, &hang_info, &bnd, &bnd_face);
+  const int64_t ntiles = (t->n + CT - 1) / CT;
+  LT_CUDA(cudaMemsetAsync(t->tile_state, 0, (size_t)(ntiles + 1) * 2 * sizeof(unsigned long long), t->stream));
+  LT_CUDA(cudaMemsetAsync(&t->d_s->ticket, 0, sizeof(unsigned), t->stream));
+  const void* fn = t->g.dim == 2 ? (const void*)k_connect<2> : (const void*)k_connect<3>;
+  int per_sm = 0;
+  LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, CT, 0));
+  if (per_sm < 1) per_sm = 1;
+  const int G = t->num_sms * per_sm;
   if (t->g.dim == 2)
-    k_connect_tables<2><<<G, CT, 0, t->stream>>>(t->d_s, t->nbr, t->kind, t->d_sums3, t->face_rows, t->face_bytes);
+    k_connect<2><<<G, CT, 0, t->stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->nbr, t->kind, conf,
+                                          conf_axis, hang, hang_info, bnd, bnd_face, t->tile_state,
+                                          &t->d_s->ticket);
   else
-    k_connect_tables<3><<<G, CT, 0, t->stream>>>(t->d_s, t->nbr, t->kind, t->d_sums3, t->face_rows, t->face_bytes);
+    k_connect<3><<<G, CT, 0, t->stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->nbr, t->kind, conf,
+                                          conf_axis, hang, hang_info, bnd, bnd_face, t->tile_state,
+                                          &t->d_s->ticket);
   t->launches++;
   LT_CUDA(cudaGetLastError());
   return LT_OK;

@@ -51,9 +51,12 @@ struct Tree {
   // connectivity
   int32_t* nbr;
   uint8_t* kind;
-  // face-table pool [cap*nf] rows: conf | hang | bnd back to back (lt_connect)
-  int32_t* face_rows;     // [cap*nf*2]
-  uint8_t* face_bytes;    // [cap*nf]
+  // face-table pool, fixed regions (face_regions() in lt_connect.cu):
+  //   rows  = conf [dim*cap][2] | hang [dim*cap][2] | bnd [nf*cap]      (int32)
+  //   bytes = conf_axis [dim*cap] | hang_info [dim*cap] | bnd_face [nf*cap]
+  int32_t* face_rows;
+  uint8_t* face_bytes;
+  unsigned long long* tile_state;  // [2*(cap/256 + 2)] look-back status of k_connect
 
   // Alg. 7 map
   int32_t* map_src;
@@ -101,8 +104,9 @@ int launch_decode(int dim, int maxl, const uint64_t* d_keys, int64_t n, int32_t*
 int launch_check_tiling(Tree* t);
 
 // ---- lt_connect.cu
-int launch_connect_search(Tree* t, int G);
-int launch_connect_tables(Tree* t, int G);
+int launch_connect(Tree* t);
+void face_regions(const Tree* t, int32_t** conf, uint8_t** conf_axis, int32_t** hang, uint8_t** hang_info,
+                  int32_t** bnd, uint8_t** bnd_face);
 
 // ---- lt_transfer.cu
 int launch_map(Tree* t);

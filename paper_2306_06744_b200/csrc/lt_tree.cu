@@ -296,14 +296,20 @@ struct BalanceArgs {
   int full_sweeps;
 };
 
+// Only the DIM faces of a leaf that are exterior to its parent are examined: an interior face
+// looks at a sibling's cell, which is tiled by leaves at least as fine as the leaf itself
+// (the parent is subdivided), so it can never meet a coarser neighbour.  The exterior face
+// on axis a is the minus face if bit a of the child id is 0, the plus face otherwise.
 template <int DIM>
 __device__ __forceinline__ void balance_examine(const Geo& g, const uint64_t* __restrict__ keys,
-                                                const int* __restrict__ first, uint8_t* mark, int i, int f) {
+                                                const int* __restrict__ first, uint8_t* mark, int i, int a) {
   const uint64_t key = keys[i];
   const int l = key_level(key);
   if (l < g.base + 2) return;  // no leaf is coarser than the base level
+  const uint64_t m = key_morton(key);
+  const int f = 2 * a + ((child_id<DIM>(g, m, l) >> a) & 1);
   uint64_t mn;
-  if (!face_neighbour<DIM>(g, key_morton(key), l, f, &mn)) return;
+  if (!face_neighbour<DIM>(g, m, l, f, &mn)) return;
   const int j = locate(g, keys, first, mn);
   const int lj = key_level(keys[j]);
   if (lj < l - 1) {
@@ -314,7 +320,7 @@ __device__ __forceinline__ void balance_examine(const Geo& g, const uint64_t* __
 
 template <int DIM>
 __global__ void __launch_bounds__(BT) k_balance(BalanceArgs a) {
-  constexpr int NC = Dim<DIM>::NC, NF = Dim<DIM>::NF;
+  constexpr int NC = Dim<DIM>::NC;
   __shared__ unsigned long long sm[33];
   cg::grid_group grid = cg::this_grid();
   const Geo g = a.g;
@@ -331,12 +337,12 @@ __global__ void __launch_bounds__(BT) k_balance(BalanceArgs a) {
     const int* first = a.first[par];
     // ---- sweep
     if (nfront < 0) {
-      for (int64_t sidx = gtid; sidx < n * NF; sidx += gsize)
-        balance_examine<DIM>(g, keys, first, a.mark, (int)(sidx / NF), (int)(sidx % NF));
+      for (int64_t sidx = gtid; sidx < n * DIM; sidx += gsize)
+        balance_examine<DIM>(g, keys, first, a.mark, (int)(sidx / DIM), (int)(sidx % DIM));
     } else {
       const int* fr = a.frontier[fpar];
-      for (int64_t sidx = gtid; sidx < nfront * NF; sidx += gsize)
-        balance_examine<DIM>(g, keys, first, a.mark, fr[sidx / NF], (int)(sidx % NF));
+      for (int64_t sidx = gtid; sidx < nfront * DIM; sidx += gsize)
+        balance_examine<DIM>(g, keys, first, a.mark, fr[sidx / DIM], (int)(sidx % DIM));
     }
     grid.sync();
     // ---- count: low 32 = leaves out, high 32 = frontier entries out

@@ -245,7 +245,7 @@ class Tree:
         out = (C.c_float * 8)()
         _check(lib().lt_timings(self._h, out), "lt_timings")
         return dict(adapt=out[0], balance=out[1], connect=out[2], transfer=out[3], k_map=out[4], k_transfer=out[5],
-                    k_connect_search=out[6], k_connect_tables=out[7])
+                    k_connect=out[6])
 
     def launch_count(self) -> int:
         return int(lib().lt_launch_count(self._h))
