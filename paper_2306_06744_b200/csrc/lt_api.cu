@@ -141,8 +141,10 @@ static int new_tree(int dim, int base, int maxl, const double* domain, const int
   g.dim = dim;
   g.base = base;
   g.maxl = maxl;
-  g.ilevel = base;
-  while (dim * g.ilevel > 24) --g.ilevel;  // bucket index of at most 2^24 cells
+  // bucket index one level below the base tree (buckets of at most 2^(dim*(maxl-base-1)) keys),
+  // of at most 2^24 cells
+  g.ilevel = base + 1 <= maxl ? base + 1 : maxl;
+  while (dim * g.ilevel > 24) --g.ilevel;
   g.ishift = dim * (maxl - g.ilevel);
   g.nbuckets = 1 << (dim * g.ilevel);
   g.periodic = 0;

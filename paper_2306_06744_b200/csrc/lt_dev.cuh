@@ -16,7 +16,7 @@ constexpr uint64_t kLevelMask = 31;
 // Static description of a tree, passed by value to every kernel.
 struct Geo {
   int dim, base, maxl;
-  int ilevel;       // level of the bucket index (<= base), see locate()
+  int ilevel;       // level of the bucket index (<= base + 1), see locate()
   int ishift;       // dim * (maxl - ilevel): morton >> ishift = bucket
   int nbuckets;     // 2^(dim*ilevel)
   int periodic;     // bit a set = axis a periodic
@@ -137,9 +137,10 @@ __device__ __forceinline__ bool face_neighbour(const Geo& g, uint64_t m, int l, 
 
 // Point location (the lower-bound search of PAPER.md:134-143, Eq. 7, in one form):
 // index of the leaf whose cell contains the finest-level point with morton code `mn`,
-// i.e. the last j with morton(keys[j]) <= mn.  `first` is the bucket index: first[b] =
-// index of the first leaf inside cell b of the uniform level-`ilevel` grid (every leaf
-// has level >= ilevel, so every bucket starts with a leaf whose anchor is the bucket's).
+// i.e. the last j with morton(keys[j]) <= mn.  `first` is the bucket index over the uniform
+// level-`ilevel` grid: first[b] = index of the first leaf inside cell b, or, where a leaf is
+// coarser than the grid, the index of that leaf in every cell it covers (the search range of
+// such a cell is empty or holds only larger keys, and the leaf itself is returned).
 __device__ __forceinline__ int locate(const Geo& g, const uint64_t* __restrict__ keys,
                                       const int* __restrict__ first, uint64_t mn) {
   const uint32_t b = (uint32_t)(mn >> g.ishift);
@@ -150,6 +151,18 @@ __device__ __forceinline__ int locate(const Geo& g, const uint64_t* __restrict__
     if (keys[mid] <= bound) lo = mid; else hi = mid;
   }
   return lo;
+}
+
+// Record the leaf (m, l) stored at position `pos` in the bucket index (see locate()).
+template <int DIM>
+__device__ __forceinline__ void index_write(const Geo& g, int* __restrict__ first, uint64_t m, int l, int pos) {
+  if (l >= g.ilevel) {
+    if ((m & ((1ull << g.ishift) - 1)) == 0) first[m >> g.ishift] = pos;
+  } else {
+    const int span = 1 << (DIM * (g.ilevel - l));
+    const uint32_t b = (uint32_t)(m >> g.ishift);
+    for (int c = 0; c < span; ++c) first[b + c] = pos;
+  }
 }
 
 // ---- block-wide exclusive scan (blockDim.x multiple of 32, <= 1024) ------------------

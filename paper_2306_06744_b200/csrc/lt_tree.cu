@@ -70,10 +70,9 @@ template <int DIM>
 __global__ void k_build_uniform(Geo g, uint64_t* __restrict__ keys, int* __restrict__ first, DevScalars* s) {
   const int64_t nb = 1ll << (DIM * g.base);
   const int pad = DIM * (g.maxl - g.base);
-  const int sub = DIM * (g.base - g.ilevel);
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < nb; i += (int64_t)gridDim.x * blockDim.x) {
     keys[i] = make_key((uint64_t)i << pad, g.base);
-    if ((i & ((1ll << sub) - 1)) == 0) first[i >> sub] = (int)i;
+    index_write<DIM>(g, first, (uint64_t)i << pad, g.base, (int)i);
     if (i == 0) {
       first[g.nbuckets] = (int)nb;
       s->n = (int)nb;
@@ -85,10 +84,9 @@ template <int DIM>
 __global__ void k_build_index(Geo g, const uint64_t* __restrict__ keys, const DevScalars* __restrict__ s,
                               int* __restrict__ first) {
   const int64_t n = s->n;
-  const uint64_t bmask = (1ull << g.ishift) - 1;
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-    uint64_t m = key_morton(keys[i]);
-    if ((m & bmask) == 0) first[m >> g.ishift] = (int)i;
+    const uint64_t k = keys[i];
+    index_write<DIM>(g, first, key_morton(k), key_level(k), (int)i);
     if (i == 0) first[g.nbuckets] = (int)n;
   }
 }
@@ -192,7 +190,6 @@ __global__ void __launch_bounds__(BT) k_adapt_scatter(Geo g, const uint64_t* __r
   int64_t lo, hi;
   block_chunk(n, gridDim.x, blockIdx.x, BT, &lo, &hi);
   int64_t run = (int64_t)(before & 0xffffffffull);
-  const uint64_t bmask = (1ull << g.ishift) - 1;
   for (int64_t t0 = lo; t0 < hi; t0 += BT) {
     const int64_t i = t0 + threadIdx.x;
     int act = ACT_DROP;
@@ -209,15 +206,20 @@ __global__ void __launch_bounds__(BT) k_adapt_scatter(Geo g, const uint64_t* __r
     if (c == 0) continue;
     const int l = key_level(key);
     const uint64_t m = key_morton(key);
-    if ((m & bmask) == 0) first_out[m >> g.ishift] = (int)pos;
     if (act == ACT_KEEP) {
       out[pos] = key;
+      index_write<DIM>(g, first_out, m, l, (int)pos);
     } else if (act == ACT_PARENT) {
       out[pos] = make_key(m, l - 1);  // child 0 has the parent's anchor
+      index_write<DIM>(g, first_out, m, l - 1, (int)pos);
     } else {
       const int sh = DIM * (g.maxl - l - 1);
 #pragma unroll
-      for (int k = 0; k < NC; ++k) out[pos + k] = make_key(m | ((uint64_t)k << sh), l + 1);  // reading A-6
+      for (int k = 0; k < NC; ++k) {
+        const uint64_t mc = m | ((uint64_t)k << sh);  // reading A-6
+        out[pos + k] = make_key(mc, l + 1);
+        index_write<DIM>(g, first_out, mc, l + 1, (int)(pos + k));
+      }
     }
   }
   if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -326,7 +328,6 @@ __global__ void __launch_bounds__(BT) k_balance(BalanceArgs a) {
   const Geo g = a.g;
   const int64_t gtid = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   const int64_t gsize = (int64_t)gridDim.x * blockDim.x;
-  const uint64_t bmask = (1ull << g.ishift) - 1;
   int64_t n = a.s->n;
   int par = 0, iters = 0, fpar = 0;
   int64_t nfront = -1;  // -1: full sweep
@@ -391,16 +392,18 @@ __global__ void __launch_bounds__(BT) k_balance(BalanceArgs a) {
       if (i >= hi) continue;
       const int l = key_level(key);
       const uint64_t m = key_morton(key);
-      if ((m & bmask) == 0) first_out[m >> g.ishift] = (int)pos;
       if (mk & 1) {
         const int sh = DIM * (g.maxl - l - 1);
 #pragma unroll
         for (int k = 0; k < NC; ++k) {
-          out[pos + k] = make_key(m | ((uint64_t)k << sh), l + 1);
+          const uint64_t mc = m | ((uint64_t)k << sh);
+          out[pos + k] = make_key(mc, l + 1);
+          index_write<DIM>(g, first_out, mc, l + 1, (int)(pos + k));
           fr_out[fpos + k] = (int)(pos + k);
         }
       } else {
         out[pos] = key;
+        index_write<DIM>(g, first_out, m, l, (int)pos);
         if (mk & 2) fr_out[fpos] = (int)pos;
       }
     }

@@ -1,0 +1,103 @@
+"""Parity at BASELINE.json's full size, in the launch configuration bench.py times: config 5
+(3-D octree, periodic, base 64^3, max level +3, p = 3, 5 fp64 variables) driven through cycles
+0..3 on both sides -- cycle 3 (8,863,051 -> 13,473,692 leaves) is the first step bench.py times.
+
+Trees, balance iteration counts, the face tables and the Alg. 7 map are compared IN FULL, bit
+for bit, against the CPU oracle (which builds its own pointer tree of 13.5 M leaves: about two
+minutes of host time); the transferred solution is compared on sampled slabs of new elements
+that the oracle computes one by one (dense M^-1 S_c, Eq. 12), within the 1e-12 bound of
+DESIGN.md reading E-8.  No oracle input comes from the CUDA path: flags and the initial
+solution come from the shared seeded generators (workloads.py), evaluated on the oracle's own
+leaf boxes / copied from the generator's output.
+"""
+import numpy as np
+import pytest
+import torch
+
+import parity as P
+from paper_2306_06744_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+CYCLES = 4           # cycles 0..3
+SLAB = 96            # new elements per sampled slab
+N_SLABS = 40
+
+
+def _analytic_u(cfg, gt, out):
+    lvl, xyz = gt.leaf_boxes()
+    M = lvl.shape[0]
+    step = 1 << 20
+    for a in range(0, M, step):
+        b = min(a + step, M)
+        out[a:b] = W.initial_solution(cfg, lvl[a:b], xyz[a:b])
+
+
+def test_config5_full_size_cycle3():
+    cfg = W.CONFIGS["c5"]
+    p, nvars = cfg["p"], cfg["nvars"]
+    N = (p + 1) ** cfg["dim"]
+    free, _ = torch.cuda.mem_get_info()
+    if free < 70 * 2 ** 30:
+        pytest.skip("needs ~60 GB of device memory")
+    gt, ot = P.new_pair(cfg)
+    ug = None
+    for c in range(CYCLES):
+        tag = "c5 full size, cycle %d" % c
+        f = P.host_flags(cfg, c, ot)
+        if c == CYCLES - 1:
+            # the old solution: analytic vortex on the old tree (the GPU's decoder was checked
+            # against the oracle's boxes in the keys comparison of the previous cycle)
+            M0 = gt.num_leaves()
+            ug = torch.empty((M0, nvars, N), dtype=torch.float64, device="cuda")
+            _analytic_u(cfg, gt, ug)
+        ot.adapt(f)
+        gt.adapt(torch.from_numpy(f).cuda())
+        it_o = ot.balance()
+        it_g = gt.balance()
+        assert it_g == it_o, "%s: balance iters %d vs oracle %d" % (tag, it_g, it_o)
+        P.assert_keys_equal(gt, ot, tag)
+        if c < CYCLES - 1:
+            ot.drop_snapshot()
+    M1 = ot.num_leaves()
+    assert (M0, M1) == (8863051, 13473692)  # the step bench.py times first
+    # ---- connectivity, in full
+    Fg, Fo = gt.connect(), ot.connect()
+    P.assert_faces_equal(Fg, Fo, "c5 full size connect")
+    nf = 6
+    assert nf * M1 == 2 * Fo["n_conf"] + Fo["n_hang"] + Fo["n_hang"] // 4 + Fo["n_bnd"]
+    del Fg, Fo
+    # ---- map, in full; transfer on sampled slabs
+    src_o, kind_o = ot.build_map()
+    un_g = gt.transfer(ug, p, nvars)
+    gt.sync()
+    src_g, kind_g = gt.map()
+    assert np.array_equal(src_g.cpu().numpy(), src_o), "map src"
+    assert np.array_equal(kind_g.cpu().numpy(), kind_o), "map kind"
+    rng = np.random.default_rng(5)
+    starts = [0, M1 - SLAB] + [int(v) for v in rng.integers(0, M1 - SLAB, N_SLABS - 2)]
+    # make sure every kind is sampled: add slabs that start at a refined / a coarsened element
+    for k in (1, 2):
+        idx = np.flatnonzero((kind_o & 15) == k)
+        assert idx.size > 0
+        starts += [int(min(idx[idx.size // 3], M1 - SLAB)), int(min(idx[2 * idx.size // 3], M1 - SLAB))]
+    # a host array of the full u_old shape whose pages are only touched where a slab needs them
+    uo = np.empty((M0, nvars, N), dtype=np.float64)
+    seen = np.zeros(3, np.int64)
+    worst = 0.0
+    for j0 in starts:
+        j1 = j0 + SLAB
+        lo = int(src_o[j0:j1].min())
+        hi = min(M0, int(src_o[j0:j1].max()) + 8)
+        uo[lo:hi] = ug[lo:hi].cpu().numpy()
+        ref = ot.transfer_rows(uo, p, nvars, j0, j1)
+        got = un_g[j0:j1].cpu().numpy()
+        for v in range(nvars):
+            tol = 1e-12 * max(1.0, np.abs(ref[:, v]).max())
+            err = np.abs(got[:, v] - ref[:, v]).max()
+            worst = max(worst, err)
+            assert err <= tol, "slab %d var %d: |diff| %.3e > %.3e" % (j0, v, err, tol)
+        for k in range(3):
+            seen[k] += int(((kind_o[j0:j1] & 15) == k).sum())
+    assert (seen > 0).all(), "sampled slabs must cover copy, refine and coarsen: %s" % seen
+    print("c5 full size: sampled %d elements (copy/refine/coarsen %s), worst |diff| %.2e" % (seen.sum(), seen, worst))
