@@ -334,14 +334,18 @@ def run_ours(args):
     tr_bytes = sum(b["transfer"] for b in by)
     tr_ms = sum(s["tm"]["k_transfer"] for s in steps)
     achieved = tr_bytes / (tr_ms * 1e-3) / 1e9
-    traffic = None
-    try:
-        tj = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
-        traffic = tj.get("k_transfer", {}).get("dram_bytes_per_launch")
+    traffic = traffic_note = None
+    try:  # profiles/traffic.txt: "<kernel> <dram bytes per launch> <algorithmic bytes of that launch>"
+        for line in open(os.path.join(ROOT, "profiles", "traffic.txt")):
+            w = line.split()
+            if len(w) >= 3 and w[0] == "k_transfer":
+                traffic = int(w[1])
+                traffic_note = ("ncu --set full of the config-5 cycle-3 launch (profiles/r1b_step_full.md); "
+                                "algorithmic bytes of that launch: %d" % int(w[2]))
     except Exception:
         pass
     roofline = {"bound": "hbm", "kernel": "k_transfer<3,4>", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": traffic, "traffic_note": traffic_note, "peak_source": peak_src,
                 "bytes_per_launch": tr_bytes / K, "ms_per_launch": tr_ms / K,
                 "share_of_step": tr_ms / sum(s["ms"] for s in steps)}
     cyc_bytes = sum(sum(b.values()) for b in by)
