@@ -51,6 +51,14 @@ def lib():
         L.lto_build_from_keys.restype = C.c_void_p
         L.lto_build_from_keys.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int),
                                           C.POINTER(C.c_uint64), C.c_int64]
+        L.lto_build_complete.restype = C.c_void_p
+        L.lto_build_complete.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int),
+                                         C.POINTER(C.c_uint64), C.c_int64]
+        L.lto_build_from_points.restype = C.c_void_p
+        L.lto_build_from_points.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int),
+                                            C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_int64]
+        L.lto_point_cell.restype = C.c_uint32
+        L.lto_point_cell.argtypes = [C.c_double, C.c_double, C.c_double, C.c_int]
         L.lto_free.restype = None
         L.lto_free.argtypes = [C.c_void_p]
         L.lto_num_leaves.restype = C.c_int64
@@ -115,6 +123,11 @@ def decode(dim, maxl, key):
     return lvl.value, tuple(int(v) for v in xx[:dim])
 
 
+def point_cell(x, lo, hi, maxl):
+    """Reading G-1: depth-D_max integer cell of a scattered coordinate."""
+    return int(lib().lto_point_cell(float(x), float(lo), float(hi), int(maxl)))
+
+
 def sort_linearise(dim, maxl, keys):
     k = np.ascontiguousarray(keys, dtype=np.uint64).copy()
     m = lib().lto_sort_linearise(dim, maxl, _p(k, C.c_uint64), k.size)
@@ -148,13 +161,27 @@ class OracleError(RuntimeError):
 class Tree:
     """Pointer-based linear-tree oracle.  Same verbs as the product's C ABI."""
 
-    def __init__(self, dim, base_level, max_level, periodic=None, keys=None):
+    def __init__(self, dim, base_level, max_level, periodic=None, keys=None, complete=False, points=None,
+                 domain=None):
+        """keys: unsorted IDs that must tile the domain (sort + linearise, Alg. 3);
+        keys + complete=True: Alg. 2 completion of the octants over the uniform base tree;
+        points [n][dim] fp64 + domain (lo.., hi..): Alg. 2 from scattered points."""
         self.dim, self.base, self.maxl = dim, base_level, max_level
         self.nc, self.nf = 1 << dim, 2 * dim
         per = np.zeros(3, np.int32)
         if periodic is not None:
             per[:dim] = np.asarray(periodic, np.int32)[:dim]
-        if keys is None:
+        if points is not None:
+            pts = np.ascontiguousarray(points, dtype=np.float64).reshape(-1, dim)
+            dom = np.ascontiguousarray(domain, dtype=np.float64)
+            assert dom.size == 2 * dim
+            self._h = lib().lto_build_from_points(dim, base_level, max_level, _p(per, C.c_int),
+                                                  _p(dom, C.c_double), _p(pts, C.c_double), pts.shape[0])
+        elif keys is not None and complete:
+            k = np.ascontiguousarray(keys, dtype=np.uint64)
+            self._h = lib().lto_build_complete(dim, base_level, max_level, _p(per, C.c_int),
+                                               _p(k, C.c_uint64), k.size)
+        elif keys is None:
             self._h = lib().lto_build(dim, base_level, max_level, _p(per, C.c_int))
         else:
             k = np.ascontiguousarray(keys, dtype=np.uint64)

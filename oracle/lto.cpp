@@ -746,6 +746,42 @@ void refine_uniform(Tree* t, Node* n, int to_level) {
   for (int c = 0; c < t->nc; ++c) refine_uniform(t, n->child[c], to_level);
 }
 
+
+// ---------------------------------------------------------------- Alg. 2
+// Tree construction from scattered points and completion, PAPER.md:105-120 (section 3.1,
+// Alg. 2).  The paper completes the sorted initial octants by splitting the largest common
+// ancestor of consecutive octants and keeping the children that lie between them; the
+// result it reaches is the plainly defined one computed here (readings G-2, G-3 of
+// DESIGN.md): the COARSEST complete tree that refines the uniform depth-D_min tree
+// (D_min = base_level) and has every input octant as a leaf -- or as
+// an interior node when a finer input octant lies inside it (linearisation keeps the
+// finer one, Alg. 3).  On a pointer tree that is: walk from the root to
+// the octant and split every leaf met on the way.  Order of insertion does not matter.
+void insert_octant(Tree* t, int lvl, const uint32_t* x) {
+  Node* nd = t->root;
+  while (nd->level < lvl) {
+    if (nd->is_leaf()) split(t, nd);
+    int sh = t->maxl - nd->level - 1;
+    int c = 0;
+    for (int a = 0; a < t->dim; ++a) c |= (int)((x[a] >> sh) & 1u) << a;
+    nd = nd->child[c];
+  }
+}
+
+// Alg. 1 steps 1-2 / Alg. 2 step 1 for a scattered point: integer
+// coordinate of the depth-D_max cell that contains it (half-open cells).
+// Reading G-1: xi = floor((x - lo) / (hi - lo) * 2^D_max) evaluated in fp64 in exactly
+// this order, clamped to [0, 2^D_max - 1] (points on or beyond the upper boundary fall
+// into the last cell).
+uint32_t point_cell(double x, double lo, double hi, int maxl) {
+  double s = (x - lo) / (hi - lo);
+  double v = std::floor(s * (double)((uint64_t)1 << maxl));
+  double top = (double)(((uint64_t)1 << maxl) - 1);
+  if (!(v >= 0.0)) v = 0.0;  // also catches NaN
+  if (v > top) v = top;
+  return (uint32_t)v;
+}
+
 }  // namespace
 
 // ======================================================================= C ABI
@@ -810,6 +846,45 @@ void* lto_build_from_keys(int dim, int base, int maxl, const int* periodic, cons
   relist(t);
   return t;
 }
+
+// Alg. 2 on octants: complete the key set (any order, duplicates / ancestors allowed)
+// over the uniform depth-`base` tree.  NULL on bad arguments or a key above base level.
+void* lto_build_complete(int dim, int base, int maxl, const int* periodic, const uint64_t* keys, int64_t n) {
+  Tree* t = new_tree(dim, base, maxl, periodic);
+  if (!t) return nullptr;
+  refine_uniform(t, t->root, base);
+  for (int64_t i = 0; i < n; ++i) {
+    int lvl;
+    uint32_t x[3];
+    decode(dim, maxl, keys[i], &lvl, x);
+    if (lvl < base || lvl > maxl) {
+      free_subtree(t->root);
+      delete t;
+      return nullptr;
+    }
+    insert_octant(t, lvl, x);
+  }
+  relist(t);
+  return t;
+}
+
+// Alg. 2 from scattered points: xyz [n][dim] fp64, domain lo_hi = lo_x.., hi_x..; every
+// point becomes its depth-D_max cell (point_cell), then completion as above.
+void* lto_build_from_points(int dim, int base, int maxl, const int* periodic, const double* lo_hi,
+                            const double* xyz, int64_t n) {
+  Tree* t = new_tree(dim, base, maxl, periodic);
+  if (!t) return nullptr;
+  refine_uniform(t, t->root, base);
+  for (int64_t i = 0; i < n; ++i) {
+    uint32_t x[3] = {0, 0, 0};
+    for (int a = 0; a < dim; ++a) x[a] = point_cell(xyz[i * dim + a], lo_hi[a], lo_hi[dim + a], maxl);
+    insert_octant(t, maxl, x);
+  }
+  relist(t);
+  return t;
+}
+
+uint32_t lto_point_cell(double x, double lo, double hi, int maxl) { return point_cell(x, lo, hi, maxl); }
 
 void lto_free(void* h) {
   Tree* t = (Tree*)h;

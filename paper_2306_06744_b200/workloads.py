@@ -201,3 +201,46 @@ def initial_solution(name_or_cfg, level: torch.Tensor, xyz: torch.Tensor) -> tor
     comps.append(E)
     out = torch.stack(comps[:nvars], dim=1)
     return out.contiguous()
+
+
+# ---------------------------------------------------------------------------------------
+# Scattered points for tree construction (Alg. 2).  The paper builds its
+# construction / balance benchmark from the Stanford bunny surface, which is
+# not available here; these seeded synthetic surfaces stand in for it.
+POINT_CLOUDS = {
+    # name: dim, base (the paper's D_min = 4), maxl, surface, points
+    "pc_tiny": dict(dim=2, base=1, maxl=5, lo=0.0, hi=1.0, periodic=(0, 0), surface="sphere", n=40, seed=3),
+    "pc2": dict(dim=2, base=2, maxl=9, lo=0.0, hi=1.0, periodic=(0, 0), surface="sphere", n=4000, seed=4),
+    "pc3_small": dict(dim=3, base=2, maxl=6, lo=0.0, hi=1.0, periodic=(0, 0, 0), surface="torus", n=3000, seed=5),
+    "pc9": dict(dim=3, base=4, maxl=9, lo=-1.0, hi=1.0, periodic=(0, 0, 0), surface="torus", n=4_000_000, seed=6),
+    "pc10": dict(dim=3, base=4, maxl=10, lo=-1.0, hi=1.0, periodic=(0, 0, 0), surface="sphere", n=16_000_000,
+                 seed=7),
+}
+
+
+def surface_points(cfg, device="cpu", n=None) -> torch.Tensor:
+    """float64 [n, dim] points on a closed surface inside the domain: "sphere" (circle in 2-D)
+    of radius 0.35 widths about the centre, or "torus" (major 0.30, minor 0.12 widths, axis z;
+    2-D: an annulus boundary pair).  Drawn from the counter generator, so the cloud depends only
+    on (seed, index).  Trigonometric results may differ in the last bit between devices: generate
+    ONCE and hand the same bytes to both sides."""
+    dim, lo, hi = cfg["dim"], cfg["lo"], cfg["hi"]
+    n = int(cfg["n"] if n is None else n)
+    i = torch.arange(n, dtype=torch.int64, device=device)
+    u = counter_uniform(cfg["seed"], 11, i)
+    v = counter_uniform(cfg["seed"], 12, i)
+    w = hi - lo
+    c = 0.5 * (lo + hi)
+    two_pi = 2.0 * math.pi
+    if dim == 2:
+        r = 0.35 * w if cfg["surface"] == "sphere" else torch.where(v < 0.5, 0.18 * w, 0.42 * w)
+        return torch.stack([c + r * torch.cos(two_pi * u), c + r * torch.sin(two_pi * u)], dim=1)
+    if cfg["surface"] == "sphere":
+        z = 2.0 * v - 1.0
+        s = torch.sqrt(torch.clamp(1.0 - z * z, min=0.0))
+        r = 0.35 * w
+        return torch.stack([c + r * s * torch.cos(two_pi * u), c + r * s * torch.sin(two_pi * u), c + r * z], dim=1)
+    R, r = 0.30 * w, 0.12 * w
+    q = R + r * torch.cos(two_pi * v)
+    return torch.stack([c + q * torch.cos(two_pi * u), c + q * torch.sin(two_pi * u),
+                        c + r * torch.sin(two_pi * v)], dim=1)

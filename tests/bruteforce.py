@@ -137,3 +137,28 @@ def volume(mesh, maxl):
 def to_cells(level, xyz, dim, maxl):
     """oracle/GPU leaf boxes (anchor in finest units) -> list of set-model cells, array order."""
     return [(int(l),) + tuple(int(x) >> (maxl - int(l)) for x in X[:dim]) for l, X in zip(level, xyz)]
+
+
+def complete(cells, dim, base):
+    """Alg. 2's result by set algebra (readings G-2, G-3): the
+    coarsest complete mesh that refines the uniform level-`base` mesh and in which every input
+    cell is a leaf or an interior node.  interior = every strict ancestor of an input cell
+    plus every cell above `base`; leaves = children of interior cells that are not interior."""
+    interior = set()
+    for l in range(base):
+        interior |= uniform(dim, l)
+    for cell in cells:
+        c = cell
+        while c[0] > 0:
+            c = parent(c)
+            if c in interior:
+                break
+            interior.add(c)
+    if not interior:
+        return {(0,) + (0,) * dim}
+    leaves = set()
+    for c in interior:
+        for ch in children(c):
+            if ch not in interior:
+                leaves.add(ch)
+    return leaves
