@@ -103,6 +103,29 @@ int lt_build_from_keys(int dim, int base_level, int max_level, const double* dom
                        const int* periodic, void* cuda_stream, const uint64_t* d_keys, int64_t n,
                        lt_tree** out);
 
+/* Alg. 2 on octants: n unsorted device keys (levels in [base_level,
+ * max_level]; duplicates and ancestors allowed) -> radix sort, linearise (Alg. 3), then
+ * COMPLETION: the result is the coarsest complete tree that refines the uniform depth-
+ * base_level tree (base_level = the paper's D_min) and keeps every
+ * linearised input octant as a leaf (readings G-2, G-3).  The gaps between
+ * consecutive octants, and before the first / after the last one, are filled in Morton
+ * order by a closed form of the two neighbouring keys: no atomics, no append, no second
+ * sort.  The tree is NOT 2:1 balanced: call lt_balance (Alg. 4) next.
+ * LT_ERR_ARG if a key is outside [base_level, max_level] or misaligned; LT_ERR_CAPACITY if
+ * the completed tree would exceed 2^31 - 1024 leaves.  Synchronises. */
+int lt_build_complete_from_keys(int dim, int base_level, int max_level, const double* domain,
+                                const int* periodic, void* cuda_stream, const uint64_t* d_keys,
+                                int64_t n, lt_tree** out);
+
+/* Alg. 2 from scattered points (PAPER.md:109 step 1): d_xyz device fp64 [n][dim].  Every point
+ * becomes its depth-max_level cell, xi = floor((x - lo) / (hi - lo) * 2^max_level) evaluated
+ * in fp64 in this order and clamped to [0, 2^max_level - 1] (reading G-1; cells are half-
+ * open), then as lt_build_complete_from_keys.  domain (host [2*dim]) is
+ * required, hi > lo on every axis.  Synchronises. */
+int lt_build_from_points(int dim, int base_level, int max_level, const double* domain,
+                         const int* periodic, void* cuda_stream, const double* d_xyz, int64_t n,
+                         lt_tree** out);
+
 void lt_free(lt_tree*);
 
 /* Make room for `n_leaves` leaves in every tree-owned buffer (buffers also grow on

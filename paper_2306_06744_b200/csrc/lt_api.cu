@@ -180,6 +180,42 @@ static int new_tree(int dim, int base, int maxl, const double* domain, const int
   return LT_OK;
 }
 
+// Alg. 2 behind lt_build_complete_from_keys / lt_build_from_points: `work` holds n unsorted
+// keys (device, owned by the caller).  Radix sort, linearise (Alg. 3), then the completed
+// tree is written in Morton order straight into the tree's key buffer (lt_construct.cu).
+static int complete_from_unsorted(Tree* t, uint64_t* work, int64_t n) {
+  const int dim = t->g.dim, maxl = t->g.maxl;
+  SortScratch sc = {nullptr, 0, nullptr, nullptr, 0, nullptr};
+  int rc = sort_keys(work, n, dim * maxl + kLevelBits, &sc, t->stream, &t->launches);
+  t->sort_tmp = sc.tmp; t->sort_cap = sc.cap; t->sort_hist = sc.hist; t->sort_status = sc.status;
+  t->sort_status_cap = sc.status_cap;
+  if (rc != LT_OK) return rc;
+  uint64_t* lin = nullptr;
+  uint32_t* offs = nullptr;
+  if ((rc = alloc_dev(&lin, n)) != LT_OK) return rc;
+  auto done = [&](int code) {
+    cudaStreamSynchronize(t->stream);
+    free_dev(lin);
+    free_dev(offs);
+    return code;
+  };
+  int64_t m = 0, total = 0;
+  rc = linearise_keys(dim, maxl, work, lin, n, &m, t->d_sums, &t->d_s->aux, (int*)t->h_sums, grid_for(t, 4),
+                      t->stream, &t->launches);
+  if (rc != LT_OK) return done(rc);
+  if ((rc = alloc_dev(&offs, m + 2)) != LT_OK) return done(rc);
+  if ((rc = launch_complete_count(t, lin, m, offs, &total)) != LT_OK) return done(rc);
+  const int st = take_status(t);
+  if (st != LT_OK) return done(st);
+  if (total >= (1ll << 31) - 1024) return done(LT_ERR_CAPACITY);
+  if ((rc = grow(t, total)) != LT_OK) return done(rc);
+  if ((rc = launch_complete_fill(t, lin, m, offs, total)) != LT_OK) return done(rc);
+  t->n = total;
+  t->n_valid = true;
+  if ((rc = launch_build_index(t, t->cur)) != LT_OK) return done(rc);
+  return done(LT_OK);
+}
+
 }  // namespace lt
 
 using namespace lt;
@@ -585,6 +621,53 @@ int lt_build_from_keys(int dim, int base_level, int max_level, const double* dom
   if (st != LT_OK) return fail(st);
   if (t->h_s->volume != (1ull << (dim * max_level))) return fail(LT_ERR_INCOMPLETE);
   if ((rc = launch_build_index(t, t->cur)) != LT_OK) return fail(rc);
+  *out = (lt_tree*)t;
+  return LT_OK;
+}
+
+int lt_build_complete_from_keys(int dim, int base_level, int max_level, const double* domain, const int* periodic,
+                                void* cuda_stream, const uint64_t* d_keys, int64_t n, lt_tree** out) {
+  if (!d_keys || n < 1 || n >= (1ll << 30)) return LT_ERR_ARG;
+  Tree* t = nullptr;
+  int rc = new_tree(dim, base_level, max_level, domain, periodic, cuda_stream, &t);
+  if (rc != LT_OK) return rc;
+  uint64_t* work = nullptr;
+  if ((rc = alloc_dev(&work, n)) == LT_OK) {
+    if (cudaMemcpyAsync(work, d_keys, (size_t)n * 8, cudaMemcpyDeviceToDevice, t->stream) != cudaSuccess)
+      rc = LT_ERR_CUDA;
+    else
+      rc = complete_from_unsorted(t, work, n);
+  }
+  cudaStreamSynchronize(t->stream);
+  free_dev(work);
+  if (rc != LT_OK) {
+    lt_free((lt_tree*)t);
+    return rc;
+  }
+  *out = (lt_tree*)t;
+  return LT_OK;
+}
+
+int lt_build_from_points(int dim, int base_level, int max_level, const double* domain, const int* periodic,
+                         void* cuda_stream, const double* d_xyz, int64_t n, lt_tree** out) {
+  if (!d_xyz || !domain || n < 1 || n >= (1ll << 30)) return LT_ERR_ARG;
+  if (dim == 2 || dim == 3)
+    for (int a = 0; a < dim; ++a)
+      if (!(domain[dim + a] > domain[a])) return LT_ERR_ARG;
+  Tree* t = nullptr;
+  int rc = new_tree(dim, base_level, max_level, domain, periodic, cuda_stream, &t);
+  if (rc != LT_OK) return rc;
+  uint64_t* work = nullptr;
+  if ((rc = alloc_dev(&work, n)) == LT_OK) {
+    rc = launch_points_to_keys(dim, max_level, t->domain, d_xyz, n, work, grid_for(t, 8), t->stream, &t->launches);
+    if (rc == LT_OK) rc = complete_from_unsorted(t, work, n);
+  }
+  cudaStreamSynchronize(t->stream);
+  free_dev(work);
+  if (rc != LT_OK) {
+    lt_free((lt_tree*)t);
+    return rc;
+  }
   *out = (lt_tree*)t;
   return LT_OK;
 }

@@ -113,6 +113,12 @@ int launch_map(Tree* t);
 int launch_transfer(Tree* t, const double* d_u_old, double* d_u_new, int p, int nvars);
 int build_operators(Tree* t, int p);
 
+// ---- lt_construct.cu (Alg. 2)
+int launch_points_to_keys(int dim, int maxl, const double* domain, const double* d_xyz, int64_t n, uint64_t* d_keys,
+                          int G, cudaStream_t s, int64_t* launches);
+int launch_complete_count(Tree* t, const uint64_t* d_in, int64_t n, uint32_t* d_offs, int64_t* total);
+int launch_complete_fill(Tree* t, const uint64_t* d_in, int64_t n, const uint32_t* d_offs, int64_t total);
+
 // ---- lt_sort.cu
 struct SortScratch {
   uint64_t* tmp; int64_t cap; unsigned* hist; unsigned* status; int64_t status_cap; int* counter;

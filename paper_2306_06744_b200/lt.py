@@ -42,6 +42,8 @@ _P, _I, _I64 = C.c_void_p, C.c_int, C.c_int64
 SIGNATURES = {
     "lt_build": (_I, [_I, _I, _I, _P, _P, _P, C.POINTER(_P)]),
     "lt_build_from_keys": (_I, [_I, _I, _I, _P, _P, _P, _P, _I64, C.POINTER(_P)]),
+    "lt_build_complete_from_keys": (_I, [_I, _I, _I, _P, _P, _P, _P, _I64, C.POINTER(_P)]),
+    "lt_build_from_points": (_I, [_I, _I, _I, _P, _P, _P, _P, _I64, C.POINTER(_P)]),
     "lt_free": (None, [_P]),
     "lt_reserve": (_I, [_P, _I64]),
     "lt_adapt": (_I, [_P, _P]),
@@ -124,7 +126,8 @@ def _dptr(t: torch.Tensor, dtype, where):
 class Tree:
     """One linear quadtree / octree on the current CUDA device (handle of lt_build)."""
 
-    def __init__(self, dim, base_level, max_level, domain=None, periodic=None, keys=None, device=None):
+    def __init__(self, dim, base_level, max_level, domain=None, periodic=None, keys=None, device=None,
+                 complete=False, points=None):
         self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
         self.dim, self.base, self.maxl = dim, base_level, max_level
         self.nc, self.nf = 1 << dim, 2 * dim
@@ -133,7 +136,19 @@ class Tree:
         h = C.c_void_p()
         with torch.cuda.device(self.device):
             self._stream = torch.cuda.current_stream(self.device)
-            if keys is None:
+            if points is not None:
+                x = points.contiguous()
+                if x.dim() != 2 or x.shape[1] != dim:
+                    raise ValueError("lt_build_from_points: points must be [n, dim]")
+                rc = lib().lt_build_from_points(dim, base_level, max_level, dom, per, _stream_ptr(self.device),
+                                                _dptr(x, torch.float64, "points"), x.shape[0], C.byref(h))
+            elif keys is not None and complete:
+                k = keys.contiguous()
+                rc = lib().lt_build_complete_from_keys(dim, base_level, max_level, dom, per,
+                                                       _stream_ptr(self.device),
+                                                       _dptr(k.view(torch.int64), torch.int64, "keys"), k.numel(),
+                                                       C.byref(h))
+            elif keys is None:
                 rc = lib().lt_build(dim, base_level, max_level, dom, per, _stream_ptr(self.device), C.byref(h))
             else:
                 k = keys.contiguous()
@@ -259,6 +274,16 @@ def build(dim, base_level, max_level, domain=None, periodic=None) -> Tree:
 def build_from_keys(dim, base_level, max_level, keys, domain=None, periodic=None) -> Tree:
     """lt_build_from_keys: keys = int64 CUDA tensor holding the uint64 IDs."""
     return Tree(dim, base_level, max_level, domain, periodic, keys=keys)
+
+
+def build_complete_from_keys(dim, base_level, max_level, keys, domain=None, periodic=None) -> Tree:
+    """lt_build_complete_from_keys (Alg. 2 on octants): keys = int64 CUDA tensor of uint64 IDs."""
+    return Tree(dim, base_level, max_level, domain, periodic, keys=keys, complete=True)
+
+
+def build_from_points(dim, base_level, max_level, points, domain, periodic=None) -> Tree:
+    """lt_build_from_points (Alg. 2): points = float64 CUDA tensor [n, dim]."""
+    return Tree(dim, base_level, max_level, domain, periodic, points=points)
 
 
 def encode(dim, max_level, xyz: torch.Tensor, level: torch.Tensor) -> torch.Tensor:
