@@ -463,8 +463,111 @@ def run_e2e(R, args, world, dev):
     ms = ev0.elapsed_time(ev1)
     assert t.num_leaves() == M1
     return {"ms": ms, "leaves": M1, "h2d": M0 * Bu + M0, "d2h": M1 * Bu + 64, "cycle": pick,
-            "note": "config-5 cycle %d (%d -> %d leaves); host budget %.0f GB; includes first-use staging "
-                    "allocation inside lt_transfer_host" % (pick, M0, M1, budget / 2 ** 30)}
+            "note": "config-5 cycle %d (%d -> %d leaves); host budget %.0f GB; lt_transfer_host pipelines "
+                    "upload / kernel / download in slabs (three streams, 3-slab staging ring)" % (pick, M0, M1, budget / 2 ** 30)}
+
+
+# --------------------------------------------------------------------------- construction leg
+CONSTRUCT_METRIC = "leaves/s per tree construction from a point cloud (Alg. 2) + full-depth 2:1 balance + connectivity"
+
+
+def oracle_construct(pc, pts_host):
+    """The oracle on the same points: Alg. 2 + balance + connect.  Returns (leaves, seconds)."""
+    import oracle
+    dim = pc["dim"]
+    dom = [pc["lo"]] * dim + [pc["hi"]] * dim
+    t0 = time.perf_counter()
+    ot = oracle.Tree(dim, pc["base"], pc["maxl"], pc["periodic"], points=pts_host, domain=dom)
+    ot.balance()
+    ot.connect()
+    return ot.num_leaves(), time.perf_counter() - t0
+
+
+def run_construct(args):
+    """--workload construct: SURVEY.md 8(f)-1.  A step = lt_build_from_points (encode, radix sort,
+    linearise, completion) + lt_balance + lt_connect on the seeded surface cloud `pc10`
+    (16 M points, D_min 4, D_max 10: the stand-in for the paper's bunny run)."""
+    import torch
+    from paper_2306_06744_b200 import build as B
+    B.build()
+    from paper_2306_06744_b200 import lt
+    from paper_2306_06744_b200 import workloads as W
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    name = args.cloud
+    pc = W.POINT_CLOUDS[name]
+    dim = pc["dim"]
+    dom = [pc["lo"]] * dim + [pc["hi"]] * dim
+    pts = W.surface_points(pc, device=dev)
+    h_pts = pts.cpu().pin_memory()
+    stream = torch.cuda.current_stream(dev)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+
+    def step(from_host=False):
+        torch.cuda.synchronize(dev)
+        ev[0].record(stream)
+        x = h_pts.to(dev, non_blocking=True) if from_host else pts
+        t = lt.build_from_points(dim, pc["base"], pc["maxl"], x, dom, pc["periodic"])
+        ev[1].record(stream)
+        n0 = t.num_leaves()
+        it = t.balance()
+        ev[2].record(stream)
+        F = t.connect()
+        h_keys = t.keys().cpu() if from_host else None
+        ev[3].record(stream)
+        torch.cuda.synchronize(dev)
+        r = dict(n0=n0, n1=t.num_leaves(), iters=it, faces=int(F["n_conf"] + F["n_hang"] + F["n_bnd"]),
+                 ms=ev[0].elapsed_time(ev[3]), build=ev[0].elapsed_time(ev[1]), balance=ev[1].elapsed_time(ev[2]),
+                 connect=ev[2].elapsed_time(ev[3]), launches=t.launch_count(),
+                 d2h=0 if h_keys is None else h_keys.numel() * 8)
+        t.free()
+        return r
+
+    for _ in range(max(args.warmup, 0)):
+        step()
+    sampler = ClockSampler(0)
+    sampler.start()
+    steps = [step() for _ in range(args.steps)]
+    clocks = sampler.stop()
+    tot = sum(s["ms"] for s in steps)
+    leaves = sum(s["n1"] for s in steps)
+    e = [step(from_host=True) for _ in range(max(1, min(args.steps, 3)))]
+    e_ms = sum(s["ms"] for s in e)
+    cpu = None
+    if not args.no_cpu_baseline:
+        small = W.POINT_CLOUDS["pc9"]
+        hp = W.surface_points(small).numpy()
+        n, dt = oracle_construct(small, hp)
+        cpu = {"value": n / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
+               "sample": "cloud pc9 in full (4 M points, D_min 4, D_max 9 -> %d leaves): Alg. 2 + balance + connect" % n}
+    peak, peak_src = hbm_peak()
+    s0 = steps[0]
+    out = {
+        "metric": CONSTRUCT_METRIC, "value": leaves / (tot * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": tot / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "int64", "data": "synthetic",
+        "config": {"workload": "construct/%s: %d seeded points on a %s surface, %d-D, D_min %d, D_max %d -> %d leaves "
+                               "after completion, %d after balance (%d sweeps), %d faces"
+                               % (name, pts.shape[0], pc["surface"], dim, pc["base"], pc["maxl"], s0["n0"], s0["n1"],
+                                  s0["iters"], s0["faces"]),
+                   "l2": "each step builds a new tree from the 384 MB point array (larger than L2)",
+                   "timing": "CUDA events around lt_build_from_points + lt_balance + lt_connect; includes the "
+                             "library's own device allocations"},
+        "ms_per_call": {k: sum(s[k] for s in steps) / args.steps for k in ("build", "balance", "connect")},
+        "points_per_s": pts.shape[0] * args.steps / (sum(s["build"] for s in steps) * 1e-3),
+        "roofline": {"bound": "hbm", "kernel": "whole construction call (allocation-bound, see profiles/r1c_construct.md)",
+                     "achieved": (24 * pts.shape[0] + 8 * s0["n0"]) * args.steps / (sum(s["build"] for s in steps) * 1e-3) / 1e9,
+                     "peak": peak, "unit": "GB/s", "peak_source": peak_src, "traffic": None,
+                     "frac": (24 * pts.shape[0] + 8 * s0["n0"]) * args.steps / (sum(s["build"] for s in steps) * 1e-3) / 1e9 / peak},
+        "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": sum(s["launches"] for s in steps),
+        "e2e": {"value": sum(s["n1"] for s in e) / (e_ms * 1e-3), "unit": UNIT,
+                "h2d_bytes_per_step": h_pts.numel() * 8, "d2h_bytes_per_step": e[0]["d2h"], "ms_per_step": e_ms / len(e)},
+    }
+    print(json.dumps(out), flush=True)
 
 
 def main():
@@ -475,6 +578,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", default="cycle", choices=["cycle", "construct"],
+                    help="cycle (default): the adaptation cycle BASELINE.json's metric is quoted on; construct: "
+                         "tree construction from a point cloud (SURVEY.md 8(f)-1)")
+    ap.add_argument("--cloud", default="pc10", help="point cloud of --workload construct (workloads.POINT_CLOUDS)")
     ap.add_argument("--cycles", default=None,
                     help="consecutive config-5 cycles a step cycles through (default 3,4,5 = the bench "
                          "workload; smaller ones, e.g. 2, keep an ncu --set full capture short)")
@@ -486,7 +593,9 @@ def main():
         PREP_CYCLES = PERIOD[0]
     if args.steps < 1:
         args.steps = 1
-    if args.impl == "reference":
+    if args.workload == "construct" and args.impl == "ours":
+        run_construct(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -169,8 +169,11 @@ int lt_connect(lt_tree*, lt_faces* out);
  * lt_sync reports it otherwise. */
 int lt_transfer(lt_tree*, const double* d_u_old, double* d_u_new, int p, int nvars);
 
-/* Same as lt_transfer with HOST arrays: copies h_u_old in, runs the transfer, copies
- * h_u_new out (device staging buffers owned by the tree).  Synchronises. */
+/* Same as lt_transfer with HOST arrays (pinned memory for full speed).  Pipelined in slabs of
+ * consecutive new leaves: slab k reads one contiguous range of old leaves (the map is
+ * monotone), so the upload of slab k+1, the kernel on slab k and the download of slab k-1
+ * overlap on three streams and only a ring of three slab pairs is staged in device memory
+ * (owned by the tree).  Synchronises. */
 int lt_transfer_host(lt_tree*, const double* h_u_old, double* h_u_new, int p, int nvars);
 
 /* ---- accessors --------------------------------------------------------------------- */
@@ -210,8 +213,10 @@ int lt_sync(lt_tree*);
 typedef enum {
   LT_OPT_ADAPT_SORT = 1, /* 0 (default): ordered expansion; 1: append + sort + linearise */
   LT_OPT_BALANCE_FULL_SWEEPS = 2, /* 1: every sweep examines every leaf (debug)         */
-  LT_OPT_DEBUG_BALANCE_SLACK = 3  /* v > 0: lt_balance pretends its buffers hold only n + v
+  LT_OPT_DEBUG_BALANCE_SLACK = 3, /* v > 0: lt_balance pretends its buffers hold only n + v
                                      leaves, to exercise the LT_ERR_CAPACITY retry (tests) */
+  LT_OPT_HOST_SLAB_LEAVES = 4     /* v > 0: new leaves per slab of lt_transfer_host's copy /
+                                     compute pipeline (default: about 128 MB of solution)   */
 } lt_option;
 int lt_set_option(lt_tree*, int option, int value);
 

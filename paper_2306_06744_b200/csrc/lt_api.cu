@@ -14,16 +14,50 @@ namespace lt {
 
 thread_local int g_last_cuda_error = 0;
 
-static void free_dev(void* p) {
-  if (p) cudaFree(p);
+// Device memory comes from the device's default stream-ordered pool (cudaMallocAsync): a
+// freed block is reused by the next allocation on the tree's stream without a driver call,
+// so building a tree (two dozen buffers) costs microseconds of allocation once the pool is
+// warm.  The pool keeps at most kPoolKeepBytes cached across synchronisation points.
+constexpr unsigned long long kPoolKeepBytes = 8ull << 30;
+
+static void pool_setup() {
+  static thread_local int done_for = -1;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev == done_for) return;
+  cudaMemPool_t pool;
+  if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+    unsigned long long cur = 0;
+    cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &cur);
+    if (cur < kPoolKeepBytes) {
+      unsigned long long keep = kPoolKeepBytes;
+      cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+  }
+  cudaGetLastError();
+  done_for = dev;
 }
 
-template <typename T>
-static int alloc_dev(T** p, int64_t count) {
+int dev_alloc(void** p, size_t bytes, cudaStream_t s) {
   *p = nullptr;
-  if (count <= 0) count = 1;
-  LT_CUDA(cudaMalloc((void**)p, (size_t)count * sizeof(T)));
+  if (bytes == 0) bytes = 16;
+  pool_setup();
+  LT_CUDA(cudaMallocAsync(p, bytes, s));
   return LT_OK;
+}
+
+void dev_free(void* p, cudaStream_t s) {
+  if (p && cudaFreeAsync(p, s) != cudaSuccess) {
+    cudaGetLastError();
+    cudaFree(p);
+  }
+}
+
+static void free_dev(cudaStream_t s, void* p) { dev_free(p, s); }
+
+template <typename T>
+static int alloc_dev(cudaStream_t s, T** p, int64_t count) {
+  if (count <= 0) count = 1;
+  return dev_alloc((void**)p, (size_t)count * sizeof(T), s);
 }
 
 static int64_t round_cap(int64_t n) { return (n + 1023) / 1024 * 1024; }
@@ -48,23 +82,23 @@ static int grow(Tree* t, int64_t need) {
   uint8_t* fbytes = nullptr;
   unsigned long long* tstate = nullptr;
   int rc = LT_OK;
-  for (int b = 0; b < 3 && rc == LT_OK; ++b) rc = alloc_dev(&nk[b], cap);
-  if (rc == LT_OK) rc = alloc_dev(&mark, cap);
-  if (rc == LT_OK) rc = alloc_dev(&fr[0], cap);
-  if (rc == LT_OK) rc = alloc_dev(&fr[1], cap);
-  if (rc == LT_OK) rc = alloc_dev(&nbr, cap * nf);
-  if (rc == LT_OK) rc = alloc_dev(&kind, cap * nf);
-  if (rc == LT_OK) rc = alloc_dev(&msrc, cap);
-  if (rc == LT_OK) rc = alloc_dev(&mkind, cap);
+  for (int b = 0; b < 3 && rc == LT_OK; ++b) rc = alloc_dev(t->stream, &nk[b], cap);
+  if (rc == LT_OK) rc = alloc_dev(t->stream, &mark, cap);
+  if (rc == LT_OK) rc = alloc_dev(t->stream, &fr[0], cap);
+  if (rc == LT_OK) rc = alloc_dev(t->stream, &fr[1], cap);
+  if (rc == LT_OK) rc = alloc_dev(t->stream, &nbr, cap * nf);
+  if (rc == LT_OK) rc = alloc_dev(t->stream, &kind, cap * nf);
+  if (rc == LT_OK) rc = alloc_dev(t->stream, &msrc, cap);
+  if (rc == LT_OK) rc = alloc_dev(t->stream, &mkind, cap);
   // face-table pool with fixed regions (lt_connect.cu face_regions): n_conf, n_hang <= dim*M
   // rows of 2 int32, n_bnd <= nf*M rows of 1 int32, one byte per row
-  if (rc == LT_OK) rc = alloc_dev(&frows, cap * (4 * dim + nf));
-  if (rc == LT_OK) rc = alloc_dev(&fbytes, cap * (2 * dim + nf));
-  if (rc == LT_OK) rc = alloc_dev(&tstate, 2 * (cap / 256 + 2));
+  if (rc == LT_OK) rc = alloc_dev(t->stream, &frows, cap * (4 * dim + nf));
+  if (rc == LT_OK) rc = alloc_dev(t->stream, &fbytes, cap * (2 * dim + nf));
+  if (rc == LT_OK) rc = alloc_dev(t->stream, &tstate, 2 * (cap / 256 + 2));
   if (rc != LT_OK) {
-    for (int b = 0; b < 3; ++b) free_dev(nk[b]);
-    free_dev(mark); free_dev(fr[0]); free_dev(fr[1]); free_dev(nbr); free_dev(kind); free_dev(msrc); free_dev(mkind);
-    free_dev(frows); free_dev(fbytes); free_dev(tstate);
+    for (int b = 0; b < 3; ++b) free_dev(t->stream, nk[b]);
+    free_dev(t->stream, mark); free_dev(t->stream, fr[0]); free_dev(t->stream, fr[1]); free_dev(t->stream, nbr); free_dev(t->stream, kind); free_dev(t->stream, msrc); free_dev(t->stream, mkind);
+    free_dev(t->stream, frows); free_dev(t->stream, fbytes); free_dev(t->stream, tstate);
     return rc;
   }
   if (t->keys[t->cur] && t->n_valid && t->n > 0)
@@ -74,19 +108,19 @@ static int grow(Tree* t, int64_t need) {
   LT_CUDA(cudaMemsetAsync(mark, 0, (size_t)cap, t->stream));
   LT_CUDA(cudaStreamSynchronize(t->stream));
   for (int b = 0; b < 3; ++b) {
-    free_dev(t->keys[b]);
+    free_dev(t->stream, t->keys[b]);
     t->keys[b] = nk[b];
   }
-  free_dev(t->mark); t->mark = mark;
-  free_dev(t->frontier[0]); t->frontier[0] = fr[0];
-  free_dev(t->frontier[1]); t->frontier[1] = fr[1];
-  free_dev(t->nbr); t->nbr = nbr;
-  free_dev(t->kind); t->kind = kind;
-  free_dev(t->map_src); t->map_src = msrc;
-  free_dev(t->map_kind); t->map_kind = mkind;
-  free_dev(t->face_rows); t->face_rows = frows;
-  free_dev(t->face_bytes); t->face_bytes = fbytes;
-  free_dev(t->tile_state); t->tile_state = tstate;
+  free_dev(t->stream, t->mark); t->mark = mark;
+  free_dev(t->stream, t->frontier[0]); t->frontier[0] = fr[0];
+  free_dev(t->stream, t->frontier[1]); t->frontier[1] = fr[1];
+  free_dev(t->stream, t->nbr); t->nbr = nbr;
+  free_dev(t->stream, t->kind); t->kind = kind;
+  free_dev(t->stream, t->map_src); t->map_src = msrc;
+  free_dev(t->stream, t->map_kind); t->map_kind = mkind;
+  free_dev(t->stream, t->face_rows); t->face_rows = frows;
+  free_dev(t->stream, t->face_bytes); t->face_bytes = fbytes;
+  free_dev(t->stream, t->tile_state); t->tile_state = tstate;
   t->map_valid = false;
   t->cap = cap;
   return LT_OK;
@@ -165,10 +199,10 @@ static int new_tree(int dim, int base, int maxl, const double* domain, const int
     return code;
   };
   for (int b = 0; b < 3; ++b)
-    if ((rc = alloc_dev(&t->first[b], (int64_t)g.nbuckets + 1)) != LT_OK) return fail(rc);
-  if ((rc = alloc_dev(&t->d_s, 1)) != LT_OK) return fail(rc);
-  if ((rc = alloc_dev(&t->d_sums, kMaxGrid)) != LT_OK) return fail(rc);
-  if ((rc = alloc_dev(&t->d_sums3, 3 * kMaxGrid)) != LT_OK) return fail(rc);
+    if ((rc = alloc_dev(t->stream, &t->first[b], (int64_t)g.nbuckets + 1)) != LT_OK) return fail(rc);
+  if ((rc = alloc_dev(t->stream, &t->d_s, 1)) != LT_OK) return fail(rc);
+  if ((rc = alloc_dev(t->stream, &t->d_sums, kMaxGrid)) != LT_OK) return fail(rc);
+  if ((rc = alloc_dev(t->stream, &t->d_sums3, 3 * kMaxGrid)) != LT_OK) return fail(rc);
   if (cudaMallocHost((void**)&t->h_s, sizeof(DevScalars)) != cudaSuccess) return fail(LT_ERR_OOM);
   if (cudaMallocHost((void**)&t->h_sums, (3 * kMaxGrid + 16) * sizeof(unsigned long long)) != cudaSuccess)
     return fail(LT_ERR_OOM);
@@ -192,18 +226,18 @@ static int complete_from_unsorted(Tree* t, uint64_t* work, int64_t n) {
   if (rc != LT_OK) return rc;
   uint64_t* lin = nullptr;
   uint32_t* offs = nullptr;
-  if ((rc = alloc_dev(&lin, n)) != LT_OK) return rc;
+  if ((rc = alloc_dev(t->stream, &lin, n)) != LT_OK) return rc;
   auto done = [&](int code) {
     cudaStreamSynchronize(t->stream);
-    free_dev(lin);
-    free_dev(offs);
+    free_dev(t->stream, lin);
+    free_dev(t->stream, offs);
     return code;
   };
   int64_t m = 0, total = 0;
   rc = linearise_keys(dim, maxl, work, lin, n, &m, t->d_sums, &t->d_s->aux, (int*)t->h_sums, grid_for(t, 4),
                       t->stream, &t->launches);
   if (rc != LT_OK) return done(rc);
-  if ((rc = alloc_dev(&offs, m + 2)) != LT_OK) return done(rc);
+  if ((rc = alloc_dev(t->stream, &offs, m + 2)) != LT_OK) return done(rc);
   if ((rc = launch_complete_count(t, lin, m, offs, &total)) != LT_OK) return done(rc);
   const int st = take_status(t);
   if (st != LT_OK) return done(st);
@@ -243,18 +277,28 @@ void lt_free(lt_tree* t) {
   if (!t) return;
   cudaStreamSynchronize(t->stream);
   for (int b = 0; b < 3; ++b) {
-    free_dev(t->keys[b]);
-    free_dev(t->first[b]);
+    free_dev(t->stream, t->keys[b]);
+    free_dev(t->stream, t->first[b]);
   }
-  free_dev(t->d_s); free_dev(t->d_sums); free_dev(t->d_sums3);
+  free_dev(t->stream, t->d_s); free_dev(t->stream, t->d_sums); free_dev(t->stream, t->d_sums3);
   if (t->h_s) cudaFreeHost(t->h_s);
   if (t->h_sums) cudaFreeHost(t->h_sums);
-  free_dev(t->mark); free_dev(t->frontier[0]); free_dev(t->frontier[1]);
-  free_dev(t->nbr); free_dev(t->kind);
-  free_dev(t->face_rows); free_dev(t->face_bytes); free_dev(t->tile_state);
-  free_dev(t->map_src); free_dev(t->map_kind); free_dev(t->d_ops);
-  free_dev(t->stage_old); free_dev(t->stage_new);
-  free_dev(t->sort_tmp); free_dev(t->sort_hist); free_dev(t->sort_status);
+  free_dev(t->stream, t->mark); free_dev(t->stream, t->frontier[0]); free_dev(t->stream, t->frontier[1]);
+  free_dev(t->stream, t->nbr); free_dev(t->stream, t->kind);
+  free_dev(t->stream, t->face_rows); free_dev(t->stream, t->face_bytes); free_dev(t->stream, t->tile_state);
+  free_dev(t->stream, t->map_src); free_dev(t->stream, t->map_kind); free_dev(t->stream, t->d_ops);
+  for (int r = 0; r < Tree::kRing; ++r) {
+    free_dev(t->stream, t->ring_old[r]);
+    free_dev(t->stream, t->ring_new[r]);
+    if (t->ev_in[r]) cudaEventDestroy(t->ev_in[r]);
+    if (t->ev_done[r]) cudaEventDestroy(t->ev_done[r]);
+    if (t->ev_out[r]) cudaEventDestroy(t->ev_out[r]);
+  }
+  free_dev(t->stream, t->d_bounds);
+  if (t->h_bounds) cudaFreeHost(t->h_bounds);
+  if (t->s_in) cudaStreamDestroy(t->s_in);
+  if (t->s_out) cudaStreamDestroy(t->s_out);
+  free_dev(t->stream, t->sort_tmp); free_dev(t->stream, t->sort_hist); free_dev(t->stream, t->sort_status);
   for (int i = 0; i < 16; ++i)
     if (t->ev[i]) cudaEventDestroy(t->ev[i]);
   delete t;
@@ -321,6 +365,7 @@ int lt_set_option(lt_tree* t, int option, int value) {
   if (option == LT_OPT_ADAPT_SORT) t->opt_adapt_sort = value != 0;
   else if (option == LT_OPT_BALANCE_FULL_SWEEPS) t->opt_full_sweeps = value != 0;
   else if (option == LT_OPT_DEBUG_BALANCE_SLACK) t->opt_debug_slack = value > 0 ? value : 0;
+  else if (option == LT_OPT_HOST_SLAB_LEAVES) t->opt_host_slab = value > 0 ? value : 0;
   else return LT_ERR_ARG;
   return LT_OK;
 }
@@ -524,30 +569,100 @@ int lt_map(lt_tree* t, const int32_t** d_src, const uint8_t** d_kind) {
   return LT_OK;
 }
 
+// Host arrays: the transfer is pipelined in slabs of consecutive new leaves.  Slab k needs the
+// contiguous old range [o_k, o_k+1) (the map is monotone), so while the kernel works on slab
+// k the copy-in stream uploads slab k+1 and the copy-out stream downloads slab k-1: both PCIe
+// directions stay busy and only a ring of kRing slab pairs lives in device memory.
 int lt_transfer_host(lt_tree* t, const double* h_u_old, double* h_u_new, int p, int nvars) {
   if (!t || !h_u_old || !h_u_new || p < 0 || p > 7 || nvars < 1) return LT_ERR_ARG;
   int rc;
   if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
+  if ((rc = build_operators(t, p)) != LT_OK) return rc;
   int64_t E = nvars;
   for (int a = 0; a < t->g.dim; ++a) E *= (p + 1);
   const int64_t n_old = t->have_old ? t->n_old : t->n, n_new = t->n;
-  if (t->stage_old_cap < n_old * E) {
-    free_dev(t->stage_old);
-    t->stage_old_cap = 0;
-    if ((rc = alloc_dev(&t->stage_old, n_old * E)) != LT_OK) return rc;
-    t->stage_old_cap = n_old * E;
+  constexpr int R = Tree::kRing;
+  if (!t->s_in) {
+    LT_CUDA(cudaStreamCreateWithFlags(&t->s_in, cudaStreamNonBlocking));
+    LT_CUDA(cudaStreamCreateWithFlags(&t->s_out, cudaStreamNonBlocking));
+    for (int r = 0; r < R; ++r) {
+      LT_CUDA(cudaEventCreateWithFlags(&t->ev_in[r], cudaEventDisableTiming));
+      LT_CUDA(cudaEventCreateWithFlags(&t->ev_done[r], cudaEventDisableTiming));
+      LT_CUDA(cudaEventCreateWithFlags(&t->ev_out[r], cudaEventDisableTiming));
+    }
   }
-  if (t->stage_new_cap < n_new * E) {
-    free_dev(t->stage_new);
-    t->stage_new_cap = 0;
-    if ((rc = alloc_dev(&t->stage_new, n_new * E)) != LT_OK) return rc;
-    t->stage_new_cap = n_new * E;
+  // slabs of about 128 MB of new solution, a multiple of 1024 leaves, at most 4096 slabs
+  int64_t slab = ((128ll << 20) / (E * 8) + 1023) / 1024 * 1024;
+  if (slab < 1024) slab = 1024;
+  if (t->opt_host_slab > 0) slab = t->opt_host_slab;
+  while ((n_new + slab - 1) / slab > 4096) slab *= 2;
+  const int S = (int)((n_new + slab - 1) / slab);
+  if (t->bounds_cap < S + 1) {
+    free_dev(t->stream, t->d_bounds);
+    if (t->h_bounds) cudaFreeHost(t->h_bounds);
+    t->d_bounds = nullptr; t->h_bounds = nullptr; t->bounds_cap = 0;
+    if ((rc = alloc_dev(t->stream, &t->d_bounds, 2 * (int64_t)(S + 1))) != LT_OK) return rc;
+    LT_CUDA(cudaMallocHost((void**)&t->h_bounds, 2 * (size_t)(S + 1) * sizeof(int64_t)));
+    t->bounds_cap = S + 1;
   }
-  LT_CUDA(cudaMemcpyAsync(t->stage_old, h_u_old, (size_t)n_old * E * 8, cudaMemcpyHostToDevice, t->stream));
-  if ((rc = lt_transfer(t, t->stage_old, t->stage_new, p, nvars)) != LT_OK) return rc;
-  LT_CUDA(cudaMemcpyAsync(h_u_new, t->stage_new, (size_t)n_new * E * 8, cudaMemcpyDeviceToHost, t->stream));
-  rc = fetch_scalars(t);
-  if (rc != LT_OK) return rc;
+  tic(t, 3);
+  tic(t, 4);
+  if ((rc = launch_map(t)) != LT_OK) return rc;
+  toc(t, 4);
+  if ((rc = launch_slab_bounds(t, n_old, slab, S, t->d_bounds)) != LT_OK) return rc;
+  LT_CUDA(cudaMemcpyAsync(t->h_bounds, t->d_bounds, 2 * (size_t)(S + 1) * sizeof(int64_t), cudaMemcpyDeviceToHost,
+                          t->stream));
+  if ((rc = fetch_scalars(t)) != LT_OK) return rc;
+  int st = take_status(t);
+  if (st != LT_OK) return st;
+  const int64_t* B = t->h_bounds;
+  int64_t max_new = 0, max_old = 0;
+  for (int k = 0; k < S; ++k) {
+    if (B[2 * k + 2] - B[2 * k] > max_new) max_new = B[2 * k + 2] - B[2 * k];
+    if (B[2 * k + 3] - B[2 * k + 1] > max_old) max_old = B[2 * k + 3] - B[2 * k + 1];
+  }
+  if (t->ring_old_cap < max_old * E || t->ring_new_cap < max_new * E) {
+    for (int r = 0; r < R; ++r) {
+      free_dev(t->stream, t->ring_old[r]); t->ring_old[r] = nullptr;
+      free_dev(t->stream, t->ring_new[r]); t->ring_new[r] = nullptr;
+    }
+    t->ring_old_cap = t->ring_new_cap = 0;
+    for (int r = 0; r < R; ++r) {
+      if ((rc = alloc_dev(t->stream, &t->ring_old[r], max_old * E)) != LT_OK) return rc;
+      if ((rc = alloc_dev(t->stream, &t->ring_new[r], max_new * E)) != LT_OK) return rc;
+    }
+    t->ring_old_cap = max_old * E;
+    t->ring_new_cap = max_new * E;
+  }
+  // the copy streams must not run ahead of the (stream-ordered) ring allocation
+  LT_CUDA(cudaEventRecord(t->ev_done[0], t->stream));
+  LT_CUDA(cudaStreamWaitEvent(t->s_in, t->ev_done[0], 0));
+  LT_CUDA(cudaStreamWaitEvent(t->s_out, t->ev_done[0], 0));
+  tic(t, 5);
+  int used = 0;
+  for (int k = 0; k < S; ++k) {
+    const int64_t jk = B[2 * k], ok = B[2 * k + 1], jn = B[2 * k + 2], on = B[2 * k + 3];
+    if (jn <= jk) continue;
+    const int r = used % R;
+    if (used >= R) LT_CUDA(cudaStreamWaitEvent(t->s_in, t->ev_done[r], 0));
+    LT_CUDA(cudaMemcpyAsync(t->ring_old[r], h_u_old + ok * E, (size_t)(on - ok) * E * 8, cudaMemcpyHostToDevice, t->s_in));
+    LT_CUDA(cudaEventRecord(t->ev_in[r], t->s_in));
+    LT_CUDA(cudaStreamWaitEvent(t->stream, t->ev_in[r], 0));
+    if (used >= R) LT_CUDA(cudaStreamWaitEvent(t->stream, t->ev_out[r], 0));
+    if ((rc = launch_transfer(t, t->ring_old[r] - ok * E, t->ring_new[r] - jk * E, p, nvars, jk, jn)) != LT_OK) return rc;
+    LT_CUDA(cudaEventRecord(t->ev_done[r], t->stream));
+    LT_CUDA(cudaStreamWaitEvent(t->s_out, t->ev_done[r], 0));
+    LT_CUDA(cudaMemcpyAsync(h_u_new + jk * E, t->ring_new[r], (size_t)(jn - jk) * E * 8, cudaMemcpyDeviceToHost, t->s_out));
+    LT_CUDA(cudaEventRecord(t->ev_out[r], t->s_out));
+    ++used;
+  }
+  for (int r = 0; r < R && r < used; ++r) LT_CUDA(cudaStreamWaitEvent(t->stream, t->ev_out[r], 0));
+  toc(t, 5);
+  t->have_old = false;
+  t->n_old = 0;
+  t->map_valid = true;
+  toc(t, 3);
+  if ((rc = fetch_scalars(t)) != LT_OK) return rc;
   return take_status(t);
 }
 
@@ -567,8 +682,7 @@ int lt_sort_keys(int dim, int max_level, uint64_t* d_keys, int64_t n, int linear
     int* h_total = nullptr;
     uint64_t* d_out = nullptr;
     const int G = 148 * 4;
-    if (cudaMalloc(&d_sums, G * sizeof(unsigned long long)) != cudaSuccess ||
-        cudaMalloc(&d_total, sizeof(int)) != cudaSuccess || cudaMalloc(&d_out, (size_t)n * 8) != cudaSuccess ||
+    if (alloc_dev(s, &d_sums, G) != LT_OK || alloc_dev(s, &d_total, 1) != LT_OK || alloc_dev(s, &d_out, n) != LT_OK ||
         cudaMallocHost((void**)&h_total, sizeof(int)) != cudaSuccess) {
       rc = LT_ERR_OOM;
     } else {
@@ -577,11 +691,11 @@ int lt_sort_keys(int dim, int max_level, uint64_t* d_keys, int64_t n, int linear
         rc = LT_ERR_CUDA;
     }
     cudaStreamSynchronize(s);
-    free_dev(d_sums); free_dev(d_total); free_dev(d_out);
+    free_dev(s, d_sums); free_dev(s, d_total); free_dev(s, d_out);
     if (h_total) cudaFreeHost(h_total);
   }
   if (cudaStreamSynchronize(s) != cudaSuccess && rc == LT_OK) rc = LT_ERR_CUDA;
-  free_dev(sc.tmp); free_dev(sc.hist); free_dev(sc.status);
+  free_dev(s, sc.tmp); free_dev(s, sc.hist); free_dev(s, sc.status);
   if (n_out) *n_out = m;
   return rc;
 }
@@ -632,14 +746,14 @@ int lt_build_complete_from_keys(int dim, int base_level, int max_level, const do
   int rc = new_tree(dim, base_level, max_level, domain, periodic, cuda_stream, &t);
   if (rc != LT_OK) return rc;
   uint64_t* work = nullptr;
-  if ((rc = alloc_dev(&work, n)) == LT_OK) {
+  if ((rc = alloc_dev(t->stream, &work, n)) == LT_OK) {
     if (cudaMemcpyAsync(work, d_keys, (size_t)n * 8, cudaMemcpyDeviceToDevice, t->stream) != cudaSuccess)
       rc = LT_ERR_CUDA;
     else
       rc = complete_from_unsorted(t, work, n);
   }
   cudaStreamSynchronize(t->stream);
-  free_dev(work);
+  free_dev(t->stream, work);
   if (rc != LT_OK) {
     lt_free((lt_tree*)t);
     return rc;
@@ -658,12 +772,12 @@ int lt_build_from_points(int dim, int base_level, int max_level, const double* d
   int rc = new_tree(dim, base_level, max_level, domain, periodic, cuda_stream, &t);
   if (rc != LT_OK) return rc;
   uint64_t* work = nullptr;
-  if ((rc = alloc_dev(&work, n)) == LT_OK) {
+  if ((rc = alloc_dev(t->stream, &work, n)) == LT_OK) {
     rc = launch_points_to_keys(dim, max_level, t->domain, d_xyz, n, work, grid_for(t, 8), t->stream, &t->launches);
     if (rc == LT_OK) rc = complete_from_unsorted(t, work, n);
   }
   cudaStreamSynchronize(t->stream);
-  free_dev(work);
+  free_dev(t->stream, work);
   if (rc != LT_OK) {
     lt_free((lt_tree*)t);
     return rc;

@@ -67,13 +67,17 @@ struct Tree {
   double* d_ops;
   int ops_p;
 
-  // host staging for lt_transfer_host
-  double* stage_old; double* stage_new; int64_t stage_old_cap, stage_new_cap;
+  // lt_transfer_host: ring of device staging slabs, copy-in / copy-out streams, slab bounds
+  static constexpr int kRing = 3;
+  double* ring_old[kRing]; double* ring_new[kRing]; int64_t ring_old_cap, ring_new_cap;
+  cudaStream_t s_in, s_out;
+  cudaEvent_t ev_in[kRing], ev_done[kRing], ev_out[kRing];
+  int64_t* d_bounds; int64_t* h_bounds; int bounds_cap;
 
   // sort scratch
   uint64_t* sort_tmp; int64_t sort_cap; unsigned* sort_hist; unsigned* sort_status; int64_t sort_status_cap;
 
-  int opt_adapt_sort, opt_full_sweeps, opt_debug_slack;
+  int opt_adapt_sort, opt_full_sweeps, opt_debug_slack, opt_host_slab;
   cudaEvent_t ev[16];
   bool ev_set[8];
   int64_t launches;
@@ -91,6 +95,9 @@ extern thread_local int g_last_cuda_error;
   } while (0)
 
 int grid_for(const Tree* t, int blocks_per_sm);
+// stream-ordered device memory (lt_api.cu): the device's default cudaMallocAsync pool
+int dev_alloc(void** p, size_t bytes, cudaStream_t s);
+void dev_free(void* p, cudaStream_t s);
 
 // ---- lt_tree.cu
 int launch_build_uniform(Tree* t);
@@ -110,7 +117,9 @@ void face_regions(const Tree* t, int32_t** conf, uint8_t** conf_axis, int32_t** 
 
 // ---- lt_transfer.cu
 int launch_map(Tree* t);
-int launch_transfer(Tree* t, const double* d_u_old, double* d_u_new, int p, int nvars);
+int launch_transfer(Tree* t, const double* d_u_old, double* d_u_new, int p, int nvars, int64_t jb = 0,
+                    int64_t je = -1);
+int launch_slab_bounds(Tree* t, int64_t n_old, int64_t slab, int S, int64_t* d_out);
 int build_operators(Tree* t, int p);
 
 // ---- lt_construct.cu (Alg. 2)

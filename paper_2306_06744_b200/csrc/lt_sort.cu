@@ -111,16 +111,21 @@ int sort_keys(uint64_t* d_keys, int64_t n, int key_bits, SortScratch* sc, cudaSt
   if (passes < 1 || passes > 8) return LT_ERR_ARG;
   const int64_t tiles = (n + STILE - 1) / STILE;
   if (sc->cap < n) {
-    if (sc->tmp) cudaFree(sc->tmp);
+    dev_free(sc->tmp, s);
     sc->tmp = nullptr;
-    LT_CUDA(cudaMalloc(&sc->tmp, (size_t)n * sizeof(uint64_t)));
+    int rc = dev_alloc((void**)&sc->tmp, (size_t)n * sizeof(uint64_t), s);
+    if (rc != LT_OK) return rc;
     sc->cap = n;
   }
-  if (!sc->hist) LT_CUDA(cudaMalloc(&sc->hist, (8 * 256 + 8) * sizeof(unsigned)));
+  if (!sc->hist) {
+    int rc = dev_alloc((void**)&sc->hist, (8 * 256 + 8) * sizeof(unsigned), s);
+    if (rc != LT_OK) return rc;
+  }
   if (sc->status_cap < tiles) {
-    if (sc->status) cudaFree(sc->status);
+    dev_free(sc->status, s);
     sc->status = nullptr;
-    LT_CUDA(cudaMalloc(&sc->status, (size_t)tiles * 256 * sizeof(unsigned)));
+    int rc = dev_alloc((void**)&sc->status, (size_t)tiles * 256 * sizeof(unsigned), s);
+    if (rc != LT_OK) return rc;
     sc->status_cap = tiles;
   }
   int* tickets = (int*)(sc->hist + 8 * 256);

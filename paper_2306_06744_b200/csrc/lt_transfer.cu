@@ -396,7 +396,11 @@ __global__ void __launch_bounds__(256, 4) k_transfer(const DevScalars* s,
                                                   const int32_t* __restrict__ map_src,
                                                   const uint8_t* __restrict__ map_kind,
                                                   const double* __restrict__ u_old, double* __restrict__ u_new,
-                                                  int nvars, int vec2, int sl_log2, unsigned* ticket) {
+                                                  int nvars, int vec2, int sl_log2, unsigned* ticket,
+                                                  int64_t jb, int64_t je) {
+  // [jb, je) = the slab of new leaves this launch handles (je < 0: up to the leaf count);
+  // u_old / u_new are indexed by ABSOLUTE old / new leaf numbers (lt_transfer_host passes
+  // staging pointers shifted by the slab origins)
   using X = Xfer<DIM, P1>;
   extern __shared__ double smem[];
   // tile << 8 | next sub-chunk; sub-chunk == kSubs: exhausted, > kSubs: a warp is fetching a ticket
@@ -404,9 +408,9 @@ __global__ void __launch_bounds__(256, 4) k_transfer(const DevScalars* s,
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   double* wsm = smem + (size_t)w * X::SMEM_DOUBLES;
   const size_t E = (size_t)nvars * X::N;
-  const int64_t n = s->n;
+  const int64_t n = je < 0 ? (int64_t)s->n : je;
   const int SL = 1 << sl_log2, TL = kSubs << sl_log2;
-  const int64_t ntiles = (n + TL - 1) / TL;
+  const int64_t ntiles = (n - jb + TL - 1) / TL;
   if (threadIdx.x == 0) s_word = kSubs;
   __syncthreads();
   for (;;) {
@@ -428,7 +432,7 @@ __global__ void __launch_bounds__(256, 4) k_transfer(const DevScalars* s,
             tile = atomicAdd(ticket, 1u);
             sub = 0;
             // the map entries of the tile this block is likely to claim next: into L2
-            const int64_t jp = ((int64_t)tile + gridDim.x) * TL;
+            const int64_t jp = jb + ((int64_t)tile + gridDim.x) * TL;
             if (jp < n) {
               asm volatile("prefetch.global.L2 [%0];" ::"l"(map_src + jp));
               asm volatile("prefetch.global.L2 [%0];" ::"l"(map_kind + jp));
@@ -442,7 +446,7 @@ __global__ void __launch_bounds__(256, 4) k_transfer(const DevScalars* s,
     tile = __shfl_sync(0xffffffffu, tile, 0);
     sub = __shfl_sync(0xffffffffu, sub, 0);
     if ((int64_t)tile >= ntiles) break;
-    const int64_t j0 = (int64_t)tile * TL + (int64_t)sub * SL;
+    const int64_t j0 = jb + (int64_t)tile * TL + (int64_t)sub * SL;
     int kd = 255, so = 0;
     if (lane < SL && j0 + lane < n) {
       kd = map_kind[j0 + lane];
@@ -562,7 +566,8 @@ int launch_map(Tree* t) {
 }
 
 template <int DIM, int P1>
-static int launch_transfer_t(Tree* t, const double* u_old, double* u_new, int nvars, int vec2) {
+static int launch_transfer_t(Tree* t, const double* u_old, double* u_new, int nvars, int vec2, int64_t jb,
+                             int64_t je) {
   using X = Xfer<DIM, P1>;
   int warps = 8;
   const size_t per_warp = (size_t)X::SMEM_DOUBLES * sizeof(double);
@@ -580,34 +585,59 @@ static int launch_transfer_t(Tree* t, const double* u_old, double* u_new, int nv
   while (sl_log2 < 5 && ((size_t)2 << sl_log2) * Bu <= 10240) ++sl_log2;
   LT_CUDA(cudaMemsetAsync(&t->d_s->ticket, 0, sizeof(unsigned), t->stream));
   fn<<<G, warps * 32, smem, t->stream>>>(t->d_s, t->map_src, t->map_kind, u_old, u_new, nvars, vec2, sl_log2,
-                                         &t->d_s->ticket);
+                                         &t->d_s->ticket, jb, je);
   t->launches++;
   LT_CUDA(cudaGetLastError());
   return LT_OK;
 }
 
 template <int DIM>
-static int launch_transfer_d(Tree* t, const double* u_old, double* u_new, int p, int nvars, int vec2) {
+static int launch_transfer_d(Tree* t, const double* u_old, double* u_new, int p, int nvars, int vec2, int64_t jb,
+                             int64_t je) {
   switch (p) {
-    case 0: return launch_transfer_t<DIM, 1>(t, u_old, u_new, nvars, vec2);
-    case 1: return launch_transfer_t<DIM, 2>(t, u_old, u_new, nvars, vec2);
-    case 2: return launch_transfer_t<DIM, 3>(t, u_old, u_new, nvars, vec2);
-    case 3: return launch_transfer_t<DIM, 4>(t, u_old, u_new, nvars, vec2);
-    case 4: return launch_transfer_t<DIM, 5>(t, u_old, u_new, nvars, vec2);
-    case 5: return launch_transfer_t<DIM, 6>(t, u_old, u_new, nvars, vec2);
-    case 6: return launch_transfer_t<DIM, 7>(t, u_old, u_new, nvars, vec2);
-    case 7: return launch_transfer_t<DIM, 8>(t, u_old, u_new, nvars, vec2);
+    case 0: return launch_transfer_t<DIM, 1>(t, u_old, u_new, nvars, vec2, jb, je);
+    case 1: return launch_transfer_t<DIM, 2>(t, u_old, u_new, nvars, vec2, jb, je);
+    case 2: return launch_transfer_t<DIM, 3>(t, u_old, u_new, nvars, vec2, jb, je);
+    case 3: return launch_transfer_t<DIM, 4>(t, u_old, u_new, nvars, vec2, jb, je);
+    case 4: return launch_transfer_t<DIM, 5>(t, u_old, u_new, nvars, vec2, jb, je);
+    case 5: return launch_transfer_t<DIM, 6>(t, u_old, u_new, nvars, vec2, jb, je);
+    case 6: return launch_transfer_t<DIM, 7>(t, u_old, u_new, nvars, vec2, jb, je);
+    case 7: return launch_transfer_t<DIM, 8>(t, u_old, u_new, nvars, vec2, jb, je);
   }
   return LT_ERR_ARG;
 }
 
-int launch_transfer(Tree* t, const double* d_u_old, double* d_u_new, int p, int nvars) {
+int launch_transfer(Tree* t, const double* d_u_old, double* d_u_new, int p, int nvars, int64_t jb, int64_t je) {
   int N = 1;
   for (int a = 0; a < t->g.dim; ++a) N *= (p + 1);
   const int E = nvars * N;
   const int vec2 = (E % 2 == 0) && (((uintptr_t)d_u_old & 15) == 0) && (((uintptr_t)d_u_new & 15) == 0);
-  return t->g.dim == 2 ? launch_transfer_d<2>(t, d_u_old, d_u_new, p, nvars, vec2)
-                       : launch_transfer_d<3>(t, d_u_old, d_u_new, p, nvars, vec2);
+  return t->g.dim == 2 ? launch_transfer_d<2>(t, d_u_old, d_u_new, p, nvars, vec2, jb, je)
+                       : launch_transfer_d<3>(t, d_u_old, d_u_new, p, nvars, vec2, jb, je);
+}
+
+// Slab boundaries for the pipelined host transfer: candidate k (k = 0..S) is moved forward to
+// the next new leaf that does not sit inside a refined sibling group (children 1..nc-1 are
+// written by the warp that owns child 0), so that slab [j_k, j_k+1) reads exactly the old
+// leaves [o_k, o_k+1): the map is monotone and partitions T_old (Alg. 7).
+__global__ void k_slab_bounds(const DevScalars* s, const int32_t* __restrict__ map_src,
+                              const uint8_t* __restrict__ map_kind, int64_t n_old, int64_t slab, int S,
+                              int64_t* __restrict__ out /* [S+1][2] */) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k > S) return;
+  const int64_t n = s->n;
+  int64_t j = (int64_t)k * slab;
+  if (j > n || k == S) j = n;
+  while (j < n && (map_kind[j] & 15) == 1 && (map_kind[j] >> 4) != 0) ++j;
+  out[2 * k] = j;
+  out[2 * k + 1] = j < n ? (int64_t)map_src[j] : n_old;
+}
+
+int launch_slab_bounds(Tree* t, int64_t n_old, int64_t slab, int S, int64_t* d_out) {
+  k_slab_bounds<<<(S + 1 + 127) / 128, 128, 0, t->stream>>>(t->d_s, t->map_src, t->map_kind, n_old, slab, S, d_out);
+  t->launches++;
+  LT_CUDA(cudaGetLastError());
+  return LT_OK;
 }
 
 }  // namespace lt

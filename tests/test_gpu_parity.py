@@ -187,6 +187,41 @@ def test_transfer_host_buffers():
     P.assert_u_close(h_new, un_o, "host transfer")
 
 
+@pytest.mark.parametrize("slab,pinned", [(1, True), (37, True), (37, False), (1000, True), (0, True)])
+def test_transfer_host_pipelined_slabs(slab, pinned):
+    # many slabs through the 3-deep staging ring, with refined groups and coarsened groups
+    # crossing the candidate slab boundaries; 3-D, copy + interpolate + project in one cycle
+    cfg = dict(W.CONFIGS["c4"], base=3, maxl=5)
+    gt, ot = P.new_pair(cfg)
+    rng = np.random.default_rng(5)
+    for c in range(2):
+        f = rng.integers(0, 2, ot.num_leaves()).astype(np.int8)
+        ot.adapt(f); ot.balance(); ot.drop_snapshot()
+        gt.adapt(torch.from_numpy(f).cuda()); gt.balance()
+    p, nvars = 2, 3
+    uo = rng.uniform(-1, 1, (ot.num_leaves(), nvars, 27))
+    f = rng.integers(-1, 2, ot.num_leaves()).astype(np.int8)
+    ot.adapt(f); ot.balance()
+    gt.adapt(torch.from_numpy(f).cuda()); gt.balance()
+    un_o = ot.transfer(uo, p, nvars)
+    h_old = torch.from_numpy(uo.copy())
+    h_new = torch.full((gt.num_leaves(), nvars, 27), float("nan"), dtype=torch.float64)
+    if pinned:
+        h_old, h_new = h_old.pin_memory(), h_new.pin_memory()
+    gt.set_option(4, slab)
+    gt.transfer_host(h_old, h_new, p, nvars)
+    assert not torch.isnan(h_new).any()
+    P.assert_u_close(h_new, un_o, "pipelined host transfer, slab %d" % slab)
+    src, kind = gt.map()
+    assert len(set((kind.cpu().numpy() & 15).tolist())) == 3  # copy, refine and coarsen all present
+    # the tree stays usable: a second cycle through the device path
+    f = rng.integers(-1, 2, ot.num_leaves()).astype(np.int8)
+    ot.adapt(f); ot.balance()
+    gt.adapt(torch.from_numpy(f).cuda()); gt.balance()
+    un_g = gt.transfer(torch.from_numpy(un_o).cuda(), p, nvars)
+    P.assert_u_close(un_g, ot.transfer(un_o, p, nvars), "device transfer after host transfer")
+
+
 def test_transfer_without_snapshot_is_copy():
     gt = lt.Tree(2, 3, 5)
     u = torch.rand((64, 2, 9), dtype=torch.float64, device="cuda")
