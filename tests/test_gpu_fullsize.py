@@ -14,7 +14,9 @@ import numpy as np
 import pytest
 import torch
 
+import oracle
 import parity as P
+from paper_2306_06744_b200 import lt
 from paper_2306_06744_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
@@ -101,3 +103,21 @@ def test_config5_full_size_cycle3():
             seen[k] += int(((kind_o[j0:j1] & 15) == k).sum())
     assert (seen > 0).all(), "sampled slabs must cover copy, refine and coarsen: %s" % seen
     print("c5 full size: sampled %d elements (copy/refine/coarsen %s), worst |diff| %.2e" % (seen.sum(), seen, worst))
+
+
+def test_construction_full_size_pc9():
+    """SURVEY 8(f)-1 at the size bench.py's cpu_baseline uses: 4 M points, D_min 4, D_max 9 ->
+    1.19 M leaves after completion, 1.40 M after the full-depth balance; keys, sweep count and
+    face tables bit-exact against the oracle."""
+    pc = W.POINT_CLOUDS["pc9"]
+    dom = [pc["lo"]] * 3 + [pc["hi"]] * 3
+    pts = W.surface_points(pc).numpy()
+    ot = oracle.Tree(3, pc["base"], pc["maxl"], pc["periodic"], points=pts, domain=dom)
+    gt = lt.build_from_points(3, pc["base"], pc["maxl"], torch.from_numpy(pts).cuda(), dom, pc["periodic"])
+    P.assert_keys_equal(gt, ot, "pc9 completion")
+    assert gt.num_leaves() == 1190953
+    it_o, it_g = ot.balance(), gt.balance()
+    assert it_o == it_g == 4
+    P.assert_keys_equal(gt, ot, "pc9 balance")
+    assert gt.num_leaves() == 1402682
+    P.assert_faces_equal(gt.connect(), ot.connect(), "pc9 connect")
