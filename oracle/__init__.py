@@ -73,6 +73,8 @@ def lib():
         L.lto_adapt.argtypes = [C.c_void_p, C.POINTER(C.c_int8)]
         L.lto_balance.restype = C.c_int
         L.lto_balance.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
+        L.lto_balance_conn.restype = C.c_int
+        L.lto_balance_conn.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.c_int]
         L.lto_connect.restype = C.c_int
         L.lto_connect.argtypes = [C.c_void_p, C.c_int]
         L.lto_face_counts.restype = None
@@ -224,9 +226,13 @@ class Tree:
         assert f.size == self.num_leaves()
         lib().lto_adapt(self._h, _p(f, C.c_int8))
 
-    def balance(self):
+    def balance(self, conn=1):
+        """conn: 1 faces (default), 2 + edges (3-D: the paper's strong balance; 2-D: corners),
+        3 + corners (3-D)."""
         ns = C.c_int64(0)
-        it = lib().lto_balance(self._h, C.byref(ns))
+        it = lib().lto_balance_conn(self._h, C.byref(ns), int(conn))
+        if it < 0:
+            raise OracleError("oracle balance: bad connectivity %r" % (conn,))
         self.last_balance_splits = ns.value
         return int(it)
 

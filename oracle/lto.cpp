@@ -265,21 +265,50 @@ void adapt(Tree* t, const int8_t* flags) {
 // the start of the sweep; every face-neighbour leaf with level < level(L) - 1
 // is marked; all marked leaves are split once.  Returns the number of sweeps
 // that split at least one leaf.
-int balance(Tree* t, int64_t* n_split_total) {
+// `conn` selects which neighbours count (reading C-1 / C-9): 1 = leaves sharing a face
+// (BASELINE.json's contract); 2 = faces and edges -- the paper's own "strong" balance in
+// 3-D, "any two adjacent octants that share either an edge or a face"; 3 =
+// faces, edges and corners.  In 2-D a quadrant's edges ARE its faces, so 1 is already the
+// paper's strong balance and 2 adds the corners.  A neighbour direction is an offset
+// o in {-1,0,+1}^dim with 1 <= |o|_0 <= conn; the same-level neighbour anchor is x + o*w
+// with periodic wrap per axis, directions leaving a non-periodic domain
+// are skipped.
+bool offset_anchor(const Tree* t, const Node* n, const int* o, uint32_t* nx) {
+  const int64_t w = (int64_t)1 << (t->maxl - n->level);
+  const int64_t L = (int64_t)1 << t->maxl;
+  for (int b = 0; b < 3; ++b) nx[b] = n->x[b];
+  for (int a = 0; a < t->dim; ++a) {
+    if (!o[a]) continue;
+    int64_t v = (int64_t)n->x[a] + o[a] * w;
+    if (v < 0 || v >= L) {
+      if (!t->periodic[a]) return false;
+      v = (v + L) % L;
+    }
+    nx[a] = (uint32_t)v;
+  }
+  return true;
+}
+
+int balance(Tree* t, int64_t* n_split_total, int conn) {
   int iters = 0;
   int64_t total = 0;
   for (;;) {
     std::vector<Node*> marked;
     for (Node* L : t->leaves) {
-      for (int f = 0; f < t->nf; ++f) {
-        uint32_t nx[3];
-        if (!neighbour_anchor(t, L, f, nx)) continue;
-        Node* N = locate(t, t->root, nx, L->level);
-        if (N->is_leaf() && N->level < L->level - 1 && !N->mark) {
-          N->mark = true;
-          marked.push_back(N);
-        }
-      }
+      int o[3] = {0, 0, 0};
+      for (o[0] = -1; o[0] <= 1; ++o[0])
+        for (o[1] = -1; o[1] <= 1; ++o[1])
+          for (o[2] = (t->dim == 3 ? -1 : 0); o[2] <= (t->dim == 3 ? 1 : 0); ++o[2]) {
+            const int nnz = (o[0] != 0) + (o[1] != 0) + (o[2] != 0);
+            if (nnz < 1 || nnz > conn) continue;
+            uint32_t nx[3];
+            if (!offset_anchor(t, L, o, nx)) continue;
+            Node* N = locate(t, t->root, nx, L->level);
+            if (N->is_leaf() && N->level < L->level - 1 && !N->mark) {
+              N->mark = true;
+              marked.push_back(N);
+            }
+          }
     }
     if (marked.empty()) break;
     for (Node* N : marked) {
@@ -919,7 +948,11 @@ int lto_dfs_is_sorted(void* h) {
 }
 
 void lto_adapt(void* h, const int8_t* flags) { adapt((Tree*)h, flags); }
-int lto_balance(void* h, int64_t* n_split) { return balance((Tree*)h, n_split); }
+int lto_balance(void* h, int64_t* n_split) { return balance((Tree*)h, n_split, 1); }
+int lto_balance_conn(void* h, int64_t* n_split, int conn) {
+  if (conn < 1 || conn > ((Tree*)h)->dim) return -1;
+  return balance((Tree*)h, n_split, conn);
+}
 
 // method: 0 = point-location descent, 1 = brute force O(N^2)
 int lto_connect(void* h, int method) {

@@ -68,17 +68,35 @@ def adapt(mesh, flag_of, base, maxl):
     return out
 
 
-def balance(mesh, periodic):
-    """Jacobi ripple; returns (mesh, iters, splits)."""
+def offset_neighbour(cell, offs, periodic):
+    """Same-level cell at integer offset `offs` (one entry per axis), periodic wrap per axis."""
+    l, c = cell[0], list(cell[1:])
+    n = 1 << l
+    for a, o in enumerate(offs):
+        c[a] += o
+        if c[a] < 0 or c[a] >= n:
+            if not periodic[a]:
+                return None
+            c[a] %= n
+    return (l,) + tuple(c)
+
+
+def directions(dim, conn):
+    """Offsets with between 1 and `conn` non-zero entries: faces, + edges, + corners."""
+    return [o for o in product((-1, 0, 1), repeat=dim) if 1 <= sum(1 for v in o if v) <= conn]
+
+
+def balance(mesh, periodic, conn=1):
+    """Jacobi ripple; returns (mesh, iters, splits).  conn: see directions()."""
     mesh = set(mesh)
     dim = len(next(iter(mesh))) - 1
+    dirs = directions(dim, conn)
     iters = splits = 0
     while True:
         marked = set()
         for cell in mesh:
-            for axis in range(dim):
-                for sign in (-1, 1):
-                    nb = face_neighbour(cell, axis, sign, periodic)
+            for o in dirs:
+                    nb = offset_neighbour(cell, o, periodic)
                     if nb is None:
                         continue
                     leaf = containing_leaf(mesh, nb)
@@ -103,6 +121,38 @@ def is_balanced(mesh, periodic):
                     continue
                 leaf = containing_leaf(mesh, nb)
                 if leaf is not None and leaf[0] < cell[0] - 1:
+                    return False
+    return True
+
+
+def is_balanced_boxes(mesh, periodic, conn, maxl):
+    """Geometric 2:1 check with no neighbour keys at all: two leaves are adjacent when their
+    closed boxes (any periodic image) touch in a set of dimension >= dim - conn, i.e. on every
+    axis the intervals overlap or touch, and they touch on between 1 and conn axes.  O(N^2)."""
+    cells = sorted(mesh)
+    dim = len(cells[0]) - 1
+    L = 1 << maxl
+    boxes = []
+    for c in cells:
+        w = 1 << (maxl - c[0])
+        boxes.append((c[0], [ci * w for ci in c[1:]], w))
+    for i, (la, xa, wa) in enumerate(boxes):
+        for lb, xb, wb in boxes[i + 1:]:
+            if abs(la - lb) < 2:
+                continue
+            shifts = [(-L, 0, L) if periodic[a] else (0,) for a in range(dim)]
+            for sh in product(*shifts):
+                touch = 0
+                ok = True
+                for a in range(dim):
+                    lo = max(xa[a], xb[a] + sh[a])
+                    hi = min(xa[a] + wa, xb[a] + sh[a] + wb)
+                    if hi < lo:
+                        ok = False
+                        break
+                    if hi == lo:
+                        touch += 1
+                if ok and 1 <= touch <= conn:
                     return False
     return True
 
