@@ -30,6 +30,7 @@ if ROOT not in sys.path:
 METRIC = "leaves/s per full adapt+2:1 balance+connectivity+transfer cycle"
 UNIT = "leaves/s"
 PREP_CYCLES = 3           # config-5 cycles 0..2 run untimed to develop the tree
+CONNECTIVITY = 1          # --connectivity: 1 face balance (BASELINE.json), 2 the paper's strong balance
 PERIOD = (3, 4, 5)        # config-5 cycles a step runs (--cycles a,b,.. overrides: profiling aid)
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 
@@ -179,6 +180,8 @@ class Runner:
         self.tree = self.lt.Tree(cfg["dim"], cfg["base"], cfg["maxl"], dom, cfg["periodic"])
         if reserve:
             self.tree.reserve(reserve)
+        if CONNECTIVITY != 1:
+            self.tree.set_option(self.lt.LT_OPT_BALANCE_CONNECTIVITY, CONNECTIVITY)
         for c in range(PREP_CYCLES):
             self.tree.adapt(self.flags(c))
             self.tree.balance()
@@ -391,7 +394,7 @@ def run_ours(args):
                        "step": "one adaptation cycle; steps run config-5 cycles %s after an untimed tree-only "
                                "replay of cycles 0-%d" % (list(PERIOD), PREP_CYCLES - 1),
                        "leaves_out_per_step": [s["M1"] for s in steps], "leaves_in_per_step": [s["M0"] for s in steps],
-                       "balance_iters": [s["iters"] for s in steps],
+                       "balance_iters": [s["iters"] for s in steps], "balance_connectivity": CONNECTIVITY,
                        "l2": "inputs larger than L2 (u_old + u_new are 57-115 GB per step)",
                        "parallelism": "replicas only (one independent tree per GPU)" if world > 1 else "single GPU",
                        "timing": "CUDA events on the tree's stream around lt_adapt..lt_transfer of each step; "
@@ -418,6 +421,8 @@ def run_e2e(R, args, world, dev):
     # leaf counts of cycles 0..PERIOD[0] (tree only)
     dom = [cfg["lo"]] * cfg["dim"] + [cfg["hi"]] * cfg["dim"]
     t = R.lt.Tree(cfg["dim"], cfg["base"], cfg["maxl"], dom, cfg["periodic"])
+    if CONNECTIVITY != 1:
+        t.set_option(R.lt.LT_OPT_BALANCE_CONNECTIVITY, CONNECTIVITY)
     R.tree = t
     counts = []
     for c in range(PERIOD[0] + 1):
@@ -431,6 +436,8 @@ def run_e2e(R, args, world, dev):
             pick = c
     t.free()
     t = R.lt.Tree(cfg["dim"], cfg["base"], cfg["maxl"], dom, cfg["periodic"])
+    if CONNECTIVITY != 1:
+        t.set_option(R.lt.LT_OPT_BALANCE_CONNECTIVITY, CONNECTIVITY)
     R.tree = t
     for c in range(pick):
         t.adapt(R.flags(c))
@@ -582,10 +589,15 @@ def main():
                     help="cycle (default): the adaptation cycle BASELINE.json's metric is quoted on; construct: "
                          "tree construction from a point cloud (SURVEY.md 8(f)-1)")
     ap.add_argument("--cloud", default="pc10", help="point cloud of --workload construct (workloads.POINT_CLOUDS)")
+    ap.add_argument("--connectivity", type=int, default=1,
+                    help="2:1 balance across faces (1, default = BASELINE.json's contract), faces + edges (2, the "
+                         "paper's strong balance, PAPER.md:132) or faces + edges + corners (3)")
     ap.add_argument("--cycles", default=None,
                     help="consecutive config-5 cycles a step cycles through (default 3,4,5 = the bench "
                          "workload; smaller ones, e.g. 2, keep an ncu --set full capture short)")
     args = ap.parse_args()
+    global CONNECTIVITY
+    CONNECTIVITY = args.connectivity
     if args.cycles:
         global PERIOD, PREP_CYCLES
         PERIOD = tuple(int(c) for c in args.cycles.split(","))

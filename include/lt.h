@@ -215,8 +215,14 @@ typedef enum {
   LT_OPT_BALANCE_FULL_SWEEPS = 2, /* 1: every sweep examines every leaf (debug)         */
   LT_OPT_DEBUG_BALANCE_SLACK = 3, /* v > 0: lt_balance pretends its buffers hold only n + v
                                      leaves, to exercise the LT_ERR_CAPACITY retry (tests) */
-  LT_OPT_HOST_SLAB_LEAVES = 4     /* v > 0: new leaves per slab of lt_transfer_host's copy /
+  LT_OPT_HOST_SLAB_LEAVES = 4,    /* v > 0: new leaves per slab of lt_transfer_host's copy /
                                      compute pipeline (default: about 128 MB of solution)   */
+  LT_OPT_BALANCE_CONNECTIVITY = 5 /* which neighbours lt_balance keeps within one level:
+                                     1 (default) leaves sharing a face; 2 + leaves sharing an
+                                     edge -- the paper's "strong" balance in 3-D (
+                                     in 2-D this adds the corner neighbours, a quadrant's edges
+                                     being its faces); 3 (3-D) + leaves sharing only a corner.
+                                     Values outside 1..dim: LT_ERR_ARG                       */
 } lt_option;
 int lt_set_option(lt_tree*, int option, int value);
 

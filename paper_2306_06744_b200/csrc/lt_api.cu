@@ -366,6 +366,10 @@ int lt_set_option(lt_tree* t, int option, int value) {
   else if (option == LT_OPT_BALANCE_FULL_SWEEPS) t->opt_full_sweeps = value != 0;
   else if (option == LT_OPT_DEBUG_BALANCE_SLACK) t->opt_debug_slack = value > 0 ? value : 0;
   else if (option == LT_OPT_HOST_SLAB_LEAVES) t->opt_host_slab = value > 0 ? value : 0;
+  else if (option == LT_OPT_BALANCE_CONNECTIVITY) {
+    if (value < 1 || value > t->g.dim) return LT_ERR_ARG;
+    t->opt_balance_conn = value;
+  }
   else return LT_ERR_ARG;
   return LT_OK;
 }

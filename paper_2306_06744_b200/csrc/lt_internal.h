@@ -77,7 +77,7 @@ struct Tree {
   // sort scratch
   uint64_t* sort_tmp; int64_t sort_cap; unsigned* sort_hist; unsigned* sort_status; int64_t sort_status_cap;
 
-  int opt_adapt_sort, opt_full_sweeps, opt_debug_slack, opt_host_slab;
+  int opt_adapt_sort, opt_full_sweeps, opt_debug_slack, opt_host_slab, opt_balance_conn;
   cudaEvent_t ev[16];
   bool ev_set[8];
   int64_t launches;

@@ -296,22 +296,40 @@ struct BalanceArgs {
   DevScalars* s;
   int64_t cap;
   int full_sweeps;
+  // neighbour directions examined per leaf (reading C-9): 2 bits per axis, 0 = no move,
+  // 1 = move across the leaf's parent-EXTERIOR side on that axis, 2 = across the interior side
+  int ndirs;
+  uint8_t dirs[20];
 };
 
-// Only the DIM faces of a leaf that are exterior to its parent are examined: an interior face
-// looks at a sibling's cell, which is tiled by leaves at least as fine as the leaf itself
-// (the parent is subdivided), so it can never meet a coarser neighbour.  The exterior face
-// on axis a is the minus face if bit a of the child id is 0, the plus face otherwise.
+// Face balance examines only the DIM faces of a leaf that are exterior to its parent: an
+// interior face looks at a sibling's cell, which is tiled by leaves at least as fine as the
+// leaf itself (the parent is subdivided), so it can never meet a coarser neighbour.  The
+// exterior side on axis a is the minus side if bit a of the child id is 0, the plus side
+// otherwise.  Strong balance (neighbours across edges, optionally corners) adds
+// the directions that move on two / three axes; a direction whose moves are ALL interior lands
+// inside the parent and is skipped for the same reason, so 3 + 9 (+ 7) directions per leaf are
+// examined in 3-D.  The neighbour key is formed by chaining the one-axis step.
 template <int DIM>
 __device__ __forceinline__ void balance_examine(const Geo& g, const uint64_t* __restrict__ keys,
-                                                const int* __restrict__ first, uint8_t* mark, int i, int a) {
+                                                const int* __restrict__ first, uint8_t* mark, int i, int code) {
   const uint64_t key = keys[i];
   const int l = key_level(key);
   if (l < g.base + 2) return;  // no leaf is coarser than the base level
   const uint64_t m = key_morton(key);
-  const int f = 2 * a + ((child_id<DIM>(g, m, l) >> a) & 1);
-  uint64_t mn;
-  if (!face_neighbour<DIM>(g, m, l, f, &mn)) return;
+  const int cid = child_id<DIM>(g, m, l);
+  uint64_t mn = m;
+#pragma unroll
+  for (int a = 0; a < DIM; ++a) {
+    const int c = (code >> (2 * a)) & 3;
+    if (c) {
+      const int bit = (cid >> a) & 1;
+      const int f = 2 * a + (c == 1 ? bit : (bit ^ 1));
+      uint64_t nx;
+      if (!face_neighbour<DIM>(g, mn, l, f, &nx)) return;
+      mn = nx;
+    }
+  }
   const int j = locate(g, keys, first, mn);
   const int lj = key_level(keys[j]);
   if (lj < l - 1) {
@@ -324,8 +342,11 @@ template <int DIM>
 __global__ void __launch_bounds__(BT) k_balance(BalanceArgs a) {
   constexpr int NC = Dim<DIM>::NC;
   __shared__ unsigned long long sm[33];
+  __shared__ uint8_t s_dirs[20];
   cg::grid_group grid = cg::this_grid();
   const Geo g = a.g;
+  if (threadIdx.x < 20) s_dirs[threadIdx.x] = a.dirs[threadIdx.x];
+  __syncthreads();
   const int64_t gtid = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   const int64_t gsize = (int64_t)gridDim.x * blockDim.x;
   int64_t n = a.s->n;
@@ -337,13 +358,25 @@ __global__ void __launch_bounds__(BT) k_balance(BalanceArgs a) {
     const uint64_t* keys = a.keys[par];
     const int* first = a.first[par];
     // ---- sweep
-    if (nfront < 0) {
-      for (int64_t sidx = gtid; sidx < n * DIM; sidx += gsize)
-        balance_examine<DIM>(g, keys, first, a.mark, (int)(sidx / DIM), (int)(sidx % DIM));
+    if (a.ndirs == DIM) {  // face balance: direction d = the exterior face on axis d
+      if (nfront < 0) {
+        for (int64_t sidx = gtid; sidx < n * DIM; sidx += gsize)
+          balance_examine<DIM>(g, keys, first, a.mark, (int)(sidx / DIM), 1 << (2 * (int)(sidx % DIM)));
+      } else {
+        const int* fr = a.frontier[fpar];
+        for (int64_t sidx = gtid; sidx < nfront * DIM; sidx += gsize)
+          balance_examine<DIM>(g, keys, first, a.mark, fr[sidx / DIM], 1 << (2 * (int)(sidx % DIM)));
+      }
     } else {
-      const int* fr = a.frontier[fpar];
-      for (int64_t sidx = gtid; sidx < nfront * DIM; sidx += gsize)
-        balance_examine<DIM>(g, keys, first, a.mark, fr[sidx / DIM], (int)(sidx % DIM));
+      const int nd = a.ndirs;
+      if (nfront < 0) {
+        for (int64_t sidx = gtid; sidx < n * nd; sidx += gsize)
+          balance_examine<DIM>(g, keys, first, a.mark, (int)(sidx / nd), s_dirs[sidx % nd]);
+      } else {
+        const int* fr = a.frontier[fpar];
+        for (int64_t sidx = gtid; sidx < nfront * nd; sidx += gsize)
+          balance_examine<DIM>(g, keys, first, a.mark, fr[sidx / nd], s_dirs[sidx % nd]);
+      }
     }
     grid.sync();
     // ---- count: low 32 = leaves out, high 32 = frontier entries out
@@ -504,6 +537,21 @@ int launch_balance(Tree* t, int64_t cap_told) {
   a.s = t->d_s;
   a.cap = cap_told;
   a.full_sweeps = t->opt_full_sweeps;
+  // directions: per axis none / exterior / interior, at least one exterior move, at most
+  // `conn` moves (conn 1: the dim exterior faces, in axis order)
+  const int conn = t->opt_balance_conn > 0 ? t->opt_balance_conn : 1;
+  a.ndirs = 0;
+  for (int moves = 1; moves <= conn; ++moves)
+    for (int code = 1; code < (1 << (2 * t->g.dim)); ++code) {
+      int nz = 0, ext = 0, bad = 0;
+      for (int ax = 0; ax < t->g.dim; ++ax) {
+        const int c = (code >> (2 * ax)) & 3;
+        if (c == 3) bad = 1;
+        nz += c != 0;
+        ext += c == 1;
+      }
+      if (!bad && nz == moves && ext >= 1) a.dirs[a.ndirs++] = (uint8_t)code;
+    }
   void* fn = t->g.dim == 2 ? (void*)k_balance<2> : (void*)k_balance<3>;
   int per_sm = 0;
   LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, BT, 0));

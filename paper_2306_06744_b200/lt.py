@@ -21,6 +21,7 @@ _lib = None
 LT_OK, LT_ERR_ARG, LT_ERR_CUDA, LT_ERR_OOM, LT_ERR_CAPACITY = 0, -1, -2, -3, -4
 LT_ERR_UNBALANCED, LT_ERR_MAPPING, LT_ERR_INCOMPLETE = -5, -6, -7
 LT_OPT_ADAPT_SORT, LT_OPT_BALANCE_FULL_SWEEPS, LT_OPT_DEBUG_BALANCE_SLACK = 1, 2, 3
+LT_OPT_HOST_SLAB_LEAVES, LT_OPT_BALANCE_CONNECTIVITY = 4, 5
 
 
 class LtError(RuntimeError):
@@ -176,7 +177,11 @@ class Tree:
             raise ValueError("lt_adapt: flags must have one entry per leaf")
         _check(lib().lt_adapt(self._h, _dptr(flags, torch.int8, "flags")), "lt_adapt")
 
-    def balance(self) -> int:
+    def balance(self, connectivity=None) -> int:
+        """lt_balance; connectivity (sticky option LT_OPT_BALANCE_CONNECTIVITY): 1 faces,
+        2 + edges (the paper's strong balance in 3-D), 3 + corners."""
+        if connectivity is not None:
+            self.set_option(LT_OPT_BALANCE_CONNECTIVITY, int(connectivity))
         it = C.c_int(0)
         _check(lib().lt_balance(self._h, C.byref(it)), "lt_balance")
         return it.value
