@@ -99,6 +99,12 @@ def lib():
         L.lto_drop_snapshot.argtypes = [C.c_void_p]
         L.lto_operators.restype = C.c_int
         L.lto_operators.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_double)]
+        L.lto_mortar_project.restype = C.c_int
+        L.lto_mortar_project.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_int, C.c_int]
+        L.lto_mortar_gather.restype = C.c_int
+        L.lto_mortar_gather.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_int, C.c_int]
+        L.lto_face_operators.restype = C.c_int
+        L.lto_face_operators.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_double)]
         L.lto_gauss_legendre.restype = None
         L.lto_gauss_legendre.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         _lib = L
@@ -154,6 +160,19 @@ def operators(dim, p):
         assert rc == 0
         out[name] = a
     return out
+
+
+def face_operators(dim, p):
+    """(to_mortar [ns,N,N] of Eq. 17, from_mortar [ns,N,N] = M^-1 S^s of Eq. 20) for the
+    (dim-1)-dimensional faces; ns = 2^(dim-1), N = (p+1)^(dim-1)."""
+    ns, N = 1 << (dim - 1), (p + 1) ** (dim - 1)
+    out = []
+    for which in (0, 1):
+        a = np.zeros((ns, N, N))
+        if lib().lto_face_operators(dim, p, which, _p(a, C.c_double)) != 0:
+            raise OracleError("oracle face operators: bad arguments")
+        out.append(a)
+    return tuple(out)
 
 
 class OracleError(RuntimeError):
@@ -286,6 +305,30 @@ class Tree:
         self.build_map()
         out = self.transfer_rows(u_old, p, nvars, 0, self.num_leaves())
         lib().lto_drop_snapshot(self._h)
+        return out
+
+    def mortar_project(self, u_face, p, nvars):
+        """Alg. 8 step 2: u_face [M, nf, nvars, Nf] -> neighbour traces on kind 1 / 2 slots
+        (other slots are returned as NaN)."""
+        Nf = (p + 1) ** (self.dim - 1)
+        uf = np.ascontiguousarray(u_face, dtype=np.float64)
+        assert uf.shape == (self.num_leaves(), self.nf, nvars, Nf)
+        out = np.full(uf.shape, np.nan)
+        rc = lib().lto_mortar_project(self._h, _p(uf, C.c_double), _p(out, C.c_double), p, nvars)
+        if rc != 0:
+            raise OracleError("oracle mortar_project: rc=%d (connect first)" % rc)
+        return out
+
+    def mortar_gather(self, f_mortar, p, nvars):
+        """Alg. 8 step 4: f_mortar [M, nf, nvars, Nf] -> coarse-face fluxes on kind 3 slots
+        (other slots are returned as NaN)."""
+        Nf = (p + 1) ** (self.dim - 1)
+        fm = np.ascontiguousarray(f_mortar, dtype=np.float64)
+        assert fm.shape == (self.num_leaves(), self.nf, nvars, Nf)
+        out = np.full(fm.shape, np.nan)
+        rc = lib().lto_mortar_gather(self._h, _p(fm, C.c_double), _p(out, C.c_double), p, nvars)
+        if rc != 0:
+            raise OracleError("oracle mortar_gather: rc=%d" % rc)
         return out
 
     def drop_snapshot(self):

@@ -616,10 +616,9 @@ void solve_dense(std::vector<double> A, int n, std::vector<double>& B, int m) {
 //  M, S_c    : Eq. 13 by (p+6)-point tensor Gauss quadrature, S_c integrated over
 //              child c's region (reading E-3)
 //  proj[c]   = M^{-1} S_c by dense Gaussian elimination               (Eq. 12)
-void build_ops(Tree* t, int p) {
-  Ops& o = t->ops;
-  if (o.p == p && o.dim == t->dim) return;
-  const int dim = t->dim, nc = t->nc, P1 = p + 1;
+void build_ops_dim(Ops& o, int dim, int p) {
+  if (o.p == p && o.dim == dim) return;
+  const int nc = 1 << dim, P1 = p + 1;
   int N = 1;
   for (int a = 0; a < dim; ++a) N *= P1;
   o.dim = dim; o.p = p; o.N = N;
@@ -688,6 +687,8 @@ void build_ops(Tree* t, int p) {
     std::copy(B.begin(), B.end(), o.proj.begin() + (size_t)c * N * N);
   }
 }
+
+void build_ops(Tree* t, int p) { build_ops_dim(t->ops, t->dim, p); }
 
 // u[e][v][n] (reading E-5).  Rows [j0, j1) of the new tree are produced.
 void transfer_rows(Tree* t, const double* u_old, double* u_new_rows, int nvars, int64_t j0, int64_t j1) {
@@ -809,6 +810,134 @@ uint32_t point_cell(double x, double lo, double hi, int maxl) {
   if (!(v >= 0.0)) v = 0.0;  // also catches NaN
   if (v > top) v = top;
   return (uint32_t)v;
+}
+
+
+// ---------------------------------------------------------------- Alg. 8 (mortars)
+// Common-flux plumbing on nonconforming faces, PAPER.md:265-314 (section 4.3, Alg. 8 steps
+// 2 and 4, Eq. 14-20); readings H-1..H-4 of DESIGN.md.
+//  face points : the (p+1)^(dim-1) Gauss-Legendre points of the face, tangential axes in
+//                ascending order, lower axis fastest; N = (k+1)^(dim-1) (Eq. 14)      (H-1)
+//  mortars     : the 2^(dim-1) mortar faces of a coarse face coincide with the fine
+//                neighbours' faces, mortar s = slot s of lt_connect (fine side <-> mortar
+//                is "a direct copy", :273)                                              (H-2)
+//  Eq. 17      : M^ u^ = S u,  M^_ji = int_Xi l^_j l^_i dz,  S_ji = int_Xi l^_j l_i(xi(z)) dz
+//  Eq. 20      : M F = sum_s S^s F^s,  M_ji = int_Oc l_j l_i dxi,  S^s_ji = int_Oc^s l_j l^_i dxi
+//                (the sum runs over the 2^(dim-1) mortars; "2^dim - 1" at :310 is a typo) (H-3)
+// All integrals by (p+6)-point tensor Gauss quadrature, systems solved densely.
+struct FaceOps {
+  int fdim = -1, p = -1, N = 0;
+  Ops coarse;                  // operators of the (dim-1)-dimensional face: .proj[s] = M^-1 S^s (Eq. 20)
+  std::vector<double> to_mortar;  // [ns][N][N]  (M^)^-1 S of Eq. 17 for mortar s
+};
+
+void build_face_ops(FaceOps& fo, int dim, int p) {
+  const int fdim = dim - 1;
+  if (fo.fdim == fdim && fo.p == p) return;
+  build_ops_dim(fo.coarse, fdim, p);
+  const int P1 = p + 1, ns = 1 << fdim, Q = p + 6;
+  int N = 1, NQ = 1;
+  for (int a = 0; a < fdim; ++a) { N *= P1; NQ *= Q; }
+  fo.fdim = fdim; fo.p = p; fo.N = N;
+  std::vector<double> z, w, qz, qw;
+  gauss_legendre(P1, z, w);
+  gauss_legendre(Q, qz, qw);
+  fo.to_mortar.assign((size_t)ns * N * N, 0.0);
+  for (int s = 0; s < ns; ++s) {
+    std::vector<double> Mh((size_t)N * N, 0.0), Sh((size_t)N * N, 0.0);
+    for (int q = 0; q < NQ; ++q) {
+      double zeta[3] = {0, 0, 0}, xi[3] = {0, 0, 0}, wq = 1.0;  // zeta: mortar coordinates, xi: coarse-face coordinates
+      int r = q;
+      for (int a = 0; a < fdim; ++a) {
+        const int b = (s >> a) & 1;
+        zeta[a] = qz[r % Q];
+        xi[a] = 0.5 * (zeta[a] + 2.0 * b - 1.0);
+        wq *= qw[r % Q];
+        r /= Q;
+      }
+      std::vector<double> lh(N), lc(N);
+      for (int n = 0; n < N; ++n) {
+        lh[n] = tensor_lagrange(z, fdim, n, zeta);
+        lc[n] = tensor_lagrange(z, fdim, n, xi);
+      }
+      for (int j = 0; j < N; ++j)
+        for (int i = 0; i < N; ++i) {
+          Mh[(size_t)j * N + i] += wq * lh[j] * lh[i];
+          Sh[(size_t)j * N + i] += wq * lh[j] * lc[i];
+        }
+    }
+    solve_dense(Mh, N, Sh, N);
+    std::copy(Sh.begin(), Sh.end(), fo.to_mortar.begin() + (size_t)s * N * N);
+  }
+}
+
+// Alg. 8 step 2 for every face slot (e, f); face arrays are [n_leaves][nf][nvars][N] (H-4):
+//   kind 1 (conforming):        u_nb[e][f] = u_f[nbr][f^1]                   (copy)
+//   kind 2 (neighbour coarser): u_nb[e][f] = (M^)^-1 S u_f[nbr][f^1] for mortar `slot` (Eq. 17)
+//   kind 0 / 3:                 left untouched
+void mortar_project(Tree* t, const FaceOps& fo, const double* uf, double* unb, int nvars) {
+  const int nf = t->nf, N = fo.N;
+  const size_t E = (size_t)nvars * N;
+  const int64_t M = (int64_t)t->leaves.size();
+  for (int64_t e = 0; e < M; ++e)
+    for (int f = 0; f < nf; ++f) {
+      const size_t sl = (size_t)e * nf + f;
+      const int kd = t->faces.kind[sl] & 15, slot = t->faces.kind[sl] >> 4;
+      if (kd != 1 && kd != 2) continue;
+      const double* src = uf + ((size_t)t->faces.nbr[sl] * nf + (f ^ 1)) * E;
+      double* dst = unb + sl * E;
+      for (int v = 0; v < nvars; ++v)
+        for (int n = 0; n < N; ++n) {
+          if (kd == 1) {
+            dst[(size_t)v * N + n] = src[(size_t)v * N + n];
+          } else {
+            double acc = 0.0;
+            for (int m = 0; m < N; ++m) acc += fo.to_mortar[((size_t)slot * N + n) * N + m] * src[(size_t)v * N + m];
+            dst[(size_t)v * N + n] = acc;
+          }
+        }
+    }
+}
+
+// Alg. 8 step 4 for every coarse face slot (kind 3): F[e][f] = M^-1 sum_s S^s F^[e_s][f^1]
+// (Eq. 20), e_s = the fine neighbour occupying mortar s.  Other slots are left untouched.
+// Returns -1 if a fine neighbour is missing (tree not balanced).
+int mortar_gather(Tree* t, const FaceOps& fo, const double* fm, double* ff, int nvars) {
+  const int nf = t->nf, N = fo.N, ns = 1 << (t->dim - 1);
+  const size_t E = (size_t)nvars * N;
+  const int64_t M = (int64_t)t->leaves.size();
+  for (int64_t e = 0; e < M; ++e)
+    for (int f = 0; f < nf; ++f) {
+      const size_t sl = (size_t)e * nf + f;
+      if ((t->faces.kind[sl] & 15) != 3) continue;
+      Node* L = t->leaves[e];
+      uint32_t nx[3];
+      if (!neighbour_anchor(t, L, f, nx)) return -1;
+      Node* Nn = locate(t, t->root, nx, L->level);
+      if (Nn->is_leaf() || Nn->level != L->level) return -1;
+      const int axis = f >> 1;
+      std::vector<double> acc(E, 0.0);
+      for (int s = 0; s < ns; ++s) {
+        // the child of the neighbour cell that touches the face and sits at tangential position s
+        int c = (f & 1) ? 0 : (1 << axis), bit = 0;
+        for (int a = 0; a < t->dim; ++a) {
+          if (a == axis) continue;
+          c |= ((s >> bit) & 1) << a;
+          ++bit;
+        }
+        Node* F = Nn->child[c];
+        if (!F->is_leaf()) return -1;
+        const double* src = fm + ((size_t)F->idx * nf + (f ^ 1)) * E;
+        for (int v = 0; v < nvars; ++v)
+          for (int n = 0; n < N; ++n) {
+            double a2 = 0.0;
+            for (int m = 0; m < N; ++m) a2 += fo.coarse.proj[((size_t)s * N + n) * N + m] * src[(size_t)v * N + m];
+            acc[(size_t)v * N + n] += a2;
+          }
+      }
+      std::copy(acc.begin(), acc.end(), ff + sl * E);
+    }
+  return 0;
 }
 
 }  // namespace
@@ -1023,6 +1152,31 @@ int lto_operators(int dim, int p, int which, double* out) {
   std::memcpy(out, v->data(), v->size() * sizeof(double));
   free_subtree(t->root);
   delete t;
+  return 0;
+}
+// Alg. 8 steps 2 / 4 on the face arrays [n_leaves][nf][nvars][(p+1)^(dim-1)]; lto_connect
+// must have run on the current tree.  which = 0: to_mortar (Eq. 17), 1: M^-1 S^s (Eq. 20).
+int lto_mortar_project(void* h, const double* uf, double* unb, int p, int nvars) {
+  Tree* t = (Tree*)h;
+  if (t->faces.kind.size() != t->leaves.size() * (size_t)t->nf) return -2;
+  FaceOps fo;
+  build_face_ops(fo, t->dim, p);
+  mortar_project(t, fo, uf, unb, nvars);
+  return 0;
+}
+int lto_mortar_gather(void* h, const double* fm, double* ff, int p, int nvars) {
+  Tree* t = (Tree*)h;
+  if (t->faces.kind.size() != t->leaves.size() * (size_t)t->nf) return -2;
+  FaceOps fo;
+  build_face_ops(fo, t->dim, p);
+  return mortar_gather(t, fo, fm, ff, nvars);
+}
+int lto_face_operators(int dim, int p, int which, double* out) {
+  if (dim != 2 && dim != 3) return -1;
+  FaceOps fo;
+  build_face_ops(fo, dim, p);
+  const std::vector<double>& v = which == 0 ? fo.to_mortar : fo.coarse.proj;
+  std::memcpy(out, v.data(), v.size() * sizeof(double));
   return 0;
 }
 void lto_gauss_legendre(int n, double* z, double* w) {
