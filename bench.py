@@ -577,6 +577,98 @@ def run_construct(args):
     print(json.dumps(out), flush=True)
 
 
+# --------------------------------------------------------------------------- mortar leg
+def run_mortar(args):
+    """--workload mortar: SURVEY.md 8(f)-2.  A step = lt_mortar_project + lt_mortar_gather over
+    the face arrays [M][6][5][16] (p = 3, 5 fp64 variables) of the config-5 mesh after cycles
+    0-2 (8.86 M leaves, 34 GB per face array)."""
+    import torch
+    from paper_2306_06744_b200 import build as B
+    B.build()
+    from paper_2306_06744_b200 import workloads as W
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    cfg = W.CONFIGS["c5"]
+    R = Runner(cfg, dev)
+    M = R.prepare()
+    t = R.tree
+    F = t.connect()
+    kind = F["kind"] & 15
+    n1, n2, n3 = int((kind == 1).sum()), int((kind == 2).sum()), int((kind == 3).sum())
+    p, nvars, nf = cfg["p"], cfg["nvars"], 6
+    Nf = (p + 1) ** 2
+    Bf = 8 * nvars * Nf
+    uf = torch.empty((M, nf, nvars, Nf), dtype=torch.float64, device=dev)
+    step = 1 << 19
+    for a in range(0, M, step):  # seeded face data, slab by slab
+        b = min(a + step, M)
+        i = torch.arange(a * nf * nvars * Nf, b * nf * nvars * Nf, dtype=torch.int64, device=dev)
+        uf[a:b] = (2.0 * W.counter_uniform(5, 21, i) - 1.0).view(b - a, nf, nvars, Nf)
+        del i
+    out = torch.empty_like(uf)
+    stream = torch.cuda.current_stream(dev)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+
+    def step_once():
+        torch.cuda.synchronize(dev)
+        ev[0].record(stream)
+        t.mortar_project(uf, p, nvars, u_nb=out)
+        ev[1].record(stream)
+        t.mortar_gather(uf, p, nvars, f_face=out)
+        ev[2].record(stream)
+        torch.cuda.synchronize(dev)
+        t.sync()
+        return ev[0].elapsed_time(ev[1]), ev[1].elapsed_time(ev[2])
+
+    for _ in range(max(args.warmup, 0)):
+        step_once()
+    sampler = ClockSampler(0)
+    sampler.start()
+    times = [step_once() for _ in range(args.steps)]
+    clocks = sampler.stop()
+    ms_p = sum(a for a, _ in times) / args.steps
+    ms_g = sum(b for _, b in times) / args.steps
+    bytes_p = 2 * Bf * (n1 + n2) + 5 * nf * M
+    bytes_g = Bf * (n2 + n3) + (nf + 8) * M
+    peak, peak_src = hbm_peak()
+    ach = bytes_p / (ms_p * 1e-3) / 1e9
+    cpu = None
+    if not args.no_cpu_baseline:
+        import numpy as np
+        import oracle
+        ot = oracle.Tree(cfg["dim"], cfg["base"], cfg["maxl"], cfg["periodic"])
+        lvl, xyz = ot.leaf_boxes()
+        ot.adapt(W.flags(cfg, 0, torch.from_numpy(lvl), torch.from_numpy(xyz.astype(np.int64))).numpy())
+        ot.balance()
+        ot.connect()
+        h = np.random.default_rng(0).uniform(-1, 1, (ot.num_leaves(), nf, nvars, Nf))
+        t0 = time.perf_counter()
+        ot.mortar_project(h, p, nvars)
+        ot.mortar_gather(h, p, nvars)
+        dt = time.perf_counter() - t0
+        cpu = {"value": ot.num_leaves() * nf / dt, "unit": "face slots/s", "cores": 1, "kind": "oracle", "seconds": dt,
+               "sample": "config-5 mesh after cycle 0 (%d leaves): project + gather" % ot.num_leaves()}
+    print(json.dumps({
+        "metric": "face slots/s through lt_mortar_project + lt_mortar_gather (Alg. 8 steps 2 and 4)",
+        "value": M * nf / ((ms_p + ms_g) * 1e-3), "unit": "face slots/s", "n_gpus": 1, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_p + ms_g, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "mortar: config-5 mesh after cycles 0-2 (%d leaves; %d conforming, %d fine-side and %d "
+                               "coarse-side hanging face slots), p=3, 5 fp64 vars, face arrays [M][6][5][16]"
+                               % (M, n1, n2, n3),
+                   "l2": "face arrays of %.1f GB each, larger than L2" % (uf.numel() * 8 / 1e9)},
+        "ms_per_call": {"mortar_project": ms_p, "mortar_gather": ms_g},
+        "roofline": {"bound": "hbm", "kernel": "k_mortar_project<3>", "achieved": ach, "peak": peak, "unit": "GB/s",
+                     "frac": ach / peak, "traffic": None, "peak_source": peak_src, "bytes_per_launch": bytes_p,
+                     "gather_GBps": bytes_g / (ms_g * 1e-3) / 1e9, "gather_bytes_per_launch": bytes_g},
+        "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": 2 * args.steps,
+        "e2e": None}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -585,7 +677,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--workload", default="cycle", choices=["cycle", "construct"],
+    ap.add_argument("--workload", default="cycle", choices=["cycle", "construct", "mortar"],
                     help="cycle (default): the adaptation cycle BASELINE.json's metric is quoted on; construct: "
                          "tree construction from a point cloud (SURVEY.md 8(f)-1)")
     ap.add_argument("--cloud", default="pc10", help="point cloud of --workload construct (workloads.POINT_CLOUDS)")
@@ -607,6 +699,8 @@ def main():
         args.steps = 1
     if args.workload == "construct" and args.impl == "ours":
         run_construct(args)
+    elif args.workload == "mortar" and args.impl == "ours":
+        run_mortar(args)
     elif args.impl == "reference":
         run_reference(args)
     else:

@@ -176,6 +176,29 @@ int lt_transfer(lt_tree*, const double* d_u_old, double* d_u_new, int p, int nva
  * (owned by the tree).  Synchronises. */
 int lt_transfer_host(lt_tree*, const double* h_u_old, double* h_u_new, int p, int nvars);
 
+/* ---- mortars on nonconforming faces (Alg. 8 steps 2 and 4) -------------
+ * Face arrays: device fp64 [lt_num_leaves][nf][nvars][Nf], Nf = (p+1)^(dim-1) Gauss-Legendre
+ * face points, tangential axes in ascending order, lower axis fastest (readings H-1, H-4).
+ * The 2^(dim-1) mortars of a coarse face coincide with the faces of its fine neighbours
+ * (mortar s = slot s of lt_connect; fine side <-> mortar is "a direct copy"),
+ * so mortar data lives in the fine element's face slot.  Both calls need lt_connect on the
+ * current tree (LT_ERR_ARG otherwise), 0 <= p <= 7, nvars >= 1.  Asynchronous.
+ *
+ * lt_mortar_project -- step 2, Eq. 14-17: for every face slot (e, f) the neighbour's trace as
+ * seen from e:   kind 1: d_u_nb[e][f] = d_u_face[nbr][f^1]  (conforming, copy);
+ *                kind 2: d_u_nb[e][f] = L2 projection of the coarse trace d_u_face[nbr][f^1]
+ *                        onto mortar `slot` (Eq. 17);   kind 0 / 3: left untouched.
+ * The arrays must not overlap.
+ *
+ * lt_mortar_gather -- step 4, Eq. 18-20: for every coarse face slot (kind 3)
+ *   d_f_face[e][f] = M^-1 sum_s S^s d_f_mortar[e_s][f^1],  e_s = the fine neighbour on mortar s;
+ * other slots are left untouched, so d_f_face may be d_f_mortar itself (in place).  The paper
+ * scatters these contributions with atomicAdd; here each coarse face gathers its
+ * mortars, which makes the result deterministic.  A missing fine neighbour sets the sticky
+ * status LT_ERR_UNBALANCED (reported by lt_sync). */
+int lt_mortar_project(lt_tree*, const double* d_u_face, double* d_u_nb, int p, int nvars);
+int lt_mortar_gather(lt_tree*, const double* d_f_mortar, double* d_f_face, int p, int nvars);
+
 /* ---- accessors --------------------------------------------------------------------- */
 
 int64_t lt_num_leaves(lt_tree*);       /* synchronises only if the count is not cached   */
@@ -229,7 +252,7 @@ int lt_set_option(lt_tree*, int option, int value);
 /* Device times of the last cycle in milliseconds (CUDA events on the tree's stream):
  * out[0..3] = the calls lt_adapt, lt_balance, lt_connect, lt_transfer; out[4] = the Alg. 7
  * map kernel alone, out[5] = the solution-transfer kernel alone, out[6] = the connectivity
- * kernel alone, out[7] = reserved (0); 0 where not run.
+ * kernel alone, out[7] = the last mortar kernel (lt_mortar_project / lt_mortar_gather); 0 where not run.
  * Synchronises. */
 int lt_timings(lt_tree*, float* out8);
 /* Number of kernels liblt launched on this tree since it was built. */

@@ -122,6 +122,7 @@ static int grow(Tree* t, int64_t need) {
   free_dev(t->stream, t->face_bytes); t->face_bytes = fbytes;
   free_dev(t->stream, t->tile_state); t->tile_state = tstate;
   t->map_valid = false;
+  t->faces_valid = false;
   t->cap = cap;
   return LT_OK;
 }
@@ -468,6 +469,7 @@ int lt_adapt(lt_tree* t, const int8_t* d_flags) {
   t->n_old = n_in;
   t->n_valid = true;
   t->map_valid = false;
+  t->faces_valid = false;
   toc(t, 0);
   return LT_OK;
 }
@@ -506,6 +508,7 @@ int lt_balance(lt_tree* t, int* iters) {
   }
   if (iters) *iters = total_iters;
   t->map_valid = false;
+  t->faces_valid = false;
   toc(t, 1);
   return LT_OK;
 }
@@ -541,7 +544,29 @@ int lt_connect(lt_tree* t, lt_faces* out) {
     out->bnd_face = bnd_face;
   }
   toc(t, 2);
+  t->faces_valid = true;
   return LT_OK;
+}
+
+// ---------------------------------------------------------------------------- mortars
+static int mortar_call(lt_tree* t, int which, const double* d_in, double* d_out, int p, int nvars) {
+  if (!t || !d_in || !d_out || p < 0 || p > 7 || nvars < 1) return LT_ERR_ARG;
+  if (!t->faces_valid) return LT_ERR_ARG;  // lt_connect must describe the current tree
+  int rc;
+  if ((rc = build_operators(t, p)) != LT_OK) return rc;
+  tic(t, 7);
+  if ((rc = launch_mortar(t, which, d_in, d_out, p, nvars)) != LT_OK) return rc;
+  toc(t, 7);
+  return LT_OK;
+}
+
+int lt_mortar_project(lt_tree* t, const double* d_u_face, double* d_u_nb, int p, int nvars) {
+  if (d_u_face == d_u_nb) return LT_ERR_ARG;
+  return mortar_call(t, 0, d_u_face, d_u_nb, p, nvars);
+}
+
+int lt_mortar_gather(lt_tree* t, const double* d_f_mortar, double* d_f_face, int p, int nvars) {
+  return mortar_call(t, 1, d_f_mortar, d_f_face, p, nvars);
 }
 
 // ---------------------------------------------------------------------------- transfer

@@ -549,6 +549,153 @@ int build_operators(Tree* t, int p) {
   return LT_OK;
 }
 
+// ------------------------------------------------------------------------ mortars (Alg. 8)
+// Common-flux plumbing on nonconforming faces, PAPER.md:265-314 (Alg. 8 steps 2 and 4,
+// Eq. 14-20; readings H-1..H-4).  Face arrays are [n_leaves][nf][nvars][Nf], Nf =
+// (p+1)^(dim-1) Gauss-Legendre face points, tangential axes ascending, lower axis fastest.
+// The 2^(dim-1) mortars of a coarse face coincide with the fine neighbours' faces (mortar s
+// = slot s of lt_connect), so with Gauss-Legendre points the Eq. 17 projection onto mortar s
+// is the tensor product of the 1-D interpolations I^b and the Eq. 20 projection back is the
+// tensor product of R^b = (1/2) W^-1 (I^b)^T W -- the same 1-D operators as the volume
+// transfer, one dimension lower.  One warp per leaf; both kernels stream the face arrays
+// once, coalesced, and are HBM-bound.  The paper scatters Eq. 20 with atomicAdd;
+// here the coarse face GATHERS its mortars (found by 2^(dim-1) bucketed searches), so the
+// result is deterministic.
+__device__ __forceinline__ void load_ops_1d(int P1, double (*sI)[8][8], double (*sR)[8][8]) {
+  for (int i = threadIdx.x; i < 2 * 64; i += blockDim.x) {
+    const int b = i >> 6, r = (i >> 3) & 7, c = i & 7;
+    sI[b][r][c] = c_ops[P1 - 1][b][r][c];
+    sR[b][r][c] = c_ops[P1 - 1][2 + b][r][c];
+  }
+  __syncthreads();
+}
+
+template <int DIM>
+__global__ void __launch_bounds__(256) k_mortar_project(const DevScalars* s, const int32_t* __restrict__ nbr,
+                                                        const uint8_t* __restrict__ kind,
+                                                        const double* __restrict__ uf, double* __restrict__ unb,
+                                                        int P1, int nvars) {
+  constexpr int NF = Dim<DIM>::NF;
+  __shared__ double sI[2][8][8], sR[2][8][8];
+  load_ops_1d(P1, sI, sR);
+  const int Nf = DIM == 2 ? P1 : P1 * P1, E = nvars * Nf;
+  const int lane = threadIdx.x & 31;
+  const int64_t n = s->n;
+  const int64_t nw = (int64_t)gridDim.x * (blockDim.x >> 5);
+  for (int64_t e = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); e < n; e += nw) {
+    for (int r = lane; r < NF * E; r += 32) {
+      const int f = r / E, q = r - f * E;
+      const size_t sl = (size_t)e * NF + f;
+      const int kd = kind[sl], k = kd & 15;
+      if (k != 1 && k != 2) continue;
+      const double* src = uf + ((size_t)nbr[sl] * NF + (f ^ 1)) * E;
+      double out;
+      if (k == 1) {
+        out = src[q];  // conforming: the mortar is the face itself
+      } else {
+        const int slot = kd >> 4, v = q / Nf, nn = q - v * Nf;
+        src += (size_t)v * Nf;
+        out = 0.0;
+        if (DIM == 2) {
+          for (int m = 0; m < P1; ++m) out += sI[slot & 1][nn][m] * src[m];
+        } else {
+          const int n1 = nn / P1, n0 = nn - n1 * P1;
+          for (int m1 = 0; m1 < P1; ++m1) {
+            double row = 0.0;
+            for (int m0 = 0; m0 < P1; ++m0) row += sI[slot & 1][n0][m0] * src[m1 * P1 + m0];
+            out += sI[slot >> 1][n1][m1] * row;
+          }
+        }
+      }
+      unb[sl * E + q] = out;
+    }
+  }
+}
+
+template <int DIM>
+__global__ void __launch_bounds__(256) k_mortar_gather(Geo g, const uint64_t* __restrict__ keys,
+                                                       const int* __restrict__ first, DevScalars* s,
+                                                       const uint8_t* __restrict__ kind,
+                                                       const double* __restrict__ fm, double* __restrict__ ff, int P1,
+                                                       int nvars) {
+  constexpr int NF = Dim<DIM>::NF, NS = 1 << (DIM - 1);
+  __shared__ double sI[2][8][8], sR[2][8][8];
+  load_ops_1d(P1, sI, sR);
+  const int Nf = DIM == 2 ? P1 : P1 * P1, E = nvars * Nf;
+  const int lane = threadIdx.x & 31;
+  const int64_t n = s->n;
+  const int64_t nw = (int64_t)gridDim.x * (blockDim.x >> 5);
+  for (int64_t e = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); e < n; e += nw) {
+    const uint64_t key = keys[e];
+    const int l = key_level(key);
+    const uint64_t m = key_morton(key);
+    for (int f = 0; f < NF; ++f) {
+      const size_t sl = (size_t)e * NF + f;
+      if ((kind[sl] & 15) != 3) continue;  // warp-uniform
+      // lane s < NS finds the fine neighbour on mortar s: the child of the same-level neighbour
+      // cell that touches the face, tangential child bits = s (ascending axis order)
+      const int axis = f >> 1;
+      uint64_t mn = 0;
+      face_neighbour<DIM>(g, m, l, f, &mn);
+      int es = 0;
+      if (lane < NS) {
+        int c = (f & 1) ? 0 : (1 << axis), bit = 0;
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+          if (a == axis) continue;
+          c |= ((lane >> bit) & 1) << a;
+          ++bit;
+        }
+        es = locate(g, keys, first, mn | ((uint64_t)c << (DIM * (g.maxl - l - 1))));
+        if (key_level(keys[es]) != l + 1) set_status(&s->status, LT_ERR_UNBALANCED);
+      }
+      int e_of[NS];
+#pragma unroll
+      for (int sidx = 0; sidx < NS; ++sidx) e_of[sidx] = __shfl_sync(0xffffffffu, es, sidx);
+      for (int q = lane; q < E; q += 32) {
+        const int v = q / Nf, nn = q - v * Nf;
+        double acc = 0.0;
+#pragma unroll
+        for (int sidx = 0; sidx < NS; ++sidx) {
+          const double* src = fm + ((size_t)e_of[sidx] * NF + (f ^ 1)) * E + (size_t)v * Nf;
+          if (DIM == 2) {
+            for (int mm = 0; mm < P1; ++mm) acc += sR[sidx & 1][nn][mm] * src[mm];
+          } else {
+            const int n1 = nn / P1, n0 = nn - n1 * P1;
+            for (int m1 = 0; m1 < P1; ++m1) {
+              double row = 0.0;
+              for (int m0 = 0; m0 < P1; ++m0) row += sR[sidx & 1][n0][m0] * src[m1 * P1 + m0];
+              acc += sR[sidx >> 1][n1][m1] * row;
+            }
+          }
+        }
+        ff[sl * E + q] = acc;
+      }
+    }
+  }
+}
+
+int launch_mortar(Tree* t, int which, const double* d_in, double* d_out, int p, int nvars) {
+  const int G = t->num_sms * 8;
+  const int P1 = p + 1;
+  if (which == 0) {
+    if (t->g.dim == 2)
+      k_mortar_project<2><<<G, 256, 0, t->stream>>>(t->d_s, t->nbr, t->kind, d_in, d_out, P1, nvars);
+    else
+      k_mortar_project<3><<<G, 256, 0, t->stream>>>(t->d_s, t->nbr, t->kind, d_in, d_out, P1, nvars);
+  } else {
+    if (t->g.dim == 2)
+      k_mortar_gather<2><<<G, 256, 0, t->stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->kind, d_in,
+                                                   d_out, P1, nvars);
+    else
+      k_mortar_gather<3><<<G, 256, 0, t->stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->kind, d_in,
+                                                   d_out, P1, nvars);
+  }
+  t->launches++;
+  LT_CUDA(cudaGetLastError());
+  return LT_OK;
+}
+
 int launch_map(Tree* t) {
   int G = grid_for(t, 8);
   if (!t->have_old) {

@@ -52,6 +52,8 @@ SIGNATURES = {
     "lt_connect": (_I, [_P, C.POINTER(lt_faces)]),
     "lt_transfer": (_I, [_P, _P, _P, _I, _I]),
     "lt_transfer_host": (_I, [_P, _P, _P, _I, _I]),
+    "lt_mortar_project": (_I, [_P, _P, _P, _I, _I]),
+    "lt_mortar_gather": (_I, [_P, _P, _P, _I, _I]),
     "lt_num_leaves": (_I64, [_P]),
     "lt_num_old_leaves": (_I64, [_P]),
     "lt_keys": (_P, [_P]),
@@ -214,6 +216,31 @@ class Tree:
                                  p, nvars), "lt_transfer")
         return u_new
 
+    def _face_shape(self, p, nvars):
+        return (self.num_leaves(), self.nf, nvars, (p + 1) ** (self.dim - 1))
+
+    def mortar_project(self, u_face: torch.Tensor, p: int, nvars: int, u_nb: torch.Tensor = None) -> torch.Tensor:
+        """lt_mortar_project (Alg. 8 step 2): u_face [M, nf, nvars, Nf] -> neighbour traces; slots
+        of kind 0 / 3 keep what u_nb held (NaN when it is allocated here)."""
+        if tuple(u_face.shape) != self._face_shape(p, nvars):
+            raise ValueError("lt_mortar_project: u_face must be %s" % (self._face_shape(p, nvars),))
+        if u_nb is None:
+            u_nb = torch.full_like(u_face, float("nan"))
+        _check(lib().lt_mortar_project(self._h, _dptr(u_face, torch.float64, "u_face"),
+                                       _dptr(u_nb, torch.float64, "u_nb"), p, nvars), "lt_mortar_project")
+        return u_nb
+
+    def mortar_gather(self, f_mortar: torch.Tensor, p: int, nvars: int, f_face: torch.Tensor = None) -> torch.Tensor:
+        """lt_mortar_gather (Alg. 8 step 4): f_mortar [M, nf, nvars, Nf] -> coarse-face fluxes on kind 3
+        slots of f_face (default: a NaN-filled array; pass f_mortar itself to work in place)."""
+        if tuple(f_mortar.shape) != self._face_shape(p, nvars):
+            raise ValueError("lt_mortar_gather: f_mortar must be %s" % (self._face_shape(p, nvars),))
+        if f_face is None:
+            f_face = torch.full_like(f_mortar, float("nan"))
+        _check(lib().lt_mortar_gather(self._h, _dptr(f_mortar, torch.float64, "f_mortar"),
+                                      _dptr(f_face, torch.float64, "f_face"), p, nvars), "lt_mortar_gather")
+        return f_face
+
     def transfer_host(self, u_old: torch.Tensor, u_new: torch.Tensor, p: int, nvars: int):
         """lt_transfer_host: HOST tensors (pinned or pageable), copies inside the call."""
         if u_old.is_cuda or u_new.is_cuda or u_old.dtype != torch.float64 or u_new.dtype != torch.float64:
@@ -265,7 +292,7 @@ class Tree:
         out = (C.c_float * 8)()
         _check(lib().lt_timings(self._h, out), "lt_timings")
         return dict(adapt=out[0], balance=out[1], connect=out[2], transfer=out[3], k_map=out[4], k_transfer=out[5],
-                    k_connect=out[6])
+                    k_connect=out[6], k_mortar=out[7])
 
     def launch_count(self) -> int:
         return int(lib().lt_launch_count(self._h))
