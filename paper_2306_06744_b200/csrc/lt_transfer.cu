@@ -12,6 +12,8 @@
 
 #include <vector>
 
+#include <type_traits>
+
 #include "lt_internal.h"
 
 namespace lt {
@@ -570,127 +572,245 @@ __device__ __forceinline__ void load_ops_1d(int P1, double (*sI)[8][8], double (
   __syncthreads();
 }
 
-template <int DIM>
+// value q (= v * Nf + nn) of the Eq. 17 projection of the coarse trace `src` onto mortar `slot`
+template <int DIM, int P1>
+__device__ __forceinline__ double mortar_value(const double (*sI)[8][8], const double* __restrict__ src, int slot,
+                                               int q) {
+  constexpr int Nf = DIM == 2 ? P1 : P1 * P1;
+  const int v = q / Nf, nn = q - v * Nf;
+  src += (size_t)v * Nf;
+  double out = 0.0;
+  if (DIM == 2) {
+#pragma unroll
+    for (int m = 0; m < P1; ++m) out += sI[slot & 1][nn][m] * src[m];
+  } else {
+    const int n1 = nn / P1, n0 = nn - n1 * P1;
+#pragma unroll
+    for (int m1 = 0; m1 < P1; ++m1) {
+      double row = 0.0;
+#pragma unroll
+      for (int m0 = 0; m0 < P1; ++m0) row += sI[slot & 1][n0][m0] * src[m1 * P1 + m0];
+      out += sI[slot >> 1][n1][m1] * row;
+    }
+  }
+  return out;
+}
+
+// One warp per leaf.  The leaf's nf (kind, nbr) pairs are staged per warp in shared memory.
+// Pass A streams the conforming faces: for every 64 * VEC doubles of a face block the loads of
+// ALL nf faces are issued before the first store (2 * nf independent 128-bit loads per lane),
+// no per-element index arithmetic.  Pass B handles the few fine-side hanging faces (Eq. 17).
+template <int DIM, int VEC, int P1>
 __global__ void __launch_bounds__(256) k_mortar_project(const DevScalars* s, const int32_t* __restrict__ nbr,
                                                         const uint8_t* __restrict__ kind,
                                                         const double* __restrict__ uf, double* __restrict__ unb,
-                                                        int P1, int nvars) {
+                                                        int nvars) {
   constexpr int NF = Dim<DIM>::NF;
+  typedef typename std::conditional<VEC == 2, double2, double>::type V;
   __shared__ double sI[2][8][8], sR[2][8][8];
+  __shared__ int s_nb[8][8];
+  __shared__ int s_kd[8][8];
   load_ops_1d(P1, sI, sR);
-  const int Nf = DIM == 2 ? P1 : P1 * P1, E = nvars * Nf;
-  const int lane = threadIdx.x & 31;
+  constexpr int Nf = DIM == 2 ? P1 : P1 * P1;
+  const int E = nvars * Nf, EV = E / VEC;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int64_t n = s->n;
   const int64_t nw = (int64_t)gridDim.x * (blockDim.x >> 5);
-  for (int64_t e = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); e < n; e += nw) {
-    for (int r = lane; r < NF * E; r += 32) {
-      const int f = r / E, q = r - f * E;
-      const size_t sl = (size_t)e * NF + f;
-      const int kd = kind[sl], k = kd & 15;
-      if (k != 1 && k != 2) continue;
-      const double* src = uf + ((size_t)nbr[sl] * NF + (f ^ 1)) * E;
-      double out;
-      if (k == 1) {
-        out = src[q];  // conforming: the mortar is the face itself
-      } else {
-        const int slot = kd >> 4, v = q / Nf, nn = q - v * Nf;
-        src += (size_t)v * Nf;
-        out = 0.0;
-        if (DIM == 2) {
-          for (int m = 0; m < P1; ++m) out += sI[slot & 1][nn][m] * src[m];
-        } else {
-          const int n1 = nn / P1, n0 = nn - n1 * P1;
-          for (int m1 = 0; m1 < P1; ++m1) {
-            double row = 0.0;
-            for (int m0 = 0; m0 < P1; ++m0) row += sI[slot & 1][n0][m0] * src[m1 * P1 + m0];
-            out += sI[slot >> 1][n1][m1] * row;
-          }
-        }
+  for (int64_t e = (int64_t)blockIdx.x * (blockDim.x >> 5) + w; e < n; e += nw) {
+    __syncwarp();
+    if (lane < NF) {
+      s_kd[w][lane] = kind[(size_t)e * NF + lane];
+      s_nb[w][lane] = nbr[(size_t)e * NF + lane];
+    }
+    __syncwarp();
+    V* dst = reinterpret_cast<V*>(unb + (size_t)e * NF * E);
+    const V* src[NF];
+    bool conf[NF];
+    bool any2 = false;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      const int k = s_kd[w][f] & 15;
+      conf[f] = k == 1;
+      any2 = any2 || k == 2;
+      // conforming: the mortar is the face itself
+      src[f] = reinterpret_cast<const V*>(uf + ((size_t)(conf[f] ? s_nb[w][f] : 0) * NF + (f ^ 1)) * E);
+    }
+    for (int q0 = 0; q0 < EV; q0 += 64) {
+      V v0[NF], v1[NF];
+      const int qa = q0 + lane, qb = q0 + 32 + lane;
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        if (conf[f] && qa < EV) v0[f] = __ldcs(src[f] + qa);
+        if (conf[f] && qb < EV) v1[f] = __ldcs(src[f] + qb);
       }
-      unb[sl * E + q] = out;
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        if (conf[f] && qa < EV) __stcs(dst + f * EV + qa, v0[f]);
+        if (conf[f] && qb < EV) __stcs(dst + f * EV + qb, v1[f]);
+      }
+    }
+    if (any2) {
+#pragma unroll 1
+      for (int f = 0; f < NF; ++f) {
+        const int kd = s_kd[w][f];
+        if ((kd & 15) != 2) continue;
+        const double* sp = uf + ((size_t)s_nb[w][f] * NF + (f ^ 1)) * E;
+        double* dp = unb + ((size_t)e * NF + f) * E;
+        for (int q = lane; q < E; q += 32) dp[q] = mortar_value<DIM, P1>(sI, sp, kd >> 4, q);
+      }
     }
   }
 }
 
-template <int DIM>
-__global__ void __launch_bounds__(256) k_mortar_gather(Geo g, const uint64_t* __restrict__ keys,
-                                                       const int* __restrict__ first, DevScalars* s,
-                                                       const uint8_t* __restrict__ kind,
-                                                       const double* __restrict__ fm, double* __restrict__ ff, int P1,
-                                                       int nvars) {
+// Coarse face (e, f) of kind 3: gather its 2^(dim-1) mortars (Eq. 20), the whole warp on one
+// face.  Lanes < NS locate the fine neighbours.  Per variable the NS mortar blocks are staged
+// in shared memory as ONE fine grid G[M1][M0], M = s * P1 + m, and the projection is applied
+// sum-factorised with the concatenated 1-D operator Rc[n][M] = R^s[n][m]:
+//   T[M1][n0] = sum_M0 Rc[n0][M0] G[M1][M0],   F[n1][n0] = sum_M1 Rc[n1][M1] T[M1][n0].
+template <int DIM, int P1>
+__device__ __forceinline__ void gather_face(const Geo& g, const uint64_t* __restrict__ keys,
+                                            const int* __restrict__ first, DevScalars* s, const double (*sR)[8][8],
+                                            double* __restrict__ wsm, const double* __restrict__ fm,
+                                            double* __restrict__ ff, int64_t e, int f, int nvars, int lane) {
   constexpr int NF = Dim<DIM>::NF, NS = 1 << (DIM - 1);
-  __shared__ double sI[2][8][8], sR[2][8][8];
-  load_ops_1d(P1, sI, sR);
-  const int Nf = DIM == 2 ? P1 : P1 * P1, E = nvars * Nf;
-  const int lane = threadIdx.x & 31;
-  const int64_t n = s->n;
-  const int64_t nw = (int64_t)gridDim.x * (blockDim.x >> 5);
-  for (int64_t e = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); e < n; e += nw) {
-    const uint64_t key = keys[e];
-    const int l = key_level(key);
-    const uint64_t m = key_morton(key);
-    for (int f = 0; f < NF; ++f) {
-      const size_t sl = (size_t)e * NF + f;
-      if ((kind[sl] & 15) != 3) continue;  // warp-uniform
-      // lane s < NS finds the fine neighbour on mortar s: the child of the same-level neighbour
-      // cell that touches the face, tangential child bits = s (ascending axis order)
-      const int axis = f >> 1;
-      uint64_t mn = 0;
-      face_neighbour<DIM>(g, m, l, f, &mn);
-      int es = 0;
-      if (lane < NS) {
-        int c = (f & 1) ? 0 : (1 << axis), bit = 0;
+  constexpr int Nf = DIM == 2 ? P1 : P1 * P1, P2 = 2 * P1;
+  const int E = nvars * Nf;
+  const uint64_t key = keys[e];
+  const int l = key_level(key);
+  const uint64_t m = key_morton(key);
+  const int axis = f >> 1;
+  uint64_t mn = 0;
+  face_neighbour<DIM>(g, m, l, f, &mn);
+  int es = 0;
+  if (lane < NS) {
+    // the child of the same-level neighbour cell that touches the face, tangential bits = lane
+    int c = (f & 1) ? 0 : (1 << axis), bit = 0;
 #pragma unroll
-        for (int a = 0; a < DIM; ++a) {
-          if (a == axis) continue;
-          c |= ((lane >> bit) & 1) << a;
-          ++bit;
-        }
-        es = locate(g, keys, first, mn | ((uint64_t)c << (DIM * (g.maxl - l - 1))));
-        if (key_level(keys[es]) != l + 1) set_status(&s->status, LT_ERR_UNBALANCED);
+    for (int a = 0; a < DIM; ++a) {
+      if (a == axis) continue;
+      c |= ((lane >> bit) & 1) << a;
+      ++bit;
+    }
+    es = locate(g, keys, first, mn | ((uint64_t)c << (DIM * (g.maxl - l - 1))));
+    if (key_level(keys[es]) != l + 1) set_status(&s->status, LT_ERR_UNBALANCED);
+  }
+  const double* srcs[NS];
+#pragma unroll
+  for (int sidx = 0; sidx < NS; ++sidx)
+    srcs[sidx] = fm + ((size_t)__shfl_sync(0xffffffffu, es, sidx) * NF + (f ^ 1)) * E;
+  double* dst = ff + ((size_t)e * NF + f) * E;
+  double* G = wsm;             // [P2][P2] (3-D) / [P2] (2-D)
+  double* T = wsm + 256;       // [P2][P1]
+  for (int v = 0; v < nvars; ++v) {
+    __syncwarp();
+    for (int i = lane; i < NS * Nf; i += 32) {
+      const int sidx = i / Nf, mm = i - sidx * Nf;
+      double val = 0.0;
+#pragma unroll
+      for (int k = 0; k < NS; ++k)
+        if (k == sidx) val = srcs[k][(size_t)v * Nf + mm];
+      if (DIM == 2) {
+        G[sidx * P1 + mm] = val;
+      } else {
+        const int m1 = mm / P1, m0 = mm - m1 * P1;
+        G[((sidx >> 1) * P1 + m1) * P2 + (sidx & 1) * P1 + m0] = val;
       }
-      int e_of[NS];
-#pragma unroll
-      for (int sidx = 0; sidx < NS; ++sidx) e_of[sidx] = __shfl_sync(0xffffffffu, es, sidx);
-      for (int q = lane; q < E; q += 32) {
-        const int v = q / Nf, nn = q - v * Nf;
+    }
+    __syncwarp();
+    if (DIM == 2) {
+      for (int n0 = lane; n0 < P1; n0 += 32) {
         double acc = 0.0;
 #pragma unroll
-        for (int sidx = 0; sidx < NS; ++sidx) {
-          const double* src = fm + ((size_t)e_of[sidx] * NF + (f ^ 1)) * E + (size_t)v * Nf;
-          if (DIM == 2) {
-            for (int mm = 0; mm < P1; ++mm) acc += sR[sidx & 1][nn][mm] * src[mm];
-          } else {
-            const int n1 = nn / P1, n0 = nn - n1 * P1;
-            for (int m1 = 0; m1 < P1; ++m1) {
-              double row = 0.0;
-              for (int m0 = 0; m0 < P1; ++m0) row += sR[sidx & 1][n0][m0] * src[m1 * P1 + m0];
-              acc += sR[sidx >> 1][n1][m1] * row;
-            }
-          }
-        }
-        ff[sl * E + q] = acc;
+        for (int M0 = 0; M0 < P2; ++M0) acc += sR[M0 >= P1][n0][M0 >= P1 ? M0 - P1 : M0] * G[M0];
+        dst[(size_t)v * Nf + n0] = acc;
+      }
+    } else {
+      for (int i = lane; i < P2 * P1; i += 32) {
+        const int M1 = i / P1, n0 = i - M1 * P1;
+        double acc = 0.0;
+#pragma unroll
+        for (int M0 = 0; M0 < P2; ++M0) acc += sR[M0 >= P1][n0][M0 >= P1 ? M0 - P1 : M0] * G[M1 * P2 + M0];
+        T[i] = acc;
+      }
+      __syncwarp();
+      for (int i = lane; i < Nf; i += 32) {
+        const int n1 = i / P1, n0 = i - n1 * P1;
+        double acc = 0.0;
+#pragma unroll
+        for (int M1 = 0; M1 < P2; ++M1) acc += sR[M1 >= P1][n1][M1 >= P1 ? M1 - P1 : M1] * T[M1 * P1 + n0];
+        dst[(size_t)v * Nf + i] = acc;
       }
     }
   }
+}
+
+// A warp scans the kind bytes of 32 consecutive leaves (nf coalesced rounds), ballots the
+// coarse-side hanging slots (a few per cent of all slots) and processes each hit together.
+template <int DIM, int P1>
+__global__ void __launch_bounds__(256) k_mortar_gather(Geo g, const uint64_t* __restrict__ keys,
+                                                       const int* __restrict__ first, DevScalars* s,
+                                                       const uint8_t* __restrict__ kind,
+                                                       const double* __restrict__ fm, double* __restrict__ ff,
+                                                       int nvars) {
+  constexpr int NF = Dim<DIM>::NF;
+  __shared__ double sI[2][8][8], sR[2][8][8];
+  __shared__ double s_work[8][384];  // per warp: G [16][16] + T [16][8]
+  load_ops_1d(P1, sI, sR);
+  const int lane = threadIdx.x & 31;
+  const int64_t nslots = (int64_t)s->n * NF;
+  const int64_t nw = (int64_t)gridDim.x * (blockDim.x >> 5);
+  for (int64_t c0 = ((int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 32 * NF; c0 < nslots;
+       c0 += nw * 32 * NF) {
+#pragma unroll 1
+    for (int c = 0; c < NF; ++c) {
+      const int64_t idx = c0 + c * 32 + lane;
+      const bool hit = idx < nslots && (kind[idx] & 15) == 3;
+      unsigned mask = __ballot_sync(0xffffffffu, hit);
+      while (mask) {
+        const int b = __ffs(mask) - 1;
+        mask &= mask - 1;
+        const int64_t sl = c0 + c * 32 + b;
+        const int64_t e = sl / NF;
+        gather_face<DIM, P1>(g, keys, first, s, sR, s_work[threadIdx.x >> 5], fm, ff, e, (int)(sl - e * NF), nvars, lane);
+      }
+    }
+  }
+}
+
+template <int DIM, int P1>
+static void launch_mortar_t(Tree* t, int which, const double* d_in, double* d_out, int nvars, int G) {
+  constexpr int Nf = DIM == 2 ? P1 : P1 * P1;
+  if (which == 0) {
+    const bool vec2 = ((nvars * Nf) % 2 == 0) && (((uintptr_t)d_in | (uintptr_t)d_out) & 15) == 0;
+    if (vec2) k_mortar_project<DIM, 2, P1><<<G, 256, 0, t->stream>>>(t->d_s, t->nbr, t->kind, d_in, d_out, nvars);
+    else k_mortar_project<DIM, 1, P1><<<G, 256, 0, t->stream>>>(t->d_s, t->nbr, t->kind, d_in, d_out, nvars);
+  } else {
+    k_mortar_gather<DIM, P1><<<G, 256, 0, t->stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->kind,
+                                                       d_in, d_out, nvars);
+  }
+}
+
+template <int DIM>
+static int launch_mortar_d(Tree* t, int which, const double* d_in, double* d_out, int p, int nvars, int G) {
+  switch (p) {
+    case 0: launch_mortar_t<DIM, 1>(t, which, d_in, d_out, nvars, G); break;
+    case 1: launch_mortar_t<DIM, 2>(t, which, d_in, d_out, nvars, G); break;
+    case 2: launch_mortar_t<DIM, 3>(t, which, d_in, d_out, nvars, G); break;
+    case 3: launch_mortar_t<DIM, 4>(t, which, d_in, d_out, nvars, G); break;
+    case 4: launch_mortar_t<DIM, 5>(t, which, d_in, d_out, nvars, G); break;
+    case 5: launch_mortar_t<DIM, 6>(t, which, d_in, d_out, nvars, G); break;
+    case 6: launch_mortar_t<DIM, 7>(t, which, d_in, d_out, nvars, G); break;
+    case 7: launch_mortar_t<DIM, 8>(t, which, d_in, d_out, nvars, G); break;
+    default: return LT_ERR_ARG;
+  }
+  return LT_OK;
 }
 
 int launch_mortar(Tree* t, int which, const double* d_in, double* d_out, int p, int nvars) {
   const int G = t->num_sms * 8;
-  const int P1 = p + 1;
-  if (which == 0) {
-    if (t->g.dim == 2)
-      k_mortar_project<2><<<G, 256, 0, t->stream>>>(t->d_s, t->nbr, t->kind, d_in, d_out, P1, nvars);
-    else
-      k_mortar_project<3><<<G, 256, 0, t->stream>>>(t->d_s, t->nbr, t->kind, d_in, d_out, P1, nvars);
-  } else {
-    if (t->g.dim == 2)
-      k_mortar_gather<2><<<G, 256, 0, t->stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->kind, d_in,
-                                                   d_out, P1, nvars);
-    else
-      k_mortar_gather<3><<<G, 256, 0, t->stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->kind, d_in,
-                                                   d_out, P1, nvars);
-  }
+  const int rc = t->g.dim == 2 ? launch_mortar_d<2>(t, which, d_in, d_out, p, nvars, G)
+                               : launch_mortar_d<3>(t, which, d_in, d_out, p, nvars, G);
+  if (rc != LT_OK) return rc;
   t->launches++;
   LT_CUDA(cudaGetLastError());
   return LT_OK;
