@@ -11,7 +11,7 @@
 namespace lt {
 
 constexpr int ST = 256;                 // threads per sort block (= number of digit values)
-constexpr int SITEMS = 8;               // keys per thread
+constexpr int SITEMS = 16;              // keys per thread
 constexpr int STILE = ST * SITEMS;      // keys per tile
 constexpr unsigned FLAG_AGG = 1u << 30, FLAG_INC = 2u << 30, VAL_MASK = (1u << 30) - 1;
 
@@ -37,11 +37,26 @@ __global__ void __launch_bounds__(256) k_sort_scan_hist(unsigned* __restrict__ h
   hist[blockIdx.x * 256 + threadIdx.x] = ex;
 }
 
+// status words are polled with GPU-scope relaxed loads (a volatile access is system scope and
+// is not pipelined); the word carries its own payload, so no fence is needed
+__device__ __forceinline__ unsigned ld_status(const volatile unsigned* p) {
+  unsigned v;
+  asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_status(volatile unsigned* p, unsigned v) {
+  asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
 __global__ void __launch_bounds__(ST) k_sort_pass(const uint64_t* __restrict__ in, uint64_t* __restrict__ out,
                                                   int64_t n, int shift, const unsigned* __restrict__ base,
                                                   volatile unsigned* status, int* ticket) {
   __shared__ unsigned wcnt[(ST / 32) * 256];
   __shared__ unsigned gbase[256];
+  __shared__ unsigned loff[256];
+  __shared__ unsigned s_scan[33];
+  __shared__ unsigned s_ntile;
+  __shared__ uint64_t s_keys[STILE];
   __shared__ int s_tile;
   if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1);
   for (int i = threadIdx.x; i < (ST / 32) * 256; i += ST) wcnt[i] = 0;
@@ -85,23 +100,54 @@ __global__ void __launch_bounds__(ST) k_sort_pass(const uint64_t* __restrict__ i
     }
     unsigned excl = 0;
     if (tile == 0) {
-      status[d] = run | FLAG_INC;
+      st_status(status + d, run | FLAG_INC);
     } else {
-      status[(size_t)tile * 256 + d] = run | FLAG_AGG;
-      for (int t = tile - 1; t >= 0; --t) {
-        unsigned v;
-        do { v = status[(size_t)t * 256 + d]; } while ((v >> 30) == 0);
-        excl += v & VAL_MASK;
-        if ((v >> 30) == 2) break;
+      st_status(status + (size_t)tile * 256 + d, run | FLAG_AGG);
+      // look back over the earlier tiles, LB status words per round trip: in the first wave
+      // every resident tile publishes its aggregate at about the same time, so the chain to
+      // the nearest inclusive prefix can be hundreds of tiles long -- batching the (independent)
+      // loads keeps it from being a chain of dependent L2 latencies
+      constexpr int LB = 8;
+      bool done = false;
+      for (int t = tile - 1; t >= 0 && !done; t -= LB) {
+        unsigned v[LB];
+#pragma unroll
+        for (int j = 0; j < LB; ++j) v[j] = t - j >= 0 ? ld_status(status + (size_t)(t - j) * 256 + d) : (2u << 30);
+#pragma unroll
+        for (int j = 0; j < LB; ++j) {
+          if (done) break;
+          while ((v[j] >> 30) == 0) v[j] = ld_status(status + (size_t)(t - j) * 256 + d);
+          excl += v[j] & VAL_MASK;
+          if ((v[j] >> 30) == 2) done = true;
+        }
       }
-      status[(size_t)tile * 256 + d] = ((excl + run) & VAL_MASK) | FLAG_INC;
+      st_status(status + (size_t)tile * 256 + d, ((excl + run) & VAL_MASK) | FLAG_INC);
     }
-    gbase[d] = base[d] + excl;
+    // position of digit d's run inside the tile (exclusive scan of the tile histogram) and the
+    // global address of the run's first key minus that position
+    unsigned ntile;
+    const unsigned tex = block_excl_scan<unsigned>(run, s_scan, &ntile);
+    loff[d] = tex;
+    gbase[d] = base[d] + excl - tex;
+    if (d == 0) s_ntile = ntile;
   }
   __syncthreads();
+  // reorder the tile by digit in shared memory, then write it out in tile order: consecutive
+  // threads store consecutive addresses inside every digit run (instead of one scattered 8-byte
+  // store per key, 25 sectors per request in the first version)
 #pragma unroll
   for (int k = 0; k < SITEMS; ++k)
-    if (dig[k] < 256) out[(size_t)gbase[dig[k]] + wcnt[w * 256 + dig[k]] + rank[k]] = key[k];
+    if (dig[k] < 256) s_keys[loff[dig[k]] + wcnt[w * 256 + dig[k]] + rank[k]] = key[k];
+  __syncthreads();
+  const int nt = (int)s_ntile;
+#pragma unroll
+  for (int k = 0; k < SITEMS; ++k) {
+    const int i = k * ST + threadIdx.x;
+    if (i < nt) {
+      const uint64_t kk = s_keys[i];
+      out[(size_t)gbase[(int)((kk >> shift) & 255)] + i] = kk;
+    }
+  }
 }
 
 int sort_keys(uint64_t* d_keys, int64_t n, int key_bits, SortScratch* sc, cudaStream_t s, int64_t* launches) {
