@@ -1,8 +1,9 @@
 // lt_connect.cu -- face connectivity (Alg. 5) for sm_100a, ONE kernel, one
 // pass over the leaves:
-//   - a tile of 256 consecutive leaves is claimed through a ticket; one thread per (leaf,
-//     local face) slot builds the same-level search key, finds it (sibling shortcut or
-//     bucketed lower bound, Eq. 7) and classifies the face into shared memory;
+//   - a tile of 256 consecutive leaves is claimed through a ticket; one thread per leaf
+//     classifies first its dim parent-interior faces (sibling shortcut) and then its dim
+//     exterior faces (same-level search key, bucketed lower bound, Eq. 7) into shared memory
+//     -- two warp-uniform phases;
 //   - nbr / kind (the paper's face array F) leave in slot order, coalesced;
 //   - one thread per leaf counts its rows, a packed block scan orders them inside the tile,
 //     a decoupled look-back over the earlier tiles orders the tiles, and the three face
@@ -26,31 +27,15 @@ __device__ __forceinline__ int face_slot(int cid, int axis) {
   return cid & 3;
 }
 
-// Classify face f of leaf i.  Returns kind; *nb_out = neighbour index (or -1).
+// Face f of leaf (m, l) at position i by search: same-level neighbour key (periodic wrap /
+// domain boundary), bucketed lower bound (Eq. 7), classification.  Returns kind; *nb_out =
+// neighbour index (or -1).
 template <int DIM>
-__device__ __forceinline__ int connect_face(const Geo& g, const uint64_t* __restrict__ keys,
-                                            const int* __restrict__ first, int n, int i, int f, int* status,
-                                            int* nb_out) {
-  constexpr int NC = Dim<DIM>::NC;
-  const uint64_t key = keys[i];
-  const int l = key_level(key);
-  const uint64_t m = key_morton(key);
+__device__ __forceinline__ int face_by_search(const Geo& g, const uint64_t* __restrict__ keys,
+                                              const int* __restrict__ first, uint64_t m, int l, int f, int* status,
+                                              int* nb_out) {
   const int a = f >> 1;
   *nb_out = -1;
-  if (l > 0) {
-    // A face interior to the parent looks at a sibling.  If that sibling is a leaf and every
-    // sibling between the two is a leaf too, it sits exactly (cid' - cid) entries away
-    // (PAPER.md:200): one key comparison decides, no search.
-    const int sh = DIM * (g.maxl - l);
-    const int cid = (int)((m >> sh) & (uint64_t)(NC - 1));
-    if (((cid >> a) & 1) != (f & 1)) {
-      const int j = i + ((cid ^ (1 << a)) - cid);
-      if (j >= 0 && j < n && keys[j] == make_key(m ^ (1ull << (sh + a)), l)) {
-        *nb_out = j;
-        return 1;
-      }
-    }
-  }
   uint64_t mn;
   if (!face_neighbour<DIM>(g, m, l, f, &mn)) return 0;  // domain boundary
   const int j = locate(g, keys, first, mn);
@@ -77,6 +62,21 @@ __device__ __forceinline__ int connect_face(const Geo& g, const uint64_t* __rest
   if (key_level(keys[j2]) != l + 1) set_status(status, LT_ERR_UNBALANCED);
   *nb_out = j2;
   return 3;
+}
+
+// The face of leaf i on axis a that is INTERIOR to its parent looks at a sibling.  If that
+// sibling is a leaf and every sibling between the two is a leaf too, it sits exactly
+// (cid' - cid) entries away: one key comparison decides, no search.
+template <int DIM>
+__device__ __forceinline__ bool face_by_sibling(const Geo& g, const uint64_t* __restrict__ keys, int n, int i,
+                                                uint64_t m, int l, int cid, int a, int* nb_out) {
+  const int sh = DIM * (g.maxl - l);
+  const int j = i + ((cid ^ (1 << a)) - cid);
+  if (j >= 0 && j < n && keys[j] == make_key(m ^ (1ull << (sh + a)), l)) {
+    *nb_out = j;
+    return true;
+  }
+  return false;
 }
 
 // Tile status words of the decoupled look-back, two independent channels per tile:
@@ -132,22 +132,45 @@ __global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restric
     if (tile >= ntiles) break;
     const int e0 = tile * CT;
     const int ne = min(CT, n - e0);
-    // ---- search: one thread per slot, NF rounds; F leaves in slot order, coalesced
-#pragma unroll 1
-    for (int r = 0; r < NF; ++r) {
-      const int sl = r * CT + threadIdx.x;
-      const int le = sl / NF, f = sl - le * NF;
-      if (le < ne) {
+    // ---- classify: one thread per leaf, two warp-uniform phases -- first the DIM faces
+    // interior to the parent (sibling shortcut, one compare), then the DIM exterior faces
+    // (search) -- so that a warp never executes both code paths for every slot
+    if ((int)threadIdx.x < ne) {
+      constexpr int NC = Dim<DIM>::NC;
+      const int i = e0 + threadIdx.x;
+      const uint64_t key = keys[i];
+      const int l = key_level(key);
+      const uint64_t m = key_morton(key);
+      const int cid = l > 0 ? (int)((m >> (DIM * (g.maxl - l))) & (uint64_t)(NC - 1)) : 0;
+#pragma unroll
+      for (int a = 0; a < DIM; ++a) {
+        const int f = 2 * a + (((cid >> a) & 1) ^ 1);
+        int nb, kd = 1;
+        if (l == 0 || !face_by_sibling<DIM>(g, keys, n, i, m, l, cid, a, &nb))
+          kd = face_by_search<DIM>(g, keys, first, m, l, f, &s->status, &nb);
+        s_nb[threadIdx.x * NF + f] = nb;
+        s_kd[threadIdx.x * NF + f] = (uint8_t)kd;
+      }
+#pragma unroll
+      for (int a = 0; a < DIM; ++a) {
+        const int f = 2 * a + ((cid >> a) & 1);
         int nb;
-        const int kd = connect_face<DIM>(g, keys, first, n, e0 + le, f, &s->status, &nb);
-        s_nb[sl] = nb;
-        s_kd[sl] = (uint8_t)kd;
-        const size_t gs = (size_t)e0 * NF + sl;
-        nbr[gs] = nb;
-        kind[gs] = (uint8_t)kd;
+        const int kd = face_by_search<DIM>(g, keys, first, m, l, f, &s->status, &nb);
+        s_nb[threadIdx.x * NF + f] = nb;
+        s_kd[threadIdx.x * NF + f] = (uint8_t)kd;
       }
     }
     __syncthreads();
+    // F (the paper's face array) leaves in slot order, coalesced
+#pragma unroll
+    for (int r = 0; r < NF; ++r) {
+      const int sl = r * CT + threadIdx.x;
+      if (sl < ne * NF) {
+        const size_t gs = (size_t)e0 * NF + sl;
+        nbr[gs] = s_nb[sl];
+        kind[gs] = s_kd[sl];
+      }
+    }
     // ---- rows of this thread's leaf: conf | hang << 21 | bnd << 42
     unsigned long long cnt = 0;
     if ((int)threadIdx.x < ne) {
