@@ -295,6 +295,7 @@ void lt_free(lt_tree* t) {
     if (t->ev_done[r]) cudaEventDestroy(t->ev_done[r]);
     if (t->ev_out[r]) cudaEventDestroy(t->ev_out[r]);
   }
+  free_dev(t->stream, t->mortar_hits);
   free_dev(t->stream, t->d_bounds);
   if (t->h_bounds) cudaFreeHost(t->h_bounds);
   if (t->s_in) cudaStreamDestroy(t->s_in);
@@ -555,6 +556,9 @@ static int mortar_call(lt_tree* t, int which, const double* d_in, double* d_out,
   int rc;
   if ((rc = build_operators(t, p)) != LT_OK) return rc;
   tic(t, 7);
+  // the gather works from the list of coarse-side hanging faces (rebuilt per call: d_s->aux,
+  // its counter, is shared scratch)
+  if (which == 1 && (rc = launch_mortar_hits(t)) != LT_OK) return rc;
   if ((rc = launch_mortar(t, which, d_in, d_out, p, nvars)) != LT_OK) return rc;
   toc(t, 7);
   return LT_OK;
@@ -627,7 +631,8 @@ int lt_transfer_host(lt_tree* t, const double* h_u_old, double* h_u_new, int p, 
   while ((n_new + slab - 1) / slab > 4096) slab *= 2;
   const int S = (int)((n_new + slab - 1) / slab);
   if (t->bounds_cap < S + 1) {
-    free_dev(t->stream, t->d_bounds);
+    free_dev(t->stream, t->mortar_hits);
+  free_dev(t->stream, t->d_bounds);
     if (t->h_bounds) cudaFreeHost(t->h_bounds);
     t->d_bounds = nullptr; t->h_bounds = nullptr; t->bounds_cap = 0;
     if ((rc = alloc_dev(t->stream, &t->d_bounds, 2 * (int64_t)(S + 1))) != LT_OK) return rc;

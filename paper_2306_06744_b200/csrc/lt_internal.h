@@ -63,6 +63,8 @@ struct Tree {
   uint8_t* map_kind;
   bool map_valid;
   bool faces_valid;       // nbr / kind describe the current tree (set by lt_connect)
+  int* mortar_hits;       // [hits][2 + 2^(dim-1)]: coarse-side hanging faces (e, f, fine neighbours)
+  int64_t mortar_hits_cap;
 
   // transfer operators on the device for (dim, p): I^0,I^1,R^0,R^1, each [P1][P1]
   double* d_ops;
@@ -122,6 +124,7 @@ int launch_transfer(Tree* t, const double* d_u_old, double* d_u_new, int p, int 
                     int64_t je = -1);
 int launch_slab_bounds(Tree* t, int64_t n_old, int64_t slab, int S, int64_t* d_out);
 int build_operators(Tree* t, int p);
+int launch_mortar_hits(Tree* t);
 int launch_mortar(Tree* t, int which, const double* d_in, double* d_out, int p, int nvars);
 
 // ---- lt_construct.cu (Alg. 2)

@@ -662,117 +662,152 @@ __global__ void __launch_bounds__(256) k_mortar_project(const DevScalars* s, con
   }
 }
 
-// Coarse face (e, f) of kind 3: gather its 2^(dim-1) mortars (Eq. 20), the whole warp on one
-// face.  Lanes < NS locate the fine neighbours.  Per variable the NS mortar blocks are staged
-// in shared memory as ONE fine grid G[M1][M0], M = s * P1 + m, and the projection is applied
-// sum-factorised with the concatenated 1-D operator Rc[n][M] = R^s[n][m]:
-//   T[M1][n0] = sum_M0 Rc[n0][M0] G[M1][M0],   F[n1][n0] = sum_M1 Rc[n1][M1] T[M1][n0].
-template <int DIM, int P1>
-__device__ __forceinline__ void gather_face(const Geo& g, const uint64_t* __restrict__ keys,
-                                            const int* __restrict__ first, DevScalars* s, const double (*sR)[8][8],
-                                            double* __restrict__ wsm, const double* __restrict__ fm,
-                                            double* __restrict__ ff, int64_t e, int f, int nvars, int lane) {
-  constexpr int NF = Dim<DIM>::NF, NS = 1 << (DIM - 1);
-  constexpr int Nf = DIM == 2 ? P1 : P1 * P1, P2 = 2 * P1;
-  const int E = nvars * Nf;
+// Coarse face (e, f) of kind 3, step 1 (ONE LANE per face, so a warp resolves up to 32 faces
+// with their dependent loads in flight together): the fine neighbour on mortar s is the child
+// of the same-level neighbour cell that touches the face with tangential child bits s.
+// lt_connect stored the slot-0 neighbour j0; when the siblings in between are leaves the others
+// sit (c - c0) entries further: one key compare, else a bucketed search.
+template <int DIM>
+__device__ __forceinline__ void gather_resolve(const Geo& g, const uint64_t* __restrict__ keys,
+                                               const int* __restrict__ first, DevScalars* s, int64_t e, int f,
+                                               int j0, int* es /* [2^(DIM-1)] */) {
+  constexpr int NS = 1 << (DIM - 1);
   const uint64_t key = keys[e];
   const int l = key_level(key);
   const uint64_t m = key_morton(key);
   const int axis = f >> 1;
   uint64_t mn = 0;
   face_neighbour<DIM>(g, m, l, f, &mn);
-  int es = 0;
-  if (lane < NS) {
-    // the child of the same-level neighbour cell that touches the face, tangential bits = lane
-    int c = (f & 1) ? 0 : (1 << axis), bit = 0;
+  const int c0 = (f & 1) ? 0 : (1 << axis);
+  const int n = s->n;
+#pragma unroll
+  for (int sidx = 0; sidx < NS; ++sidx) {
+    int c = c0, bit = 0;
 #pragma unroll
     for (int a = 0; a < DIM; ++a) {
       if (a == axis) continue;
-      c |= ((lane >> bit) & 1) << a;
+      c |= ((sidx >> bit) & 1) << a;
       ++bit;
     }
-    es = locate(g, keys, first, mn | ((uint64_t)c << (DIM * (g.maxl - l - 1))));
-    if (key_level(keys[es]) != l + 1) set_status(&s->status, LT_ERR_UNBALANCED);
-  }
-  const double* srcs[NS];
-#pragma unroll
-  for (int sidx = 0; sidx < NS; ++sidx)
-    srcs[sidx] = fm + ((size_t)__shfl_sync(0xffffffffu, es, sidx) * NF + (f ^ 1)) * E;
-  double* dst = ff + ((size_t)e * NF + f) * E;
-  double* G = wsm;             // [P2][P2] (3-D) / [P2] (2-D)
-  double* T = wsm + 256;       // [P2][P1]
-  for (int v = 0; v < nvars; ++v) {
-    __syncwarp();
-    for (int i = lane; i < NS * Nf; i += 32) {
-      const int sidx = i / Nf, mm = i - sidx * Nf;
-      double val = 0.0;
-#pragma unroll
-      for (int k = 0; k < NS; ++k)
-        if (k == sidx) val = srcs[k][(size_t)v * Nf + mm];
-      if (DIM == 2) {
-        G[sidx * P1 + mm] = val;
-      } else {
-        const int m1 = mm / P1, m0 = mm - m1 * P1;
-        G[((sidx >> 1) * P1 + m1) * P2 + (sidx & 1) * P1 + m0] = val;
-      }
-    }
-    __syncwarp();
-    if (DIM == 2) {
-      for (int n0 = lane; n0 < P1; n0 += 32) {
-        double acc = 0.0;
-#pragma unroll
-        for (int M0 = 0; M0 < P2; ++M0) acc += sR[M0 >= P1][n0][M0 >= P1 ? M0 - P1 : M0] * G[M0];
-        dst[(size_t)v * Nf + n0] = acc;
-      }
+    const uint64_t cm = mn | ((uint64_t)c << (DIM * (g.maxl - l - 1)));
+    const int64_t cand = (int64_t)j0 + (c - c0);
+    if (cand >= 0 && cand < n && keys[cand] == make_key(cm, l + 1)) {
+      es[sidx] = (int)cand;
     } else {
-      for (int i = lane; i < P2 * P1; i += 32) {
-        const int M1 = i / P1, n0 = i - M1 * P1;
-        double acc = 0.0;
+      es[sidx] = locate(g, keys, first, cm);
+      if (key_level(keys[es[sidx]]) != l + 1) set_status(&s->status, LT_ERR_UNBALANCED);
+    }
+  }
+}
+
+// Step 1 kernel: a warp scans the kind bytes of 32 consecutive leaves (nf coalesced rounds); every
+// coarse-side hanging slot (a few per cent of all slots) is resolved by its own lane and appended
+// to the hit list: (e, f, es[0..NS)).  The order of the list is arbitrary, the result is not:
+// every hit owns its output block.
+template <int DIM>
+__global__ void __launch_bounds__(256) k_mortar_hits(Geo g, const uint64_t* __restrict__ keys,
+                                                     const int* __restrict__ first, DevScalars* s,
+                                                     const int32_t* __restrict__ nbr,
+                                                     const uint8_t* __restrict__ kind, int* __restrict__ hits,
+                                                     int max_hits) {
+  constexpr int NF = Dim<DIM>::NF, NS = 1 << (DIM - 1), HW = 2 + NS;
+  const int lane = threadIdx.x & 31;
+  const int64_t nslots = (int64_t)s->n * NF;
+  const int64_t nw = (int64_t)gridDim.x * (blockDim.x >> 5);
+  for (int64_t c0 = ((int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 32; c0 < nslots;
+       c0 += nw * 32) {
+    const int64_t idx = c0 + lane;
+    const bool hit = idx < nslots && (kind[idx] & 15) == 3;
+    const unsigned mask = __ballot_sync(0xffffffffu, hit);
+    if (mask == 0) continue;
+    int base = 0;
+    if (lane == 0) base = atomicAdd(&s->aux, __popc(mask));
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (hit) {
+      const int64_t e = idx / NF;
+      const int f = (int)(idx - e * NF);
+      int es[NS];
+      gather_resolve<DIM>(g, keys, first, s, e, f, nbr[idx], es);
+      const int h = base + __popc(mask & ((1u << lane) - 1));
+      if (h < max_hits) {
+        hits[(size_t)h * HW] = (int)e;
+        hits[(size_t)h * HW + 1] = f;
 #pragma unroll
-        for (int M0 = 0; M0 < P2; ++M0) acc += sR[M0 >= P1][n0][M0 >= P1 ? M0 - P1 : M0] * G[M1 * P2 + M0];
-        T[i] = acc;
-      }
-      __syncwarp();
-      for (int i = lane; i < Nf; i += 32) {
-        const int n1 = i / P1, n0 = i - n1 * P1;
-        double acc = 0.0;
-#pragma unroll
-        for (int M1 = 0; M1 < P2; ++M1) acc += sR[M1 >= P1][n1][M1 >= P1 ? M1 - P1 : M1] * T[M1 * P1 + n0];
-        dst[(size_t)v * Nf + i] = acc;
+        for (int sidx = 0; sidx < NS; ++sidx) hits[(size_t)h * HW + 2 + sidx] = es[sidx];
+      } else {
+        set_status(&s->status, LT_ERR_UNBALANCED);
       }
     }
   }
 }
 
-// A warp scans the kind bytes of 32 consecutive leaves (nf coalesced rounds), ballots the
-// coarse-side hanging slots (a few per cent of all slots) and processes each hit together.
+// Step 2 kernel: one thread per output value F[e][f][v][n] of every hit (Eq. 20):
+//   F = sum_s (R^{s1} (x) R^{s0}) F^_s, applied as a row pass and a column pass per mortar.
+// The NS * Nf inputs of a (hit, variable) pair are shared by Nf neighbouring threads and stay
+// in L1; the 1-D operators sit in shared memory.
 template <int DIM, int P1>
-__global__ void __launch_bounds__(256) k_mortar_gather(Geo g, const uint64_t* __restrict__ keys,
-                                                       const int* __restrict__ first, DevScalars* s,
-                                                       const uint8_t* __restrict__ kind,
-                                                       const double* __restrict__ fm, double* __restrict__ ff,
-                                                       int nvars) {
-  constexpr int NF = Dim<DIM>::NF;
+__global__ void __launch_bounds__(256) k_mortar_apply(const DevScalars* s, const int* __restrict__ hits,
+                                                      const double* __restrict__ fm, double* __restrict__ ff,
+                                                      int nvars) {
+  constexpr int NF = Dim<DIM>::NF, NS = 1 << (DIM - 1), HW = 2 + NS;
+  constexpr int Nf = DIM == 2 ? P1 : P1 * P1;
   __shared__ double sI[2][8][8], sR[2][8][8];
-  __shared__ double s_work[8][384];  // per warp: G [16][16] + T [16][8]
   load_ops_1d(P1, sI, sR);
-  const int lane = threadIdx.x & 31;
-  const int64_t nslots = (int64_t)s->n * NF;
-  const int64_t nw = (int64_t)gridDim.x * (blockDim.x >> 5);
-  for (int64_t c0 = ((int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 32 * NF; c0 < nslots;
-       c0 += nw * 32 * NF) {
-#pragma unroll 1
-    for (int c = 0; c < NF; ++c) {
-      const int64_t idx = c0 + c * 32 + lane;
-      const bool hit = idx < nslots && (kind[idx] & 15) == 3;
-      unsigned mask = __ballot_sync(0xffffffffu, hit);
-      while (mask) {
-        const int b = __ffs(mask) - 1;
-        mask &= mask - 1;
-        const int64_t sl = c0 + c * 32 + b;
-        const int64_t e = sl / NF;
-        gather_face<DIM, P1>(g, keys, first, s, sR, s_work[threadIdx.x >> 5], fm, ff, e, (int)(sl - e * NF), nvars, lane);
+  const int E = nvars * Nf;
+  if (DIM == 2) {
+    const int64_t total = (int64_t)s->aux * E;
+    for (int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; idx < total;
+         idx += (int64_t)gridDim.x * blockDim.x) {
+      const int64_t h = idx / E;
+      const int q = (int)(idx - h * E);
+      const int v = q / Nf, nn = q - v * Nf;
+      const int* hp = hits + (size_t)h * HW;
+      const int e = hp[0], f = hp[1];
+      double acc = 0.0;
+#pragma unroll
+      for (int sidx = 0; sidx < NS; ++sidx) {
+        const double* src = fm + ((size_t)hp[2 + sidx] * NF + (f ^ 1)) * E + (size_t)v * Nf;
+#pragma unroll
+        for (int mm = 0; mm < P1; ++mm) acc += sR[sidx][nn][mm] * src[mm];
       }
+      ff[((size_t)e * NF + f) * E + q] = acc;
+    }
+  } else {
+    // 3-D: one thread per output ROW (h, v, n1): every input row is loaded once and feeds the P1
+    // outputs of the thread (5x fewer loads than one thread per value)
+    const int RW = nvars * P1;  // rows per hit
+    const int64_t total = (int64_t)s->aux * RW;
+    for (int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; idx < total;
+         idx += (int64_t)gridDim.x * blockDim.x) {
+      const int64_t h = idx / RW;
+      const int q = (int)(idx - h * RW);
+      const int v = q / P1, n1 = q - v * P1;
+      const int* hp = hits + (size_t)h * HW;
+      const int e = hp[0], f = hp[1];
+      double acc[P1];
+#pragma unroll
+      for (int n0 = 0; n0 < P1; ++n0) acc[n0] = 0.0;
+#pragma unroll
+      for (int sidx = 0; sidx < NS; ++sidx) {
+        const double* src = fm + ((size_t)hp[2 + sidx] * NF + (f ^ 1)) * E + (size_t)v * Nf;
+#pragma unroll
+        for (int m1 = 0; m1 < P1; ++m1) {
+          double in[P1];
+#pragma unroll
+          for (int m0 = 0; m0 < P1; ++m0) in[m0] = src[m1 * P1 + m0];
+          const double r1 = sR[sidx >> 1][n1][m1];
+#pragma unroll
+          for (int n0 = 0; n0 < P1; ++n0) {
+            double row = 0.0;
+#pragma unroll
+            for (int m0 = 0; m0 < P1; ++m0) row += sR[sidx & 1][n0][m0] * in[m0];
+            acc[n0] += r1 * row;
+          }
+        }
+      }
+      double* dst = ff + ((size_t)e * NF + f) * E + (size_t)v * Nf + n1 * P1;
+#pragma unroll
+      for (int n0 = 0; n0 < P1; ++n0) dst[n0] = acc[n0];
     }
   }
 }
@@ -785,8 +820,7 @@ static void launch_mortar_t(Tree* t, int which, const double* d_in, double* d_ou
     if (vec2) k_mortar_project<DIM, 2, P1><<<G, 256, 0, t->stream>>>(t->d_s, t->nbr, t->kind, d_in, d_out, nvars);
     else k_mortar_project<DIM, 1, P1><<<G, 256, 0, t->stream>>>(t->d_s, t->nbr, t->kind, d_in, d_out, nvars);
   } else {
-    k_mortar_gather<DIM, P1><<<G, 256, 0, t->stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->kind,
-                                                       d_in, d_out, nvars);
+    k_mortar_apply<DIM, P1><<<G, 256, 0, t->stream>>>(t->d_s, t->mortar_hits, d_in, d_out, nvars);
   }
 }
 
@@ -803,6 +837,32 @@ static int launch_mortar_d(Tree* t, int which, const double* d_in, double* d_out
     case 7: launch_mortar_t<DIM, 8>(t, which, d_in, d_out, nvars, G); break;
     default: return LT_ERR_ARG;
   }
+  return LT_OK;
+}
+
+// (Re)build the list of coarse-side hanging faces with their fine neighbours; valid until the
+// tree or its connectivity changes.
+int launch_mortar_hits(Tree* t) {
+  const int NS = 1 << (t->g.dim - 1), HW = 2 + NS;
+  const int64_t max_hits = t->h_s->n_face[1] / NS + 1;  // every coarse face has exactly NS fine faces
+  if (t->mortar_hits_cap < max_hits) {
+    dev_free(t->mortar_hits, t->stream);
+    t->mortar_hits = nullptr;
+    t->mortar_hits_cap = 0;
+    int rc = dev_alloc((void**)&t->mortar_hits, (size_t)max_hits * HW * sizeof(int), t->stream);
+    if (rc != LT_OK) return rc;
+    t->mortar_hits_cap = max_hits;
+  }
+  LT_CUDA(cudaMemsetAsync(&t->d_s->aux, 0, sizeof(int), t->stream));
+  const int G = t->num_sms * 8;
+  if (t->g.dim == 2)
+    k_mortar_hits<2><<<G, 256, 0, t->stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->nbr, t->kind,
+                                               t->mortar_hits, (int)max_hits);
+  else
+    k_mortar_hits<3><<<G, 256, 0, t->stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->nbr, t->kind,
+                                               t->mortar_hits, (int)max_hits);
+  t->launches++;
+  LT_CUDA(cudaGetLastError());
   return LT_OK;
 }
 

@@ -103,6 +103,23 @@ def test_config5_full_size_cycle3():
             seen[k] += int(((kind_o[j0:j1] & 15) == k).sum())
     assert (seen > 0).all(), "sampled slabs must cover copy, refine and coarsen: %s" % seen
     print("c5 full size: sampled %d elements (copy/refine/coarsen %s), worst |diff| %.2e" % (seen.sum(), seen, worst))
+    # ---- mortars (Alg. 8 steps 2 and 4) on the same 13.5 M-leaf mesh, every face slot, p = 3 with
+    # one variable so that the host arrays stay at 10 GB each
+    del un_g, ug, uo
+    torch.cuda.empty_cache()
+    Nf = (p + 1) ** 2
+    uf = np.random.default_rng(11).uniform(-1.0, 1.0, (M1, nf, 1, Nf))
+    d_uf = torch.from_numpy(uf).cuda()
+    for name in ("mortar_project", "mortar_gather"):
+        want = getattr(ot, name)(uf, p, 1)
+        got = getattr(gt, name)(d_uf, p, 1).cpu().numpy()
+        gt.sync()
+        m = ~np.isnan(want)
+        assert np.array_equal(np.isnan(got), ~m), name + ": touched slots differ"
+        err = float(np.abs(got[m] - want[m]).max())
+        assert err <= 1e-12, "%s at full size: |diff| %.3e" % (name, err)
+        print("c5 full size %s: %d values, worst |diff| %.2e" % (name, int(m.sum()), err))
+        del want, got, m
 
 
 def test_construction_full_size_pc9():
