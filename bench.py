@@ -343,7 +343,7 @@ def run_ours(args):
             w = line.split()
             if len(w) >= 3 and w[0] == "k_transfer":
                 traffic = int(w[1])
-                traffic_note = ("ncu --set full of the config-5 cycle-3 launch (profiles/r1b_step_full.md); "
+                traffic_note = ("ncu --set full of the config-5 cycle-3 launch (profiles/r1f_step_full.md); "
                                 "algorithmic bytes of that launch: %d" % int(w[2]))
     except Exception:
         pass

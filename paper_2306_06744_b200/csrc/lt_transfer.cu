@@ -616,11 +616,23 @@ __global__ void __launch_bounds__(256) k_mortar_project(const DevScalars* s, con
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int64_t n = s->n;
   const int64_t nw = (int64_t)gridDim.x * (blockDim.x >> 5);
-  for (int64_t e = (int64_t)blockIdx.x * (blockDim.x >> 5) + w; e < n; e += nw) {
+  // the (kind, nbr) pairs of the warp's NEXT leaf are fetched while the current one streams, so a
+  // leaf costs one DRAM round trip, not two dependent ones
+  int64_t e = (int64_t)blockIdx.x * (blockDim.x >> 5) + w;
+  int pk = 0, pn = 0;
+  if (e < n && lane < NF) {
+    pk = kind[(size_t)e * NF + lane];
+    pn = nbr[(size_t)e * NF + lane];
+  }
+  for (; e < n; e += nw) {
     __syncwarp();
     if (lane < NF) {
-      s_kd[w][lane] = kind[(size_t)e * NF + lane];
-      s_nb[w][lane] = nbr[(size_t)e * NF + lane];
+      s_kd[w][lane] = pk;
+      s_nb[w][lane] = pn;
+      if (e + nw < n) {
+        pk = kind[(size_t)(e + nw) * NF + lane];
+        pn = nbr[(size_t)(e + nw) * NF + lane];
+      }
     }
     __syncwarp();
     V* dst = reinterpret_cast<V*>(unb + (size_t)e * NF * E);
