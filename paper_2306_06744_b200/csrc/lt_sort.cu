@@ -76,14 +76,29 @@ __global__ void __launch_bounds__(ST) k_sort_pass(const uint64_t* __restrict__ i
     dig[k] = valid ? (int)((key[k] >> shift) & 255) : 256;
   }
   // stable rank of every key among the equal-digit keys of its warp (warp-striped order)
+  // all match operations are issued before the (serial, shared-memory) counter updates: MATCH
+  // has a long latency and the loop below would otherwise expose it SITEMS times
+  // (peers by 9 ballots over the digit bits rather than MATCH.ANY, whose latency grows with the
+  // number of distinct values in the warp -- about 28 of 32 for a random digit)
+  unsigned peers[SITEMS];
 #pragma unroll
   for (int k = 0; k < SITEMS; ++k) {
-    const unsigned peers = __match_any_sync(0xffffffffu, dig[k]);
-    const unsigned before = __popc(peers & lt_mask);
+    unsigned pm = 0xffffffffu;
+#pragma unroll
+    for (int b = 0; b < 9; ++b) {
+      const bool bit = (dig[k] >> b) & 1;
+      const unsigned vote = __ballot_sync(0xffffffffu, bit);
+      pm &= bit ? vote : ~vote;
+    }
+    peers[k] = pm;
+  }
+#pragma unroll
+  for (int k = 0; k < SITEMS; ++k) {
+    const unsigned before = __popc(peers[k] & lt_mask);
     unsigned pre = 0;
     if (dig[k] < 256) pre = wcnt[w * 256 + dig[k]];
     __syncwarp();
-    if (dig[k] < 256 && before == 0) wcnt[w * 256 + dig[k]] = pre + __popc(peers);
+    if (dig[k] < 256 && before == 0) wcnt[w * 256 + dig[k]] = pre + __popc(peers[k]);
     __syncwarp();
     rank[k] = pre + before;
   }
