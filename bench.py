@@ -511,20 +511,28 @@ def run_construct(args):
     dom = [pc["lo"]] * dim + [pc["hi"]] * dim
     pts = W.surface_points(pc, device=dev)
     h_pts = pts.cpu().pin_memory()
+    d_in = torch.empty_like(pts)                                           # e2e: upload target
+    h_out = torch.empty(pts.shape[0], dtype=torch.int64).pin_memory()      # e2e: keys back (leaves <= points here)
     stream = torch.cuda.current_stream(dev)
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
 
     def step(from_host=False):
         torch.cuda.synchronize(dev)
         ev[0].record(stream)
-        x = h_pts.to(dev, non_blocking=True) if from_host else pts
+        if from_host:
+            d_in.copy_(h_pts, non_blocking=True)
+        x = d_in if from_host else pts
         t = lt.build_from_points(dim, pc["base"], pc["maxl"], x, dom, pc["periodic"])
         ev[1].record(stream)
         n0 = t.num_leaves()
         it = t.balance()
         ev[2].record(stream)
         F = t.connect()
-        h_keys = t.keys().cpu() if from_host else None
+        h_keys = None
+        if from_host:
+            k = t.keys()
+            h_keys = h_out[:k.numel()]
+            h_keys.copy_(k, non_blocking=True)
         ev[3].record(stream)
         torch.cuda.synchronize(dev)
         r = dict(n0=n0, n1=t.num_leaves(), iters=it, faces=int(F["n_conf"] + F["n_hang"] + F["n_bnd"]),

@@ -6,7 +6,9 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
+#include <vector>
 
 #include "lt_internal.h"
 
@@ -53,6 +55,37 @@ void dev_free(void* p, cudaStream_t s) {
 }
 
 static void free_dev(cudaStream_t s, void* p) { dev_free(p, s); }
+
+// Pinned host mirrors (device scalars + chunk sums) are recycled through a small process-wide
+// cache: cudaMallocHost / cudaFreeHost cost hundreds of microseconds each, which is most of the
+// host time of building a tree from points.
+constexpr size_t kMirrorBytes = 256 + (3 * kMaxGrid + 16) * sizeof(unsigned long long);
+static std::mutex g_mirror_mu;
+static std::vector<void*> g_mirror_free;
+
+static void* mirror_get() {
+  {
+    std::lock_guard<std::mutex> lk(g_mirror_mu);
+    if (!g_mirror_free.empty()) {
+      void* p = g_mirror_free.back();
+      g_mirror_free.pop_back();
+      return p;
+    }
+  }
+  void* p = nullptr;
+  if (cudaMallocHost(&p, kMirrorBytes) != cudaSuccess) {
+    cudaGetLastError();
+    return nullptr;
+  }
+  return p;
+}
+
+static void mirror_put(void* p) {
+  if (!p) return;
+  std::lock_guard<std::mutex> lk(g_mirror_mu);
+  if (g_mirror_free.size() < 16) g_mirror_free.push_back(p);
+  else cudaFreeHost(p);
+}
 
 template <typename T>
 static int alloc_dev(cudaStream_t s, T** p, int64_t count) {
@@ -204,9 +237,10 @@ static int new_tree(int dim, int base, int maxl, const double* domain, const int
   if ((rc = alloc_dev(t->stream, &t->d_s, 1)) != LT_OK) return fail(rc);
   if ((rc = alloc_dev(t->stream, &t->d_sums, kMaxGrid)) != LT_OK) return fail(rc);
   if ((rc = alloc_dev(t->stream, &t->d_sums3, 3 * kMaxGrid)) != LT_OK) return fail(rc);
-  if (cudaMallocHost((void**)&t->h_s, sizeof(DevScalars)) != cudaSuccess) return fail(LT_ERR_OOM);
-  if (cudaMallocHost((void**)&t->h_sums, (3 * kMaxGrid + 16) * sizeof(unsigned long long)) != cudaSuccess)
-    return fail(LT_ERR_OOM);
+  static_assert(sizeof(DevScalars) <= 256, "mirror layout");
+  t->h_s = (DevScalars*)mirror_get();  // one pinned block: scalars | chunk sums
+  if (!t->h_s) return fail(LT_ERR_OOM);
+  t->h_sums = (int*)((char*)t->h_s + 256);
   memset(t->h_s, 0, sizeof(DevScalars));
   if (cudaMemsetAsync(t->d_s, 0, sizeof(DevScalars), t->stream) != cudaSuccess) return fail(LT_ERR_CUDA);
   for (int i = 0; i < 16; ++i)
@@ -282,8 +316,7 @@ void lt_free(lt_tree* t) {
     free_dev(t->stream, t->first[b]);
   }
   free_dev(t->stream, t->d_s); free_dev(t->stream, t->d_sums); free_dev(t->stream, t->d_sums3);
-  if (t->h_s) cudaFreeHost(t->h_s);
-  if (t->h_sums) cudaFreeHost(t->h_sums);
+  mirror_put(t->h_s);
   free_dev(t->stream, t->mark); free_dev(t->stream, t->frontier[0]); free_dev(t->stream, t->frontier[1]);
   free_dev(t->stream, t->nbr); free_dev(t->stream, t->kind);
   free_dev(t->stream, t->face_rows); free_dev(t->stream, t->face_bytes); free_dev(t->stream, t->tile_state);
