@@ -512,7 +512,7 @@ def run_construct(args):
     pts = W.surface_points(pc, device=dev)
     h_pts = pts.cpu().pin_memory()
     d_in = torch.empty_like(pts)                                           # e2e: upload target
-    h_out = torch.empty(pts.shape[0], dtype=torch.int64).pin_memory()      # e2e: keys back (leaves <= points here)
+    h_out = torch.empty(max(pts.shape[0], 1 << 22), dtype=torch.int64).pin_memory()  # e2e: keys back
     stream = torch.cuda.current_stream(dev)
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
 
@@ -531,6 +531,8 @@ def run_construct(args):
         h_keys = None
         if from_host:
             k = t.keys()
+            if k.numel() > h_out.numel():
+                raise SystemExit("bench.py: the e2e key buffer is smaller than the tree (sparse cloud)")
             h_keys = h_out[:k.numel()]
             h_keys.copy_(k, non_blocking=True)
         ev[3].record(stream)
