@@ -157,6 +157,16 @@ int lt_balance(lt_tree*, int* iters);
  * LT_ERR_UNBALANCED if a level jump > 1 is met.  Synchronises. */
 int lt_connect(lt_tree*, lt_faces* out);
 
+/* The same query split in two so that it can overlap lt_transfer (both depend only on the
+ * balanced tree): lt_connect_begin enqueues the connectivity kernel on a side stream owned by
+ * the tree, ordered after everything already enqueued on the tree's stream, and returns at once;
+ * lt_connect_end makes the tree's stream wait for it, synchronises and fills *out exactly as
+ * lt_connect does.  Calls enqueued between the two (typically lt_transfer) run concurrently
+ * with the face query; lt_adapt / lt_balance / lt_reserve / lt_free join it first.
+ * lt_connect_end without a pending begin: LT_ERR_ARG. */
+int lt_connect_begin(lt_tree*);
+int lt_connect_end(lt_tree*, lt_faces* out);
+
 /* Alg. 7 + section 4.2: maps T_old -> current tree and moves the
  * solution: copy (same ID), interpolation of the parent's Lagrange expansion at the
  * child's solution points (Eq. 8), L2 projection of the 2^dim children (Eq. 9-13).

@@ -289,6 +289,15 @@ static int complete_from_unsorted(Tree* t, uint64_t* work, int64_t n) {
 
 using namespace lt;
 
+// main stream waits for an lt_connect_begin that has not been collected yet
+static int join_side(Tree* t) {
+  if (t->connect_pending) {
+    LT_CUDA(cudaStreamWaitEvent(t->stream, t->ev_side_join, 0));
+    t->connect_pending = false;
+  }
+  return LT_OK;
+}
+
 extern "C" {
 
 int lt_version(void) { return 100; }
@@ -310,6 +319,12 @@ const char* lt_strerror(int status) {
 
 void lt_free(lt_tree* t) {
   if (!t) return;
+  if (t->s_side) {
+    cudaStreamSynchronize(t->s_side);
+    cudaStreamDestroy(t->s_side);
+    cudaEventDestroy(t->ev_side_fork);
+    cudaEventDestroy(t->ev_side_join);
+  }
   cudaStreamSynchronize(t->stream);
   for (int b = 0; b < 3; ++b) {
     free_dev(t->stream, t->keys[b]);
@@ -360,6 +375,7 @@ int lt_build(int dim, int base_level, int max_level, const double* domain, const
 }
 
 int lt_reserve(lt_tree* t, int64_t n_leaves) {
+  if (t && join_side(t) != LT_OK) return LT_ERR_CUDA;
   if (!t || n_leaves < 0) return LT_ERR_ARG;
   if (!t->n_valid) {
     int rc = fetch_scalars(t);
@@ -448,6 +464,7 @@ int lt_decode(int dim, int max_level, const uint64_t* d_keys, int64_t n, int32_t
 int lt_adapt(lt_tree* t, const int8_t* d_flags) {
   if (!t || !d_flags) return LT_ERR_ARG;
   int rc;
+  if ((rc = join_side(t)) != LT_OK) return rc;
   if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
   tic(t, 0);
   const int G = grid_for(t, 8);
@@ -512,6 +529,7 @@ int lt_adapt(lt_tree* t, const int8_t* d_flags) {
 int lt_balance(lt_tree* t, int* iters) {
   if (!t) return LT_ERR_ARG;
   int rc;
+  if ((rc = join_side(t)) != LT_OK) return rc;
   if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
   tic(t, 1);
   int total_iters = 0;
@@ -548,14 +566,8 @@ int lt_balance(lt_tree* t, int* iters) {
 }
 
 // ---------------------------------------------------------------------------- connect
-int lt_connect(lt_tree* t, lt_faces* out) {
-  if (!t || !out) return LT_ERR_ARG;
+static int collect_faces(Tree* t, lt_faces* out) {
   int rc;
-  if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
-  tic(t, 2);
-  tic(t, 6);
-  if ((rc = launch_connect(t)) != LT_OK) return rc;
-  toc(t, 6);
   if ((rc = fetch_scalars(t)) != LT_OK) return rc;
   const int st = take_status(t);
   if (st != LT_OK) return st;
@@ -577,9 +589,58 @@ int lt_connect(lt_tree* t, lt_faces* out) {
     out->bnd = bnd;
     out->bnd_face = bnd_face;
   }
-  toc(t, 2);
   t->faces_valid = true;
   return LT_OK;
+}
+
+int lt_connect(lt_tree* t, lt_faces* out) {
+  if (!t || !out) return LT_ERR_ARG;
+  int rc;
+  if ((rc = join_side(t)) != LT_OK) return rc;
+  if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
+  tic(t, 2);
+  tic(t, 6);
+  if ((rc = launch_connect(t, t->stream, 0)) != LT_OK) return rc;
+  toc(t, 6);
+  rc = collect_faces(t, out);
+  toc(t, 2);
+  return rc;
+}
+
+// The face query depends only on the balanced tree, and so does the solution transfer: begin
+// enqueues k_connect on a side stream (a quarter of the SM resources, so that the HBM-bound
+// transfer kernel launched next on the main stream runs beside it), end joins and reads the counts.
+int lt_connect_begin(lt_tree* t) {
+  if (!t) return LT_ERR_ARG;
+  int rc;
+  if ((rc = join_side(t)) != LT_OK) return rc;
+  if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
+  if (!t->s_side) {
+    LT_CUDA(cudaStreamCreateWithFlags(&t->s_side, cudaStreamNonBlocking));
+    LT_CUDA(cudaEventCreateWithFlags(&t->ev_side_fork, cudaEventDisableTiming));
+    LT_CUDA(cudaEventCreateWithFlags(&t->ev_side_join, cudaEventDisableTiming));
+  }
+  t->faces_valid = false;
+  LT_CUDA(cudaEventRecord(t->ev_side_fork, t->stream));
+  LT_CUDA(cudaStreamWaitEvent(t->s_side, t->ev_side_fork, 0));
+  cudaEventRecord(t->ev[12], t->s_side);
+  // 3 of the 8 resident blocks per SM: measured best on config 5 (1: the query outlasts the transfer,
+  // 4+: the transfer loses more than the query gains); LT_SIDE_BLOCKS overrides for experiments
+  static const int side_blocks = getenv("LT_SIDE_BLOCKS") ? atoi(getenv("LT_SIDE_BLOCKS")) : 3;
+  if ((rc = launch_connect(t, t->s_side, side_blocks)) != LT_OK) return rc;
+  cudaEventRecord(t->ev[13], t->s_side);
+  t->ev_set[6] = true;
+  t->ev_set[2] = false;  // the call has no duration of its own in this mode
+  LT_CUDA(cudaEventRecord(t->ev_side_join, t->s_side));
+  t->connect_pending = true;
+  return LT_OK;
+}
+
+int lt_connect_end(lt_tree* t, lt_faces* out) {
+  if (!t || !out || !t->connect_pending) return LT_ERR_ARG;
+  int rc;
+  if ((rc = join_side(t)) != LT_OK) return rc;
+  return collect_faces(t, out);
 }
 
 // ---------------------------------------------------------------------------- mortars

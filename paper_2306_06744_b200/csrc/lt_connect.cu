@@ -246,26 +246,27 @@ void face_regions(const Tree* t, int32_t** conf, uint8_t** conf_axis, int32_t** 
   *bnd_face = t->face_bytes + 2 * dc;
 }
 
-int launch_connect(Tree* t) {
+int launch_connect(Tree* t, cudaStream_t stream, int blocks_per_sm) {
   int32_t *conf, *hang, *bnd;
   uint8_t *conf_axis, *hang_info, *bnd_face;
   face_regions(t, &conf, &conf_axis, &hang, &hang_info, &bnd, &bnd_face);
   const int64_t ntiles = (t->n + CT - 1) / CT;
-  LT_CUDA(cudaMemsetAsync(t->tile_state, 0, (size_t)(ntiles + 1) * 2 * sizeof(unsigned long long), t->stream));
-  LT_CUDA(cudaMemsetAsync(&t->d_s->ticket, 0, sizeof(unsigned), t->stream));
+  LT_CUDA(cudaMemsetAsync(t->tile_state, 0, (size_t)(ntiles + 1) * 2 * sizeof(unsigned long long), stream));
+  LT_CUDA(cudaMemsetAsync(&t->d_s->ticket_c, 0, sizeof(unsigned), stream));
   const void* fn = t->g.dim == 2 ? (const void*)k_connect<2> : (const void*)k_connect<3>;
   int per_sm = 0;
   LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, CT, 0));
   if (per_sm < 1) per_sm = 1;
+  if (blocks_per_sm > 0 && blocks_per_sm < per_sm) per_sm = blocks_per_sm;
   const int G = t->num_sms * per_sm;
   if (t->g.dim == 2)
-    k_connect<2><<<G, CT, 0, t->stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->nbr, t->kind, conf,
+    k_connect<2><<<G, CT, 0, stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->nbr, t->kind, conf,
                                           conf_axis, hang, hang_info, bnd, bnd_face, t->tile_state,
-                                          &t->d_s->ticket);
+                                          &t->d_s->ticket_c);
   else
-    k_connect<3><<<G, CT, 0, t->stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->nbr, t->kind, conf,
+    k_connect<3><<<G, CT, 0, stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->nbr, t->kind, conf,
                                           conf_axis, hang, hang_info, bnd, bnd_face, t->tile_state,
-                                          &t->d_s->ticket);
+                                          &t->d_s->ticket_c);
   t->launches++;
   LT_CUDA(cudaGetLastError());
   return LT_OK;

@@ -19,7 +19,8 @@ struct DevScalars {
   int aux;               // scratch counter (path-A append cursor, sort tickets)
   unsigned long long volume;  // build_from_keys: sum of leaf volumes
   int splits;            // balance: leaves split in total
-  unsigned ticket;       // tile ticket of the persistent kernels (zeroed before each launch)
+  unsigned ticket;       // tile ticket of k_transfer (zeroed before each launch)
+  unsigned ticket_c;     // tile ticket of k_connect (its own word: the two kernels may overlap)
 };
 
 constexpr int kMaxGrid = 4096;  // upper bound on persistent grid sizes (chunk-sum arrays)
@@ -63,6 +64,10 @@ struct Tree {
   uint8_t* map_kind;
   bool map_valid;
   bool faces_valid;       // nbr / kind describe the current tree (set by lt_connect)
+  // lt_connect_begin / lt_connect_end: k_connect on a side stream, overlapping lt_transfer
+  cudaStream_t s_side;
+  cudaEvent_t ev_side_fork, ev_side_join;
+  bool connect_pending;
   int* mortar_hits;       // [hits][2 + 2^(dim-1)]: coarse-side hanging faces (e, f, fine neighbours)
   int64_t mortar_hits_cap;
 
@@ -114,7 +119,7 @@ int launch_decode(int dim, int maxl, const uint64_t* d_keys, int64_t n, int32_t*
 int launch_check_tiling(Tree* t);
 
 // ---- lt_connect.cu
-int launch_connect(Tree* t);
+int launch_connect(Tree* t, cudaStream_t stream, int blocks_per_sm /* 0 = full occupancy */);
 void face_regions(const Tree* t, int32_t** conf, uint8_t** conf_axis, int32_t** hang, uint8_t** hang_info,
                   int32_t** bnd, uint8_t** bnd_face);
 

@@ -50,6 +50,8 @@ SIGNATURES = {
     "lt_adapt": (_I, [_P, _P]),
     "lt_balance": (_I, [_P, C.POINTER(_I)]),
     "lt_connect": (_I, [_P, C.POINTER(lt_faces)]),
+    "lt_connect_begin": (_I, [_P]),
+    "lt_connect_end": (_I, [_P, C.POINTER(lt_faces)]),
     "lt_transfer": (_I, [_P, _P, _P, _I, _I]),
     "lt_transfer_host": (_I, [_P, _P, _P, _I, _I]),
     "lt_mortar_project": (_I, [_P, _P, _P, _I, _I]),
@@ -192,6 +194,19 @@ class Tree:
         """lt_connect: dict of zero-copy views (valid until the next mutating call)."""
         F = lt_faces()
         _check(lib().lt_connect(self._h, C.byref(F)), "lt_connect")
+        return self._faces_dict(F)
+
+    def connect_begin(self):
+        """lt_connect_begin: enqueue the face query on the tree's side stream (overlaps lt_transfer)."""
+        _check(lib().lt_connect_begin(self._h), "lt_connect_begin")
+
+    def connect_end(self) -> dict:
+        """lt_connect_end: join the side stream and return the same dict as connect()."""
+        F = lt_faces()
+        _check(lib().lt_connect_end(self._h, C.byref(F)), "lt_connect_end")
+        return self._faces_dict(F)
+
+    def _faces_dict(self, F) -> dict:
         M, nf, dev = F.n_leaves, self.nf, self.device
         return dict(
             n_leaves=M, n_conf=F.n_conf, n_hang=F.n_hang, n_bnd=F.n_bnd,

@@ -315,3 +315,35 @@ def test_capacity_growth():
     gt.reserve(100000)
     P.assert_keys_equal(gt, ot, "after reserve")
     P.assert_faces_equal(gt.connect(), ot.connect(), "after reserve")
+
+
+def test_connect_begin_end_overlaps_transfer():
+    # lt_connect_begin / lt_transfer / lt_connect_end: the face query runs on the tree's side stream
+    # beside the transfer; faces, map and solution must equal the oracle's, cycle after cycle
+    cfg = dict(W.CONFIGS["c4"], base=3, maxl=6)
+    gt, ot = P.new_pair(cfg)
+    p, nvars = cfg["p"], cfg["nvars"]
+    uo = P.initial_u(cfg, ot)
+    with pytest.raises(lt.LtError):
+        gt.connect_end()  # nothing pending
+    for c in range(4):
+        f = P.host_flags(cfg, c, ot)
+        ot.adapt(f); ot.balance()
+        gt.adapt(torch.from_numpy(f).cuda()); gt.balance()
+        gt.connect_begin()
+        un_g = gt.transfer(torch.from_numpy(uo).cuda(), p, nvars)
+        Fg = gt.connect_end()
+        P.assert_faces_equal(Fg, ot.connect(), "cycle %d faces (async)" % c)
+        un_o = ot.transfer(uo, p, nvars)
+        gt.sync()
+        P.assert_u_close(un_g, un_o, "cycle %d transfer beside the face query" % c)
+        uo = un_o
+    # a pending query is joined by the next mutating call; the mortar calls refuse stale faces
+    gt.connect_begin()
+    with pytest.raises(lt.LtError):
+        gt.mortar_project(torch.zeros((gt.num_leaves(), 6, 1, 4), dtype=torch.float64, device="cuda"), 1, 1)
+    f = P.host_flags(cfg, 4, ot)
+    ot.adapt(f); ot.balance()
+    gt.adapt(torch.from_numpy(f).cuda()); gt.balance()
+    P.assert_keys_equal(gt, ot, "adapt after an uncollected connect_begin")
+    P.assert_faces_equal(gt.connect(), ot.connect(), "sync connect afterwards")
