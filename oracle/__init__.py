@@ -103,6 +103,8 @@ def lib():
         L.lto_mortar_project.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_int, C.c_int]
         L.lto_mortar_gather.restype = C.c_int
         L.lto_mortar_gather.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_int, C.c_int]
+        L.lto_face_interp.restype = C.c_int
+        L.lto_face_interp.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_int, C.c_int]
         L.lto_face_operators.restype = C.c_int
         L.lto_face_operators.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_double)]
         L.lto_gauss_legendre.restype = None
@@ -305,6 +307,16 @@ class Tree:
         self.build_map()
         out = self.transfer_rows(u_old, p, nvars, 0, self.num_leaves())
         lib().lto_drop_snapshot(self._h)
+        return out
+
+    def face_interp(self, u, p, nvars):
+        """Alg. 8 step 1: u [M, nvars, N] -> u_face [M, nf, nvars, Nf] (solution at the face points)."""
+        N, Nf = (p + 1) ** self.dim, (p + 1) ** (self.dim - 1)
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        assert u.shape == (self.num_leaves(), nvars, N)
+        out = np.zeros((self.num_leaves(), self.nf, nvars, Nf))
+        if lib().lto_face_interp(self._h, _p(u, C.c_double), _p(out, C.c_double), p, nvars) != 0:
+            raise OracleError("oracle face_interp: bad arguments")
         return out
 
     def mortar_project(self, u_face, p, nvars):

@@ -940,6 +940,51 @@ int mortar_gather(Tree* t, const FaceOps& fo, const double* fm, double* ff, int 
   return 0;
 }
 
+
+// Alg. 8 step 1: "Interpolate the solution from interior solution points to local
+// flux points."  The solution of an element is the tensor Lagrange expansion on its (p+1)^dim
+// Gauss-Legendre points (Eq. 8 / reading E-1); the flux points of face f are the Gauss-Legendre
+// points of the face (reading H-1), i.e. the reference point xi with xi_axis = -1 (f even) or +1
+// (f odd) and the tangential coordinates z[n_t].  Evaluated directly:
+//   u_f[e][f][v][n] = sum_m l_m(xi_n) u[e][v][m].
+void face_interp(const Tree* t, int p, const double* u, double* uf, int nvars) {
+  const int dim = t->dim, nf = t->nf, P1 = p + 1;
+  int N = 1, Nf = 1;
+  for (int a = 0; a < dim; ++a) N *= P1;
+  for (int a = 0; a + 1 < dim; ++a) Nf *= P1;
+  std::vector<double> z, w;
+  gauss_legendre(P1, z, w);
+  const int64_t M = (int64_t)t->leaves.size();
+  for (int f = 0; f < nf; ++f) {
+    const int axis = f >> 1;
+    // row n of the face operator: values of the N volume basis functions at face point n
+    std::vector<double> op((size_t)Nf * N);
+    for (int n = 0; n < Nf; ++n) {
+      double xi[3] = {0, 0, 0};
+      int r = n;
+      for (int a = 0; a < dim; ++a) {
+        if (a == axis) {
+          xi[a] = (f & 1) ? 1.0 : -1.0;
+        } else {
+          xi[a] = z[r % P1];
+          r /= P1;
+        }
+      }
+      for (int m = 0; m < N; ++m) op[(size_t)n * N + m] = tensor_lagrange(z, dim, m, xi);
+    }
+    for (int64_t e = 0; e < M; ++e)
+      for (int v = 0; v < nvars; ++v) {
+        const double* src = u + ((size_t)e * nvars + v) * N;
+        double* dst = uf + (((size_t)e * nf + f) * nvars + v) * Nf;
+        for (int n = 0; n < Nf; ++n) {
+          double acc = 0.0;
+          for (int m = 0; m < N; ++m) acc += op[(size_t)n * N + m] * src[m];
+          dst[n] = acc;
+        }
+      }
+  }
+}
+
 }  // namespace
 
 // ======================================================================= C ABI
@@ -1170,6 +1215,11 @@ int lto_mortar_gather(void* h, const double* fm, double* ff, int p, int nvars) {
   FaceOps fo;
   build_face_ops(fo, t->dim, p);
   return mortar_gather(t, fo, fm, ff, nvars);
+}
+int lto_face_interp(void* h, const double* u, double* uf, int p, int nvars) {
+  if (p < 0 || nvars < 1) return -1;
+  face_interp((Tree*)h, p, u, uf, nvars);
+  return 0;
 }
 int lto_face_operators(int dim, int p, int which, double* out) {
   if (dim != 2 && dim != 3) return -1;

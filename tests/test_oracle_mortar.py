@@ -75,7 +75,7 @@ def adapted_tree(dim, periodic, seed, base=2, maxl=4):
     return t
 
 
-def face_points(t, p):
+def face_points(t, p, wrap=True):
     """Physical coordinates [M, nf, Nf, dim] of every face's Gauss-Legendre points on the unit
     domain; the normal coordinate is the face plane taken modulo the domain (a periodic face and
     its image share it), tangential axes ascending, lower axis fastest (reading H-1)."""
@@ -96,7 +96,8 @@ def face_points(t, p):
                 for a in tang:
                     out[e, f, n, a] = (xyz[e, a] + 0.5 * w * (1 + z[r % P1])) / L
                     r //= P1
-                out[e, f, n, ax] = ((xyz[e, ax] + (w if f & 1 else 0.0)) % L) / L
+                plane = xyz[e, ax] + (w if f & 1 else 0.0)
+                out[e, f, n, ax] = ((plane % L) if wrap else plane) / L
     return out
 
 
@@ -163,3 +164,46 @@ def test_gather_conserves_random_fluxes(dim):
     for (e, f), val in coarse_int.items():
         assert (kind[e, f] & 15) == 3
         assert np.max(np.abs(ff[e, f] @ wf - val)) < 1e-13
+
+
+# ---------------------------------------------------------------- Alg. 8 step 1: volume -> face points
+def volume_points(t, p):
+    """Physical coordinates [M, N, dim] of the solution points (reading E-5: x fastest)."""
+    lvl, xyz = t.leaf_boxes()
+    dim, D = t.dim, t.maxl
+    z, _ = gl(p + 1)
+    P1 = p + 1
+    N = P1 ** dim
+    L = float(1 << D)
+    out = np.zeros((len(lvl), N, dim))
+    for n in range(N):
+        r = n
+        for a in range(dim):
+            out[:, n, a] = (xyz[:, a] + 0.5 * (1 << (D - lvl.astype(np.int64))) * (1 + z[r % P1])) / L
+            r //= P1
+    return out
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+@pytest.mark.parametrize("p", [0, 1, 2, 3])
+def test_face_interp_reproduces_polynomials(dim, p):
+    t = adapted_tree(dim, (0,) * dim, 3 + p)
+    XV, XF = volume_points(t, p), face_points(t, p, wrap=False)
+    u = np.stack([poly(XV, p, dim), 1.0 - 2.0 * poly(XV, p, dim)], axis=1)       # [M, 2, N]
+    want = np.stack([poly(XF, p, dim), 1.0 - 2.0 * poly(XF, p, dim)], axis=2)    # [M, nf, 2, Nf]
+    got = t.face_interp(u, p, 2)
+    assert np.max(np.abs(got - want)) < 1e-13 * max(1.0, np.max(np.abs(want)))
+
+
+def test_face_interp_p1_closed_form():
+    # p = 1: l_0(-1) = (1 + sqrt 3)/2, l_1(-1) = (1 - sqrt 3)/2 (Lagrange basis on +-1/sqrt 3), mirrored at +1
+    t = oracle.Tree(2, 0, 1)
+    a, b = (1 + np.sqrt(3.0)) / 2, (1 - np.sqrt(3.0)) / 2
+    u = np.arange(4, dtype=np.float64).reshape(1, 1, 4)  # u[iy*2 + ix]
+    uf = t.face_interp(u, 1, 1)[0, :, 0, :]
+    assert np.allclose(uf[0], [a * 0 + b * 1, a * 2 + b * 3], atol=1e-15)   # -x face, points along y
+    assert np.allclose(uf[1], [b * 0 + a * 1, b * 2 + a * 3], atol=1e-15)   # +x
+    assert np.allclose(uf[2], [a * 0 + b * 2, a * 1 + b * 3], atol=1e-15)   # -y face, points along x
+    assert np.allclose(uf[3], [b * 0 + a * 2, b * 1 + a * 3], atol=1e-15)   # +y
+    # constants are reproduced (the basis sums to one)
+    assert np.allclose(t.face_interp(np.ones((1, 3, 16)), 3, 3), 1.0, atol=1e-14)
