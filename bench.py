@@ -645,11 +645,17 @@ def run_mortar(args):
         uf[a:b] = (2.0 * W.counter_uniform(5, 21, i) - 1.0).view(b - a, nf, nvars, Nf)
         del i
     out = torch.empty_like(uf)
+    N = (p + 1) ** 3
+    u = torch.empty((M, nvars, N), dtype=torch.float64, device=dev)  # Alg. 8 step 1 input
+    R.analytic_u(u)
     stream = torch.cuda.current_stream(dev)
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    ms_i_all = []
 
     def step_once():
         torch.cuda.synchronize(dev)
+        ev[3].record(stream)
+        t.face_interp(u, p, nvars, u_face=out)
         ev[0].record(stream)
         t.mortar_project(uf, p, nvars, u_nb=out)
         ev[1].record(stream)
@@ -657,14 +663,18 @@ def run_mortar(args):
         ev[2].record(stream)
         torch.cuda.synchronize(dev)
         t.sync()
+        ms_i_all.append(ev[3].elapsed_time(ev[0]))
         return ev[0].elapsed_time(ev[1]), ev[1].elapsed_time(ev[2])
 
     for _ in range(max(args.warmup, 0)):
         step_once()
     sampler = ClockSampler(0)
     sampler.start()
+    del ms_i_all[:]
     times = [step_once() for _ in range(args.steps)]
     clocks = sampler.stop()
+    ms_i = sum(ms_i_all) / args.steps
+    bytes_i = (8 * nvars * N + nf * Bf) * M
     ms_p = sum(a for a, _ in times) / args.steps
     ms_g = sum(b for _, b in times) / args.steps
     bytes_p = 2 * Bf * (n1 + n2) + 5 * nf * M
@@ -696,11 +706,14 @@ def run_mortar(args):
                                "coarse-side hanging face slots), p=3, 5 fp64 vars, face arrays [M][6][5][16]"
                                % (M, n1, n2, n3),
                    "l2": "face arrays of %.1f GB each, larger than L2" % (uf.numel() * 8 / 1e9)},
-        "ms_per_call": {"mortar_project": ms_p, "mortar_gather": ms_g},
+        "ms_per_call": {"face_interp": ms_i, "mortar_project": ms_p, "mortar_gather": ms_g},
+        "face_interp": {"GBps": bytes_i / (ms_i * 1e-3) / 1e9, "bytes_per_launch": bytes_i,
+                        "frac": bytes_i / (ms_i * 1e-3) / 1e9 / peak,
+                        "note": "Alg. 8 step 1, timed before the mortar step; not part of `value`"},
         "roofline": {"bound": "hbm", "kernel": "k_mortar_project<3>", "achieved": ach, "peak": peak, "unit": "GB/s",
                      "frac": ach / peak, "traffic": None, "peak_source": peak_src, "bytes_per_launch": bytes_p,
                      "gather_GBps": bytes_g / (ms_g * 1e-3) / 1e9, "gather_bytes_per_launch": bytes_g},
-        "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": 2 * args.steps,
+        "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": 4 * args.steps,
         "e2e": None}), flush=True)
 
 

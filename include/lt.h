@@ -207,6 +207,13 @@ int lt_transfer_host(lt_tree*, const double* h_u_old, double* h_u_new, int p, in
  * mortars, which makes the result deterministic.  A missing fine neighbour sets the sticky
  * status LT_ERR_UNBALANCED (reported by lt_sync). */
 int lt_mortar_project(lt_tree*, const double* d_u_face, double* d_u_nb, int p, int nvars);
+
+/* Alg. 8 step 1: the solution at the face flux points,
+ *   d_u_face[e][f][v][n_t] = sum_i l_i(-1 | +1) d_u[e][v][.. i on the face's axis ..],
+ * d_u device [lt_num_leaves][nvars][(p+1)^dim] (layout of lt_transfer), d_u_face a face array as
+ * above; l_i = the Lagrange basis on the Gauss-Legendre solution points.  Needs no connectivity.
+ * The arrays must not overlap.  Asynchronous. */
+int lt_face_interp(lt_tree*, const double* d_u, double* d_u_face, int p, int nvars);
 int lt_mortar_gather(lt_tree*, const double* d_f_mortar, double* d_f_face, int p, int nvars);
 
 /* ---- accessors --------------------------------------------------------------------- */

@@ -658,6 +658,17 @@ static int mortar_call(lt_tree* t, int which, const double* d_in, double* d_out,
   return LT_OK;
 }
 
+int lt_face_interp(lt_tree* t, const double* d_u, double* d_u_face, int p, int nvars) {
+  if (!t || !d_u || !d_u_face || d_u == d_u_face || p < 0 || p > 7 || nvars < 1) return LT_ERR_ARG;
+  int rc;
+  if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
+  if ((rc = build_operators(t, p)) != LT_OK) return rc;
+  tic(t, 7);
+  if ((rc = launch_face_interp(t, d_u, d_u_face, p, nvars)) != LT_OK) return rc;
+  toc(t, 7);
+  return LT_OK;
+}
+
 int lt_mortar_project(lt_tree* t, const double* d_u_face, double* d_u_nb, int p, int nvars) {
   if (d_u_face == d_u_nb) return LT_ERR_ARG;
   return mortar_call(t, 0, d_u_face, d_u_nb, p, nvars);

@@ -129,6 +129,7 @@ int launch_transfer(Tree* t, const double* d_u_old, double* d_u_new, int p, int 
                     int64_t je = -1);
 int launch_slab_bounds(Tree* t, int64_t n_old, int64_t slab, int S, int64_t* d_out);
 int build_operators(Tree* t, int p);
+int launch_face_interp(Tree* t, const double* d_u, double* d_uf, int p, int nvars);
 int launch_mortar_hits(Tree* t);
 int launch_mortar(Tree* t, int which, const double* d_in, double* d_out, int p, int nvars);
 

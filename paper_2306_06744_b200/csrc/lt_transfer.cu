@@ -85,6 +85,9 @@ __global__ void k_map_identity(const DevScalars* __restrict__ s, int32_t* __rest
 //
 // c_ops[P1-1][which][row][col]: which 0,1 = I^0, I^1 (Eq. 8); 2,3 = R^0, R^1 (Eq. 12).
 __constant__ double c_ops[8][4][8][8];
+// c_edge[P1-1][side][i] = l_i(-1) (side 0) / l_i(+1) (side 1): the solution-point basis at the
+// element boundary (Alg. 8 step 1)
+__constant__ double c_edge[8][2][8];
 
 template <int P1> struct Pad {  // z-plane stride in shared memory (doubles): de-conflicts banks
   static constexpr int PP = P1 * P1;
@@ -547,6 +550,16 @@ int build_operators(Tree* t, int p) {
     }
   LT_CUDA(cudaMemcpyToSymbol(c_ops, h.data(), 4 * 64 * sizeof(double), (size_t)p * 4 * 64 * sizeof(double),
                              cudaMemcpyHostToDevice));
+  double he[2][8] = {{0}};
+  for (int side = 0; side < 2; ++side)
+    for (int i = 0; i < P1; ++i) {
+      const long double x = side ? 1.0L : -1.0L;
+      long double v = 1.0L;
+      for (int k = 0; k < P1; ++k)
+        if (k != i) v *= (x - z[k]) / (z[i] - z[k]);
+      he[side][i] = (double)v;
+    }
+  LT_CUDA(cudaMemcpyToSymbol(c_edge, he, sizeof(he), (size_t)p * sizeof(he), cudaMemcpyHostToDevice));
   uploaded[dev][p] = true;
   return LT_OK;
 }
@@ -882,6 +895,102 @@ int launch_mortar(Tree* t, int which, const double* d_in, double* d_out, int p, 
   const int G = t->num_sms * 8;
   const int rc = t->g.dim == 2 ? launch_mortar_d<2>(t, which, d_in, d_out, p, nvars, G)
                                : launch_mortar_d<3>(t, which, d_in, d_out, p, nvars, G);
+  if (rc != LT_OK) return rc;
+  t->launches++;
+  LT_CUDA(cudaGetLastError());
+  return LT_OK;
+}
+
+// ------------------------------------------------------------------------ Alg. 8 step 1
+// Solution at the face flux points (readings E-5, H-1): u_f[e][f][v][n_t] =
+// sum_i l_i(-1 | +1) u[e][v][.. i on the face's axis, n_t on the others ..].  One warp per leaf,
+// one variable at a time through shared memory; reads u once (coalesced), writes the nf face
+// blocks in full 128-bit sectors.  HBM-bound: Bu in, nf * Bf out per leaf.
+template <int DIM, int P1>
+__global__ void __launch_bounds__(256) k_face_interp(const DevScalars* s, const double* __restrict__ u,
+                                                     double* __restrict__ uf, int nvars, int vec2) {
+  constexpr int NF = Dim<DIM>::NF;
+  constexpr int N = DIM == 2 ? P1 * P1 : P1 * P1 * P1, Nf = DIM == 2 ? P1 : P1 * P1;
+  extern __shared__ double su_all[];  // [warps][nvars][N]: the whole element, staged once
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int EV = nvars * N, E = nvars * Nf;
+  double* su = su_all + (size_t)w * EV;
+  const int64_t n = s->n;
+  const int64_t nw = (int64_t)gridDim.x * (blockDim.x >> 5);
+  for (int64_t e = (int64_t)blockIdx.x * (blockDim.x >> 5) + w; e < n; e += nw) {
+    __syncwarp();
+    const double* src = u + (size_t)e * EV;
+    if (vec2) {
+      for (int i = lane; i < EV / 2; i += 32)
+        reinterpret_cast<double2*>(su)[i] = __ldcs(reinterpret_cast<const double2*>(src) + i);
+    } else {
+      for (int i = lane; i < EV; i += 32) su[i] = __ldcs(src + i);
+    }
+    __syncwarp();
+    double* dst = uf + (size_t)e * NF * E;
+    // outputs in memory order (f, v, n_t): consecutive lanes store consecutive doubles
+    for (int idx = lane; idx < NF * E; idx += 32) {
+      const int f = idx / E, r = idx - f * E;
+      const int v = r / Nf, nt = r - v * Nf;
+      const int axis = f >> 1, side = f & 1;
+      int base, stride;
+      if (DIM == 2) {  // tangential axis = the other one
+        stride = axis == 0 ? 1 : P1;
+        base = nt * (axis == 0 ? P1 : 1);
+      } else {
+        const int n1 = nt / P1, n0 = nt - n1 * P1;  // lower tangential axis fastest
+        stride = axis == 0 ? 1 : (axis == 1 ? P1 : P1 * P1);
+        const int s0 = axis == 0 ? P1 : 1;                 // stride of the lower tangential axis
+        const int s1 = axis == 2 ? P1 : P1 * P1;           // stride of the higher one
+        base = n0 * s0 + n1 * s1;
+      }
+      const double* sv = su + v * N + base;
+      double acc = 0.0;
+#pragma unroll
+      for (int i = 0; i < P1; ++i) acc += c_edge[P1 - 1][side][i] * sv[i * stride];
+      __stcs(dst + idx, acc);
+    }
+  }
+}
+
+template <int DIM, int P1>
+static int launch_face_interp_t(Tree* t, const double* d_u, double* d_uf, int nvars) {
+  constexpr int N = DIM == 2 ? P1 * P1 : P1 * P1 * P1;
+  int warps = 8;
+  const size_t per_warp = (size_t)nvars * N * sizeof(double);
+  while (warps > 1 && warps * per_warp > 64 * 1024) warps >>= 1;
+  const size_t smem = warps * per_warp;
+  if (smem > 200 * 1024) return LT_ERR_ARG;  // nvars * (p+1)^dim beyond one SM's shared memory
+  auto fn = k_face_interp<DIM, P1>;
+  LT_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int per_sm = 0;
+  LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, warps * 32, smem));
+  if (per_sm < 1) per_sm = 1;
+  const int vec2 = ((nvars * N) % 2 == 0) && (((uintptr_t)d_u) & 15) == 0;
+  fn<<<t->num_sms * per_sm, warps * 32, smem, t->stream>>>(t->d_s, d_u, d_uf, nvars, vec2);
+  return LT_OK;
+}
+
+template <int DIM>
+static int launch_face_interp_d(Tree* t, const double* d_u, double* d_uf, int p, int nvars, int G) {
+  switch (p) {
+    case 0: return launch_face_interp_t<DIM, 1>(t, d_u, d_uf, nvars);
+    case 1: return launch_face_interp_t<DIM, 2>(t, d_u, d_uf, nvars);
+    case 2: return launch_face_interp_t<DIM, 3>(t, d_u, d_uf, nvars);
+    case 3: return launch_face_interp_t<DIM, 4>(t, d_u, d_uf, nvars);
+    case 4: return launch_face_interp_t<DIM, 5>(t, d_u, d_uf, nvars);
+    case 5: return launch_face_interp_t<DIM, 6>(t, d_u, d_uf, nvars);
+    case 6: return launch_face_interp_t<DIM, 7>(t, d_u, d_uf, nvars);
+    case 7: return launch_face_interp_t<DIM, 8>(t, d_u, d_uf, nvars);
+    default: return LT_ERR_ARG;
+  }
+  return LT_OK;
+}
+
+int launch_face_interp(Tree* t, const double* d_u, double* d_uf, int p, int nvars) {
+  const int G = t->num_sms * 8;
+  const int rc = t->g.dim == 2 ? launch_face_interp_d<2>(t, d_u, d_uf, p, nvars, G)
+                               : launch_face_interp_d<3>(t, d_u, d_uf, p, nvars, G);
   if (rc != LT_OK) return rc;
   t->launches++;
   LT_CUDA(cudaGetLastError());

@@ -55,6 +55,7 @@ SIGNATURES = {
     "lt_transfer": (_I, [_P, _P, _P, _I, _I]),
     "lt_transfer_host": (_I, [_P, _P, _P, _I, _I]),
     "lt_mortar_project": (_I, [_P, _P, _P, _I, _I]),
+    "lt_face_interp": (_I, [_P, _P, _P, _I, _I]),
     "lt_mortar_gather": (_I, [_P, _P, _P, _I, _I]),
     "lt_num_leaves": (_I64, [_P]),
     "lt_num_old_leaves": (_I64, [_P]),
@@ -233,6 +234,16 @@ class Tree:
 
     def _face_shape(self, p, nvars):
         return (self.num_leaves(), self.nf, nvars, (p + 1) ** (self.dim - 1))
+
+    def face_interp(self, u: torch.Tensor, p: int, nvars: int, u_face: torch.Tensor = None) -> torch.Tensor:
+        """lt_face_interp (Alg. 8 step 1): u [M, nvars, N] -> u_face [M, nf, nvars, Nf]."""
+        if tuple(u.shape) != (self.num_leaves(), nvars, (p + 1) ** self.dim):
+            raise ValueError("lt_face_interp: u must be [%d, %d, %d]" % (self.num_leaves(), nvars, (p + 1) ** self.dim))
+        if u_face is None:
+            u_face = torch.empty(self._face_shape(p, nvars), dtype=torch.float64, device=self.device)
+        _check(lib().lt_face_interp(self._h, _dptr(u, torch.float64, "u"), _dptr(u_face, torch.float64, "u_face"),
+                                    p, nvars), "lt_face_interp")
+        return u_face
 
     def mortar_project(self, u_face: torch.Tensor, p: int, nvars: int, u_nb: torch.Tensor = None) -> torch.Tensor:
         """lt_mortar_project (Alg. 8 step 2): u_face [M, nf, nvars, Nf] -> neighbour traces; slots

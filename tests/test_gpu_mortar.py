@@ -119,3 +119,21 @@ def test_polynomial_trace_on_cycle_mesh():
     assert np.max(np.abs(unb[m12] - uf[m12])) < 1e-12
     ff = gt.mortar_gather(d, p, 1).cpu().numpy()
     assert (kind == 3).any() and np.max(np.abs(ff[kind == 3] - uf[kind == 3])) < 1e-12
+
+
+@pytest.mark.parametrize("dim,periodic,base,maxl", [(2, (1, 0), 2, 6), (3, (0, 0, 0), 2, 4)])
+@pytest.mark.parametrize("p,nvars", [(0, 2), (1, 1), (2, 4), (3, 5), (5, 3), (7, 2)])
+def test_face_interp_then_mortars(dim, periodic, base, maxl, p, nvars):
+    # Alg. 8 steps 1, 2, 4 chained: solution -> face points -> neighbour traces / gathered fluxes
+    gt, ot, rng = adapted_pair(dim, periodic, 17 * dim + p, base, maxl, cycles=2)
+    gt.connect(); ot.connect()
+    N = (p + 1) ** dim
+    u = rng.uniform(-1, 1, (ot.num_leaves(), nvars, N))
+    uf_o = ot.face_interp(u, p, nvars)
+    uf_g = gt.face_interp(torch.from_numpy(u).cuda(), p, nvars)
+    close(uf_g, uf_o, "face_interp")
+    close(gt.mortar_project(uf_g, p, nvars), ot.mortar_project(uf_o, p, nvars), "project after interp")
+    close(gt.mortar_gather(uf_g, p, nvars), ot.mortar_gather(uf_o, p, nvars), "gather after interp")
+    gt.sync()
+    with pytest.raises((lt.LtError, ValueError)):
+        gt.face_interp(uf_g, p, nvars)  # wrong shape
