@@ -63,15 +63,18 @@ def test_config5_full_size_cycle3():
             ot.drop_snapshot()
     M1 = ot.num_leaves()
     assert (M0, M1) == (8863051, 13473692)  # the step bench.py times first
-    # ---- connectivity, in full
-    Fg, Fo = gt.connect(), ot.connect()
+    # ---- connectivity, in full, in the form bench.py times it: the face query on the side stream
+    # beside the solution transfer (lt_connect_begin / lt_transfer / lt_connect_end)
+    gt.connect_begin()
+    un_g = gt.transfer(ug, p, nvars)
+    Fg = gt.connect_end()
+    Fo = ot.connect()
     P.assert_faces_equal(Fg, Fo, "c5 full size connect")
     nf = 6
     assert nf * M1 == 2 * Fo["n_conf"] + Fo["n_hang"] + Fo["n_hang"] // 4 + Fo["n_bnd"]
     del Fg, Fo
     # ---- map, in full; transfer on sampled slabs
     src_o, kind_o = ot.build_map()
-    un_g = gt.transfer(ug, p, nvars)
     gt.sync()
     src_g, kind_g = gt.map()
     assert np.array_equal(src_g.cpu().numpy(), src_o), "map src"
