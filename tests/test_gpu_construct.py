@@ -140,3 +140,40 @@ def test_cycle_runs_on_constructed_tree():
         gt.sync()
         P.assert_u_close(un_g, un_o, "cycle %d transfer" % c)
         uo = un_o
+
+
+@pytest.mark.parametrize("dim,maxl", [(2, 29), (3, 19)])
+def test_maximum_depth_trees(dim, maxl):
+    # key capacity (dim * max_level + 5 = 63 bits): construction, the full-depth ripple (one sweep per
+    # level), the face query and one adaptation cycle on a handful of points at the deepest level
+    rng = np.random.default_rng(maxl)
+    dom = [0.0] * dim + [1.0] * dim
+    pts = np.concatenate([rng.uniform(0, 1, (6, dim)), np.full((1, dim), 0.5 - 2.0 ** -30), np.zeros((1, dim)),
+                          np.ones((1, dim))])
+    ot = oracle.Tree(dim, 0, maxl, points=pts, domain=dom)
+    gt = lt.build_from_points(dim, 0, maxl, torch.from_numpy(pts).cuda(), dom)
+    P.assert_keys_equal(gt, ot, "deep completion")
+    assert int(P.u64(gt.keys()).max() >> np.uint64(dim * maxl + 4)) == 1  # the top key bit is in use
+    it_o, it_g = ot.balance(), gt.balance()
+    assert it_o == it_g and it_g >= maxl - 4
+    P.assert_keys_equal(gt, ot, "deep balance")
+    P.assert_faces_equal(gt.connect(), ot.connect(), "deep connect")
+    n_before = ot.num_leaves()
+    f = rng.integers(-1, 2, n_before).astype(np.int8)
+    ot.adapt(f); gt.adapt(torch.from_numpy(f).cuda())
+    assert ot.balance() == gt.balance()
+    P.assert_keys_equal(gt, ot, "deep cycle")
+    p, nvars = 1, 2
+    uo = rng.uniform(-1, 1, (n_before, nvars, (p + 1) ** dim))
+    un_o = ot.transfer(uo, p, nvars)
+    un_g = gt.transfer(torch.from_numpy(uo).cuda(), p, nvars)
+    gt.sync()
+    P.assert_u_close(un_g, un_o, "deep transfer")
+
+
+def test_empty_input_is_rejected():
+    dom = [0.0, 0.0, 1.0, 1.0]
+    with pytest.raises(lt.LtError):
+        lt.build_from_points(2, 1, 5, torch.empty((0, 2), dtype=torch.float64, device="cuda"), dom)
+    with pytest.raises(lt.LtError):
+        lt.build_complete_from_keys(2, 1, 5, torch.empty(0, dtype=torch.int64, device="cuda"))
