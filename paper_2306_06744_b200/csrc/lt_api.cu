@@ -1,7 +1,7 @@
 // lt_api.cu -- the C ABI of liblt (include/lt.h): argument checks, buffer management and
 // the sequence of kernel launches behind each call.  Product code; no CPU fallback: every
 // step of the path runs in the kernels of lt_tree.cu / lt_connect.cu / lt_transfer.cu /
-// lt_sort.cu.
+// lt_sort.cu / lt_construct.cu.
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>

@@ -8,6 +8,11 @@
 //                           R^b[j][i] = (w_i / (2 w_j)) I^b[i][j]
 // and the dim-dimensional operators are tensor products of the 1-D ones, applied one
 // direction at a time (sum factorisation).
+//
+// The same 1-D operators, one dimension lower, are the mortar projections of Alg. 8
+// (PAPER.md:265-314), so the face kernels live in this translation unit as well (they share
+// the operators in constant memory): k_face_interp (step 1), k_mortar_project (step 2,
+// Eq. 17), k_mortar_hits + k_mortar_apply (step 4, Eq. 20).
 #include <math.h>
 
 #include <vector>
