@@ -103,6 +103,12 @@ def lib():
         L.lto_mortar_project.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_int, C.c_int]
         L.lto_mortar_gather.restype = C.c_int
         L.lto_mortar_gather.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_int, C.c_int]
+        L.lto_common_flux.restype = C.c_int
+        L.lto_common_flux.argtypes = [C.c_void_p] + [C.POINTER(C.c_double)] * 3 + [C.c_int]
+        L.lto_fr_rhs.restype = C.c_int
+        L.lto_fr_rhs.argtypes = [C.c_void_p] + [C.POINTER(C.c_double)] * 4 + [C.c_int]
+        L.lto_fr_operators.restype = C.c_int
+        L.lto_fr_operators.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
         L.lto_face_interp.restype = C.c_int
         L.lto_face_interp.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_int, C.c_int]
         L.lto_face_operators.restype = C.c_int
@@ -173,6 +179,17 @@ def face_operators(dim, p):
         a = np.zeros((ns, N, N))
         if lib().lto_face_operators(dim, p, which, _p(a, C.c_double)) != 0:
             raise OracleError("oracle face operators: bad arguments")
+        out.append(a)
+    return tuple(out)
+
+
+def fr_operators(p):
+    """(D [P1,P1] = l_j'(z_i), l(-1) [P1], l(+1) [P1], g_L'(z) [P1], g_R'(z) [P1]) of Eq. 3-4 with Radau g."""
+    P1 = p + 1
+    out = []
+    for which, shape in enumerate([(P1, P1), (P1,), (P1,), (P1,), (P1,)]):
+        a = np.zeros(shape)
+        lib().lto_fr_operators(p, which, _p(a, C.c_double))
         out.append(a)
     return tuple(out)
 
@@ -317,6 +334,27 @@ class Tree:
         out = np.zeros((self.num_leaves(), self.nf, nvars, Nf))
         if lib().lto_face_interp(self._h, _p(u, C.c_double), _p(out, C.c_double), p, nvars) != 0:
             raise OracleError("oracle face_interp: bad arguments")
+        return out
+
+    def common_flux(self, u_face, u_nb, p):
+        """Alg. 8 step 3 (Rusanov, Euler): own and neighbour traces -> F* along +axis on kind 1 / 2 slots
+        (NaN elsewhere).  nvars = dim + 2."""
+        uf = np.ascontiguousarray(u_face, dtype=np.float64)
+        un = np.ascontiguousarray(u_nb, dtype=np.float64)
+        assert uf.shape == un.shape == (self.num_leaves(), self.nf, self.dim + 2, (p + 1) ** (self.dim - 1))
+        out = np.full(uf.shape, np.nan)
+        if lib().lto_common_flux(self._h, _p(uf, C.c_double), _p(un, C.c_double), _p(out, C.c_double), p) != 0:
+            raise OracleError("oracle common_flux: connect first")
+        return out
+
+    def fr_rhs(self, u, f_star, p, width):
+        """Eq. 2-5: u [M, dim+2, N], f_star [M, nf, dim+2, Nf] -> R [M, dim+2, N]."""
+        u = np.ascontiguousarray(u, dtype=np.float64)
+        fs = np.ascontiguousarray(f_star, dtype=np.float64)
+        wd = np.ascontiguousarray(width, dtype=np.float64)
+        assert u.shape == (self.num_leaves(), self.dim + 2, (p + 1) ** self.dim) and wd.size == self.dim
+        out = np.zeros(u.shape)
+        lib().lto_fr_rhs(self._h, _p(wd, C.c_double), _p(u, C.c_double), _p(fs, C.c_double), _p(out, C.c_double), p)
         return out
 
     def mortar_project(self, u_face, p, nvars):

@@ -985,6 +985,168 @@ void face_interp(const Tree* t, int p, const double* u, double* uf, int nvars) {
   }
 }
 
+
+// ---------------------------------------------------------------- FR right-hand side (Eq. 1-6)
+// The flux reconstruction update around the adaptation cycle, PAPER.md:51-76 (section 2.1) and
+// Alg. 8 step 3 ("we use a Rusanov solver"); readings I-1..I-5 of DESIGN.md.
+//  I-1  conservation law = compressible Euler (the paper's vortex test, Eq. 21),
+//       conserved variables (rho, rho u, rho v[, rho w], E), gamma = 1.4,
+//       p = (gamma-1)(E - rho |v|^2 / 2), flux along axis a:
+//       F_a = (rho v_a, rho v v_a + p e_a, (E + p) v_a).
+//  I-2  Rusanov common flux along +a between the minus-side state uL and the plus-side state uR:
+//       F* = (F_a(uL) + F_a(uR))/2 - lambda (uR - uL)/2, lambda = max(|v_a| + c) over both, c^2 = gamma p / rho.
+//  I-3  correction functions = Radau polynomials ("to recover the discontinuous Galerkin method",
+//       PAPER.md:67): g_L = (-1)^(k+1) (P_(k+1) - P_k)/2 (g_L(-1) = 1, g_L(1) = 0), g_R(xi) = g_L(-xi).
+//  I-4  Eq. 4-5 per axis: d f/dx = (2/dx) [ sum_j l_j'(z_i) f_j + g_L'(z_i)(F*_- - f(-1)) + g_R'(z_i)(F*_+ - f(1)) ],
+//       f(+-1) = sum_j l_j(+-1) f_j (Eq. 3), dx = domain width / 2^level ("inferred from the encoded
+//       information of each element"); R = - sum_a d F_a / d x_a.
+//  I-5  F* lives in the face array at the element's own slot (e, 2a) / (e, 2a+1), always as the
+//       flux along +a, at the face point whose tangential indices are those of the solution point.
+double legendre(int n, double x) {
+  double pm = 1.0, pc = x;
+  if (n == 0) return 1.0;
+  for (int k = 1; k < n; ++k) {
+    double pn = ((2 * k + 1) * x * pc - k * pm) / (k + 1);
+    pm = pc;
+    pc = pn;
+  }
+  return pc;
+}
+double legendre_d(int n, double x) {  // P_n'(x) = n (x P_n - P_(n-1)) / (x^2 - 1), interior x
+  if (n == 0) return 0.0;
+  return n * (x * legendre(n, x) - legendre(n - 1, x)) / (x * x - 1.0);
+}
+double lagrange_d(const std::vector<double>& z, int j, double x) {  // l_j'(x)
+  double s = 0.0;
+  for (size_t m = 0; m < z.size(); ++m) {
+    if ((int)m == j) continue;
+    double t = 1.0 / (z[j] - z[m]);
+    for (size_t k = 0; k < z.size(); ++k)
+      if ((int)k != j && k != m) t *= (x - z[k]) / (z[j] - z[k]);
+    s += t;
+  }
+  return s;
+}
+
+struct FrOps {
+  int p = -1;
+  std::vector<double> z, w, D, lm, lp, gl, gr;  // D[i][j] = l_j'(z_i); lm/lp[j] = l_j(-1/+1); gl/gr[i] = g_L'/g_R'(z_i)
+};
+void build_fr_ops(FrOps& o, int p) {
+  if (o.p == p) return;
+  const int P1 = p + 1;
+  o.p = p;
+  gauss_legendre(P1, o.z, o.w);
+  o.D.assign((size_t)P1 * P1, 0.0);
+  o.lm.assign(P1, 0.0); o.lp.assign(P1, 0.0); o.gl.assign(P1, 0.0); o.gr.assign(P1, 0.0);
+  const double sgn = ((p + 1) % 2) ? -1.0 : 1.0;  // (-1)^(k+1), k = p
+  for (int i = 0; i < P1; ++i) {
+    for (int j = 0; j < P1; ++j) o.D[(size_t)i * P1 + j] = lagrange_d(o.z, j, o.z[i]);
+    o.lm[i] = lagrange(o.z, i, -1.0);
+    o.lp[i] = lagrange(o.z, i, 1.0);
+    o.gl[i] = 0.5 * sgn * (legendre_d(p + 1, o.z[i]) - legendre_d(p, o.z[i]));
+    o.gr[i] = -0.5 * sgn * (legendre_d(p + 1, -o.z[i]) - legendre_d(p, -o.z[i]));  // d/dxi g_L(-xi)
+  }
+}
+
+constexpr double kGamma = 1.4;
+void euler_flux(int dim, int a, const double* u, double* F) {
+  const double rho = u[0], E = u[dim + 1];
+  double v[3] = {0, 0, 0}, q = 0.0;
+  for (int b = 0; b < dim; ++b) { v[b] = u[1 + b] / rho; q += v[b] * v[b]; }
+  const double pr = (kGamma - 1.0) * (E - 0.5 * rho * q);
+  F[0] = rho * v[a];
+  for (int b = 0; b < dim; ++b) F[1 + b] = u[1 + b] * v[a] + (b == a ? pr : 0.0);
+  F[dim + 1] = (E + pr) * v[a];
+}
+double wave_speed(int dim, int a, const double* u) {
+  const double rho = u[0], E = u[dim + 1];
+  double q = 0.0;
+  for (int b = 0; b < dim; ++b) q += (u[1 + b] / rho) * (u[1 + b] / rho);
+  const double pr = (kGamma - 1.0) * (E - 0.5 * rho * q);
+  return std::fabs(u[1 + a] / rho) + std::sqrt(kGamma * pr / rho);
+}
+void rusanov(int dim, int a, const double* uL, const double* uR, double* F) {
+  double FL[5], FR[5];
+  euler_flux(dim, a, uL, FL);
+  euler_flux(dim, a, uR, FR);
+  const double lam = std::max(wave_speed(dim, a, uL), wave_speed(dim, a, uR));
+  for (int v = 0; v < dim + 2; ++v) F[v] = 0.5 * (FL[v] + FR[v]) - 0.5 * lam * (uR[v] - uL[v]);
+}
+
+// Alg. 8 step 3 on every kind 1 / kind 2 slot: own trace u_f[e][f], neighbour trace u_nb[e][f]
+// (mortar_project); the minus-side state is the own one on an odd face, the neighbour's on an even one.
+void common_flux(Tree* t, int Nf, const double* uf, const double* unb, double* fs) {
+  const int dim = t->dim, nf = t->nf, nv = dim + 2;
+  const int64_t M = (int64_t)t->leaves.size();
+  for (int64_t e = 0; e < M; ++e)
+    for (int f = 0; f < nf; ++f) {
+      const size_t sl = (size_t)e * nf + f;
+      const int kd = t->faces.kind[sl] & 15;
+      if (kd != 1 && kd != 2) continue;
+      for (int n = 0; n < Nf; ++n) {
+        double own[5], nb[5], F[5];
+        for (int v = 0; v < nv; ++v) {
+          own[v] = uf[(sl * nv + v) * Nf + n];
+          nb[v] = unb[(sl * nv + v) * Nf + n];
+        }
+        if (f & 1) rusanov(dim, f >> 1, own, nb, F); else rusanov(dim, f >> 1, nb, own, F);
+        for (int v = 0; v < nv; ++v) fs[(sl * nv + v) * Nf + n] = F[v];
+      }
+    }
+}
+
+// Eq. 2-5 for every element; width[a] = physical domain width along axis a.
+void fr_rhs(Tree* t, const FrOps& o, const double* width, const double* u, const double* fs, double* R) {
+  const int dim = t->dim, nf = t->nf, nv = dim + 2, P1 = o.p + 1;
+  int N = 1, Nf = 1;
+  for (int a = 0; a < dim; ++a) N *= P1;
+  for (int a = 0; a + 1 < dim; ++a) Nf *= P1;
+  const int64_t M = (int64_t)t->leaves.size();
+  std::vector<double> F((size_t)N * nv);
+  for (int64_t e = 0; e < M; ++e) {
+    const double* ue = u + (size_t)e * nv * N;
+    double* Re = R + (size_t)e * nv * N;
+    for (int i = 0; i < nv * N; ++i) Re[i] = 0.0;
+    for (int a = 0; a < dim; ++a) {
+      const double dx = width[a] / (double)((uint64_t)1 << t->leaves[e]->level);
+      int stride = 1;
+      for (int b = 0; b < a; ++b) stride *= P1;
+      for (int n = 0; n < N; ++n) {  // flux along a at every solution point
+        double us[5], Fs[5];
+        for (int v = 0; v < nv; ++v) us[v] = ue[(size_t)v * N + n];
+        euler_flux(dim, a, us, Fs);
+        for (int v = 0; v < nv; ++v) F[(size_t)v * N + n] = Fs[v];
+      }
+      for (int n = 0; n < N; ++n) {
+        const int ia = (n / stride) % P1;          // index along a
+        const int line = n - ia * stride;          // first point of the line through n
+        int nt = 0, mul = 1, r = n;                // tangential face-point index (lower axis fastest)
+        for (int b = 0; b < dim; ++b) {
+          const int ib = r % P1;
+          r /= P1;
+          if (b == a) continue;
+          nt += ib * mul;
+          mul *= P1;
+        }
+        for (int v = 0; v < nv; ++v) {
+          double d = 0.0, fm = 0.0, fp = 0.0;
+          for (int j = 0; j < P1; ++j) {
+            const double fj = F[(size_t)v * N + line + j * stride];
+            d += o.D[(size_t)ia * P1 + j] * fj;
+            fm += o.lm[j] * fj;
+            fp += o.lp[j] * fj;
+          }
+          const double Fm = fs[((((size_t)e * nf + 2 * a) * nv) + v) * Nf + nt];
+          const double Fp = fs[((((size_t)e * nf + 2 * a + 1) * nv) + v) * Nf + nt];
+          d += o.gl[ia] * (Fm - fm) + o.gr[ia] * (Fp - fp);
+          Re[(size_t)v * N + n] -= (2.0 / dx) * d;
+        }
+      }
+    }
+  }
+}
+
 }  // namespace
 
 // ======================================================================= C ABI
@@ -1215,6 +1377,30 @@ int lto_mortar_gather(void* h, const double* fm, double* ff, int p, int nvars) {
   FaceOps fo;
   build_face_ops(fo, t->dim, p);
   return mortar_gather(t, fo, fm, ff, nvars);
+}
+// FR solver pieces around the cycle (Eq. 1-6, Alg. 8 step 3); Euler equations, nvars = dim + 2.
+int lto_common_flux(void* h, const double* uf, const double* unb, double* fs, int p) {
+  Tree* t = (Tree*)h;
+  if (t->faces.kind.size() != t->leaves.size() * (size_t)t->nf) return -2;
+  int Nf = 1;
+  for (int a = 0; a + 1 < t->dim; ++a) Nf *= p + 1;
+  common_flux(t, Nf, uf, unb, fs);
+  return 0;
+}
+int lto_fr_rhs(void* h, const double* width, const double* u, const double* fs, double* R, int p) {
+  FrOps o;
+  build_fr_ops(o, p);
+  fr_rhs((Tree*)h, o, width, u, fs, R);
+  return 0;
+}
+// which: 0 D [P1][P1], 1 l(-1) [P1], 2 l(+1) [P1], 3 g_L' [P1], 4 g_R' [P1]
+int lto_fr_operators(int p, int which, double* out) {
+  FrOps o;
+  build_fr_ops(o, p);
+  const std::vector<double>* v[5] = {&o.D, &o.lm, &o.lp, &o.gl, &o.gr};
+  if (which < 0 || which > 4) return -1;
+  std::memcpy(out, v[which]->data(), v[which]->size() * sizeof(double));
+  return 0;
 }
 int lto_face_interp(void* h, const double* u, double* uf, int p, int nvars) {
   if (p < 0 || nvars < 1) return -1;
