@@ -216,6 +216,27 @@ int lt_mortar_project(lt_tree*, const double* d_u_face, double* d_u_nb, int p, i
 int lt_face_interp(lt_tree*, const double* d_u, double* d_u_face, int p, int nvars);
 int lt_mortar_gather(lt_tree*, const double* d_f_mortar, double* d_f_face, int p, int nvars);
 
+/* ---- the flux-reconstruction update around the cycle (Eq. 1-6; Alg. 8 step 3) ---
+ * Compressible Euler equations, conserved variables (rho, rho u, rho v[, rho w], E), nvars = dim + 2,
+ * gamma = 1.4 (the paper's vortex test); readings I-1..I-5 of DESIGN.md.  Solution
+ * arrays [lt_num_leaves][dim+2][(p+1)^dim], face arrays [lt_num_leaves][nf][dim+2][(p+1)^(dim-1)].
+ *
+ * lt_common_flux -- Alg. 8 step 3 ("a Rusanov solver"): on every kind 1 / kind 2 slot
+ *   F* = (F_a(uL) + F_a(uR))/2 - max(|v_a| + c)(uR - uL)/2, the flux along +a (a = f >> 1); the minus-
+ *   side state uL is the element's own trace d_u_face on an odd face and the neighbour's trace d_u_nb
+ *   (lt_mortar_project) on an even one.  Kind 0 / 3 slots are left untouched (kind 3: lt_mortar_gather;
+ *   boundary conditions other than periodic are the caller's).  Needs lt_connect on the current tree.
+ * lt_fr_rhs -- Eq. 2-5 with Radau correction functions: R = - sum_a (2/dx_a) [ D f_a +
+ *   g_L' (F*_(a-) - f_a(-1)) + g_R' (F*_(a+) - f_a(+1)) ], dx_a = domain width / 2^level;
+ *   d_f_star holds the common flux along +a in the element's own slots 2a and 2a+1.
+ * lt_rk3_stage -- Eq. 6, stage = 1, 2, 3: d_u_out = a u_n + b (u_stage + dt R), (a, b) = (0, 1),
+ *   (3/4, 1/4), (1/3, 2/3); d_u_out may be d_u_stage.
+ * All three are asynchronous. */
+int lt_common_flux(lt_tree*, const double* d_u_face, const double* d_u_nb, double* d_f_star, int p);
+int lt_fr_rhs(lt_tree*, const double* d_u, const double* d_f_star, double* d_rhs, int p);
+int lt_rk3_stage(lt_tree*, int stage, double dt, const double* d_u_n, const double* d_u_stage,
+                 const double* d_rhs, double* d_u_out, int p);
+
 /* ---- accessors --------------------------------------------------------------------- */
 
 int64_t lt_num_leaves(lt_tree*);       /* synchronises only if the count is not cached   */

@@ -925,4 +925,37 @@ int lt_build_from_points(int dim, int base_level, int max_level, const double* d
   return LT_OK;
 }
 
+// ---------------------------------------------------------------------------- FR pieces (Eq. 1-6)
+int lt_common_flux(lt_tree* t, const double* d_u_face, const double* d_u_nb, double* d_f_star, int p) {
+  if (!t || !d_u_face || !d_u_nb || !d_f_star || p < 0 || p > 7) return LT_ERR_ARG;
+  if (!t->faces_valid) return LT_ERR_ARG;
+  tic(t, 7);
+  int rc = launch_common_flux(t, d_u_face, d_u_nb, d_f_star, p);
+  toc(t, 7);
+  return rc;
+}
+
+int lt_fr_rhs(lt_tree* t, const double* d_u, const double* d_f_star, double* d_rhs, int p) {
+  if (!t || !d_u || !d_f_star || !d_rhs || d_u == d_rhs || p < 0 || p > 7) return LT_ERR_ARG;
+  int rc;
+  if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
+  if ((rc = build_fr_operators(t, p)) != LT_OK) return rc;
+  tic(t, 7);
+  rc = launch_fr_rhs(t, d_u, d_f_star, d_rhs, p);
+  toc(t, 7);
+  return rc;
+}
+
+int lt_rk3_stage(lt_tree* t, int stage, double dt, const double* d_u_n, const double* d_u_stage, const double* d_rhs,
+                 double* d_u_out, int p) {
+  if (!t || !d_u_n || !d_u_stage || !d_rhs || !d_u_out || stage < 1 || stage > 3 || p < 0 || p > 7) return LT_ERR_ARG;
+  int rc;
+  if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
+  int64_t n = t->n * (t->g.dim + 2);
+  for (int a = 0; a < t->g.dim; ++a) n *= (p + 1);
+  const double a = stage == 1 ? 0.0 : (stage == 2 ? 0.75 : 1.0 / 3.0);
+  const double b = stage == 1 ? 1.0 : (stage == 2 ? 0.25 : 2.0 / 3.0);
+  return launch_rk_update(t, n, a, b, dt, d_u_n, d_u_stage, d_rhs, d_u_out);
+}
+
 }  // extern "C"

@@ -139,6 +139,13 @@ int launch_points_to_keys(int dim, int maxl, const double* domain, const double*
 int launch_complete_count(Tree* t, const uint64_t* d_in, int64_t n, uint32_t* d_offs, int64_t* total);
 int launch_complete_fill(Tree* t, const uint64_t* d_in, int64_t n, const uint32_t* d_offs, int64_t total);
 
+// ---- lt_fr.cu (Eq. 1-6, Alg. 8 step 3)
+int build_fr_operators(Tree* t, int p);
+int launch_common_flux(Tree* t, const double* d_uf, const double* d_unb, double* d_fs, int p);
+int launch_fr_rhs(Tree* t, const double* d_u, const double* d_fs, double* d_R, int p);
+int launch_rk_update(Tree* t, int64_t n, double a, double b, double dt, const double* un, const double* us,
+                     const double* R, double* out);
+
 // ---- lt_sort.cu
 struct SortScratch {
   uint64_t* tmp; int64_t cap; unsigned* hist; unsigned* status; int64_t status_cap; int* counter;

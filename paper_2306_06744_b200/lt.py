@@ -56,6 +56,9 @@ SIGNATURES = {
     "lt_transfer_host": (_I, [_P, _P, _P, _I, _I]),
     "lt_mortar_project": (_I, [_P, _P, _P, _I, _I]),
     "lt_face_interp": (_I, [_P, _P, _P, _I, _I]),
+    "lt_common_flux": (_I, [_P, _P, _P, _P, _I]),
+    "lt_fr_rhs": (_I, [_P, _P, _P, _P, _I]),
+    "lt_rk3_stage": (_I, [_P, _I, C.c_double, _P, _P, _P, _P, _I]),
     "lt_mortar_gather": (_I, [_P, _P, _P, _I, _I]),
     "lt_num_leaves": (_I64, [_P]),
     "lt_num_old_leaves": (_I64, [_P]),
@@ -244,6 +247,39 @@ class Tree:
         _check(lib().lt_face_interp(self._h, _dptr(u, torch.float64, "u"), _dptr(u_face, torch.float64, "u_face"),
                                     p, nvars), "lt_face_interp")
         return u_face
+
+    def common_flux(self, u_face: torch.Tensor, u_nb: torch.Tensor, p: int, f_star: torch.Tensor = None):
+        """lt_common_flux (Alg. 8 step 3, Rusanov / Euler): kind 1 / 2 slots of f_star (NaN-filled when
+        allocated here)."""
+        shp = self._face_shape(p, self.dim + 2)
+        if tuple(u_face.shape) != shp or tuple(u_nb.shape) != shp:
+            raise ValueError("lt_common_flux: face arrays must be %s" % (shp,))
+        if f_star is None:
+            f_star = torch.full_like(u_face, float("nan"))
+        _check(lib().lt_common_flux(self._h, _dptr(u_face, torch.float64, "u_face"), _dptr(u_nb, torch.float64, "u_nb"),
+                                    _dptr(f_star, torch.float64, "f_star"), p), "lt_common_flux")
+        return f_star
+
+    def fr_rhs(self, u: torch.Tensor, f_star: torch.Tensor, p: int, rhs: torch.Tensor = None) -> torch.Tensor:
+        """lt_fr_rhs (Eq. 2-5): u [M, dim+2, N], f_star face array -> R [M, dim+2, N]."""
+        if tuple(u.shape) != (self.num_leaves(), self.dim + 2, (p + 1) ** self.dim):
+            raise ValueError("lt_fr_rhs: u must be [M, dim+2, (p+1)^dim]")
+        if tuple(f_star.shape) != self._face_shape(p, self.dim + 2):
+            raise ValueError("lt_fr_rhs: f_star must be %s" % (self._face_shape(p, self.dim + 2),))
+        if rhs is None:
+            rhs = torch.empty_like(u)
+        _check(lib().lt_fr_rhs(self._h, _dptr(u, torch.float64, "u"), _dptr(f_star, torch.float64, "f_star"),
+                               _dptr(rhs, torch.float64, "rhs"), p), "lt_fr_rhs")
+        return rhs
+
+    def rk3_stage(self, stage: int, dt: float, u_n, u_stage, rhs, p: int, out=None):
+        """lt_rk3_stage (Eq. 6)."""
+        if out is None:
+            out = torch.empty_like(u_n)
+        _check(lib().lt_rk3_stage(self._h, stage, dt, _dptr(u_n, torch.float64, "u_n"),
+                                  _dptr(u_stage, torch.float64, "u_stage"), _dptr(rhs, torch.float64, "rhs"),
+                                  _dptr(out, torch.float64, "out"), p), "lt_rk3_stage")
+        return out
 
     def mortar_project(self, u_face: torch.Tensor, p: int, nvars: int, u_nb: torch.Tensor = None) -> torch.Tensor:
         """lt_mortar_project (Alg. 8 step 2): u_face [M, nf, nvars, Nf] -> neighbour traces; slots

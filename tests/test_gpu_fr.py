@@ -1,0 +1,145 @@
+"""GPU parity for the FR pieces around the cycle (Eq. 1-6; Alg. 8 step 3): Rusanov
+common flux, the right-hand side with Radau corrections, the SSP-RK3 stages, and the whole chain
+face_interp -> mortar_project -> common_flux -> mortar_gather -> fr_rhs, against the oracle.
+Tolerance: fluxes max|gpu - ref| <= 1e-12 * max(1, max|ref|); the right-hand side is a sum of terms of size
+(2/dx) |operator| |flux| that largely cancel, so its bound is 1e-12 * max(1, max|ref|, (2/dx_min) max|F*|)
+(reading I-6)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import parity as P
+from paper_2306_06744_b200 import lt
+from test_gpu_mortar import adapted_pair, close
+from test_oracle_fr import random_states
+
+pytestmark = pytest.mark.gpu
+
+
+def gpu_pipeline(gt, d_u, p):
+    nv = gt.dim + 2
+    uf = gt.face_interp(d_u, p, nv)
+    unb = gt.mortar_project(uf, p, nv)
+    fs = gt.common_flux(uf, unb, p)
+    gt.mortar_gather(fs, p, nv, f_face=fs)   # in place: the coarse-side hanging slots
+    return fs, gt.fr_rhs(d_u, fs, p)
+
+
+def close_rhs(got, want, fs, ot, what):
+    lvl, _ = ot.leaf_boxes()
+    scale = max(1.0, float(np.max(np.abs(want))), float(2 << int(lvl.max())) * float(np.nanmax(np.abs(fs))))
+    err = float(np.max(np.abs(got.cpu().numpy() - want)))
+    assert err <= 1e-12 * scale, "%s: error %.3e > 1e-12 * %.3g" % (what, err, scale)
+
+
+def oracle_pipeline(ot, u, p):
+    nv = ot.dim + 2
+    uf = ot.face_interp(u, p, nv)
+    unb = ot.mortar_project(uf, p, nv)
+    fs = ot.common_flux(uf, unb, p)
+    g = ot.mortar_gather(fs, p, nv)
+    fs = np.where(np.isnan(fs), g, fs)
+    return fs, ot.fr_rhs(u, fs, p, [1.0] * ot.dim)
+
+
+@pytest.mark.parametrize("dim,base,maxl", [(2, 2, 6), (3, 2, 4)])
+@pytest.mark.parametrize("p", [0, 1, 2, 3, 5, 7])
+def test_flux_rhs_and_chain_match_oracle(dim, base, maxl, p):
+    if dim == 3 and p == 7:
+        maxl = 3
+    gt, ot, rng = adapted_pair(dim, (1,) * dim, 51 * dim + p, base, maxl, cycles=2)
+    gt.connect(); ot.connect()
+    M, N, Nf, nv = ot.num_leaves(), (p + 1) ** dim, (p + 1) ** (dim - 1), dim + 2
+    # (1) common flux on random admissible traces
+    a = np.moveaxis(random_states(rng, (M, 2 * dim, Nf), dim), -1, 2).copy()
+    b = np.moveaxis(random_states(rng, (M, 2 * dim, Nf), dim), -1, 2).copy()
+    close(gt.common_flux(torch.from_numpy(a).cuda(), torch.from_numpy(b).cuda(), p), ot.common_flux(a, b, p), "common_flux")
+    # (2) right-hand side on random states and random common fluxes
+    u = np.moveaxis(random_states(rng, (M, N), dim), -1, 1).copy()
+    fs = rng.uniform(-1, 1, (M, 2 * dim, nv, Nf))
+    close_rhs(gt.fr_rhs(torch.from_numpy(u).cuda(), torch.from_numpy(fs).cuda(), p), ot.fr_rhs(u, fs, p, [1.0] * dim),
+              fs, ot, "fr_rhs")
+    # (3) the whole chain, on a smooth admissible state (a random one stops being admissible once it
+    # is extrapolated to the faces: negative densities, NaN wave speeds)
+    lvl, xyz = ot.leaf_boxes()
+    z, _ = np.polynomial.legendre.leggauss(p + 1)
+    Lw = float(1 << ot.maxl)
+    wd = (1 << (ot.maxl - lvl.astype(np.int64))) / Lw
+    X = np.zeros((M, N, dim))
+    for n in range(N):
+        r = n
+        for a2 in range(dim):
+            X[:, n, a2] = xyz[:, a2] / Lw + 0.5 * wd * (1 + z[r % (p + 1)])
+            r //= p + 1
+    ph = 2 * np.pi * X
+    rho = 1.0 + 0.2 * np.prod(np.sin(ph), axis=-1)
+    vel = np.stack([0.4 + 0.1 * np.cos(ph[..., (a2 + 1) % dim]) for a2 in range(dim)], axis=-1)
+    pr = 1.0 + 0.1 * np.cos(ph[..., 0])
+    u = np.concatenate([rho[:, None], np.moveaxis(rho[..., None] * vel, -1, 1),
+                        (pr / 0.4 + 0.5 * rho * np.sum(vel * vel, -1))[:, None]], axis=1).copy()
+    fs_g, R_g = gpu_pipeline(gt, torch.from_numpy(u).cuda(), p)
+    fs_o, R_o = oracle_pipeline(ot, u, p)
+    close(fs_g, fs_o, "chain: common fluxes")
+    close_rhs(R_g, R_o, fs_o, ot, "chain: rhs")
+    gt.sync()
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_free_stream_and_rk3_on_gpu(dim):
+    p = 3 if dim == 2 else 2
+    gt, ot, rng = adapted_pair(dim, (1,) * dim, 7, 2, 5 if dim == 2 else 4, cycles=2)
+    gt.connect()
+    M, N = ot.num_leaves(), (p + 1) ** dim
+    state = random_states(np.random.default_rng(2), (), dim)
+    u = torch.from_numpy(np.tile(state[None, :, None], (M, 1, N))).cuda()
+    _, R = gpu_pipeline(gt, u, p)
+    assert float(R.abs().max()) < 1e-9
+    # Eq. 6 against the formula, with arbitrary arrays
+    un, us, r = (torch.from_numpy(rng.uniform(-1, 1, (M, dim + 2, N))).cuda() for _ in range(3))
+    dt = 0.37
+    for stage, (ca, cb) in enumerate([(0.0, 1.0), (0.75, 0.25), (1.0 / 3.0, 2.0 / 3.0)], start=1):
+        want = ca * un + cb * (us + dt * r)
+        got = gt.rk3_stage(stage, dt, un, us, r, p)
+        assert float((got - want).abs().max()) < 1e-15
+    inplace = us.clone()
+    gt.rk3_stage(2, dt, un, inplace, r, p, out=inplace)
+    assert float((inplace - (0.75 * un + 0.25 * (us + dt * r))).abs().max()) < 1e-15
+
+
+def test_full_step_conserves_mass_momentum_energy():
+    # one SSP-RK3 step of the isentropic-vortex-like state on an adapted periodic mesh with hanging
+    # faces: the mortar projections are conservative, so the domain integrals of all
+    # conserved variables are unchanged to round-off
+    dim, p = 2, 2
+    gt, ot, rng = adapted_pair(dim, (1, 1), 3, 3, 6, cycles=2)
+    F = gt.connect()
+    assert int(F["n_hang"]) > 0
+    lvl, xyz = gt.leaf_boxes()
+    M, N = lvl.numel(), (p + 1) ** dim
+    z, w = np.polynomial.legendre.leggauss(p + 1)
+    L = float(1 << 6)
+    wd = (1 << (6 - lvl.cpu().numpy().astype(np.int64))) / L
+    X = np.zeros((M, N, 2))
+    for n in range(N):
+        X[:, n, 0] = xyz[:, 0].cpu().numpy() / L + 0.5 * wd * (1 + z[n % (p + 1)])
+        X[:, n, 1] = xyz[:, 1].cpu().numpy() / L + 0.5 * wd * (1 + z[n // (p + 1)])
+    rho = 1.0 + 0.2 * np.sin(2 * np.pi * X[..., 0]) * np.cos(2 * np.pi * X[..., 1])
+    vx, vy, pr = 0.5 + 0.1 * np.cos(2 * np.pi * X[..., 1]), -0.3 + 0.1 * np.sin(2 * np.pi * X[..., 0]), 1.0
+    U = np.stack([rho, rho * vx, rho * vy, pr / 0.4 + 0.5 * rho * (vx ** 2 + vy ** 2)], axis=1)
+    un = torch.from_numpy(U).cuda()
+    wv = torch.from_numpy(np.kron(w, w)).cuda()
+    vol = torch.from_numpy((wd / 2) ** 2).cuda()
+
+    def integral(u):
+        return ((u @ wv) * vol[:, None]).sum(0)
+
+    dt = 1e-3
+    _, R = gpu_pipeline(gt, un, p)
+    u1 = gt.rk3_stage(1, dt, un, un, R, p)
+    _, R = gpu_pipeline(gt, u1, p)
+    u2 = gt.rk3_stage(2, dt, un, u1, R, p)
+    _, R = gpu_pipeline(gt, u2, p)
+    u3 = gt.rk3_stage(3, dt, un, u2, R, p)
+    assert float((u3 - un).abs().max()) > 1e-5                      # the step did something
+    assert float((integral(u3) - integral(un)).abs().max()) < 1e-13
