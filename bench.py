@@ -717,6 +717,116 @@ def run_mortar(args):
         "e2e": None}), flush=True)
 
 
+# --------------------------------------------------------------------------- solver leg
+def run_solver(args):
+    """--workload solver: SURVEY.md 8(f)-4, the paper's headline (adaptation below
+    2 % of wall clock in 3-D with one adaptation every 10 steps of the 3-stage RK scheme).
+    Config-5 mesh: one adaptation cycle (cycle 2: 1.9 M -> 8.86 M leaves, with the solution transfer),
+    then 10 SSP-RK3 steps (30 right-hand sides = Alg. 8 steps 1-4 + Eq. 2-5 + Eq. 6) on the adapted mesh."""
+    import torch
+    from paper_2306_06744_b200 import build as B
+    B.build()
+    from paper_2306_06744_b200 import workloads as W
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
+    global PREP_CYCLES
+    PREP_CYCLES = 2
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    cfg = W.CONFIGS["c5"]
+    R = Runner(cfg, dev)
+    p, nvars, nf = cfg["p"], cfg["nvars"], 6
+    N, Nf = (p + 1) ** 3, (p + 1) ** 2
+    stream = torch.cuda.current_stream(dev)
+
+    def timed(fn):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(dev)
+        e0.record(stream)
+        out = fn()
+        e1.record(stream)
+        torch.cuda.synchronize(dev)
+        return e0.elapsed_time(e1), out
+
+    def adapt_cycle():
+        """untimed set-up of the pre-adaptation state, then the timed cycle 2"""
+        M0 = R.prepare()
+        t = R.tree
+        u_old = torch.empty((M0, nvars, N), dtype=torch.float64, device=dev)
+        R.analytic_u(u_old)
+        f = R.flags(2)
+
+        def cyc():
+            t.adapt(f)
+            t.balance()
+            M1 = t.num_leaves()
+            u_new = torch.empty((M1, nvars, N), dtype=torch.float64, device=dev)
+            t.connect_begin()
+            t.transfer(u_old, p, nvars, u_new)
+            F = t.connect_end()
+            return u_new, F
+        ms, (u_new, F) = timed(cyc)
+        t.sync()
+        return ms, M0, u_new, F
+
+    adapt_cycle()                                  # warm-up (allocations, operators)
+    ms_adapt, M0, u, F = adapt_cycle()
+    t = R.tree
+    M = t.num_leaves()
+    uf = torch.empty((M, nf, nvars, Nf), dtype=torch.float64, device=dev)
+    fs = torch.empty_like(uf)
+    rhs, us = torch.empty_like(u), torch.empty_like(u)
+    dt = 2e-4  # finest cell 20 / 512, p = 3, |v| + c about 4.2: well inside the RK3 stability limit
+
+    def rhs_of(x):
+        t.face_interp(x, p, nvars, u_face=uf)
+        t.mortar_project(uf, p, nvars, u_nb=fs)
+        t.common_flux(uf, fs, p, f_star=fs)        # in place over the neighbour traces
+        t.mortar_gather(fs, p, nvars, f_face=fs)
+        t.fr_rhs(x, fs, p, rhs=rhs)
+
+    def rk3_step():
+        rhs_of(u)
+        t.rk3_stage(1, dt, u, u, rhs, p, out=us)
+        rhs_of(us)
+        t.rk3_stage(2, dt, u, us, rhs, p, out=us)
+        rhs_of(us)
+        t.rk3_stage(3, dt, u, us, rhs, p, out=u)
+
+    rk3_step()                                     # warm-up
+    ms_solve, _ = timed(lambda: [rk3_step() for _ in range(10)])
+    ms_rhs, _ = timed(lambda: rhs_of(u))
+    sampler = ClockSampler(0)
+    sampler.start()
+    ms_solve2, _ = timed(lambda: [rk3_step() for _ in range(10)])
+    clocks = sampler.stop()
+    ms_solve = min(ms_solve, ms_solve2)
+    assert bool(torch.isfinite(u).all()), "the solution blew up"
+    frac = ms_adapt / (ms_adapt + ms_solve)
+    Bu, Bf = 8 * nvars * N, 8 * nvars * Nf
+    # algorithmic bytes of one right-hand side + RK update: face_interp (Bu + 6 Bf) + project (~2 * 6 Bf) +
+    # common flux (3 * 6 Bf) + rhs (2 Bu + 6 Bf) + update (4 Bu)
+    bytes_stage = M * (7 * Bu + 6 * Bf * 7)
+    peak, peak_src = hbm_peak()
+    print(json.dumps({
+        "metric": "adaptation share of wall clock, one adaptation cycle per 10 SSP-RK3 steps (PAPER.md:449)",
+        "value": frac, "unit": "fraction", "n_gpus": 1, "steps": 1, "warmup": 1,
+        "ms_per_step": ms_adapt + ms_solve, "higher_is_better": False, "scaling": "weak", "vs_baseline": frac / 0.0194,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "solver: config-5 cycle 2 (%d -> %d leaves, p=3, 5 fp64 vars, Euler) + 10 RK3 steps "
+                               "(30 right-hand sides) on the adapted mesh" % (M0, M),
+                   "baseline": "paper Table 5, p2 D_max 8, RTX 2060: 81.39 s / 4193.54 s = 1.94 % (160 k elements)",
+                   "l2": "arrays of 22.7-34 GB, larger than L2"},
+        "ms_per_call": {"adaptation_cycle": ms_adapt, "ten_rk3_steps": ms_solve, "one_rhs_chain": ms_rhs},
+        "roofline": {"bound": "hbm", "kernel": "RK stage (face_interp, mortar_project, common_flux, mortar_gather, "
+                                               "fr_rhs, rk3_stage)", "achieved": bytes_stage * 30 / (ms_solve * 1e-3) / 1e9,
+                     "peak": peak, "unit": "GB/s", "frac": bytes_stage * 30 / (ms_solve * 1e-3) / 1e9 / peak,
+                     "traffic": None, "peak_source": peak_src, "bytes_per_launch": bytes_stage},
+        "elements_per_s_rhs": M * 30 / (ms_solve * 1e-3),
+        "cpu_baseline": None, "clocks": clocks, "gpu_launches": 30 * 7 + 6, "e2e": None}), flush=True)
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -725,7 +835,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--workload", default="cycle", choices=["cycle", "construct", "mortar"],
+    ap.add_argument("--workload", default="cycle", choices=["cycle", "construct", "mortar", "solver"],
                     help="cycle (default): the adaptation cycle BASELINE.json's metric is quoted on; construct: "
                          "tree construction from a point cloud (SURVEY.md 8(f)-1)")
     ap.add_argument("--cloud", default="pc10", help="point cloud of --workload construct (workloads.POINT_CLOUDS)")
@@ -753,6 +863,8 @@ def main():
         run_construct(args)
     elif args.workload == "mortar" and args.impl == "ours":
         run_mortar(args)
+    elif args.workload == "solver" and args.impl == "ours":
+        run_solver(args)
     elif args.impl == "reference":
         run_reference(args)
     else:

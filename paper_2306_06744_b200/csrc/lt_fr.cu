@@ -61,8 +61,8 @@ __device__ __forceinline__ double wave_speed(int a, const double* u) {
 // Alg. 8 step 3: one thread per (slot, face point).  Own trace on an odd face = minus side.
 template <int DIM>
 __global__ void __launch_bounds__(256) k_common_flux(const DevScalars* s, const uint8_t* __restrict__ kind,
-                                                     const double* __restrict__ uf, const double* __restrict__ unb,
-                                                     double* __restrict__ fs, int Nf) {
+                                                     const double* __restrict__ uf, const double* unb,
+                                                     double* fs, int Nf) {  // fs may be unb (in place)
   constexpr int NF = Dim<DIM>::NF, NV = DIM + 2;
   const int64_t total = (int64_t)s->n * NF * Nf;
   for (int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; idx < total;
@@ -160,8 +160,8 @@ __global__ void __launch_bounds__(256) k_fr_rhs(Geo g, const uint64_t* __restric
 
 // Eq. 6: u_out = a u_n + b (u_s + dt R), (a, b) = (0, 1), (3/4, 1/4), (1/3, 2/3) for stages 1, 2, 3.
 __global__ void __launch_bounds__(256) k_rk_update(int64_t n, double a, double b, double dt,
-                                                   const double* __restrict__ un, const double* us,
-                                                   const double* __restrict__ R, double* out) {
+                                                   const double* un, const double* us,
+                                                   const double* __restrict__ R, double* out) {  // out may be un / us
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
     out[i] = a * un[i] + b * (us[i] + dt * R[i]);
 }
