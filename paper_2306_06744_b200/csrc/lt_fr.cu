@@ -128,28 +128,34 @@ __global__ void __launch_bounds__(256) k_fr_rhs(Geo g, const uint64_t* __restric
         for (int v = 0; v < NV; ++v) sF[v * N + p] = Fp[v];
       }
       __syncwarp();
-      for (int idx = lane; idx < EV; idx += 32) {
-        const int v = idx / N, p = idx - v * N;
-        const int ia = (p / stride) % P1, line = p - ia * stride;
-        int nt;  // tangential face-point index, lower axis fastest
+      // one lane per LINE of P1 points along a: its P1 point fluxes are read once, f(-1), f(+1)
+      // and the two common fluxes are formed once per line, then the P1 derivatives
+      constexpr int LINES = NV * Nf;  // lines per element along one axis
+      for (int ln = lane; ln < LINES; ln += 32) {
+        const int v = ln / Nf, nt = ln - v * Nf;  // nt = tangential face-point index, lower axis fastest
+        int first;                                // first point of the line
         if (DIM == 2) {
-          nt = a == 0 ? p / P1 : p % P1;
+          first = a == 0 ? nt * P1 : nt;
         } else {
-          const int ix = p % P1, iy = (p / P1) % P1, iz = p / (P1 * P1);
-          nt = a == 0 ? iy + P1 * iz : (a == 1 ? ix + P1 * iz : ix + P1 * iy);
+          const int n0 = nt % P1, n1 = nt / P1;
+          first = a == 0 ? n0 * P1 + n1 * P1 * P1 : (a == 1 ? n0 + n1 * P1 * P1 : n0 + n1 * P1);
         }
-        double d = 0.0, fm = 0.0, fp = 0.0;
+        double fj[P1], fm = 0.0, fp = 0.0;
 #pragma unroll
         for (int j = 0; j < P1; ++j) {
-          const double fj = sF[v * N + line + j * stride];
-          d += c.D[ia][j] * fj;
-          fm += c.lm[j] * fj;
-          fp += c.lp[j] * fj;
+          fj[j] = sF[v * N + first + j * stride];
+          fm += c.lm[j] * fj[j];
+          fp += c.lp[j] * fj[j];
         }
-        const double Fm = fs[(((size_t)e * NF + 2 * a) * NV + v) * Nf + nt];
-        const double Fp = fs[(((size_t)e * NF + 2 * a + 1) * NV + v) * Nf + nt];
-        d += c.gl[ia] * (Fm - fm) + c.gr[ia] * (Fp - fp);
-        sR[idx] -= scale * d;
+        const double dm = fs[(((size_t)e * NF + 2 * a) * NV + v) * Nf + nt] - fm;
+        const double dp = fs[(((size_t)e * NF + 2 * a + 1) * NV + v) * Nf + nt] - fp;
+#pragma unroll
+        for (int i = 0; i < P1; ++i) {
+          double d = c.gl[i] * dm + c.gr[i] * dp;
+#pragma unroll
+          for (int j = 0; j < P1; ++j) d += c.D[i][j] * fj[j];
+          sR[v * N + first + i * stride] -= scale * d;
+        }
       }
     }
     __syncwarp();
