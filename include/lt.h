@@ -232,11 +232,15 @@ int lt_mortar_gather(lt_tree*, const double* d_f_mortar, double* d_f_face, int p
  *   d_f_star holds the common flux along +a in the element's own slots 2a and 2a+1.
  * lt_rk3_stage -- Eq. 6, stage = 1, 2, 3: d_u_out = a u_n + b (u_stage + dt R), (a, b) = (0, 1),
  *   (3/4, 1/4), (1/3, 2/3); d_u_out may be d_u_stage or d_u_n.
- * All three are asynchronous. */
+ * lt_fr_stage -- lt_fr_rhs and lt_rk3_stage in one pass: d_u_out = a u_n + b (u_stage + dt R(u_stage, F*));
+ *   the right-hand side never goes to memory.  d_u_out may be d_u_stage or d_u_n.
+ * All four are asynchronous. */
 int lt_common_flux(lt_tree*, const double* d_u_face, const double* d_u_nb, double* d_f_star, int p);
 int lt_fr_rhs(lt_tree*, const double* d_u, const double* d_f_star, double* d_rhs, int p);
 int lt_rk3_stage(lt_tree*, int stage, double dt, const double* d_u_n, const double* d_u_stage,
                  const double* d_rhs, double* d_u_out, int p);
+int lt_fr_stage(lt_tree*, int stage, double dt, const double* d_u_n, const double* d_u_stage,
+                const double* d_f_star, double* d_u_out, int p);
 
 /* ---- accessors --------------------------------------------------------------------- */
 

@@ -93,8 +93,11 @@ __global__ void __launch_bounds__(256) k_common_flux(const DevScalars* s, const 
 // element live in shared memory; the common fluxes come from the element's own face slots.
 template <int DIM, int P1>
 __global__ void __launch_bounds__(256) k_fr_rhs(Geo g, const uint64_t* __restrict__ keys, const DevScalars* s,
-                                                const double* __restrict__ u, const double* __restrict__ fs,
-                                                double* __restrict__ R, double w0, double w1, double w2) {
+                                                const double* u, const double* __restrict__ fs, double* R,
+                                                double w0, double w1, double w2, const double* un, double ca,
+                                                double cb, double dt) {
+  // un == nullptr: R = right-hand side.  Otherwise the RK stage of Eq. 6 is applied on the fly:
+  // R (= u_out) = ca * un + cb * (u + dt * rhs); u_out may be u or un (element-local access).
   constexpr int NF = Dim<DIM>::NF, NV = DIM + 2;
   constexpr int N = DIM == 2 ? P1 * P1 : P1 * P1 * P1, Nf = DIM == 2 ? P1 : P1 * P1, EV = NV * N;
   extern __shared__ double sm_all[];  // [warps][3][NV][N]: u | F | R
@@ -160,7 +163,12 @@ __global__ void __launch_bounds__(256) k_fr_rhs(Geo g, const uint64_t* __restric
     }
     __syncwarp();
     double* dst = R + (size_t)e * EV;
-    for (int i = lane; i < EV; i += 32) __stcs(dst + i, sR[i]);
+    if (un == nullptr) {
+      for (int i = lane; i < EV; i += 32) __stcs(dst + i, sR[i]);
+    } else {
+      const double* sn = un + (size_t)e * EV;
+      for (int i = lane; i < EV; i += 32) dst[i] = ca * sn[i] + cb * (su[i] + dt * sR[i]);
+    }
   }
 }
 
@@ -252,7 +260,8 @@ int launch_common_flux(Tree* t, const double* d_uf, const double* d_unb, double*
 }
 
 template <int DIM, int P1>
-static int launch_fr_rhs_t(Tree* t, const double* d_u, const double* d_fs, double* d_R) {
+static int launch_fr_rhs_t(Tree* t, const double* d_u, const double* d_fs, double* d_R, const double* d_un, double ca,
+                           double cb, double dt) {
   constexpr int N = DIM == 2 ? P1 * P1 : P1 * P1 * P1;
   int warps = 8;
   const size_t per_warp = (size_t)3 * (DIM + 2) * N * sizeof(double);
@@ -266,27 +275,30 @@ static int launch_fr_rhs_t(Tree* t, const double* d_u, const double* d_fs, doubl
   const double w0 = t->domain[DIM] - t->domain[0], w1 = t->domain[DIM + 1] - t->domain[1];
   const double w2 = DIM == 3 ? t->domain[DIM + 2] - t->domain[2] : 1.0;
   fn<<<t->num_sms * per_sm, warps * 32, smem, t->stream>>>(t->g, t->keys[t->cur], t->d_s, d_u, d_fs, d_R, w0, w1,
-                                                            w2);
+                                                            w2, d_un, ca, cb, dt);
   return LT_OK;
 }
 
 template <int DIM>
-static int launch_fr_rhs_d(Tree* t, const double* d_u, const double* d_fs, double* d_R, int p) {
+static int launch_fr_rhs_d(Tree* t, const double* d_u, const double* d_fs, double* d_R, int p, const double* d_un,
+                           double ca, double cb, double dt) {
   switch (p) {
-    case 0: return launch_fr_rhs_t<DIM, 1>(t, d_u, d_fs, d_R);
-    case 1: return launch_fr_rhs_t<DIM, 2>(t, d_u, d_fs, d_R);
-    case 2: return launch_fr_rhs_t<DIM, 3>(t, d_u, d_fs, d_R);
-    case 3: return launch_fr_rhs_t<DIM, 4>(t, d_u, d_fs, d_R);
-    case 4: return launch_fr_rhs_t<DIM, 5>(t, d_u, d_fs, d_R);
-    case 5: return launch_fr_rhs_t<DIM, 6>(t, d_u, d_fs, d_R);
-    case 6: return launch_fr_rhs_t<DIM, 7>(t, d_u, d_fs, d_R);
-    case 7: return launch_fr_rhs_t<DIM, 8>(t, d_u, d_fs, d_R);
+    case 0: return launch_fr_rhs_t<DIM, 1>(t, d_u, d_fs, d_R, d_un, ca, cb, dt);
+    case 1: return launch_fr_rhs_t<DIM, 2>(t, d_u, d_fs, d_R, d_un, ca, cb, dt);
+    case 2: return launch_fr_rhs_t<DIM, 3>(t, d_u, d_fs, d_R, d_un, ca, cb, dt);
+    case 3: return launch_fr_rhs_t<DIM, 4>(t, d_u, d_fs, d_R, d_un, ca, cb, dt);
+    case 4: return launch_fr_rhs_t<DIM, 5>(t, d_u, d_fs, d_R, d_un, ca, cb, dt);
+    case 5: return launch_fr_rhs_t<DIM, 6>(t, d_u, d_fs, d_R, d_un, ca, cb, dt);
+    case 6: return launch_fr_rhs_t<DIM, 7>(t, d_u, d_fs, d_R, d_un, ca, cb, dt);
+    case 7: return launch_fr_rhs_t<DIM, 8>(t, d_u, d_fs, d_R, d_un, ca, cb, dt);
   }
   return LT_ERR_ARG;
 }
 
-int launch_fr_rhs(Tree* t, const double* d_u, const double* d_fs, double* d_R, int p) {
-  const int rc = t->g.dim == 2 ? launch_fr_rhs_d<2>(t, d_u, d_fs, d_R, p) : launch_fr_rhs_d<3>(t, d_u, d_fs, d_R, p);
+int launch_fr_rhs(Tree* t, const double* d_u, const double* d_fs, double* d_R, int p, const double* d_un, double ca,
+                  double cb, double dt) {
+  const int rc = t->g.dim == 2 ? launch_fr_rhs_d<2>(t, d_u, d_fs, d_R, p, d_un, ca, cb, dt)
+                               : launch_fr_rhs_d<3>(t, d_u, d_fs, d_R, p, d_un, ca, cb, dt);
   if (rc != LT_OK) return rc;
   t->launches++;
   LT_CUDA(cudaGetLastError());

@@ -142,7 +142,8 @@ int launch_complete_fill(Tree* t, const uint64_t* d_in, int64_t n, const uint32_
 // ---- lt_fr.cu (Eq. 1-6, Alg. 8 step 3)
 int build_fr_operators(Tree* t, int p);
 int launch_common_flux(Tree* t, const double* d_uf, const double* d_unb, double* d_fs, int p);
-int launch_fr_rhs(Tree* t, const double* d_u, const double* d_fs, double* d_R, int p);
+int launch_fr_rhs(Tree* t, const double* d_u, const double* d_fs, double* d_R, int p, const double* d_un = nullptr,
+                  double ca = 0.0, double cb = 0.0, double dt = 0.0);
 int launch_rk_update(Tree* t, int64_t n, double a, double b, double dt, const double* un, const double* us,
                      const double* R, double* out);
 

@@ -59,6 +59,7 @@ SIGNATURES = {
     "lt_common_flux": (_I, [_P, _P, _P, _P, _I]),
     "lt_fr_rhs": (_I, [_P, _P, _P, _P, _I]),
     "lt_rk3_stage": (_I, [_P, _I, C.c_double, _P, _P, _P, _P, _I]),
+    "lt_fr_stage": (_I, [_P, _I, C.c_double, _P, _P, _P, _P, _I]),
     "lt_mortar_gather": (_I, [_P, _P, _P, _I, _I]),
     "lt_num_leaves": (_I64, [_P]),
     "lt_num_old_leaves": (_I64, [_P]),
@@ -279,6 +280,15 @@ class Tree:
         _check(lib().lt_rk3_stage(self._h, stage, dt, _dptr(u_n, torch.float64, "u_n"),
                                   _dptr(u_stage, torch.float64, "u_stage"), _dptr(rhs, torch.float64, "rhs"),
                                   _dptr(out, torch.float64, "out"), p), "lt_rk3_stage")
+        return out
+
+    def fr_stage(self, stage: int, dt: float, u_n, u_stage, f_star, p: int, out=None):
+        """lt_fr_stage: right-hand side + RK stage of Eq. 6 in one pass."""
+        if out is None:
+            out = torch.empty_like(u_n)
+        _check(lib().lt_fr_stage(self._h, stage, dt, _dptr(u_n, torch.float64, "u_n"),
+                                 _dptr(u_stage, torch.float64, "u_stage"), _dptr(f_star, torch.float64, "f_star"),
+                                 _dptr(out, torch.float64, "out"), p), "lt_fr_stage")
         return out
 
     def mortar_project(self, u_face: torch.Tensor, p: int, nvars: int, u_nb: torch.Tensor = None) -> torch.Tensor:

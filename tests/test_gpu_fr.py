@@ -102,6 +102,18 @@ def test_free_stream_and_rk3_on_gpu(dim):
         want = ca * un + cb * (us + dt * r)
         got = gt.rk3_stage(stage, dt, un, us, r, p)
         assert float((got - want).abs().max()) < 1e-15
+    # lt_fr_stage = lt_fr_rhs + lt_rk3_stage in one pass, also in place over u_stage / u_n
+    fs, R = gpu_pipeline(gt, un.abs() + 1.0 if False else u, p)
+    base_n = torch.from_numpy(rng.uniform(0.9, 1.1, (M, dim + 2, N))).cuda() * u
+    for stage in (1, 2, 3):
+        want = gt.rk3_stage(stage, dt, base_n, u, R, p)
+        got = gt.fr_stage(stage, dt, base_n, u, fs, p)
+        assert float((got - want).abs().max()) <= 1e-12 * max(1.0, float(want.abs().max()))
+        w1 = u.clone()
+        gt.fr_stage(stage, dt, base_n, w1, fs, p, out=w1)
+        w2 = base_n.clone()
+        gt.fr_stage(stage, dt, w2, u, fs, p, out=w2)
+        assert torch.equal(w1, got) and torch.equal(w2, got)
     inplace = us.clone()
     gt.rk3_stage(2, dt, un, inplace, r, p, out=inplace)
     assert float((inplace - (0.75 * un + 0.25 * (us + dt * r))).abs().max()) < 1e-15
@@ -135,11 +147,11 @@ def test_full_step_conserves_mass_momentum_energy():
         return ((u @ wv) * vol[:, None]).sum(0)
 
     dt = 1e-3
-    _, R = gpu_pipeline(gt, un, p)
+    fs, R = gpu_pipeline(gt, un, p)
     u1 = gt.rk3_stage(1, dt, un, un, R, p)
-    _, R = gpu_pipeline(gt, u1, p)
-    u2 = gt.rk3_stage(2, dt, un, u1, R, p)
-    _, R = gpu_pipeline(gt, u2, p)
-    u3 = gt.rk3_stage(3, dt, un, u2, R, p)
+    fs, _ = gpu_pipeline(gt, u1, p)
+    u2 = gt.fr_stage(2, dt, un, u1, fs, p)          # fused right-hand side + stage
+    fs, _ = gpu_pipeline(gt, u2, p)
+    u3 = gt.fr_stage(3, dt, un, u2, fs, p)
     assert float((u3 - un).abs().max()) > 1e-5                      # the step did something
     assert float((integral(u3) - integral(un)).abs().max()) < 1e-13
