@@ -115,6 +115,17 @@ __global__ void __launch_bounds__(256) k_fr_rhs(Geo g, const uint64_t* __restric
       su[i] = __ldcs(src + i);
       sR[i] = 0.0;
     }
+    // fused stage: u_n is fetched now, so that its latency hides behind the arithmetic
+    constexpr int KN = (EV + 31) / 32;
+    constexpr bool PREF = KN <= 16;
+    double pn[PREF ? KN : 1];
+    if (PREF && un != nullptr) {
+#pragma unroll
+      for (int k = 0; k < KN; ++k) {
+        const int i = lane + 32 * k;
+        pn[k] = i < EV ? __ldcs(un + (size_t)e * EV + i) : 0.0;
+      }
+    }
     const int level = key_level(keys[e]);
     const double inv2l = (double)(1ull << level);
 #pragma unroll
@@ -166,8 +177,16 @@ __global__ void __launch_bounds__(256) k_fr_rhs(Geo g, const uint64_t* __restric
     if (un == nullptr) {
       for (int i = lane; i < EV; i += 32) __stcs(dst + i, sR[i]);
     } else {
-      const double* sn = un + (size_t)e * EV;
-      for (int i = lane; i < EV; i += 32) dst[i] = ca * sn[i] + cb * (su[i] + dt * sR[i]);
+      if (PREF) {
+#pragma unroll
+        for (int k = 0; k < KN; ++k) {
+          const int i = lane + 32 * k;
+          if (i < EV) __stcs(dst + i, ca * pn[k] + cb * (su[i] + dt * sR[i]));
+        }
+      } else {
+        const double* sn = un + (size_t)e * EV;
+        for (int i = lane; i < EV; i += 32) dst[i] = ca * sn[i] + cb * (su[i] + dt * sR[i]);
+      }
     }
   }
 }
