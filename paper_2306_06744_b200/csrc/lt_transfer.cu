@@ -933,27 +933,31 @@ __global__ void __launch_bounds__(256) k_face_interp(const DevScalars* s, const 
     }
     __syncwarp();
     double* dst = uf + (size_t)e * NF * E;
-    // outputs in memory order (f, v, n_t): consecutive lanes store consecutive doubles
-    for (int idx = lane; idx < NF * E; idx += 32) {
-      const int f = idx / E, r = idx - f * E;
-      const int v = r / Nf, nt = r - v * Nf;
-      const int axis = f >> 1, side = f & 1;
-      int base, stride;
-      if (DIM == 2) {  // tangential axis = the other one
-        stride = axis == 0 ? 1 : P1;
-        base = nt * (axis == 0 ? P1 : 1);
-      } else {
-        const int n1 = nt / P1, n0 = nt - n1 * P1;  // lower tangential axis fastest
-        stride = axis == 0 ? 1 : (axis == 1 ? P1 : P1 * P1);
-        const int s0 = axis == 0 ? P1 : 1;                 // stride of the lower tangential axis
-        const int s1 = axis == 2 ? P1 : P1 * P1;           // stride of the higher one
-        base = n0 * s0 + n1 * s1;
-      }
-      const double* sv = su + v * N + base;
-      double acc = 0.0;
+    // one lane per LINE of P1 points along an axis: the line is read once and gives the trace on
+    // the minus AND the plus face of that axis; consecutive lanes store consecutive doubles
 #pragma unroll
-      for (int i = 0; i < P1; ++i) acc += c_edge[P1 - 1][side][i] * sv[i * stride];
-      __stcs(dst + idx, acc);
+    for (int a = 0; a < DIM; ++a) {
+      const int stride = a == 0 ? 1 : (a == 1 ? P1 : P1 * P1);
+      for (int ln = lane; ln < E; ln += 32) {
+        const int v = ln / Nf, nt = ln - v * Nf;
+        int first;
+        if (DIM == 2) {
+          first = a == 0 ? nt * P1 : nt;
+        } else {
+          const int n1 = nt / P1, n0 = nt - n1 * P1;  // lower tangential axis fastest
+          first = a == 0 ? n0 * P1 + n1 * P1 * P1 : (a == 1 ? n0 + n1 * P1 * P1 : n0 + n1 * P1);
+        }
+        const double* sv = su + v * N + first;
+        double lo = 0.0, hi = 0.0;
+#pragma unroll
+        for (int i = 0; i < P1; ++i) {
+          const double x = sv[i * stride];
+          lo += c_edge[P1 - 1][0][i] * x;
+          hi += c_edge[P1 - 1][1][i] * x;
+        }
+        __stcs(dst + (2 * a) * E + ln, lo);
+        __stcs(dst + (2 * a + 1) * E + ln, hi);
+      }
     }
   }
 }
