@@ -666,17 +666,21 @@ __global__ void __launch_bounds__(256) k_mortar_project(const DevScalars* s, con
       src[f] = reinterpret_cast<const V*>(uf + ((size_t)(conf[f] ? s_nb[w][f] : 0) * NF + (f ^ 1)) * E);
     }
     for (int q0 = 0; q0 < EV; q0 += 64) {
-      V v0[NF], v1[NF];
       const int qa = q0 + lane, qb = q0 + 32 + lane;
 #pragma unroll
-      for (int f = 0; f < NF; ++f) {
-        if (conf[f] && qa < EV) v0[f] = __ldcs(src[f] + qa);
-        if (conf[f] && qb < EV) v1[f] = __ldcs(src[f] + qb);
-      }
+      constexpr int FC = NF / 2;  // faces per round: 2 * FC loads in flight per lane (all NF at once costs 20 registers more and a resident block)
+      for (int fh = 0; fh < NF; fh += FC) {
+        V v0[FC], v1[FC];
 #pragma unroll
-      for (int f = 0; f < NF; ++f) {
-        if (conf[f] && qa < EV) __stcs(dst + f * EV + qa, v0[f]);
-        if (conf[f] && qb < EV) __stcs(dst + f * EV + qb, v1[f]);
+        for (int f = 0; f < FC; ++f) {
+          if (conf[fh + f] && qa < EV) v0[f] = __ldcs(src[fh + f] + qa);
+          if (conf[fh + f] && qb < EV) v1[f] = __ldcs(src[fh + f] + qb);
+        }
+#pragma unroll
+        for (int f = 0; f < FC; ++f) {
+          if (conf[fh + f] && qa < EV) __stcs(dst + (fh + f) * EV + qa, v0[f]);
+          if (conf[fh + f] && qb < EV) __stcs(dst + (fh + f) * EV + qb, v1[f]);
+        }
       }
     }
     if (any2) {
