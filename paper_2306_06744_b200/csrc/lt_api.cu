@@ -156,6 +156,7 @@ static int grow(Tree* t, int64_t need) {
   free_dev(t->stream, t->tile_state); t->tile_state = tstate;
   t->map_valid = false;
   t->faces_valid = false;
+  t->front_ok = false;  // the frontier buffers were reallocated
   t->cap = cap;
   return LT_OK;
 }
@@ -371,6 +372,7 @@ int lt_build(int dim, int base_level, int max_level, const double* domain, const
   t->n = nb;
   t->n_valid = true;
   *out = (lt_tree*)t;
+  t->balanced_conn = 3;  // a uniform tree is balanced for every connectivity
   return LT_OK;
 }
 
@@ -466,6 +468,7 @@ int lt_adapt(lt_tree* t, const int8_t* d_flags) {
   int rc;
   if ((rc = join_side(t)) != LT_OK) return rc;
   if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
+  bool front_ok = false;
   tic(t, 0);
   const int G = grid_for(t, 8);
   if ((rc = launch_adapt_count(t, d_flags, G)) != LT_OK) return rc;
@@ -483,8 +486,12 @@ int lt_adapt(lt_tree* t, const int8_t* d_flags) {
   const int64_t need = t->opt_adapt_sort ? n_kept + n_b : n_b;
   if ((rc = grow(t, need)) != LT_OK) return rc;
   if (!t->opt_adapt_sort) {
-    // path B: ordered expansion cur -> tmp
-    if ((rc = launch_adapt_scatter(t, d_flags, G, 0)) != LT_OK) return rc;
+    // path B: ordered expansion cur -> tmp.  If the tree was balanced, the leaves created here
+    // become the frontier of lt_balance's first sweep.
+    const int emit = t->balanced_conn >= 1;
+    if (emit) LT_CUDA(cudaMemsetAsync(&t->d_s->nfront0, 0, sizeof(int), t->stream));
+    if ((rc = launch_adapt_scatter(t, d_flags, G, 0, emit)) != LT_OK) return rc;
+    front_ok = emit != 0;
     const int o = t->old;
     t->old = t->cur;
     t->cur = t->tmp;
@@ -493,7 +500,7 @@ int lt_adapt(lt_tree* t, const int8_t* d_flags) {
   } else {
     // path A (Alg. 6 as printed): append -> radix sort -> linearise
     LT_CUDA(cudaMemsetAsync(&t->d_s->aux, 0, sizeof(int), t->stream));
-    if ((rc = launch_adapt_scatter(t, d_flags, G, 1)) != LT_OK) return rc;
+    if ((rc = launch_adapt_scatter(t, d_flags, G, 1, 0)) != LT_OK) return rc;
     if ((rc = fetch_scalars(t)) != LT_OK) return rc;
     t->n = n_in;  // fetch_scalars read the (unchanged) device count
     const int64_t n_app = n_kept + t->h_s->aux;
@@ -521,6 +528,8 @@ int lt_adapt(lt_tree* t, const int8_t* d_flags) {
   t->n_valid = true;
   t->map_valid = false;
   t->faces_valid = false;
+  t->front_ok = front_ok;
+  t->balanced_conn = 0;
   toc(t, 0);
   return LT_OK;
 }
@@ -532,12 +541,16 @@ int lt_balance(lt_tree* t, int* iters) {
   if ((rc = join_side(t)) != LT_OK) return rc;
   if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
   tic(t, 1);
+  const bool had_front = t->front_ok;  // consumed by this call whatever happens
+  t->front_ok = false;
   int total_iters = 0;
   int64_t slack = t->opt_debug_slack;
   for (int attempt = 0;; ++attempt) {
     // (testing aid: pretend the buffers hold only n + slack leaves, to exercise the retry)
     const int64_t cap_told = slack > 0 && t->n + slack < t->cap ? t->n + slack : t->cap;
-    if ((rc = launch_balance(t, cap_told)) != LT_OK) return rc;
+    const int conn = t->opt_balance_conn > 0 ? t->opt_balance_conn : 1;
+    const int use_front = attempt == 0 && had_front && conn == 1 && !t->opt_full_sweeps;
+    if ((rc = launch_balance(t, cap_told, use_front)) != LT_OK) return rc;
     if ((rc = fetch_scalars(t)) != LT_OK) return rc;
     if (t->h_s->parity) {
       const int c = t->cur;
@@ -559,6 +572,8 @@ int lt_balance(lt_tree* t, int* iters) {
     if ((rc = grow(t, t->cap * 2)) != LT_OK) return rc == LT_ERR_OOM ? LT_ERR_CAPACITY : rc;
   }
   if (iters) *iters = total_iters;
+  t->front_ok = false;
+  t->balanced_conn = t->opt_balance_conn > 0 ? t->opt_balance_conn : 1;
   t->map_valid = false;
   t->faces_valid = false;
   toc(t, 1);

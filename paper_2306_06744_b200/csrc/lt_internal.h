@@ -21,6 +21,7 @@ struct DevScalars {
   int splits;            // balance: leaves split in total
   unsigned ticket;       // tile ticket of k_transfer (zeroed before each launch)
   unsigned ticket_c;     // tile ticket of k_connect (its own word: the two kernels may overlap)
+  int nfront0;           // entries of lt_adapt's frontier for lt_balance's first sweep
 };
 
 constexpr int kMaxGrid = 4096;  // upper bound on persistent grid sizes (chunk-sum arrays)
@@ -68,6 +69,8 @@ struct Tree {
   cudaStream_t s_side;
   cudaEvent_t ev_side_fork, ev_side_join;
   bool connect_pending;
+  int balanced_conn;      // the tree is 2:1 balanced with this connectivity (0: unknown)
+  bool front_ok;          // frontier[0] / d_s->nfront0 list the leaves created by the last lt_adapt
   int* mortar_hits;       // [hits][2 + 2^(dim-1)]: coarse-side hanging faces (e, f, fine neighbours)
   int64_t mortar_hits_cap;
 
@@ -111,8 +114,8 @@ void dev_free(void* p, cudaStream_t s);
 int launch_build_uniform(Tree* t);
 int launch_build_index(Tree* t, int buf);
 int launch_adapt_count(Tree* t, const int8_t* d_flags, int G);
-int launch_adapt_scatter(Tree* t, const int8_t* d_flags, int G, int path_a);
-int launch_balance(Tree* t, int64_t cap_told);
+int launch_adapt_scatter(Tree* t, const int8_t* d_flags, int G, int path_a, int emit_front);
+int launch_balance(Tree* t, int64_t cap_told, int use_front);
 int launch_leaf_boxes(Tree* t, int32_t* d_level, uint32_t* d_xyz);
 int launch_encode(int dim, int maxl, const uint32_t* d_xyz, const int32_t* d_level, int64_t n, uint64_t* d_keys, cudaStream_t s);
 int launch_decode(int dim, int maxl, const uint64_t* d_keys, int64_t n, int32_t* d_level, uint32_t* d_xyz, cudaStream_t s);

@@ -176,7 +176,10 @@ __global__ void __launch_bounds__(BT) k_adapt_scatter(Geo g, const uint64_t* __r
                                                       const int8_t* __restrict__ flags, DevScalars* s,
                                                       const unsigned long long* __restrict__ sums,
                                                       uint64_t* __restrict__ out, int* __restrict__ first_out,
-                                                      int64_t cap) {
+                                                      int64_t cap, int* __restrict__ front) {
+  // front != nullptr: the tree entering lt_adapt was 2:1 balanced, so only the leaves created here
+  // can be part of a violation; they are listed (children by index, merged parents as ~index) as
+  // the frontier of lt_balance's first sweep (s->nfront0 entries, any order)
   constexpr int NC = Dim<DIM>::NC;
   __shared__ unsigned long long sm[33];
   const int64_t n = s->n;
@@ -203,6 +206,18 @@ __global__ void __launch_bounds__(BT) k_adapt_scatter(Geo g, const uint64_t* __r
     unsigned long long ex = block_excl_scan<unsigned long long>((unsigned long long)c, sm, &tile_total);
     int64_t pos = run + (int64_t)ex;
     run += (int64_t)tile_total;
+    int fpos = 0;
+    if (front != nullptr) {  // warp-aggregated append
+      const int cf = act == ACT_REFINE ? NC : (act == ACT_PARENT ? 1 : 0);
+      const int inc = warp_incl_scan(cf);
+      const int tot = __shfl_sync(0xffffffffu, inc, 31);
+      int base = 0;
+      if (tot) {
+        if ((threadIdx.x & 31) == 0) base = atomicAdd(&s->nfront0, tot);
+        base = __shfl_sync(0xffffffffu, base, 0);
+      }
+      fpos = base + inc - cf;
+    }
     if (c == 0) continue;
     const int l = key_level(key);
     const uint64_t m = key_morton(key);
@@ -212,7 +227,10 @@ __global__ void __launch_bounds__(BT) k_adapt_scatter(Geo g, const uint64_t* __r
     } else if (act == ACT_PARENT) {
       out[pos] = make_key(m, l - 1);  // child 0 has the parent's anchor
       index_write<DIM>(g, first_out, m, l - 1, (int)pos);
+      if (front != nullptr) front[fpos] = ~(int)pos;
     } else {
+      if (front != nullptr)
+        for (int k = 0; k < NC; ++k) front[fpos + k] = (int)(pos + k);
       const int sh = DIM * (g.maxl - l - 1);
 #pragma unroll
       for (int k = 0; k < NC; ++k) {
@@ -296,6 +314,7 @@ struct BalanceArgs {
   DevScalars* s;
   int64_t cap;
   int full_sweeps;
+  int front0;  // 1: frontier[0] holds lt_adapt's list of new leaves (s->nfront0 entries) for sweep 1
   // neighbour directions examined per leaf (reading C-9): 2 bits per axis, 0 = no move,
   // 1 = move across the leaf's parent-EXTERIOR side on that axis, 2 = across the interior side
   int ndirs;
@@ -338,6 +357,37 @@ __device__ __forceinline__ void balance_examine(const Geo& g, const uint64_t* __
   }
 }
 
+// A parent created by lt_adapt (level l) is too coarse iff, across one of its faces, a level-(l+1)
+// cell of the neighbouring level-l cell is itself subdivided (its leaves are >= 2 levels finer).
+// Checked from the parent's side for the two faces of axis a; marks the parent itself.
+template <int DIM>
+__device__ __forceinline__ void balance_selfcheck(const Geo& g, const uint64_t* __restrict__ keys,
+                                                  const int* __restrict__ first, uint8_t* mark, int i, int a) {
+  const uint64_t key = keys[i];
+  const int l = key_level(key);
+  if (l + 2 > g.maxl) return;
+  const uint64_t m = key_morton(key);
+  bool hit = false;
+#pragma unroll
+  for (int side = 0; side < 2; ++side) {
+    uint64_t mn;
+    if (!face_neighbour<DIM>(g, m, l, 2 * a + side, &mn)) continue;
+#pragma unroll
+    for (int sidx = 0; sidx < (1 << (DIM - 1)); ++sidx) {
+      int c = side ? 0 : (1 << a), bit = 0;
+#pragma unroll
+      for (int b = 0; b < DIM; ++b) {
+        if (b == a) continue;
+        c |= ((sidx >> bit) & 1) << b;
+        ++bit;
+      }
+      const int j = locate(g, keys, first, mn | ((uint64_t)c << (DIM * (g.maxl - l - 1))));
+      hit = hit || key_level(keys[j]) >= l + 2;
+    }
+  }
+  if (hit) atomicOr((unsigned*)(mark + (i & ~3)), 1u << (8 * (i & 3)));
+}
+
 template <int DIM>
 __global__ void __launch_bounds__(BT) k_balance(BalanceArgs a) {
   constexpr int NC = Dim<DIM>::NC;
@@ -351,7 +401,7 @@ __global__ void __launch_bounds__(BT) k_balance(BalanceArgs a) {
   const int64_t gsize = (int64_t)gridDim.x * blockDim.x;
   int64_t n = a.s->n;
   int par = 0, iters = 0, fpar = 0;
-  int64_t nfront = -1;  // -1: full sweep
+  int64_t nfront = a.front0 ? (int64_t)a.s->nfront0 : -1;  // -1: full sweep
   int64_t splits = 0;
   int err = 0;
   for (;;) {
@@ -364,8 +414,11 @@ __global__ void __launch_bounds__(BT) k_balance(BalanceArgs a) {
           balance_examine<DIM>(g, keys, first, a.mark, (int)(sidx / DIM), 1 << (2 * (int)(sidx % DIM)));
       } else {
         const int* fr = a.frontier[fpar];
-        for (int64_t sidx = gtid; sidx < nfront * DIM; sidx += gsize)
-          balance_examine<DIM>(g, keys, first, a.mark, fr[sidx / DIM], 1 << (2 * (int)(sidx % DIM)));
+        for (int64_t sidx = gtid; sidx < nfront * DIM; sidx += gsize) {
+          const int ent = fr[sidx / DIM];
+          if (ent >= 0) balance_examine<DIM>(g, keys, first, a.mark, ent, 1 << (2 * (int)(sidx % DIM)));
+          else balance_selfcheck<DIM>(g, keys, first, a.mark, ~ent, (int)(sidx % DIM));  // only in sweep 1
+        }
       }
     } else {
       const int nd = a.ndirs;
@@ -504,7 +557,8 @@ int launch_adapt_count(Tree* t, const int8_t* d_flags, int G) {
   return LT_OK;
 }
 
-int launch_adapt_scatter(Tree* t, const int8_t* d_flags, int G, int path_a) {
+int launch_adapt_scatter(Tree* t, const int8_t* d_flags, int G, int path_a, int emit_front) {
+  int* front = (emit_front && !path_a) ? t->frontier[0] : nullptr;
   if (path_a) {
     LT_DISPATCH_DIM(t,
                     (k_adapt_append<2><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], d_flags, t->d_s, t->d_sums,
@@ -514,16 +568,16 @@ int launch_adapt_scatter(Tree* t, const int8_t* d_flags, int G, int path_a) {
   } else {
     LT_DISPATCH_DIM(t,
                     (k_adapt_scatter<2><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], d_flags, t->d_s, t->d_sums,
-                                                                 t->keys[t->tmp], t->first[t->tmp], t->cap)),
+                                                                 t->keys[t->tmp], t->first[t->tmp], t->cap, front)),
                     (k_adapt_scatter<3><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], d_flags, t->d_s, t->d_sums,
-                                                                 t->keys[t->tmp], t->first[t->tmp], t->cap)));
+                                                                 t->keys[t->tmp], t->first[t->tmp], t->cap, front)));
   }
   t->launches++;
   LT_CUDA(cudaGetLastError());
   return LT_OK;
 }
 
-int launch_balance(Tree* t, int64_t cap_told) {
+int launch_balance(Tree* t, int64_t cap_told, int use_front) {
   BalanceArgs a;
   a.g = t->g;
   a.keys[0] = t->keys[t->cur];
@@ -537,6 +591,7 @@ int launch_balance(Tree* t, int64_t cap_told) {
   a.s = t->d_s;
   a.cap = cap_told;
   a.full_sweeps = t->opt_full_sweeps;
+  a.front0 = use_front;
   // directions: per axis none / exterior / interior, at least one exterior move, at most
   // `conn` moves (conn 1: the dim exterior faces, in axis order)
   const int conn = t->opt_balance_conn > 0 ? t->opt_balance_conn : 1;

@@ -347,3 +347,28 @@ def test_connect_begin_end_overlaps_transfer():
     gt.adapt(torch.from_numpy(f).cuda()); gt.balance()
     P.assert_keys_equal(gt, ot, "adapt after an uncollected connect_begin")
     P.assert_faces_equal(gt.connect(), ot.connect(), "sync connect afterwards")
+
+
+@pytest.mark.parametrize("dim,base,maxl,periodic", [(2, 2, 7, (1, 0)), (3, 1, 5, (1, 1, 1)), (3, 2, 5, (0, 0, 0))])
+def test_balance_after_adapt_uses_the_adapt_frontier(dim, base, maxl, periodic):
+    # lt_balance's first sweep looks only at the leaves lt_adapt created (children examined as fine
+    # leaves, merged parents checked from their own side); with coarsening-heavy random flags the
+    # result, the sweep count and the split count must still be the oracle's -- and the same as with
+    # full sweeps
+    rng = np.random.default_rng(dim * 100 + maxl)
+    dom = [0.0] * dim + [1.0] * dim
+    gt, gf = lt.Tree(dim, base, maxl, dom, periodic), lt.Tree(dim, base, maxl, dom, periodic)
+    gf.set_option(lt.LT_OPT_BALANCE_FULL_SWEEPS, 1)
+    ot = oracle.Tree(dim, base, maxl, periodic)
+    for c in range(10):
+        pr = [0.45, 0.25, 0.30] if c % 2 else [0.15, 0.25, 0.60]   # coarsen-heavy / refine-heavy
+        f = rng.choice(np.array([-1, 0, 1], np.int8), size=ot.num_leaves(), p=pr)
+        ot.adapt(f); it_o = ot.balance(); ot.drop_snapshot()
+        for g in (gt, gf):
+            g.adapt(torch.from_numpy(f).cuda())
+            assert g.balance() == it_o, "cycle %d" % c
+            P.assert_keys_equal(g, ot, "cycle %d" % c)
+        if c == 4:  # two adapts without a balance in between: the second one has no valid frontier
+            f2 = rng.choice(np.array([-1, 0, 1], np.int8), size=ot.num_leaves(), p=[0.2, 0.5, 0.3])
+            ot.adapt(f2); ot.drop_snapshot()
+            gt.adapt(torch.from_numpy(f2).cuda()); gf.adapt(torch.from_numpy(f2).cuda())
