@@ -149,6 +149,8 @@ int lt_adapt(lt_tree*, const int8_t* d_flags);
  * refinement in which leaves sharing a (dim-1)-face (periodic images included) differ by
  * at most one level, by Jacobi ripple sweeps run in ONE cooperative kernel (no host round
  * trip per sweep).  *iters (host, may be NULL) = number of sweeps that split >= 1 leaf.
+ * If the tree was balanced when the preceding lt_adapt was called, the first sweep examines only
+ * the leaves that call created (same result, sweep count and splits as a full sweep).
  * Synchronises at the end (reads leaf count / status).  On LT_ERR_CAPACITY (growth
  * impossible) the tree is a valid, partially balanced refinement of the input. */
 int lt_balance(lt_tree*, int* iters);
