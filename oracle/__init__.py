@@ -107,6 +107,8 @@ def lib():
         L.lto_common_flux.argtypes = [C.c_void_p] + [C.POINTER(C.c_double)] * 3 + [C.c_int]
         L.lto_fr_rhs.restype = C.c_int
         L.lto_fr_rhs.argtypes = [C.c_void_p] + [C.POINTER(C.c_double)] * 4 + [C.c_int]
+        L.lto_rk3_stage.restype = C.c_int
+        L.lto_rk3_stage.argtypes = [C.c_int, C.c_double, C.c_int64] + [C.POINTER(C.c_double)] * 4
         L.lto_fr_operators.restype = C.c_int
         L.lto_fr_operators.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
         L.lto_face_interp.restype = C.c_int
@@ -192,6 +194,20 @@ def fr_operators(p):
         lib().lto_fr_operators(p, which, _p(a, C.c_double))
         out.append(a)
     return tuple(out)
+
+
+def rk3_stage(stage, dt, u_n, u_stage, rhs):
+    """Eq. 6 (PAPER.md:75), one stage: stage 1 u^n + dt R; stage 2 3/4 u^n + 1/4 u^1 + 1/4 dt R(u^1);
+    stage 3 1/3 u^n + 2/3 u^2 + 2/3 dt R(u^2).  u_stage is the vector R was evaluated at."""
+    un = np.ascontiguousarray(u_n, dtype=np.float64)
+    us = np.ascontiguousarray(u_stage, dtype=np.float64)
+    R = np.ascontiguousarray(rhs, dtype=np.float64)
+    assert un.shape == us.shape == R.shape
+    out = np.zeros(un.shape)
+    if lib().lto_rk3_stage(int(stage), float(dt), un.size, _p(un, C.c_double), _p(us, C.c_double),
+                           _p(R, C.c_double), _p(out, C.c_double)) != 0:
+        raise OracleError("oracle rk3_stage: stage must be 1, 2 or 3")
+    return out
 
 
 class OracleError(RuntimeError):

@@ -1147,6 +1147,28 @@ void fr_rhs(Tree* t, const FrOps& o, const double* width, const double* u, const
   }
 }
 
+// Eq. 6: the three-stage, third-order explicit Runge-Kutta method, one stage per call,
+// written as printed:
+//   stage 1:  u^1     = u^n + dt R(u^n)
+//   stage 2:  u^2     = 3/4 u^n + 1/4 u^1 + 1/4 dt R(u^1)
+//   stage 3:  u^(n+1) = 1/3 u^n + 2/3 u^2 + 2/3 dt R(u^2)
+// un = u^n, us = the stage vector the right-hand side R was evaluated at (u^n, u^1, u^2; unused in
+// stage 1, where it is u^n by definition), R = R(us).  Pinned by the scheme's amplification
+// polynomial 1 + z + z^2/2 + z^3/6 on u' = lambda u and by third-order convergence
+// (tests/test_oracle_fr.py).
+int rk3_stage(int stage, double dt, int64_t n, const double* un, const double* us, const double* R, double* out) {
+  if (stage == 1) {
+    for (int64_t i = 0; i < n; ++i) out[i] = un[i] + dt * R[i];
+  } else if (stage == 2) {
+    for (int64_t i = 0; i < n; ++i) out[i] = 3.0 / 4.0 * un[i] + 1.0 / 4.0 * us[i] + 1.0 / 4.0 * dt * R[i];
+  } else if (stage == 3) {
+    for (int64_t i = 0; i < n; ++i) out[i] = 1.0 / 3.0 * un[i] + 2.0 / 3.0 * us[i] + 2.0 / 3.0 * dt * R[i];
+  } else {
+    return -1;
+  }
+  return 0;
+}
+
 }  // namespace
 
 // ======================================================================= C ABI
@@ -1392,6 +1414,9 @@ int lto_fr_rhs(void* h, const double* width, const double* u, const double* fs, 
   build_fr_ops(o, p);
   fr_rhs((Tree*)h, o, width, u, fs, R);
   return 0;
+}
+int lto_rk3_stage(int stage, double dt, int64_t n, const double* un, const double* us, const double* R, double* out) {
+  return rk3_stage(stage, dt, n, un, us, R, out);
 }
 // which: 0 D [P1][P1], 1 l(-1) [P1], 2 l(+1) [P1], 3 g_L' [P1], 4 g_R' [P1]
 int lto_fr_operators(int p, int which, double* out) {

@@ -751,8 +751,7 @@ int lt_transfer_host(lt_tree* t, const double* h_u_old, double* h_u_new, int p, 
   while ((n_new + slab - 1) / slab > 4096) slab *= 2;
   const int S = (int)((n_new + slab - 1) / slab);
   if (t->bounds_cap < S + 1) {
-    free_dev(t->stream, t->mortar_hits);
-  free_dev(t->stream, t->d_bounds);
+    free_dev(t->stream, t->d_bounds);
     if (t->h_bounds) cudaFreeHost(t->h_bounds);
     t->d_bounds = nullptr; t->h_bounds = nullptr; t->bounds_cap = 0;
     if ((rc = alloc_dev(t->stream, &t->d_bounds, 2 * (int64_t)(S + 1))) != LT_OK) return rc;

@@ -230,3 +230,137 @@ def test_p0_is_first_order_finite_volume():
     for a in range(dim):
         want -= (fs[:, 2 * a + 1, :, 0] - fs[:, 2 * a, :, 0]) / dx[:, None]
     assert np.max(np.abs(R[:, :, 0] - want)) < 1e-11
+
+
+# ---------------------------------------------------------------- pins that do not re-type the flux formula
+def _read_fractions(name):
+    import os
+    from fractions import Fraction
+    out = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", name)) as fh:
+        for line in fh:
+            if line.startswith("#") or not line.strip():
+                continue
+            k, a, b = line.split()
+            out[k] = Fraction(int(a), int(b))
+    return out
+
+
+@pytest.mark.parametrize("dim,axis", [(2, 0), (2, 1), (3, 0), (3, 2)])
+def test_rusanov_hand_computed_value(dim, axis):
+    """tests/golden/rusanov_hand.txt: both states move, so a dropped '+ p' in (E + p) v_a or a wrong
+    sound speed changes the stored numbers.  Other axes / 3-D: the same states with the velocity
+    components permuted (the Euler flux is isotropic), w = 0 in 3-D."""
+    g = _read_fractions("rusanov_hand.txt")
+    uL = np.array([float(g["uL_%d" % k]) for k in range(4)])
+    uR = np.array([float(g["uR_%d" % k]) for k in range(4)])
+    want = np.array([float(g["Fstar_%d" % k]) for k in range(4)])
+    tang = [b for b in range(dim) if b != axis][0]     # the axis that receives the stored vy
+
+    def embed(v4):
+        out = np.zeros(dim + 2)
+        out[0], out[dim + 1] = v4[0], v4[3]
+        out[1 + axis], out[1 + tang] = v4[1], v4[2]
+        return out
+    t = oracle.Tree(dim, 0, 1, (1,) * dim)
+    t.connect()
+    own = np.tile(embed(uL)[None, None, :, None], (1, 2 * dim, 1, 1))
+    nb = np.tile(embed(uR)[None, None, :, None], (1, 2 * dim, 1, 1))
+    fs = t.common_flux(own, nb, 0)[0, 2 * axis + 1, :, 0]      # plus face: own = minus-side state
+    assert np.max(np.abs(fs - embed(want))) < 4e-16 * 4
+    # seen from the other element (minus face, own = plus-side state) it is the same flux along +a
+    fs2 = t.common_flux(nb, own, 0)[0, 2 * axis, :, 0]
+    assert np.array_equal(fs, fs2)
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+@pytest.mark.parametrize("p", [1, 2, 3])
+def test_manufactured_pressure_field_pins_energy_flux(dim, p):
+    """Constant density rho0 and velocity v0, pressure = polynomial of degree <= p per coordinate:
+    every flux is affine in the pressure, the traces are continuous (Rusanov = exact flux, exact
+    through the mortars) and the divergence is known in closed form,
+        R_rho = 0,   R_(rho v_a) = -d p / d x_a,   R_E = -gamma/(gamma-1) v0 . grad p,
+    because (E + p) v0 = (gamma/(gamma-1) p + rho0 |v0|^2 / 2) v0.  With E v0 instead of (E + p) v0
+    the last component would be -1/(gamma-1) v0 . grad p: the case separates the two."""
+    t = adapted_tree(dim, (0,) * dim, 60 + p)
+    F = t.connect()
+    kind = F["kind"].reshape(-1, t.nf) & 15
+    X, XF = volume_points(t, p), face_points(t, p, wrap=False)
+    v0 = np.array([0.6, -0.35, 0.45][:dim])
+    rho0 = 1.3
+
+    def pr_of(Xp):
+        r = np.ones(Xp.shape[:-1]) * 2.5
+        for a in range(dim):
+            r = r + sum((0.3 - 0.07 * a + 0.04 * k) * Xp[..., a] ** k for k in range(1, p + 1))
+        return r
+
+    def grad_pr(Xp):
+        g = np.zeros(Xp.shape)
+        for a in range(dim):
+            g[..., a] = sum(k * (0.3 - 0.07 * a + 0.04 * k) * Xp[..., a] ** (k - 1) for k in range(1, p + 1))
+        return g
+
+    def state(pr):
+        U = np.empty(pr.shape + (dim + 2,))
+        U[..., 0] = rho0
+        U[..., 1:1 + dim] = rho0 * v0
+        U[..., dim + 1] = pr / (G - 1) + 0.5 * rho0 * (v0 @ v0)
+        return U
+    nv = dim + 2
+    u = np.moveaxis(state(pr_of(X)), -1, 1)
+    uf = t.face_interp(u, p, nv)
+    assert np.max(np.abs(uf - np.moveaxis(state(pr_of(XF)), -1, 2))) < 1e-12
+    unb = t.mortar_project(uf, p, nv)
+    fs = t.common_flux(uf, unb, p)
+    g = t.mortar_gather(fs, p, nv)
+    fs = np.where(np.isnan(fs), g, fs)
+    # boundary slots: the exact flux, written out for THIS state (not through a flux routine):
+    # F_a = (rho0 v0_a, rho0 v0 v0_a + p e_a, (gamma/(gamma-1) p + rho0 |v0|^2/2) v0_a)
+    prF = pr_of(XF)                                                # [M, nf, Nf]
+    for f in range(t.nf):
+        a = f >> 1
+        ex = np.zeros((t.num_leaves(), nv, prF.shape[-1]))
+        ex[:, 0] = rho0 * v0[a]
+        for b in range(dim):
+            ex[:, 1 + b] = rho0 * v0[b] * v0[a] + (prF[:, f] if b == a else 0.0)
+        ex[:, dim + 1] = (G / (G - 1) * prF[:, f] + 0.5 * rho0 * (v0 @ v0)) * v0[a]
+        bsel = kind[:, f] == 0
+        fs[bsel, f] = ex[bsel]
+        # and on the interior slots the common flux IS this exact flux (continuous traces)
+        isel = ~bsel
+        assert np.max(np.abs(fs[isel, f] - ex[isel])) < 1e-11
+    assert not np.isnan(fs).any()
+    R = t.fr_rhs(u, fs, p, [1.0] * dim)
+    gp = grad_pr(X)                                                # [M, N, dim]
+    want = np.stack([np.zeros(gp.shape[:2])] + [-gp[..., b] for b in range(dim)] + [-(G / (G - 1)) * (gp @ v0)], axis=1)
+    assert np.max(np.abs(R - want)) < 1e-9 * max(1.0, np.max(np.abs(want)))
+
+
+# ---------------------------------------------------------------- Eq. 6
+def test_rk3_amplification_polynomial_and_order():
+    """Eq. 6 on u' = lambda u: one step multiplies u by 1 + z + z^2/2 + z^3/6, z = lambda dt
+    (the three-stage third-order scheme reproduces the Taylor polynomial of e^z); any swapped or
+    misplaced coefficient changes the polynomial.  Then third-order convergence on a nonlinear ODE."""
+    rng = np.random.default_rng(0)
+    un = rng.uniform(0.5, 1.5, 7)
+    for lam, dt in ((-1.3, 0.2), (0.7, 0.5), (-4.0, 0.05)):
+        u1 = oracle.rk3_stage(1, dt, un, un, lam * un)
+        u2 = oracle.rk3_stage(2, dt, un, u1, lam * u1)
+        u3 = oracle.rk3_stage(3, dt, un, u2, lam * u2)
+        z = lam * dt
+        assert np.max(np.abs(u1 - (1 + z) * un)) < 1e-15
+        assert np.max(np.abs(u3 - (1 + z + z * z / 2 + z ** 3 / 6) * un)) < 2e-15
+    # u' = -u^2, u(0) = 1 -> u(t) = 1/(1+t): error at t = 1 falls by ~8 when dt is halved
+    errs = []
+    for nsteps in (20, 40, 80):
+        u = np.array([1.0])
+        dt = 1.0 / nsteps
+        for _ in range(nsteps):
+            u1 = oracle.rk3_stage(1, dt, u, u, -u * u)
+            u2 = oracle.rk3_stage(2, dt, u, u1, -u1 * u1)
+            u = oracle.rk3_stage(3, dt, u, u2, -u2 * u2)
+        errs.append(abs(u[0] - 0.5))
+    assert 7.0 < errs[0] / errs[1] < 9.0 and 7.0 < errs[1] / errs[2] < 9.0
+    with pytest.raises(oracle.OracleError):
+        oracle.rk3_stage(4, 0.1, un, un, un)
