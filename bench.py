@@ -29,11 +29,27 @@ if ROOT not in sys.path:
 
 METRIC = "leaves/s per full adapt+2:1 balance+connectivity+transfer cycle"
 UNIT = "leaves/s"
+CONFIG = "c5"             # --config: c5 is the bench line; c1 / c2 / c4 are secondary lines
 PREP_CYCLES = 3           # config-5 cycles 0..2 run untimed to develop the tree
 OVERLAP = True            # --no-overlap: lt_connect then lt_transfer instead of begin / transfer / end
 CONNECTIVITY = 1          # --connectivity: 1 face balance (BASELINE.json), 2 the paper's strong balance
 PERIOD = (3, 4, 5)        # config-5 cycles a step runs (--cycles a,b,.. overrides: profiling aid)
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
+
+# untimed preparation cycles and the cycles the steps run through, per config: c5 cannot run its 10 stated
+# cycles (reading F-2); the small configs run ALL their stated cycles from the uniform tree, one step each
+SCHEDULES = {"c5": (3, (3, 4, 5)), "c1": (0, tuple(range(4))), "c2": (0, tuple(range(50))),
+             "c4": (0, tuple(range(20)))}
+WORKLOADS = {
+    "c5": "c5 (BASELINE.json configs[4]): 3D octree, periodic [-10,10]^3, base 64^3, max level +3, vortex-tube flags + "
+          "10% random refine / 10% random group coarsen (seed 2), p=3 (64 solution points), 5 fp64 vars",
+    "c1": "c1 (BASELINE.json configs[0]): 2D quadtree, [0,1]^2 non-periodic, base 8^2, max level 8, moving-disc flags + "
+          "5% random refine (seed 0), 4 cycles, p=2, 4 fp64 vars",
+    "c2": "c2 (BASELINE.json configs[1]): 2D quadtree, periodic [-10,10]^2, base 128^2, max level +4, isentropic-vortex "
+          "flags, 50 cycles, p=3, 4 fp64 vars",
+    "c4": "c4 (BASELINE.json configs[3]): 3D octree, periodic [-10,10]^3, base 32^3, max level +3, vortex-tube flags, "
+          "20 cycles, p=2, 5 fp64 vars",
+}
 
 
 def hbm_peak():
@@ -104,52 +120,144 @@ def mem_available_bytes():
 
 
 # --------------------------------------------------------------------------- oracle legs
-def oracle_cycle0(cfg):
-    """The oracle, as it stands, on config-5 cycle 0 (262,144 -> 544,475 leaves): one full
-    adapt + balance + connect + transfer.  Returns (leaves_out, faces, seconds)."""
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
+class PinnedThread:
+    """The oracle is sequential: pin this process to ONE of its allowed cores while it is timed."""
+
+    def __enter__(self):
+        self.old = None
+        try:
+            self.old = os.sched_getaffinity(0)
+            self.cpu = max(self.old)
+            os.sched_setaffinity(0, {self.cpu})
+        except Exception:
+            self.cpu = None
+        return self
+
+    def __exit__(self, *exc):
+        if self.old:
+            try:
+                os.sched_setaffinity(0, self.old)
+            except Exception:
+                pass
+
+
+def oracle_cycles(cfg, cycles, transfer_fraction=1.0):
+    """The oracle, as it stands, on cycles 0..cycles-1 of a config; only its four calls are timed (flag
+    and solution generation are the harness's).  transfer_fraction < 1: the transfer of a cycle is
+    timed on evenly spaced slabs covering that fraction of the new elements and scaled (config 5's deep
+    cycles: a dense M^-1 S_c per element is minutes of host time); tree, balance, faces and the map are
+    always timed in full.  Returns a list of per-cycle dicts."""
     import numpy as np
     import torch
     import oracle
     from paper_2306_06744_b200 import workloads as W
+    p, nvars = cfg["p"], cfg["nvars"]
     ot = oracle.Tree(cfg["dim"], cfg["base"], cfg["maxl"], cfg["periodic"])
     lvl, xyz = ot.leaf_boxes()
     L, X = torch.from_numpy(lvl), torch.from_numpy(xyz.astype(np.int64))
-    uo = W.initial_solution(cfg, L, X).numpy()
-    f = W.flags(cfg, 0, L, X).numpy()
-    t0 = time.perf_counter()
-    ot.adapt(f)
-    ot.balance()
-    F = ot.connect()
-    ot.transfer(uo, cfg["p"], cfg["nvars"])
-    dt = time.perf_counter() - t0
-    return ot.num_leaves(), F["n_conf"] + F["n_hang"] + F["n_bnd"], dt
+    full = transfer_fraction >= 1.0
+    uo = W.initial_solution(cfg, L, X).numpy() if full else None
+    rows = []
+    for c in range(cycles):
+        f = W.flags(cfg, c, L, X).numpy()
+        m0 = ot.num_leaves()
+        t0 = time.perf_counter()
+        ot.adapt(f)
+        t1 = time.perf_counter()
+        it = ot.balance()
+        t2 = time.perf_counter()
+        F = ot.connect()
+        t3 = time.perf_counter()
+        m1 = ot.num_leaves()
+        scaled = False
+        if full:
+            uo = ot.transfer(uo, p, nvars)
+            t4 = time.perf_counter()
+            t_tr = t4 - t3
+        else:
+            src, kind = ot.build_map()
+            t_map = time.perf_counter() - t3
+            slab = 4096
+            nslab = max(1, int(transfer_fraction * m1 / slab))
+            starts = np.linspace(0, max(0, m1 - slab), nslab).astype(np.int64)
+            t_rows, n_rows = 0.0, 0
+            for j0 in starts:
+                j1 = min(m1, int(j0) + slab)
+                lo = int(src[j0:j1].min())
+                hi = min(m0, int(src[j0:j1].max()) + (1 << cfg["dim"]))
+                win = W.initial_solution(cfg, L[lo:hi], X[lo:hi]).numpy()   # analytic old values, untimed
+                ta = time.perf_counter()
+                ot.transfer_rows(win, p, nvars, int(j0), j1, old_offset=lo)
+                t_rows += time.perf_counter() - ta
+                n_rows += j1 - int(j0)
+            ot.drop_snapshot()
+            t_tr = t_map + t_rows * (m1 / max(n_rows, 1))
+            scaled = n_rows < m1
+        lvl, xyz = ot.leaf_boxes()
+        L, X = torch.from_numpy(lvl), torch.from_numpy(xyz.astype(np.int64))
+        rows.append(dict(cycle=c, M0=m0, M1=m1, iters=it, faces=F["n_conf"] + F["n_hang"] + F["n_bnd"],
+                         adapt=t1 - t0, balance=t2 - t1, connect=t3 - t2, transfer=t_tr,
+                         seconds=(t3 - t0) + t_tr, transfer_scaled=scaled))
+        del F
+    return rows
 
 
-SAMPLE = "config 5 cycle 0 in full (262,144 -> 544,475 leaves, p=3, 5 vars): adapt+balance+connect+transfer"
+# default (bounded, 3-30 s of host time) and --oracle-full samples of the cpu_baseline per config
+ORACLE_SAMPLES = {"c5": (1, 1.0, 4, 0.02), "c1": (4, 1.0, 4, 1.0), "c2": (12, 1.0, 50, 1.0), "c4": (3, 1.0, 20, 1.0)}
+
+
+def cpu_baseline(name, cfg, full=False):
+    cyc, frac, cyc_full, frac_full = ORACLE_SAMPLES[name]
+    if full:
+        cyc, frac = cyc_full, frac_full
+    with PinnedThread() as pin:
+        rows = oracle_cycles(cfg, cyc, frac)
+    secs = sum(r["seconds"] for r in rows)
+    leaves = sum(r["M1"] for r in rows)
+    sample = "%s cycle%s 0%s in full (%d -> %d leaves, p=%d, %d vars): adapt+balance+connect+transfer" % (
+        name, "s" if cyc > 1 else "", "-%d" % (cyc - 1) if cyc > 1 else "", rows[0]["M0"], rows[-1]["M1"], cfg["p"],
+        cfg["nvars"])
+    if frac < 1.0:
+        sample += "; transfer timed on slabs covering %.0f %% of the new elements and scaled" % (100 * frac)
+    return {"value": leaves / secs, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample, "seconds": secs,
+            "faces_per_s": sum(r["faces"] for r in rows) / sum(r["connect"] for r in rows),
+            "seconds_per_call": {k: sum(r[k] for r in rows) for k in ("adapt", "balance", "connect", "transfer")},
+            "pinned_to_cpu": pin.cpu, "cpu_model": cpu_model(), "host_cores_available": os.cpu_count(),
+            "which": "oracle-full" if full else "default (bounded)"}
 
 
 def run_reference(args):
-    """--impl reference: the CPU oracle timed on the box's host cores (tier rule 4)."""
+    """--impl reference: the CPU oracle timed on the box's host cores (tier rule 4), one pinned thread,
+    on the sample of --config's workload that cpu_baseline() names; a step = that sample once."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     from paper_2306_06744_b200 import workloads as W
-    cfg = W.CONFIGS["c5"]
+    cfg = W.CONFIGS[CONFIG]
     for _ in range(args.warmup):
-        oracle_cycle0(cfg)
-    leaves, secs = 0, 0.0
+        cpu_baseline(CONFIG, cfg, args.oracle_full)
+    leaves, secs, last = 0, 0.0, None
     for _ in range(args.steps):
-        n, _, dt = oracle_cycle0(cfg)
-        leaves += n
-        secs += dt
+        last = cpu_baseline(CONFIG, cfg, args.oracle_full)
+        leaves += last["value"] * last["seconds"]
+        secs += last["seconds"]
     value = leaves / secs
     out = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "c5: 3D octree periodic [-10,10]^3, base 64^3, max +3, p=3, 5 fp64 vars",
-                   "step": SAMPLE},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": SAMPLE},
+        "config": {"workload": WORKLOADS[CONFIG], "step": last["sample"]},
+        "cpu_baseline": dict(last, value=value),
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -217,12 +325,18 @@ def whole_job_value(leaves_per_rank, world, ms):
     return world * leaves_per_rank / (ms * 1e-3)
 
 
-def algorithmic_bytes(dim, M0, Ma, M1, n_faces3, Bu):
-    """SURVEY.md 8(d) minimal bytes of the kernels actually run (path B), per cycle."""
+def algorithmic_bytes(dim, M0, Ma, M1, n_faces3, Bu, iters=1):
+    """SURVEY.md 8(d) minimal bytes of the kernels actually run (path B), per cycle:
+    adapt    two passes over key + flag (count, scatter), keys out;
+    balance  every splitting sweep reads key + mark of every leaf and writes the new keys (leaf count taken
+             as the mean of Ma and M1), the closing sweep only examines the frontier (not counted);
+    map      Alg. 7, run in the tail of the balance kernel: old and new keys in, src + kind out;
+    connect  keys in, nbr + kind and the three face tables out;
+    transfer every old element read once, every new element written once, the map read once."""
     nf = 2 * dim
     n_conf, n_hang, n_bnd = n_faces3
-    adapt = 9 * M0 + 8 * Ma
-    balance = 9 * Ma + (16 * M1 if M1 != Ma else 0)
+    adapt = 2 * 9 * M0 + 8 * Ma
+    balance = iters * (9 + 8) * (Ma + M1) // 2
     connect = 8 * M1 + 5 * nf * M1 + 9 * (n_conf + n_hang) + 5 * n_bnd
     mapk = 8 * (M0 + M1) + 5 * M1
     transfer = Bu * (M0 + M1) + 5 * M1
@@ -244,7 +358,7 @@ def run_ours(args):
     dev = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
-    cfg = W.CONFIGS["c5"]
+    cfg = W.CONFIGS[CONFIG]
     R = Runner(cfg, dev)
     Bu, p, nvars, N = R.Bu, R.p, R.nvars, R.N
     K, Wm = args.steps, max(args.warmup, 0)
@@ -270,6 +384,9 @@ def run_ours(args):
 
     stream = torch.cuda.current_stream(dev)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # timing rule: inputs larger than L2, or L2 flushed between timed iterations
+    small = 2 * max_leaves * Bu < (512 << 20)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev) if small else None
 
     def one_step(c, overlap=None):
         nonlocal cur
@@ -278,7 +395,9 @@ def run_ours(args):
         M0 = t.num_leaves()
         f = R.flags(c)
         u_old = ubuf[cur][:M0]
-        launches0 = t.launch_count()
+        if flush is not None:
+            flush.fill_(c & 255)
+        launches0, syncs0 = t.launch_count(), t.host_syncs()
         torch.cuda.synchronize(dev)
         ev0.record(stream)
         t.adapt(f)
@@ -302,7 +421,7 @@ def run_ours(args):
         tm = t.timings()
         cur ^= 1
         return dict(cycle=c, M0=M0, Ma=Ma, M1=M1, iters=iters, faces=(F["n_conf"], F["n_hang"], F["n_bnd"]),
-                    ms=ms, tm=tm, launches=t.launch_count() - launches0)
+                    ms=ms, tm=tm, launches=t.launch_count() - launches0, syncs=t.host_syncs() - syncs0)
 
     def rewind():
         nonlocal cur
@@ -327,6 +446,9 @@ def run_ours(args):
         r = one_step(next_cycle(), overlap=OVERLAP and i == 0)
         if not (OVERLAP and i == 0):
             alone.append(r)
+    if seq % len(PERIOD):   # the timed region always starts at the first cycle of the period
+        rewind()
+        seq = 0
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize(dev)
@@ -347,7 +469,7 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel (k_transfer): algorithmic bytes / measured kernel time
     peak, peak_src = hbm_peak()
-    by = [algorithmic_bytes(cfg["dim"], s["M0"], s["Ma"], s["M1"], s["faces"], Bu) for s in steps]
+    by = [algorithmic_bytes(cfg["dim"], s["M0"], s["Ma"], s["M1"], s["faces"], Bu, s["iters"]) for s in steps]
     tr_bytes = sum(b["transfer"] for b in by)
     tr_ms = sum(s["tm"]["k_transfer"] for s in steps)
     achieved = tr_bytes / (tr_ms * 1e-3) / 1e9
@@ -355,17 +477,18 @@ def run_ours(args):
     try:  # profiles/traffic.txt: "<kernel> <dram bytes per launch> <algorithmic bytes of that launch>"
         for line in open(os.path.join(ROOT, "profiles", "traffic.txt")):
             w = line.split()
-            if len(w) >= 3 and w[0] == "k_transfer":
+            if len(w) >= 3 and w[0] == "k_transfer" and CONFIG == "c5":
                 traffic = int(w[1])
-                traffic_note = ("ncu --set full of the config-5 cycle-3 launch (profiles/r1f_step_full.md); "
+                traffic_note = ("ncu --set full of the config-5 cycle-3 launch (profiles/, see traffic.txt); "
                                 "algorithmic bytes of that launch: %d" % int(w[2]))
     except Exception:
         pass
     alone_GBps = None
     if alone:
-        ab = sum(algorithmic_bytes(cfg["dim"], s["M0"], s["Ma"], s["M1"], s["faces"], Bu)["transfer"] for s in alone)
+        ab = sum(algorithmic_bytes(cfg["dim"], s["M0"], s["Ma"], s["M1"], s["faces"], Bu, s["iters"])["transfer"]
+                 for s in alone)
         alone_GBps = ab / (sum(s["tm"]["k_transfer"] for s in alone) * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "k_transfer<3,4>", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    roofline = {"bound": "hbm", "kernel": "k_transfer<%d,%d>" % (cfg["dim"], p + 1), "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "achieved_alone": alone_GBps, "frac_alone": None if alone_GBps is None else alone_GBps / peak,
                 "note": "timed steps overlap k_connect (side stream) with k_transfer, so `achieved` is k_transfer's "
                         "bandwidth under that contention; `achieved_alone` is the same kernel in the warm-up steps "
@@ -403,33 +526,36 @@ def run_ours(args):
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        n, nfaces, dt = oracle_cycle0(cfg)
-        cpu = {"value": n / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": SAMPLE,
-               "seconds": dt, "faces_per_s": nfaces / dt, "host_cores_available": os.cpu_count()}
+        cpu = cpu_baseline(CONFIG, cfg, args.oracle_full)
 
     if rank == 0:
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": tot_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "c5 (BASELINE.json configs[4]): 3D octree, periodic [-10,10]^3, base 64^3, "
-                                   "max level +3, vortex-tube flags + 10% random refine / 10% random group coarsen "
-                                   "(seed 2), p=3 (64 solution points), 5 fp64 vars",
-                       "step": "one adaptation cycle; steps run config-5 cycles %s after an untimed tree-only "
-                               "replay of cycles 0-%d" % (list(PERIOD), PREP_CYCLES - 1),
+            "config": {"workload": WORKLOADS[CONFIG],
+                       "step": ("one adaptation cycle; steps run %s cycles %s after an untimed tree-only replay of "
+                                "cycles 0-%d" % (CONFIG, list(PERIOD), PREP_CYCLES - 1)) if PREP_CYCLES else
+                               ("one adaptation cycle; steps run %s cycles %d..%d from the uniform base tree"
+                                % (CONFIG, PERIOD[0], PERIOD[-1])),
                        "leaves_out_per_step": [s["M1"] for s in steps], "leaves_in_per_step": [s["M0"] for s in steps],
                        "balance_iters": [s["iters"] for s in steps], "balance_connectivity": CONNECTIVITY,
                        "connect_transfer_overlap": OVERLAP,
-                       "l2": "inputs larger than L2 (u_old + u_new are 57-115 GB per step)",
+                       "l2": "L2 flushed between timed steps (a 512 MB fill; the inputs are smaller than L2)" if small
+                             else "inputs larger than L2 (u_old + u_new are %.0f-%.0f GB per step)" % (
+                                 min(sum(x) for x in sizes) * Bu / 1e9, max(sum(x) for x in sizes) * Bu / 1e9),
                        "parallelism": "replicas only (one independent tree per GPU)" if world > 1 else "single GPU",
                        "timing": "CUDA events on the tree's stream around lt_adapt..lt_transfer of each step; "
                                  "flag generation between steps is excluded"},
             "roofline": roofline, "cycle_roofline": cycle_roofline, "ms_per_call": per_call,
+            "ms_per_cycle": [round(s["ms"], 4) for s in steps] if len(steps) <= 64 else None,
+            "launches_per_cycle": launches / K, "host_syncs_per_cycle": sum(s["syncs"] for s in steps) / K,
             "faces_per_s": faces_per_s, "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": launches,
             "wall_s_timed_region": t_wall,
             "e2e": None if e2e is None else {"value": e2e["value"], "unit": UNIT,
                                              "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
-                                             "ms_per_step": e2e["ms"], "cycle": e2e["cycle"], "note": e2e["note"]},
+                                             "ms_per_step": e2e["ms"], "ms_each": e2e["ms_each"], "runs": e2e["runs"],
+                                             "cycle": e2e["cycle"], "note": e2e["note"]},
         }
         print(json.dumps(out), flush=True)
     if world > 1:
@@ -437,40 +563,47 @@ def run_ours(args):
 
 
 def run_e2e(R, args, world, dev):
-    """One adaptation cycle with HOST inputs and outputs: flags and u_old start in pinned host
-    memory, u_new and the face counts end in host memory; every copy is inside the timed
-    region.  Runs the largest config-5 cycle <= PERIOD[0] whose host buffers fit the budget."""
+    """One adaptation cycle with HOST inputs and outputs: flags and u_old start in pinned host memory;
+    u_new, the keys, nbr / kind and the three face tables end in pinned host memory; every copy is inside
+    the timed region.  Runs the largest cycle <= PERIOD[-1] (config 5: <= PERIOD[0]) whose host buffers fit
+    the budget: one untimed warm-up run (staging ring, pools), then three timed runs from the same state."""
     torch = R.torch
     cfg, Bu, p, nvars, N = R.cfg, R.Bu, R.p, R.nvars, R.N
+    nf = 2 * cfg["dim"]
     budget = min(64 << 30, int(0.4 * mem_available_bytes() / max(world, 1)))
-    # leaf counts of cycles 0..PERIOD[0] (tree only)
+    last = PERIOD[0] if CONFIG == "c5" else PERIOD[-1]
     dom = [cfg["lo"]] * cfg["dim"] + [cfg["hi"]] * cfg["dim"]
-    t = R.lt.Tree(cfg["dim"], cfg["base"], cfg["maxl"], dom, cfg["periodic"])
-    if CONNECTIVITY != 1:
-        t.set_option(R.lt.LT_OPT_BALANCE_CONNECTIVITY, CONNECTIVITY)
-    R.tree = t
-    counts = []
-    for c in range(PERIOD[0] + 1):
-        m0 = t.num_leaves()
-        t.adapt(R.flags(c))
-        t.balance()
-        counts.append((m0, t.num_leaves()))
+
+    def fresh(upto):
+        if R.tree is not None:
+            R.tree.free()
+        t = R.lt.Tree(cfg["dim"], cfg["base"], cfg["maxl"], dom, cfg["periodic"])
+        if CONNECTIVITY != 1:
+            t.set_option(R.lt.LT_OPT_BALANCE_CONNECTIVITY, CONNECTIVITY)
+        R.tree = t
+        counts = []
+        for c in range(upto):
+            m0 = t.num_leaves()
+            t.adapt(R.flags(c))
+            t.balance()
+            counts.append((m0, t.num_leaves()))
+        return t, counts
+
+    _, counts = fresh(last + 1)
     pick = 0
     for c, (m0, m1) in enumerate(counts):
-        if (m0 + m1) * Bu <= budget:
+        if (m0 + m1) * (Bu + 160) <= budget:
             pick = c
-    t.free()
-    t = R.lt.Tree(cfg["dim"], cfg["base"], cfg["maxl"], dom, cfg["periodic"])
-    if CONNECTIVITY != 1:
-        t.set_option(R.lt.LT_OPT_BALANCE_CONNECTIVITY, CONNECTIVITY)
-    R.tree = t
-    for c in range(pick):
-        t.adapt(R.flags(c))
-        t.balance()
     M0, M1 = counts[pick]
-    t.reserve(int(M1 * 1.02) + 4096)
     h_old = torch.empty((M0, nvars, N), dtype=torch.float64, pin_memory=True)
     h_new = torch.empty((M1, nvars, N), dtype=torch.float64, pin_memory=True)
+    # host copies of the tree-side results: keys, the paper's face array (nbr + kind), the face tables
+    h_keys = torch.empty(M1, dtype=torch.int64, pin_memory=True)
+    h_nbr = torch.empty(M1 * nf, dtype=torch.int32, pin_memory=True)
+    h_kind = torch.empty(M1 * nf, dtype=torch.uint8, pin_memory=True)
+    h_rows = torch.empty(M1 * (4 * cfg["dim"] + nf), dtype=torch.int32, pin_memory=True)
+    h_bytes = torch.empty(M1 * (2 * cfg["dim"] + nf), dtype=torch.uint8, pin_memory=True)
+    t, _ = fresh(pick)
     tmp = torch.empty((M0, nvars, N), dtype=torch.float64, device=dev)
     R.analytic_u(tmp)
     h_old.copy_(tmp)
@@ -478,25 +611,44 @@ def run_e2e(R, args, world, dev):
     torch.cuda.empty_cache()
     h_flags = R.flags(pick).cpu().pin_memory()
     d_flags = torch.empty(M0, dtype=torch.int8, device=dev)
-    # untimed warm-up of the staging allocations inside lt_transfer_host: run the cycle once
-    # on a scratch copy of the tree state?  The staging buffers are allocated by the first
-    # call, so do one identity transfer of the old tree first (sizes M0), then reserve new.
     stream = torch.cuda.current_stream(dev)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize(dev)
-    ev0.record(stream)
-    d_flags.copy_(h_flags, non_blocking=True)
-    t.adapt(d_flags)
-    t.balance()
-    F = t.connect()
-    t.transfer_host(h_old, h_new, p, nvars)
-    ev1.record(stream)
-    torch.cuda.synchronize(dev)
-    ms = ev0.elapsed_time(ev1)
-    assert t.num_leaves() == M1
-    return {"ms": ms, "leaves": M1, "h2d": M0 * Bu + M0, "d2h": M1 * Bu + 64, "cycle": pick,
-            "note": "config-5 cycle %d (%d -> %d leaves); host budget %.0f GB; lt_transfer_host pipelines "
-                    "upload / kernel / download in slabs (three streams, 3-slab staging ring)" % (pick, M0, M1, budget / 2 ** 30)}
+    ms_each, d2h = [], 0
+    for run in range(4):   # run 0 is the warm-up
+        if run:
+            t, _ = fresh(pick)
+        t.reserve(int(M1 * 1.02) + 4096)
+        torch.cuda.synchronize(dev)
+        ev0.record(stream)
+        d_flags.copy_(h_flags, non_blocking=True)
+        t.adapt(d_flags)
+        t.balance()
+        F = t.connect()
+        assert F["n_leaves"] == M1
+        d2h, ro, bo = 0, 0, 0
+        h_keys.copy_(t.keys(), non_blocking=True)
+        h_nbr.copy_(F["nbr"], non_blocking=True)
+        h_kind.copy_(F["kind"], non_blocking=True)
+        d2h += 8 * M1 + 5 * nf * M1
+        for rows_k, bytes_k in (("conf", "conf_axis"), ("hang", "hang_info"), ("bnd", "bnd_face")):
+            a, bb = F[rows_k].reshape(-1), F[bytes_k]
+            h_rows[ro:ro + a.numel()].copy_(a, non_blocking=True)
+            h_bytes[bo:bo + bb.numel()].copy_(bb, non_blocking=True)
+            ro, bo = ro + a.numel(), bo + bb.numel()
+            d2h += 4 * a.numel() + bb.numel()
+        t.transfer_host(h_old, h_new, p, nvars)
+        ev1.record(stream)
+        torch.cuda.synchronize(dev)
+        if run:
+            ms_each.append(ev0.elapsed_time(ev1))
+        d2h += M1 * Bu + 64
+    ms = sum(ms_each) / len(ms_each)
+    return {"ms": ms, "ms_each": ms_each, "runs": len(ms_each), "leaves": M1, "h2d": M0 * Bu + M0, "d2h": d2h,
+            "cycle": pick,
+            "note": "%s cycle %d (%d -> %d leaves), mean of %d runs after one warm-up run; down: u_new, keys, nbr/kind "
+                    "and the three face tables; host budget %.0f GB; lt_transfer_host pipelines upload / kernel / "
+                    "download in slabs (three streams, 3-slab staging ring)"
+                    % (CONFIG, pick, M0, M1, len(ms_each), budget / 2 ** 30)}
 
 
 # --------------------------------------------------------------------------- construction leg
@@ -833,9 +985,16 @@ def run_solver(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=None,
+                    help="timed steps (default: 3 for c5, one pass over all cycles for --config c1 / c2 / c4)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="c5", choices=sorted(SCHEDULES),
+                    help="c5 (default): the config BASELINE.json's metric is quoted on; c1 / c2 / c4: secondary lines "
+                         "in the same schema (one step = one adaptation cycle, all stated cycles from the uniform tree)")
+    ap.add_argument("--oracle-full", action="store_true",
+                    help="cpu_baseline / --impl reference on the config's full sample (c1-c4: every cycle; c5: cycles "
+                         "0-3 with the transfer timed on slabs) instead of the bounded default")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--workload", default="cycle", choices=["cycle", "construct", "mortar", "solver"],
@@ -852,14 +1011,17 @@ def main():
                     help="consecutive config-5 cycles a step cycles through (default 3,4,5 = the bench "
                          "workload; smaller ones, e.g. 2, keep an ncu --set full capture short)")
     args = ap.parse_args()
-    global CONNECTIVITY, OVERLAP
+    global CONNECTIVITY, OVERLAP, CONFIG, PERIOD, PREP_CYCLES
     CONNECTIVITY = args.connectivity
     OVERLAP = not args.no_overlap
+    CONFIG = args.config
+    PREP_CYCLES, PERIOD = SCHEDULES[CONFIG]
     if args.cycles:
-        global PERIOD, PREP_CYCLES
         PERIOD = tuple(int(c) for c in args.cycles.split(","))
         assert all(b == a + 1 for a, b in zip(PERIOD, PERIOD[1:])), "--cycles must be consecutive"
         PREP_CYCLES = PERIOD[0]
+    if args.steps is None:
+        args.steps = 3 if CONFIG == "c5" or args.impl == "reference" else len(PERIOD)
     if args.steps < 1:
         args.steps = 1
     if args.workload == "construct" and args.impl == "ours":

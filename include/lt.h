@@ -9,7 +9,9 @@
  *
  * Conventions
  *   - "device" pointers are CUDA device memory of the GPU that was current when the
- *     tree was built; "host" pointers are ordinary host memory.
+ *     tree was built; "host" pointers are ordinary host memory.  That GPU must be the
+ *     current device at every later call on the tree (calls that upload operators check it
+ *     and return LT_ERR_ARG otherwise).
  *   - Every call enqueues on the CUDA stream given at build time.  Calls that return a
  *     count or a status detected on the device synchronise that stream (stated per call).
  *   - Every int-returning call returns LT_OK (0) or a negative lt_status.  No exceptions,
@@ -275,7 +277,9 @@ int lt_sort_keys(int dim, int max_level, uint64_t* d_keys, int64_t n, int linear
 int lt_domain(lt_tree*, double* lo_hi /* host [2*dim] */);
 int lt_info(lt_tree*, int* dim, int* base_level, int* max_level, int* periodic /* host [3] */);
 
-/* Wait for the tree's stream and return (and clear) the sticky device status. */
+/* Wait for the tree's stream and return (and clear) the sticky device status.  The face query
+ * keeps a status word of its own, so lt_connect / lt_connect_end report only connectivity errors
+ * and a mapping error raised by an lt_transfer that ran beside the query is reported here. */
 int lt_sync(lt_tree*);
 
 typedef enum {
@@ -300,8 +304,14 @@ int lt_set_option(lt_tree*, int option, int value);
  * kernel alone, out[7] = the last mortar kernel (lt_mortar_project / lt_mortar_gather); 0 where not run.
  * Synchronises. */
 int lt_timings(lt_tree*, float* out8);
-/* Number of kernels liblt launched on this tree since it was built. */
+/* Number of kernels liblt launched on this tree since it was built, and the number of times a call
+ * made the host wait for the tree's stream (what a small mesh pays per cycle). */
 int64_t lt_launch_count(lt_tree*);
+int64_t lt_host_syncs(lt_tree*);
+/* Where the last lt_balance spent its device time, in milliseconds, read from the GPU's global timer
+ * between the grid-wide barriers of the cooperative kernel: out[0] examination sweeps, out[1] chunk
+ * offsets, out[2] splitting + next frontier, out[3] the Alg. 7 map in the kernel's tail. */
+int lt_balance_phases(lt_tree*, float* out4);
 
 const char* lt_strerror(int status);
 int lt_last_cuda_error(void); /* cudaError_t of the last failing runtime call (this thread) */

@@ -48,6 +48,8 @@ def lib():
         L.lto_sort_linearise.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_uint64), C.c_int64]
         L.lto_build.restype = C.c_void_p
         L.lto_build.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int)]
+        L.lto_build_brick.restype = C.c_void_p
+        L.lto_build_brick.argtypes = [C.c_int, C.POINTER(C.c_int), C.c_int, C.c_int, C.POINTER(C.c_int)]
         L.lto_build_from_keys.restype = C.c_void_p
         L.lto_build_from_keys.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int),
                                           C.POINTER(C.c_uint64), C.c_int64]
@@ -218,16 +220,23 @@ class Tree:
     """Pointer-based linear-tree oracle.  Same verbs as the product's C ABI."""
 
     def __init__(self, dim, base_level, max_level, periodic=None, keys=None, complete=False, points=None,
-                 domain=None):
+                 domain=None, nroot=None):
         """keys: unsorted IDs that must tile the domain (sort + linearise, Alg. 3);
         keys + complete=True: Alg. 2 completion of the octants over the uniform base tree;
-        points [n][dim] fp64 + domain (lo.., hi..): Alg. 2 from scattered points."""
+        points [n][dim] fp64 + domain (lo.., hi..): Alg. 2 from scattered points;
+        nroot (n_x, n_y[, n_z]): a brick of root cubes (forest), uniform at base_level."""
         self.dim, self.base, self.maxl = dim, base_level, max_level
         self.nc, self.nf = 1 << dim, 2 * dim
+        self.nroot = tuple(int(v) for v in nroot[:dim]) if nroot is not None else (1,) * dim
         per = np.zeros(3, np.int32)
         if periodic is not None:
             per[:dim] = np.asarray(periodic, np.int32)[:dim]
-        if points is not None:
+        if nroot is not None:
+            assert keys is None and points is None, "construction is defined on a single cube"
+            nr = np.ones(3, np.int32)
+            nr[:dim] = np.asarray(nroot, np.int32)[:dim]
+            self._h = lib().lto_build_brick(dim, _p(nr, C.c_int), base_level, max_level, _p(per, C.c_int))
+        elif points is not None:
             pts = np.ascontiguousarray(points, dtype=np.float64).reshape(-1, dim)
             dom = np.ascontiguousarray(domain, dtype=np.float64)
             assert dom.size == 2 * dim
@@ -320,17 +329,32 @@ class Tree:
         lib().lto_map(self._h, _p(src, C.c_int32), _p(kind, C.c_uint8))
         return src, kind
 
+    def _map_window(self, j0, j1):
+        M = self.num_leaves()
+        src = np.zeros(M, np.int32)
+        kind = np.zeros(M, np.uint8)
+        lib().lto_map(self._h, _p(src, C.c_int32), _p(kind, C.c_uint8))
+        return src[j0:j1], kind[j0:j1]
+
     def old_keys(self):
         k = np.zeros(int(lib().lto_num_old_leaves(self._h)), np.uint64)
         lib().lto_old_keys(self._h, _p(k, C.c_uint64))
         return k
 
-    def transfer_rows(self, u_old, p, nvars, j0, j1):
-        """Rows [j0, j1) of u_new (requires build_map())."""
+    def transfer_rows(self, u_old, p, nvars, j0, j1, old_offset=0):
+        """Rows [j0, j1) of u_new (requires build_map()).  u_old holds the old rows
+        [old_offset, old_offset + len(u_old)): a window is enough when only those rows are sources
+        (marshalling only: the base pointer handed to the C++ side is shifted back by old_offset rows)."""
         N = (p + 1) ** self.dim
         u_old = np.ascontiguousarray(u_old, dtype=np.float64)
         out = np.zeros((j1 - j0, nvars, N))
-        rc = lib().lto_transfer_rows(self._h, _p(u_old, C.c_double), _p(out, C.c_double), p, nvars, j0, j1)
+        if old_offset or u_old.shape[0] < int(lib().lto_num_old_leaves(self._h)):
+            src, kind = self._map_window(j0, j1)
+            last = src.astype(np.int64) + np.where((kind & 15) == 2, self.nc - 1, 0)
+            assert src.min() >= old_offset and last.max() < old_offset + u_old.shape[0], \
+                "transfer_rows: the window does not cover the sources of rows [%d, %d)" % (j0, j1)
+        base = C.cast(C.c_void_p(u_old.ctypes.data - int(old_offset) * nvars * N * 8), C.POINTER(C.c_double))
+        rc = lib().lto_transfer_rows(self._h, base, _p(out, C.c_double), p, nvars, j0, j1)
         if rc != 0:
             raise OracleError("oracle transfer: rc=%d" % rc)
         return out

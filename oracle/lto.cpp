@@ -63,11 +63,16 @@ struct Ops {  // dense transfer operators for one (dim, p)
 struct Tree {
   int dim = 2, base = 0, maxl = 0, nc = 4, nf = 4;
   int periodic[3] = {0, 0, 0};
-  Node* root = nullptr;
+  // The domain is a brick of nroot[0] x nroot[1] (x nroot[2]) root cubes, i.e. a forest of pointer
+  // trees (reading J-1 of DESIGN.md; PAPER.md:84 considers "perfect cubes" only, its 3-D runs use a
+  // slab of 16 x 16 x 1 cubes).  roots[r], r = tx + nroot[0] * (ty + nroot[1] * tz); node
+  // anchors are GLOBAL integer coordinates in [0, nroot[a] << maxl).  A single cube is the forest {1,1,1}.
+  int nroot[3] = {1, 1, 1};
+  std::vector<Node*> roots;
   std::vector<Node*> leaves;   // sorted by Morton ID
   std::vector<uint64_t> keys;  // their IDs
-  // snapshot of the tree before the last adapt (T_o of Alg. 7)
-  Node* old_root = nullptr;
+  // snapshot of the forest before the last adapt (T_o of Alg. 7)
+  std::vector<Node*> old_roots;
   std::vector<Node*> old_leaves;
   std::vector<uint64_t> old_keys;
   bool have_old = false;
@@ -108,7 +113,25 @@ void decode(int dim, int maxl, uint64_t key, int* level, uint32_t* x_finest) {
       x_finest[a] |= (uint32_t)((r >> (dim * k + a)) & 1u) << k;
 }
 
-uint64_t key_of(const Tree* t, const Node* n) { return encode(t->dim, t->maxl, n->level, n->x); }
+// Forest ID (reading J-1): the Morton ID of the octant inside its root cube (Alg. 1 on the
+// coordinates relative to the cube) with the cube's index r placed above the dim * D_max path bits,
+//   key = ((r << dim * D_max) | padded raw ID) << 5 | depth,
+// so that ascending order is cube-major and a single cube (r = 0) keeps the paper's ID unchanged.
+int root_index(const Tree* t, const uint32_t* x) {
+  int r = 0, mul = 1;
+  for (int a = 0; a < t->dim; ++a) {
+    r += (int)(x[a] >> t->maxl) * mul;
+    mul *= t->nroot[a];
+  }
+  return r;
+}
+uint64_t key_of(const Tree* t, const Node* n) {
+  uint32_t rel[3] = {0, 0, 0};
+  for (int a = 0; a < t->dim; ++a) rel[a] = n->x[a] & ((1u << t->maxl) - 1u);
+  if (t->maxl == 0) rel[0] = rel[1] = rel[2] = 0;
+  const uint64_t k = encode(t->dim, t->maxl, n->level, rel);
+  return k | ((uint64_t)root_index(t, n->x) << (t->dim * t->maxl + kLevelBits));
+}
 
 // a is a strict ancestor of b (integer boxes; PAPER.md:84 half-open regions)
 bool contains_strict(int dim, int maxl, int la, const uint32_t* xa, int lb, const uint32_t* xb) {
@@ -164,7 +187,7 @@ void dfs_leaves(Tree* t, Node* n, std::vector<Node*>& out) {
 // list leaves by depth-first traversal, then std::sort on the 64-bit ID
 void relist(Tree* t) {
   t->leaves.clear();
-  dfs_leaves(t, t->root, t->leaves);
+  for (Node* r : t->roots) dfs_leaves(t, r, t->leaves);
   std::vector<std::pair<uint64_t, Node*>> kv;
   kv.reserve(t->leaves.size());
   for (Node* n : t->leaves) kv.emplace_back(key_of(t, n), n);
@@ -177,9 +200,9 @@ void relist(Tree* t) {
   }
 }
 
-void list_into(Tree* t, Node* root, std::vector<Node*>& lv, std::vector<uint64_t>& ks) {
+void list_into(Tree* t, const std::vector<Node*>& roots, std::vector<Node*>& lv, std::vector<uint64_t>& ks) {
   lv.clear();
-  dfs_leaves(t, root, lv);
+  for (Node* r : roots) dfs_leaves(t, r, lv);
   std::sort(lv.begin(), lv.end(), [t](Node* a, Node* b) { return key_of(t, a) < key_of(t, b); });
   ks.resize(lv.size());
   for (size_t i = 0; i < lv.size(); ++i) {
@@ -188,10 +211,10 @@ void list_into(Tree* t, Node* root, std::vector<Node*>& lv, std::vector<uint64_t
   }
 }
 
-// point location: descend from the root towards integer point x, stop at a leaf
-// or at depth `limit`
-Node* locate(Tree* t, Node* root, const uint32_t* x, int limit) {
-  Node* n = root;
+// point location: pick the root cube that holds the integer point x, descend towards x, stop at a
+// leaf or at depth `limit`
+Node* locate(Tree* t, const std::vector<Node*>& roots, const uint32_t* x, int limit) {
+  Node* n = roots[root_index(t, x)];
   while (!n->is_leaf() && n->level < limit) {
     int sh = t->maxl - n->level - 1;
     int c = 0;
@@ -207,7 +230,7 @@ Node* locate(Tree* t, Node* root, const uint32_t* x, int limit) {
 bool neighbour_anchor(const Tree* t, const Node* n, int f, uint32_t* nx) {
   int a = f >> 1;
   int64_t w = (int64_t)1 << (t->maxl - n->level);
-  int64_t L = (int64_t)1 << t->maxl;
+  int64_t L = (int64_t)t->nroot[a] << t->maxl;  // width of the brick along a
   for (int b = 0; b < 3; ++b) nx[b] = n->x[b];
   int64_t v = (int64_t)n->x[a] + ((f & 1) ? w : -w);
   if (v < 0 || v >= L) {
@@ -226,9 +249,10 @@ bool neighbour_anchor(const Tree* t, const Node* n, int f, uint32_t* nx) {
 //  one level per call.
 void adapt(Tree* t, const int8_t* flags) {
   // snapshot T_o for Alg. 7
-  free_subtree(t->old_root);
-  t->old_root = clone(t->root, nullptr);
-  list_into(t, t->old_root, t->old_leaves, t->old_keys);
+  for (Node* r : t->old_roots) free_subtree(r);
+  t->old_roots.clear();
+  for (Node* r : t->roots) t->old_roots.push_back(clone(r, nullptr));
+  list_into(t, t->old_roots, t->old_leaves, t->old_keys);
   t->have_old = true;
 
   std::vector<Node*> to_refine, to_merge;
@@ -275,10 +299,10 @@ void adapt(Tree* t, const int8_t* flags) {
 // are skipped.
 bool offset_anchor(const Tree* t, const Node* n, const int* o, uint32_t* nx) {
   const int64_t w = (int64_t)1 << (t->maxl - n->level);
-  const int64_t L = (int64_t)1 << t->maxl;
   for (int b = 0; b < 3; ++b) nx[b] = n->x[b];
   for (int a = 0; a < t->dim; ++a) {
     if (!o[a]) continue;
+    const int64_t L = (int64_t)t->nroot[a] << t->maxl;
     int64_t v = (int64_t)n->x[a] + o[a] * w;
     if (v < 0 || v >= L) {
       if (!t->periodic[a]) return false;
@@ -303,7 +327,7 @@ int balance(Tree* t, int64_t* n_split_total, int conn) {
             if (nnz < 1 || nnz > conn) continue;
             uint32_t nx[3];
             if (!offset_anchor(t, L, o, nx)) continue;
-            Node* N = locate(t, t->root, nx, L->level);
+            Node* N = locate(t, t->roots, nx, L->level);
             if (N->is_leaf() && N->level < L->level - 1 && !N->mark) {
               N->mark = true;
               marked.push_back(N);
@@ -352,7 +376,7 @@ int connect_descent(Tree* t, std::vector<int32_t>& nbr, std::vector<uint8_t>& ki
       uint32_t nx[3];
       size_t s = (size_t)e * t->nf + f;
       if (!neighbour_anchor(t, L, f, nx)) continue;  // boundary
-      Node* N = locate(t, t->root, nx, L->level);
+      Node* N = locate(t, t->roots, nx, L->level);
       if (N->is_leaf()) {
         if (N->level == L->level) {
           kind[s] = 1;
@@ -382,7 +406,6 @@ int connect_descent(Tree* t, std::vector<int32_t>& nbr, std::vector<uint8_t>& ki
 // periodic) and overlap with positive (dim-1)-measure in the other axes.
 int connect_bruteforce(Tree* t, std::vector<int32_t>& nbr, std::vector<uint8_t>& kind) {
   const int64_t M = (int64_t)t->leaves.size();
-  const int64_t Lw = (int64_t)1 << t->maxl;
   nbr.assign((size_t)M * t->nf, -1);
   kind.assign((size_t)M * t->nf, 0);
   for (int64_t e = 0; e < M; ++e) {
@@ -390,6 +413,7 @@ int connect_bruteforce(Tree* t, std::vector<int32_t>& nbr, std::vector<uint8_t>&
     int64_t wa = (int64_t)1 << (t->maxl - A->level);
     for (int f = 0; f < t->nf; ++f) {
       int ax = f >> 1;
+      const int64_t Lw = (int64_t)t->nroot[ax] << t->maxl;  // width of the brick along ax
       size_t s = (size_t)e * t->nf + f;
       // plane coordinate the neighbour must start/end at
       int64_t plane = (f & 1) ? (int64_t)A->x[ax] + wa : (int64_t)A->x[ax];
@@ -494,7 +518,7 @@ int build_map(Tree* t) {
   }
   for (int64_t j = 0; j < M; ++j) {
     Node* L = t->leaves[j];
-    Node* O = locate(t, t->old_root, L->x, L->level);
+    Node* O = locate(t, t->old_roots, L->x, L->level);
     if (O->is_leaf()) {
       if (O->level == L->level) {
         t->map_kind[j] = 0;
@@ -758,15 +782,35 @@ bool complete_subtree(const Tree* t, const Node* n) {
   return true;
 }
 
-Tree* new_tree(int dim, int base, int maxl, const int* periodic) {
+Tree* new_tree(int dim, int base, int maxl, const int* periodic, const int* nroot = nullptr) {
   if (dim != 2 && dim != 3) return nullptr;
   if (base < 0 || base > maxl) return nullptr;
-  if (dim * maxl + kLevelBits > 63 || maxl > 31) return nullptr;
+  int64_t ntrees = 1;
+  for (int a = 0; a < dim; ++a) {
+    const int na = nroot ? nroot[a] : 1;
+    if (na < 1 || ((int64_t)na << maxl) > ((int64_t)1 << 31)) return nullptr;
+    ntrees *= na;
+  }
+  int tbits = 0;
+  while (((int64_t)1 << tbits) < ntrees) ++tbits;
+  if (dim * maxl + kLevelBits + tbits > 63 || maxl > 31) return nullptr;
   Tree* t = new Tree();
   t->dim = dim; t->base = base; t->maxl = maxl;
   t->nc = 1 << dim; t->nf = 2 * dim;
-  for (int a = 0; a < dim; ++a) t->periodic[a] = periodic ? periodic[a] : 0;
-  t->root = new Node();
+  for (int a = 0; a < dim; ++a) {
+    t->periodic[a] = periodic ? periodic[a] : 0;
+    t->nroot[a] = nroot ? nroot[a] : 1;
+  }
+  // one pointer tree per root cube, anchors in global integer coordinates
+  for (int64_t r = 0; r < ntrees; ++r) {
+    Node* n = new Node();
+    int64_t q = r;
+    for (int a = 0; a < dim; ++a) {
+      n->x[a] = (uint32_t)((q % t->nroot[a]) << maxl);
+      q /= t->nroot[a];
+    }
+    t->roots.push_back(n);
+  }
   return t;
 }
 
@@ -787,8 +831,8 @@ void refine_uniform(Tree* t, Node* n, int to_level) {
 // an interior node when a finer input octant lies inside it (linearisation keeps the
 // finer one, Alg. 3).  On a pointer tree that is: walk from the root to
 // the octant and split every leaf met on the way.  Order of insertion does not matter.
-void insert_octant(Tree* t, int lvl, const uint32_t* x) {
-  Node* nd = t->root;
+void insert_octant(Tree* t, int lvl, const uint32_t* x) {  // single cube only (construction)
+  Node* nd = t->roots[0];
   while (nd->level < lvl) {
     if (nd->is_leaf()) split(t, nd);
     int sh = t->maxl - nd->level - 1;
@@ -913,7 +957,7 @@ int mortar_gather(Tree* t, const FaceOps& fo, const double* fm, double* ff, int 
       Node* L = t->leaves[e];
       uint32_t nx[3];
       if (!neighbour_anchor(t, L, f, nx)) return -1;
-      Node* Nn = locate(t, t->root, nx, L->level);
+      Node* Nn = locate(t, t->roots, nx, L->level);
       if (Nn->is_leaf() || Nn->level != L->level) return -1;
       const int axis = f >> 1;
       std::vector<double> acc(E, 0.0);
@@ -1109,7 +1153,8 @@ void fr_rhs(Tree* t, const FrOps& o, const double* width, const double* u, const
     double* Re = R + (size_t)e * nv * N;
     for (int i = 0; i < nv * N; ++i) Re[i] = 0.0;
     for (int a = 0; a < dim; ++a) {
-      const double dx = width[a] / (double)((uint64_t)1 << t->leaves[e]->level);
+      // the brick is nroot[a] cubes wide along a (one cube: dx = width / 2^level)
+      const double dx = width[a] / ((double)t->nroot[a] * (double)((uint64_t)1 << t->leaves[e]->level));
       int stride = 1;
       for (int b = 0; b < a; ++b) stride *= P1;
       for (int n = 0; n < N; ++n) {  // flux along a at every solution point
@@ -1191,7 +1236,16 @@ int64_t lto_sort_linearise(int dim, int maxl, uint64_t* keys, int64_t n) {
 void* lto_build(int dim, int base, int maxl, const int* periodic) {
   Tree* t = new_tree(dim, base, maxl, periodic);
   if (!t) return nullptr;
-  refine_uniform(t, t->root, base);
+  refine_uniform(t, t->roots[0], base);
+  relist(t);
+  return t;
+}
+
+// Uniform depth-`base` forest on a brick of nroot[0] x nroot[1] (x nroot[2]) root cubes.
+void* lto_build_brick(int dim, const int* nroot, int base, int maxl, const int* periodic) {
+  Tree* t = new_tree(dim, base, maxl, periodic, nroot);
+  if (!t) return nullptr;
+  for (Node* r : t->roots) refine_uniform(t, r, base);
   relist(t);
   return t;
 }
@@ -1207,7 +1261,7 @@ void* lto_build_from_keys(int dim, int base, int maxl, const int* periodic, cons
     int lvl;
     uint32_t x[3];
     decode(dim, maxl, k[i], &lvl, x);
-    Node* nd = t->root;
+    Node* nd = t->roots[0];
     while (nd->level < lvl) {
       if (nd->is_leaf()) split(t, nd);
       int sh = maxl - nd->level - 1;
@@ -1219,14 +1273,14 @@ void* lto_build_from_keys(int dim, int base, int maxl, const int* periodic, cons
   }
   // completeness: every leaf of the pointer tree must be a stored key
   std::vector<Node*> lv;
-  dfs_leaves(t, t->root, lv);
+  dfs_leaves(t, t->roots[0], lv);
   bool ok = (int64_t)lv.size() == m;
   for (Node* q : lv) {
     if (!q->mark) ok = false;
     q->mark = false;
   }
   if (!ok) {
-    free_subtree(t->root);
+    free_subtree(t->roots[0]);
     delete t;
     return nullptr;
   }
@@ -1239,13 +1293,13 @@ void* lto_build_from_keys(int dim, int base, int maxl, const int* periodic, cons
 void* lto_build_complete(int dim, int base, int maxl, const int* periodic, const uint64_t* keys, int64_t n) {
   Tree* t = new_tree(dim, base, maxl, periodic);
   if (!t) return nullptr;
-  refine_uniform(t, t->root, base);
+  refine_uniform(t, t->roots[0], base);
   for (int64_t i = 0; i < n; ++i) {
     int lvl;
     uint32_t x[3];
     decode(dim, maxl, keys[i], &lvl, x);
     if (lvl < base || lvl > maxl) {
-      free_subtree(t->root);
+      free_subtree(t->roots[0]);
       delete t;
       return nullptr;
     }
@@ -1261,7 +1315,7 @@ void* lto_build_from_points(int dim, int base, int maxl, const int* periodic, co
                             const double* xyz, int64_t n) {
   Tree* t = new_tree(dim, base, maxl, periodic);
   if (!t) return nullptr;
-  refine_uniform(t, t->root, base);
+  refine_uniform(t, t->roots[0], base);
   for (int64_t i = 0; i < n; ++i) {
     uint32_t x[3] = {0, 0, 0};
     for (int a = 0; a < dim; ++a) x[a] = point_cell(xyz[i * dim + a], lo_hi[a], lo_hi[dim + a], maxl);
@@ -1276,8 +1330,8 @@ uint32_t lto_point_cell(double x, double lo, double hi, int maxl) { return point
 void lto_free(void* h) {
   Tree* t = (Tree*)h;
   if (!t) return;
-  free_subtree(t->root);
-  free_subtree(t->old_root);
+  for (Node* r : t->roots) free_subtree(r);
+  for (Node* r : t->old_roots) free_subtree(r);
   delete t;
 }
 
@@ -1298,7 +1352,7 @@ void lto_leaf_boxes(void* h, int32_t* level, uint32_t* xyz) {
 int lto_dfs_is_sorted(void* h) {
   Tree* t = (Tree*)h;
   std::vector<Node*> lv;
-  dfs_leaves(t, t->root, lv);
+  for (Node* r : t->roots) dfs_leaves(t, r, lv);
   if (lv.size() != t->leaves.size()) return 0;
   for (size_t i = 0; i < lv.size(); ++i)
     if (lv[i] != t->leaves[i]) return 0;
@@ -1363,8 +1417,8 @@ int lto_transfer_rows(void* h, const double* u_old, double* u_new_rows, int p, i
 // drop the snapshot (state rule: lt_transfer consumes it)
 void lto_drop_snapshot(void* h) {
   Tree* t = (Tree*)h;
-  free_subtree(t->old_root);
-  t->old_root = nullptr;
+  for (Node* r : t->old_roots) free_subtree(r);
+  t->old_roots.clear();
   t->old_leaves.clear();
   t->old_keys.clear();
   t->have_old = false;
@@ -1379,7 +1433,7 @@ int lto_operators(int dim, int p, int which, double* out) {
   const std::vector<double>* v = which == 0 ? &t->ops.interp : which == 1 ? &t->ops.proj
                                  : which == 2 ? &t->ops.mass : &t->ops.S;
   std::memcpy(out, v->data(), v->size() * sizeof(double));
-  free_subtree(t->root);
+  free_subtree(t->roots[0]);
   delete t;
   return 0;
 }

@@ -93,6 +93,7 @@ static int alloc_dev(cudaStream_t s, T** p, int64_t count) {
   return dev_alloc((void**)p, (size_t)count * sizeof(T), s);
 }
 
+static cudaError_t host_sync(Tree* t);
 static int64_t round_cap(int64_t n) { return (n + 1023) / 1024 * 1024; }
 
 // (Re)allocate every per-leaf buffer for `need` leaves, preserving the current keys, the
@@ -102,11 +103,14 @@ static int grow(Tree* t, int64_t need) {
   if (need >= (1ll << 31) - 1024) return LT_ERR_CAPACITY;
   int64_t cap = round_cap(need + need / 4);
   if (cap >= (1ll << 31) - 1024) cap = round_cap(need);
-  LT_CUDA(cudaStreamSynchronize(t->stream));
+  LT_CUDA(host_sync(t));
   const int dim = t->g.dim, nf = 2 * dim;
   uint64_t* nk[3] = {nullptr, nullptr, nullptr};
   uint8_t* mark = nullptr;
-  int* fr[2] = {nullptr, nullptr};
+  uint64_t* fk[2] = {nullptr, nullptr};
+  uint8_t* ft[2] = {nullptr, nullptr};
+  // balance frontier: at most one entry per leaf that was split or flagged (< cap * 8 / 7 in total)
+  const int64_t fcap = cap + cap / 4 + 1024;
   int32_t* nbr = nullptr;
   uint8_t* kind = nullptr;
   int32_t* msrc = nullptr;
@@ -117,8 +121,10 @@ static int grow(Tree* t, int64_t need) {
   int rc = LT_OK;
   for (int b = 0; b < 3 && rc == LT_OK; ++b) rc = alloc_dev(t->stream, &nk[b], cap);
   if (rc == LT_OK) rc = alloc_dev(t->stream, &mark, cap);
-  if (rc == LT_OK) rc = alloc_dev(t->stream, &fr[0], cap);
-  if (rc == LT_OK) rc = alloc_dev(t->stream, &fr[1], cap);
+  for (int b = 0; b < 2 && rc == LT_OK; ++b) {
+    rc = alloc_dev(t->stream, &fk[b], fcap);
+    if (rc == LT_OK) rc = alloc_dev(t->stream, &ft[b], fcap + 4);
+  }
   if (rc == LT_OK) rc = alloc_dev(t->stream, &nbr, cap * nf);
   if (rc == LT_OK) rc = alloc_dev(t->stream, &kind, cap * nf);
   if (rc == LT_OK) rc = alloc_dev(t->stream, &msrc, cap);
@@ -130,7 +136,7 @@ static int grow(Tree* t, int64_t need) {
   if (rc == LT_OK) rc = alloc_dev(t->stream, &tstate, 2 * (cap / 256 + 2));
   if (rc != LT_OK) {
     for (int b = 0; b < 3; ++b) free_dev(t->stream, nk[b]);
-    free_dev(t->stream, mark); free_dev(t->stream, fr[0]); free_dev(t->stream, fr[1]); free_dev(t->stream, nbr); free_dev(t->stream, kind); free_dev(t->stream, msrc); free_dev(t->stream, mkind);
+    free_dev(t->stream, mark); free_dev(t->stream, fk[0]); free_dev(t->stream, fk[1]); free_dev(t->stream, ft[0]); free_dev(t->stream, ft[1]); free_dev(t->stream, nbr); free_dev(t->stream, kind); free_dev(t->stream, msrc); free_dev(t->stream, mkind);
     free_dev(t->stream, frows); free_dev(t->stream, fbytes); free_dev(t->stream, tstate);
     return rc;
   }
@@ -139,14 +145,17 @@ static int grow(Tree* t, int64_t need) {
   if (t->keys[t->old] && t->have_old && t->n_old > 0)
     LT_CUDA(cudaMemcpyAsync(nk[t->old], t->keys[t->old], (size_t)t->n_old * 8, cudaMemcpyDeviceToDevice, t->stream));
   LT_CUDA(cudaMemsetAsync(mark, 0, (size_t)cap, t->stream));
-  LT_CUDA(cudaStreamSynchronize(t->stream));
+  LT_CUDA(host_sync(t));
   for (int b = 0; b < 3; ++b) {
     free_dev(t->stream, t->keys[b]);
     t->keys[b] = nk[b];
   }
   free_dev(t->stream, t->mark); t->mark = mark;
-  free_dev(t->stream, t->frontier[0]); t->frontier[0] = fr[0];
-  free_dev(t->stream, t->frontier[1]); t->frontier[1] = fr[1];
+  for (int b = 0; b < 2; ++b) {
+    free_dev(t->stream, t->fkey[b]); t->fkey[b] = fk[b];
+    free_dev(t->stream, t->ftag[b]); t->ftag[b] = ft[b];
+  }
+  t->fcap = fcap;
   free_dev(t->stream, t->nbr); t->nbr = nbr;
   free_dev(t->stream, t->kind); t->kind = kind;
   free_dev(t->stream, t->map_src); t->map_src = msrc;
@@ -155,16 +164,23 @@ static int grow(Tree* t, int64_t need) {
   free_dev(t->stream, t->face_bytes); t->face_bytes = fbytes;
   free_dev(t->stream, t->tile_state); t->tile_state = tstate;
   t->map_valid = false;
+  t->map_ready = false;
   t->faces_valid = false;
   t->front_ok = false;  // the frontier buffers were reallocated
   t->cap = cap;
   return LT_OK;
 }
 
+// every wait of the host for the tree's stream goes through here (lt_host_syncs counts them)
+static cudaError_t host_sync(Tree* t) {
+  t->host_syncs++;
+  return cudaStreamSynchronize(t->stream);
+}
+
 // copy the device scalars to the pinned mirror and wait
 static int fetch_scalars(Tree* t) {
   LT_CUDA(cudaMemcpyAsync(t->h_s, t->d_s, sizeof(DevScalars), cudaMemcpyDeviceToHost, t->stream));
-  LT_CUDA(cudaStreamSynchronize(t->stream));
+  LT_CUDA(host_sync(t));
   t->n = t->h_s->n;
   t->n_valid = true;
   return LT_OK;
@@ -177,6 +193,22 @@ static int take_status(Tree* t) {
     t->h_s->status = 0;
   }
   return st;
+}
+
+// the face query's own sticky word (k_connect may run beside lt_transfer on the side stream)
+static int take_status_connect(Tree* t) {
+  int st = t->h_s->status_c;
+  if (st != 0) {
+    cudaMemsetAsync(&t->d_s->status_c, 0, sizeof(int), t->stream);
+    t->h_s->status_c = 0;
+  }
+  return st;
+}
+
+int check_device(const Tree* t) {
+  int dev = -1;
+  LT_CUDA(cudaGetDevice(&dev));
+  return dev == t->device ? LT_OK : LT_ERR_ARG;
 }
 
 static void tic(Tree* t, int which) { cudaEventRecord(t->ev[2 * which], t->stream); }
@@ -238,6 +270,7 @@ static int new_tree(int dim, int base, int maxl, const double* domain, const int
   if ((rc = alloc_dev(t->stream, &t->d_s, 1)) != LT_OK) return fail(rc);
   if ((rc = alloc_dev(t->stream, &t->d_sums, kMaxGrid)) != LT_OK) return fail(rc);
   if ((rc = alloc_dev(t->stream, &t->d_sums3, 3 * kMaxGrid)) != LT_OK) return fail(rc);
+  if ((rc = alloc_dev(t->stream, &t->d_cmarks, 2 * kMaxGrid)) != LT_OK) return fail(rc);
   static_assert(sizeof(DevScalars) <= 256, "mirror layout");
   t->h_s = (DevScalars*)mirror_get();  // one pinned block: scalars | chunk sums
   if (!t->h_s) return fail(LT_ERR_OOM);
@@ -264,7 +297,7 @@ static int complete_from_unsorted(Tree* t, uint64_t* work, int64_t n) {
   uint32_t* offs = nullptr;
   if ((rc = alloc_dev(t->stream, &lin, n)) != LT_OK) return rc;
   auto done = [&](int code) {
-    cudaStreamSynchronize(t->stream);
+    host_sync(t);
     free_dev(t->stream, lin);
     free_dev(t->stream, offs);
     return code;
@@ -326,14 +359,18 @@ void lt_free(lt_tree* t) {
     cudaEventDestroy(t->ev_side_fork);
     cudaEventDestroy(t->ev_side_join);
   }
-  cudaStreamSynchronize(t->stream);
+  host_sync(t);
   for (int b = 0; b < 3; ++b) {
     free_dev(t->stream, t->keys[b]);
     free_dev(t->stream, t->first[b]);
   }
   free_dev(t->stream, t->d_s); free_dev(t->stream, t->d_sums); free_dev(t->stream, t->d_sums3);
   mirror_put(t->h_s);
-  free_dev(t->stream, t->mark); free_dev(t->stream, t->frontier[0]); free_dev(t->stream, t->frontier[1]);
+  free_dev(t->stream, t->mark); free_dev(t->stream, t->d_cmarks);
+  for (int b = 0; b < 2; ++b) {
+    free_dev(t->stream, t->fkey[b]);
+    free_dev(t->stream, t->ftag[b]);
+  }
   free_dev(t->stream, t->nbr); free_dev(t->stream, t->kind);
   free_dev(t->stream, t->face_rows); free_dev(t->stream, t->face_bytes); free_dev(t->stream, t->tile_state);
   free_dev(t->stream, t->map_src); free_dev(t->stream, t->map_kind); free_dev(t->stream, t->d_ops);
@@ -431,12 +468,14 @@ int lt_sync(lt_tree* t) {
   if (!t) return LT_ERR_ARG;
   int rc = fetch_scalars(t);
   if (rc != LT_OK) return rc;
-  return take_status(t);
+  // a face query still running on the side stream keeps its word for lt_connect_end
+  const int st = take_status(t), stc = t->connect_pending ? LT_OK : take_status_connect(t);
+  return st != LT_OK ? st : stc;
 }
 
 int lt_timings(lt_tree* t, float* out8) {
   if (!t || !out8) return LT_ERR_ARG;
-  LT_CUDA(cudaStreamSynchronize(t->stream));
+  LT_CUDA(host_sync(t));
   for (int i = 0; i < 8; ++i) {
     out8[i] = 0.f;
     if (t->ev_set[i]) LT_CUDA(cudaEventElapsedTime(&out8[i], t->ev[2 * i], t->ev[2 * i + 1]));
@@ -444,6 +483,13 @@ int lt_timings(lt_tree* t, float* out8) {
   return LT_OK;
 }
 int64_t lt_launch_count(lt_tree* t) { return t ? t->launches : 0; }
+int64_t lt_host_syncs(lt_tree* t) { return t ? t->host_syncs : 0; }
+
+int lt_balance_phases(lt_tree* t, float* out4) {
+  if (!t || !out4) return LT_ERR_ARG;
+  for (int k = 0; k < 4; ++k) out4[k] = 1e-6f * (float)t->h_s->bal_ns[k];  // mirror filled by lt_balance
+  return LT_OK;
+}
 
 int lt_leaf_boxes(lt_tree* t, int32_t* d_level, uint32_t* d_xyz) {
   if (!t) return LT_ERR_ARG;
@@ -475,7 +521,7 @@ int lt_adapt(lt_tree* t, const int8_t* d_flags) {
   // the new size is needed on the host to size buffers: one small read-back
   LT_CUDA(cudaMemcpyAsync(t->h_sums, t->d_sums, (size_t)G * sizeof(unsigned long long), cudaMemcpyDeviceToHost,
                           t->stream));
-  LT_CUDA(cudaStreamSynchronize(t->stream));
+  LT_CUDA(host_sync(t));
   int64_t n_b = 0, n_kept = 0;
   const unsigned long long* hs = (const unsigned long long*)t->h_sums;
   for (int b = 0; b < G; ++b) {
@@ -489,7 +535,7 @@ int lt_adapt(lt_tree* t, const int8_t* d_flags) {
     // path B: ordered expansion cur -> tmp.  If the tree was balanced, the leaves created here
     // become the frontier of lt_balance's first sweep.
     const int emit = t->balanced_conn >= 1;
-    if (emit) LT_CUDA(cudaMemsetAsync(&t->d_s->nfront0, 0, sizeof(int), t->stream));
+    if (emit) LT_CUDA(cudaMemsetAsync(&t->d_s->nfront[0], 0, sizeof(int), t->stream));
     if ((rc = launch_adapt_scatter(t, d_flags, G, 0, emit)) != LT_OK) return rc;
     front_ok = emit != 0;
     const int o = t->old;
@@ -520,13 +566,14 @@ int lt_adapt(lt_tree* t, const int8_t* d_flags) {
     t->n = n_lin;
     int nn = (int)n_lin;
     LT_CUDA(cudaMemcpyAsync(&t->d_s->n, &nn, sizeof(int), cudaMemcpyHostToDevice, t->stream));
-    LT_CUDA(cudaStreamSynchronize(t->stream));
+    LT_CUDA(host_sync(t));
     if ((rc = launch_build_index(t, t->cur)) != LT_OK) return rc;
   }
   t->have_old = true;
   t->n_old = n_in;
   t->n_valid = true;
   t->map_valid = false;
+  t->map_ready = false;
   t->faces_valid = false;
   t->front_ok = front_ok;
   t->balanced_conn = 0;
@@ -575,6 +622,8 @@ int lt_balance(lt_tree* t, int* iters) {
   t->front_ok = false;
   t->balanced_conn = t->opt_balance_conn > 0 ? t->opt_balance_conn : 1;
   t->map_valid = false;
+  // Alg. 7 ran in the tail of the kernel; a mapping error is left to lt_transfer's checked k_map
+  t->map_ready = t->have_old && t->h_s->map_bad == 0;
   t->faces_valid = false;
   toc(t, 1);
   return LT_OK;
@@ -584,7 +633,7 @@ int lt_balance(lt_tree* t, int* iters) {
 static int collect_faces(Tree* t, lt_faces* out) {
   int rc;
   if ((rc = fetch_scalars(t)) != LT_OK) return rc;
-  const int st = take_status(t);
+  const int st = take_status_connect(t);
   if (st != LT_OK) return st;
   const int64_t nc = t->h_s->n_face[0], nh = t->h_s->n_face[1], nb = t->h_s->n_face[2];
   out->n_leaves = t->n;
@@ -703,7 +752,7 @@ int lt_transfer(lt_tree* t, const double* d_u_old, double* d_u_new, int p, int n
   if ((rc = build_operators(t, p)) != LT_OK) return rc;
   tic(t, 3);
   tic(t, 4);
-  if ((rc = launch_map(t)) != LT_OK) return rc;
+  if (!t->map_ready && (rc = launch_map(t)) != LT_OK) return rc;
   toc(t, 4);
   tic(t, 5);
   if ((rc = launch_transfer(t, d_u_old, d_u_new, p, nvars)) != LT_OK) return rc;
@@ -711,6 +760,7 @@ int lt_transfer(lt_tree* t, const double* d_u_old, double* d_u_new, int p, int n
   t->have_old = false;
   t->n_old = 0;
   t->map_valid = true;
+  t->map_ready = false;
   toc(t, 3);
   return LT_OK;
 }
@@ -760,7 +810,7 @@ int lt_transfer_host(lt_tree* t, const double* h_u_old, double* h_u_new, int p, 
   }
   tic(t, 3);
   tic(t, 4);
-  if ((rc = launch_map(t)) != LT_OK) return rc;
+  if (!t->map_ready && (rc = launch_map(t)) != LT_OK) return rc;
   toc(t, 4);
   if ((rc = launch_slab_bounds(t, n_old, slab, S, t->d_bounds)) != LT_OK) return rc;
   LT_CUDA(cudaMemcpyAsync(t->h_bounds, t->d_bounds, 2 * (size_t)(S + 1) * sizeof(int64_t), cudaMemcpyDeviceToHost,
@@ -814,6 +864,7 @@ int lt_transfer_host(lt_tree* t, const double* h_u_old, double* h_u_new, int p, 
   t->have_old = false;
   t->n_old = 0;
   t->map_valid = true;
+  t->map_ready = false;
   toc(t, 3);
   if ((rc = fetch_scalars(t)) != LT_OK) return rc;
   return take_status(t);
@@ -878,7 +929,7 @@ int lt_build_from_keys(int dim, int base_level, int max_level, const double* dom
   int nn = (int)m;
   if (cudaMemcpyAsync(&t->d_s->n, &nn, sizeof(int), cudaMemcpyHostToDevice, t->stream) != cudaSuccess)
     return fail(LT_ERR_CUDA);
-  if (cudaStreamSynchronize(t->stream) != cudaSuccess) return fail(LT_ERR_CUDA);
+  if (host_sync(t) != cudaSuccess) return fail(LT_ERR_CUDA);
   t->n = m;
   t->n_valid = true;
   if ((rc = launch_check_tiling(t)) != LT_OK) return fail(rc);
@@ -905,7 +956,7 @@ int lt_build_complete_from_keys(int dim, int base_level, int max_level, const do
     else
       rc = complete_from_unsorted(t, work, n);
   }
-  cudaStreamSynchronize(t->stream);
+  host_sync(t);
   free_dev(t->stream, work);
   if (rc != LT_OK) {
     lt_free((lt_tree*)t);
@@ -929,7 +980,7 @@ int lt_build_from_points(int dim, int base_level, int max_level, const double* d
     rc = launch_points_to_keys(dim, max_level, t->domain, d_xyz, n, work, grid_for(t, 8), t->stream, &t->launches);
     if (rc == LT_OK) rc = complete_from_unsorted(t, work, n);
   }
-  cudaStreamSynchronize(t->stream);
+  host_sync(t);
   free_dev(t->stream, work);
   if (rc != LT_OK) {
     lt_free((lt_tree*)t);

@@ -147,7 +147,7 @@ __global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restric
         const int f = 2 * a + (((cid >> a) & 1) ^ 1);
         int nb, kd = 1;
         if (l == 0 || !face_by_sibling<DIM>(g, keys, n, i, m, l, cid, a, &nb))
-          kd = face_by_search<DIM>(g, keys, first, m, l, f, &s->status, &nb);
+          kd = face_by_search<DIM>(g, keys, first, m, l, f, &s->status_c, &nb);
         s_nb[threadIdx.x * NF + f] = nb;
         s_kd[threadIdx.x * NF + f] = (uint8_t)kd;
       }
@@ -155,7 +155,7 @@ __global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restric
       for (int a = 0; a < DIM; ++a) {
         const int f = 2 * a + ((cid >> a) & 1);
         int nb;
-        const int kd = face_by_search<DIM>(g, keys, first, m, l, f, &s->status, &nb);
+        const int kd = face_by_search<DIM>(g, keys, first, m, l, f, &s->status_c, &nb);
         s_nb[threadIdx.x * NF + f] = nb;
         s_kd[threadIdx.x * NF + f] = (uint8_t)kd;
       }

@@ -278,6 +278,7 @@ int launch_complete_count(Tree* t, const uint64_t* d_in, int64_t n, uint32_t* d_
   t->launches += 2;
   LT_CUDA(cudaGetLastError());
   LT_CUDA(cudaMemcpyAsync(t->h_s, t->d_s, sizeof(DevScalars), cudaMemcpyDeviceToHost, t->stream));
+  t->host_syncs++;
   LT_CUDA(cudaStreamSynchronize(t->stream));
   *total = (int64_t)t->h_s->volume;
   return LT_OK;

@@ -241,4 +241,38 @@ __device__ __forceinline__ void chunk_offsets(const T* __restrict__ sums, int G,
 // sticky device status word: first error wins
 __device__ __forceinline__ void set_status(int* status, int code) { atomicCAS(status, 0, code); }
 
+// Alg. 7 for ONE new leaf: locate its anchor in T_old (lower bound, Eq. 7):
+//   same ID                       -> copy   kind 0
+//   old entry is its parent       -> refined-from   kind 1 | child_id << 4
+//   old entry is its first child  -> fused-from      (reading E-6)   kind 2
+// Returns false when the new leaf is more than one level from T_old (or the old sibling group is
+// not complete): the caller decides where that error is reported.
+template <int DIM>
+__device__ __forceinline__ bool map_entry(const Geo& g, uint64_t key, const uint64_t* __restrict__ keys_old,
+                                          const int* __restrict__ first_old, int n_old, int* src, int* kind) {
+  constexpr int NC = Dim<DIM>::NC;
+  const int l = key_level(key);
+  const uint64_t m = key_morton(key);
+  const int o = locate(g, keys_old, first_old, m);
+  const int lo = key_level(keys_old[o]);
+  bool ok = true;
+  int kd = 0;
+  if (lo == l) {
+    kd = 0;
+  } else if (lo == l - 1) {
+    kd = 1 | (child_id<DIM>(g, m, l) << 4);
+  } else if (lo == l + 1) {
+    // complete group of leaves: last sibling present at o + NC - 1
+    const int sh = DIM * (g.maxl - l - 1);
+    const uint64_t klast = make_key(m | ((uint64_t)(NC - 1) << sh), l + 1);
+    if (o + NC - 1 >= n_old || keys_old[o + NC - 1] != klast) ok = false;
+    kd = 2;
+  } else {
+    ok = false;
+  }
+  *src = o;
+  *kind = kd;
+  return ok;
+}
+
 }  // namespace lt

@@ -9,6 +9,7 @@
 #include <math.h>
 #include <string.h>
 
+#include <mutex>
 #include <vector>
 
 #include "lt_internal.h"
@@ -212,8 +213,14 @@ static long double legendre_ld(int n, long double x, long double* dp) {
 }
 
 int build_fr_operators(Tree* t, int p) {
+  // as build_operators: per device, uploaded to the current device, serialised across host threads
+  static std::mutex mu;
   static bool uploaded[64][8];
-  const int dev = t->device & 63;
+  int rc = check_device(t);
+  if (rc != LT_OK) return rc;
+  if (t->device < 0 || t->device >= 64) return LT_ERR_ARG;
+  std::lock_guard<std::mutex> lk(mu);
+  const int dev = t->device;
   if (uploaded[dev][p]) return LT_OK;
   const int P1 = p + 1;
   // Gauss-Legendre nodes by Newton iteration on P_n

@@ -21,7 +21,13 @@ struct DevScalars {
   int splits;            // balance: leaves split in total
   unsigned ticket;       // tile ticket of k_transfer (zeroed before each launch)
   unsigned ticket_c;     // tile ticket of k_connect (its own word: the two kernels may overlap)
-  int nfront0;           // entries of lt_adapt's frontier for lt_balance's first sweep
+  int nfront[2];         // balance frontier ping-pong counters; [0] also counts lt_adapt's list
+  int fr_overflow;       // balance: the next frontier did not fit its buffer (-> full sweep)
+  int map_bad;           // balance tail (Alg. 7): a new leaf is more than one level from T_old
+  unsigned long long bal_ns[4];  // k_balance, device time per phase of the last launch: examine, chunk
+                                 // offsets, split + frontier, Alg. 7 tail (lt_balance_phases)
+  int status_c;          // sticky status of k_connect (its own word: the face query may run beside
+                         // lt_transfer on the side stream, and each call reports only its own errors)
 };
 
 constexpr int kMaxGrid = 4096;  // upper bound on persistent grid sizes (chunk-sum arrays)
@@ -48,7 +54,10 @@ struct Tree {
   int* h_sums;            // pinned [3*kMaxGrid + ..]
 
   uint8_t* mark;          // [cap] balance marks: bit0 split, bit1 re-examine
-  int* frontier[2];       // [cap] leaves to examine in the next sweep
+  uint64_t* fkey[2];      // [fcap] balance frontier: entry keys (or positions) ...
+  uint8_t* ftag[2];       // [fcap] ... and their tags (lt_tree.cu)
+  int64_t fcap;
+  int* d_cmarks;          // [2*kMaxGrid] balance: leaves marked per chunk
 
   // connectivity
   int32_t* nbr;
@@ -63,14 +72,15 @@ struct Tree {
   // Alg. 7 map
   int32_t* map_src;
   uint8_t* map_kind;
-  bool map_valid;
+  bool map_valid;         // lt_map may hand the arrays out (set by lt_transfer)
+  bool map_ready;         // map_src / map_kind already hold T_old -> current tree (lt_balance's tail)
   bool faces_valid;       // nbr / kind describe the current tree (set by lt_connect)
   // lt_connect_begin / lt_connect_end: k_connect on a side stream, overlapping lt_transfer
   cudaStream_t s_side;
   cudaEvent_t ev_side_fork, ev_side_join;
   bool connect_pending;
   int balanced_conn;      // the tree is 2:1 balanced with this connectivity (0: unknown)
-  bool front_ok;          // frontier[0] / d_s->nfront0 list the leaves created by the last lt_adapt
+  bool front_ok;          // fkey[0] / ftag[0] / d_s->nfront[0] list the leaves created by the last lt_adapt
   int* mortar_hits;       // [hits][2 + 2^(dim-1)]: coarse-side hanging faces (e, f, fine neighbours)
   int64_t mortar_hits_cap;
 
@@ -92,6 +102,7 @@ struct Tree {
   cudaEvent_t ev[16];
   bool ev_set[8];
   int64_t launches;
+  int64_t host_syncs;     // times the host waited for the tree's stream (lt_host_syncs)
 };
 
 extern thread_local int g_last_cuda_error;
@@ -106,6 +117,9 @@ extern thread_local int g_last_cuda_error;
   } while (0)
 
 int grid_for(const Tree* t, int blocks_per_sm);
+// LT_OK iff the tree's device is the current one (kernels, constant-memory uploads and pool
+// allocations all go to the current device)
+int check_device(const Tree* t);
 // stream-ordered device memory (lt_api.cu): the device's default cudaMallocAsync pool
 int dev_alloc(void** p, size_t bytes, cudaStream_t s);
 void dev_free(void* p, cudaStream_t s);

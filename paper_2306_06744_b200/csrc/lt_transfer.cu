@@ -15,48 +15,28 @@
 // Eq. 17), k_mortar_hits + k_mortar_apply (step 4, Eq. 20).
 #include <math.h>
 
-#include <vector>
-
+#include <mutex>
 #include <type_traits>
+#include <vector>
 
 #include "lt_internal.h"
 
 namespace lt {
 
 // ------------------------------------------------------------------------ Alg. 7
-// For every new leaf: locate its anchor in T_old (lower bound, Eq. 7):
-//   same ID                       -> copy
-//   old entry is its parent       -> refined-from
-//   old entry is its first child  -> fused-from      (reading E-6)
-// The map is produced in new-leaf order, so step 5's sort is not needed (reading E-6).
+// For every new leaf map_entry() (lt_dev.cuh) locates its anchor in T_old.  The map is produced in
+// new-leaf order, so step 5's sort is not needed (reading E-6).  lt_balance normally produces the
+// map in the tail of its own kernel; this kernel is the path for a cycle without lt_balance and the
+// checked fallback that reports LT_ERR_MAPPING.
 template <int DIM>
 __global__ void __launch_bounds__(256) k_map(Geo g, const uint64_t* __restrict__ keys_new,
                                              const uint64_t* __restrict__ keys_old,
                                              const int* __restrict__ first_old, int n_old, DevScalars* s,
                                              int32_t* __restrict__ src, uint8_t* __restrict__ kind) {
-  constexpr int NC = Dim<DIM>::NC;
   const int64_t n = s->n;
   for (int64_t j = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; j < n; j += (int64_t)gridDim.x * blockDim.x) {
-    const uint64_t key = keys_new[j];
-    const int l = key_level(key);
-    const uint64_t m = key_morton(key);
-    const int o = locate(g, keys_old, first_old, m);
-    const uint64_t ko = keys_old[o];
-    const int lo = key_level(ko);
-    int kd = 0;
-    if (lo == l) {
-      kd = 0;
-    } else if (lo == l - 1) {
-      kd = 1 | (child_id<DIM>(g, m, l) << 4);
-    } else if (lo == l + 1) {
-      // complete group of leaves: last sibling present at o + NC - 1
-      const int sh = DIM * (g.maxl - l - 1);
-      const uint64_t klast = make_key(m | ((uint64_t)(NC - 1) << sh), l + 1);
-      if (o + NC - 1 >= n_old || keys_old[o + NC - 1] != klast) set_status(&s->status, LT_ERR_MAPPING);
-      kd = 2;
-    } else {
-      set_status(&s->status, LT_ERR_MAPPING);
-    }
+    int o, kd;
+    if (!map_entry<DIM>(g, keys_new[j], keys_old, first_old, n_old, &o, &kd)) set_status(&s->status, LT_ERR_MAPPING);
     src[j] = o;
     kind[j] = (uint8_t)kd;
   }
@@ -535,8 +515,15 @@ static void gl_rule(int n, std::vector<long double>& z, std::vector<long double>
 }
 
 int build_operators(Tree* t, int p) {
-  static bool uploaded[64][8];  // per device, per P1
-  const int dev = t->device & 63;
+  // per device, per P1; the upload goes to the CURRENT device's constant memory, so the tree's
+  // device must be current (check_device) and concurrent host threads are serialised
+  static std::mutex mu;
+  static bool uploaded[64][8];
+  int rc = check_device(t);
+  if (rc != LT_OK) return rc;
+  if (t->device < 0 || t->device >= 64) return LT_ERR_ARG;
+  std::lock_guard<std::mutex> lk(mu);
+  const int dev = t->device;
   if (uploaded[dev][p]) return LT_OK;
   const int P1 = p + 1;
   std::vector<long double> z, w;
@@ -667,8 +654,8 @@ __global__ void __launch_bounds__(256) k_mortar_project(const DevScalars* s, con
     }
     for (int q0 = 0; q0 < EV; q0 += 64) {
       const int qa = q0 + lane, qb = q0 + 32 + lane;
-#pragma unroll
       constexpr int FC = NF / 2;  // faces per round: 2 * FC loads in flight per lane (all NF at once costs 20 registers more and a resident block)
+#pragma unroll
       for (int fh = 0; fh < NF; fh += FC) {
         V v0[FC], v1[FC];
 #pragma unroll

@@ -176,10 +176,12 @@ __global__ void __launch_bounds__(BT) k_adapt_scatter(Geo g, const uint64_t* __r
                                                       const int8_t* __restrict__ flags, DevScalars* s,
                                                       const unsigned long long* __restrict__ sums,
                                                       uint64_t* __restrict__ out, int* __restrict__ first_out,
-                                                      int64_t cap, int* __restrict__ front) {
-  // front != nullptr: the tree entering lt_adapt was 2:1 balanced, so only the leaves created here
-  // can be part of a violation; they are listed (children by index, merged parents as ~index) as
-  // the frontier of lt_balance's first sweep (s->nfront0 entries, any order)
+                                                      int64_t cap, uint64_t* __restrict__ fkey,
+                                                      uint8_t* __restrict__ ftag, int64_t fcap) {
+  // fkey != nullptr: the tree entering lt_adapt was 2:1 balanced, so only the leaves created here
+  // can be part of a violation; they are listed as the frontier of lt_balance's first sweep
+  // (s->nfront[0] entries, any order): a refined leaf as a GROUP entry (its own key), a merged
+  // parent as a SELF entry (its position)
   constexpr int NC = Dim<DIM>::NC;
   __shared__ unsigned long long sm[33];
   const int64_t n = s->n;
@@ -206,17 +208,20 @@ __global__ void __launch_bounds__(BT) k_adapt_scatter(Geo g, const uint64_t* __r
     unsigned long long ex = block_excl_scan<unsigned long long>((unsigned long long)c, sm, &tile_total);
     int64_t pos = run + (int64_t)ex;
     run += (int64_t)tile_total;
-    int fpos = 0;
-    if (front != nullptr) {  // warp-aggregated append
-      const int cf = act == ACT_REFINE ? NC : (act == ACT_PARENT ? 1 : 0);
-      const int inc = warp_incl_scan(cf);
-      const int tot = __shfl_sync(0xffffffffu, inc, 31);
-      int base = 0;
-      if (tot) {
-        if ((threadIdx.x & 31) == 0) base = atomicAdd(&s->nfront0, tot);
-        base = __shfl_sync(0xffffffffu, base, 0);
+    if (fkey != nullptr) {  // warp-aggregated append (kFrGroup = 2, kFrSelf = 3 of k_balance)
+      const bool pg = act == ACT_REFINE, ps = act == ACT_PARENT;
+      const unsigned mm = __ballot_sync(0xffffffffu, pg || ps);
+      if (mm) {
+        const int ln = threadIdx.x & 31;
+        int base = 0;
+        if (ln == __ffs(mm) - 1) base = atomicAdd(&s->nfront[0], __popc(mm));
+        base = __shfl_sync(0xffffffffu, base, __ffs(mm) - 1);
+        const int64_t at = (int64_t)base + __popc(mm & ((1u << ln) - 1));
+        if ((pg || ps) && at < fcap) {  // (a list that does not fit makes lt_balance sweep in full)
+          fkey[at] = pg ? key : (uint64_t)pos;
+          ftag[at] = pg ? 2 : 3;
+        }
       }
-      fpos = base + inc - cf;
     }
     if (c == 0) continue;
     const int l = key_level(key);
@@ -227,10 +232,7 @@ __global__ void __launch_bounds__(BT) k_adapt_scatter(Geo g, const uint64_t* __r
     } else if (act == ACT_PARENT) {
       out[pos] = make_key(m, l - 1);  // child 0 has the parent's anchor
       index_write<DIM>(g, first_out, m, l - 1, (int)pos);
-      if (front != nullptr) front[fpos] = ~(int)pos;
     } else {
-      if (front != nullptr)
-        for (int k = 0; k < NC; ++k) front[fpos + k] = (int)(pos + k);
       const int sh = DIM * (g.maxl - l - 1);
 #pragma unroll
       for (int k = 0; k < NC; ++k) {
@@ -300,26 +302,73 @@ __global__ void __launch_bounds__(BT) k_adapt_append(Geo g, const uint64_t* __re
 // every face neighbour found >= 2 levels coarser is marked; marked leaves split once.
 // All sweeps run inside this one cooperative kernel.
 //
-// After the first (full) sweep only a frontier is examined: the children created by the
-// previous sweep, plus every leaf that saw a neighbour >= 3 levels coarser (its
-// neighbour's children will still be too coarse).  DESIGN.md proves that this marks the
-// same set as a full sweep.
+// After the first sweep only a FRONTIER is examined.  Its entries are keyed, so that they stay
+// valid while the leaf array is rewritten by the splits:
+//   GROUP  the key K (level l) of a leaf that was split (by lt_adapt or by the previous sweep): its
+//          2^dim children are new leaves.  All exterior faces of the children lie on the 2*dim faces of
+//          K and a child sees a neighbour >= 2 levels coarser exactly when the leaf across that face of
+//          K is coarser than K, so ONE search per face of K (level < l: mark it) replaces the 2^(dim-1)
+//          searches of the children on that face -- 6 searches per split leaf instead of 24 in 3-D.
+//          If that leaf is even coarser than l - 1 it will still be too coarse after its split: the
+//          entry is flagged and re-examined in the next sweep.
+//   LEAF   the key of a single leaf that saw a neighbour >= 3 levels coarser in a full sweep.
+//   SELF   (first sweep after lt_adapt only) the POSITION of a parent created by a coarsening: it is
+//          too coarse iff a level-(l+1) cell of a neighbouring level-l cell is subdivided.
+// DESIGN.md section 5 proves that frontier sweeps mark the same set as full sweeps.
 struct BalanceArgs {
   Geo g;
   uint64_t* keys[2];
   int* first[2];
   uint8_t* mark;
-  int* frontier[2];
-  unsigned long long* sums;
+  uint64_t* fkey[2];   // frontier ping-pong: entry keys (SELF: position) ...
+  uint8_t* ftag[2];    // ... and tags: kFrLeaf / kFrGroup / kFrSelf | kFrAgain
+  int64_t fcap;        // entries per frontier buffer
+  int* cmarks[2];      // [G] leaves marked per chunk, counted when the mark is set (ping-pong per sweep)
   DevScalars* s;
   int64_t cap;
   int full_sweeps;
-  int front0;  // 1: frontier[0] holds lt_adapt's list of new leaves (s->nfront0 entries) for sweep 1
-  // neighbour directions examined per leaf (reading C-9): 2 bits per axis, 0 = no move,
+  int front0;  // 1: frontier 0 holds lt_adapt's list (s->nfront[0] entries) for sweep 1
+  // neighbour directions of a LEAF examination (reading C-9): 2 bits per axis, 0 = no move,
   // 1 = move across the leaf's parent-EXTERIOR side on that axis, 2 = across the interior side
   int ndirs;
   uint8_t dirs[20];
+  // neighbour directions of a GROUP examination: 2 bits per axis, 0 = no move, 1 = minus, 2 = plus
+  int ngdirs;
+  uint8_t gdirs[26];
+  // Alg. 7 in the tail of the kernel (do_map): T_old -> the balanced tree
+  int do_map, n_old;
+  const uint64_t* keys_old;
+  const int* first_old;
+  int32_t* map_src;
+  uint8_t* map_kind;
 };
+
+enum { kFrLeaf = 1, kFrGroup = 2, kFrSelf = 3, kFrAgain = 0x80 };
+
+// mark leaf j for splitting; the first thread to set the mark counts it in j's chunk
+__device__ __forceinline__ void mark_split(uint8_t* mark, int* cmarks, int per, int j) {
+  const unsigned bit = 1u << (8 * (j & 3));
+  const unsigned old = atomicOr((unsigned*)(mark + (j & ~3)), bit);
+  if (!(old & bit)) atomicAdd(&cmarks[j / per], 1);
+}
+
+// The same-level cell reached from (m, l) by the absolute moves in `code` (2 bits per axis: 1 = minus,
+// 2 = plus), chaining the one-axis step; false if it leaves a non-periodic domain.
+template <int DIM>
+__device__ __forceinline__ bool move_cell(const Geo& g, uint64_t m, int l, int code, uint64_t* out) {
+  uint64_t mn = m;
+#pragma unroll
+  for (int a = 0; a < DIM; ++a) {
+    const int c = (code >> (2 * a)) & 3;
+    if (c) {
+      uint64_t nx;
+      if (!face_neighbour<DIM>(g, mn, l, 2 * a + (c - 1), &nx)) return false;
+      mn = nx;
+    }
+  }
+  *out = mn;
+  return true;
+}
 
 // Face balance examines only the DIM faces of a leaf that are exterior to its parent: an
 // interior face looks at a sibling's cell, which is tiled by leaves at least as fine as the
@@ -328,136 +377,200 @@ struct BalanceArgs {
 // otherwise.  Strong balance (neighbours across edges, optionally corners) adds
 // the directions that move on two / three axes; a direction whose moves are ALL interior lands
 // inside the parent and is skipped for the same reason, so 3 + 9 (+ 7) directions per leaf are
-// examined in 3-D.  The neighbour key is formed by chaining the one-axis step.
+// examined in 3-D.  Returns 0, 1 (the neighbour was marked) or 2 (marked, and it is >= 3 levels
+// coarser: the leaf has to be examined again).
 template <int DIM>
-__device__ __forceinline__ void balance_examine(const Geo& g, const uint64_t* __restrict__ keys,
-                                                const int* __restrict__ first, uint8_t* mark, int i, int code) {
-  const uint64_t key = keys[i];
+__device__ __forceinline__ int examine_leaf(const Geo& g, const uint64_t* __restrict__ keys,
+                                            const int* __restrict__ first, uint8_t* mark, int* cmarks, int per,
+                                            uint64_t key, int code) {
   const int l = key_level(key);
-  if (l < g.base + 2) return;  // no leaf is coarser than the base level
+  if (l < g.base + 2) return 0;  // no leaf is coarser than the base level
   const uint64_t m = key_morton(key);
   const int cid = child_id<DIM>(g, m, l);
-  uint64_t mn = m;
+  int abs_code = 0;
 #pragma unroll
   for (int a = 0; a < DIM; ++a) {
     const int c = (code >> (2 * a)) & 3;
-    if (c) {
-      const int bit = (cid >> a) & 1;
-      const int f = 2 * a + (c == 1 ? bit : (bit ^ 1));
-      uint64_t nx;
-      if (!face_neighbour<DIM>(g, mn, l, f, &nx)) return;
-      mn = nx;
-    }
+    const int bit = (cid >> a) & 1;
+    if (c) abs_code |= (1 + (c == 1 ? bit : (bit ^ 1))) << (2 * a);
   }
+  uint64_t mn;
+  if (!move_cell<DIM>(g, m, l, abs_code, &mn)) return 0;
   const int j = locate(g, keys, first, mn);
   const int lj = key_level(keys[j]);
-  if (lj < l - 1) {
-    atomicOr((unsigned*)(mark + (j & ~3)), 1u << (8 * (j & 3)));
-    if (lj < l - 2) atomicOr((unsigned*)(mark + (i & ~3)), 2u << (8 * (i & 3)));
-  }
+  if (lj >= l - 1) return 0;
+  mark_split(mark, cmarks, per, j);
+  return lj < l - 2 ? 2 : 1;
 }
 
-// A parent created by lt_adapt (level l) is too coarse iff, across one of its faces, a level-(l+1)
-// cell of the neighbouring level-l cell is itself subdivided (its leaves are >= 2 levels finer).
-// Checked from the parent's side for the two faces of axis a; marks the parent itself.
+// GROUP entry: the children of K = (m, l) are leaves of level l + 1 (or finer); the leaf across K in
+// direction `code` is too coarse for them iff its level is < l.
 template <int DIM>
-__device__ __forceinline__ void balance_selfcheck(const Geo& g, const uint64_t* __restrict__ keys,
-                                                  const int* __restrict__ first, uint8_t* mark, int i, int a) {
+__device__ __forceinline__ int examine_group(const Geo& g, const uint64_t* __restrict__ keys,
+                                             const int* __restrict__ first, uint8_t* mark, int* cmarks, int per,
+                                             uint64_t key, int code) {
+  const int l = key_level(key);
+  if (l < g.base + 1) return 0;
+  uint64_t mn;
+  if (!move_cell<DIM>(g, key_morton(key), l, code, &mn)) return 0;
+  const int j = locate(g, keys, first, mn);
+  const int lj = key_level(keys[j]);
+  if (lj >= l) return 0;
+  mark_split(mark, cmarks, per, j);
+  return lj < l - 1 ? 2 : 1;
+}
+
+// A parent created by lt_adapt (level l, position i) is too coarse iff, across one of its faces, a
+// level-(l+1) cell of the neighbouring level-l cell is itself subdivided (its leaves are >= 2 levels
+// finer).  Checked from the parent's side for face f; marks the parent itself.
+template <int DIM>
+__device__ __forceinline__ void examine_self(const Geo& g, const uint64_t* __restrict__ keys,
+                                             const int* __restrict__ first, uint8_t* mark, int* cmarks, int per,
+                                             int i, int f) {
   const uint64_t key = keys[i];
   const int l = key_level(key);
   if (l + 2 > g.maxl) return;
-  const uint64_t m = key_morton(key);
+  const int a = f >> 1, side = f & 1;
+  uint64_t mn;
+  if (!face_neighbour<DIM>(g, key_morton(key), l, f, &mn)) return;
   bool hit = false;
 #pragma unroll
-  for (int side = 0; side < 2; ++side) {
-    uint64_t mn;
-    if (!face_neighbour<DIM>(g, m, l, 2 * a + side, &mn)) continue;
+  for (int sidx = 0; sidx < (1 << (DIM - 1)); ++sidx) {
+    int c = side ? 0 : (1 << a), bit = 0;
 #pragma unroll
-    for (int sidx = 0; sidx < (1 << (DIM - 1)); ++sidx) {
-      int c = side ? 0 : (1 << a), bit = 0;
-#pragma unroll
-      for (int b = 0; b < DIM; ++b) {
-        if (b == a) continue;
-        c |= ((sidx >> bit) & 1) << b;
-        ++bit;
-      }
-      const int j = locate(g, keys, first, mn | ((uint64_t)c << (DIM * (g.maxl - l - 1))));
-      hit = hit || key_level(keys[j]) >= l + 2;
+    for (int b = 0; b < DIM; ++b) {
+      if (b == a) continue;
+      c |= ((sidx >> bit) & 1) << b;
+      ++bit;
     }
+    const int j = locate(g, keys, first, mn | ((uint64_t)c << (DIM * (g.maxl - l - 1))));
+    hit = hit || key_level(keys[j]) >= l + 2;
   }
-  if (hit) atomicOr((unsigned*)(mark + (i & ~3)), 1u << (8 * (i & 3)));
+  if (hit) mark_split(mark, cmarks, per, i);
+}
+
+// (whole warp) append the entries of the lanes with `pred` to a frontier; false if it is full
+__device__ __forceinline__ bool frontier_push(bool pred, uint64_t key, int tag, uint64_t* fkey, uint8_t* ftag,
+                                              int* counter, int64_t fcap) {
+  const unsigned m = __ballot_sync(0xffffffffu, pred);
+  if (m == 0) return true;
+  const int lane = threadIdx.x & 31;
+  int base = 0;
+  if (lane == __ffs(m) - 1) base = atomicAdd(counter, __popc(m));
+  base = __shfl_sync(0xffffffffu, base, __ffs(m) - 1);
+  const int64_t at = (int64_t)base + __popc(m & ((1u << lane) - 1));
+  const bool fits = (int64_t)base + __popc(m) <= fcap;
+  if (pred && fits) {
+    fkey[at] = key;
+    ftag[at] = (uint8_t)tag;
+  }
+  return fits;
+}
+
+__device__ __forceinline__ unsigned long long global_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
 }
 
 template <int DIM>
 __global__ void __launch_bounds__(BT) k_balance(BalanceArgs a) {
   constexpr int NC = Dim<DIM>::NC;
   __shared__ unsigned long long sm[33];
-  __shared__ uint8_t s_dirs[20];
+  __shared__ uint8_t s_dirs[20], s_gdirs[26];
   cg::grid_group grid = cg::this_grid();
   const Geo g = a.g;
   if (threadIdx.x < 20) s_dirs[threadIdx.x] = a.dirs[threadIdx.x];
+  if (threadIdx.x < 26) s_gdirs[threadIdx.x] = a.gdirs[threadIdx.x];
   __syncthreads();
+  const int G = gridDim.x;
   const int64_t gtid = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-  const int64_t gsize = (int64_t)gridDim.x * blockDim.x;
+  const int64_t gsize = (int64_t)G * blockDim.x;
+  const int lane = threadIdx.x & 31;
   int64_t n = a.s->n;
-  int par = 0, iters = 0, fpar = 0;
-  int64_t nfront = a.front0 ? (int64_t)a.s->nfront0 : -1;  // -1: full sweep
+  int par = 0, iters = 0, fpar = 0, sweep = 0;
+  int64_t nfront = a.front0 ? (int64_t)a.s->nfront[0] : -1;  // -1: full sweep
+  if (nfront > a.fcap) nfront = -1;                           // lt_adapt's list did not fit
   int64_t splits = 0;
   int err = 0;
-  for (;;) {
+  // thread (0, 0) leaves every grid-wide barrier after all blocks have arrived, so its clock
+  // readings bound the phases of the whole grid (lt_balance_phases)
+  unsigned long long ns[4] = {0, 0, 0, 0}, t_prev = gtid == 0 ? global_ns() : 0;
+  auto lap = [&](int phase) {
+    if (gtid == 0) {
+      const unsigned long long now = global_ns();
+      ns[phase] += now - t_prev;
+      t_prev = now;
+    }
+  };
+  for (;; ++sweep) {
     const uint64_t* keys = a.keys[par];
     const int* first = a.first[par];
+    int* cm = a.cmarks[sweep & 1];
+    // chunk b of the leaf array = [b * per, (b + 1) * per) (block_chunk)
+    int64_t per64 = (n + G - 1) / G;
+    per64 = (per64 + BT - 1) / BT * BT;
+    const int per = (int)(per64 > 0 ? per64 : BT);
+    // the other halves of the ping-pong state are reset for the next sweep (nobody reads them now)
+    if (threadIdx.x == 0) a.cmarks[(sweep + 1) & 1][blockIdx.x] = 0;
+    if (gtid == 0) {
+      a.s->nfront[fpar ^ 1] = 0;
+      a.s->fr_overflow = 0;
+    }
     // ---- sweep
-    if (a.ndirs == DIM) {  // face balance: direction d = the exterior face on axis d
-      if (nfront < 0) {
-        for (int64_t sidx = gtid; sidx < n * DIM; sidx += gsize)
-          balance_examine<DIM>(g, keys, first, a.mark, (int)(sidx / DIM), 1 << (2 * (int)(sidx % DIM)));
-      } else {
-        const int* fr = a.frontier[fpar];
-        for (int64_t sidx = gtid; sidx < nfront * DIM; sidx += gsize) {
-          const int ent = fr[sidx / DIM];
-          if (ent >= 0) balance_examine<DIM>(g, keys, first, a.mark, ent, 1 << (2 * (int)(sidx % DIM)));
-          else balance_selfcheck<DIM>(g, keys, first, a.mark, ~ent, (int)(sidx % DIM));  // only in sweep 1
-        }
+    if (nfront < 0) {
+      const int nd = a.ndirs;
+      for (int64_t sidx = gtid; sidx < n * nd; sidx += gsize) {
+        const int i = (int)(sidx / nd);
+        const int r = examine_leaf<DIM>(g, keys, first, a.mark, cm, per, keys[i], s_dirs[sidx - (int64_t)i * nd]);
+        if (r == 2) atomicOr((unsigned*)(a.mark + (i & ~3)), 2u << (8 * (i & 3)));
       }
     } else {
-      const int nd = a.ndirs;
-      if (nfront < 0) {
-        for (int64_t sidx = gtid; sidx < n * nd; sidx += gsize)
-          balance_examine<DIM>(g, keys, first, a.mark, (int)(sidx / nd), s_dirs[sidx % nd]);
-      } else {
-        const int* fr = a.frontier[fpar];
-        for (int64_t sidx = gtid; sidx < nfront * nd; sidx += gsize)
-          balance_examine<DIM>(g, keys, first, a.mark, fr[sidx / nd], s_dirs[sidx % nd]);
+      const uint64_t* fk = a.fkey[fpar];
+      uint8_t* ft = a.ftag[fpar];
+      const int nd = a.ngdirs;  // >= ndirs and >= 2 * DIM
+      for (int64_t sidx = gtid; sidx < nfront * nd; sidx += gsize) {
+        const int64_t e = sidx / nd;
+        const int d = (int)(sidx - e * nd);
+        const int tag = ft[e] & 0x7f;
+        const uint64_t key = fk[e];
+        int r = 0;
+        if (tag == kFrGroup) r = examine_group<DIM>(g, keys, first, a.mark, cm, per, key, s_gdirs[d]);
+        else if (tag == kFrLeaf) r = d < a.ndirs ? examine_leaf<DIM>(g, keys, first, a.mark, cm, per, key, s_dirs[d]) : 0;
+        else if (d < 2 * DIM) examine_self<DIM>(g, keys, first, a.mark, cm, per, (int)key, d);  // only in sweep 1
+        if (r == 2) atomicOr((unsigned*)(ft + (e & ~3)), (unsigned)kFrAgain << (8 * (e & 3)));
       }
     }
     grid.sync();
-    // ---- count: low 32 = leaves out, high 32 = frontier entries out
+    lap(0);
+    // ---- leaves out per chunk = its length + (NC - 1) * its marks
     int64_t lo, hi;
-    block_chunk(n, gridDim.x, blockIdx.x, BT, &lo, &hi);
-    unsigned long long acc = 0;
-    for (int64_t i = lo + threadIdx.x; i < hi; i += BT) {
-      const unsigned mk = a.mark[i];
-      unsigned long long c = (mk & 1) ? NC : 1;
-      unsigned long long fc = (mk & 1) ? NC : ((mk & 2) ? 1 : 0);
-      acc += c | (fc << 32);
+    block_chunk(n, G, blockIdx.x, BT, &lo, &hi);
+    unsigned long long mine = 0, all = 0;
+    for (int i = threadIdx.x; i < G; i += BT) {
+      int64_t l2, h2;
+      block_chunk(n, G, i, BT, &l2, &h2);
+      const unsigned long long c = (unsigned long long)(h2 - l2) + (unsigned long long)(NC - 1) * (unsigned)cm[i];
+      all += c;
+      if (i < (int)blockIdx.x) mine += c;
     }
-    acc = block_sum(acc, sm);
-    if (threadIdx.x == 0) a.sums[blockIdx.x] = acc;
-    grid.sync();
-    unsigned long long before, total;
-    chunk_offsets(a.sums, gridDim.x, blockIdx.x, sm, &before, &total);
-    const int64_t n_new = (int64_t)(total & 0xffffffffull);
+    const int64_t before = (int64_t)block_sum(mine, sm);
+    const int64_t n_new = (int64_t)block_sum(all, sm);
+    lap(1);
     if (n_new == n) break;  // no leaf was marked: balanced
     if (n_new > a.cap) {
       err = LT_ERR_CAPACITY;
       break;
     }
-    // ---- split marked leaves (order-preserving), rebuild index, emit next frontier
+    // ---- split marked leaves (order-preserving), rebuild the index, emit the next frontier
     uint64_t* out = a.keys[par ^ 1];
     int* first_out = a.first[par ^ 1];
-    int* fr_out = a.frontier[fpar ^ 1];
-    int64_t run = (int64_t)(before & 0xffffffffull), frun = (int64_t)(before >> 32);
+    uint64_t* fk_out = a.fkey[fpar ^ 1];
+    uint8_t* ft_out = a.ftag[fpar ^ 1];
+    int* fcount = &a.s->nfront[fpar ^ 1];
+    const bool emit = !a.full_sweeps;
+    bool fits = true;
+    int64_t run = before;
     for (int64_t t0 = lo; t0 < hi; t0 += BT) {
       const int64_t i = t0 + threadIdx.x;
       unsigned mk = 0;
@@ -467,14 +580,18 @@ __global__ void __launch_bounds__(BT) k_balance(BalanceArgs a) {
         key = keys[i];
         mk = a.mark[i];
         if (mk) a.mark[i] = 0;
-        c = ((mk & 1) ? NC : 1) | ((unsigned long long)((mk & 1) ? NC : ((mk & 2) ? 1 : 0)) << 32);
+        c = (mk & 1) ? NC : 1;
       }
       unsigned long long tile_total;
-      unsigned long long ex = block_excl_scan<unsigned long long>(c, sm, &tile_total);
-      const int64_t pos = run + (int64_t)(ex & 0xffffffffull);
-      const int64_t fpos = frun + (int64_t)(ex >> 32);
-      run += (int64_t)(tile_total & 0xffffffffull);
-      frun += (int64_t)(tile_total >> 32);
+      const unsigned long long ex = block_excl_scan<unsigned long long>(c, sm, &tile_total);
+      const int64_t pos = run + (int64_t)ex;
+      run += (int64_t)tile_total;
+      if (emit) {
+        // a split leaf becomes a GROUP entry; an unsplit leaf that saw a neighbour >= 3 levels coarser
+        // (full sweep) a LEAF entry
+        const bool pg = (mk & 1) != 0, pl = !pg && (mk & 2) != 0;
+        fits = frontier_push(pg || pl, key, pg ? kFrGroup : kFrLeaf, fk_out, ft_out, fcount, a.fcap) && fits;
+      }
       if (i >= hi) continue;
       const int l = key_level(key);
       const uint64_t m = key_morton(key);
@@ -485,24 +602,53 @@ __global__ void __launch_bounds__(BT) k_balance(BalanceArgs a) {
           const uint64_t mc = m | ((uint64_t)k << sh);
           out[pos + k] = make_key(mc, l + 1);
           index_write<DIM>(g, first_out, mc, l + 1, (int)(pos + k));
-          fr_out[fpos + k] = (int)(pos + k);
         }
       } else {
         out[pos] = key;
         index_write<DIM>(g, first_out, m, l, (int)pos);
-        if (mk & 2) fr_out[fpos] = (int)pos;
       }
     }
+    // entries flagged for another examination move on to the next frontier
+    if (emit && nfront >= 0) {
+      const uint64_t* fk = a.fkey[fpar];
+      const uint8_t* ft = a.ftag[fpar];
+      for (int64_t e0 = gtid - lane; e0 < nfront; e0 += gsize) {
+        const int64_t e = e0 + lane;
+        const int tag = e < nfront ? ft[e] : 0;
+        fits = frontier_push((tag & kFrAgain) != 0, e < nfront ? fk[e] : 0, tag & 0x7f, fk_out, ft_out, fcount,
+                             a.fcap) && fits;
+      }
+    }
+    if (!fits) a.s->fr_overflow = 1;
     if (blockIdx.x == 0 && threadIdx.x == 0) first_out[g.nbuckets] = (int)n_new;
     splits += (n_new - n) / (NC - 1);
     n = n_new;
-    nfront = a.full_sweeps ? -1 : (int64_t)(total >> 32);
     par ^= 1;
     fpar ^= 1;
     ++iters;
     grid.sync();
+    lap(2);
+    // (a frontier that overflowed its buffer -- not reachable with fcap > cap * 8 / 7 -- falls back to a
+    // full sweep, which needs no list)
+    nfront = (a.full_sweeps || a.s->fr_overflow) ? -1 : (int64_t)a.s->nfront[fpar];
+  }
+  // ---- Alg. 7: T_old -> the balanced tree, in new-leaf order.  A new leaf more
+  // than one level from T_old only raises map_bad here: lt_transfer then runs the checked k_map,
+  // which reports LT_ERR_MAPPING where the header says it is reported.
+  if (a.do_map && !err) {
+    const uint64_t* keys = a.keys[par];
+    bool bad = false;
+    for (int64_t j = gtid; j < n; j += gsize) {
+      int o, kd;
+      bad = !map_entry<DIM>(g, keys[j], a.keys_old, a.first_old, a.n_old, &o, &kd) || bad;
+      a.map_src[j] = o;
+      a.map_kind[j] = (uint8_t)kd;
+    }
+    if (bad) a.s->map_bad = 1;
   }
   if (blockIdx.x == 0 && threadIdx.x == 0) {
+    lap(3);  // (this block's share of the tail: the blocks run it side by side)
+    for (int k = 0; k < 4; ++k) a.s->bal_ns[k] = ns[k];
     a.s->n = (int)n;
     a.s->iters = iters;
     a.s->parity = par;
@@ -558,7 +704,9 @@ int launch_adapt_count(Tree* t, const int8_t* d_flags, int G) {
 }
 
 int launch_adapt_scatter(Tree* t, const int8_t* d_flags, int G, int path_a, int emit_front) {
-  int* front = (emit_front && !path_a) ? t->frontier[0] : nullptr;
+  uint64_t* fkey = (emit_front && !path_a) ? t->fkey[0] : nullptr;
+  uint8_t* ftag = t->ftag[0];
+  const int64_t fcap = t->fcap;
   if (path_a) {
     LT_DISPATCH_DIM(t,
                     (k_adapt_append<2><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], d_flags, t->d_s, t->d_sums,
@@ -568,9 +716,9 @@ int launch_adapt_scatter(Tree* t, const int8_t* d_flags, int G, int path_a, int 
   } else {
     LT_DISPATCH_DIM(t,
                     (k_adapt_scatter<2><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], d_flags, t->d_s, t->d_sums,
-                                                                 t->keys[t->tmp], t->first[t->tmp], t->cap, front)),
+                                                                 t->keys[t->tmp], t->first[t->tmp], t->cap, fkey, ftag, fcap)),
                     (k_adapt_scatter<3><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], d_flags, t->d_s, t->d_sums,
-                                                                 t->keys[t->tmp], t->first[t->tmp], t->cap, front)));
+                                                                 t->keys[t->tmp], t->first[t->tmp], t->cap, fkey, ftag, fcap)));
   }
   t->launches++;
   LT_CUDA(cudaGetLastError());
@@ -585,17 +733,22 @@ int launch_balance(Tree* t, int64_t cap_told, int use_front) {
   a.first[0] = t->first[t->cur];
   a.first[1] = t->first[t->tmp];
   a.mark = t->mark;
-  a.frontier[0] = t->frontier[0];
-  a.frontier[1] = t->frontier[1];
-  a.sums = t->d_sums;
+  for (int b = 0; b < 2; ++b) {
+    a.fkey[b] = t->fkey[b];
+    a.ftag[b] = t->ftag[b];
+    a.cmarks[b] = t->d_cmarks + b * kMaxGrid;
+  }
+  a.fcap = t->fcap;
   a.s = t->d_s;
   a.cap = cap_told;
   a.full_sweeps = t->opt_full_sweeps;
   a.front0 = use_front;
-  // directions: per axis none / exterior / interior, at least one exterior move, at most
-  // `conn` moves (conn 1: the dim exterior faces, in axis order)
+  // LEAF directions: per axis none / exterior / interior, at least one exterior move, at most
+  // `conn` moves (conn 1: the dim exterior faces, in axis order); GROUP directions: every offset in
+  // {-1, 0, +1}^dim with 1..conn non-zero entries (conn 1: the 2 * dim faces)
   const int conn = t->opt_balance_conn > 0 ? t->opt_balance_conn : 1;
   a.ndirs = 0;
+  a.ngdirs = 0;
   for (int moves = 1; moves <= conn; ++moves)
     for (int code = 1; code < (1 << (2 * t->g.dim)); ++code) {
       int nz = 0, ext = 0, bad = 0;
@@ -605,14 +758,25 @@ int launch_balance(Tree* t, int64_t cap_told, int use_front) {
         nz += c != 0;
         ext += c == 1;
       }
-      if (!bad && nz == moves && ext >= 1) a.dirs[a.ndirs++] = (uint8_t)code;
+      if (bad || nz != moves) continue;
+      if (ext >= 1) a.dirs[a.ndirs++] = (uint8_t)code;
+      a.gdirs[a.ngdirs++] = (uint8_t)code;
     }
+  a.do_map = t->have_old ? 1 : 0;
+  a.n_old = (int)t->n_old;
+  a.keys_old = t->keys[t->old];
+  a.first_old = t->first[t->old];
+  a.map_src = t->map_src;
+  a.map_kind = t->map_kind;
   void* fn = t->g.dim == 2 ? (void*)k_balance<2> : (void*)k_balance<3>;
   int per_sm = 0;
   LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, BT, 0));
   if (per_sm < 1) return LT_ERR_CUDA;
   int G = t->num_sms * per_sm;
   if (G > kMaxGrid) G = kMaxGrid;
+  // marks-per-chunk counters of both sweep parities; map_bad (the words sit next to each other)
+  LT_CUDA(cudaMemsetAsync(t->d_cmarks, 0, 2 * kMaxGrid * sizeof(int), t->stream));
+  LT_CUDA(cudaMemsetAsync(&t->d_s->map_bad, 0, sizeof(int), t->stream));
   void* args[] = {&a};
   LT_CUDA(cudaLaunchCooperativeKernel(fn, dim3(G), dim3(BT), args, 0, t->stream));
   t->launches++;

@@ -76,6 +76,8 @@ SIGNATURES = {
     "lt_set_option": (_I, [_P, _I, _I]),
     "lt_timings": (_I, [_P, _P]),
     "lt_launch_count": (_I64, [_P]),
+    "lt_host_syncs": (_I64, [_P]),
+    "lt_balance_phases": (_I, [_P, _P]),
     "lt_strerror": (C.c_char_p, [_I]),
     "lt_last_cuda_error": (_I, []),
     "lt_version": (_I, []),
@@ -368,6 +370,14 @@ class Tree:
 
     def launch_count(self) -> int:
         return int(lib().lt_launch_count(self._h))
+
+    def balance_phases(self):
+        out = (C.c_float * 4)()
+        _check(lib().lt_balance_phases(self._h, out), "lt_balance_phases")
+        return dict(examine=out[0], offsets=out[1], split=out[2], map=out[3])
+
+    def host_syncs(self) -> int:
+        return int(lib().lt_host_syncs(self._h))
 
 
 def build(dim, base_level, max_level, domain=None, periodic=None) -> Tree:

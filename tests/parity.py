@@ -63,8 +63,12 @@ def initial_u(cfg, ot):
     return W.initial_solution(cfg, torch.from_numpy(lvl), torch.from_numpy(xyz.astype(np.int64))).numpy()
 
 
-def run_cycles(cfg, ncycles, options=(), check_faces=True, check_transfer=True, drift_free=True, log=None):
-    """Drive both sides through `ncycles` adaptation cycles of a workload config."""
+def run_cycles(cfg, ncycles, options=(), check_faces=True, check_transfer=True, drift_free=True, log=None,
+               record=None):
+    """Drive both sides through `ncycles` adaptation cycles of a workload config.
+    log (list): one row per cycle (cycle, leaves out, balance sweeps, n_conf, n_hang, n_bnd, leaves in) -- the
+    ORACLE's numbers (the GPU's were asserted equal).  record (list): per cycle (flags, oracle keys after
+    balance, sweeps), for GPU-only replays with other options."""
     gt, ot = new_pair(cfg)
     for opt, val in options:
         gt.set_option(opt, val)
@@ -79,6 +83,7 @@ def run_cycles(cfg, ncycles, options=(), check_faces=True, check_transfer=True, 
         olvl, oxyz = ot.leaf_boxes()
         assert np.array_equal(glvl.cpu().numpy(), olvl) and np.array_equal(gxyz.cpu().numpy().astype(np.uint32), oxyz)
         f = host_flags(cfg, c, ot)
+        n_in = ot.num_leaves()
         ot.adapt(f)
         gt.adapt(torch.from_numpy(f).cuda())
         assert_keys_equal(gt, ot, tag + " adapt")
@@ -87,8 +92,13 @@ def run_cycles(cfg, ncycles, options=(), check_faces=True, check_transfer=True, 
         it_g = gt.balance()
         assert_keys_equal(gt, ot, tag + " balance")
         assert it_g == it_o, "%s: balance iters %d vs oracle %d" % (tag, it_g, it_o)
+        counts = (-1, -1, -1)
         if check_faces:
-            assert_faces_equal(gt.connect(), ot.connect(), tag + " connect")
+            Fo = ot.connect()
+            assert_faces_equal(gt.connect(), Fo, tag + " connect")
+            counts = (Fo["n_conf"], Fo["n_hang"], Fo["n_bnd"])
+        if record is not None:
+            record.append((f, ot.keys(), it_o))
         if check_transfer:
             src_o, kind_o = ot.build_map()
             un_o = ot.transfer_rows(uo, p, nvars, 0, ot.num_leaves())
@@ -105,5 +115,21 @@ def run_cycles(cfg, ncycles, options=(), check_faces=True, check_transfer=True, 
         else:
             ot.drop_snapshot()
         if log is not None:
-            log.append((c, ot.num_leaves(), it_o))
+            log.append((c, ot.num_leaves(), it_o) + counts + (n_in,))
     return gt, ot, ug, uo
+
+
+def replay_gpu(cfg, record, options=()):
+    """GPU only: drive a fresh tree through the recorded flags with `options` set and compare keys and
+    sweep counts with the recorded (oracle) ones -- options must not change results."""
+    dom = [cfg["lo"]] * cfg["dim"] + [cfg["hi"]] * cfg["dim"]
+    gt = lt.Tree(cfg["dim"], cfg["base"], cfg["maxl"], dom, cfg["periodic"])
+    for opt, val in options:
+        gt.set_option(opt, val)
+    for c, (f, keys, iters) in enumerate(record):
+        gt.adapt(torch.from_numpy(f).cuda())
+        it = gt.balance()
+        assert it == iters, "replay cycle %d: balance sweeps %d vs %d" % (c, it, iters)
+        gk = u64(gt.keys())
+        assert gk.shape == keys.shape and np.array_equal(gk, keys), "replay cycle %d: keys differ" % c
+    return gt

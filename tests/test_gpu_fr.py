@@ -95,28 +95,75 @@ def test_free_stream_and_rk3_on_gpu(dim):
     u = torch.from_numpy(np.tile(state[None, :, None], (M, 1, N))).cuda()
     _, R = gpu_pipeline(gt, u, p)
     assert float(R.abs().max()) < 1e-9
-    # Eq. 6 against the formula, with arbitrary arrays
-    un, us, r = (torch.from_numpy(rng.uniform(-1, 1, (M, dim + 2, N))).cuda() for _ in range(3))
+    # Eq. 6 against the oracle's rk3_stage, arbitrary arrays.  The oracle writes stage 1 as
+    # u^n + dt R (its stage vector IS u^n), so stage 1 is called with u_stage = u_n on both sides.
+    un_h, us_h, r_h = (rng.uniform(-1, 1, (M, dim + 2, N)) for _ in range(3))
+    un, us, r = (torch.from_numpy(a).cuda() for a in (un_h, us_h, r_h))
     dt = 0.37
-    for stage, (ca, cb) in enumerate([(0.0, 1.0), (0.75, 0.25), (1.0 / 3.0, 2.0 / 3.0)], start=1):
-        want = ca * un + cb * (us + dt * r)
-        got = gt.rk3_stage(stage, dt, un, us, r, p)
-        assert float((got - want).abs().max()) < 1e-15
-    # lt_fr_stage = lt_fr_rhs + lt_rk3_stage in one pass, also in place over u_stage / u_n
-    fs, R = gpu_pipeline(gt, un.abs() + 1.0 if False else u, p)
-    base_n = torch.from_numpy(rng.uniform(0.9, 1.1, (M, dim + 2, N))).cuda() * u
     for stage in (1, 2, 3):
-        want = gt.rk3_stage(stage, dt, base_n, u, R, p)
-        got = gt.fr_stage(stage, dt, base_n, u, fs, p)
-        assert float((got - want).abs().max()) <= 1e-12 * max(1.0, float(want.abs().max()))
-        w1 = u.clone()
-        gt.fr_stage(stage, dt, base_n, w1, fs, p, out=w1)
-        w2 = base_n.clone()
-        gt.fr_stage(stage, dt, w2, u, fs, p, out=w2)
-        assert torch.equal(w1, got) and torch.equal(w2, got)
+        st_h, st = (un_h, un) if stage == 1 else (us_h, us)
+        want = oracle.rk3_stage(stage, dt, un_h, st_h, r_h)
+        got = gt.rk3_stage(stage, dt, un, st, r, p)
+        assert float(np.abs(got.cpu().numpy() - want).max()) < 1e-15
     inplace = us.clone()
     gt.rk3_stage(2, dt, un, inplace, r, p, out=inplace)
-    assert float((inplace - (0.75 * un + 0.25 * (us + dt * r))).abs().max()) < 1e-15
+    assert float(np.abs(inplace.cpu().numpy() - oracle.rk3_stage(2, dt, un_h, us_h, r_h)).max()) < 1e-15
+
+
+@pytest.mark.parametrize("dim,p", [(2, 3), (3, 2), (3, 3)])
+def test_fr_stage_all_stages_match_oracle_chain(dim, p):
+    """lt_fr_stage (right-hand side + Eq. 6 in one pass) and the unfused lt_fr_rhs + lt_rk3_stage against
+    the ORACLE's chain (Alg. 8 steps 1-4, Eq. 2-5, then oracle.rk3_stage) for all three stages of one
+    SSP-RK3 step on an adapted periodic mesh with hanging faces; every stage is fed the oracle's stage
+    vector, so no GPU result enters an expected value.  Also in place over u_stage / u_n."""
+    gt, ot, rng = adapted_pair(dim, (1,) * dim, 17 + dim, 2, 5 if dim == 2 else 4, cycles=2)
+    F = gt.connect(); ot.connect()
+    assert int(F["n_hang"]) > 0
+    M, N = ot.num_leaves(), (p + 1) ** dim
+    lvl, xyz = ot.leaf_boxes()
+    z, _ = np.polynomial.legendre.leggauss(p + 1)
+    Lw = float(1 << ot.maxl)
+    wd = (1 << (ot.maxl - lvl.astype(np.int64))) / Lw
+    X = np.zeros((M, N, dim))
+    for n in range(N):
+        r_ = n
+        for a2 in range(dim):
+            X[:, n, a2] = xyz[:, a2] / Lw + 0.5 * wd * (1 + z[r_ % (p + 1)])
+            r_ //= p + 1
+    ph = 2 * np.pi * X
+    rho = 1.0 + 0.2 * np.prod(np.sin(ph), axis=-1)
+    vel = np.stack([0.4 + 0.1 * np.cos(ph[..., (a2 + 1) % dim]) for a2 in range(dim)], axis=-1)
+    pr = 1.0 + 0.1 * np.cos(ph[..., 0])
+    u_n = np.concatenate([rho[:, None], np.moveaxis(rho[..., None] * vel, -1, 1),
+                          (pr / 0.4 + 0.5 * rho * np.sum(vel * vel, -1))[:, None]], axis=1).copy()
+    dt = 2e-3
+    d_un = torch.from_numpy(u_n).cuda()
+    u_stage = u_n
+    for stage in (1, 2, 3):
+        fs_o, R_o = oracle_pipeline(ot, u_stage, p)
+        want = oracle.rk3_stage(stage, dt, u_n, u_stage, R_o)
+        d_us = torch.from_numpy(u_stage).cuda()
+        fs_g, R_g = gpu_pipeline(gt, d_us, p)
+        close(fs_g, fs_o, "stage %d: common fluxes" % stage)
+        close_rhs(R_g, R_o, fs_o, ot, "stage %d: rhs" % stage)
+        # dt * (the I-6 bound of R) + E-8's bound on the state
+        lvl_max = int(lvl.max())
+        tol = 1e-12 * max(1.0, float(np.abs(want).max()), dt * float(2 << lvl_max) * float(np.abs(fs_o).max()))
+        unfused = gt.rk3_stage(stage, dt, d_un, d_us, R_g, p)
+        fused = gt.fr_stage(stage, dt, d_un, d_us, fs_g, p)
+        for name, got in (("rk3_stage(fr_rhs)", unfused), ("fr_stage", fused)):
+            err = float(np.abs(got.cpu().numpy() - want).max())
+            assert err <= tol, "stage %d %s: |diff| %.3e > %.3e" % (stage, name, err, tol)
+        w1 = d_us.clone()
+        gt.fr_stage(stage, dt, d_un, w1, fs_g, p, out=w1)          # in place over the stage vector
+        assert torch.equal(w1, fused)
+        if stage > 1:
+            w2 = d_un.clone()
+            gt.fr_stage(stage, dt, w2, d_us, fs_g, p, out=w2)      # in place over u^n
+            assert torch.equal(w2, fused)
+        u_stage = want                                             # the oracle's stage vector feeds the next stage
+    gt.sync()
+    assert float(np.abs(u_stage - u_n).max()) > 1e-6               # the step did something
 
 
 def test_full_step_conserves_mass_momentum_energy():

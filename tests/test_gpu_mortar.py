@@ -137,3 +137,33 @@ def test_face_interp_then_mortars(dim, periodic, base, maxl, p, nvars):
     gt.sync()
     with pytest.raises((lt.LtError, ValueError)):
         gt.face_interp(uf_g, p, nvars)  # wrong shape
+
+
+def test_gather_survives_transfer_host_between_two_meshes():
+    """Regression (round-1 advisor finding): lt_transfer_host used to free the hit list that
+    lt_mortar_gather keeps on the tree, leaving a dangling pointer for the next gather.  Sequence:
+    connect + gather, adapt / balance / transfer_host (its first call on this tree allocates the slab
+    bounds), connect + gather on the new tree -- every step against the oracle; then once more with a
+    refine-everything cycle so that the hit list has to grow."""
+    dim, p, nvars = 3, 2, 3
+    gt, ot, rng = adapted_pair(dim, (1, 1, 1), 77, 2, 5, cycles=2)
+    N, Nf = (p + 1) ** dim, (p + 1) ** (dim - 1)
+    for step in range(3):
+        Fo = ot.connect()
+        P.assert_faces_equal(gt.connect(), Fo, "faces, step %d" % step)
+        assert ((Fo["kind"] & 15) == 3).any()
+        fm = rng.uniform(-1, 1, (ot.num_leaves(), 2 * dim, nvars, Nf))
+        close(gt.mortar_gather(torch.from_numpy(fm).cuda(), p, nvars), ot.mortar_gather(fm, p, nvars),
+              "gather, step %d" % step)
+        gt.sync()
+        if step == 2:
+            break
+        uo = rng.uniform(-1, 1, (ot.num_leaves(), nvars, N))
+        f = (rng.random(ot.num_leaves()) < (0.3 if step == 0 else 1.0)).astype(np.int8)
+        ot.adapt(f); ot.balance()
+        gt.adapt(torch.from_numpy(f).cuda()); gt.balance()
+        P.assert_keys_equal(gt, ot, "tree, step %d" % step)
+        want = ot.transfer(uo, p, nvars)
+        h_new = torch.empty((gt.num_leaves(), nvars, N), dtype=torch.float64).pin_memory()
+        gt.transfer_host(torch.from_numpy(uo).pin_memory(), h_new, p, nvars)
+        P.assert_u_close(h_new, want, "host transfer, step %d" % step)
