@@ -15,6 +15,9 @@
 // follows; readings of silent/garbled passages are the ones listed in
 // DESIGN.md (section "Readings").
 //
+// The domain may be a brick of root cubes (a forest of pointer trees, reading J-1 of DESIGN.md;
+// PAPER.md:410 runs on a slab of 16 x 16 x 1 cubes): one cube reproduces the single-tree oracle bit for bit.
+//
 // Pins (tests/test_oracle_*.py, -m "not gpu"): see DESIGN.md section "Oracle
 // pins".  No function here is "parity unpinned".
 //

@@ -9,8 +9,11 @@ few thousand cells.
 from itertools import product
 
 
-def uniform(dim, level):
-    return {(level,) + c for c in product(range(1 << level), repeat=dim)}
+def uniform(dim, level, nroot=None):
+    """nroot: the domain is a brick of nroot[a] root cubes along axis a (cells of level l then have
+    coordinates in [0, nroot[a] << l)); None = one cube."""
+    nr = nroot or (1,) * dim
+    return {(level,) + c for c in product(*[range(nr[a] << level) for a in range(dim)])}
 
 
 def children(cell):
@@ -34,10 +37,10 @@ def containing_leaf(mesh, cell):
     return None
 
 
-def face_neighbour(cell, axis, sign, periodic):
+def face_neighbour(cell, axis, sign, periodic, nroot=None):
     l, c = cell[0], list(cell[1:])
     c[axis] += sign
-    n = 1 << l
+    n = (nroot[axis] if nroot else 1) << l
     if c[axis] < 0 or c[axis] >= n:
         if not periodic[axis]:
             return None
@@ -68,11 +71,11 @@ def adapt(mesh, flag_of, base, maxl):
     return out
 
 
-def offset_neighbour(cell, offs, periodic):
+def offset_neighbour(cell, offs, periodic, nroot=None):
     """Same-level cell at integer offset `offs` (one entry per axis), periodic wrap per axis."""
     l, c = cell[0], list(cell[1:])
-    n = 1 << l
     for a, o in enumerate(offs):
+        n = (nroot[a] if nroot else 1) << l
         c[a] += o
         if c[a] < 0 or c[a] >= n:
             if not periodic[a]:
@@ -86,7 +89,7 @@ def directions(dim, conn):
     return [o for o in product((-1, 0, 1), repeat=dim) if 1 <= sum(1 for v in o if v) <= conn]
 
 
-def balance(mesh, periodic, conn=1):
+def balance(mesh, periodic, conn=1, nroot=None):
     """Jacobi ripple; returns (mesh, iters, splits).  conn: see directions()."""
     mesh = set(mesh)
     dim = len(next(iter(mesh))) - 1
@@ -96,7 +99,7 @@ def balance(mesh, periodic, conn=1):
         marked = set()
         for cell in mesh:
             for o in dirs:
-                    nb = offset_neighbour(cell, o, periodic)
+                    nb = offset_neighbour(cell, o, periodic, nroot)
                     if nb is None:
                         continue
                     leaf = containing_leaf(mesh, nb)
@@ -111,12 +114,12 @@ def balance(mesh, periodic, conn=1):
         splits += len(marked)
 
 
-def is_balanced(mesh, periodic):
+def is_balanced(mesh, periodic, nroot=None):
     dim = len(next(iter(mesh))) - 1
     for cell in mesh:
         for axis in range(dim):
             for sign in (-1, 1):
-                nb = face_neighbour(cell, axis, sign, periodic)
+                nb = face_neighbour(cell, axis, sign, periodic, nroot)
                 if nb is None:
                     continue
                 leaf = containing_leaf(mesh, nb)
@@ -157,14 +160,14 @@ def is_balanced_boxes(mesh, periodic, conn, maxl):
     return True
 
 
-def face_census(mesh, periodic):
+def face_census(mesh, periodic, nroot=None):
     """(n_conf, n_hang, n_bnd) counted from every cell's own faces."""
     dim = len(next(iter(mesh))) - 1
     conf2 = hang = bnd = 0
     for cell in mesh:
         for axis in range(dim):
             for sign in (-1, 1):
-                nb = face_neighbour(cell, axis, sign, periodic)
+                nb = face_neighbour(cell, axis, sign, periodic, nroot)
                 if nb is None:
                     bnd += 1
                     continue
