@@ -12,6 +12,7 @@ namespace lt {
 // Device-resident scalars of a tree (one allocation).
 struct DevScalars {
   int n;                 // current leaf count
+  int n_in;              // lt_adapt: the count of the tree being adapted (snapshot taken by pass 1)
   int status;            // sticky lt_status detected on the device (0 = ok)
   int iters;             // balance: sweeps that split >= 1 leaf
   int parity;            // balance: 0 = result in the buffer it started in, 1 = in the other

@@ -12,6 +12,7 @@ namespace cg = cooperative_groups;
 namespace lt {
 
 constexpr int BT = 256;  // threads per block of the tree kernels
+constexpr int kScanTiles = 4;  // tiles of BT leaves ordered by ONE block scan (16-bit packed counts)
 
 enum { ACT_KEEP = 0, ACT_REFINE = 1, ACT_PARENT = 2, ACT_DROP = 3 };
 
@@ -149,12 +150,14 @@ __device__ __forceinline__ int adapt_action(const Geo& g, const uint64_t* __rest
 // pass 1: per-chunk output counts.  sums[b] = (kept << 32) | count_B   (see lt_adapt)
 template <int DIM>
 __global__ void __launch_bounds__(BT) k_adapt_count(Geo g, const uint64_t* __restrict__ keys,
-                                                    const int8_t* __restrict__ flags,
-                                                    const DevScalars* __restrict__ s,
+                                                    const int8_t* __restrict__ flags, DevScalars* s,
                                                     unsigned long long* __restrict__ sums) {
   constexpr int NC = Dim<DIM>::NC;
   __shared__ unsigned long long sm[33];
   const int64_t n = s->n;
+  // pass 2 overwrites s->n with the new count while its later blocks are still starting: they read the
+  // count of the tree they work on from this snapshot
+  if (blockIdx.x == 0 && threadIdx.x == 0) s->n_in = (int)n;
   int64_t lo, hi;
   block_chunk(n, gridDim.x, blockIdx.x, BT, &lo, &hi);
   unsigned long long acc = 0;
@@ -184,7 +187,7 @@ __global__ void __launch_bounds__(BT) k_adapt_scatter(Geo g, const uint64_t* __r
   // parent as a SELF entry (its position)
   constexpr int NC = Dim<DIM>::NC;
   __shared__ unsigned long long sm[33];
-  const int64_t n = s->n;
+  const int64_t n = s->n_in;  // (not s->n: block 0 of this kernel overwrites it, see k_adapt_count)
   unsigned long long before, total;
   chunk_offsets(sums, gridDim.x, blockIdx.x, sm, &before, &total);
   const int64_t n_out = (int64_t)(total & 0xffffffffull);
@@ -195,50 +198,62 @@ __global__ void __launch_bounds__(BT) k_adapt_scatter(Geo g, const uint64_t* __r
   int64_t lo, hi;
   block_chunk(n, gridDim.x, blockIdx.x, BT, &lo, &hi);
   int64_t run = (int64_t)(before & 0xffffffffull);
-  for (int64_t t0 = lo; t0 < hi; t0 += BT) {
-    const int64_t i = t0 + threadIdx.x;
-    int act = ACT_DROP;
-    uint64_t key = 0;
-    if (i < hi) {
-      key = keys[i];
-      act = adapt_action<DIM>(g, keys, flags, i, n, key);
+  // kScanTiles tiles of BT leaves share one block scan (counts packed in 16-bit fields)
+  for (int64_t t0 = lo; t0 < hi; t0 += kScanTiles * BT) {
+    uint64_t keyq[kScanTiles];
+    int actq[kScanTiles];
+    unsigned long long packed = 0;
+#pragma unroll
+    for (int q = 0; q < kScanTiles; ++q) {
+      const int64_t i = t0 + q * BT + threadIdx.x;
+      actq[q] = ACT_DROP;
+      keyq[q] = 0;
+      if (i < hi) {
+        keyq[q] = keys[i];
+        actq[q] = adapt_action<DIM>(g, keys, flags, i, n, keyq[q]);
+      }
+      packed |= (unsigned long long)(actq[q] == ACT_REFINE ? NC : (actq[q] == ACT_DROP ? 0 : 1)) << (16 * q);
     }
-    int c = act == ACT_REFINE ? NC : (act == ACT_DROP ? 0 : 1);
     unsigned long long tile_total;
-    unsigned long long ex = block_excl_scan<unsigned long long>((unsigned long long)c, sm, &tile_total);
-    int64_t pos = run + (int64_t)ex;
-    run += (int64_t)tile_total;
-    if (fkey != nullptr) {  // warp-aggregated append (kFrGroup = 2, kFrSelf = 3 of k_balance)
-      const bool pg = act == ACT_REFINE, ps = act == ACT_PARENT;
-      const unsigned mm = __ballot_sync(0xffffffffu, pg || ps);
-      if (mm) {
-        const int ln = threadIdx.x & 31;
-        int base = 0;
-        if (ln == __ffs(mm) - 1) base = atomicAdd(&s->nfront[0], __popc(mm));
-        base = __shfl_sync(0xffffffffu, base, __ffs(mm) - 1);
-        const int64_t at = (int64_t)base + __popc(mm & ((1u << ln) - 1));
-        if ((pg || ps) && at < fcap) {  // (a list that does not fit makes lt_balance sweep in full)
-          fkey[at] = pg ? key : (uint64_t)pos;
-          ftag[at] = pg ? 2 : 3;
+    const unsigned long long ex = block_excl_scan<unsigned long long>(packed, sm, &tile_total);
+#pragma unroll
+    for (int q = 0; q < kScanTiles; ++q) {
+      const int act = actq[q];
+      const uint64_t key = keyq[q];
+      const int64_t pos = run + (int64_t)((ex >> (16 * q)) & 0xffff);
+      run += (int64_t)((tile_total >> (16 * q)) & 0xffff);
+      if (fkey != nullptr) {  // warp-aggregated append (kFrGroup = 2, kFrSelf = 3 of k_balance)
+        const bool pg = act == ACT_REFINE, ps = act == ACT_PARENT;
+        const unsigned mm = __ballot_sync(0xffffffffu, pg || ps);
+        if (mm) {
+          const int ln = threadIdx.x & 31;
+          int base = 0;
+          if (ln == __ffs(mm) - 1) base = atomicAdd(&s->nfront[0], __popc(mm));
+          base = __shfl_sync(0xffffffffu, base, __ffs(mm) - 1);
+          const int64_t at = (int64_t)base + __popc(mm & ((1u << ln) - 1));
+          if ((pg || ps) && at < fcap) {  // (a list that does not fit makes lt_balance sweep in full)
+            fkey[at] = pg ? key : (uint64_t)pos;
+            ftag[at] = pg ? 2 : 3;
+          }
         }
       }
-    }
-    if (c == 0) continue;
-    const int l = key_level(key);
-    const uint64_t m = key_morton(key);
-    if (act == ACT_KEEP) {
-      out[pos] = key;
-      index_write<DIM>(g, first_out, m, l, (int)pos);
-    } else if (act == ACT_PARENT) {
-      out[pos] = make_key(m, l - 1);  // child 0 has the parent's anchor
-      index_write<DIM>(g, first_out, m, l - 1, (int)pos);
-    } else {
-      const int sh = DIM * (g.maxl - l - 1);
+      if (act == ACT_DROP) continue;
+      const int l = key_level(key);
+      const uint64_t m = key_morton(key);
+      if (act == ACT_KEEP) {
+        out[pos] = key;
+        index_write<DIM>(g, first_out, m, l, (int)pos);
+      } else if (act == ACT_PARENT) {
+        out[pos] = make_key(m, l - 1);  // child 0 has the parent's anchor
+        index_write<DIM>(g, first_out, m, l - 1, (int)pos);
+      } else {
+        const int sh = DIM * (g.maxl - l - 1);
 #pragma unroll
-      for (int k = 0; k < NC; ++k) {
-        const uint64_t mc = m | ((uint64_t)k << sh);  // reading A-6
-        out[pos + k] = make_key(mc, l + 1);
-        index_write<DIM>(g, first_out, mc, l + 1, (int)(pos + k));
+        for (int k = 0; k < NC; ++k) {
+          const uint64_t mc = m | ((uint64_t)k << sh);  // reading A-6
+          out[pos + k] = make_key(mc, l + 1);
+          index_write<DIM>(g, first_out, mc, l + 1, (int)(pos + k));
+        }
       }
     }
   }
@@ -258,7 +273,7 @@ __global__ void __launch_bounds__(BT) k_adapt_append(Geo g, const uint64_t* __re
                                                      uint64_t* __restrict__ out, int64_t cap) {
   constexpr int NC = Dim<DIM>::NC;
   __shared__ unsigned long long sm[33];
-  const int64_t n = s->n;
+  const int64_t n = s->n_in;  // (not s->n: block 0 of this kernel overwrites it, see k_adapt_count)
   unsigned long long before, total;
   chunk_offsets(sums, gridDim.x, blockIdx.x, sm, &before, &total);
   const int64_t n_kept = (int64_t)(total >> 32);
@@ -571,41 +586,60 @@ __global__ void __launch_bounds__(BT) k_balance(BalanceArgs a) {
     const bool emit = !a.full_sweeps;
     bool fits = true;
     int64_t run = before;
-    for (int64_t t0 = lo; t0 < hi; t0 += BT) {
-      const int64_t i = t0 + threadIdx.x;
-      unsigned mk = 0;
-      uint64_t key = 0;
-      unsigned long long c = 0;
-      if (i < hi) {
-        key = keys[i];
-        mk = a.mark[i];
-        if (mk) a.mark[i] = 0;
-        c = (mk & 1) ? NC : 1;
+    // kScanTiles tiles of BT leaves share one block scan: the counts (<= NC * BT < 2^16 per tile) are
+    // packed in 16-bit fields, and the loads of all tiles are issued before the first barrier (requesting
+    // the NEXT group's loads as well before the barriers was tried: slower, 0.34 -> 0.40-0.43 ms for the
+    // three splitting sweeps of config-5 cycle 3, because of the registers it takes)
+    for (int64_t t0 = lo; t0 < hi; t0 += kScanTiles * BT) {
+      uint64_t key[kScanTiles];
+      unsigned mk[kScanTiles];
+      unsigned long long packed = 0;
+#pragma unroll
+      for (int q = 0; q < kScanTiles; ++q) {
+        const int64_t i = t0 + q * BT + threadIdx.x;
+        key[q] = 0;
+        mk[q] = 0;
+        if (i < hi) {
+          key[q] = keys[i];
+          mk[q] = a.mark[i];
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < kScanTiles; ++q) {
+        const int64_t i = t0 + q * BT + threadIdx.x;
+        if (i < hi) {
+          if (mk[q]) a.mark[i] = 0;
+          packed |= (unsigned long long)((mk[q] & 1) ? NC : 1) << (16 * q);
+        }
       }
       unsigned long long tile_total;
-      const unsigned long long ex = block_excl_scan<unsigned long long>(c, sm, &tile_total);
-      const int64_t pos = run + (int64_t)ex;
-      run += (int64_t)tile_total;
-      if (emit) {
-        // a split leaf becomes a GROUP entry; an unsplit leaf that saw a neighbour >= 3 levels coarser
-        // (full sweep) a LEAF entry
-        const bool pg = (mk & 1) != 0, pl = !pg && (mk & 2) != 0;
-        fits = frontier_push(pg || pl, key, pg ? kFrGroup : kFrLeaf, fk_out, ft_out, fcount, a.fcap) && fits;
-      }
-      if (i >= hi) continue;
-      const int l = key_level(key);
-      const uint64_t m = key_morton(key);
-      if (mk & 1) {
-        const int sh = DIM * (g.maxl - l - 1);
+      const unsigned long long ex = block_excl_scan<unsigned long long>(packed, sm, &tile_total);
 #pragma unroll
-        for (int k = 0; k < NC; ++k) {
-          const uint64_t mc = m | ((uint64_t)k << sh);
-          out[pos + k] = make_key(mc, l + 1);
-          index_write<DIM>(g, first_out, mc, l + 1, (int)(pos + k));
+      for (int q = 0; q < kScanTiles; ++q) {
+        const int64_t i = t0 + q * BT + threadIdx.x;
+        const int64_t pos = run + (int64_t)((ex >> (16 * q)) & 0xffff);
+        run += (int64_t)((tile_total >> (16 * q)) & 0xffff);
+        if (emit) {
+          // a split leaf becomes a GROUP entry; an unsplit leaf that saw a neighbour >= 3 levels coarser
+          // (full sweep) a LEAF entry
+          const bool pg = (mk[q] & 1) != 0, pl = !pg && (mk[q] & 2) != 0;
+          fits = frontier_push(pg || pl, key[q], pg ? kFrGroup : kFrLeaf, fk_out, ft_out, fcount, a.fcap) && fits;
         }
-      } else {
-        out[pos] = key;
-        index_write<DIM>(g, first_out, m, l, (int)pos);
+        if (i >= hi) continue;
+        const int l = key_level(key[q]);
+        const uint64_t m = key_morton(key[q]);
+        if (mk[q] & 1) {
+          const int sh = DIM * (g.maxl - l - 1);
+#pragma unroll
+          for (int k = 0; k < NC; ++k) {
+            const uint64_t mc = m | ((uint64_t)k << sh);
+            out[pos + k] = make_key(mc, l + 1);
+            index_write<DIM>(g, first_out, mc, l + 1, (int)(pos + k));
+          }
+        } else {
+          out[pos] = key[q];
+          index_write<DIM>(g, first_out, m, l, (int)pos);
+        }
       }
     }
     // entries flagged for another examination move on to the next frontier
