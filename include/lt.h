@@ -97,6 +97,23 @@ typedef struct {
 int lt_build(int dim, int base_level, int max_level, const double* domain, const int* periodic,
              void* cuda_stream, lt_tree** out);
 
+/* The same on a BRICK of nroot[0] x nroot[1] (x nroot[2]) root cubes (host [dim], NULL = one cube): a
+ * forest of linear trees for domains that are not a cube, e.g. the paper's 3-D slab
+ * [-12.5, 12.5]^2 x 1.5625 = 16 x 16 x 1 cubes, one element thick at D_min (PAPER.md:84
+ * treats "perfect cubes" only; reading J-1).  Levels count from the root cubes; base_level
+ * leaves per cube edge = 2^base_level.  The index r = tx + nroot[0] * (ty + nroot[1] * tz) of a leaf's
+ * cube sits above the path bits of its ID,
+ *     key = (((r << dim * max_level) | interleave(x - cube origin)) << 5) | level,
+ * so leaves are stored cube by cube, in Morton order inside each cube, and one cube gives lt_build's
+ * keys.  Needs dim * max_level + 5 + ceil(log2(#cubes)) <= 63 and nroot[a] * 2^max_level <= 2^31.
+ * `domain` is the whole brick (its cubes have edge (hi_a - lo_a) / nroot[a], equal on all axes for a
+ * conforming mesh); `periodic` wraps the whole brick.  lt_adapt, lt_balance, lt_connect, lt_transfer
+ * and the mortar / FR calls work unchanged; lt_leaf_boxes returns anchors in global finest-cell
+ * units, [0, nroot[a] * 2^max_level).  Construction from points / keys is defined on one cube. */
+int lt_build_brick(int dim, const int* nroot, int base_level, int max_level, const double* domain,
+                   const int* periodic, void* cuda_stream, lt_tree** out);
+int lt_roots(lt_tree*, int* nroot /* host [3] */);
+
 /* Tree from n unsorted device keys (any levels >= base_level; duplicates and ancestors
  * allowed): LSD radix sort over the used key bits, then linearisation (Alg. 3,
  * drop duplicates and every key that is an ancestor of its successor).

@@ -218,13 +218,24 @@ static void toc(Tree* t, int which) {
 }
 
 static int new_tree(int dim, int base, int maxl, const double* domain, const int* periodic, void* stream,
-                    Tree** out) {
+                    Tree** out, const int* nroot = nullptr) {
   if (!out) return LT_ERR_ARG;
   *out = nullptr;
   if (dim != 2 && dim != 3) return LT_ERR_ARG;
   if (base < 0 || maxl < base) return LT_ERR_ARG;
-  if (dim * maxl + kLevelBits > 63 || maxl > 29) return LT_ERR_ARG;
-  if ((int64_t)dim * base > 30) return LT_ERR_ARG;  // 2^(dim*base) leaves must fit an int32 index
+  // the brick of root cubes: the cube index takes tbits key bits above the path bits, and the
+  // global integer coordinates (nroot[a] << maxl) must fit 31 bits
+  int64_t ntrees = 1;
+  for (int a = 0; a < dim; ++a) {
+    const int na = nroot ? nroot[a] : 1;
+    if (na < 1 || ((int64_t)na << maxl) > (1ll << 31)) return LT_ERR_ARG;
+    ntrees *= na;
+    if (ntrees > (1ll << 24)) return LT_ERR_ARG;
+  }
+  int tbits = 0;
+  while ((1ll << tbits) < ntrees) ++tbits;
+  if (dim * maxl + kLevelBits + tbits > 63 || maxl > 29) return LT_ERR_ARG;
+  if ((int64_t)dim * base + tbits > 30) return LT_ERR_ARG;  // the base leaves must fit an int32 index
   int dev = 0;
   LT_CUDA(cudaGetDevice(&dev));
   lt_tree* t = new (std::nothrow) lt_tree();
@@ -245,9 +256,13 @@ static int new_tree(int dim, int base, int maxl, const double* domain, const int
   // bucket index one level below the base tree (buckets of at most 2^(dim*(maxl-base-1)) keys),
   // of at most 2^24 cells
   g.ilevel = base + 1 <= maxl ? base + 1 : maxl;
-  while (dim * g.ilevel > 24) --g.ilevel;
+  while (g.ilevel > 0 && dim * g.ilevel + tbits > 24) --g.ilevel;
   g.ishift = dim * (maxl - g.ilevel);
-  g.nbuckets = 1 << (dim * g.ilevel);
+  g.nbuckets = (int)(ntrees << (dim * g.ilevel));
+  g.tshift = dim * maxl;
+  g.ntrees = (int)ntrees;
+  g.keybits = dim * maxl + kLevelBits + tbits;
+  for (int a = 0; a < 3; ++a) g.nroot[a] = (nroot && a < dim) ? nroot[a] : 1;
   g.periodic = 0;
   for (int a = 0; a < dim; ++a)
     if (periodic && periodic[a]) g.periodic |= 1 << a;
@@ -394,10 +409,21 @@ void lt_free(lt_tree* t) {
 
 int lt_build(int dim, int base_level, int max_level, const double* domain, const int* periodic,
              void* cuda_stream, lt_tree** out) {
+  return lt_build_brick(dim, nullptr, base_level, max_level, domain, periodic, cuda_stream, out);
+}
+
+int lt_roots(lt_tree* t, int* nroot) {
+  if (!t || !nroot) return LT_ERR_ARG;
+  for (int a = 0; a < 3; ++a) nroot[a] = t->g.nroot[a];
+  return LT_OK;
+}
+
+int lt_build_brick(int dim, const int* nroot, int base_level, int max_level, const double* domain,
+                   const int* periodic, void* cuda_stream, lt_tree** out) {
   Tree* t = nullptr;
-  int rc = new_tree(dim, base_level, max_level, domain, periodic, cuda_stream, &t);
+  int rc = new_tree(dim, base_level, max_level, domain, periodic, cuda_stream, &t, nroot);
   if (rc != LT_OK) return rc;
-  const int64_t nb = 1ll << (dim * base_level);
+  const int64_t nb = (int64_t)t->g.ntrees << (dim * base_level);
   if ((rc = grow(t, nb * 2)) != LT_OK) {
     lt_free((lt_tree*)t);
     return rc;
@@ -551,7 +577,7 @@ int lt_adapt(lt_tree* t, const int8_t* d_flags) {
     t->n = n_in;  // fetch_scalars read the (unchanged) device count
     const int64_t n_app = n_kept + t->h_s->aux;
     SortScratch sc = {t->sort_tmp, t->sort_cap, t->sort_hist, t->sort_status, t->sort_status_cap, nullptr};
-    rc = sort_keys(t->keys[t->tmp], n_app, t->g.dim * t->g.maxl + kLevelBits, &sc, t->stream, &t->launches);
+    rc = sort_keys(t->keys[t->tmp], n_app, t->g.keybits, &sc, t->stream, &t->launches);
     t->sort_tmp = sc.tmp; t->sort_cap = sc.cap; t->sort_hist = sc.hist; t->sort_status = sc.status;
     t->sort_status_cap = sc.status_cap;
     if (rc != LT_OK) return rc;

@@ -3,6 +3,9 @@
 //
 // Key format (include/lt.h; Alg. 1):  key = (morton << 5) | level,
 // morton = bit-interleaved integer anchor in finest-cell units, x lowest.
+// On a brick of root cubes (lt_build_brick; reading J-1) the index r of the cube sits above the
+// dim * maxl path bits: morton = (r << dim * maxl) | in-cube morton, r = tx + nroot[0] * (ty + nroot[1] * tz).
+// Every routine below works on this "global" morton code; a single cube has r = 0.
 #pragma once
 #include <cooperative_groups.h>
 #include <cuda_runtime.h>
@@ -20,7 +23,11 @@ struct Geo {
   int ishift;       // dim * (maxl - ilevel): morton >> ishift = bucket
   int nbuckets;     // 2^(dim*ilevel)
   int periodic;     // bit a set = axis a periodic
-  uint64_t total;   // (1 << dim*maxl) - 1 : all morton bits in use
+  uint64_t total;   // (1 << dim*maxl) - 1 : all in-cube morton bits
+  int tshift;       // dim * maxl: the cube index sits above the path bits
+  int ntrees;       // nroot[0] * nroot[1] * nroot[2] root cubes
+  int nroot[3];     // the brick (1, 1, 1: a single cube)
+  int keybits;      // bits of a key in use: dim * maxl + 5 + bits of the cube index
 };
 
 template <int DIM> struct Dim;
@@ -112,9 +119,10 @@ __device__ __forceinline__ bool is_ancestor(const Geo& g, uint64_t ka, uint64_t 
 
 // Same-level face neighbour of the cell (m, l) across local face f (0=-x 1=+x 2=-y ...),
 // computed on the dilated integer: add / subtract the cell width on one axis with the
-// carry rippling over the other axes' bit positions.  Coordinates wrap mod 2^maxl
-// (periodic treatment).  Returns false when the face lies on the domain
-// boundary of a non-periodic axis; *wrapped tells whether the wrap was used.
+// carry rippling over the other axes' bit positions.  Inside a cube the coordinate wraps mod
+// 2^maxl; a step over the cube's face moves to the adjacent cube of the brick, with the periodic
+// wrap of the whole domain or, on a non-periodic axis, ends at the domain boundary
+// (returns false).  The cube index bits of m are carried along.
 template <int DIM>
 __device__ __forceinline__ bool face_neighbour(const Geo& g, uint64_t m, int l, int f, uint64_t* mn) {
   const int a = f >> 1;
@@ -132,7 +140,19 @@ __device__ __forceinline__ bool face_neighbour(const Geo& g, uint64_t m, int l, 
     na = ((m & maskA) - wbit) & maskA;
   }
   *mn = (m & ~maskA) | na;
-  return !(edge && !((g.periodic >> a) & 1));
+  if (!edge) return true;
+  const bool per = (g.periodic >> a) & 1;
+  if (g.nroot[a] == 1) return per;  // one cube along this axis: its own periodic image
+  const int stride = a == 0 ? 1 : (a == 1 ? g.nroot[0] : g.nroot[0] * g.nroot[1]);
+  const int tree = (int)(m >> g.tshift);
+  const int ta = (tree / stride) % g.nroot[a];
+  int tn = ta + ((f & 1) ? 1 : -1);
+  if (tn < 0 || tn >= g.nroot[a]) {
+    if (!per) return false;
+    tn = tn < 0 ? g.nroot[a] - 1 : 0;
+  }
+  *mn = ((uint64_t)(tree + (tn - ta) * stride) << g.tshift) | (*mn & g.total);
+  return true;
 }
 
 // Point location (the lower-bound search of PAPER.md:134-143, Eq. 7, in one form):

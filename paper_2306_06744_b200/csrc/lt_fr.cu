@@ -298,8 +298,10 @@ static int launch_fr_rhs_t(Tree* t, const double* d_u, const double* d_fs, doubl
   int per_sm = 0;
   LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, warps * 32, smem));
   if (per_sm < 1) per_sm = 1;
-  const double w0 = t->domain[DIM] - t->domain[0], w1 = t->domain[DIM + 1] - t->domain[1];
-  const double w2 = DIM == 3 ? t->domain[DIM + 2] - t->domain[2] : 1.0;
+  // width of a root cube along each axis (a single cube: the domain width)
+  const double w0 = (t->domain[DIM] - t->domain[0]) / t->g.nroot[0];
+  const double w1 = (t->domain[DIM + 1] - t->domain[1]) / t->g.nroot[1];
+  const double w2 = DIM == 3 ? (t->domain[DIM + 2] - t->domain[2]) / t->g.nroot[2] : 1.0;
   fn<<<t->num_sms * per_sm, warps * 32, smem, t->stream>>>(t->g, t->keys[t->cur], t->d_s, d_u, d_fs, d_R, w0, w1,
                                                             w2, d_un, ca, cb, dt);
   return LT_OK;

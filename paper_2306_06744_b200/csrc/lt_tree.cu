@@ -47,14 +47,23 @@ __global__ void k_decode(const uint64_t* __restrict__ keys, int64_t n, int32_t* 
   }
 }
 
+// (leaves of a tree: anchors in GLOBAL finest-cell units, the cube's offset in the brick added)
 template <int DIM>
-__global__ void k_decode_n(const uint64_t* __restrict__ keys, const DevScalars* __restrict__ s,
+__global__ void k_decode_n(Geo g, const uint64_t* __restrict__ keys, const DevScalars* __restrict__ s,
                            int32_t* __restrict__ level, uint32_t* __restrict__ xyz) {
   const int64_t n = s->n;
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
     uint64_t k = keys[i];
     uint32_t x[3];
-    deinterleave<DIM>(key_morton(k), x);
+    deinterleave<DIM>(key_morton(k) & g.total, x);
+    if (g.ntrees > 1) {
+      int tree = (int)(key_morton(k) >> g.tshift);
+#pragma unroll
+      for (int a = 0; a < DIM; ++a) {
+        x[a] += (uint32_t)(tree % g.nroot[a]) << g.maxl;
+        tree /= g.nroot[a];
+      }
+    }
     if (level) level[i] = key_level(k);
     if (xyz) {
       xyz[3 * i] = x[0];
@@ -66,10 +75,12 @@ __global__ void k_decode_n(const uint64_t* __restrict__ keys, const DevScalars* 
 
 // ------------------------------------------------------------------------ uniform build
 // Leaf i of the uniform level-`base` tree has raw ID i (Morton order), key =
-// (i << dim*(maxl-base)) << 5 | base (Alg. 1 with the padding of step 4).
+// (i << dim*(maxl-base)) << 5 | base (Alg. 1 with the padding of step 4).  On a brick the cubes follow
+// one another: leaf i of cube r is entry r * 2^(dim*base) + i, and the same formula places r above the
+// path bits.
 template <int DIM>
 __global__ void k_build_uniform(Geo g, uint64_t* __restrict__ keys, int* __restrict__ first, DevScalars* s) {
-  const int64_t nb = 1ll << (DIM * g.base);
+  const int64_t nb = (int64_t)g.ntrees << (DIM * g.base);
   const int pad = DIM * (g.maxl - g.base);
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < nb; i += (int64_t)gridDim.x * blockDim.x) {
     keys[i] = make_key((uint64_t)i << pad, g.base);
@@ -819,8 +830,8 @@ int launch_balance(Tree* t, int64_t cap_told, int use_front) {
 
 int launch_leaf_boxes(Tree* t, int32_t* d_level, uint32_t* d_xyz) {
   int G = grid_for(t, 8);
-  LT_DISPATCH_DIM(t, (k_decode_n<2><<<G, BT, 0, t->stream>>>(t->keys[t->cur], t->d_s, d_level, d_xyz)),
-                  (k_decode_n<3><<<G, BT, 0, t->stream>>>(t->keys[t->cur], t->d_s, d_level, d_xyz)));
+  LT_DISPATCH_DIM(t, (k_decode_n<2><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], t->d_s, d_level, d_xyz)),
+                  (k_decode_n<3><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], t->d_s, d_level, d_xyz)));
   t->launches++;
   LT_CUDA(cudaGetLastError());
   return LT_OK;

@@ -77,6 +77,8 @@ SIGNATURES = {
     "lt_timings": (_I, [_P, _P]),
     "lt_launch_count": (_I64, [_P]),
     "lt_host_syncs": (_I64, [_P]),
+    "lt_build_brick": (_I, [_I, _P, _I, _I, _P, _P, _P, C.POINTER(_P)]),
+    "lt_roots": (_I, [_P, _P]),
     "lt_balance_phases": (_I, [_P, _P]),
     "lt_strerror": (C.c_char_p, [_I]),
     "lt_last_cuda_error": (_I, []),
@@ -139,7 +141,7 @@ class Tree:
     """One linear quadtree / octree on the current CUDA device (handle of lt_build)."""
 
     def __init__(self, dim, base_level, max_level, domain=None, periodic=None, keys=None, device=None,
-                 complete=False, points=None):
+                 complete=False, points=None, nroot=None):
         self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
         self.dim, self.base, self.maxl = dim, base_level, max_level
         self.nc, self.nf = 1 << dim, 2 * dim
@@ -160,6 +162,10 @@ class Tree:
                                                        _stream_ptr(self.device),
                                                        _dptr(k.view(torch.int64), torch.int64, "keys"), k.numel(),
                                                        C.byref(h))
+            elif keys is None and nroot is not None:
+                nr = (C.c_int * dim)(*[int(v) for v in nroot[:dim]])
+                rc = lib().lt_build_brick(dim, nr, base_level, max_level, dom, per, _stream_ptr(self.device),
+                                          C.byref(h))
             elif keys is None:
                 rc = lib().lt_build(dim, base_level, max_level, dom, per, _stream_ptr(self.device), C.byref(h))
             else:
@@ -353,6 +359,11 @@ class Tree:
         _check(lib().lt_leaf_boxes(self._h, C.c_void_p(lvl.data_ptr()), C.c_void_p(xyz.data_ptr())), "lt_leaf_boxes")
         return lvl, xyz
 
+    def roots(self):
+        out = (C.c_int * 3)()
+        _check(lib().lt_roots(self._h, out), "lt_roots")
+        return tuple(out[: self.dim])
+
     def reserve(self, n):
         _check(lib().lt_reserve(self._h, int(n)), "lt_reserve")
 
@@ -383,6 +394,11 @@ class Tree:
 def build(dim, base_level, max_level, domain=None, periodic=None) -> Tree:
     """lt_build"""
     return Tree(dim, base_level, max_level, domain, periodic)
+
+
+def build_brick(dim, nroot, base_level, max_level, domain=None, periodic=None) -> Tree:
+    """lt_build_brick: a forest on nroot[0] x nroot[1] (x nroot[2]) root cubes."""
+    return Tree(dim, base_level, max_level, domain, periodic, nroot=nroot)
 
 
 def build_from_keys(dim, base_level, max_level, keys, domain=None, periodic=None) -> Tree:

@@ -37,7 +37,29 @@ CONFIGS = {
                flags="vortex", seed=0, rand_refine=0.0, rand_coarsen=0.0, u0="vortex"),
     "c5": dict(dim=3, base=6, maxl=9, lo=-10.0, hi=10.0, periodic=(1, 1, 1), cycles=10, p=3, nvars=5,
                flags="vortex", seed=2, rand_refine=0.10, rand_coarsen=0.10, u0="vortex"),
+    # The paper's own 3-D domain (Table 5): the slab [-12.5, 12.5]^2 x [0, 1.5625], one element
+    # thick at D_min = 4 -- a brick of 16 x 16 x 1 root cubes of edge 1.5625 (lt_build_brick), levels counted
+    # from the cubes: max level +4 = the paper's D_max 8 (dx_min = 25/256).  Flags: config 4's vortex-tube
+    # recipe.  "lo" is per axis, "cube" the edge of a root cube; hi = lo + nroot * cube.
+    "slab": dict(dim=3, nroot=(16, 16, 1), base=0, maxl=4, lo=(-12.5, -12.5, 0.0), cube=1.5625, periodic=(1, 1, 1),
+                 cycles=20, p=2, nvars=5, flags="vortex", seed=0, rand_refine=0.0, rand_coarsen=0.0, u0="vortex"),
 }
+
+
+def geometry(cfg: dict):
+    """(lo[dim], cube edge, nroot[dim]) of a config: a single cube [lo, hi]^dim unless "nroot" is given."""
+    dim = cfg["dim"]
+    nroot = tuple(cfg.get("nroot", (1,) * dim))
+    lo = cfg["lo"]
+    lo = tuple(float(v) for v in lo) if isinstance(lo, (tuple, list)) else (float(lo),) * dim
+    cube = float(cfg["cube"]) if "cube" in cfg else float(cfg["hi"]) - lo[0]
+    return lo, cube, nroot
+
+
+def domain(cfg: dict):
+    """lo_x.., hi_x.. of the whole domain (the `domain` argument of lt_build / lt_build_brick)."""
+    lo, cube, nroot = geometry(cfg)
+    return list(lo) + [lo[a] + nroot[a] * cube for a in range(cfg["dim"])]
 
 _M64 = (1 << 64) - 1
 
@@ -82,9 +104,11 @@ def counter_uniform(seed: int, stream: int, *ints: torch.Tensor) -> torch.Tensor
 def centres(cfg: dict, level: torch.Tensor, xyz: torch.Tensor) -> torch.Tensor:
     """Leaf centres [M,dim] float64: lo + (x + w/2) (hi-lo)/2^Dmax, w = 2^(Dmax-level)."""
     dim, maxl = cfg["dim"], cfg["maxl"]
+    lo, cube, _ = geometry(cfg)
     w = torch.pow(2.0, (maxl - level.to(torch.int64)).to(torch.float64))
-    scale = (cfg["hi"] - cfg["lo"]) / float(1 << maxl)
-    return cfg["lo"] + (xyz[:, :dim].to(torch.float64) + 0.5 * w[:, None]) * scale
+    scale = cube / float(1 << maxl)
+    lo_t = torch.tensor(lo, dtype=torch.float64, device=level.device)
+    return lo_t[None, :] + (xyz[:, :dim].to(torch.float64) + 0.5 * w[:, None]) * scale
 
 
 def _min_image(d: torch.Tensor, period: float) -> torch.Tensor:
@@ -94,13 +118,13 @@ def _min_image(d: torch.Tensor, period: float) -> torch.Tensor:
 def _vortex_w(cfg: dict, cycle: int, pos: torch.Tensor) -> torch.Tensor:
     """Relative vorticity magnitude |1 - r^2/2| exp(-r^2/2) of the vortex of Eq. 21
     (tube along z in 3-D) centred at (0.2 c, 0.2 c), minimum-image distance."""
-    L = cfg["hi"] - cfg["lo"]
+    _, cube, nroot = geometry(cfg)
     dx = pos[:, 0] - 0.2 * cycle
     dy = pos[:, 1] - 0.2 * cycle
     if cfg["periodic"][0]:
-        dx = _min_image(dx, L)
+        dx = _min_image(dx, nroot[0] * cube)
     if cfg["periodic"][1]:
-        dy = _min_image(dy, L)
+        dy = _min_image(dy, nroot[1] * cube)
     r2 = dx * dx + dy * dy
     return torch.abs(1.0 - 0.5 * r2) * torch.exp(-0.5 * r2)
 
@@ -126,11 +150,12 @@ def flags(name_or_cfg, cycle: int, level: torch.Tensor, xyz: torch.Tensor) -> to
     elif kind == "point":
         half = cfg["cycles"] // 2
         if cycle < half:  # refine the leaf containing the point
-            scale = float(1 << maxl) / (cfg["hi"] - cfg["lo"])
+            glo, gcube, _ = geometry(cfg)
+            scale = float(1 << maxl) / gcube
             inside = torch.ones(M, dtype=torch.bool, device=lvl.device)
             wd = torch.ones_like(lvl) << (maxl - lvl)
             for a in range(dim):
-                pi = int(math.floor((cfg["point"][a] - cfg["lo"]) * scale))
+                pi = int(math.floor((cfg["point"][a] - glo[a]) * scale))
                 inside &= (X[:, a] <= pi) & (pi < X[:, a] + wd)
             f[inside] = 1
         else:  # coarsen everything
@@ -174,12 +199,13 @@ def initial_solution(name_or_cfg, level: torch.Tensor, xyz: torch.Tensor) -> tor
     # analytic vortex, conserved variables at the solution points (SURVEY 8(d) relations)
     z = torch.as_tensor(_gl_nodes(p), dtype=torch.float64, device=dev)
     w = torch.pow(2.0, (maxl - lvl).to(torch.float64))
-    scale = (cfg["hi"] - cfg["lo"]) / float(1 << maxl)
+    glo, gcube, _ = geometry(cfg)
+    scale = gcube / float(1 << maxl)
     idx = torch.arange(N, device=dev)
     pos = []
     for a in range(dim):
         ia = (idx // (P1 ** a)) % P1
-        pos.append(cfg["lo"] + (X[:, a].to(torch.float64)[:, None] + 0.5 * w[:, None] * (1.0 + z[ia][None, :])) * scale)
+        pos.append(glo[a] + (X[:, a].to(torch.float64)[:, None] + 0.5 * w[:, None] * (1.0 + z[ia][None, :])) * scale)
     alpha, phi, gamma = 5.0, 0.5, 1.4
     dx, dy = pos[0], pos[1]
     r2 = dx * dx + dy * dy

@@ -52,9 +52,10 @@ def host_flags(cfg, cycle, ot):
 
 
 def new_pair(cfg):
-    dom = [cfg["lo"]] * cfg["dim"] + [cfg["hi"]] * cfg["dim"]
-    gt = lt.Tree(cfg["dim"], cfg["base"], cfg["maxl"], dom, cfg["periodic"])
-    ot = oracle.Tree(cfg["dim"], cfg["base"], cfg["maxl"], cfg["periodic"])
+    """Both sides on the config's domain: one cube, or a brick of root cubes when cfg has "nroot"."""
+    nroot = cfg.get("nroot")
+    gt = lt.Tree(cfg["dim"], cfg["base"], cfg["maxl"], W.domain(cfg), cfg["periodic"], nroot=nroot)
+    ot = oracle.Tree(cfg["dim"], cfg["base"], cfg["maxl"], cfg["periodic"], nroot=nroot)
     return gt, ot
 
 
@@ -122,8 +123,7 @@ def run_cycles(cfg, ncycles, options=(), check_faces=True, check_transfer=True, 
 def replay_gpu(cfg, record, options=()):
     """GPU only: drive a fresh tree through the recorded flags with `options` set and compare keys and
     sweep counts with the recorded (oracle) ones -- options must not change results."""
-    dom = [cfg["lo"]] * cfg["dim"] + [cfg["hi"]] * cfg["dim"]
-    gt = lt.Tree(cfg["dim"], cfg["base"], cfg["maxl"], dom, cfg["periodic"])
+    gt = lt.Tree(cfg["dim"], cfg["base"], cfg["maxl"], W.domain(cfg), cfg["periodic"], nroot=cfg.get("nroot"))
     for opt, val in options:
         gt.set_option(opt, val)
     for c, (f, keys, iters) in enumerate(record):
