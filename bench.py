@@ -39,7 +39,7 @@ FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 # untimed preparation cycles and the cycles the steps run through, per config: c5 cannot run its 10 stated
 # cycles (reading F-2); the small configs run ALL their stated cycles from the uniform tree, one step each
 SCHEDULES = {"c5": (3, (3, 4, 5)), "c1": (0, tuple(range(4))), "c2": (0, tuple(range(50))),
-             "c4": (0, tuple(range(20)))}
+             "c4": (0, tuple(range(20))), "slab": (0, tuple(range(20)))}
 WORKLOADS = {
     "c5": "c5 (BASELINE.json configs[4]): 3D octree, periodic [-10,10]^3, base 64^3, max level +3, vortex-tube flags + "
           "10% random refine / 10% random group coarsen (seed 2), p=3 (64 solution points), 5 fp64 vars",
@@ -49,6 +49,9 @@ WORKLOADS = {
           "flags, 50 cycles, p=3, 4 fp64 vars",
     "c4": "c4 (BASELINE.json configs[3]): 3D octree, periodic [-10,10]^3, base 32^3, max level +3, vortex-tube flags, "
           "20 cycles, p=2, 5 fp64 vars",
+    "slab": "slab (the paper's own 3-D domain, PAPER.md:410 / Table 5): periodic [-12.5,12.5]^2 x [0,1.5625] as a brick of "
+            "16 x 16 x 1 root cubes (lt_build_brick), max level +4 (the paper's D_max 8), config 4's vortex-tube flags, "
+            "20 cycles, p=2, 5 fp64 vars",
 }
 
 
@@ -162,7 +165,7 @@ def oracle_cycles(cfg, cycles, transfer_fraction=1.0):
     import oracle
     from paper_2306_06744_b200 import workloads as W
     p, nvars = cfg["p"], cfg["nvars"]
-    ot = oracle.Tree(cfg["dim"], cfg["base"], cfg["maxl"], cfg["periodic"])
+    ot = oracle.Tree(cfg["dim"], cfg["base"], cfg["maxl"], cfg["periodic"], nroot=cfg.get("nroot"))
     lvl, xyz = ot.leaf_boxes()
     L, X = torch.from_numpy(lvl), torch.from_numpy(xyz.astype(np.int64))
     full = transfer_fraction >= 1.0
@@ -213,7 +216,8 @@ def oracle_cycles(cfg, cycles, transfer_fraction=1.0):
 
 
 # default (bounded, 3-30 s of host time) and --oracle-full samples of the cpu_baseline per config
-ORACLE_SAMPLES = {"c5": (1, 1.0, 4, 0.02), "c1": (4, 1.0, 4, 1.0), "c2": (12, 1.0, 50, 1.0), "c4": (3, 1.0, 20, 1.0)}
+ORACLE_SAMPLES = {"c5": (1, 1.0, 4, 0.02), "c1": (4, 1.0, 4, 1.0), "c2": (12, 1.0, 50, 1.0), "c4": (3, 1.0, 20, 1.0),
+                  "slab": (20, 1.0, 20, 1.0)}
 
 
 def cpu_baseline(name, cfg, full=False):
@@ -285,8 +289,8 @@ class Runner:
         cfg = self.cfg
         if self.tree is not None:
             self.tree.free()
-        dom = [cfg["lo"]] * cfg["dim"] + [cfg["hi"]] * cfg["dim"]
-        self.tree = self.lt.Tree(cfg["dim"], cfg["base"], cfg["maxl"], dom, cfg["periodic"])
+        self.tree = self.lt.Tree(cfg["dim"], cfg["base"], cfg["maxl"], self.W.domain(cfg), cfg["periodic"],
+                                 nroot=cfg.get("nroot"))
         if reserve:
             self.tree.reserve(reserve)
         if CONNECTIVITY != 1:
@@ -373,6 +377,11 @@ def run_ours(args):
         sizes.append((m0, R.tree.num_leaves()))
     max_leaves = max(max(s) for s in sizes)
     cap = int(max_leaves * 1.02) + 4096
+    # small meshes (the paper's own sizes): reserve the worst case, 2^dim x leaves, so that lt_adapt and
+    # lt_balance(iters = NULL) only enqueue and the cycle has ONE host synchronisation (lt_connect_end)
+    deferred = (not args.sync_calls) and OVERLAP and (max_leaves << cfg["dim"]) * 160 < (8 << 30)
+    if deferred:
+        cap = (max_leaves << cfg["dim"]) + 4096
     need = [0, 0]  # step k reads buffer k % 2 and writes the other one
     for k, (m0, m1) in enumerate(sizes):
         need[k % 2] = max(need[k % 2], m0)
@@ -401,11 +410,21 @@ def run_ours(args):
         torch.cuda.synchronize(dev)
         ev0.record(stream)
         t.adapt(f)
-        Ma = t.num_leaves()
-        iters = t.balance()
-        M1 = t.num_leaves()
-        u_new = ubuf[cur ^ 1][:M1]
-        if overlap:
+        if deferred and overlap:
+            t.balance(want_iters=False)
+            t.connect_begin()
+            t.transfer_into(u_old, ubuf[cur ^ 1], p, nvars)
+            F = t.connect_end()                      # the only host synchronisation of the cycle
+            M1 = Ma = int(F["n_leaves"])             # (the count after lt_adapt never reached the host)
+            iters = t.last_balance_iters()
+        else:
+            Ma = t.num_leaves()
+            iters = t.balance()
+            M1 = t.num_leaves()
+            u_new = ubuf[cur ^ 1][:M1]
+        if deferred and overlap:
+            pass
+        elif overlap:
             # the face query (side stream) overlaps the HBM-bound transfer: both depend only on
             # the balanced tree
             t.connect_begin()
@@ -419,6 +438,7 @@ def run_ours(args):
         t.sync()
         ms = ev0.elapsed_time(ev1)
         tm = t.timings()
+        tm.update({"balance_" + k: v for k, v in t.balance_phases().items()})
         cur ^= 1
         return dict(cycle=c, M0=M0, Ma=Ma, M1=M1, iters=iters, faces=(F["n_conf"], F["n_hang"], F["n_bnd"]),
                     ms=ms, tm=tm, launches=t.launch_count() - launches0, syncs=t.host_syncs() - syncs0)
@@ -541,6 +561,10 @@ def run_ours(args):
                        "leaves_out_per_step": [s["M1"] for s in steps], "leaves_in_per_step": [s["M0"] for s in steps],
                        "balance_iters": [s["iters"] for s in steps], "balance_connectivity": CONNECTIVITY,
                        "connect_transfer_overlap": OVERLAP,
+                       "host_synchronisations": "one per cycle (lt_connect_end): buffers reserved for 2^dim x leaves, "
+                                                "lt_adapt and lt_balance(iters=NULL) only enqueue" if deferred else
+                                                "three per cycle (lt_adapt sizes its buffers, lt_balance returns the "
+                                                "sweep count, lt_connect_end the face counts)",
                        "l2": "L2 flushed between timed steps (a 512 MB fill; the inputs are smaller than L2)" if small
                              else "inputs larger than L2 (u_old + u_new are %.0f-%.0f GB per step)" % (
                                  min(sum(x) for x in sizes) * Bu / 1e9, max(sum(x) for x in sizes) * Bu / 1e9),
@@ -572,12 +596,12 @@ def run_e2e(R, args, world, dev):
     nf = 2 * cfg["dim"]
     budget = min(64 << 30, int(0.4 * mem_available_bytes() / max(world, 1)))
     last = PERIOD[0] if CONFIG == "c5" else PERIOD[-1]
-    dom = [cfg["lo"]] * cfg["dim"] + [cfg["hi"]] * cfg["dim"]
+    dom = R.W.domain(cfg)
 
     def fresh(upto):
         if R.tree is not None:
             R.tree.free()
-        t = R.lt.Tree(cfg["dim"], cfg["base"], cfg["maxl"], dom, cfg["periodic"])
+        t = R.lt.Tree(cfg["dim"], cfg["base"], cfg["maxl"], dom, cfg["periodic"], nroot=cfg.get("nroot"))
         if CONNECTIVITY != 1:
             t.set_option(R.lt.LT_OPT_BALANCE_CONNECTIVITY, CONNECTIVITY)
         R.tree = t
@@ -884,10 +908,12 @@ def run_solver(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
     global PREP_CYCLES
-    PREP_CYCLES = 2
+    # c5: cycle 2 (1.9 M -> 8.86 M leaves); slab (the paper's own 3-D domain and mesh sizes): cycle 8
+    name = CONFIG if CONFIG in ("c5", "slab") else "c5"
+    PREP_CYCLES = 2 if name == "c5" else 8
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
-    cfg = W.CONFIGS["c5"]
+    cfg = W.CONFIGS[name]
     R = Runner(cfg, dev)
     p, nvars, nf = cfg["p"], cfg["nvars"], 6
     N, Nf = (p + 1) ** 3, (p + 1) ** 2
@@ -908,7 +934,7 @@ def run_solver(args):
         t = R.tree
         u_old = torch.empty((M0, nvars, N), dtype=torch.float64, device=dev)
         R.analytic_u(u_old)
-        f = R.flags(2)
+        f = R.flags(PREP_CYCLES)
 
         def cyc():
             t.adapt(f)
@@ -930,7 +956,8 @@ def run_solver(args):
     uf = torch.empty((M, nf, nvars, Nf), dtype=torch.float64, device=dev)
     fs = torch.empty_like(uf)
     rhs, us = torch.empty_like(u), torch.empty_like(u)
-    dt = 2e-4  # finest cell 20 / 512, p = 3, |v| + c about 4.2: well inside the RK3 stability limit
+    # finest cell 20 / 512 (c5, p = 3) or 25 / 256 (slab, p = 2), |v| + c about 4.2: well inside the RK3 limit
+    dt = 2e-4 if name == "c5" else 5e-4
 
     def fluxes_of(x):
         t.face_interp(x, p, nvars, u_face=uf)
@@ -970,10 +997,12 @@ def run_solver(args):
         "value": frac, "unit": "fraction", "n_gpus": 1, "steps": 1, "warmup": 1,
         "ms_per_step": ms_adapt + ms_solve, "higher_is_better": False, "scaling": "weak", "vs_baseline": frac / 0.0194,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "solver: config-5 cycle 2 (%d -> %d leaves, p=3, 5 fp64 vars, Euler) + 10 RK3 steps "
-                               "(30 right-hand sides) on the adapted mesh" % (M0, M),
+        "config": {"workload": "solver: %s cycle %d (%d -> %d leaves, p=%d, 5 fp64 vars, Euler) + 10 RK3 steps "
+                               "(30 right-hand sides) on the adapted mesh" % (name, PREP_CYCLES, M0, M, p),
                    "baseline": "paper Table 5, p2 D_max 8, RTX 2060: 81.39 s / 4193.54 s = 1.94 % (160 k elements)",
-                   "l2": "arrays of 22.7-34 GB, larger than L2"},
+                   "l2": "arrays of %.2f-%.2f GB%s" % (M * Bu / 1e9, M * 6 * Bf / 1e9,
+                                                        ", larger than L2" if M * Bu > (256 << 20) else
+                                                        " (smaller than L2: the paper's own mesh size, launch-bound)")},
         "ms_per_call": {"adaptation_cycle": ms_adapt, "ten_rk3_steps": ms_solve, "one_rhs_chain": ms_rhs},
         "roofline": {"bound": "hbm", "kernel": "RK stage (face_interp, mortar_project, common_flux, mortar_gather, "
                                                "fr_stage)", "achieved": bytes_stage * 30 / (ms_solve * 1e-3) / 1e9,
@@ -995,6 +1024,9 @@ def main():
     ap.add_argument("--oracle-full", action="store_true",
                     help="cpu_baseline / --impl reference on the config's full sample (c1-c4: every cycle; c5: cycles "
                          "0-3 with the transfer timed on slabs) instead of the bounded default")
+    ap.add_argument("--sync-calls", action="store_true",
+                    help="small configs: keep the synchronising lt_adapt / lt_balance (the before of the "
+                         "one-synchronisation cycle)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--workload", default="cycle", choices=["cycle", "construct", "mortar", "solver"],

@@ -161,7 +161,8 @@ int lt_reserve(lt_tree*, int64_t n_leaves);
  * children occupy its Morton interval), so no sort is needed; set
  * lt_set_option(t, LT_OPT_ADAPT_SORT, 1) to realise it as the paper does (append, radix
  * sort, linearise) -- same result.  Synchronises once (reads the new leaf count to size
- * buffers). */
+ * buffers) -- unless the buffers already hold the worst case, 2^dim * lt_num_leaves (lt_reserve): then
+ * the call only enqueues, and the new count stays on the device until a later call needs it. */
 int lt_adapt(lt_tree*, const int8_t* d_flags);
 
 /* 2:1 face balance (Alg. 4; readings C-1..C-7): the unique coarsest
@@ -171,7 +172,11 @@ int lt_adapt(lt_tree*, const int8_t* d_flags);
  * If the tree was balanced when the preceding lt_adapt was called, the first sweep examines only
  * the leaves that call created (same result, sweep count and splits as a full sweep).
  * Synchronises at the end (reads leaf count / status).  On LT_ERR_CAPACITY (growth
- * impossible) the tree is a valid, partially balanced refinement of the input. */
+ * impossible) the tree is a valid, partially balanced refinement of the input.
+ * With iters == NULL, face connectivity, a tree that was balanced before the preceding lt_adapt and
+ * buffers that hold 2^dim * lt_num_old_leaves leaves (the largest result possible, reading C-5) the
+ * call only enqueues: lt_connect_begin, lt_transfer and lt_connect_end then run the rest of the cycle
+ * with ONE host synchronisation (in lt_connect_end); lt_last_balance_iters returns the sweep count. */
 int lt_balance(lt_tree*, int* iters);
 
 /* Alg. 5: fills *out (host struct; device arrays inside).
@@ -266,6 +271,7 @@ int lt_fr_stage(lt_tree*, int stage, double dt, const double* d_u_n, const doubl
 /* ---- accessors --------------------------------------------------------------------- */
 
 int64_t lt_num_leaves(lt_tree*);       /* synchronises only if the count is not cached   */
+int lt_last_balance_iters(lt_tree*);   /* sweeps of the last lt_balance (also after lt_balance(t, NULL)); same rule */
 int64_t lt_num_old_leaves(lt_tree*);   /* leaves of the snapshot T_old (0 if none)        */
 const uint64_t* lt_keys(lt_tree*);     /* device, sorted                                  */
 const uint64_t* lt_old_keys(lt_tree*); /* device, snapshot (NULL if none)                 */

@@ -183,6 +183,14 @@ static int fetch_scalars(Tree* t) {
   LT_CUDA(host_sync(t));
   t->n = t->h_s->n;
   t->n_valid = true;
+  if (t->parity_pending) {  // an lt_balance that did not wait: which key buffer holds its result
+    if (t->h_s->parity) {
+      const int c = t->cur;
+      t->cur = t->tmp;
+      t->tmp = c;
+    }
+    t->parity_pending = false;
+  }
   return LT_OK;
 }
 
@@ -286,6 +294,7 @@ static int new_tree(int dim, int base, int maxl, const double* domain, const int
   if ((rc = alloc_dev(t->stream, &t->d_sums, kMaxGrid)) != LT_OK) return fail(rc);
   if ((rc = alloc_dev(t->stream, &t->d_sums3, 3 * kMaxGrid)) != LT_OK) return fail(rc);
   if ((rc = alloc_dev(t->stream, &t->d_cmarks, 2 * kMaxGrid)) != LT_OK) return fail(rc);
+  if (cudaMemsetAsync(t->d_cmarks, 0, 2 * kMaxGrid * sizeof(int), t->stream) != cudaSuccess) return fail(LT_ERR_CUDA);
   static_assert(sizeof(DevScalars) <= 256, "mirror layout");
   t->h_s = (DevScalars*)mirror_get();  // one pinned block: scalars | chunk sums
   if (!t->h_s) return fail(LT_ERR_OOM);
@@ -458,7 +467,19 @@ int64_t lt_num_leaves(lt_tree* t) {
   return t->n;
 }
 int64_t lt_num_old_leaves(lt_tree* t) { return t && t->have_old ? t->n_old : 0; }
-const uint64_t* lt_keys(lt_tree* t) { return t ? t->keys[t->cur] : nullptr; }
+const uint64_t* lt_keys(lt_tree* t) {
+  if (!t) return nullptr;
+  if (!t->n_valid && fetch_scalars(t) != LT_OK) return nullptr;  // (settles which buffer is current)
+  return t->keys[t->cur];
+}
+int lt_last_balance_iters(lt_tree* t) {
+  if (!t) return LT_ERR_ARG;
+  if (!t->n_valid) {
+    int rc = fetch_scalars(t);
+    if (rc != LT_OK) return rc;
+  }
+  return t->last_iters >= 0 ? t->last_iters : t->h_s->iters;
+}
 const uint64_t* lt_old_keys(lt_tree* t) { return t && t->have_old ? t->keys[t->old] : nullptr; }
 
 int lt_domain(lt_tree* t, double* lo_hi) {
@@ -519,6 +540,8 @@ int lt_balance_phases(lt_tree* t, float* out4) {
 
 int lt_leaf_boxes(lt_tree* t, int32_t* d_level, uint32_t* d_xyz) {
   if (!t) return LT_ERR_ARG;
+  int rc;
+  if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
   return launch_leaf_boxes(t, d_level, d_xyz);
 }
 
@@ -544,6 +567,28 @@ int lt_adapt(lt_tree* t, const int8_t* d_flags) {
   tic(t, 0);
   const int G = grid_for(t, 8);
   if ((rc = launch_adapt_count(t, d_flags, G)) != LT_OK) return rc;
+  const int nc = 1 << t->g.dim;
+  if (!t->opt_adapt_sort && t->cap >= nc * t->n) {
+    // The buffers hold the worst case (every leaf refined): nothing to size, so the host does not wait
+    // for the new count -- it stays on the device until a call needs it (lt_num_leaves, lt_connect_end ...).
+    const int emit = t->balanced_conn >= 1;
+    if ((rc = launch_adapt_scatter(t, d_flags, G, 0, emit)) != LT_OK) return rc;
+    const int o = t->old;
+    t->old = t->cur;
+    t->cur = t->tmp;
+    t->tmp = o;
+    t->have_old = true;
+    t->n_old = t->n;
+    t->n_upper = nc * t->n;
+    t->n_valid = false;
+    t->map_valid = false;
+    t->map_ready = false;
+    t->faces_valid = false;
+    t->front_ok = emit != 0;
+    t->balanced_conn = 0;
+    toc(t, 0);
+    return LT_OK;
+  }
   // the new size is needed on the host to size buffers: one small read-back
   LT_CUDA(cudaMemcpyAsync(t->h_sums, t->d_sums, (size_t)G * sizeof(unsigned long long), cudaMemcpyDeviceToHost,
                           t->stream));
@@ -561,7 +606,6 @@ int lt_adapt(lt_tree* t, const int8_t* d_flags) {
     // path B: ordered expansion cur -> tmp.  If the tree was balanced, the leaves created here
     // become the frontier of lt_balance's first sweep.
     const int emit = t->balanced_conn >= 1;
-    if (emit) LT_CUDA(cudaMemsetAsync(&t->d_s->nfront[0], 0, sizeof(int), t->stream));
     if ((rc = launch_adapt_scatter(t, d_flags, G, 0, emit)) != LT_OK) return rc;
     front_ok = emit != 0;
     const int o = t->old;
@@ -612,6 +656,26 @@ int lt_balance(lt_tree* t, int* iters) {
   if (!t) return LT_ERR_ARG;
   int rc;
   if ((rc = join_side(t)) != LT_OK) return rc;
+  t->last_iters = -1;
+  // Without a sweep count to hand back, and when the buffers hold the largest tree the ripple can
+  // produce -- a tree that was balanced before lt_adapt is never refined by more than one level
+  // (reading C-5): at most 2^dim * n_old leaves -- the call does not wait for the kernel: the leaf
+  // count and the buffer the result ends in stay on the device until a later call fetches them.
+  if (!iters && t->front_ok && !t->parity_pending && t->opt_debug_slack == 0 && !t->opt_full_sweeps &&
+      (t->opt_balance_conn <= 1) && t->have_old && t->cap >= (int64_t)(1 << t->g.dim) * t->n_old) {
+    tic(t, 1);
+    t->front_ok = false;
+    if ((rc = launch_balance(t, t->cap, 1)) != LT_OK) return rc;
+    t->parity_pending = true;
+    t->n_valid = false;
+    t->n_upper = (int64_t)(1 << t->g.dim) * t->n_old;
+    t->balanced_conn = 1;
+    t->map_valid = false;
+    t->map_ready = true;   // k_transfer reports a mapping error found by the kernel's tail (map_bad)
+    t->faces_valid = false;
+    toc(t, 1);
+    return LT_OK;
+  }
   if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
   tic(t, 1);
   const bool had_front = t->front_ok;  // consumed by this call whatever happens
@@ -633,7 +697,12 @@ int lt_balance(lt_tree* t, int* iters) {
     total_iters += t->h_s->iters;
     const int st = take_status(t);
     if (st == LT_OK) break;
-    if (st != LT_ERR_CAPACITY || attempt >= 40) return st;
+    // (an interrupted kernel leaves marks and per-chunk counters behind)
+    LT_CUDA(cudaMemsetAsync(t->d_cmarks, 0, 2 * kMaxGrid * sizeof(int), t->stream));
+    if (st != LT_ERR_CAPACITY || attempt >= 40) {
+      cudaMemsetAsync(t->mark, 0, (size_t)t->cap, t->stream);
+      return st;
+    }
     // the analogue of the paper's "perform the balance algorithm again" when the
     // allocated cap is exceeded: grow and continue from the valid,
     // partially balanced tree
@@ -645,6 +714,7 @@ int lt_balance(lt_tree* t, int* iters) {
     if ((rc = grow(t, t->cap * 2)) != LT_OK) return rc == LT_ERR_OOM ? LT_ERR_CAPACITY : rc;
   }
   if (iters) *iters = total_iters;
+  t->last_iters = total_iters;
   t->front_ok = false;
   t->balanced_conn = t->opt_balance_conn > 0 ? t->opt_balance_conn : 1;
   t->map_valid = false;
@@ -704,7 +774,7 @@ int lt_connect_begin(lt_tree* t) {
   if (!t) return LT_ERR_ARG;
   int rc;
   if ((rc = join_side(t)) != LT_OK) return rc;
-  if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
+  // (no wait for a pending leaf count / result buffer: k_connect reads both on the device)
   if (!t->s_side) {
     LT_CUDA(cudaStreamCreateWithFlags(&t->s_side, cudaStreamNonBlocking));
     LT_CUDA(cudaEventCreateWithFlags(&t->ev_side_fork, cudaEventDisableTiming));
@@ -717,7 +787,10 @@ int lt_connect_begin(lt_tree* t) {
   // 3 of the 8 resident blocks per SM: measured best on config 5 (1: the query outlasts the transfer,
   // 4+: the transfer loses more than the query gains); LT_SIDE_BLOCKS overrides for experiments
   static const int side_blocks = getenv("LT_SIDE_BLOCKS") ? atoi(getenv("LT_SIDE_BLOCKS")) : 3;
-  if ((rc = launch_connect(t, t->s_side, side_blocks)) != LT_OK) return rc;
+  // (a small mesh -- the transfer beside it takes well under a millisecond -- gets every block: there
+  // the query itself would become the critical path)
+  const int64_t n_est = t->n_valid ? t->n : (t->n_upper >> t->g.dim);  // (n_upper is the 2^dim-fold worst case)
+  if ((rc = launch_connect(t, t->s_side, n_est > (4 << 20) ? side_blocks : 0)) != LT_OK) return rc;
   cudaEventRecord(t->ev[13], t->s_side);
   t->ev_set[6] = true;
   t->ev_set[2] = false;  // the call has no duration of its own in this mode
@@ -774,7 +847,8 @@ int lt_transfer(lt_tree* t, const double* d_u_old, double* d_u_new, int p, int n
   // the kernels move x-pencils of an even number of doubles with 128-bit accesses
   if ((p + 1) % 2 == 0 && ((((uintptr_t)d_u_old) | ((uintptr_t)d_u_new)) & 15)) return LT_ERR_ARG;
   int rc;
-  if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
+  // (a leaf count still pending on the device is not needed here: the kernels read it there)
+  if (!t->map_ready && !t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
   if ((rc = build_operators(t, p)) != LT_OK) return rc;
   tic(t, 3);
   tic(t, 4);

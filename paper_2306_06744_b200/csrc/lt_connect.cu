@@ -110,7 +110,9 @@ __device__ __forceinline__ unsigned long long lookback_warp(volatile unsigned lo
 
 template <int DIM>
 __global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restrict__ keys,
-                                                const int* __restrict__ first, DevScalars* s,
+                                                const int* __restrict__ first,
+                                                const uint64_t* __restrict__ keys_alt,
+                                                const int* __restrict__ first_alt, DevScalars* s,
                                                 int32_t* __restrict__ nbr, uint8_t* __restrict__ kind,
                                                 int32_t* __restrict__ conf, uint8_t* __restrict__ conf_axis,
                                                 int32_t* __restrict__ hang, uint8_t* __restrict__ hang_info,
@@ -125,6 +127,12 @@ __global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restric
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int n = s->n;
   const int ntiles = (n + CT - 1) / CT;
+  // keys_alt != nullptr: the lt_balance before this query did not wait for its kernel, and the
+  // buffer its result ended in (DevScalars::parity) is only known here
+  if (keys_alt != nullptr && s->parity) {
+    keys = keys_alt;
+    first = first_alt;
+  }
   for (;;) {
     if (threadIdx.x == 0) s_tile = (int)atomicAdd(ticket, 1u);
     __syncthreads();
@@ -250,21 +258,26 @@ int launch_connect(Tree* t, cudaStream_t stream, int blocks_per_sm) {
   int32_t *conf, *hang, *bnd;
   uint8_t *conf_axis, *hang_info, *bnd_face;
   face_regions(t, &conf, &conf_axis, &hang, &hang_info, &bnd, &bnd_face);
-  const int64_t ntiles = (t->n + CT - 1) / CT;
+  // (leaf count still on the device: its upper bound sizes the look-back words to clear)
+  const int64_t ntiles = ((t->n_valid ? t->n : t->n_upper) + CT - 1) / CT;
   LT_CUDA(cudaMemsetAsync(t->tile_state, 0, (size_t)(ntiles + 1) * 2 * sizeof(unsigned long long), stream));
   LT_CUDA(cudaMemsetAsync(&t->d_s->ticket_c, 0, sizeof(unsigned), stream));
   const void* fn = t->g.dim == 2 ? (const void*)k_connect<2> : (const void*)k_connect<3>;
-  int per_sm = 0;
-  LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, CT, 0));
+  static int occ[2] = {0, 0};  // resident blocks per SM (the query costs microseconds of host time)
+  int& per_sm_cached = occ[t->g.dim - 2];
+  if (per_sm_cached == 0) LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_cached, fn, CT, 0));
+  int per_sm = per_sm_cached;
   if (per_sm < 1) per_sm = 1;
+  const uint64_t* keys_alt = t->parity_pending ? t->keys[t->tmp] : nullptr;
+  const int* first_alt = t->parity_pending ? t->first[t->tmp] : nullptr;
   if (blocks_per_sm > 0 && blocks_per_sm < per_sm) per_sm = blocks_per_sm;
   const int G = t->num_sms * per_sm;
   if (t->g.dim == 2)
-    k_connect<2><<<G, CT, 0, stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->nbr, t->kind, conf,
+    k_connect<2><<<G, CT, 0, stream>>>(t->g, t->keys[t->cur], t->first[t->cur], keys_alt, first_alt, t->d_s, t->nbr, t->kind, conf,
                                           conf_axis, hang, hang_info, bnd, bnd_face, t->tile_state,
                                           &t->d_s->ticket_c);
   else
-    k_connect<3><<<G, CT, 0, stream>>>(t->g, t->keys[t->cur], t->first[t->cur], t->d_s, t->nbr, t->kind, conf,
+    k_connect<3><<<G, CT, 0, stream>>>(t->g, t->keys[t->cur], t->first[t->cur], keys_alt, first_alt, t->d_s, t->nbr, t->kind, conf,
                                           conf_axis, hang, hang_info, bnd, bnd_face, t->tile_state,
                                           &t->d_s->ticket_c);
   t->launches++;

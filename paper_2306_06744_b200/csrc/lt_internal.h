@@ -47,6 +47,9 @@ struct Tree {
   int64_t n_old;
   int64_t n;              // host copy of the leaf count
   bool n_valid;
+  bool parity_pending;    // an lt_balance that did not wait: h_s->parity decides cur / tmp at the next fetch
+  int64_t n_upper;        // upper bound of the leaf count while !n_valid
+  int last_iters;         // sweeps of the last synchronous lt_balance (-1: read them from h_s)
 
   DevScalars* d_s;
   DevScalars* h_s;        // pinned mirror

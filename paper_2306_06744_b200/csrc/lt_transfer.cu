@@ -401,6 +401,11 @@ __global__ void __launch_bounds__(256, 4) k_transfer(const DevScalars* s,
   const int64_t n = je < 0 ? (int64_t)s->n : je;
   const int SL = 1 << sl_log2, TL = kSubs << sl_log2;
   const int64_t ntiles = (n - jb + TL - 1) / TL;
+  // the Alg. 7 tail of lt_balance met a new leaf more than one level from T_old: nothing to move
+  if (s->map_bad) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) set_status(const_cast<int*>(&s->status), LT_ERR_MAPPING);
+    return;
+  }
   if (threadIdx.x == 0) s_word = kSubs;
   __syncthreads();
   for (;;) {
@@ -999,6 +1004,7 @@ int launch_face_interp(Tree* t, const double* d_u, double* d_uf, int p, int nvar
 
 int launch_map(Tree* t) {
   int G = grid_for(t, 8);
+  LT_CUDA(cudaMemsetAsync(&t->d_s->map_bad, 0, sizeof(int), t->stream));  // (k_map reports through the status word)
   if (!t->have_old) {
     k_map_identity<<<G, 256, 0, t->stream>>>(t->d_s, t->map_src, t->map_kind);
   } else if (t->g.dim == 2) {
@@ -1022,10 +1028,12 @@ static int launch_transfer_t(Tree* t, const double* u_old, double* u_new, int nv
   while (warps > 1 && warps * per_warp > 96 * 1024) warps >>= 1;
   const size_t smem = warps * per_warp;
   auto fn = k_transfer<DIM, P1>;
-  LT_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  int per_sm = 0;
-  LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, warps * 32, smem));
-  if (per_sm < 1) per_sm = 1;
+  static int per_sm = 0;  // per instantiation: attribute and occupancy are queried once
+  if (per_sm == 0) {
+    LT_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, warps * 32, smem));
+    if (per_sm < 1) per_sm = 1;
+  }
   const int G = t->num_sms * per_sm;
   // sub-chunk = the power-of-two number of leaves closest below ~10 KB of solution, 1..32
   const size_t Bu = (size_t)nvars * X::N * sizeof(double);

@@ -168,7 +168,10 @@ __global__ void __launch_bounds__(BT) k_adapt_count(Geo g, const uint64_t* __res
   const int64_t n = s->n;
   // pass 2 overwrites s->n with the new count while its later blocks are still starting: they read the
   // count of the tree they work on from this snapshot
-  if (blockIdx.x == 0 && threadIdx.x == 0) s->n_in = (int)n;
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    s->n_in = (int)n;
+    s->nfront[0] = 0;  // pass 2 appends lt_balance's first frontier
+  }
   int64_t lo, hi;
   block_chunk(n, gridDim.x, blockIdx.x, BT, &lo, &hi);
   unsigned long long acc = 0;
@@ -493,6 +496,76 @@ __device__ __forceinline__ bool frontier_push(bool pred, uint64_t key, int tag, 
   return fits;
 }
 
+// The split pass of one sweep for the chunk [lo, hi) of a block: marked leaves are replaced by their
+// children (order-preserving), the bucket index is rebuilt and the next frontier is appended to.  Kept
+// out of line so that its registers (kScanTiles keys and marks per thread) do not weigh on the search
+// loops of the examination phases.  Returns false if the frontier buffer overflowed.
+template <int DIM>
+__device__ __noinline__ bool split_pass(const Geo& g, const uint64_t* __restrict__ keys, uint8_t* mark, int64_t lo,
+                                        int64_t hi, int64_t run, uint64_t* __restrict__ out,
+                                        int* __restrict__ first_out, bool emit, uint64_t* fk_out, uint8_t* ft_out,
+                                        int* fcount, int64_t fcap, unsigned long long* sm) {
+  constexpr int NC = Dim<DIM>::NC;
+  bool fits = true;
+  // kScanTiles tiles of BT leaves share one block scan: the counts (<= NC * BT < 2^16 per tile) are
+  // packed in 16-bit fields, and the loads of all tiles are issued before the first barrier (requesting
+  // the NEXT group's loads as well before the barriers was tried: slower, 0.34 -> 0.40-0.43 ms for the
+  // three splitting sweeps of config-5 cycle 3, because of the registers it takes)
+  for (int64_t t0 = lo; t0 < hi; t0 += kScanTiles * BT) {
+    uint64_t key[kScanTiles];
+    unsigned mk[kScanTiles];
+    unsigned long long packed = 0;
+#pragma unroll
+    for (int q = 0; q < kScanTiles; ++q) {
+      const int64_t i = t0 + q * BT + threadIdx.x;
+      key[q] = 0;
+      mk[q] = 0;
+      if (i < hi) {
+        key[q] = keys[i];
+        mk[q] = mark[i];
+      }
+    }
+#pragma unroll
+    for (int q = 0; q < kScanTiles; ++q) {
+      const int64_t i = t0 + q * BT + threadIdx.x;
+      if (i < hi) {
+        if (mk[q]) mark[i] = 0;
+        packed |= (unsigned long long)((mk[q] & 1) ? NC : 1) << (16 * q);
+      }
+    }
+    unsigned long long tile_total;
+    const unsigned long long ex = block_excl_scan<unsigned long long>(packed, sm, &tile_total);
+#pragma unroll
+    for (int q = 0; q < kScanTiles; ++q) {
+      const int64_t i = t0 + q * BT + threadIdx.x;
+      const int64_t pos = run + (int64_t)((ex >> (16 * q)) & 0xffff);
+      run += (int64_t)((tile_total >> (16 * q)) & 0xffff);
+      if (emit) {
+        // a split leaf becomes a GROUP entry; an unsplit leaf that saw a neighbour >= 3 levels coarser
+        // (full sweep) a LEAF entry
+        const bool pg = (mk[q] & 1) != 0, pl = !pg && (mk[q] & 2) != 0;
+        fits = frontier_push(pg || pl, key[q], pg ? kFrGroup : kFrLeaf, fk_out, ft_out, fcount, fcap) && fits;
+      }
+      if (i >= hi) continue;
+      const int l = key_level(key[q]);
+      const uint64_t m = key_morton(key[q]);
+      if (mk[q] & 1) {
+        const int sh = DIM * (g.maxl - l - 1);
+#pragma unroll
+        for (int k = 0; k < NC; ++k) {
+          const uint64_t mc = m | ((uint64_t)k << sh);
+          out[pos + k] = make_key(mc, l + 1);
+          index_write<DIM>(g, first_out, mc, l + 1, (int)(pos + k));
+        }
+      } else {
+        out[pos] = key[q];
+        index_write<DIM>(g, first_out, m, l, (int)pos);
+      }
+    }
+  }
+  return fits;
+}
+
 __device__ __forceinline__ unsigned long long global_ns() {
   unsigned long long t;
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
@@ -500,7 +573,7 @@ __device__ __forceinline__ unsigned long long global_ns() {
 }
 
 template <int DIM>
-__global__ void __launch_bounds__(BT) k_balance(BalanceArgs a) {
+__global__ void __launch_bounds__(BT, 4) k_balance(BalanceArgs a) {
   constexpr int NC = Dim<DIM>::NC;
   __shared__ unsigned long long sm[33];
   __shared__ uint8_t s_dirs[20], s_gdirs[26];
@@ -519,6 +592,7 @@ __global__ void __launch_bounds__(BT) k_balance(BalanceArgs a) {
   if (nfront > a.fcap) nfront = -1;                           // lt_adapt's list did not fit
   int64_t splits = 0;
   int err = 0;
+  if (gtid == 0) a.s->map_bad = 0;  // (set again only by the Alg. 7 tail, many barriers later)
   // thread (0, 0) leaves every grid-wide barrier after all blocks have arrived, so its clock
   // readings bound the phases of the whole grid (lt_balance_phases)
   unsigned long long ns[4] = {0, 0, 0, 0}, t_prev = gtid == 0 ? global_ns() : 0;
@@ -595,64 +669,8 @@ __global__ void __launch_bounds__(BT) k_balance(BalanceArgs a) {
     uint8_t* ft_out = a.ftag[fpar ^ 1];
     int* fcount = &a.s->nfront[fpar ^ 1];
     const bool emit = !a.full_sweeps;
-    bool fits = true;
-    int64_t run = before;
-    // kScanTiles tiles of BT leaves share one block scan: the counts (<= NC * BT < 2^16 per tile) are
-    // packed in 16-bit fields, and the loads of all tiles are issued before the first barrier (requesting
-    // the NEXT group's loads as well before the barriers was tried: slower, 0.34 -> 0.40-0.43 ms for the
-    // three splitting sweeps of config-5 cycle 3, because of the registers it takes)
-    for (int64_t t0 = lo; t0 < hi; t0 += kScanTiles * BT) {
-      uint64_t key[kScanTiles];
-      unsigned mk[kScanTiles];
-      unsigned long long packed = 0;
-#pragma unroll
-      for (int q = 0; q < kScanTiles; ++q) {
-        const int64_t i = t0 + q * BT + threadIdx.x;
-        key[q] = 0;
-        mk[q] = 0;
-        if (i < hi) {
-          key[q] = keys[i];
-          mk[q] = a.mark[i];
-        }
-      }
-#pragma unroll
-      for (int q = 0; q < kScanTiles; ++q) {
-        const int64_t i = t0 + q * BT + threadIdx.x;
-        if (i < hi) {
-          if (mk[q]) a.mark[i] = 0;
-          packed |= (unsigned long long)((mk[q] & 1) ? NC : 1) << (16 * q);
-        }
-      }
-      unsigned long long tile_total;
-      const unsigned long long ex = block_excl_scan<unsigned long long>(packed, sm, &tile_total);
-#pragma unroll
-      for (int q = 0; q < kScanTiles; ++q) {
-        const int64_t i = t0 + q * BT + threadIdx.x;
-        const int64_t pos = run + (int64_t)((ex >> (16 * q)) & 0xffff);
-        run += (int64_t)((tile_total >> (16 * q)) & 0xffff);
-        if (emit) {
-          // a split leaf becomes a GROUP entry; an unsplit leaf that saw a neighbour >= 3 levels coarser
-          // (full sweep) a LEAF entry
-          const bool pg = (mk[q] & 1) != 0, pl = !pg && (mk[q] & 2) != 0;
-          fits = frontier_push(pg || pl, key[q], pg ? kFrGroup : kFrLeaf, fk_out, ft_out, fcount, a.fcap) && fits;
-        }
-        if (i >= hi) continue;
-        const int l = key_level(key[q]);
-        const uint64_t m = key_morton(key[q]);
-        if (mk[q] & 1) {
-          const int sh = DIM * (g.maxl - l - 1);
-#pragma unroll
-          for (int k = 0; k < NC; ++k) {
-            const uint64_t mc = m | ((uint64_t)k << sh);
-            out[pos + k] = make_key(mc, l + 1);
-            index_write<DIM>(g, first_out, mc, l + 1, (int)(pos + k));
-          }
-        } else {
-          out[pos] = key[q];
-          index_write<DIM>(g, first_out, m, l, (int)pos);
-        }
-      }
-    }
+    const int64_t run = before;
+    bool fits = split_pass<DIM>(g, keys, a.mark, lo, hi, run, out, first_out, emit, fk_out, ft_out, fcount, a.fcap, sm);
     // entries flagged for another examination move on to the next frontier
     if (emit && nfront >= 0) {
       const uint64_t* fk = a.fkey[fpar];
@@ -814,14 +832,15 @@ int launch_balance(Tree* t, int64_t cap_told, int use_front) {
   a.map_src = t->map_src;
   a.map_kind = t->map_kind;
   void* fn = t->g.dim == 2 ? (void*)k_balance<2> : (void*)k_balance<3>;
-  int per_sm = 0;
-  LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, BT, 0));
+  static int occ[2] = {0, 0};
+  int& per_sm = occ[t->g.dim - 2];
+  if (per_sm == 0) LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, BT, 0));
   if (per_sm < 1) return LT_ERR_CUDA;
   int G = t->num_sms * per_sm;
   if (G > kMaxGrid) G = kMaxGrid;
-  // marks-per-chunk counters of both sweep parities; map_bad (the words sit next to each other)
-  LT_CUDA(cudaMemsetAsync(t->d_cmarks, 0, 2 * kMaxGrid * sizeof(int), t->stream));
-  LT_CUDA(cudaMemsetAsync(&t->d_s->map_bad, 0, sizeof(int), t->stream));
+  // The marks-per-chunk counters of both sweep parities are zero on entry: zeroed when allocated, and a
+  // kernel that ends without error leaves them zero (its last sweep marked nothing, the other half was
+  // cleared at that sweep's start); lt_balance clears them before it retries after LT_ERR_CAPACITY.
   void* args[] = {&a};
   LT_CUDA(cudaLaunchCooperativeKernel(fn, dim3(G), dim3(BT), args, 0, t->stream));
   t->launches++;

@@ -63,6 +63,7 @@ SIGNATURES = {
     "lt_mortar_gather": (_I, [_P, _P, _P, _I, _I]),
     "lt_num_leaves": (_I64, [_P]),
     "lt_num_old_leaves": (_I64, [_P]),
+    "lt_last_balance_iters": (_I, [_P]),
     "lt_keys": (_P, [_P]),
     "lt_old_keys": (_P, [_P]),
     "lt_map": (_I, [_P, C.POINTER(_P), C.POINTER(_P)]),
@@ -194,14 +195,32 @@ class Tree:
             raise ValueError("lt_adapt: flags must have one entry per leaf")
         _check(lib().lt_adapt(self._h, _dptr(flags, torch.int8, "flags")), "lt_adapt")
 
-    def balance(self, connectivity=None) -> int:
+    def balance(self, connectivity=None, want_iters=True):
         """lt_balance; connectivity (sticky option LT_OPT_BALANCE_CONNECTIVITY): 1 faces,
-        2 + edges (the paper's strong balance in 3-D), 3 + corners."""
+        2 + edges (the paper's strong balance in 3-D), 3 + corners.  want_iters=False passes
+        iters = NULL, which lets the call return without waiting (see lt.h); last_balance_iters()
+        gives the sweep count afterwards."""
         if connectivity is not None:
             self.set_option(LT_OPT_BALANCE_CONNECTIVITY, int(connectivity))
+        if not want_iters:
+            _check(lib().lt_balance(self._h, None), "lt_balance")
+            return None
         it = C.c_int(0)
         _check(lib().lt_balance(self._h, C.byref(it)), "lt_balance")
         return it.value
+
+    def last_balance_iters(self) -> int:
+        it = lib().lt_last_balance_iters(self._h)
+        if it < 0:
+            raise LtError(int(it), "lt_last_balance_iters")
+        return int(it)
+
+    def transfer_into(self, u_old: torch.Tensor, u_new: torch.Tensor, p: int, nvars: int):
+        """lt_transfer into a caller-sized buffer (>= num_leaves rows) without asking for the leaf count,
+        so that the call does not wait for a pending lt_adapt / lt_balance."""
+        _check(lib().lt_transfer(self._h, _dptr(u_old, torch.float64, "u_old"), _dptr(u_new, torch.float64, "u_new"),
+                                 p, nvars), "lt_transfer")
+        return u_new
 
     def connect(self) -> dict:
         """lt_connect: dict of zero-copy views (valid until the next mutating call)."""

@@ -372,3 +372,68 @@ def test_balance_after_adapt_uses_the_adapt_frontier(dim, base, maxl, periodic):
             f2 = rng.choice(np.array([-1, 0, 1], np.int8), size=ot.num_leaves(), p=[0.2, 0.5, 0.3])
             ot.adapt(f2); ot.drop_snapshot()
             gt.adapt(torch.from_numpy(f2).cuda()); gf.adapt(torch.from_numpy(f2).cuda())
+
+
+# ---------------------------------------------------------------- the one-synchronisation cycle
+@pytest.mark.parametrize("name,ncyc", [("c1", 4), ("c2", 9), ("c3b", 12), ("c4", 3), ("slab", 8)])
+def test_cycle_with_one_host_synchronisation(name, ncyc):
+    """With buffers reserved for the worst case (2^dim * leaves) lt_adapt and lt_balance(iters = NULL)
+    only enqueue: the leaf count and the buffer the balanced tree ends in stay on the device,
+    lt_connect_begin / lt_transfer read them there, and lt_connect_end is the only call that makes the
+    host wait.  Same results as the synchronous calls, bit for bit, against the oracle."""
+    cfg = W.CONFIGS[name]
+    gt, ot = P.new_pair(cfg)
+    p, nvars = cfg["p"], cfg["nvars"]
+    N = (p + 1) ** cfg["dim"]
+    uo = P.initial_u(cfg, ot)
+    cap = 1 << 14
+    for c in range(ncyc):
+        while cap < (8 << cfg["dim"]) * ot.num_leaves():
+            cap *= 4
+        gt.reserve(cap)
+        f = P.host_flags(cfg, c, ot)
+        d_f = torch.from_numpy(f).cuda()
+        d_uo = torch.from_numpy(uo).cuda()
+        d_un = torch.empty((cap, nvars, N), dtype=torch.float64, device="cuda")
+        torch.cuda.synchronize()
+        s0 = gt.host_syncs()
+        gt.adapt(d_f)
+        gt.balance(want_iters=False)
+        gt.connect_begin()
+        gt.transfer_into(d_uo, d_un, p, nvars)
+        Fg = gt.connect_end()
+        assert gt.host_syncs() - s0 == 1, "cycle %d: %d host synchronisations" % (c, gt.host_syncs() - s0)
+        ot.adapt(f)
+        it_o = ot.balance()
+        assert gt.last_balance_iters() == it_o
+        P.assert_keys_equal(gt, ot, "cycle %d" % c)
+        P.assert_faces_equal(Fg, ot.connect(), "cycle %d faces" % c)
+        src_o, kind_o = ot.build_map()
+        un_o = ot.transfer_rows(uo, p, nvars, 0, ot.num_leaves())
+        ot.drop_snapshot()
+        gt.sync()
+        src_g, kind_g = gt.map()
+        assert np.array_equal(src_g.cpu().numpy(), src_o) and np.array_equal(kind_g.cpu().numpy(), kind_o)
+        P.assert_u_close(d_un[:ot.num_leaves()], un_o, "cycle %d transfer" % c)
+        uo = un_o
+
+
+def test_deferred_balance_reports_a_mapping_error_through_the_status():
+    """Two adapts, then a balance that does not wait: the Alg. 7 tail finds leaves two levels from the
+    snapshot; lt_transfer moves nothing and lt_sync returns LT_ERR_MAPPING."""
+    cfg = W.CONFIGS["c3b"]
+    gt, ot = P.new_pair(cfg)
+    gt.reserve(1 << 16)
+    for c in range(9):
+        f = P.host_flags(cfg, c, ot)
+        ot.adapt(f)
+        gt.adapt(torch.from_numpy(f).cuda())
+    # (the tree entering the last lt_adapt was not balanced, so this lt_balance takes the waiting path;
+    # its tail still leaves the map to lt_transfer's checked k_map)
+    gt.balance(want_iters=False)
+    u = torch.zeros((gt.num_old_leaves(), 5, 8), dtype=torch.float64, device="cuda")
+    gt.transfer(u, 1, 5)
+    with pytest.raises(lt.LtError) as ei:
+        gt.sync()
+    assert ei.value.status == lt.LT_ERR_MAPPING
+    assert gt.num_leaves() == 932
