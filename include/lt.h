@@ -339,6 +339,10 @@ int lt_balance_phases(lt_tree*, float* out4);
 const char* lt_strerror(int status);
 int lt_last_cuda_error(void); /* cudaError_t of the last failing runtime call (this thread) */
 int lt_version(void);
+/* 1 in the checked build (liblt_debug.so, compiled with -DLT_DEBUG: device-side assertions on every
+ * located index, table write position, ticket and look-back word; a failing one traps the kernel and the
+ * next synchronising call returns LT_ERR_CUDA), 0 in the release build. */
+int lt_debug_build(void);
 
 #ifdef __cplusplus
 }

@@ -358,7 +358,14 @@ static int join_side(Tree* t) {
 
 extern "C" {
 
-int lt_version(void) { return 100; }
+int lt_version(void) { return 200; }
+int lt_debug_build(void) {
+#ifdef LT_DEBUG
+  return 1;
+#else
+  return 0;
+#endif
+}
 int lt_last_cuda_error(void) { return g_last_cuda_error; }
 
 const char* lt_strerror(int status) {

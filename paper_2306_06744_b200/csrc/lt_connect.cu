@@ -39,6 +39,7 @@ __device__ __forceinline__ int face_by_search(const Geo& g, const uint64_t* __re
   uint64_t mn;
   if (!face_neighbour<DIM>(g, m, l, f, &mn)) return 0;  // domain boundary
   const int j = locate(g, keys, first, mn);
+  LT_DASSERT(j >= 0 && j < first[g.nbuckets]);
   const int lj = key_level(keys[j]);
   if (lj == l) {  // Eq. 7 case 1: the search key is in the tree -> conforming
     *nb_out = j;
@@ -95,6 +96,7 @@ __device__ __forceinline__ unsigned long long lookback_warp(volatile unsigned lo
     unsigned long long v = kFlagInc;  // before tile 0: an inclusive prefix of zero
     if (idx >= 0) {
       do { v = st[2 * (size_t)idx + ch]; } while ((v >> 62) == 0);
+      LT_DASSERT((v >> 62) <= 2);  // look-back protocol: 0 not ready, 1 own counts, 2 inclusive prefix
     }
     const unsigned inc = __ballot_sync(0xffffffffu, (v >> 62) == 2);
     const int stop = inc ? __ffs(inc) - 1 : 31;  // nearest predecessor that is already inclusive
@@ -137,6 +139,7 @@ __global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restric
     if (threadIdx.x == 0) s_tile = (int)atomicAdd(ticket, 1u);
     __syncthreads();
     const int tile = s_tile;
+    LT_DASSERT(tile >= 0 && tile < ntiles + (int)gridDim.x);  // every block draws one ticket past the end
     if (tile >= ntiles) break;
     const int e0 = tile * CT;
     const int ne = min(CT, n - e0);
@@ -214,6 +217,9 @@ __global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restric
     // ---- emit (leaf order, local faces 0..NF-1: reading D-4)
     if ((int)threadIdx.x < ne) {
       const int e = e0 + threadIdx.x;
+      // the rows of the leaves before e: at most DIM conforming, DIM hanging and NF boundary rows each
+      LT_DASSERT(p_conf >= 0 && p_conf <= (int64_t)DIM * e && p_hang >= 0 && p_hang <= (int64_t)DIM * e &&
+                 p_bnd >= 0 && p_bnd <= (int64_t)NF * e);
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
         const int kd = s_kd[threadIdx.x * NF + f];

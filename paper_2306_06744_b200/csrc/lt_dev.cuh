@@ -11,6 +11,18 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+// -DLT_DEBUG (python -m paper_2306_06744_b200.build --debug -> liblt_debug.so): device-side checks of
+// every located index, table write position, ticket and look-back word.  A failing check traps the
+// kernel (the next synchronising call returns LT_ERR_CUDA and the assertion text goes to stderr).
+// compute-sanitizer is not available on the GPU pool this library is developed on; this build and the
+// small cases of tests/test_gpu_debug_build.py stand in for it.
+#ifdef LT_DEBUG
+#include <assert.h>
+#define LT_DASSERT(cond) assert(cond)
+#else
+#define LT_DASSERT(cond) ((void)0)
+#endif
+
 namespace lt {
 
 constexpr int kLevelBits = 5;
@@ -164,18 +176,25 @@ __device__ __forceinline__ bool face_neighbour(const Geo& g, uint64_t m, int l, 
 __device__ __forceinline__ int locate(const Geo& g, const uint64_t* __restrict__ keys,
                                       const int* __restrict__ first, uint64_t mn) {
   const uint32_t b = (uint32_t)(mn >> g.ishift);
+  LT_DASSERT(b < (uint32_t)g.nbuckets);
   int lo = first[b], hi = first[b + 1];
+  LT_DASSERT(lo >= 0 && lo <= hi && hi <= first[g.nbuckets]);
   const uint64_t bound = (mn << kLevelBits) | kLevelMask;  // keys <= bound  <=>  morton <= mn
   while (hi - lo > 1) {
     int mid = (lo + hi) >> 1;
     if (keys[mid] <= bound) lo = mid; else hi = mid;
   }
+  // the located leaf starts at or before the point and ends after it (the leaves tile the domain)
+  LT_DASSERT(lo < first[g.nbuckets] && keys[lo] <= bound);
+  LT_DASSERT((mn >> (g.dim * (g.maxl - key_level(keys[lo])))) ==
+             (key_morton(keys[lo]) >> (g.dim * (g.maxl - key_level(keys[lo])))));
   return lo;
 }
 
 // Record the leaf (m, l) stored at position `pos` in the bucket index (see locate()).
 template <int DIM>
 __device__ __forceinline__ void index_write(const Geo& g, int* __restrict__ first, uint64_t m, int l, int pos) {
+  LT_DASSERT(pos >= 0 && (m >> g.ishift) < (uint64_t)g.nbuckets);
   if (l >= g.ilevel) {
     if ((m & ((1ull << g.ishift) - 1)) == 0) first[m >> g.ishift] = pos;
   } else {

@@ -132,6 +132,7 @@ __global__ void __launch_bounds__(ST) k_sort_pass(const uint64_t* __restrict__ i
         for (int j = 0; j < LB; ++j) {
           if (done) break;
           while ((v[j] >> 30) == 0) v[j] = ld_status(status + (size_t)(t - j) * 256 + d);
+          LT_DASSERT((v[j] >> 30) <= 2);  // look-back protocol: 0 not ready, 1 tile aggregate, 2 inclusive prefix
           excl += v[j] & VAL_MASK;
           if ((v[j] >> 30) == 2) done = true;
         }
@@ -152,7 +153,10 @@ __global__ void __launch_bounds__(ST) k_sort_pass(const uint64_t* __restrict__ i
   // store per key, 25 sectors per request in the first version)
 #pragma unroll
   for (int k = 0; k < SITEMS; ++k)
-    if (dig[k] < 256) s_keys[loff[dig[k]] + wcnt[w * 256 + dig[k]] + rank[k]] = key[k];
+    if (dig[k] < 256) {
+      LT_DASSERT(loff[dig[k]] + wcnt[w * 256 + dig[k]] + rank[k] < (unsigned)STILE);
+      s_keys[loff[dig[k]] + wcnt[w * 256 + dig[k]] + rank[k]] = key[k];
+    }
   __syncthreads();
   const int nt = (int)s_ntile;
 #pragma unroll
@@ -160,6 +164,7 @@ __global__ void __launch_bounds__(ST) k_sort_pass(const uint64_t* __restrict__ i
     const int i = k * ST + threadIdx.x;
     if (i < nt) {
       const uint64_t kk = s_keys[i];
+      LT_DASSERT((int64_t)gbase[(int)((kk >> shift) & 255)] + i < n);
       out[(size_t)gbase[(int)((kk >> shift) & 255)] + i] = kk;
     }
   }

@@ -446,6 +446,7 @@ __global__ void __launch_bounds__(256, 4) k_transfer(const DevScalars* s,
     if (lane < SL && j0 + lane < n) {
       kd = map_kind[j0 + lane];
       so = map_src[j0 + lane];
+      LT_DASSERT(so >= 0 && ((kd & 15) == 0 || (kd & 15) == 1 || kd == 2) && (kd >> 4) < X::NC);
     }
     const bool is_copy = kd == 0;
     const int so_prev = __shfl_up_sync(0xffffffffu, so, 1);

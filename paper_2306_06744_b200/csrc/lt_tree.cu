@@ -252,6 +252,7 @@ __global__ void __launch_bounds__(BT) k_adapt_scatter(Geo g, const uint64_t* __r
         }
       }
       if (act == ACT_DROP) continue;
+      LT_DASSERT(pos >= 0 && pos + (act == ACT_REFINE ? NC : 1) <= n_out);
       const int l = key_level(key);
       const uint64_t m = key_morton(key);
       if (act == ACT_KEEP) {
@@ -428,6 +429,7 @@ __device__ __forceinline__ int examine_leaf(const Geo& g, const uint64_t* __rest
   const int j = locate(g, keys, first, mn);
   const int lj = key_level(keys[j]);
   if (lj >= l - 1) return 0;
+  LT_DASSERT(lj >= g.base);
   mark_split(mark, cmarks, per, j);
   return lj < l - 2 ? 2 : 1;
 }
@@ -489,6 +491,7 @@ __device__ __forceinline__ bool frontier_push(bool pred, uint64_t key, int tag, 
   base = __shfl_sync(0xffffffffu, base, __ffs(m) - 1);
   const int64_t at = (int64_t)base + __popc(m & ((1u << lane) - 1));
   const bool fits = (int64_t)base + __popc(m) <= fcap;
+  LT_DASSERT(base >= 0 && at >= 0);
   if (pred && fits) {
     fkey[at] = key;
     ftag[at] = (uint8_t)tag;
@@ -504,9 +507,10 @@ template <int DIM>
 __device__ __noinline__ bool split_pass(const Geo& g, const uint64_t* __restrict__ keys, uint8_t* mark, int64_t lo,
                                         int64_t hi, int64_t run, uint64_t* __restrict__ out,
                                         int* __restrict__ first_out, bool emit, uint64_t* fk_out, uint8_t* ft_out,
-                                        int* fcount, int64_t fcap, unsigned long long* sm) {
+                                        int* fcount, int64_t fcap, unsigned long long* sm, int64_t n_new) {
   constexpr int NC = Dim<DIM>::NC;
   bool fits = true;
+  (void)n_new;
   // kScanTiles tiles of BT leaves share one block scan: the counts (<= NC * BT < 2^16 per tile) are
   // packed in 16-bit fields, and the loads of all tiles are issued before the first barrier (requesting
   // the NEXT group's loads as well before the barriers was tried: slower, 0.34 -> 0.40-0.43 ms for the
@@ -547,8 +551,10 @@ __device__ __noinline__ bool split_pass(const Geo& g, const uint64_t* __restrict
         fits = frontier_push(pg || pl, key[q], pg ? kFrGroup : kFrLeaf, fk_out, ft_out, fcount, fcap) && fits;
       }
       if (i >= hi) continue;
+      LT_DASSERT(pos >= 0 && pos + ((mk[q] & 1) ? NC : 1) <= n_new);
       const int l = key_level(key[q]);
       const uint64_t m = key_morton(key[q]);
+      LT_DASSERT(!(mk[q] & 1) || l < g.maxl);  // a leaf at the finest level is never too coarse
       if (mk[q] & 1) {
         const int sh = DIM * (g.maxl - l - 1);
 #pragma unroll
@@ -670,7 +676,7 @@ __global__ void __launch_bounds__(BT, 4) k_balance(BalanceArgs a) {
     int* fcount = &a.s->nfront[fpar ^ 1];
     const bool emit = !a.full_sweeps;
     const int64_t run = before;
-    bool fits = split_pass<DIM>(g, keys, a.mark, lo, hi, run, out, first_out, emit, fk_out, ft_out, fcount, a.fcap, sm);
+    bool fits = split_pass<DIM>(g, keys, a.mark, lo, hi, run, out, first_out, emit, fk_out, ft_out, fcount, a.fcap, sm, n_new);
     // entries flagged for another examination move on to the next frontier
     if (emit && nfront >= 0) {
       const uint64_t* fk = a.fkey[fpar];

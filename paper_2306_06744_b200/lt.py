@@ -15,7 +15,8 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "liblt.so")
+# LT_DEBUG_LIB=1 loads the checked build (python -m paper_2306_06744_b200.build --debug)
+LIB_PATH = os.path.join(_HERE, "liblt_debug.so" if os.environ.get("LT_DEBUG_LIB") == "1" else "liblt.so")
 _lib = None
 
 LT_OK, LT_ERR_ARG, LT_ERR_CUDA, LT_ERR_OOM, LT_ERR_CAPACITY = 0, -1, -2, -3, -4
@@ -84,6 +85,7 @@ SIGNATURES = {
     "lt_strerror": (C.c_char_p, [_I]),
     "lt_last_cuda_error": (_I, []),
     "lt_version": (_I, []),
+    "lt_debug_build": (_I, []),
 }
 
 
