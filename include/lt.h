@@ -233,6 +233,7 @@ int lt_transfer_host(lt_tree*, const double* h_u_old, double* h_u_new, int p, in
  * mortars, which makes the result deterministic.  A missing fine neighbour sets the sticky
  * status LT_ERR_UNBALANCED (reported by lt_sync). */
 int lt_mortar_project(lt_tree*, const double* d_u_face, double* d_u_nb, int p, int nvars);
+int lt_mortar_gather(lt_tree*, const double* d_f_mortar, double* d_f_face, int p, int nvars);
 
 /* Alg. 8 step 1: the solution at the face flux points,
  *   d_u_face[e][f][v][n_t] = sum_i l_i(-1 | +1) d_u[e][v][.. i on the face's axis ..],
@@ -240,7 +241,6 @@ int lt_mortar_project(lt_tree*, const double* d_u_face, double* d_u_nb, int p, i
  * above; l_i = the Lagrange basis on the Gauss-Legendre solution points.  Needs no connectivity.
  * The arrays must not overlap.  Asynchronous. */
 int lt_face_interp(lt_tree*, const double* d_u, double* d_u_face, int p, int nvars);
-int lt_mortar_gather(lt_tree*, const double* d_f_mortar, double* d_f_face, int p, int nvars);
 
 /* ---- the flux-reconstruction update around the cycle (Eq. 1-6; Alg. 8 step 3) ---
  * Compressible Euler equations, conserved variables (rho, rho u, rho v[, rho w], E), nvars = dim + 2,
@@ -308,8 +308,7 @@ int lt_sync(lt_tree*);
 typedef enum {
   LT_OPT_ADAPT_SORT = 1, /* 0 (default): ordered expansion; 1: append + sort + linearise */
   LT_OPT_BALANCE_FULL_SWEEPS = 2, /* 1: every sweep examines every leaf (debug)         */
-  LT_OPT_DEBUG_BALANCE_SLACK = 3, /* v > 0: lt_balance pretends its buffers hold only n + v
-                                     leaves, to exercise the LT_ERR_CAPACITY retry (tests) */
+  /* 3: reserved (a test hook of the library's own tests, see csrc/lt_internal.h) */
   LT_OPT_HOST_SLAB_LEAVES = 4,    /* v > 0: new leaves per slab of lt_transfer_host's copy /
                                      compute pipeline (default: about 128 MB of solution)   */
   LT_OPT_BALANCE_CONNECTIVITY = 5 /* which neighbours lt_balance keeps within one level:

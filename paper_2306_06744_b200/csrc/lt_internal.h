@@ -7,6 +7,10 @@
 #include "../../include/lt.h"
 #include "lt_dev.cuh"
 
+// Test hook, not part of the public enum lt_option (value 3 is reserved there): v > 0 makes lt_balance
+// pretend that its buffers hold only n + v leaves, to exercise the LT_ERR_CAPACITY retry.
+#define LT_OPT_DEBUG_BALANCE_SLACK 3
+
 namespace lt {
 
 // Device-resident scalars of a tree (one allocation).

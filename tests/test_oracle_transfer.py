@@ -91,7 +91,6 @@ def test_operator_identities(dim, p):
     z, w = np.polynomial.legendre.leggauss(p + 1)
     I1 = [one_d_interp(p, 0), one_d_interp(p, 1)]
     R1 = [0.5 * np.diag(1 / w) @ I1[b].T @ np.diag(w) for b in (0, 1)]  # reading E-4 closed form
-    wt = kron_op([w] * dim) if dim > 1 else w
     wt = w
     for _ in range(dim - 1):
         wt = np.kron(w, wt)
@@ -153,7 +152,7 @@ def sample_poly(cfg, coef, level, xyz):
             for a in range(dim):
                 term = term * pos[a] ** e[a]
             acc += term
-        out[v if False else slice(None), v, :] = acc
+        out[:, v, :] = acc
     return out
 
 
