@@ -969,14 +969,26 @@ def run_solver(args):
         fluxes_of(x)
         t.fr_rhs(x, fs, p, rhs=rhs)
 
-    def rk3_step():                                # lt_fr_stage: right-hand side + Eq. 6 in one pass
-        fluxes_of(u)
-        t.fr_stage(1, dt, u, u, fs, p, out=us)
-        fluxes_of(us)
-        t.fr_stage(2, dt, u, us, fs, p, out=us)
-        fluxes_of(us)
-        t.fr_stage(3, dt, u, us, fs, p, out=u)
+    fused = not args.unfused
 
+    def rk3_step():
+        if not fused:                              # round-1 chain: five passes per stage
+            fluxes_of(u)
+            t.fr_stage(1, dt, u, u, fs, p, out=us)
+            fluxes_of(us)
+            t.fr_stage(2, dt, u, us, fs, p, out=us)
+            fluxes_of(us)
+            t.fr_stage(3, dt, u, us, fs, p, out=u)
+            return
+        # three passes per stage: lt_face_flux (Alg. 8 steps 2 + 3, neighbour traces never stored),
+        # lt_mortar_gather, lt_fr_stage_faces (Eq. 2-6 + the traces of the result for the next stage);
+        # uf holds the traces of u on entry and on exit
+        for stage, (src, dst) in enumerate(((u, us), (us, us), (us, u)), start=1):
+            t.face_flux(uf, p, f_star=fs)
+            t.mortar_gather(fs, p, nvars, f_face=fs)
+            t.fr_stage_faces(stage, dt, u, src, fs, p, out=dst, u_face_out=uf)
+
+    t.face_interp(u, p, nvars, u_face=uf)
     rk3_step()                                     # warm-up
     ms_solve, _ = timed(lambda: [rk3_step() for _ in range(10)])
     ms_rhs, _ = timed(lambda: rhs_of(u))
@@ -990,7 +1002,7 @@ def run_solver(args):
     Bu, Bf = 8 * nvars * N, 8 * nvars * Nf
     # algorithmic bytes of one RK stage: face_interp (Bu + 6 Bf) + project (~2 * 6 Bf) + common flux (3 * 6 Bf)
     # + fused right-hand side and update (read u_stage, u_n and 6 Bf, write u_out: 3 Bu + 6 Bf)
-    bytes_stage = M * (4 * Bu + 6 * Bf * 7)
+    bytes_stage = M * (3 * Bu + 24 * Bf) if fused else M * (4 * Bu + 6 * Bf * 7)
     peak, peak_src = hbm_peak()
     print(json.dumps({
         "metric": "adaptation share of wall clock, one adaptation cycle per 10 SSP-RK3 steps (PAPER.md:449)",
@@ -1004,12 +1016,13 @@ def run_solver(args):
                                                         ", larger than L2" if M * Bu > (256 << 20) else
                                                         " (smaller than L2: the paper's own mesh size, launch-bound)")},
         "ms_per_call": {"adaptation_cycle": ms_adapt, "ten_rk3_steps": ms_solve, "one_rhs_chain": ms_rhs},
-        "roofline": {"bound": "hbm", "kernel": "RK stage (face_interp, mortar_project, common_flux, mortar_gather, "
-                                               "fr_stage)", "achieved": bytes_stage * 30 / (ms_solve * 1e-3) / 1e9,
+        "roofline": {"bound": "hbm", "kernel": "RK stage (face_flux, mortar_gather, fr_stage_faces)" if fused else
+                     "RK stage (face_interp, mortar_project, common_flux, mortar_gather, fr_stage)", "achieved": bytes_stage * 30 / (ms_solve * 1e-3) / 1e9,
                      "peak": peak, "unit": "GB/s", "frac": bytes_stage * 30 / (ms_solve * 1e-3) / 1e9 / peak,
                      "traffic": None, "peak_source": peak_src, "bytes_per_launch": bytes_stage},
         "elements_per_s_rhs": M * 30 / (ms_solve * 1e-3),
-        "cpu_baseline": None, "clocks": clocks, "gpu_launches": 30 * 6 + 6, "e2e": None}), flush=True)
+        "cpu_baseline": None, "clocks": clocks, "gpu_launches": (30 * 4 if fused else 30 * 6) + 6, "e2e": None}),
+        flush=True)
 
 def main():
     ap = argparse.ArgumentParser()
@@ -1024,6 +1037,8 @@ def main():
     ap.add_argument("--oracle-full", action="store_true",
                     help="cpu_baseline / --impl reference on the config's full sample (c1-c4: every cycle; c5: cycles "
                          "0-3 with the transfer timed on slabs) instead of the bounded default")
+    ap.add_argument("--unfused", action="store_true",
+                    help="--workload solver: the round-1 chain of five passes per RK stage instead of the three fused ones")
     ap.add_argument("--sync-calls", action="store_true",
                     help="small configs: keep the synchronising lt_adapt / lt_balance (the before of the "
                          "one-synchronisation cycle)")

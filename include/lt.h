@@ -262,11 +262,26 @@ int lt_face_interp(lt_tree*, const double* d_u, double* d_u_face, int p, int nva
  *   the right-hand side never goes to memory.  d_u_out may be d_u_stage or d_u_n.
  * All four are asynchronous. */
 int lt_common_flux(lt_tree*, const double* d_u_face, const double* d_u_nb, double* d_f_star, int p);
+/* lt_face_flux -- Alg. 8 steps 2 and 3 in ONE pass (= lt_mortar_project followed by lt_common_flux, the
+ *   neighbour traces never go to memory): d_f_star[e][f] on every kind 1 / kind 2 slot from the traces
+ *   d_u_face.  A conforming face is computed once, by the element on its minus side, and stored in both
+ *   elements' slots (both sides compute the same flux along +a).  Kind 0 / 3 slots are left untouched
+ *   (lt_mortar_gather fills kind 3).  The arrays must not overlap.  Needs lt_connect on the current
+ *   tree.  Asynchronous. */
+int lt_face_flux(lt_tree*, const double* d_u_face, double* d_f_star, int p);
 int lt_fr_rhs(lt_tree*, const double* d_u, const double* d_f_star, double* d_rhs, int p);
 int lt_rk3_stage(lt_tree*, int stage, double dt, const double* d_u_n, const double* d_u_stage,
                  const double* d_rhs, double* d_u_out, int p);
 int lt_fr_stage(lt_tree*, int stage, double dt, const double* d_u_n, const double* d_u_stage,
                 const double* d_f_star, double* d_u_out, int p);
+/* lt_fr_stage_faces -- lt_fr_stage that also writes the traces of d_u_out at the face points
+ *   (= lt_face_interp(d_u_out), Alg. 8 step 1 of the NEXT stage) while the element is still on chip;
+ *   d_u_face_out may be d_f_star (an element reads and writes only its own face slots).  With
+ *   lt_face_flux and lt_mortar_gather one RK stage is three passes:
+ *       lt_face_flux(u_face -> f_star); lt_mortar_gather(f_star, in place);
+ *       lt_fr_stage_faces(u_n, u_stage, f_star -> u_out, u_face). */
+int lt_fr_stage_faces(lt_tree*, int stage, double dt, const double* d_u_n, const double* d_u_stage,
+                      const double* d_f_star, double* d_u_out, double* d_u_face_out, int p);
 
 /* ---- accessors --------------------------------------------------------------------- */
 

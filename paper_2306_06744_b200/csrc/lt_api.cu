@@ -1107,6 +1107,17 @@ int lt_common_flux(lt_tree* t, const double* d_u_face, const double* d_u_nb, dou
   return rc;
 }
 
+int lt_face_flux(lt_tree* t, const double* d_u_face, double* d_f_star, int p) {
+  if (!t || !d_u_face || !d_f_star || d_u_face == d_f_star || p < 0 || p > 7) return LT_ERR_ARG;
+  if (!t->faces_valid) return LT_ERR_ARG;
+  int rc;
+  if ((rc = build_operators(t, p)) != LT_OK) return rc;
+  tic(t, 7);
+  rc = launch_face_flux(t, d_u_face, d_f_star, p);
+  toc(t, 7);
+  return rc;
+}
+
 int lt_fr_rhs(lt_tree* t, const double* d_u, const double* d_f_star, double* d_rhs, int p) {
   if (!t || !d_u || !d_f_star || !d_rhs || d_u == d_rhs || p < 0 || p > 7) return LT_ERR_ARG;
   int rc;
@@ -1128,6 +1139,21 @@ int lt_fr_stage(lt_tree* t, int stage, double dt, const double* d_u_n, const dou
   const double b = stage == 1 ? 1.0 : (stage == 2 ? 0.25 : 2.0 / 3.0);
   tic(t, 7);
   rc = launch_fr_rhs(t, d_u_stage, d_f_star, d_u_out, p, d_u_n, a, b, dt);
+  toc(t, 7);
+  return rc;
+}
+
+int lt_fr_stage_faces(lt_tree* t, int stage, double dt, const double* d_u_n, const double* d_u_stage,
+                      const double* d_f_star, double* d_u_out, double* d_u_face_out, int p) {
+  if (!t || !d_u_n || !d_u_stage || !d_f_star || !d_u_out || !d_u_face_out || stage < 1 || stage > 3 || p < 0 || p > 7)
+    return LT_ERR_ARG;
+  int rc;
+  if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
+  if ((rc = build_fr_operators(t, p)) != LT_OK) return rc;
+  const double a = stage == 1 ? 0.0 : (stage == 2 ? 0.75 : 1.0 / 3.0);
+  const double b = stage == 1 ? 1.0 : (stage == 2 ? 0.25 : 2.0 / 3.0);
+  tic(t, 7);
+  rc = launch_fr_rhs(t, d_u_stage, d_f_star, d_u_out, p, d_u_n, a, b, dt, d_u_face_out);
   toc(t, 7);
   return rc;
 }

@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "lt_internal.h"
+#include "lt_euler.cuh"
 
 namespace lt {
 
@@ -22,42 +23,6 @@ struct FrConst {
   double lm[8], lp[8], gl[8], gr[8];
 };
 __constant__ FrConst c_fr[8];
-
-constexpr double kGamma = 1.4;
-
-template <int DIM>
-__device__ __forceinline__ void euler_flux(int a, const double* u, double* F) {
-  const double rho = u[0], E = u[DIM + 1], ir = 1.0 / rho;
-  double v[DIM], q = 0.0;
-#pragma unroll
-  for (int b = 0; b < DIM; ++b) {
-    v[b] = u[1 + b] * ir;
-    q += v[b] * v[b];
-  }
-  const double pr = (kGamma - 1.0) * (E - 0.5 * rho * q);
-  double va = v[0];
-#pragma unroll
-  for (int b = 1; b < DIM; ++b)
-    if (b == a) va = v[b];
-  F[0] = rho * va;
-#pragma unroll
-  for (int b = 0; b < DIM; ++b) F[1 + b] = u[1 + b] * va + (b == a ? pr : 0.0);
-  F[DIM + 1] = (E + pr) * va;
-}
-
-template <int DIM>
-__device__ __forceinline__ double wave_speed(int a, const double* u) {
-  const double rho = u[0], E = u[DIM + 1], ir = 1.0 / rho;
-  double q = 0.0, va = 0.0;
-#pragma unroll
-  for (int b = 0; b < DIM; ++b) {
-    const double vb = u[1 + b] * ir;
-    q += vb * vb;
-    if (b == a) va = vb;
-  }
-  const double pr = (kGamma - 1.0) * (E - 0.5 * rho * q);
-  return fabs(va) + sqrt(kGamma * pr * ir);
-}
 
 // Alg. 8 step 3: one thread per (slot, face point).  Own trace on an odd face = minus side.
 template <int DIM>
@@ -94,11 +59,17 @@ __global__ void __launch_bounds__(256) k_common_flux(const DevScalars* s, const 
 // element live in shared memory; the common fluxes come from the element's own face slots.
 template <int DIM, int P1>
 __global__ void __launch_bounds__(256) k_fr_rhs(Geo g, const uint64_t* __restrict__ keys, const DevScalars* s,
-                                                const double* u, const double* __restrict__ fs, double* R,
+                                                const double* u, const double* fs, double* R,
                                                 double w0, double w1, double w2, const double* un, double ca,
-                                                double cb, double dt) {
+                                                double cb, double dt, double* uf_out) {
   // un == nullptr: R = right-hand side.  Otherwise the RK stage of Eq. 6 is applied on the fly:
   // R (= u_out) = ca * un + cb * (u + dt * rhs); u_out may be u or un (element-local access).
+  // uf_out != nullptr (stage mode only): the traces of u_out at the face points (Alg. 8 step 1 of the
+  // NEXT stage) are written as well, while u_out is still in shared memory; uf_out may be fs (an element
+  // reads and writes only its own face slots).
+  // (A layout with padded x-lines and 1 / rho, p stored once per point was tried: it removes the bank
+  // conflicts but needs 10.9 instead of 7.7 KB of shared memory per warp, i.e. 16 instead of 24 resident
+  // warps per SM, and the kernel is latency-bound: 35.6 instead of 25.2 ms per stage on 8.86 M elements.)
   constexpr int NF = Dim<DIM>::NF, NV = DIM + 2;
   constexpr int N = DIM == 2 ? P1 * P1 : P1 * P1 * P1, Nf = DIM == 2 ? P1 : P1 * P1, EV = NV * N;
   extern __shared__ double sm_all[];  // [warps][3][NV][N]: u | F | R
@@ -182,11 +153,48 @@ __global__ void __launch_bounds__(256) k_fr_rhs(Geo g, const uint64_t* __restric
 #pragma unroll
         for (int k = 0; k < KN; ++k) {
           const int i = lane + 32 * k;
-          if (i < EV) __stcs(dst + i, ca * pn[k] + cb * (su[i] + dt * sR[i]));
+          if (i < EV) {
+            const double o = ca * pn[k] + cb * (su[i] + dt * sR[i]);
+            __stcs(dst + i, o);
+            sF[i] = o;  // (kept for the traces below; sF is free after the last axis)
+          }
         }
       } else {
         const double* sn = un + (size_t)e * EV;
-        for (int i = lane; i < EV; i += 32) dst[i] = ca * sn[i] + cb * (su[i] + dt * sR[i]);
+        for (int i = lane; i < EV; i += 32) {
+          const double o = ca * sn[i] + cb * (su[i] + dt * sR[i]);
+          dst[i] = o;
+          sF[i] = o;
+        }
+      }
+      if (uf_out != nullptr) {
+        // Alg. 8 step 1 for the next stage: u_out at the face points, one lane per line, both end faces
+        __syncwarp();
+        constexpr int E = NV * Nf;
+        double* fd = uf_out + (size_t)e * NF * E;
+#pragma unroll
+        for (int a = 0; a < DIM; ++a) {
+          const int stride = a == 0 ? 1 : (a == 1 ? P1 : P1 * P1);
+          for (int ln = lane; ln < E; ln += 32) {
+            const int v = ln / Nf, nt = ln - v * Nf;
+            int first;
+            if (DIM == 2) {
+              first = a == 0 ? nt * P1 : nt;
+            } else {
+              const int n0 = nt % P1, n1 = nt / P1;
+              first = a == 0 ? n0 * P1 + n1 * P1 * P1 : (a == 1 ? n0 + n1 * P1 * P1 : n0 + n1 * P1);
+            }
+            double lo = 0.0, hi = 0.0;
+#pragma unroll
+            for (int i = 0; i < P1; ++i) {
+              const double x = sF[v * N + first + i * stride];
+              lo += c.lm[i] * x;
+              hi += c.lp[i] * x;
+            }
+            __stcs(fd + (2 * a) * E + ln, lo);
+            __stcs(fd + (2 * a + 1) * E + ln, hi);
+          }
+        }
       }
     }
   }
@@ -287,7 +295,7 @@ int launch_common_flux(Tree* t, const double* d_uf, const double* d_unb, double*
 
 template <int DIM, int P1>
 static int launch_fr_rhs_t(Tree* t, const double* d_u, const double* d_fs, double* d_R, const double* d_un, double ca,
-                           double cb, double dt) {
+                           double cb, double dt, double* d_uf_out) {
   constexpr int N = DIM == 2 ? P1 * P1 : P1 * P1 * P1;
   int warps = 8;
   const size_t per_warp = (size_t)3 * (DIM + 2) * N * sizeof(double);
@@ -303,30 +311,30 @@ static int launch_fr_rhs_t(Tree* t, const double* d_u, const double* d_fs, doubl
   const double w1 = (t->domain[DIM + 1] - t->domain[1]) / t->g.nroot[1];
   const double w2 = DIM == 3 ? (t->domain[DIM + 2] - t->domain[2]) / t->g.nroot[2] : 1.0;
   fn<<<t->num_sms * per_sm, warps * 32, smem, t->stream>>>(t->g, t->keys[t->cur], t->d_s, d_u, d_fs, d_R, w0, w1,
-                                                            w2, d_un, ca, cb, dt);
+                                                            w2, d_un, ca, cb, dt, d_uf_out);
   return LT_OK;
 }
 
 template <int DIM>
 static int launch_fr_rhs_d(Tree* t, const double* d_u, const double* d_fs, double* d_R, int p, const double* d_un,
-                           double ca, double cb, double dt) {
+                           double ca, double cb, double dt, double* d_uf_out) {
   switch (p) {
-    case 0: return launch_fr_rhs_t<DIM, 1>(t, d_u, d_fs, d_R, d_un, ca, cb, dt);
-    case 1: return launch_fr_rhs_t<DIM, 2>(t, d_u, d_fs, d_R, d_un, ca, cb, dt);
-    case 2: return launch_fr_rhs_t<DIM, 3>(t, d_u, d_fs, d_R, d_un, ca, cb, dt);
-    case 3: return launch_fr_rhs_t<DIM, 4>(t, d_u, d_fs, d_R, d_un, ca, cb, dt);
-    case 4: return launch_fr_rhs_t<DIM, 5>(t, d_u, d_fs, d_R, d_un, ca, cb, dt);
-    case 5: return launch_fr_rhs_t<DIM, 6>(t, d_u, d_fs, d_R, d_un, ca, cb, dt);
-    case 6: return launch_fr_rhs_t<DIM, 7>(t, d_u, d_fs, d_R, d_un, ca, cb, dt);
-    case 7: return launch_fr_rhs_t<DIM, 8>(t, d_u, d_fs, d_R, d_un, ca, cb, dt);
+    case 0: return launch_fr_rhs_t<DIM, 1>(t, d_u, d_fs, d_R, d_un, ca, cb, dt, d_uf_out);
+    case 1: return launch_fr_rhs_t<DIM, 2>(t, d_u, d_fs, d_R, d_un, ca, cb, dt, d_uf_out);
+    case 2: return launch_fr_rhs_t<DIM, 3>(t, d_u, d_fs, d_R, d_un, ca, cb, dt, d_uf_out);
+    case 3: return launch_fr_rhs_t<DIM, 4>(t, d_u, d_fs, d_R, d_un, ca, cb, dt, d_uf_out);
+    case 4: return launch_fr_rhs_t<DIM, 5>(t, d_u, d_fs, d_R, d_un, ca, cb, dt, d_uf_out);
+    case 5: return launch_fr_rhs_t<DIM, 6>(t, d_u, d_fs, d_R, d_un, ca, cb, dt, d_uf_out);
+    case 6: return launch_fr_rhs_t<DIM, 7>(t, d_u, d_fs, d_R, d_un, ca, cb, dt, d_uf_out);
+    case 7: return launch_fr_rhs_t<DIM, 8>(t, d_u, d_fs, d_R, d_un, ca, cb, dt, d_uf_out);
   }
   return LT_ERR_ARG;
 }
 
 int launch_fr_rhs(Tree* t, const double* d_u, const double* d_fs, double* d_R, int p, const double* d_un, double ca,
-                  double cb, double dt) {
-  const int rc = t->g.dim == 2 ? launch_fr_rhs_d<2>(t, d_u, d_fs, d_R, p, d_un, ca, cb, dt)
-                               : launch_fr_rhs_d<3>(t, d_u, d_fs, d_R, p, d_un, ca, cb, dt);
+                  double cb, double dt, double* d_uf_out) {
+  const int rc = t->g.dim == 2 ? launch_fr_rhs_d<2>(t, d_u, d_fs, d_R, p, d_un, ca, cb, dt, d_uf_out)
+                               : launch_fr_rhs_d<3>(t, d_u, d_fs, d_R, p, d_un, ca, cb, dt, d_uf_out);
   if (rc != LT_OK) return rc;
   t->launches++;
   LT_CUDA(cudaGetLastError());

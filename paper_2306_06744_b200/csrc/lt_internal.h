@@ -157,6 +157,7 @@ int build_operators(Tree* t, int p);
 int launch_face_interp(Tree* t, const double* d_u, double* d_uf, int p, int nvars);
 int launch_mortar_hits(Tree* t);
 int launch_mortar(Tree* t, int which, const double* d_in, double* d_out, int p, int nvars);
+int launch_face_flux(Tree* t, const double* d_uf, double* d_fs, int p);
 
 // ---- lt_construct.cu (Alg. 2)
 int launch_points_to_keys(int dim, int maxl, const double* domain, const double* d_xyz, int64_t n, uint64_t* d_keys,
@@ -168,7 +169,7 @@ int launch_complete_fill(Tree* t, const uint64_t* d_in, int64_t n, const uint32_
 int build_fr_operators(Tree* t, int p);
 int launch_common_flux(Tree* t, const double* d_uf, const double* d_unb, double* d_fs, int p);
 int launch_fr_rhs(Tree* t, const double* d_u, const double* d_fs, double* d_R, int p, const double* d_un = nullptr,
-                  double ca = 0.0, double cb = 0.0, double dt = 0.0);
+                  double ca = 0.0, double cb = 0.0, double dt = 0.0, double* d_uf_out = nullptr);
 int launch_rk_update(Tree* t, int64_t n, double a, double b, double dt, const double* un, const double* us,
                      const double* R, double* out);
 

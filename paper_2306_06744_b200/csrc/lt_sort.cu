@@ -3,9 +3,10 @@
 // (PAPER.md:117, :126-128, :161, :223).  Product code.
 //
 // One-sweep design: one histogram kernel counts all digits of all passes; each pass is a
-// single kernel in which a tile ranks its keys (warp match + per-warp digit counters in
-// shared memory), publishes its per-digit counts and obtains the counts of all earlier
-// tiles by decoupled look-back, then scatters.  Only bits [0, key_bits) are sorted.
+// single persistent kernel in which a block ranks a tile of 4096 keys (ballots over the digit bits +
+// per-warp digit counters in shared memory), publishes its per-digit counts and obtains the counts
+// of all earlier tiles by decoupled look-back, then scatters -- while the copy engine (cp.async.bulk +
+// mbarrier) already brings in the block's next tile.  Only bits [0, key_bits) are sorted.
 #include "lt_internal.h"
 
 namespace lt {
@@ -48,125 +49,192 @@ __device__ __forceinline__ void st_status(volatile unsigned* p, unsigned v) {
   asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
+// ---- TMA (bulk asynchronous copy) plumbing: one thread arms an mbarrier with the byte count of a tile and
+// issues cp.async.bulk global -> shared; the copy engine signals the barrier when the bytes have landed.
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+
+struct SortSmem {
+  alignas(128) uint64_t in[2][STILE];  // double-buffered input tiles (bulk-copy destinations)
+  uint64_t out[STILE];                 // the tile reordered by digit
+  unsigned wcnt[(ST / 32) * 256];
+  unsigned gbase[256];
+  unsigned loff[256];
+  unsigned scan[33];
+  unsigned ntile;
+  int tile[2];
+  alignas(8) uint64_t bar[2];
+};
+
+// One radix pass, PERSISTENT: a block takes tiles through a ticket and keeps TWO in flight -- while it ranks
+// and scatters tile k out of one shared-memory buffer, the copy engine fills the other buffer with the tile
+// of its next ticket (cp.async.bulk + mbarrier), so the DRAM latency of a tile load hides behind the
+// ranking of the previous one.  Keys are re-read from shared memory where they are needed instead of
+// being held in 16 x 2 registers per thread.  bulk == 0 (input not 16-byte aligned): the tile is loaded
+// by the threads instead.
 __global__ void __launch_bounds__(ST) k_sort_pass(const uint64_t* __restrict__ in, uint64_t* __restrict__ out,
                                                   int64_t n, int shift, const unsigned* __restrict__ base,
-                                                  volatile unsigned* status, int* ticket) {
-  __shared__ unsigned wcnt[(ST / 32) * 256];
-  __shared__ unsigned gbase[256];
-  __shared__ unsigned loff[256];
-  __shared__ unsigned s_scan[33];
-  __shared__ unsigned s_ntile;
-  __shared__ uint64_t s_keys[STILE];
-  __shared__ int s_tile;
-  if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1);
-  for (int i = threadIdx.x; i < (ST / 32) * 256; i += ST) wcnt[i] = 0;
-  __syncthreads();
-  const int tile = s_tile;
+                                                  volatile unsigned* status, int* ticket, int bulk) {
+  extern __shared__ __align__(128) unsigned char sort_smem_raw[];
+  SortSmem& S = *reinterpret_cast<SortSmem*>(sort_smem_raw);
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const unsigned lt_mask = (1u << lane) - 1;
-  uint64_t key[SITEMS];
-  unsigned rank[SITEMS];
-  int dig[SITEMS];
-  const int64_t t0 = (int64_t)tile * STILE + (int64_t)w * 32 * SITEMS + lane;
-#pragma unroll
-  for (int k = 0; k < SITEMS; ++k) {
-    const int64_t idx = t0 + k * 32;
-    const bool valid = idx < n;
-    key[k] = valid ? in[idx] : 0;
-    dig[k] = valid ? (int)((key[k] >> shift) & 255) : 256;
-  }
-  // stable rank of every key among the equal-digit keys of its warp (warp-striped order)
-  // all match operations are issued before the (serial, shared-memory) counter updates: MATCH
-  // has a long latency and the loop below would otherwise expose it SITEMS times
-  // (peers by 9 ballots over the digit bits rather than MATCH.ANY, whose latency grows with the
-  // number of distinct values in the warp -- about 28 of 32 for a random digit)
-  unsigned peers[SITEMS];
-#pragma unroll
-  for (int k = 0; k < SITEMS; ++k) {
-    unsigned pm = 0xffffffffu;
-#pragma unroll
-    for (int b = 0; b < 9; ++b) {
-      const bool bit = (dig[k] >> b) & 1;
-      const unsigned vote = __ballot_sync(0xffffffffu, bit);
-      pm &= bit ? vote : ~vote;
-    }
-    peers[k] = pm;
-  }
-#pragma unroll
-  for (int k = 0; k < SITEMS; ++k) {
-    const unsigned before = __popc(peers[k] & lt_mask);
-    unsigned pre = 0;
-    if (dig[k] < 256) pre = wcnt[w * 256 + dig[k]];
-    __syncwarp();
-    if (dig[k] < 256 && before == 0) wcnt[w * 256 + dig[k]] = pre + __popc(peers[k]);
-    __syncwarp();
-    rank[k] = pre + before;
+  const int ntiles = (int)((n + STILE - 1) / STILE);
+  auto tile_count = [&](int t) { return (int)min((int64_t)STILE, n - (int64_t)t * STILE); };
+  auto issue = [&](int buf, int t) {  // (one thread) request tile t into buffer buf
+    const int cnt = tile_count(t);
+    const uint32_t bytes = (uint32_t)(cnt * 8) & ~15u;
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // earlier reads of the buffer are done
+    mbar_arrive_expect_tx(&S.bar[buf], bytes);
+    if (bytes) bulk_g2s(S.in[buf], in + (size_t)t * STILE, bytes, &S.bar[buf]);
+  };
+  if (threadIdx.x == 0) {
+    mbar_init(&S.bar[0], 1);
+    mbar_init(&S.bar[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    const int t = atomicAdd(ticket, 1);
+    S.tile[0] = t;
+    if (bulk && t < ntiles) issue(0, t);
   }
   __syncthreads();
-  {
-    // thread d owns digit d: prefix over the warps, then decoupled look-back over tiles
-    const int d = threadIdx.x;
-    unsigned run = 0;
-#pragma unroll
-    for (int ww = 0; ww < ST / 32; ++ww) {
-      unsigned c = wcnt[ww * 256 + d];
-      wcnt[ww * 256 + d] = run;
-      run += c;
+  for (int it = 0;; ++it) {
+    const int b = it & 1;
+    const int tile = S.tile[b];
+    if (tile >= ntiles) break;
+    const int cnt = tile_count(tile);
+    if (threadIdx.x == 0) {  // the next ticket: its tile travels while this one is ranked
+      const int t = atomicAdd(ticket, 1);
+      S.tile[b ^ 1] = t;
+      if (bulk && t < ntiles) issue(b ^ 1, t);
     }
-    unsigned excl = 0;
-    if (tile == 0) {
-      st_status(status + d, run | FLAG_INC);
-    } else {
-      st_status(status + (size_t)tile * 256 + d, run | FLAG_AGG);
-      // look back over the earlier tiles, LB status words per round trip: in the first wave
-      // every resident tile publishes its aggregate at about the same time, so the chain to
-      // the nearest inclusive prefix can be hundreds of tiles long -- batching the (independent)
-      // loads keeps it from being a chain of dependent L2 latencies
-      constexpr int LB = 8;
-      bool done = false;
-      for (int t = tile - 1; t >= 0 && !done; t -= LB) {
-        unsigned v[LB];
-#pragma unroll
-        for (int j = 0; j < LB; ++j) v[j] = t - j >= 0 ? ld_status(status + (size_t)(t - j) * 256 + d) : (2u << 30);
-#pragma unroll
-        for (int j = 0; j < LB; ++j) {
-          if (done) break;
-          while ((v[j] >> 30) == 0) v[j] = ld_status(status + (size_t)(t - j) * 256 + d);
-          LT_DASSERT((v[j] >> 30) <= 2);  // look-back protocol: 0 not ready, 1 tile aggregate, 2 inclusive prefix
-          excl += v[j] & VAL_MASK;
-          if ((v[j] >> 30) == 2) done = true;
-        }
+    for (int i = threadIdx.x; i < (ST / 32) * 256; i += ST) S.wcnt[i] = 0;
+    const uint64_t* sk = S.in[b];
+    if (bulk) {
+      while (!mbar_try_wait(&S.bar[b], (uint32_t)((it >> 1) & 1))) {
       }
-      st_status(status + (size_t)tile * 256 + d, ((excl + run) & VAL_MASK) | FLAG_INC);
+      if ((cnt & 1) && threadIdx.x == 0) S.in[b][cnt - 1] = in[(size_t)tile * STILE + cnt - 1];  // odd tail key
+    } else {
+      for (int i = threadIdx.x; i < cnt; i += ST) S.in[b][i] = in[(size_t)tile * STILE + i];
     }
-    // position of digit d's run inside the tile (exclusive scan of the tile histogram) and the
-    // global address of the run's first key minus that position
-    unsigned ntile;
-    const unsigned tex = block_excl_scan<unsigned>(run, s_scan, &ntile);
-    loff[d] = tex;
-    gbase[d] = base[d] + excl - tex;
-    if (d == 0) s_ntile = ntile;
-  }
-  __syncthreads();
-  // reorder the tile by digit in shared memory, then write it out in tile order: consecutive
-  // threads store consecutive addresses inside every digit run (instead of one scattered 8-byte
-  // store per key, 25 sectors per request in the first version)
+    __syncthreads();
+    // stable rank of every key among the equal-digit keys of its warp (warp-striped order); peers by
+    // ballots over the digit bits (MATCH.ANY's latency grows with the number of distinct values)
+    unsigned rank[SITEMS];
+    unsigned digs[SITEMS / 4];  // the 16 digits of this thread, one byte each
 #pragma unroll
-  for (int k = 0; k < SITEMS; ++k)
-    if (dig[k] < 256) {
-      LT_DASSERT(loff[dig[k]] + wcnt[w * 256 + dig[k]] + rank[k] < (unsigned)STILE);
-      s_keys[loff[dig[k]] + wcnt[w * 256 + dig[k]] + rank[k]] = key[k];
-    }
-  __syncthreads();
-  const int nt = (int)s_ntile;
+    for (int k = 0; k < SITEMS / 4; ++k) digs[k] = 0;
+    const int i0 = w * 32 * SITEMS + lane;
+    const bool full = cnt == STILE;
 #pragma unroll
-  for (int k = 0; k < SITEMS; ++k) {
-    const int i = k * ST + threadIdx.x;
-    if (i < nt) {
-      const uint64_t kk = s_keys[i];
-      LT_DASSERT((int64_t)gbase[(int)((kk >> shift) & 255)] + i < n);
-      out[(size_t)gbase[(int)((kk >> shift) & 255)] + i] = kk;
+    for (int k = 0; k < SITEMS; ++k) {
+      const int idx = i0 + k * 32;
+      const bool valid = full || idx < cnt;
+      const int dig = valid ? (int)((sk[idx] >> shift) & 255) : 0;
+      digs[k >> 2] |= (unsigned)dig << (8 * (k & 3));
+      unsigned pm = 0xffffffffu;
+#pragma unroll
+      for (int bb = 0; bb < 8; ++bb) {
+        const bool bit = (dig >> bb) & 1;
+        const unsigned vote = __ballot_sync(0xffffffffu, bit);
+        pm &= bit ? vote : ~vote;
+      }
+      if (!full) {
+        const unsigned vv = __ballot_sync(0xffffffffu, valid);
+        pm &= valid ? vv : ~vv;
+      }
+      const unsigned before = __popc(pm & lt_mask);
+      unsigned pre = 0;
+      if (valid) pre = S.wcnt[w * 256 + dig];
+      __syncwarp();
+      if (valid && before == 0) S.wcnt[w * 256 + dig] = pre + __popc(pm);
+      __syncwarp();
+      rank[k] = pre + before;
     }
+    __syncthreads();
+    {
+      // thread d owns digit d: prefix over the warps, then decoupled look-back over tiles
+      const int d = threadIdx.x;
+      unsigned run = 0;
+#pragma unroll
+      for (int ww = 0; ww < ST / 32; ++ww) {
+        unsigned c = S.wcnt[ww * 256 + d];
+        S.wcnt[ww * 256 + d] = run;
+        run += c;
+      }
+      unsigned excl = 0;
+      if (tile == 0) {
+        st_status(status + d, run | FLAG_INC);
+      } else {
+        st_status(status + (size_t)tile * 256 + d, run | FLAG_AGG);
+        // look back over the earlier tiles, LB status words per round trip (independent loads)
+        constexpr int LB = 8;
+        bool done = false;
+        for (int t = tile - 1; t >= 0 && !done; t -= LB) {
+          unsigned v[LB];
+#pragma unroll
+          for (int j = 0; j < LB; ++j) v[j] = t - j >= 0 ? ld_status(status + (size_t)(t - j) * 256 + d) : (2u << 30);
+#pragma unroll
+          for (int j = 0; j < LB; ++j) {
+            if (done) break;
+            while ((v[j] >> 30) == 0) v[j] = ld_status(status + (size_t)(t - j) * 256 + d);
+            LT_DASSERT((v[j] >> 30) <= 2);  // look-back protocol: 0 not ready, 1 tile aggregate, 2 inclusive prefix
+            excl += v[j] & VAL_MASK;
+            if ((v[j] >> 30) == 2) done = true;
+          }
+        }
+        st_status(status + (size_t)tile * 256 + d, ((excl + run) & VAL_MASK) | FLAG_INC);
+      }
+      unsigned ntile;
+      const unsigned tex = block_excl_scan<unsigned>(run, S.scan, &ntile);
+      S.loff[d] = tex;
+      S.gbase[d] = base[d] + excl - tex;
+      if (d == 0) S.ntile = ntile;
+    }
+    __syncthreads();
+    // reorder the tile by digit in shared memory, then write it out in tile order: consecutive threads
+    // store consecutive addresses inside every digit run
+#pragma unroll
+    for (int k = 0; k < SITEMS; ++k) {
+      const int idx = i0 + k * 32;
+      if (full || idx < cnt) {
+        const int dig = (int)((digs[k >> 2] >> (8 * (k & 3))) & 255);
+        const unsigned pos = S.loff[dig] + S.wcnt[w * 256 + dig] + rank[k];
+        LT_DASSERT(pos < (unsigned)STILE);
+        S.out[pos] = sk[idx];
+      }
+    }
+    __syncthreads();
+    LT_DASSERT((int)S.ntile == cnt);
+#pragma unroll
+    for (int k = 0; k < SITEMS; ++k) {
+      const int i = k * ST + threadIdx.x;
+      if (i < cnt) {
+        const uint64_t kk = S.out[i];
+        LT_DASSERT((int64_t)S.gbase[(int)((kk >> shift) & 255)] + i < n);
+        out[(size_t)S.gbase[(int)((kk >> shift) & 255)] + i] = kk;
+      }
+    }
+    __syncthreads();  // S.out, S.wcnt, S.in[b] and S.tile[b] are reused
   }
 }
 
@@ -203,9 +271,19 @@ int sort_keys(uint64_t* d_keys, int64_t n, int key_bits, SortScratch* sc, cudaSt
   *launches += 2;
   uint64_t* src = d_keys;
   uint64_t* dst = sc->tmp;
+  static int per_sm = 0;
+  if (per_sm == 0) {
+    LT_CUDA(cudaFuncSetAttribute(k_sort_pass, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem)));
+    LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sort_pass, ST, sizeof(SortSmem)));
+    if (per_sm < 1) per_sm = 1;
+  }
+  int num_sms = 148, dev = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+  const int G = (int)(tiles < (int64_t)num_sms * per_sm ? tiles : (int64_t)num_sms * per_sm);
   for (int p = 0; p < passes; ++p) {
     LT_CUDA(cudaMemsetAsync(sc->status, 0, (size_t)tiles * 256 * sizeof(unsigned), s));
-    k_sort_pass<<<(int)tiles, ST, 0, s>>>(src, dst, n, 8 * p, sc->hist + p * 256, sc->status, tickets + p);
+    const int bulk = (((uintptr_t)src) & 15) == 0;  // cp.async.bulk needs 16-byte aligned addresses
+    k_sort_pass<<<G, ST, sizeof(SortSmem), s>>>(src, dst, n, 8 * p, sc->hist + p * 256, sc->status, tickets + p, bulk);
     *launches += 1;
     uint64_t* x = src;
     src = dst;

@@ -20,6 +20,7 @@
 #include <vector>
 
 #include "lt_internal.h"
+#include "lt_euler.cuh"
 
 namespace lt {
 
@@ -864,6 +865,89 @@ static int launch_mortar_d(Tree* t, int which, const double* d_in, double* d_out
     case 7: launch_mortar_t<DIM, 8>(t, which, d_in, d_out, nvars, G); break;
     default: return LT_ERR_ARG;
   }
+  return LT_OK;
+}
+
+// ------------------------------------------------------------------------ Alg. 8 steps 2 + 3 fused
+// lt_face_flux: the neighbour's trace is taken straight from the face array (conforming: the face
+// itself; fine side of a hanging face: the Eq. 17 projection of the coarse trace onto
+// the mortar) and fed to the Rusanov solver without going through memory.  A conforming
+// face is computed ONCE, by the element on its minus side (odd local face), and stored in both
+// elements' slots -- both sides compute the same number anyway (the flux along +a).  Per element and
+// axis this reads 2 face blocks and writes 2 instead of reading 4 and writing 4 (lt_mortar_project +
+// lt_common_flux).  One thread per (leaf, axis, face point); coarse-side hanging slots (kind 3) are left
+// to lt_mortar_gather, boundary slots to the caller.
+template <int DIM, int P1>
+__global__ void __launch_bounds__(256, 3) k_face_flux(const DevScalars* s, const int32_t* __restrict__ nbr,
+                                                   const uint8_t* __restrict__ kind,
+                                                   const double* __restrict__ uf, double* __restrict__ fs) {
+  constexpr int NF = Dim<DIM>::NF, NV = DIM + 2;
+  constexpr int Nf = DIM == 2 ? P1 : P1 * P1, E = NV * Nf;
+  __shared__ double sI[2][8][8], sR[2][8][8];
+  load_ops_1d(P1, sI, sR);
+  const int64_t total = (int64_t)s->n * DIM * Nf;
+  for (int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; idx < total;
+       idx += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t ea = idx / Nf;
+    const int pt = (int)(idx - ea * Nf);
+    const int64_t e = ea / DIM;
+    const int a = (int)(ea - e * DIM);
+#pragma unroll
+    for (int side = 1; side >= 0; --side) {
+      const int f = 2 * a + side;
+      const size_t sl = (size_t)e * NF + f;
+      const int kd = kind[sl];
+      const int k = kd & 15;
+      if (!((k == 1 && side == 1) || k == 2)) continue;
+      const size_t nsl = (size_t)nbr[sl] * NF + (f ^ 1);
+      double own[NV], nb[NV], F[NV];
+#pragma unroll
+      for (int v = 0; v < NV; ++v) own[v] = __ldcs(uf + sl * E + v * Nf + pt);
+      if (k == 1) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) nb[v] = __ldcs(uf + nsl * E + v * Nf + pt);
+      } else {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) nb[v] = mortar_value<DIM, P1>(sI, uf + nsl * E, kd >> 4, v * Nf + pt);
+      }
+      // the minus-side state is the element's own trace on an odd face
+      if (side) rusanov<DIM>(a, own, nb, F); else rusanov<DIM>(a, nb, own, F);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) __stcs(fs + sl * E + v * Nf + pt, F[v]);
+      if (k == 1) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) __stcs(fs + nsl * E + v * Nf + pt, F[v]);
+      }
+    }
+  }
+}
+
+template <int DIM, int P1>
+static void launch_face_flux_t(Tree* t, const double* d_uf, double* d_fs) {
+  k_face_flux<DIM, P1><<<t->num_sms * 8, 256, 0, t->stream>>>(t->d_s, t->nbr, t->kind, d_uf, d_fs);
+}
+
+template <int DIM>
+static int launch_face_flux_d(Tree* t, const double* d_uf, double* d_fs, int p) {
+  switch (p) {
+    case 0: launch_face_flux_t<DIM, 1>(t, d_uf, d_fs); break;
+    case 1: launch_face_flux_t<DIM, 2>(t, d_uf, d_fs); break;
+    case 2: launch_face_flux_t<DIM, 3>(t, d_uf, d_fs); break;
+    case 3: launch_face_flux_t<DIM, 4>(t, d_uf, d_fs); break;
+    case 4: launch_face_flux_t<DIM, 5>(t, d_uf, d_fs); break;
+    case 5: launch_face_flux_t<DIM, 6>(t, d_uf, d_fs); break;
+    case 6: launch_face_flux_t<DIM, 7>(t, d_uf, d_fs); break;
+    case 7: launch_face_flux_t<DIM, 8>(t, d_uf, d_fs); break;
+    default: return LT_ERR_ARG;
+  }
+  return LT_OK;
+}
+
+int launch_face_flux(Tree* t, const double* d_uf, double* d_fs, int p) {
+  const int rc = t->g.dim == 2 ? launch_face_flux_d<2>(t, d_uf, d_fs, p) : launch_face_flux_d<3>(t, d_uf, d_fs, p);
+  if (rc != LT_OK) return rc;
+  t->launches++;
+  LT_CUDA(cudaGetLastError());
   return LT_OK;
 }
 

@@ -59,6 +59,8 @@ SIGNATURES = {
     "lt_face_interp": (_I, [_P, _P, _P, _I, _I]),
     "lt_common_flux": (_I, [_P, _P, _P, _P, _I]),
     "lt_fr_rhs": (_I, [_P, _P, _P, _P, _I]),
+    "lt_face_flux": (_I, [_P, _P, _P, _I]),
+    "lt_fr_stage_faces": (_I, [_P, _I, C.c_double, _P, _P, _P, _P, _P, _I]),
     "lt_rk3_stage": (_I, [_P, _I, C.c_double, _P, _P, _P, _P, _I]),
     "lt_fr_stage": (_I, [_P, _I, C.c_double, _P, _P, _P, _P, _I]),
     "lt_mortar_gather": (_I, [_P, _P, _P, _I, _I]),
@@ -290,6 +292,17 @@ class Tree:
                                     _dptr(f_star, torch.float64, "f_star"), p), "lt_common_flux")
         return f_star
 
+    def face_flux(self, u_face: torch.Tensor, p: int, f_star: torch.Tensor = None):
+        """lt_face_flux (Alg. 8 steps 2 + 3 fused): kind 1 / 2 slots of f_star (NaN-filled when allocated here)."""
+        shp = self._face_shape(p, self.dim + 2)
+        if tuple(u_face.shape) != shp:
+            raise ValueError("lt_face_flux: u_face must be %s" % (shp,))
+        if f_star is None:
+            f_star = torch.full_like(u_face, float("nan"))
+        _check(lib().lt_face_flux(self._h, _dptr(u_face, torch.float64, "u_face"),
+                                  _dptr(f_star, torch.float64, "f_star"), p), "lt_face_flux")
+        return f_star
+
     def fr_rhs(self, u: torch.Tensor, f_star: torch.Tensor, p: int, rhs: torch.Tensor = None) -> torch.Tensor:
         """lt_fr_rhs (Eq. 2-5): u [M, dim+2, N], f_star face array -> R [M, dim+2, N]."""
         if tuple(u.shape) != (self.num_leaves(), self.dim + 2, (p + 1) ** self.dim):
@@ -319,6 +332,18 @@ class Tree:
                                  _dptr(u_stage, torch.float64, "u_stage"), _dptr(f_star, torch.float64, "f_star"),
                                  _dptr(out, torch.float64, "out"), p), "lt_fr_stage")
         return out
+
+    def fr_stage_faces(self, stage: int, dt: float, u_n, u_stage, f_star, p: int, out=None, u_face_out=None):
+        """lt_fr_stage_faces: lt_fr_stage + the traces of the result at the face points; returns (u_out, u_face)."""
+        if out is None:
+            out = torch.empty_like(u_n)
+        if u_face_out is None:
+            u_face_out = torch.empty_like(f_star)
+        _check(lib().lt_fr_stage_faces(self._h, stage, dt, _dptr(u_n, torch.float64, "u_n"),
+                                       _dptr(u_stage, torch.float64, "u_stage"), _dptr(f_star, torch.float64, "f_star"),
+                                       _dptr(out, torch.float64, "out"), _dptr(u_face_out, torch.float64, "u_face_out"),
+                                       p), "lt_fr_stage_faces")
+        return out, u_face_out
 
     def mortar_project(self, u_face: torch.Tensor, p: int, nvars: int, u_nb: torch.Tensor = None) -> torch.Tensor:
         """lt_mortar_project (Alg. 8 step 2): u_face [M, nf, nvars, Nf] -> neighbour traces; slots

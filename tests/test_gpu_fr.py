@@ -202,3 +202,63 @@ def test_full_step_conserves_mass_momentum_energy():
     u3 = gt.fr_stage(3, dt, un, u2, fs, p)
     assert float((u3 - un).abs().max()) > 1e-5                      # the step did something
     assert float((integral(u3) - integral(un)).abs().max()) < 1e-13
+
+
+@pytest.mark.parametrize("dim,base,maxl", [(2, 2, 6), (3, 2, 4)])
+@pytest.mark.parametrize("p", [0, 1, 2, 3, 5, 7])
+def test_fused_face_pass_and_stage_with_traces(dim, base, maxl, p):
+    """lt_face_flux (Alg. 8 steps 2 + 3 in one pass, a conforming face computed once for both sides) and
+    lt_fr_stage_faces (right-hand side + Eq. 6 + the traces of the result) against the oracle's unfused
+    chain: common fluxes on every kind 1 / 2 slot, untouched slots untouched, the stage result, and the
+    face traces of the stage result = the oracle's face_interp of the oracle's stage result."""
+    if dim == 3 and p == 7:
+        maxl = 3
+    gt, ot, rng = adapted_pair(dim, (1,) * dim, 71 * dim + p, base, maxl, cycles=2)
+    F = gt.connect(); ot.connect()
+    assert int(F["n_hang"]) > 0
+    M, N, nv = ot.num_leaves(), (p + 1) ** dim, dim + 2
+    lvl, xyz = ot.leaf_boxes()
+    z, _ = np.polynomial.legendre.leggauss(p + 1)
+    Lw = float(1 << ot.maxl)
+    wd = (1 << (ot.maxl - lvl.astype(np.int64))) / Lw
+    X = np.zeros((M, N, dim))
+    for n in range(N):
+        r = n
+        for a2 in range(dim):
+            X[:, n, a2] = xyz[:, a2] / Lw + 0.5 * wd * (1 + z[r % (p + 1)])
+            r //= p + 1
+    ph = 2 * np.pi * X
+    rho = 1.0 + 0.2 * np.prod(np.sin(ph), axis=-1)
+    vel = np.stack([0.4 + 0.1 * np.cos(ph[..., (a2 + 1) % dim]) for a2 in range(dim)], axis=-1)
+    pr = 1.0 + 0.1 * np.cos(ph[..., 0])
+    u = np.concatenate([rho[:, None], np.moveaxis(rho[..., None] * vel, -1, 1),
+                        (pr / 0.4 + 0.5 * rho * np.sum(vel * vel, -1))[:, None]], axis=1).copy()
+    u_n = u * (1.0 + 0.01 * rng.uniform(-1, 1, u.shape))
+    dt = 1e-3
+    # oracle, unfused
+    uf_o = ot.face_interp(u, p, nv)
+    fs_o = ot.common_flux(uf_o, ot.mortar_project(uf_o, p, nv), p)
+    fs_full = np.where(np.isnan(fs_o), ot.mortar_gather(fs_o, p, nv), fs_o)
+    R_o = ot.fr_rhs(u, fs_full, p, [1.0] * dim)
+    lvl_max = int(lvl.max())
+    for stage in (2, 3):
+        want = oracle.rk3_stage(stage, dt, u_n, u, R_o)
+        want_uf = ot.face_interp(want, p, nv)
+        # GPU, fused
+        d_u = torch.from_numpy(u).cuda()
+        uf = gt.face_interp(d_u, p, nv)
+        fs = gt.face_flux(uf, p)
+        close(fs, fs_o, "face_flux")                      # NaN (untouched) exactly on the kind 0 / 3 slots
+        gt.mortar_gather(fs, p, nv, f_face=fs)
+        close(fs, fs_full, "face_flux + gather")
+        out, uf2 = gt.fr_stage_faces(stage, dt, torch.from_numpy(u_n).cuda(), d_u, fs, p)
+        tol = 1e-12 * max(1.0, float(np.abs(want).max()), dt * float(2 << lvl_max) * float(np.abs(fs_full).max()))
+        assert float(np.abs(out.cpu().numpy() - want).max()) <= tol
+        assert float(np.abs(uf2.cpu().numpy() - want_uf).max()) <= 4 * tol
+        # the traces may overwrite the fluxes (an element touches only its own slots)
+        fs2 = fs.clone()
+        out2, uf3 = gt.fr_stage_faces(stage, dt, torch.from_numpy(u_n).cuda(), d_u, fs2, p, u_face_out=fs2)
+        assert torch.equal(out2, out) and torch.equal(uf3, uf2) and uf3.data_ptr() == fs2.data_ptr()
+        # and the plain right-hand side of the re-laid-out kernel
+        close_rhs(gt.fr_rhs(d_u, fs, p), R_o, fs_full, ot, "fr_rhs (padded layout)")
+    gt.sync()
