@@ -121,8 +121,11 @@ __global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restric
                                                 int32_t* __restrict__ bnd, uint8_t* __restrict__ bnd_face,
                                                 unsigned long long* st, unsigned* ticket) {
   constexpr int NF = Dim<DIM>::NF;
-  __shared__ int s_nb[CT * NF];
-  __shared__ uint8_t s_kd[CT * NF];
+  // per-leaf rows padded to an odd pitch: with NF = 6 (or 4) words per leaf the lanes of a warp, each
+  // writing its own leaf's slot f, hit every other bank twice (12 M conflicts per 13.5 M-leaf query)
+  constexpr int NP = NF + 1;
+  __shared__ int s_nb[CT * NP];
+  __shared__ uint8_t s_kd[CT * NP];
   __shared__ unsigned long long sm[33];
   __shared__ unsigned long long s_excl[2];
   __shared__ int s_tile;
@@ -159,16 +162,16 @@ __global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restric
         int nb, kd = 1;
         if (l == 0 || !face_by_sibling<DIM>(g, keys, n, i, m, l, cid, a, &nb))
           kd = face_by_search<DIM>(g, keys, first, m, l, f, &s->status_c, &nb);
-        s_nb[threadIdx.x * NF + f] = nb;
-        s_kd[threadIdx.x * NF + f] = (uint8_t)kd;
+        s_nb[threadIdx.x * NP + f] = nb;
+        s_kd[threadIdx.x * NP + f] = (uint8_t)kd;
       }
 #pragma unroll
       for (int a = 0; a < DIM; ++a) {
         const int f = 2 * a + ((cid >> a) & 1);
         int nb;
         const int kd = face_by_search<DIM>(g, keys, first, m, l, f, &s->status_c, &nb);
-        s_nb[threadIdx.x * NF + f] = nb;
-        s_kd[threadIdx.x * NF + f] = (uint8_t)kd;
+        s_nb[threadIdx.x * NP + f] = nb;
+        s_kd[threadIdx.x * NP + f] = (uint8_t)kd;
       }
     }
     __syncthreads();
@@ -178,8 +181,9 @@ __global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restric
       const int sl = r * CT + threadIdx.x;
       if (sl < ne * NF) {
         const size_t gs = (size_t)e0 * NF + sl;
-        nbr[gs] = s_nb[sl];
-        kind[gs] = s_kd[sl];
+        const int pl = (sl / NF) * NP + sl % NF;
+        nbr[gs] = s_nb[pl];
+        kind[gs] = s_kd[pl];
       }
     }
     // ---- rows of this thread's leaf: conf | hang << 21 | bnd << 42
@@ -187,7 +191,7 @@ __global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restric
     if ((int)threadIdx.x < ne) {
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
-        const int kd = s_kd[threadIdx.x * NF + f];
+        const int kd = s_kd[threadIdx.x * NP + f];
         cnt += (unsigned long long)((kd == 1) & (f & 1)) | ((unsigned long long)((kd & 15) == 2) << 21) |
                ((unsigned long long)(kd == 0) << 42);
       }
@@ -222,8 +226,8 @@ __global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restric
                  p_bnd >= 0 && p_bnd <= (int64_t)NF * e);
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
-        const int kd = s_kd[threadIdx.x * NF + f];
-        const int nb = s_nb[threadIdx.x * NF + f];
+        const int kd = s_kd[threadIdx.x * NP + f];
+        const int nb = s_nb[threadIdx.x * NP + f];
         if (kd == 1) {
           if (f & 1) {  // a conforming face is emitted by the element on its minus side
             reinterpret_cast<int2*>(conf)[p_conf] = make_int2(e, nb);

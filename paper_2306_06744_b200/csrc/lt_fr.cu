@@ -69,7 +69,9 @@ __global__ void __launch_bounds__(256) k_fr_rhs(Geo g, const uint64_t* __restric
   // reads and writes only its own face slots).
   // (A layout with padded x-lines and 1 / rho, p stored once per point was tried: it removes the bank
   // conflicts but needs 10.9 instead of 7.7 KB of shared memory per warp, i.e. 16 instead of 24 resident
-  // warps per SM, and the kernel is latency-bound: 35.6 instead of 25.2 ms per stage on 8.86 M elements.)
+  // warps per SM, and the kernel is latency-bound: 35.6 instead of 25.2 ms per stage on 8.86 M elements.
+  // Rotating the x / y indices by iz instead (conflict-free on all three axes at no cost in shared memory)
+  // was tried as well: 27.1 ms -- the extra index arithmetic costs more than the 4-way conflicts.)
   constexpr int NF = Dim<DIM>::NF, NV = DIM + 2;
   constexpr int N = DIM == 2 ? P1 * P1 : P1 * P1 * P1, Nf = DIM == 2 ? P1 : P1 * P1, EV = NV * N;
   extern __shared__ double sm_all[];  // [warps][3][NV][N]: u | F | R
