@@ -791,9 +791,11 @@ int lt_connect_begin(lt_tree* t) {
   LT_CUDA(cudaEventRecord(t->ev_side_fork, t->stream));
   LT_CUDA(cudaStreamWaitEvent(t->s_side, t->ev_side_fork, 0));
   cudaEventRecord(t->ev[12], t->s_side);
-  // 3 of the 8 resident blocks per SM: measured best on config 5 (1: the query outlasts the transfer,
-  // 4+: the transfer loses more than the query gains); LT_SIDE_BLOCKS overrides for experiments
-  static const int side_blocks = getenv("LT_SIDE_BLOCKS") ? atoi(getenv("LT_SIDE_BLOCKS")) : 3;
+  // 2 resident blocks per SM (k_connect handles two leaves per thread at 64 registers, so two of its blocks
+  // and two blocks of the transfer share an SM's registers): measured best on config 5 -- 1: the query
+  // outlasts the transfer (15.7 ms), 3: the transfer loses more than the query gains; LT_SIDE_BLOCKS
+  // overrides for experiments
+  static const int side_blocks = getenv("LT_SIDE_BLOCKS") ? atoi(getenv("LT_SIDE_BLOCKS")) : 2;
   // (a small mesh -- the transfer beside it takes well under a millisecond -- gets every block: there
   // the query itself would become the critical path)
   const int64_t n_est = t->n_valid ? t->n : (t->n_upper >> t->g.dim);  // (n_upper is the 2^dim-fold worst case)

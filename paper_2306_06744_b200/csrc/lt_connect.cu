@@ -14,7 +14,9 @@
 
 namespace lt {
 
-constexpr int CT = 256;  // threads per block = leaves per tile
+constexpr int CT = 256;   // threads per block
+constexpr int LPT = 2;    // leaves per thread: a tile is CT * LPT consecutive leaves (thread t: leaves t and CT + t)
+constexpr int TL = CT * LPT;
 
 // slot of a fine face inside the coarse face: the fine leaf's child-id bits on the
 // tangential axes, ascending axis order ("the first contributor along one
@@ -124,14 +126,14 @@ __global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restric
   // per-leaf rows padded to an odd pitch: with NF = 6 (or 4) words per leaf the lanes of a warp, each
   // writing its own leaf's slot f, hit every other bank twice (12 M conflicts per 13.5 M-leaf query)
   constexpr int NP = NF + 1;
-  __shared__ int s_nb[CT * NP];
-  __shared__ uint8_t s_kd[CT * NP];
+  __shared__ int s_nb[TL * NP];
+  __shared__ uint8_t s_kd[TL * NP];
   __shared__ unsigned long long sm[33];
   __shared__ unsigned long long s_excl[2];
   __shared__ int s_tile;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int n = s->n;
-  const int ntiles = (n + CT - 1) / CT;
+  const int ntiles = (n + TL - 1) / TL;
   // keys_alt != nullptr: the lt_balance before this query did not wait for its kernel, and the
   // buffer its result ended in (DevScalars::parity) is only known here
   if (keys_alt != nullptr && s->parity) {
@@ -144,44 +146,60 @@ __global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restric
     const int tile = s_tile;
     LT_DASSERT(tile >= 0 && tile < ntiles + (int)gridDim.x);  // every block draws one ticket past the end
     if (tile >= ntiles) break;
-    const int e0 = tile * CT;
-    const int ne = min(CT, n - e0);
+    const int e0 = tile * TL;
+    const int ne = min(TL, n - e0);
     // (Tried and rejected, round 2: sharing ONE search per face of the parent among the 2^(dim-1) members
     // of a complete sibling group -- the trick that pays in k_balance -- with key compares for the members'
     // own neighbours.  Bit-exact, but 2.2 instead of 1.5 ms alone and no better beside the transfer: the
     // probes it saves hit L1, the group detection, shuffles and divergence it adds do not come for free.)
-    // ---- classify: one thread per leaf, two warp-uniform phases -- first the DIM faces
-    // interior to the parent (sibling shortcut, one compare), then the DIM exterior faces
-    // (search) -- so that a warp never executes both code paths for every slot
-    if ((int)threadIdx.x < ne) {
+    // ---- classify: a thread handles LPT leaves (two independent chains of dependent probes in flight per
+    // thread, and half as many barriers, tickets and look-backs per leaf as with one), each in two
+    // warp-uniform phases -- first the DIM faces interior to the parent (sibling shortcut, one compare),
+    // then the DIM exterior faces (search) -- so that a warp never executes both code paths for every slot
+    {
       constexpr int NC = Dim<DIM>::NC;
-      const int i = e0 + threadIdx.x;
-      const uint64_t key = keys[i];
-      const int l = key_level(key);
-      const uint64_t m = key_morton(key);
-      const int cid = l > 0 ? (int)((m >> (DIM * (g.maxl - l))) & (uint64_t)(NC - 1)) : 0;
+      uint64_t mq[LPT];
+      int lq[LPT], cq[LPT];
 #pragma unroll
-      for (int a = 0; a < DIM; ++a) {
-        const int f = 2 * a + (((cid >> a) & 1) ^ 1);
-        int nb, kd = 1;
-        if (l == 0 || !face_by_sibling<DIM>(g, keys, n, i, m, l, cid, a, &nb))
-          kd = face_by_search<DIM>(g, keys, first, m, l, f, &s->status_c, &nb);
-        s_nb[threadIdx.x * NP + f] = nb;
-        s_kd[threadIdx.x * NP + f] = (uint8_t)kd;
+      for (int h = 0; h < LPT; ++h) {
+        const int li = h * CT + threadIdx.x;
+        const uint64_t key = li < ne ? keys[e0 + li] : 0;
+        lq[h] = key_level(key);
+        mq[h] = key_morton(key);
+        cq[h] = lq[h] > 0 ? (int)((mq[h] >> (DIM * (g.maxl - lq[h]))) & (uint64_t)(NC - 1)) : 0;
       }
 #pragma unroll
       for (int a = 0; a < DIM; ++a) {
-        const int f = 2 * a + ((cid >> a) & 1);
-        int nb;
-        const int kd = face_by_search<DIM>(g, keys, first, m, l, f, &s->status_c, &nb);
-        s_nb[threadIdx.x * NP + f] = nb;
-        s_kd[threadIdx.x * NP + f] = (uint8_t)kd;
+#pragma unroll
+        for (int h = 0; h < LPT; ++h) {
+          const int li = h * CT + threadIdx.x;
+          if (li >= ne) continue;
+          const int f = 2 * a + (((cq[h] >> a) & 1) ^ 1);
+          int nb, kd = 1;
+          if (lq[h] == 0 || !face_by_sibling<DIM>(g, keys, n, e0 + li, mq[h], lq[h], cq[h], a, &nb))
+            kd = face_by_search<DIM>(g, keys, first, mq[h], lq[h], f, &s->status_c, &nb);
+          s_nb[li * NP + f] = nb;
+          s_kd[li * NP + f] = (uint8_t)kd;
+        }
+      }
+#pragma unroll
+      for (int a = 0; a < DIM; ++a) {
+#pragma unroll
+        for (int h = 0; h < LPT; ++h) {
+          const int li = h * CT + threadIdx.x;
+          if (li >= ne) continue;
+          const int f = 2 * a + ((cq[h] >> a) & 1);
+          int nb;
+          const int kd = face_by_search<DIM>(g, keys, first, mq[h], lq[h], f, &s->status_c, &nb);
+          s_nb[li * NP + f] = nb;
+          s_kd[li * NP + f] = (uint8_t)kd;
+        }
       }
     }
     __syncthreads();
     // F (the paper's face array) leaves in slot order, coalesced
 #pragma unroll
-    for (int r = 0; r < NF; ++r) {
+    for (int r = 0; r < NF * LPT; ++r) {
       const int sl = r * CT + threadIdx.x;
       if (sl < ne * NF) {
         const size_t gs = (size_t)e0 * NF + sl;
@@ -190,19 +208,29 @@ __global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restric
         kind[gs] = s_kd[pl];
       }
     }
-    // ---- rows of this thread's leaf: conf | hang << 21 | bnd << 42
+    // ---- rows of this thread's leaves, packed for ONE block scan: per half of the tile (h = 0: leaves
+    // 0..CT-1, h = 1: the rest) conf (10 bits, <= DIM * CT) | hang (10 bits) | bnd (11 bits, <= NF * CT)
+    static_assert(LPT == 2 && DIM * CT < 1024 && NF * CT < 2048, "packed row counts");
     unsigned long long cnt = 0;
-    if ((int)threadIdx.x < ne) {
 #pragma unroll
-      for (int f = 0; f < NF; ++f) {
-        const int kd = s_kd[threadIdx.x * NP + f];
-        cnt += (unsigned long long)((kd == 1) & (f & 1)) | ((unsigned long long)((kd & 15) == 2) << 21) |
-               ((unsigned long long)(kd == 0) << 42);
+    for (int h = 0; h < LPT; ++h) {
+      const int li = h * CT + threadIdx.x;
+      if (li < ne) {
+        unsigned long long c = 0;
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+          const int kd = s_kd[li * NP + f];
+          c += (unsigned long long)((kd == 1) & (f & 1)) | ((unsigned long long)((kd & 15) == 2) << 10) |
+               ((unsigned long long)(kd == 0) << 20);
+        }
+        cnt |= c << (31 * h);
       }
     }
     unsigned long long tot;
     const unsigned long long ex = block_excl_scan<unsigned long long>(cnt, sm, &tot);
-    const unsigned long long t_conf = tot & 0x1fffff, t_hang = (tot >> 21) & 0x1fffff, t_bnd = (tot >> 42) & 0x1fffff;
+    const unsigned long long a_conf = tot & 0x3ff, a_hang = (tot >> 10) & 0x3ff, a_bnd = (tot >> 20) & 0x7ff;
+    const unsigned long long t_conf = a_conf + ((tot >> 31) & 0x3ff), t_hang = a_hang + ((tot >> 41) & 0x3ff),
+                             t_bnd = a_bnd + ((tot >> 51) & 0x7ff);
     // ---- order the tiles: publish the tile's own counts, then look back (warp 0: conf and
     // hang, warp 1: bnd)
     if (w < 2) {
@@ -214,24 +242,27 @@ __global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restric
     }
     __syncthreads();
     const unsigned long long x0 = s_excl[0], x1 = s_excl[1];
-    int64_t p_conf = (int64_t)(x0 >> 31) + (int64_t)(ex & 0x1fffff);
-    int64_t p_hang = (int64_t)(x0 & 0x7fffffffull) + (int64_t)((ex >> 21) & 0x1fffff);
-    int64_t p_bnd = (int64_t)x1 + (int64_t)((ex >> 42) & 0x1fffff);
     if (tile == ntiles - 1 && threadIdx.x == 0) {
       s->n_face[0] = (int)((x0 >> 31) + t_conf);
       s->n_face[1] = (int)((x0 & 0x7fffffffull) + t_hang);
       s->n_face[2] = (int)(x1 + t_bnd);
     }
     // ---- emit (leaf order, local faces 0..NF-1: reading D-4)
-    if ((int)threadIdx.x < ne) {
-      const int e = e0 + threadIdx.x;
+#pragma unroll
+    for (int h = 0; h < LPT; ++h) {
+      const int li = h * CT + threadIdx.x;
+      if (li >= ne) continue;
+      const int e = e0 + li;
+      int64_t p_conf = (int64_t)(x0 >> 31) + (int64_t)((ex >> (31 * h)) & 0x3ff) + (h ? (int64_t)a_conf : 0);
+      int64_t p_hang = (int64_t)(x0 & 0x7fffffffull) + (int64_t)((ex >> (31 * h + 10)) & 0x3ff) + (h ? (int64_t)a_hang : 0);
+      int64_t p_bnd = (int64_t)x1 + (int64_t)((ex >> (31 * h + 20)) & 0x7ff) + (h ? (int64_t)a_bnd : 0);
       // the rows of the leaves before e: at most DIM conforming, DIM hanging and NF boundary rows each
       LT_DASSERT(p_conf >= 0 && p_conf <= (int64_t)DIM * e && p_hang >= 0 && p_hang <= (int64_t)DIM * e &&
                  p_bnd >= 0 && p_bnd <= (int64_t)NF * e);
 #pragma unroll
       for (int f = 0; f < NF; ++f) {
-        const int kd = s_kd[threadIdx.x * NP + f];
-        const int nb = s_nb[threadIdx.x * NP + f];
+        const int kd = s_kd[li * NP + f];
+        const int nb = s_nb[li * NP + f];
         if (kd == 1) {
           if (f & 1) {  // a conforming face is emitted by the element on its minus side
             reinterpret_cast<int2*>(conf)[p_conf] = make_int2(e, nb);
@@ -273,7 +304,7 @@ int launch_connect(Tree* t, cudaStream_t stream, int blocks_per_sm) {
   uint8_t *conf_axis, *hang_info, *bnd_face;
   face_regions(t, &conf, &conf_axis, &hang, &hang_info, &bnd, &bnd_face);
   // (leaf count still on the device: its upper bound sizes the look-back words to clear)
-  const int64_t ntiles = ((t->n_valid ? t->n : t->n_upper) + CT - 1) / CT;
+  const int64_t ntiles = ((t->n_valid ? t->n : t->n_upper) + TL - 1) / TL;
   LT_CUDA(cudaMemsetAsync(t->tile_state, 0, (size_t)(ntiles + 1) * 2 * sizeof(unsigned long long), stream));
   LT_CUDA(cudaMemsetAsync(&t->d_s->ticket_c, 0, sizeof(unsigned), stream));
   const void* fn = t->g.dim == 2 ? (const void*)k_connect<2> : (const void*)k_connect<3>;
