@@ -434,6 +434,7 @@ def run_ours(args):
             F = t.connect()
             t.transfer(u_old, p, nvars, u_new)
         ev1.record(stream)
+        syncs = t.host_syncs() - syncs0              # before the harness's own waits below
         torch.cuda.synchronize(dev)
         t.sync()
         ms = ev0.elapsed_time(ev1)
@@ -441,7 +442,7 @@ def run_ours(args):
         tm.update({"balance_" + k: v for k, v in t.balance_phases().items()})
         cur ^= 1
         return dict(cycle=c, M0=M0, Ma=Ma, M1=M1, iters=iters, faces=(F["n_conf"], F["n_hang"], F["n_bnd"]),
-                    ms=ms, tm=tm, launches=t.launch_count() - launches0, syncs=t.host_syncs() - syncs0)
+                    ms=ms, tm=tm, launches=t.launch_count() - launches0, syncs=syncs)
 
     def rewind():
         nonlocal cur
