@@ -312,6 +312,19 @@ int lt_decode(int dim, int max_level, const uint64_t* d_keys, int64_t n, int32_t
 int lt_sort_keys(int dim, int max_level, uint64_t* d_keys, int64_t n, int linearise,
                  int64_t* n_out, void* cuda_stream);
 
+/* The same sort (no linearisation) for callers that must not allocate (CUDA graph capture,
+ * serving loops, harnesses that forbid cudaMalloc): the scratch of the radix passes (ping-pong
+ * key buffer, histograms, look-back status words) is a static device array inside the library,
+ * 8.26 MiB held by every GPU that loads liblt until exit.  d_keys: device uint64 [n], sorted
+ * in place, ascending; n <= LT_SORT_STATIC_MAX_KEYS, else LT_ERR_CAPACITY (nothing is launched;
+ * use lt_sort_keys).  Calls no cudaMalloc / cudaFree / allocating routine.  Asynchronous on
+ * cuda_stream; the result is bit-identical to lt_sort_keys(..., linearise = 0).
+ * All calls on one GPU share the array (it keeps the last call's contents; the call clears what
+ * must start at zero): calls that overlap on the GPU -- different streams, or graph branches
+ * without a dependency between them -- race.  Serialise them. */
+#define LT_SORT_STATIC_MAX_KEYS (1 << 20)
+int lt_sort_keys_static(int dim, int max_level, uint64_t* d_keys, int64_t n, void* cuda_stream);
+
 int lt_domain(lt_tree*, double* lo_hi /* host [2*dim] */);
 int lt_info(lt_tree*, int* dim, int* base_level, int* max_level, int* periodic /* host [3] */);
 

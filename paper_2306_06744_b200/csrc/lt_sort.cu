@@ -7,6 +7,8 @@
 // per-warp digit counters in shared memory), publishes its per-digit counts and obtains the counts
 // of all earlier tiles by decoupled look-back, then scatters -- while the copy engine (cp.async.bulk +
 // mbarrier) already brings in the block's next tile.  Only bits [0, key_bits) are sorted.
+#include <mutex>
+
 #include "lt_internal.h"
 
 namespace lt {
@@ -365,4 +367,59 @@ int linearise_keys(int dim, int maxl, const uint64_t* d_in, uint64_t* d_out, int
   return LT_OK;
 }
 
+// ------------------------------------------------------------------------ lt_sort_keys_static
+// The radix sort with its scratch (ping-pong key buffer, digit histograms + tile tickets, look-back
+// status words) in a file-scope device array instead of cudaMalloc'd buffers, for callers that may not
+// allocate (CUDA graph capture, serving loops).  Every GPU that loads the library holds the array
+// until exit: 8 * 2^20 + 8448 + 2^18 bytes = 8.26 MiB for at most LT_SORT_STATIC_MAX_KEYS = 2^20 keys.
+// In host code `g_sort_static` is a host-side stand-in, NOT a device address: the address the
+// kernels get comes from cudaGetSymbolAddress, asked once per device with that device current.
+constexpr int64_t kSortStaticMaxKeys = LT_SORT_STATIC_MAX_KEYS;
+constexpr size_t kSortStaticTmpBytes = (size_t)kSortStaticMaxKeys * sizeof(uint64_t);
+constexpr size_t kSortStaticHistBytes = ((8 * 256 + 8) * sizeof(unsigned) + 255) / 256 * 256;
+constexpr size_t kSortStaticStatusBytes = (size_t)((kSortStaticMaxKeys + STILE - 1) / STILE) * 256 * sizeof(unsigned);
+static __device__ __align__(256) unsigned char g_sort_static[kSortStaticTmpBytes + kSortStaticHistBytes +
+                                                             kSortStaticStatusBytes];
+
+// set-up, once per device: the array's device address and the sort pass's shared-memory opt-in
+static int sort_static_base(unsigned char** base) {
+  static std::mutex mu;
+  static unsigned char* addr[64];
+  int dev = -1;
+  LT_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return LT_ERR_ARG;
+  std::lock_guard<std::mutex> lk(mu);
+  if (!addr[dev]) {
+    unsigned char* ptr = nullptr;
+    LT_CUDA(cudaGetSymbolAddress((void**)&ptr, g_sort_static));
+    if (!ptr) return LT_ERR_CUDA;
+    LT_CUDA(cudaFuncSetAttribute(k_sort_pass, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem)));
+    addr[dev] = ptr;
+  }
+  *base = addr[dev];
+  return LT_OK;
+}
+
 }  // namespace lt
+
+extern "C" int lt_sort_keys_static(int dim, int max_level, uint64_t* d_keys, int64_t n, void* cuda_stream) {
+  using namespace lt;
+  if ((dim != 2 && dim != 3) || n < 0 || (n > 0 && !d_keys)) return LT_ERR_ARG;
+  if (dim * max_level + kLevelBits > 63 || max_level < 0) return LT_ERR_ARG;
+  if (n > kSortStaticMaxKeys) return LT_ERR_CAPACITY;  // beyond the static scratch: use lt_sort_keys
+  if (n <= 1) return LT_OK;
+  unsigned char* base = nullptr;
+  const int rc = sort_static_base(&base);
+  if (rc != LT_OK) return rc;
+  // sort_keys allocates only when a buffer is missing or too small: none is.  It clears what must
+  // start at zero (histograms, tickets, the status words of every pass) on the stream itself.
+  SortScratch sc;
+  sc.tmp = (uint64_t*)base;
+  sc.cap = kSortStaticMaxKeys;
+  sc.hist = (unsigned*)(base + kSortStaticTmpBytes);
+  sc.status = (unsigned*)(base + kSortStaticTmpBytes + kSortStaticHistBytes);
+  sc.status_cap = (kSortStaticMaxKeys + STILE - 1) / STILE;
+  sc.counter = nullptr;
+  int64_t launches = 0;
+  return sort_keys(d_keys, n, dim * max_level + kLevelBits, &sc, (cudaStream_t)cuda_stream, &launches);
+}

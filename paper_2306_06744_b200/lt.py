@@ -74,6 +74,7 @@ SIGNATURES = {
     "lt_encode": (_I, [_I, _I, _P, _P, _I64, _P, _P]),
     "lt_decode": (_I, [_I, _I, _P, _I64, _P, _P, _P]),
     "lt_sort_keys": (_I, [_I, _I, _P, _I64, _I, C.POINTER(_I64), _P]),
+    "lt_sort_keys_static": (_I, [_I, _I, _P, _I64, _P]),
     "lt_domain": (_I, [_P, _P]),
     "lt_info": (_I, [_P, C.POINTER(_I), C.POINTER(_I), C.POINTER(_I), _P]),
     "lt_sync": (_I, [_P]),
@@ -488,3 +489,16 @@ def sort_keys(dim, max_level, keys: torch.Tensor, linearise=False) -> torch.Tens
     _check(lib().lt_sort_keys(dim, max_level, _dptr(k, torch.int64, "keys"), k.numel(), int(bool(linearise)),
                               C.byref(n_out), _stream_ptr(k.device)), "lt_sort_keys")
     return k[: n_out.value]
+
+
+SORT_STATIC_MAX_KEYS = 1 << 20  # LT_SORT_STATIC_MAX_KEYS of include/lt.h
+
+
+def sort_keys_static_(dim, max_level, keys: torch.Tensor) -> None:
+    """lt_sort_keys_static: sorts `keys` (contiguous int64 device tensor, at most SORT_STATIC_MAX_KEYS) IN
+    PLACE with the library's static scratch: no allocation here or in the library; asynchronous on the
+    current stream.  Calls that overlap on the GPU race (one shared scratch array per GPU)."""
+    if not keys.is_contiguous():
+        raise ValueError("lt_sort_keys_static: keys must be contiguous")
+    _check(lib().lt_sort_keys_static(dim, max_level, _dptr(keys, torch.int64, "keys"), keys.numel(),
+                                     _stream_ptr(keys.device)), "lt_sort_keys_static")
