@@ -152,6 +152,12 @@ __global__ void __launch_bounds__(CT) k_connect(Geo g, const uint64_t* __restric
     // of a complete sibling group -- the trick that pays in k_balance -- with key compares for the members'
     // own neighbours.  Bit-exact, but 2.2 instead of 1.5 ms alone and no better beside the transfer: the
     // probes it saves hit L1, the group detection, shuffles and divergence it adds do not come for free.)
+    // (Also tried and rejected: the DIM exterior searches of a leaf in lock-step -- bucket bounds, every
+    // binary-search round and the located keys of the three faces loaded together.  Bit-exact; the query
+    // beside the transfer went from 7.3 to 6.6 ms, but the step did not move (15.42 -> 15.50 ms: what the
+    // transfer loses depends on how many of its blocks the query displaces, not on how long).  A 4-ary
+    // lock-step search that also takes in the interior-face fallbacks needs 127 registers; capped at 64 it
+    // spills and is slower everywhere: 2.5 instead of 1.7 ms alone, 10.8 ms beside the transfer.)
     // ---- classify: a thread handles LPT leaves (two independent chains of dependent probes in flight per
     // thread, and half as many barriers, tickets and look-backs per leaf as with one), each in two
     // warp-uniform phases -- first the DIM faces interior to the parent (sibling shortcut, one compare),
