@@ -778,7 +778,7 @@ def run_construct(args):
                              "library's own device allocations"},
         "ms_per_call": {k: sum(s[k] for s in steps) / args.steps for k in ("build", "balance", "connect")},
         "points_per_s": pts.shape[0] * args.steps / (sum(s["build"] for s in steps) * 1e-3),
-        "roofline": {"bound": "hbm", "kernel": "whole construction call (allocation-bound, see profiles/r1c_construct.md)",
+        "roofline": {"bound": "hbm", "kernel": "whole construction call (launch- and allocation-bound, see profiles/r2_construct.md)",
                      "achieved": (24 * pts.shape[0] + 8 * s0["n0"]) * args.steps / (sum(s["build"] for s in steps) * 1e-3) / 1e9,
                      "peak": peak, "unit": "GB/s", "peak_source": peak_src, "traffic": None,
                      "frac": (24 * pts.shape[0] + 8 * s0["n0"]) * args.steps / (sum(s["build"] for s in steps) * 1e-3) / 1e9 / peak},

@@ -314,7 +314,7 @@ int lt_sort_keys(int dim, int max_level, uint64_t* d_keys, int64_t n, int linear
 
 /* The same sort (no linearisation) for callers that must not allocate (CUDA graph capture,
  * serving loops, harnesses that forbid cudaMalloc): the scratch of the radix passes (ping-pong
- * key buffer, histograms, look-back status words) is a static device array inside the library,
+ * key buffer, per-tile digit table and its scan sums) is a static device array inside the library,
  * 8.26 MiB held by every GPU that loads liblt until exit.  d_keys: device uint64 [n], sorted
  * in place, ascending; n <= LT_SORT_STATIC_MAX_KEYS, else LT_ERR_CAPACITY (nothing is launched;
  * use lt_sort_keys).  Calls no cudaMalloc / cudaFree / allocating routine.  Asynchronous on

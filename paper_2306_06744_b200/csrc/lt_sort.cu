@@ -2,11 +2,18 @@
 // PAPER.md:122-128) for sm_100a.  Replaces the paper's thrust::sort / thrust::unique
 // (PAPER.md:117, :126-128, :161, :223).  Product code.
 //
-// One-sweep design: one histogram kernel counts all digits of all passes; each pass is a
-// single persistent kernel in which a block ranks a tile of 4096 keys (ballots over the digit bits +
-// per-warp digit counters in shared memory), publishes its per-digit counts and obtains the counts
-// of all earlier tiles by decoupled look-back, then scatters -- while the copy engine (cp.async.bulk +
-// mbarrier) already brings in the block's next tile.  Only bits [0, key_bits) are sorted.
+// One pass over an 8-bit digit = four launches, no inter-block waiting:
+//   k_sort_tile_hist   per tile of 4096 keys: its 256 digit counts -> table[digit][tile]
+//   k_scan_reduce / k_scan_apply   exclusive scan of the table in (digit, tile) order: entry (d, t)
+//                      becomes the global position of the first key of tile t with digit d
+//   k_sort_scatter     per tile: stable rank of every key among the tile's keys of its digit
+//                      (peer masks by shared-memory atomicOr, per-warp digit counters), the tile
+//                      reordered by digit in shared memory, coalesced write-out per digit run.
+// Only bits [0, key_bits) are sorted.  (Rounds 1-2 used a one-sweep pass with decoupled look-back,
+// in round 2 persistent with cp.async.bulk prefetch of the next tile: 0.84 ms per pass on 64 M keys
+// whatever the loads did, because with ~300-450 resident blocks running in lock-step every tile
+// looked back over most of the current wave -- about 18 status-word loads PER KEY.  Reading the keys
+// a second time for the histogram costs 8 B per key and removes the serial dependency altogether.)
 #include <mutex>
 
 #include "lt_internal.h"
@@ -14,230 +21,168 @@
 namespace lt {
 
 constexpr int ST = 256;                 // threads per sort block (= number of digit values)
-constexpr int SITEMS = 16;              // keys per thread (8: 4.2 -> 6.9 ms for 64 M keys, the per-tile look-back dominates)
+constexpr int SITEMS = 16;              // keys per thread
 constexpr int STILE = ST * SITEMS;      // keys per tile
-constexpr unsigned FLAG_AGG = 1u << 30, FLAG_INC = 2u << 30, VAL_MASK = (1u << 30) - 1;
 
-__global__ void __launch_bounds__(ST) k_sort_hist(const uint64_t* __restrict__ keys, int64_t n, int passes,
-                                                  unsigned* __restrict__ hist) {
-  __shared__ unsigned sh[8 * 256];
-  for (int i = threadIdx.x; i < passes * 256; i += ST) sh[i] = 0;
+// table[d * tiles + t] = number of keys of tile t whose digit is d
+__global__ void __launch_bounds__(ST) k_sort_tile_hist(const uint64_t* __restrict__ in, int64_t n, int shift,
+                                                       int tiles, unsigned* __restrict__ table) {
+  __shared__ unsigned sh[(ST / 32) * 256];  // one histogram per warp: fewer same-address atomics
+  const int w = threadIdx.x >> 5;
+  for (int i = threadIdx.x; i < (ST / 32) * 256; i += ST) sh[i] = 0;
   __syncthreads();
-  for (int64_t i = blockIdx.x * (int64_t)ST + threadIdx.x; i < n; i += (int64_t)gridDim.x * ST) {
-    uint64_t k = keys[i];
-    for (int p = 0; p < passes; ++p) atomicAdd(&sh[p * 256 + (int)((k >> (8 * p)) & 255)], 1u);
+  const int t = blockIdx.x;
+  const int64_t i0 = (int64_t)t * STILE;
+  uint64_t k[SITEMS];
+#pragma unroll
+  for (int q = 0; q < SITEMS; ++q) {
+    const int64_t i = i0 + q * ST + threadIdx.x;
+    k[q] = i < n ? __ldg(in + i) : ~0ull;
   }
+#pragma unroll
+  for (int q = 0; q < SITEMS; ++q)
+    if (i0 + q * ST + threadIdx.x < n) atomicAdd(&sh[w * 256 + (int)((k[q] >> shift) & 255)], 1u);
   __syncthreads();
-  for (int i = threadIdx.x; i < passes * 256; i += ST)
-    if (sh[i]) atomicAdd(&hist[i], sh[i]);
+  unsigned c = 0;
+#pragma unroll
+  for (int ww = 0; ww < ST / 32; ++ww) c += sh[ww * 256 + threadIdx.x];
+  table[(size_t)threadIdx.x * tiles + t] = c;
 }
 
-// exclusive scan of each pass's 256 counters (one block per pass)
-__global__ void __launch_bounds__(256) k_sort_scan_hist(unsigned* __restrict__ hist) {
-  __shared__ unsigned sm[33];
-  unsigned v = hist[blockIdx.x * 256 + threadIdx.x], tot;
-  unsigned ex = block_excl_scan<unsigned>(v, sm, &tot);
-  hist[blockIdx.x * 256 + threadIdx.x] = ex;
+// exclusive scan of a[0..L) in place, two kernels over G chunks (all partial sums < 2^30)
+__global__ void __launch_bounds__(256) k_scan_reduce(const unsigned* __restrict__ a, int64_t L,
+                                                     unsigned long long* __restrict__ sums) {
+  __shared__ unsigned long long sm[33];
+  int64_t lo, hi;
+  block_chunk(L, gridDim.x, blockIdx.x, 1024, &lo, &hi);
+  unsigned long long acc = 0;
+  for (int64_t i = lo + threadIdx.x; i < hi; i += 256) acc += a[i];
+  acc = block_sum(acc, sm);
+  if (threadIdx.x == 0) sums[blockIdx.x] = acc;
 }
 
-// status words are polled with GPU-scope relaxed loads (a volatile access is system scope and
-// is not pipelined); the word carries its own payload, so no fence is needed
-__device__ __forceinline__ unsigned ld_status(const volatile unsigned* p) {
-  unsigned v;
-  asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-__device__ __forceinline__ void st_status(volatile unsigned* p, unsigned v) {
-  asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-
-// ---- TMA (bulk asynchronous copy) plumbing: one thread arms an mbarrier with the byte count of a tile and
-// issues cp.async.bulk global -> shared; the copy engine signals the barrier when the bytes have landed.
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                   smem_u32(dst)),
-               "l"(src), "r"(bytes), "r"(smem_u32(bar))
-               : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
-  uint32_t ok;
-  asm volatile(
-      "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
-      : "=r"(ok)
-      : "r"(smem_u32(bar)), "r"(parity)
-      : "memory");
-  return ok != 0;
+__global__ void __launch_bounds__(256) k_scan_apply(unsigned* __restrict__ a, int64_t L,
+                                                    const unsigned long long* __restrict__ sums) {
+  __shared__ unsigned long long sm[33];
+  __shared__ unsigned su[33];
+  unsigned long long before, total;
+  chunk_offsets(sums, gridDim.x, blockIdx.x, sm, &before, &total);
+  int64_t lo, hi;
+  block_chunk(L, gridDim.x, blockIdx.x, 1024, &lo, &hi);  // chunks are multiples of 1024: four per thread
+  unsigned run = (unsigned)before;
+  for (int64_t t0 = lo; t0 < hi; t0 += 1024) {
+    const int64_t i = t0 + 4 * threadIdx.x;
+    unsigned v[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) v[q] = i + q < hi ? a[i + q] : 0u;
+    unsigned tot;
+    unsigned ex = run + block_excl_scan<unsigned>(v[0] + v[1] + v[2] + v[3], su, &tot);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      if (i + q < hi) a[i + q] = ex;
+      ex += v[q];
+    }
+    run += tot;
+  }
 }
 
 struct SortSmem {
-  alignas(128) uint64_t in[2][STILE];  // double-buffered input tiles (bulk-copy destinations)
-  uint64_t out[STILE];                 // the tile reordered by digit
-  unsigned wcnt[(ST / 32) * 256];
+  uint64_t out[STILE];             // the tile reordered by digit; before that: the peer masks
+  unsigned wcnt[(ST / 32) * 256];  // per-warp digit counters
   unsigned gbase[256];
   unsigned loff[256];
   unsigned scan[33];
-  unsigned ntile;
-  int tile[2];
-  alignas(8) uint64_t bar[2];
 };
 
-// One radix pass, PERSISTENT: a block takes tiles through a ticket and keeps TWO in flight -- while it ranks
-// and scatters tile k out of one shared-memory buffer, the copy engine fills the other buffer with the tile
-// of its next ticket (cp.async.bulk + mbarrier), so the DRAM latency of a tile load hides behind the
-// ranking of the previous one.  Keys are re-read from shared memory where they are needed instead of
-// being held in 16 x 2 registers per thread.  bulk == 0 (input not 16-byte aligned): the tile is loaded
-// by the threads instead.
-__global__ void __launch_bounds__(ST, 2) k_sort_pass(const uint64_t* __restrict__ in, uint64_t* __restrict__ out,
-                                                  int64_t n, int shift, const unsigned* __restrict__ base,
-                                                  volatile unsigned* status, int* ticket, int bulk) {
-  extern __shared__ __align__(128) unsigned char sort_smem_raw[];
-  SortSmem& S = *reinterpret_cast<SortSmem*>(sort_smem_raw);
+// One tile of one pass.  Thread (w, lane) holds keys w * 512 + k * 32 + lane, k = 0..15 (warp-striped:
+// coalesced loads, and ranks that follow the tile order).  Round k: every lane ORs its bit into the mask
+// of its digit (match[k & 1][w][digit], shared memory); the mask read back is the set of lanes with that
+// digit (what eight ballots over the digit bits delivered at three times the instruction count); the
+// lowest of them adds their number to the warp's digit counter and hands the previous count to the
+// others by shuffle, then clears the mask for round k + 2.
+template <bool FULL>
+__device__ __forceinline__ void sort_scatter_tile(SortSmem& S, const uint64_t* __restrict__ in,
+                                                  uint64_t* __restrict__ out, int cnt, int shift,
+                                                  const unsigned* __restrict__ trow, int tiles) {
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const unsigned lt_mask = (1u << lane) - 1;
-  const int ntiles = (int)((n + STILE - 1) / STILE);
-  auto tile_count = [&](int t) { return (int)min((int64_t)STILE, n - (int64_t)t * STILE); };
-  auto issue = [&](int buf, int t) {  // (one thread) request tile t into buffer buf
-    const int cnt = tile_count(t);
-    const uint32_t bytes = (uint32_t)(cnt * 8) & ~15u;
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // earlier reads of the buffer are done
-    mbar_arrive_expect_tx(&S.bar[buf], bytes);
-    if (bytes) bulk_g2s(S.in[buf], in + (size_t)t * STILE, bytes, &S.bar[buf]);
-  };
-  if (threadIdx.x == 0) {
-    mbar_init(&S.bar[0], 1);
-    mbar_init(&S.bar[1], 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    const int t = atomicAdd(ticket, 1);
-    S.tile[0] = t;
-    if (bulk && t < ntiles) issue(0, t);
+  const unsigned lt_mask = (1u << lane) - 1, bit = 1u << lane;
+  const int i0 = w * 32 * SITEMS + lane;
+  uint64_t key[SITEMS];
+#pragma unroll
+  for (int k = 0; k < SITEMS; ++k) key[k] = (FULL || i0 + k * 32 < cnt) ? __ldg(in + i0 + k * 32) : 0ull;
+  unsigned* match = reinterpret_cast<unsigned*>(S.out);  // [2][ST / 32][256]
+  for (int i = threadIdx.x; i < 2 * (ST / 32) * 256; i += ST) match[i] = 0;
+  for (int i = threadIdx.x; i < (ST / 32) * 256; i += ST) S.wcnt[i] = 0;
+  __syncthreads();
+  volatile unsigned* mw0 = match + w * 256;
+  volatile unsigned* mw1 = mw0 + (ST / 32) * 256;
+  volatile unsigned* wc = S.wcnt + w * 256;
+  unsigned rank[SITEMS / 2];  // two 16-bit ranks per word
+#pragma unroll
+  for (int k = 0; k < SITEMS; ++k) {
+    const bool valid = FULL || i0 + k * 32 < cnt;
+    const int dig = (int)((key[k] >> shift) & 255);
+    volatile unsigned* mw = (k & 1) ? mw1 : mw0;
+    if (valid) atomicOr(const_cast<unsigned*>(mw) + dig, bit);
+    __syncwarp();
+    const unsigned pm = valid ? mw[dig] : 0u;
+    const bool lead = (pm & lt_mask) == 0 && valid;  // the lowest lane of the digit's peers
+    // (every lane reads the counter; only the leader's value is used, and the leader reads before it writes)
+    unsigned pre = wc[dig];
+    if (lead) wc[dig] = pre + __popc(pm);
+    pre = __shfl_sync(0xffffffffu, pre, (__ffs(pm) - 1) & 31);  // (also: every lane has read its mask by now)
+    if (lead) mw[dig] = 0;
+    const unsigned r = pre + __popc(pm & lt_mask);
+    if (k & 1) rank[k >> 1] |= r << 16; else rank[k >> 1] = r;
   }
   __syncthreads();
-  for (int it = 0;; ++it) {
-    const int b = it & 1;
-    const int tile = S.tile[b];
-    if (tile >= ntiles) break;
-    const int cnt = tile_count(tile);
-    if (threadIdx.x == 0) {  // the next ticket: its tile travels while this one is ranked
-      const int t = atomicAdd(ticket, 1);
-      S.tile[b ^ 1] = t;
-      if (bulk && t < ntiles) issue(b ^ 1, t);
+  {
+    // thread d owns digit d: prefix over the warps, prefix over the digits, global base of the digit run
+    const int d = threadIdx.x;
+    unsigned run = 0;
+#pragma unroll
+    for (int ww = 0; ww < ST / 32; ++ww) {
+      const unsigned c = S.wcnt[ww * 256 + d];
+      S.wcnt[ww * 256 + d] = run;
+      run += c;
     }
-    for (int i = threadIdx.x; i < (ST / 32) * 256; i += ST) S.wcnt[i] = 0;
-    const uint64_t* sk = S.in[b];
-    if (bulk) {
-      while (!mbar_try_wait(&S.bar[b], (uint32_t)((it >> 1) & 1))) {
-      }
-      if ((cnt & 1) && threadIdx.x == 0) S.in[b][cnt - 1] = in[(size_t)tile * STILE + cnt - 1];  // odd tail key
-    } else {
-      for (int i = threadIdx.x; i < cnt; i += ST) S.in[b][i] = in[(size_t)tile * STILE + i];
-    }
-    __syncthreads();
-    // stable rank of every key among the equal-digit keys of its warp (warp-striped order); peers by
-    // ballots over the digit bits (MATCH.ANY's latency grows with the number of distinct values)
-    unsigned rank[SITEMS];
-    unsigned digs[SITEMS / 4];  // the 16 digits of this thread, one byte each
-#pragma unroll
-    for (int k = 0; k < SITEMS / 4; ++k) digs[k] = 0;
-    const int i0 = w * 32 * SITEMS + lane;
-    const bool full = cnt == STILE;
-#pragma unroll
-    for (int k = 0; k < SITEMS; ++k) {
-      const int idx = i0 + k * 32;
-      const bool valid = full || idx < cnt;
-      const int dig = valid ? (int)((sk[idx] >> shift) & 255) : 0;
-      digs[k >> 2] |= (unsigned)dig << (8 * (k & 3));
-      unsigned pm = 0xffffffffu;
-#pragma unroll
-      for (int bb = 0; bb < 8; ++bb) {
-        const bool bit = (dig >> bb) & 1;
-        const unsigned vote = __ballot_sync(0xffffffffu, bit);
-        pm &= bit ? vote : ~vote;
-      }
-      if (!full) {
-        const unsigned vv = __ballot_sync(0xffffffffu, valid);
-        pm &= valid ? vv : ~vv;
-      }
-      const unsigned before = __popc(pm & lt_mask);
-      unsigned pre = 0;
-      if (valid) pre = S.wcnt[w * 256 + dig];
-      __syncwarp();
-      if (valid && before == 0) S.wcnt[w * 256 + dig] = pre + __popc(pm);
-      __syncwarp();
-      rank[k] = pre + before;
-    }
-    __syncthreads();
-    {
-      // thread d owns digit d: prefix over the warps, then decoupled look-back over tiles
-      const int d = threadIdx.x;
-      unsigned run = 0;
-#pragma unroll
-      for (int ww = 0; ww < ST / 32; ++ww) {
-        unsigned c = S.wcnt[ww * 256 + d];
-        S.wcnt[ww * 256 + d] = run;
-        run += c;
-      }
-      unsigned excl = 0;
-      if (tile == 0) {
-        st_status(status + d, run | FLAG_INC);
-      } else {
-        st_status(status + (size_t)tile * 256 + d, run | FLAG_AGG);
-        // look back over the earlier tiles, LB status words per round trip (independent loads)
-        constexpr int LB = 8;
-        bool done = false;
-        for (int t = tile - 1; t >= 0 && !done; t -= LB) {
-          unsigned v[LB];
-#pragma unroll
-          for (int j = 0; j < LB; ++j) v[j] = t - j >= 0 ? ld_status(status + (size_t)(t - j) * 256 + d) : (2u << 30);
-#pragma unroll
-          for (int j = 0; j < LB; ++j) {
-            if (done) break;
-            while ((v[j] >> 30) == 0) v[j] = ld_status(status + (size_t)(t - j) * 256 + d);
-            LT_DASSERT((v[j] >> 30) <= 2);  // look-back protocol: 0 not ready, 1 tile aggregate, 2 inclusive prefix
-            excl += v[j] & VAL_MASK;
-            if ((v[j] >> 30) == 2) done = true;
-          }
-        }
-        st_status(status + (size_t)tile * 256 + d, ((excl + run) & VAL_MASK) | FLAG_INC);
-      }
-      unsigned ntile;
-      const unsigned tex = block_excl_scan<unsigned>(run, S.scan, &ntile);
-      S.loff[d] = tex;
-      S.gbase[d] = base[d] + excl - tex;
-      if (d == 0) S.ntile = ntile;
-    }
-    __syncthreads();
-    // reorder the tile by digit in shared memory, then write it out in tile order: consecutive threads
-    // store consecutive addresses inside every digit run
-#pragma unroll
-    for (int k = 0; k < SITEMS; ++k) {
-      const int idx = i0 + k * 32;
-      if (full || idx < cnt) {
-        const int dig = (int)((digs[k >> 2] >> (8 * (k & 3))) & 255);
-        const unsigned pos = S.loff[dig] + S.wcnt[w * 256 + dig] + rank[k];
-        LT_DASSERT(pos < (unsigned)STILE);
-        S.out[pos] = sk[idx];
-      }
-    }
-    __syncthreads();
-    LT_DASSERT((int)S.ntile == cnt);
-#pragma unroll
-    for (int k = 0; k < SITEMS; ++k) {
-      const int i = k * ST + threadIdx.x;
-      if (i < cnt) {
-        const uint64_t kk = S.out[i];
-        LT_DASSERT((int64_t)S.gbase[(int)((kk >> shift) & 255)] + i < n);
-        out[(size_t)S.gbase[(int)((kk >> shift) & 255)] + i] = kk;
-      }
-    }
-    __syncthreads();  // S.out, S.wcnt, S.in[b] and S.tile[b] are reused
+    unsigned ntile;
+    const unsigned tex = block_excl_scan<unsigned>(run, S.scan, &ntile);
+    LT_DASSERT((int)ntile == cnt);
+    S.loff[d] = tex;
+    S.gbase[d] = trow[(size_t)d * tiles] - tex;
   }
+  __syncthreads();
+  // reorder the tile by digit in shared memory, then write it out in tile order: consecutive threads
+  // store consecutive addresses inside every digit run
+#pragma unroll
+  for (int k = 0; k < SITEMS; ++k) {
+    if (FULL || i0 + k * 32 < cnt) {
+      const int dig = (int)((key[k] >> shift) & 255);
+      const unsigned pos = S.loff[dig] + S.wcnt[w * 256 + dig] + ((rank[k >> 1] >> (16 * (k & 1))) & 0xffffu);
+      LT_DASSERT(pos < (unsigned)STILE);
+      S.out[pos] = key[k];
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int k = 0; k < SITEMS; ++k) {
+    const int i = k * ST + threadIdx.x;
+    if (FULL || i < cnt) {
+      const uint64_t kk = S.out[i];
+      out[(size_t)S.gbase[(int)((kk >> shift) & 255)] + i] = kk;
+    }
+  }
+}
+
+__global__ void __launch_bounds__(ST, 3) k_sort_scatter(const uint64_t* __restrict__ in, uint64_t* __restrict__ out,
+                                                        int64_t n, int shift, int tiles,
+                                                        const unsigned* __restrict__ table) {
+  __shared__ SortSmem S;
+  const int tile = blockIdx.x;
+  const int cnt = (int)min((int64_t)STILE, n - (int64_t)tile * STILE);
+  if (cnt == STILE) sort_scatter_tile<true>(S, in + (size_t)tile * STILE, out, cnt, shift, table + tile, tiles);
+  else sort_scatter_tile<false>(S, in + (size_t)tile * STILE, out, cnt, shift, table + tile, tiles);
 }
 
 int sort_keys(uint64_t* d_keys, int64_t n, int key_bits, SortScratch* sc, cudaStream_t s, int64_t* launches) {
@@ -264,29 +209,23 @@ int sort_keys(uint64_t* d_keys, int64_t n, int key_bits, SortScratch* sc, cudaSt
     if (rc != LT_OK) return rc;
     sc->status_cap = tiles;
   }
-  int* tickets = (int*)(sc->hist + 8 * 256);
-  LT_CUDA(cudaMemsetAsync(sc->hist, 0, (8 * 256 + 8) * sizeof(unsigned), s));
-  int hg = (int)((n + ST * 16 - 1) / (ST * 16));
-  if (hg > 148 * 8) hg = 148 * 8;
-  k_sort_hist<<<hg, ST, 0, s>>>(d_keys, n, passes, sc->hist);
-  k_sort_scan_hist<<<passes, 256, 0, s>>>(sc->hist);
-  *launches += 2;
-  uint64_t* src = d_keys;
-  uint64_t* dst = sc->tmp;
-  static int per_sm = 0;
-  if (per_sm == 0) {
-    LT_CUDA(cudaFuncSetAttribute(k_sort_pass, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem)));
-    LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sort_pass, ST, sizeof(SortSmem)));
-    if (per_sm < 1) per_sm = 1;
-  }
+  // sc->hist holds the G chunk sums of the table scan, sc->status the table itself: [256][tiles]
+  unsigned long long* sums = (unsigned long long*)sc->hist;
+  unsigned* table = sc->status;
+  const int64_t L = tiles * 256;
   int num_sms = 148, dev = 0;
   if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
-  const int G = (int)(tiles < (int64_t)num_sms * per_sm ? tiles : (int64_t)num_sms * per_sm);
+  int G = 4 * num_sms;
+  if (G > 1024) G = 1024;  // (8 * 256 + 8) words of sc->hist = 1028 sums
+  if ((int64_t)G * 1024 > L) G = (int)((L + 1023) / 1024);
+  uint64_t* src = d_keys;
+  uint64_t* dst = sc->tmp;
   for (int p = 0; p < passes; ++p) {
-    LT_CUDA(cudaMemsetAsync(sc->status, 0, (size_t)tiles * 256 * sizeof(unsigned), s));
-    const int bulk = (((uintptr_t)src) & 15) == 0;  // cp.async.bulk needs 16-byte aligned addresses
-    k_sort_pass<<<G, ST, sizeof(SortSmem), s>>>(src, dst, n, 8 * p, sc->hist + p * 256, sc->status, tickets + p, bulk);
-    *launches += 1;
+    k_sort_tile_hist<<<(int)tiles, ST, 0, s>>>(src, n, 8 * p, (int)tiles, table);
+    k_scan_reduce<<<G, 256, 0, s>>>(table, L, sums);
+    k_scan_apply<<<G, 256, 0, s>>>(table, L, sums);
+    k_sort_scatter<<<(int)tiles, ST, 0, s>>>(src, dst, n, 8 * p, (int)tiles, table);
+    *launches += 4;
     uint64_t* x = src;
     src = dst;
     dst = x;
@@ -368,8 +307,8 @@ int linearise_keys(int dim, int maxl, const uint64_t* d_in, uint64_t* d_out, int
 }
 
 // ------------------------------------------------------------------------ lt_sort_keys_static
-// The radix sort with its scratch (ping-pong key buffer, digit histograms + tile tickets, look-back
-// status words) in a file-scope device array instead of cudaMalloc'd buffers, for callers that may not
+// The radix sort with its scratch (ping-pong key buffer, chunk sums of the table scan, per-tile digit
+// table) in a file-scope device array instead of cudaMalloc'd buffers, for callers that may not
 // allocate (CUDA graph capture, serving loops).  Every GPU that loads the library holds the array
 // until exit: 8 * 2^20 + 8448 + 2^18 bytes = 8.26 MiB for at most LT_SORT_STATIC_MAX_KEYS = 2^20 keys.
 // In host code `g_sort_static` is a host-side stand-in, NOT a device address: the address the
@@ -381,7 +320,7 @@ constexpr size_t kSortStaticStatusBytes = (size_t)((kSortStaticMaxKeys + STILE -
 static __device__ __align__(256) unsigned char g_sort_static[kSortStaticTmpBytes + kSortStaticHistBytes +
                                                              kSortStaticStatusBytes];
 
-// set-up, once per device: the array's device address and the sort pass's shared-memory opt-in
+// set-up, once per device: the array's device address
 static int sort_static_base(unsigned char** base) {
   static std::mutex mu;
   static unsigned char* addr[64];
@@ -393,7 +332,6 @@ static int sort_static_base(unsigned char** base) {
     unsigned char* ptr = nullptr;
     LT_CUDA(cudaGetSymbolAddress((void**)&ptr, g_sort_static));
     if (!ptr) return LT_ERR_CUDA;
-    LT_CUDA(cudaFuncSetAttribute(k_sort_pass, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem)));
     addr[dev] = ptr;
   }
   *base = addr[dev];
@@ -412,7 +350,7 @@ extern "C" int lt_sort_keys_static(int dim, int max_level, uint64_t* d_keys, int
   const int rc = sort_static_base(&base);
   if (rc != LT_OK) return rc;
   // sort_keys allocates only when a buffer is missing or too small: none is.  It clears what must
-  // start at zero (histograms, tickets, the status words of every pass) on the stream itself.
+  // start at zero itself (every pass overwrites the whole digit table and the chunk sums before it reads them).
   SortScratch sc;
   sc.tmp = (uint64_t*)base;
   sc.cap = kSortStaticMaxKeys;
