@@ -14,6 +14,7 @@
 // whatever the loads did, because with ~300-450 resident blocks running in lock-step every tile
 // looked back over most of the current wave -- about 18 status-word loads PER KEY.  Reading the keys
 // a second time for the histogram costs 8 B per key and removes the serial dependency altogether.)
+#include <cstddef>
 #include <mutex>
 
 #include "lt_internal.h"
@@ -90,16 +91,16 @@ struct SortSmem {
   uint64_t out[STILE];             // the tile reordered by digit; before that: the peer masks
   unsigned wcnt[(ST / 32) * 256];  // per-warp digit counters
   unsigned gbase[256];
-  unsigned loff[256];
   unsigned scan[33];
 };
 
 // One tile of one pass.  Thread (w, lane) holds keys w * 512 + k * 32 + lane, k = 0..15 (warp-striped:
 // coalesced loads, and ranks that follow the tile order).  Round k: every lane ORs its bit into the mask
 // of its digit (match[k & 1][w][digit], shared memory); the mask read back is the set of lanes with that
-// digit (what eight ballots over the digit bits delivered at three times the instruction count); the
-// lowest of them adds their number to the warp's digit counter and hands the previous count to the
-// others by shuffle, then clears the mask for round k + 2.
+// digit (what eight ballots over the digit bits delivered at three times the instruction count); every
+// lane reads the warp's digit counter, then the lowest lane of each digit adds the number of its peers to
+// the counter and clears the mask.  Rounds go in pairs, so that two chains of shared-memory round trips
+// are in flight (the kernel stalls on those: ncu short-scoreboard).
 template <bool FULL>
 __device__ __forceinline__ void sort_scatter_tile(SortSmem& S, const uint64_t* __restrict__ in,
                                                   uint64_t* __restrict__ out, int cnt, int shift,
@@ -111,29 +112,43 @@ __device__ __forceinline__ void sort_scatter_tile(SortSmem& S, const uint64_t* _
 #pragma unroll
   for (int k = 0; k < SITEMS; ++k) key[k] = (FULL || i0 + k * 32 < cnt) ? __ldg(in + i0 + k * 32) : 0ull;
   unsigned* match = reinterpret_cast<unsigned*>(S.out);  // [2][ST / 32][256]
-  for (int i = threadIdx.x; i < 2 * (ST / 32) * 256; i += ST) match[i] = 0;
-  for (int i = threadIdx.x; i < (ST / 32) * 256; i += ST) S.wcnt[i] = 0;
+  {
+    uint4* z = reinterpret_cast<uint4*>(S.out);  // (S.wcnt follows S.out: one run of 16 + 8 KB of zeros)
+    static_assert(offsetof(SortSmem, wcnt) == sizeof(uint64_t) * STILE, "wcnt follows out");
+    for (int i = threadIdx.x; i < (2 + 1) * (ST / 32) * 256 / 4; i += ST) {
+      const int j = i < 2 * (ST / 32) * 256 / 4 ? i : i - 2 * (ST / 32) * 256 / 4 + (int)(sizeof(uint64_t) * STILE / 16);
+      z[j] = make_uint4(0, 0, 0, 0);
+    }
+  }
   __syncthreads();
-  volatile unsigned* mw0 = match + w * 256;
-  volatile unsigned* mw1 = mw0 + (ST / 32) * 256;
+  volatile unsigned* mA = match + w * 256;             // masks of the even round of a pair
+  volatile unsigned* mB = mA + (ST / 32) * 256;        // and of the odd round
   volatile unsigned* wc = S.wcnt + w * 256;
   unsigned rank[SITEMS / 2];  // two 16-bit ranks per word
 #pragma unroll
-  for (int k = 0; k < SITEMS; ++k) {
-    const bool valid = FULL || i0 + k * 32 < cnt;
-    const int dig = (int)((key[k] >> shift) & 255);
-    volatile unsigned* mw = (k & 1) ? mw1 : mw0;
-    if (valid) atomicOr(const_cast<unsigned*>(mw) + dig, bit);
+  for (int k = 0; k < SITEMS; k += 2) {
+    // two rounds at a time: two independent chains of shared-memory round trips per iteration
+    const bool v0 = FULL || i0 + k * 32 < cnt, v1 = FULL || i0 + (k + 1) * 32 < cnt;
+    const int d0 = (int)((key[k] >> shift) & 255), d1 = (int)((key[k + 1] >> shift) & 255);
+    if (v0) atomicOr(const_cast<unsigned*>(mA) + d0, bit);
+    if (v1) atomicOr(const_cast<unsigned*>(mB) + d1, bit);
     __syncwarp();
-    const unsigned pm = valid ? mw[dig] : 0u;
-    const bool lead = (pm & lt_mask) == 0 && valid;  // the lowest lane of the digit's peers
-    // (every lane reads the counter; only the leader's value is used, and the leader reads before it writes)
-    unsigned pre = wc[dig];
-    if (lead) wc[dig] = pre + __popc(pm);
-    pre = __shfl_sync(0xffffffffu, pre, (__ffs(pm) - 1) & 31);  // (also: every lane has read its mask by now)
-    if (lead) mw[dig] = 0;
-    const unsigned r = pre + __popc(pm & lt_mask);
-    if (k & 1) rank[k >> 1] |= r << 16; else rank[k >> 1] = r;
+    const unsigned pm0 = v0 ? mA[d0] : 0u, pm1 = v1 ? mB[d1] : 0u;
+    const unsigned x01 = v1 ? mA[d1] : 0u;  // the lanes whose even-round key has the digit of my odd-round key
+    const unsigned c0 = wc[d0], c1 = wc[d1];
+    __syncwarp();  // every lane has read its masks and counters
+    if (v0 && (pm0 & lt_mask) == 0) {  // the lowest lane of a digit's peers: count them, clear the mask
+      atomicAdd(const_cast<unsigned*>(wc) + d0, (unsigned)__popc(pm0));
+      mA[d0] = 0;
+    }
+    if (v1 && (pm1 & lt_mask) == 0) {
+      atomicAdd(const_cast<unsigned*>(wc) + d1, (unsigned)__popc(pm1));
+      mB[d1] = 0;
+    }
+    __syncwarp();
+    const unsigned r0 = c0 + __popc(pm0 & lt_mask);
+    const unsigned r1 = c1 + __popc(x01) + __popc(pm1 & lt_mask);
+    rank[k >> 1] = r0 | (r1 << 16);
   }
   __syncthreads();
   {
@@ -141,16 +156,23 @@ __device__ __forceinline__ void sort_scatter_tile(SortSmem& S, const uint64_t* _
     const int d = threadIdx.x;
     unsigned run = 0;
 #pragma unroll
+    unsigned c[ST / 32];
+#pragma unroll
     for (int ww = 0; ww < ST / 32; ++ww) {
-      const unsigned c = S.wcnt[ww * 256 + d];
-      S.wcnt[ww * 256 + d] = run;
-      run += c;
+      c[ww] = S.wcnt[ww * 256 + d];
+      run += c[ww];
     }
+    const unsigned gpos = trow[(size_t)d * tiles];
     unsigned ntile;
-    const unsigned tex = block_excl_scan<unsigned>(run, S.scan, &ntile);
+    unsigned tex = block_excl_scan<unsigned>(run, S.scan, &ntile);
     LT_DASSERT((int)ntile == cnt);
-    S.loff[d] = tex;
-    S.gbase[d] = trow[(size_t)d * tiles] - tex;
+    S.gbase[d] = gpos - tex;
+    // wcnt[w][d] becomes the tile position of warp w's first key with digit d
+#pragma unroll
+    for (int ww = 0; ww < ST / 32; ++ww) {
+      S.wcnt[ww * 256 + d] = tex;
+      tex += c[ww];
+    }
   }
   __syncthreads();
   // reorder the tile by digit in shared memory, then write it out in tile order: consecutive threads
@@ -159,7 +181,7 @@ __device__ __forceinline__ void sort_scatter_tile(SortSmem& S, const uint64_t* _
   for (int k = 0; k < SITEMS; ++k) {
     if (FULL || i0 + k * 32 < cnt) {
       const int dig = (int)((key[k] >> shift) & 255);
-      const unsigned pos = S.loff[dig] + S.wcnt[w * 256 + dig] + ((rank[k >> 1] >> (16 * (k & 1))) & 0xffffu);
+      const unsigned pos = S.wcnt[w * 256 + dig] + ((rank[k >> 1] >> (16 * (k & 1))) & 0xffffu);
       LT_DASSERT(pos < (unsigned)STILE);
       S.out[pos] = key[k];
     }
