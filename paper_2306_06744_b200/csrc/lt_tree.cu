@@ -133,10 +133,9 @@ __global__ void k_check_tiling(Geo g, const uint64_t* __restrict__ keys, DevScal
 template <int DIM>
 __device__ __forceinline__ int adapt_action(const Geo& g, const uint64_t* __restrict__ keys,
                                             const int8_t* __restrict__ flags, int64_t i, int64_t n,
-                                            uint64_t key) {
+                                            uint64_t key, int8_t fl) {
   constexpr int NC = Dim<DIM>::NC;
   const int l = key_level(key);
-  const int8_t fl = flags[i];
   if (fl < 0 && l > g.base) {
     const uint64_t m = key_morton(key);
     const int sh = DIM * (g.maxl - l);
@@ -156,6 +155,47 @@ __device__ __forceinline__ int adapt_action(const Geo& g, const uint64_t* __rest
   }
   if (fl > 0 && l < g.maxl) return ACT_REFINE;
   return ACT_KEEP;
+}
+template <int DIM>
+__device__ __forceinline__ int adapt_action(const Geo& g, const uint64_t* __restrict__ keys,
+                                            const int8_t* __restrict__ flags, int64_t i, int64_t n,
+                                            uint64_t key) {
+  return adapt_action<DIM>(g, keys, flags, i, n, key, flags[i]);
+}
+
+constexpr int kGroup = kScanTiles * BT;  // leaves a block orders with one scan
+
+// Block scan of the packed per-thread counts of one group: field q (kFieldBits bits, q < kScanTiles) =
+// leaves that element (q, thread) puts out (<= 2^dim * BT = 2048 per tile), top field = frontier entries
+// the thread appends.  The lane that forms the block total reserves the group's frontier slots with ONE
+// global atomic between the two barriers of the scan (*fbase = first slot): an atomic per warp and
+// tile on the single counter word serialised in L2 (277 k atomics per lt_adapt of 8.9 M leaves, about
+// 0.85 cycles each: most of that kernel's time).  `sm` holds 34 words.  Ends with a barrier.
+constexpr int kFieldBits = 12, kFrShift = 48;
+constexpr unsigned long long kFieldMask = (1ull << kFieldBits) - 1;
+__device__ __forceinline__ unsigned long long block_scan_reserve(unsigned long long v, unsigned long long* sm,
+                                                                 unsigned long long* total, int* counter,
+                                                                 int* fbase) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  const unsigned long long inc = warp_incl_scan(v);
+  if (lane == 31) sm[w] = inc;
+  __syncthreads();
+  if (w == 0) {
+    const unsigned long long s = lane < nw ? sm[lane] : 0ull;
+    const unsigned long long si = warp_incl_scan(s);
+    sm[lane] = si - s;
+    if (lane == 31) {
+      sm[32] = si;
+      const int nfr = (int)(si >> kFrShift);
+      sm[33] = (counter != nullptr && nfr > 0) ? (unsigned long long)atomicAdd(counter, nfr) : 0ull;
+    }
+  }
+  __syncthreads();
+  const unsigned long long res = sm[w] + inc - v;
+  *total = sm[32];
+  *fbase = (int)sm[33];
+  __syncthreads();
+  return res;
 }
 
 // pass 1: per-chunk output counts.  sums[b] = (kept << 32) | count_B   (see lt_adapt)
@@ -200,8 +240,10 @@ __global__ void __launch_bounds__(BT) k_adapt_scatter(Geo g, const uint64_t* __r
   // (s->nfront[0] entries, any order): a refined leaf as a GROUP entry (its own key), a merged
   // parent as a SELF entry (its position)
   constexpr int NC = Dim<DIM>::NC;
-  __shared__ unsigned long long sm[33];
+  __shared__ unsigned long long sm[34];
   const int64_t n = s->n_in;  // (not s->n: block 0 of this kernel overwrites it, see k_adapt_count)
+  int64_t lo, hi;
+  block_chunk(n, gridDim.x, blockIdx.x, BT, &lo, &hi);
   unsigned long long before, total;
   chunk_offsets(sums, gridDim.x, blockIdx.x, sm, &before, &total);
   const int64_t n_out = (int64_t)(total & 0xffffffffull);
@@ -209,11 +251,10 @@ __global__ void __launch_bounds__(BT) k_adapt_scatter(Geo g, const uint64_t* __r
     if (threadIdx.x == 0 && blockIdx.x == 0) set_status(&s->status, LT_ERR_CAPACITY);
     return;
   }
-  int64_t lo, hi;
-  block_chunk(n, gridDim.x, blockIdx.x, BT, &lo, &hi);
   int64_t run = (int64_t)(before & 0xffffffffull);
-  // kScanTiles tiles of BT leaves share one block scan (counts packed in 16-bit fields)
-  for (int64_t t0 = lo; t0 < hi; t0 += kScanTiles * BT) {
+  int* const fcounter = fkey != nullptr ? &s->nfront[0] : nullptr;
+  // kScanTiles tiles of BT leaves share one block scan (counts packed in 12-bit fields)
+  for (int64_t t0 = lo; t0 < hi; t0 += kGroup) {
     uint64_t keyq[kScanTiles];
     int actq[kScanTiles];
     unsigned long long packed = 0;
@@ -226,30 +267,28 @@ __global__ void __launch_bounds__(BT) k_adapt_scatter(Geo g, const uint64_t* __r
         keyq[q] = keys[i];
         actq[q] = adapt_action<DIM>(g, keys, flags, i, n, keyq[q]);
       }
-      packed |= (unsigned long long)(actq[q] == ACT_REFINE ? NC : (actq[q] == ACT_DROP ? 0 : 1)) << (16 * q);
+      packed |= (unsigned long long)(actq[q] == ACT_REFINE ? NC : (actq[q] == ACT_DROP ? 0 : 1)) << (kFieldBits * q);
+      // a refined leaf (GROUP entry) and a merged parent (SELF entry) go to lt_balance's first frontier
+      if (fcounter != nullptr && (actq[q] == ACT_REFINE || actq[q] == ACT_PARENT)) packed += 1ull << kFrShift;
     }
     unsigned long long tile_total;
-    const unsigned long long ex = block_excl_scan<unsigned long long>(packed, sm, &tile_total);
+    int fbase;
+    const unsigned long long ex = block_scan_reserve(packed, sm, &tile_total, fcounter, &fbase);
+    int64_t fat = (int64_t)fbase + (int64_t)(ex >> kFrShift);
 #pragma unroll
     for (int q = 0; q < kScanTiles; ++q) {
       const int act = actq[q];
       const uint64_t key = keyq[q];
-      const int64_t pos = run + (int64_t)((ex >> (16 * q)) & 0xffff);
-      run += (int64_t)((tile_total >> (16 * q)) & 0xffff);
-      if (fkey != nullptr) {  // warp-aggregated append (kFrGroup = 2, kFrSelf = 3 of k_balance)
-        const bool pg = act == ACT_REFINE, ps = act == ACT_PARENT;
-        const unsigned mm = __ballot_sync(0xffffffffu, pg || ps);
-        if (mm) {
-          const int ln = threadIdx.x & 31;
-          int base = 0;
-          if (ln == __ffs(mm) - 1) base = atomicAdd(&s->nfront[0], __popc(mm));
-          base = __shfl_sync(0xffffffffu, base, __ffs(mm) - 1);
-          const int64_t at = (int64_t)base + __popc(mm & ((1u << ln) - 1));
-          if ((pg || ps) && at < fcap) {  // (a list that does not fit makes lt_balance sweep in full)
-            fkey[at] = pg ? key : (uint64_t)pos;
-            ftag[at] = pg ? 2 : 3;
-          }
+      const int64_t pos = run + (int64_t)((ex >> (kFieldBits * q)) & kFieldMask);
+      run += (int64_t)((tile_total >> (kFieldBits * q)) & kFieldMask);
+      if (fcounter != nullptr && (act == ACT_REFINE || act == ACT_PARENT)) {
+        // (kFrGroup = 2: its own key, kFrSelf = 3: its position; any order.  A list that does not fit
+        // makes lt_balance sweep in full)
+        if (fat < fcap) {
+          fkey[fat] = act == ACT_REFINE ? key : (uint64_t)pos;
+          ftag[fat] = act == ACT_REFINE ? 2 : 3;
         }
+        ++fat;
       }
       if (act == ACT_DROP) continue;
       LT_DASSERT(pos >= 0 && pos + (act == ACT_REFINE ? NC : 1) <= n_out);
@@ -511,11 +550,13 @@ __device__ __noinline__ bool split_pass(const Geo& g, const uint64_t* __restrict
   constexpr int NC = Dim<DIM>::NC;
   bool fits = true;
   (void)n_new;
-  // kScanTiles tiles of BT leaves share one block scan: the counts (<= NC * BT < 2^16 per tile) are
-  // packed in 16-bit fields, and the loads of all tiles are issued before the first barrier (requesting
-  // the NEXT group's loads as well before the barriers was tried: slower, 0.34 -> 0.40-0.43 ms for the
-  // three splitting sweeps of config-5 cycle 3, because of the registers it takes)
-  for (int64_t t0 = lo; t0 < hi; t0 += kScanTiles * BT) {
+  // kScanTiles tiles of BT leaves share one block scan: the counts (<= NC * BT = 2^11 per tile) are
+  // packed in 12-bit fields, the frontier entries of the group in the top field (block_scan_reserve).
+  // Requesting the NEXT group's loads into registers before the barriers was tried: slower, 0.34 ->
+  // 0.40-0.43 ms for the three splitting sweeps of config-5 cycle 3, because of the registers it takes;
+  // so was a cp.async prefetch of the next group into shared memory, which takes no registers (0.52 ->
+  // 0.54 ms, and 0.37 -> 0.38 ms in k_adapt_scatter): the pass does not wait for its loads.
+  for (int64_t t0 = lo; t0 < hi; t0 += kGroup) {
     uint64_t key[kScanTiles];
     unsigned mk[kScanTiles];
     unsigned long long packed = 0;
@@ -534,23 +575,31 @@ __device__ __noinline__ bool split_pass(const Geo& g, const uint64_t* __restrict
       const int64_t i = t0 + q * BT + threadIdx.x;
       if (i < hi) {
         if (mk[q]) mark[i] = 0;
-        packed |= (unsigned long long)((mk[q] & 1) ? NC : 1) << (16 * q);
+        packed |= (unsigned long long)((mk[q] & 1) ? NC : 1) << (kFieldBits * q);
+        // a split leaf becomes a GROUP entry; an unsplit leaf that saw a neighbour >= 3 levels coarser
+        // (full sweep) a LEAF entry
+        if (emit && (mk[q] & 3)) packed += 1ull << kFrShift;
       }
     }
     unsigned long long tile_total;
-    const unsigned long long ex = block_excl_scan<unsigned long long>(packed, sm, &tile_total);
+    int fbase;
+    const unsigned long long ex = block_scan_reserve(packed, sm, &tile_total, emit ? fcount : nullptr, &fbase);
+    int64_t fat = (int64_t)fbase + (int64_t)(ex >> kFrShift);
+    fits = fits && (int64_t)fbase + (int64_t)(tile_total >> kFrShift) <= fcap;
 #pragma unroll
     for (int q = 0; q < kScanTiles; ++q) {
       const int64_t i = t0 + q * BT + threadIdx.x;
-      const int64_t pos = run + (int64_t)((ex >> (16 * q)) & 0xffff);
-      run += (int64_t)((tile_total >> (16 * q)) & 0xffff);
-      if (emit) {
-        // a split leaf becomes a GROUP entry; an unsplit leaf that saw a neighbour >= 3 levels coarser
-        // (full sweep) a LEAF entry
-        const bool pg = (mk[q] & 1) != 0, pl = !pg && (mk[q] & 2) != 0;
-        fits = frontier_push(pg || pl, key[q], pg ? kFrGroup : kFrLeaf, fk_out, ft_out, fcount, fcap) && fits;
-      }
+      const int64_t pos = run + (int64_t)((ex >> (kFieldBits * q)) & kFieldMask);
+      run += (int64_t)((tile_total >> (kFieldBits * q)) & kFieldMask);
       if (i >= hi) continue;
+      if (emit && (mk[q] & 3)) {
+        LT_DASSERT(fat >= 0);
+        if (fat < fcap) {
+          fk_out[fat] = key[q];
+          ft_out[fat] = (uint8_t)((mk[q] & 1) ? kFrGroup : kFrLeaf);
+        }
+        ++fat;
+      }
       LT_DASSERT(pos >= 0 && pos + ((mk[q] & 1) ? NC : 1) <= n_new);
       const int l = key_level(key[q]);
       const uint64_t m = key_morton(key[q]);
@@ -581,7 +630,7 @@ __device__ __forceinline__ unsigned long long global_ns() {
 template <int DIM>
 __global__ void __launch_bounds__(BT, 4) k_balance(BalanceArgs a) {
   constexpr int NC = Dim<DIM>::NC;
-  __shared__ unsigned long long sm[33];
+  __shared__ unsigned long long sm[34];
   __shared__ uint8_t s_dirs[20], s_gdirs[26];
   cg::grid_group grid = cg::this_grid();
   const Geo g = a.g;
@@ -704,14 +753,75 @@ __global__ void __launch_bounds__(BT, 4) k_balance(BalanceArgs a) {
   // ---- Alg. 7: T_old -> the balanced tree, in new-leaf order.  A new leaf more
   // than one level from T_old only raises map_bad here: lt_transfer then runs the checked k_map,
   // which reports LT_ERR_MAPPING where the header says it is reported.
+  // The map is monotone (both arrays ascend), so the old leaves that a tile of consecutive new leaves
+  // maps to are one contiguous range: its two ends are located by the bucketed search (all tiles of a
+  // batch side by side), the range is copied to shared memory and every new leaf searches there -- one
+  // dependent chain of global probes per TILE instead of one per leaf.  A range that does not fit (a
+  // tile made of merged parents only can span 2^dim old leaves per new one) takes the per-leaf search.
   if (a.do_map && !err) {
     const uint64_t* keys = a.keys[par];
     bool bad = false;
-    for (int64_t j = gtid; j < n; j += gsize) {
-      int o, kd;
-      bad = !map_entry<DIM>(g, keys[j], a.keys_old, a.first_old, a.n_old, &o, &kd) || bad;
-      a.map_src[j] = o;
-      a.map_kind[j] = (uint8_t)kd;
+    constexpr int kWin = 2 * kGroup;  // old keys per window
+    __shared__ uint64_t win[kWin];
+    __shared__ int s_b[BT + 1];
+    int64_t lo, hi;
+    block_chunk(n, G, blockIdx.x, BT, &lo, &hi);
+    for (int64_t b0 = lo; b0 < hi; b0 += (int64_t)BT * kGroup) {
+      const int64_t bh = b0 + (int64_t)BT * kGroup < hi ? b0 + (int64_t)BT * kGroup : hi;
+      const int nt = (int)((bh - b0 + kGroup - 1) / kGroup);
+      __syncthreads();  // (s_b and the window of the previous batch are no longer read)
+      for (int k = threadIdx.x; k <= nt; k += BT) {
+        const int64_t j = b0 + (int64_t)k * kGroup < bh ? b0 + (int64_t)k * kGroup : bh - 1;
+        s_b[k] = locate(g, a.keys_old, a.first_old, key_morton(keys[j]));
+      }
+      __syncthreads();
+      for (int k = 0; k < nt; ++k) {
+        const int64_t t0 = b0 + (int64_t)k * kGroup;
+        const int o0 = s_b[k];
+        int w = s_b[k + 1] + NC - o0;  // (+ NC: the last sibling of a merged group is looked at)
+        if (w > a.n_old - o0) w = a.n_old - o0;
+        const bool in_smem = w <= kWin;
+        if (in_smem)
+          for (int x = threadIdx.x; x < w; x += BT) win[x] = a.keys_old[o0 + x];
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < kScanTiles; ++q) {
+          const int64_t j = t0 + q * BT + threadIdx.x;
+          if (j >= bh) continue;
+          const uint64_t key = keys[j];
+          int o, kd;
+          if (!in_smem) {
+            bad = !map_entry<DIM>(g, key, a.keys_old, a.first_old, a.n_old, &o, &kd) || bad;
+          } else {
+            // map_entry on the window: last old key with morton <= the new leaf's (Eq. 7)
+            const int l = key_level(key);
+            const uint64_t m = key_morton(key);
+            const uint64_t bound = (m << kLevelBits) | kLevelMask;
+            int a0 = 0, a1 = w;
+            while (a1 - a0 > 1) {
+              const int mid = (a0 + a1) >> 1;
+              if (win[mid] <= bound) a0 = mid; else a1 = mid;
+            }
+            LT_DASSERT(win[a0] <= bound);
+            const int lv = key_level(win[a0]);
+            kd = 0;
+            if (lv == l - 1) {
+              kd = 1 | (child_id<DIM>(g, m, l) << 4);
+            } else if (lv == l + 1) {
+              const int sh = DIM * (g.maxl - l - 1);
+              const uint64_t klast = make_key(m | ((uint64_t)(NC - 1) << sh), l + 1);
+              if (a0 + NC - 1 >= w || win[a0 + NC - 1] != klast) bad = true;
+              kd = 2;
+            } else if (lv != l) {
+              bad = true;
+            }
+            o = o0 + a0;
+          }
+          a.map_src[j] = o;
+          a.map_kind[j] = (uint8_t)kd;
+        }
+        __syncthreads();
+      }
     }
     if (bad) a.s->map_bad = 1;
   }
@@ -762,6 +872,20 @@ int launch_check_tiling(Tree* t) {
   t->launches++;
   LT_CUDA(cudaGetLastError());
   return LT_OK;
+}
+
+// Grid of the two adapt passes (they share the chunking): as many blocks as k_adapt_scatter keeps resident,
+// so that its chunks run as ONE wave (a grid of 8 blocks per SM ran 1.6 waves at its 5 resident blocks).
+int adapt_grid(const Tree* t) {
+  int per_sm = 0;
+  cudaError_t e = t->g.dim == 2
+                      ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_adapt_scatter<2>, BT, 0)
+                      : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_adapt_scatter<3>, BT, 0);
+  if (e != cudaSuccess || per_sm < 1) {
+    (void)cudaGetLastError();
+    per_sm = 4;
+  }
+  return grid_for(t, per_sm > 8 ? 8 : per_sm);
 }
 
 int launch_adapt_count(Tree* t, const int8_t* d_flags, int G) {

@@ -437,3 +437,46 @@ def test_deferred_balance_reports_a_mapping_error_through_the_status():
         gt.sync()
     assert ei.value.status == lt.LT_ERR_MAPPING
     assert gt.num_leaves() == 932
+
+
+@pytest.mark.parametrize("base,maxl,p,nvars,recipes", [
+    (2, 5, 1, 2, ["refine"] * 3 + ["coarsen", "mixed", "coarsen_half", "mixed"]),
+    (4, 7, 0, 1, ["refine"] * 3 + ["coarsen", "mixed"]),
+])
+def test_map_from_the_window_and_from_the_per_leaf_search(base, maxl, p, nvars, recipes):
+    """Alg. 7 in the tail of lt_balance locates a tile of 1024 new leaves in a shared-memory window of
+    2048 old keys and falls back to the per-leaf bucketed search when the tile's old range does not fit (a
+    tile of merged parents spans 2^dim old leaves per new one).  The small case stays inside the window;
+    coarsen-everything on a uniform 128^3 tree (262 144 parents of 2 097 152 leaves: 512 parents per block
+    chunk, 4096 old keys per tile) takes the fallback in every tile, the mixed cycle after it both.  Map,
+    keys and the transferred solution must be the oracle's either way."""
+    dim = 3
+    gt = lt.Tree(dim, base, maxl, None, (1, 0, 1))
+    ot = oracle.Tree(dim, base, maxl, (1, 0, 1))
+    rng = np.random.default_rng(7)
+    uo = rng.uniform(-1, 1, (ot.num_leaves(), nvars, (p + 1) ** dim))
+    for c, what in enumerate(recipes):
+        n = ot.num_leaves()
+        lvl, xyz = ot.leaf_boxes()
+        if what == "refine":
+            f = np.ones(n, np.int8)
+        elif what == "coarsen":
+            f = -np.ones(n, np.int8)
+        elif what == "coarsen_half":
+            f = np.where(xyz[:, 0] < (1 << (maxl - 1)), -1, 0).astype(np.int8)
+        else:
+            f = rng.choice(np.array([-1, 0, 1], np.int8), size=n, p=[0.5, 0.3, 0.2])
+        ot.adapt(f)
+        gt.adapt(torch.from_numpy(f).cuda())
+        assert gt.balance() == ot.balance(), "cycle %d" % c
+        P.assert_keys_equal(gt, ot, "cycle %d (%s)" % (c, what))
+        src_o, kind_o = ot.build_map()
+        un_o = ot.transfer_rows(uo, p, nvars, 0, ot.num_leaves())
+        ot.drop_snapshot()
+        un_g = gt.transfer(torch.from_numpy(uo).cuda(), p, nvars)
+        gt.sync()
+        src_g, kind_g = gt.map()
+        assert np.array_equal(src_g.cpu().numpy(), src_o), "cycle %d (%s): map src" % (c, what)
+        assert np.array_equal(kind_g.cpu().numpy(), kind_o), "cycle %d (%s): map kind" % (c, what)
+        P.assert_u_close(un_g, un_o, "cycle %d (%s)" % (c, what))
+        uo = un_o
