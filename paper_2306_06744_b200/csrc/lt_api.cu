@@ -593,6 +593,7 @@ int lt_adapt(lt_tree* t, const int8_t* d_flags) {
     t->map_ready = false;
     t->faces_valid = false;
     t->front_ok = emit != 0;
+    t->front_conn = t->balanced_conn;
     t->balanced_conn = 0;
     toc(t, 0);
     return LT_OK;
@@ -654,6 +655,7 @@ int lt_adapt(lt_tree* t, const int8_t* d_flags) {
   t->map_ready = false;
   t->faces_valid = false;
   t->front_ok = front_ok;
+  t->front_conn = t->balanced_conn;
   t->balanced_conn = 0;
   toc(t, 0);
   return LT_OK;
@@ -694,7 +696,9 @@ int lt_balance(lt_tree* t, int* iters) {
     // (testing aid: pretend the buffers hold only n + slack leaves, to exercise the retry)
     const int64_t cap_told = slack > 0 && t->n + slack < t->cap ? t->n + slack : t->cap;
     const int conn = t->opt_balance_conn > 0 ? t->opt_balance_conn : 1;
-    const int use_front = attempt == 0 && had_front && conn == 1 && !t->opt_full_sweeps;
+    // (lt_adapt's list is the whole first frontier only if the tree it adapted was balanced with at least
+    // this connectivity)
+    const int use_front = attempt == 0 && had_front && conn <= t->front_conn && !t->opt_full_sweeps;
     if ((rc = launch_balance(t, cap_told, use_front)) != LT_OK) return rc;
     if ((rc = fetch_scalars(t)) != LT_OK) return rc;
     if (t->h_s->parity) {

@@ -89,6 +89,7 @@ struct Tree {
   cudaEvent_t ev_side_fork, ev_side_join;
   bool connect_pending;
   int balanced_conn;      // the tree is 2:1 balanced with this connectivity (0: unknown)
+  int front_conn;         // balanced_conn of the tree the last lt_adapt started from
   bool front_ok;          // fkey[0] / ftag[0] / d_s->nfront[0] list the leaves created by the last lt_adapt
   int* mortar_hits;       // [hits][2 + 2^(dim-1)]: coarse-side hanging faces (e, f, fine neighbours)
   int64_t mortar_hits_cap;

@@ -490,26 +490,36 @@ __device__ __forceinline__ int examine_group(const Geo& g, const uint64_t* __res
   return lj < l - 1 ? 2 : 1;
 }
 
-// A parent created by lt_adapt (level l, position i) is too coarse iff, across one of its faces, a
-// level-(l+1) cell of the neighbouring level-l cell is itself subdivided (its leaves are >= 2 levels
-// finer).  Checked from the parent's side for face f; marks the parent itself.
+// A parent created by lt_adapt (level l, position i) is too coarse iff, in one of the neighbour directions
+// of the balance (`code`: 2 bits per axis, 1 = minus, 2 = plus; faces, and edges / corners for the strong
+// balance), a level-(l+1) cell of the neighbouring level-l cell that touches the parent is itself
+// subdivided (its leaves are >= 2 levels finer).  Those cells have, on every moved axis, the child bit of
+// the side facing the parent and any bit on the other axes: 2^(dim - moves) searches.  Checked from the
+// parent's side; marks the parent itself.
 template <int DIM>
 __device__ __forceinline__ void examine_self(const Geo& g, const uint64_t* __restrict__ keys,
                                              const int* __restrict__ first, uint8_t* mark, int* cmarks, int per,
-                                             int i, int f) {
+                                             int i, int code) {
   const uint64_t key = keys[i];
   const int l = key_level(key);
   if (l + 2 > g.maxl) return;
-  const int a = f >> 1, side = f & 1;
   uint64_t mn;
-  if (!face_neighbour<DIM>(g, key_morton(key), l, f, &mn)) return;
+  if (!move_cell<DIM>(g, key_morton(key), l, code, &mn)) return;
+  int facing = 0, nfree = 0;
+#pragma unroll
+  for (int a = 0; a < DIM; ++a) {
+    const int c = (code >> (2 * a)) & 3;
+    if (c == 1) facing |= 1 << a;  // moved to the minus side: the neighbour's plus-side children touch
+    nfree += c == 0;
+  }
   bool hit = false;
 #pragma unroll
   for (int sidx = 0; sidx < (1 << (DIM - 1)); ++sidx) {
-    int c = side ? 0 : (1 << a), bit = 0;
+    if (sidx >= (1 << nfree)) break;
+    int c = facing, bit = 0;
 #pragma unroll
     for (int b = 0; b < DIM; ++b) {
-      if (b == a) continue;
+      if ((code >> (2 * b)) & 3) continue;
       c |= ((sidx >> bit) & 1) << b;
       ++bit;
     }
@@ -692,7 +702,7 @@ __global__ void __launch_bounds__(BT, 4) k_balance(BalanceArgs a) {
         int r = 0;
         if (tag == kFrGroup) r = examine_group<DIM>(g, keys, first, a.mark, cm, per, key, s_gdirs[d]);
         else if (tag == kFrLeaf) r = d < a.ndirs ? examine_leaf<DIM>(g, keys, first, a.mark, cm, per, key, s_dirs[d]) : 0;
-        else if (d < 2 * DIM) examine_self<DIM>(g, keys, first, a.mark, cm, per, (int)key, d);  // only in sweep 1
+        else examine_self<DIM>(g, keys, first, a.mark, cm, per, (int)key, s_gdirs[d]);  // only in sweep 1
         if (r == 2) atomicOr((unsigned*)(ft + (e & ~3)), (unsigned)kFrAgain << (8 * (e & 3)));
       }
     }

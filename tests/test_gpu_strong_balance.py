@@ -88,6 +88,34 @@ def test_cycles_with_strong_balance(conn):
         uo = un_o
 
 
+@pytest.mark.parametrize("dim,base,maxl,periodic,conn", [(2, 2, 8, (1, 0), 2), (3, 1, 6, (1, 1, 1), 2),
+                                                         (3, 2, 6, (0, 0, 0), 3), (3, 1, 6, (0, 1, 0), 3)])
+def test_strong_balance_after_adapt_uses_the_adapt_frontier(dim, base, maxl, periodic, conn):
+    # a tree balanced with connectivity `conn` is adapted: the first sweep of the next strong balance looks only
+    # at the leaves lt_adapt created -- refined leaves as GROUP entries over the 18 / 26 directions, merged
+    # parents from their own side across faces, edges and corners.  Coarsening-heavy and refining-heavy
+    # random flags in turn; trees, sweep counts and faces must be the oracle's and the full sweeps'.  A
+    # balance with a STRONGER connectivity than the tree was last balanced with must not use the list.
+    rng = np.random.default_rng(dim * 1000 + conn * 10 + maxl)
+    dom = [0.0] * dim + [1.0] * dim
+    gt, gf = lt.Tree(dim, base, maxl, dom, periodic), lt.Tree(dim, base, maxl, dom, periodic)
+    gf.set_option(lt.LT_OPT_BALANCE_FULL_SWEEPS, 1)
+    ot = oracle.Tree(dim, base, maxl, periodic)
+    for c in range(10):
+        pr = [0.55, 0.33, 0.12] if c % 2 else [0.25, 0.45, 0.30]
+        f = rng.choice(np.array([-1, 0, 1], np.int8), size=ot.num_leaves(), p=pr)
+        # cycle 6 balances across faces only, cycle 7 goes back to `conn`: its tree was balanced with
+        # connectivity 1, so lt_adapt's list is not enough and the first sweep must be a full one
+        k = 1 if c == 6 else conn
+        ot.adapt(f); it_o = ot.balance(k); ot.drop_snapshot()
+        for g in (gt, gf):
+            g.adapt(torch.from_numpy(f).cuda())
+            assert g.balance(k) == it_o, "cycle %d" % c
+            P.assert_keys_equal(g, ot, "cycle %d" % c)
+        if c in (3, 9):
+            P.assert_faces_equal(gt.connect(), ot.connect(), "cycle %d" % c)
+
+
 def test_construct_then_strong_balance():
     cfg = W.POINT_CLOUDS["pc3_small"]
     pts = W.surface_points(cfg).numpy()
