@@ -240,6 +240,70 @@ def cpu_baseline(name, cfg, full=False):
             "which": "oracle-full" if full else "default (bounded)"}
 
 
+def profile_traffic(kernel):
+    """(DRAM bytes per launch under ncu, algorithmic bytes of that launch) of a kernel, from
+    profiles/traffic.txt ("<kernel> <dram bytes> <algorithmic bytes>"), or (None, None)."""
+    try:
+        for line in open(os.path.join(ROOT, "profiles", "traffic.txt")):
+            w = line.split()
+            if len(w) >= 3 and w[0] == kernel:
+                return int(w[1]), int(w[2])
+    except Exception:
+        pass
+    return None, None
+
+
+def oracle_solver_share(name="slab", prep=8):
+    """cpu_baseline of --workload solver: the oracle, as it stands, on the paper's own 3-D domain (the slab
+    config: 16 x 16 x 1 root cubes, p = 2): cycles 0..prep-1 replayed untimed, cycle `prep` timed in full
+    (adapt, balance, connect, transfer), then ONE SSP-RK3 step (three times Alg. 8 steps 1-4, Eq. 2-5 and
+    Eq. 6) timed on the adapted mesh and counted ten times -- the same metric, the adaptation share of
+    wall clock at one adaptation per ten steps."""
+    import numpy as np
+    import torch
+    import oracle
+    from paper_2306_06744_b200 import workloads as W
+    cfg = W.CONFIGS[name]
+    p, nvars = cfg["p"], cfg["nvars"]
+    lo, cube, nroot = W.geometry(cfg)
+    width = [cube * n for n in nroot]
+    with PinnedThread() as pin:
+        ot = oracle.Tree(cfg["dim"], cfg["base"], cfg["maxl"], cfg["periodic"], nroot=cfg.get("nroot"))
+        for c in range(prep + 1):
+            lvl, xyz = ot.leaf_boxes()
+            L, X = torch.from_numpy(lvl), torch.from_numpy(xyz.astype(np.int64))
+            f = W.flags(cfg, c, L, X).numpy()
+            if c < prep:
+                ot.adapt(f); ot.balance(); ot.drop_snapshot()
+                continue
+            u = W.initial_solution(cfg, L, X).numpy()
+            m0 = ot.num_leaves()
+            t0 = time.perf_counter()
+            ot.adapt(f); ot.balance(); ot.connect()
+            u = ot.transfer(u, p, nvars)
+            t_adapt = time.perf_counter() - t0
+        m1 = ot.num_leaves()
+        dt = 5e-4
+
+        def rhs(x):
+            uf = ot.face_interp(x, p, nvars)
+            fs = ot.common_flux(uf, ot.mortar_project(uf, p, nvars), p)
+            fs = np.where(np.isnan(fs), ot.mortar_gather(fs, p, nvars), fs)
+            return ot.fr_rhs(x, fs, p, width)
+        t0 = time.perf_counter()
+        u1 = oracle.rk3_stage(1, dt, u, u, rhs(u))
+        u2 = oracle.rk3_stage(2, dt, u, u1, rhs(u1))
+        u3 = oracle.rk3_stage(3, dt, u, u2, rhs(u2))
+        t_step = time.perf_counter() - t0
+        assert np.isfinite(u3).all()
+    return {"value": t_adapt / (t_adapt + 10 * t_step), "unit": "fraction", "cores": 1, "kind": "oracle",
+            "sample": "%s cycle %d in full (%d -> %d elements, p=%d) + one SSP-RK3 step timed and counted ten times"
+                      % (name, prep, m0, m1, p),
+            "seconds": t_adapt + t_step, "seconds_per_call": {"adaptation_cycle": t_adapt, "one_rk3_step": t_step},
+            "elements_per_s_rhs": 3 * m1 / t_step, "pinned_to_cpu": pin.cpu, "cpu_model": cpu_model(),
+            "host_cores_available": os.cpu_count()}
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle timed on the box's host cores (tier rule 4), one pinned thread,
     on the sample of --config's workload that cpu_baseline() names; a step = that sample once."""
@@ -495,15 +559,11 @@ def run_ours(args):
     tr_ms = sum(s["tm"]["k_transfer"] for s in steps)
     achieved = tr_bytes / (tr_ms * 1e-3) / 1e9
     traffic = traffic_note = None
-    try:  # profiles/traffic.txt: "<kernel> <dram bytes per launch> <algorithmic bytes of that launch>"
-        for line in open(os.path.join(ROOT, "profiles", "traffic.txt")):
-            w = line.split()
-            if len(w) >= 3 and w[0] == "k_transfer" and CONFIG == "c5":
-                traffic = int(w[1])
-                traffic_note = ("ncu --set full of the config-5 cycle-3 launch (profiles/, see traffic.txt); "
-                                "algorithmic bytes of that launch: %d" % int(w[2]))
-    except Exception:
-        pass
+    if CONFIG == "c5":
+        traffic, alg = profile_traffic("k_transfer")
+        if traffic is not None:
+            traffic_note = ("ncu --set full of the config-5 cycle-3 launch (profiles/, see traffic.txt); "
+                            "algorithmic bytes of that launch: %d" % alg)
     alone_GBps = None
     if alone:
         ab = sum(algorithmic_bytes(cfg["dim"], s["M0"], s["Ma"], s["M1"], s["faces"], Bu, s["iters"])["transfer"]
@@ -874,6 +934,28 @@ def run_mortar(args):
         dt = time.perf_counter() - t0
         cpu = {"value": ot.num_leaves() * nf / dt, "unit": "face slots/s", "cores": 1, "kind": "oracle", "seconds": dt,
                "sample": "config-5 mesh after cycle 0 (%d leaves): project + gather" % ot.num_leaves()}
+    e2e = None
+    if not args.no_e2e:   # the same step with the face array coming from, and the result going to, pinned host memory
+        h_in = torch.empty(uf.shape, dtype=torch.float64, pin_memory=True)
+        h_out = torch.empty(uf.shape, dtype=torch.float64, pin_memory=True)
+        h_in.copy_(uf)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ms_e = []
+        for _ in range(2):  # (the first run is the warm-up)
+            torch.cuda.synchronize(dev)
+            e0.record(stream)
+            uf.copy_(h_in, non_blocking=True)
+            t.mortar_project(uf, p, nvars, u_nb=out)
+            t.mortar_gather(uf, p, nvars, f_face=out)
+            h_out.copy_(out, non_blocking=True)
+            e1.record(stream)
+            torch.cuda.synchronize(dev)
+            ms_e.append(e0.elapsed_time(e1))
+        e2e = {"value": M * nf / (ms_e[-1] * 1e-3), "unit": "face slots/s", "h2d_bytes_per_step": uf.numel() * 8,
+               "d2h_bytes_per_step": out.numel() * 8, "ms_per_step": ms_e[-1],
+               "note": "face array uploaded from, result downloaded to pinned host memory inside the timed step"}
+        del h_in, h_out
+    traffic, traffic_alg = profile_traffic("k_mortar_project")
     print(json.dumps({
         "metric": "face slots/s through lt_mortar_project + lt_mortar_gather (Alg. 8 steps 2 and 4)",
         "value": M * nf / ((ms_p + ms_g) * 1e-3), "unit": "face slots/s", "n_gpus": 1, "steps": args.steps,
@@ -888,10 +970,13 @@ def run_mortar(args):
                         "frac": bytes_i / (ms_i * 1e-3) / 1e9 / peak,
                         "note": "Alg. 8 step 1, timed before the mortar step; not part of `value`"},
         "roofline": {"bound": "hbm", "kernel": "k_mortar_project<3>", "achieved": ach, "peak": peak, "unit": "GB/s",
-                     "frac": ach / peak, "traffic": None, "peak_source": peak_src, "bytes_per_launch": bytes_p,
+                     "frac": ach / peak, "traffic": traffic, "traffic_note": None if traffic is None else
+                     "ncu --set full of one launch on the same mesh (profiles/r1f_mortar_full.md, traffic.txt); "
+                     "algorithmic bytes of that launch: %d" % traffic_alg,
+                     "peak_source": peak_src, "bytes_per_launch": bytes_p,
                      "gather_GBps": bytes_g / (ms_g * 1e-3) / 1e9, "gather_bytes_per_launch": bytes_g},
         "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": 4 * args.steps,
-        "e2e": None}), flush=True)
+        "e2e": e2e}), flush=True)
 
 
 # --------------------------------------------------------------------------- solver leg
@@ -929,12 +1014,19 @@ def run_solver(args):
         torch.cuda.synchronize(dev)
         return e0.elapsed_time(e1), out
 
-    def adapt_cycle():
-        """untimed set-up of the pre-adaptation state, then the timed cycle 2"""
+    def adapt_cycle(host_u_old=None):
+        """untimed set-up of the pre-adaptation state, then the timed cycle 2; host_u_old: (e2e) the old
+        solution starts in pinned host memory and its upload is part of the timed cycle (None on the
+        first call of that mode, which creates the pinned copy untimed and returns it)"""
         M0 = R.prepare()
         t = R.tree
         u_old = torch.empty((M0, nvars, N), dtype=torch.float64, device=dev)
-        R.analytic_u(u_old)
+        if host_u_old is None or host_u_old is True:
+            R.analytic_u(u_old)
+        if host_u_old is True:
+            host_u_old = torch.empty(u_old.shape, dtype=torch.float64, pin_memory=True)
+            host_u_old.copy_(u_old)
+            u_old.zero_()
         f = R.flags(PREP_CYCLES)
         # a small mesh (the paper's sizes): buffers for the worst case, so that the cycle has one host wait
         small = (M0 << 3) * (160 + 8 * nvars * N) < (8 << 30)
@@ -944,6 +1036,8 @@ def run_solver(args):
             buf = torch.empty(((M0 << 3) + 4096, nvars, N), dtype=torch.float64, device=dev)
 
         def cyc():
+            if host_u_old is not None:
+                u_old.copy_(host_u_old, non_blocking=True)
             t.adapt(f)
             if small:
                 t.balance(want_iters=False)
@@ -963,6 +1057,11 @@ def run_solver(args):
         return ms, M0, u_new.contiguous(), F
 
     adapt_cycle()                                  # warm-up (allocations, operators)
+    ms_adapt_e2e = h2d = None
+    if not args.no_e2e:                            # the same cycle with u_old coming from pinned host memory
+        ms_adapt_e2e, M0e, ue, _ = adapt_cycle(host_u_old=True)
+        h2d = M0e * 8 * nvars * N
+        del ue
     ms_adapt, M0, u, F = adapt_cycle()
     t = R.tree
     M = t.num_leaves()
@@ -1011,6 +1110,19 @@ def run_solver(args):
     clocks = sampler.stop()
     ms_solve = min(ms_solve, ms_solve2)
     assert bool(torch.isfinite(u).all()), "the solution blew up"
+    e2e = None
+    if ms_adapt_e2e is not None:                   # ten steps and the result back in pinned host memory
+        h_u = torch.empty(u.shape, dtype=torch.float64, pin_memory=True)
+        ms_solve_e2e, _ = timed(lambda: ([rk3_step() for _ in range(10)], h_u.copy_(u, non_blocking=True)))
+        e2e = {"value": ms_adapt_e2e / (ms_adapt_e2e + ms_solve_e2e), "unit": "fraction",
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": u.numel() * 8,
+               "ms_per_step": ms_adapt_e2e + ms_solve_e2e, "ms_adaptation_cycle": ms_adapt_e2e,
+               "ms_ten_rk3_steps": ms_solve_e2e,
+               "note": "u_old uploaded from pinned host memory inside the timed cycle; the solution after the ten "
+                       "steps downloaded to pinned host memory inside the timed solve"}
+        del h_u
+    cpu = None if args.no_cpu_baseline else oracle_solver_share()
+    traffic, traffic_alg = profile_traffic("rk_stage") if (name == "c5" and fused) else (None, None)
     frac = ms_adapt / (ms_adapt + ms_solve)
     Bu, Bf = 8 * nvars * N, 8 * nvars * Nf
     # algorithmic bytes of one RK stage: face_interp (Bu + 6 Bf) + project (~2 * 6 Bf) + common flux (3 * 6 Bf)
@@ -1032,9 +1144,12 @@ def run_solver(args):
         "roofline": {"bound": "hbm", "kernel": "RK stage (face_flux, mortar_gather, fr_stage_faces)" if fused else
                      "RK stage (face_interp, mortar_project, common_flux, mortar_gather, fr_stage)", "achieved": bytes_stage * 30 / (ms_solve * 1e-3) / 1e9,
                      "peak": peak, "unit": "GB/s", "frac": bytes_stage * 30 / (ms_solve * 1e-3) / 1e9 / peak,
-                     "traffic": None, "peak_source": peak_src, "bytes_per_launch": bytes_stage},
+                     "traffic": traffic, "traffic_note": None if traffic is None else
+                     "stage 1 of the fused chain under ncu --set full (profiles/r2_solver.md, traffic.txt); "
+                     "algorithmic bytes of that stage: %d" % traffic_alg,
+                     "peak_source": peak_src, "bytes_per_launch": bytes_stage},
         "elements_per_s_rhs": M * 30 / (ms_solve * 1e-3),
-        "cpu_baseline": None, "clocks": clocks, "gpu_launches": (30 * 4 if fused else 30 * 6) + 6, "e2e": None}),
+        "cpu_baseline": cpu, "clocks": clocks, "gpu_launches": (30 * 4 if fused else 30 * 6) + 6, "e2e": e2e}),
         flush=True)
 
 def main():

@@ -572,8 +572,9 @@ int lt_adapt(lt_tree* t, const int8_t* d_flags) {
   if (!t->n_valid && (rc = fetch_scalars(t)) != LT_OK) return rc;
   bool front_ok = false;
   tic(t, 0);
-  if (t->adapt_G <= 0) t->adapt_G = adapt_grid(t);
-  const int G = t->adapt_G;
+  // (a grid of exactly the blocks k_adapt_scatter keeps resident -- 5 per SM, one wave instead of 1.6 --
+  // was measured: slower, 0.177 -> 0.193 ms under ncu; the smaller chunks of the larger grid balance better)
+  const int G = grid_for(t, 8);
   if ((rc = launch_adapt_count(t, d_flags, G)) != LT_OK) return rc;
   const int nc = 1 << t->g.dim;
   if (!t->opt_adapt_sort && t->cap >= nc * t->n) {

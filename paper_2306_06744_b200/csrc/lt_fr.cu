@@ -109,6 +109,33 @@ __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) 
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
+// ---- TMA (bulk asynchronous copy) plumbing: one lane arms an mbarrier with the byte count and issues
+// cp.async.bulk global -> shared; the copy engine signals the barrier when the bytes have landed.  The copy
+// does not go through the LSU / shared-memory data pipe that bounds these kernels.  Addresses and size
+// must be multiples of 16 bytes.
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+
 // The kernel for blocks of at most 16 entries per lane (2-D: every p; 3-D: p <= 3).  A warp keeps four
 // buffers: u, u_n, the element's 2 DIM common-flux blocks, and F.  The three inputs of the warp's NEXT
 // element are fetched by cp.async as soon as their buffer is dead -- u_n right after the accumulators
@@ -279,6 +306,10 @@ __global__ void __launch_bounds__(256, 2) k_fr_rhs(Geo g, const uint64_t* __rest
 // costing two); here only the six common-flux blocks of the element go through shared memory (prefetched
 // by cp.async), u and u_n of the warp's NEXT element are loaded into registers when the tail of the
 // current one begins, and the traces of u_out are reduced over the line's lanes by shuffles.
+// BULK: the element's six flux blocks are one contiguous run of 3840 bytes, fetched by ONE cp.async.bulk of
+// the warp's lane 0 onto the warp's own mbarrier instead of 15 LDGSTS per lane (BULK = false when the
+// caller's flux array is not 16-byte aligned).
+template <bool BULK>
 __global__ void __launch_bounds__(256, 2) k_fr_rhs_p3(const uint64_t* __restrict__ keys, const DevScalars* s,
                                                       const double* u, const double* fs, double* R, double w0,
                                                       double w1, double w2, const double* un, double ca, double cb,
@@ -286,10 +317,28 @@ __global__ void __launch_bounds__(256, 2) k_fr_rhs_p3(const uint64_t* __restrict
   constexpr int DIM = 3, P1 = 4, NV = 5, N = 64, Nf = 16, EV = 320, KN = 10, E = NV * Nf, FB = 6 * E;
   constexpr int CP = P1 + 2, CT = P1 * CP;
   constexpr unsigned FULL = 0xffffffffu;
-  extern __shared__ double sm_all[];  // [warps]: f*[FB]
+  extern __shared__ __align__(128) double sm_p3[];  // [warps]: f*[FB]
   __shared__ double sc[CT + 2 * P1];  // D'[i][0..3] | g_L'(z_i) | g_R'(z_i) per row, then l(-1), l(+1)
+  __shared__ uint64_t bars[8];        // one mbarrier per warp (BULK)
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  double* sfs = sm_all + (size_t)w * FB;
+  double* sfs = sm_p3 + (size_t)w * FB;
+  uint64_t* bar = &bars[w];
+  uint32_t phase = 0;
+  if (BULK && lane == 0) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  // the flux blocks of element `el` -> this warp's buffer (all lanes call it; the buffer must be dead)
+  auto fetch_fluxes = [&](int64_t el) {
+    if (BULK) {
+      if (lane == 0) {
+        mbar_arrive_expect_tx(bar, FB * 8);
+        bulk_g2s(sfs, fs + (size_t)el * FB, FB * 8, bar);
+      }
+    } else {
+      for (int i = lane; i < FB; i += 32) cp_async8(sfs + i, fs + (size_t)el * FB + i);
+    }
+  };
   {
     const FrConst& c = c_fr[P1 - 1];
     for (int t = threadIdx.x; t < CT + 2 * P1; t += blockDim.x) {
@@ -310,7 +359,7 @@ __global__ void __launch_bounds__(256, 2) k_fr_rhs_p3(const uint64_t* __restrict
   int64_t e = (int64_t)blockIdx.x * (blockDim.x >> 5) + w;
   double nu[KN], nn[KN];  // u and u_n of the element about to be processed
   if (e < n) {
-    for (int i = lane; i < FB; i += 32) cp_async8(sfs + i, fs + (size_t)e * FB + i);
+    fetch_fluxes(e);
 #pragma unroll
     for (int k = 0; k < KN; ++k) {
       nu[k] = __ldcs(u + (size_t)e * EV + lane + 32 * k);
@@ -326,8 +375,14 @@ __global__ void __launch_bounds__(256, 2) k_fr_rhs_p3(const uint64_t* __restrict
       uo[k] = nu[k];
       acc[k] = stage ? ca * nn[k] + cb * nu[k] : 0.0;
     }
-    cp_async_wait_all();
-    __syncwarp();
+    if (BULK) {
+      while (!mbar_try_wait(bar, phase)) {
+      }
+      phase ^= 1;
+    } else {
+      cp_async_wait_all();
+      __syncwarp();
+    }
     const int level = key_level(keys[e]);
     const double inv2l = (double)(1ull << level);
     const double wgt = stage ? cb * dt : 1.0;
@@ -400,7 +455,7 @@ __global__ void __launch_bounds__(256, 2) k_fr_rhs_p3(const uint64_t* __restrict
     }
     __syncwarp();
     if (e_next < n) {  // the flux blocks are dead: the next element's; its u and u_n go to registers
-      for (int i = lane; i < FB; i += 32) cp_async8(sfs + i, fs + (size_t)e_next * FB + i);
+      fetch_fluxes(e_next);
 #pragma unroll
       for (int k = 0; k < KN; ++k) {
         nu[k] = __ldcs(u + (size_t)e_next * EV + lane + 32 * k);
@@ -676,11 +731,15 @@ static int launch_fr_rhs_t(Tree* t, const double* d_u, const double* d_fs, doubl
     static int per_sm3 = 0;
     if (per_sm3 == 0) {
       int q = 0;
-      LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&q, k_fr_rhs_p3, 256, smem3));
+      LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&q, k_fr_rhs_p3<true>, 256, smem3));
       per_sm3 = q < 1 ? 1 : q;
     }
-    k_fr_rhs_p3<<<t->num_sms * per_sm3, 256, smem3, t->stream>>>(t->keys[t->cur], t->d_s, d_u, d_fs, d_R, w0, w1, w2,
-                                                                 d_un, ca, cb, dt, d_uf_out);
+    if ((reinterpret_cast<uintptr_t>(d_fs) & 15) == 0)  // cp.async.bulk needs 16-byte aligned addresses
+      k_fr_rhs_p3<true><<<t->num_sms * per_sm3, 256, smem3, t->stream>>>(t->keys[t->cur], t->d_s, d_u, d_fs, d_R, w0,
+                                                                         w1, w2, d_un, ca, cb, dt, d_uf_out);
+    else
+      k_fr_rhs_p3<false><<<t->num_sms * per_sm3, 256, smem3, t->stream>>>(t->keys[t->cur], t->d_s, d_u, d_fs, d_R, w0,
+                                                                          w1, w2, d_un, ca, cb, dt, d_uf_out);
     return LT_OK;
   }
   int warps = 8;

@@ -42,7 +42,6 @@ struct Tree {
   double domain[6];
   cudaStream_t stream;
   int device, num_sms;
-  int adapt_G = 0;        // grid of the adapt passes (adapt_grid), set at the first lt_adapt
 
   int64_t cap;            // leaf capacity of every per-leaf buffer
   uint64_t* keys[3];      // cur / old (snapshot) / tmp rotate through these
@@ -127,7 +126,6 @@ extern thread_local int g_last_cuda_error;
   } while (0)
 
 int grid_for(const Tree* t, int blocks_per_sm);
-int adapt_grid(const Tree* t);  // one resident wave of k_adapt_scatter
 // LT_OK iff the tree's device is the current one (kernels, constant-memory uploads and pool
 // allocations all go to the current device)
 int check_device(const Tree* t);

@@ -884,20 +884,6 @@ int launch_check_tiling(Tree* t) {
   return LT_OK;
 }
 
-// Grid of the two adapt passes (they share the chunking): as many blocks as k_adapt_scatter keeps resident,
-// so that its chunks run as ONE wave (a grid of 8 blocks per SM ran 1.6 waves at its 5 resident blocks).
-int adapt_grid(const Tree* t) {
-  int per_sm = 0;
-  cudaError_t e = t->g.dim == 2
-                      ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_adapt_scatter<2>, BT, 0)
-                      : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_adapt_scatter<3>, BT, 0);
-  if (e != cudaSuccess || per_sm < 1) {
-    (void)cudaGetLastError();
-    per_sm = 4;
-  }
-  return grid_for(t, per_sm > 8 ? 8 : per_sm);
-}
-
 int launch_adapt_count(Tree* t, const int8_t* d_flags, int G) {
   LT_DISPATCH_DIM(t, (k_adapt_count<2><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], d_flags, t->d_s, t->d_sums)),
                   (k_adapt_count<3><<<G, BT, 0, t->stream>>>(t->g, t->keys[t->cur], d_flags, t->d_s, t->d_sums)));
