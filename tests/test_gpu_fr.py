@@ -204,7 +204,7 @@ def test_full_step_conserves_mass_momentum_energy():
     assert float((integral(u3) - integral(un)).abs().max()) < 1e-13
 
 
-@pytest.mark.parametrize("dim,base,maxl", [(2, 2, 6), (3, 2, 4)])
+@pytest.mark.parametrize("dim,base,maxl", [(2, 2, 6), (3, 2, 4), (3, 4, 6), (2, 7, 9)])
 @pytest.mark.parametrize("p", [0, 1, 2, 3, 5, 7])
 def test_fused_face_pass_and_stage_with_traces(dim, base, maxl, p):
     """lt_face_flux (Alg. 8 steps 2 + 3 in one pass, a conforming face computed once for both sides) and
@@ -213,6 +213,8 @@ def test_fused_face_pass_and_stage_with_traces(dim, base, maxl, p):
     face traces of the stage result = the oracle's face_interp of the oracle's stage result."""
     if dim == 3 and p == 7:
         maxl = 3
+    if base > 2 and p not in (1, 3):
+        pytest.skip("the larger meshes (many tiles per block of the bulk-copy face pass) run p = 1 and 3 only")
     gt, ot, rng = adapted_pair(dim, (1,) * dim, 71 * dim + p, base, maxl, cycles=2)
     F = gt.connect(); ot.connect()
     assert int(F["n_hang"]) > 0
@@ -261,4 +263,13 @@ def test_fused_face_pass_and_stage_with_traces(dim, base, maxl, p):
         assert torch.equal(out2, out) and torch.equal(uf3, uf2) and uf3.data_ptr() == fs2.data_ptr()
         # and the plain right-hand side of the re-laid-out kernel
         close_rhs(gt.fr_rhs(d_u, fs, p), R_o, fs_full, ot, "fr_rhs (padded layout)")
+        if dim == 3 and p == 3 and stage == 2:
+            # the 3-D p = 3 kernel fetches an element's flux blocks by cp.async.bulk when the flux array is
+            # 16-byte aligned and by 8-byte cp.async otherwise: a flux array that starts 8 bytes into an
+            # allocation takes the second path and must give the same bits
+            raw = torch.empty(fs.numel() + 1, dtype=torch.float64, device="cuda")
+            fs_odd = raw[1:].view(fs.shape)
+            fs_odd.copy_(fs)
+            assert fs.data_ptr() % 16 == 0 and fs_odd.data_ptr() % 16 == 8
+            assert torch.equal(gt.fr_stage(stage, dt, torch.from_numpy(u_n).cuda(), d_u, fs_odd, p), out)
     gt.sync()
