@@ -992,27 +992,52 @@ int launch_mortar(Tree* t, int which, const double* d_in, double* d_out, int p, 
 // sum_i l_i(-1 | +1) u[e][v][.. i on the face's axis, n_t on the others ..].  One warp per leaf,
 // one variable at a time through shared memory; reads u once (coalesced), writes the nf face
 // blocks in full 128-bit sectors.  HBM-bound: Bu in, nf * Bf out per leaf.
-template <int DIM, int P1>
+// BULK (the element block is a multiple of 16 bytes and u is 16-byte aligned): the element arrives by ONE
+// cp.async.bulk of lane 0 onto the warp's mbarrier, into the other half of a double buffer while the
+// current element is being worked on -- no load or shared-memory store instruction, and the DRAM latency
+// of the next element hides behind the arithmetic and the stores of this one.
+template <int DIM, int P1, bool BULK>
 __global__ void __launch_bounds__(256) k_face_interp(const DevScalars* s, const double* __restrict__ u,
-                                                     double* __restrict__ uf, int nvars, int vec2) {
+                                                     double* __restrict__ uf, int nvars) {
   constexpr int NF = Dim<DIM>::NF;
   constexpr int N = DIM == 2 ? P1 * P1 : P1 * P1 * P1, Nf = DIM == 2 ? P1 : P1 * P1;
-  extern __shared__ double su_all[];  // [warps][nvars][N]: the whole element, staged once
+  extern __shared__ __align__(128) double su_all[];  // [warps][1 or 2][nvars][N]: the whole element, staged once
+  __shared__ uint64_t bars[8][2];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int EV = nvars * N, E = nvars * Nf;
-  double* su = su_all + (size_t)w * EV;
+  double* su0 = su_all + (size_t)w * EV * (BULK ? 2 : 1);
   const int64_t n = s->n;
   const int64_t nw = (int64_t)gridDim.x * (blockDim.x >> 5);
-  for (int64_t e = (int64_t)blockIdx.x * (blockDim.x >> 5) + w; e < n; e += nw) {
-    __syncwarp();
-    const double* src = u + (size_t)e * EV;
-    if (vec2) {
-      for (int i = lane; i < EV / 2; i += 32)
-        reinterpret_cast<double2*>(su)[i] = __ldcs(reinterpret_cast<const double2*>(src) + i);
-    } else {
-      for (int i = lane; i < EV; i += 32) su[i] = __ldcs(src + i);
+  int64_t e = (int64_t)blockIdx.x * (blockDim.x >> 5) + w;
+  uint32_t phase[2] = {0, 0};
+  int buf = 0;
+  auto fetch = [&](int b, int64_t el) {  // (lane 0)
+    mbar_arrive_expect_tx(&bars[w][b], (uint32_t)EV * 8u);
+    bulk_g2s(su0 + (size_t)b * EV, u + (size_t)el * EV, (uint32_t)EV * 8u, &bars[w][b]);
+  };
+  if (BULK) {
+    if (lane == 0) {
+      mbar_init(&bars[w][0], 1);
+      mbar_init(&bars[w][1], 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+      if (e < n) fetch(0, e);
     }
     __syncwarp();
+  }
+  for (; e < n; e += nw, buf ^= 1) {
+    __syncwarp();  // (the buffer about to be refilled was read in the previous iteration)
+    const double* su = su0;
+    if (BULK) {
+      if (lane == 0 && e + nw < n) fetch(buf ^ 1, e + nw);
+      while (!mbar_try_wait(&bars[w][buf], phase[buf])) {
+      }
+      phase[buf] ^= 1;
+      su = su0 + (size_t)buf * EV;
+    } else {
+      const double* src = u + (size_t)e * EV;
+      for (int i = lane; i < EV; i += 32) su0[i] = __ldcs(src + i);
+      __syncwarp();
+    }
     double* dst = uf + (size_t)e * NF * E;
     // one lane per LINE of P1 points along an axis: the line is read once and gives the trace on
     // the minus AND the plus face of that axis; consecutive lanes store consecutive doubles
@@ -1047,17 +1072,18 @@ template <int DIM, int P1>
 static int launch_face_interp_t(Tree* t, const double* d_u, double* d_uf, int nvars) {
   constexpr int N = DIM == 2 ? P1 * P1 : P1 * P1 * P1;
   int warps = 8;
-  const size_t per_warp = (size_t)nvars * N * sizeof(double);
+  // the copy engine needs 16-byte multiples: an even number of doubles per element, u 16-byte aligned
+  const bool bulk = ((nvars * N) % 2 == 0) && (((uintptr_t)d_u) & 15) == 0;
+  const size_t per_warp = (size_t)nvars * N * sizeof(double) * (bulk ? 2 : 1);
   while (warps > 1 && warps * per_warp > 64 * 1024) warps >>= 1;
   const size_t smem = warps * per_warp;
   if (smem > 200 * 1024) return LT_ERR_ARG;  // nvars * (p+1)^dim beyond one SM's shared memory
-  auto fn = k_face_interp<DIM, P1>;
+  auto fn = bulk ? k_face_interp<DIM, P1, true> : k_face_interp<DIM, P1, false>;
   LT_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int per_sm = 0;
   LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, warps * 32, smem));
   if (per_sm < 1) per_sm = 1;
-  const int vec2 = ((nvars * N) % 2 == 0) && (((uintptr_t)d_u) & 15) == 0;
-  fn<<<t->num_sms * per_sm, warps * 32, smem, t->stream>>>(t->d_s, d_u, d_uf, nvars, vec2);
+  fn<<<t->num_sms * per_sm, warps * 32, smem, t->stream>>>(t->d_s, d_u, d_uf, nvars);
   return LT_OK;
 }
 
