@@ -79,6 +79,7 @@ struct FrShape {
   static constexpr bool REG = KN <= 16;  // a lane's accumulators in registers: k_fr_rhs, else k_fr_rhs_big
   // doubles of shared memory per warp: u | u_n | F | the 2 DIM face blocks, or u | F | R
   static constexpr int PER_WARP = REG ? 3 * EV + 2 * DIM * NV * Nf : 3 * EV;
+  static constexpr int PER_WARP_EVEN = (PER_WARP + 1) & ~1;
 };
 
 // entry p of an element and axis a: index along the line, first point of the line, face-point index
@@ -121,7 +122,7 @@ template <int DIM, int P1>
 __global__ void __launch_bounds__(256, 2) k_fr_rhs(Geo g, const uint64_t* __restrict__ keys, const DevScalars* s,
                                                    const double* u, const double* fs, double* R,
                                                    double w0, double w1, double w2, const double* un, double ca,
-                                                   double cb, double dt, double* uf_out) {
+                                                   double cb, double dt, double* uf_out, int bulk) {
   // un == nullptr: R = right-hand side.  Otherwise the RK stage of Eq. 6 is applied on the fly:
   // R (= u_out) = ca * un + cb * (u + dt * rhs); u_out may be u or un (element-local access: a warp
   // prefetches only elements that it will write itself, later).
@@ -134,13 +135,14 @@ __global__ void __launch_bounds__(256, 2) k_fr_rhs(Geo g, const uint64_t* __rest
   constexpr int E = NV * Nf, FB = NF * E;  // one face block, all face blocks of an element
   constexpr int CP = P1 + 2;               // operator table: row i = D'[i][0..P1-1] | g_L'(z_i) | g_R'(z_i)
   constexpr int CT = P1 * CP;              // then l(-1)[0..P1-1] | l(+1)[0..P1-1]
-  extern __shared__ double sm_all[];       // [warps]: u[EV] | u_n[EV] | F[EV] | f*[FB]
+  // [warps]: f*[FB] | u[EV] | u_n[EV] | F[EV], every warp's part a multiple of 16 bytes (bulk-copy destinations)
+  extern __shared__ __align__(16) double sm_gen[];
   __shared__ double sc[CT + 2 * P1];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  double* su = sm_all + (size_t)w * S::PER_WARP;
+  double* sfs = sm_gen + (size_t)w * S::PER_WARP_EVEN;
+  double* su = sfs + FB;
   double* sn = su + EV;
   double* sF = sn + EV;
-  double* sfs = sF + EV;
   {
     const FrConst& c = c_fr[P1 - 1];
     for (int t = threadIdx.x; t < CT + 2 * P1; t += blockDim.x) {
@@ -157,19 +159,45 @@ __global__ void __launch_bounds__(256, 2) k_fr_rhs(Geo g, const uint64_t* __rest
   const int64_t n = s->n;
   const int64_t nw = (int64_t)gridDim.x * (blockDim.x >> 5);
   const bool stage = un != nullptr;
-  auto fetch = [&](double* dst, const double* src, int count) {
-    for (int i = lane; i < count; i += 32) cp_async8(dst + i, src + i);
+  // A block of the element is fetched by ONE cp.async.bulk of lane 0 (the copy engine: no LSU work, no
+  // shared-memory store instructions) when its size is a multiple of 16 bytes and its array 16-byte aligned
+  // (bulk bit 0: the flux blocks, always a multiple; bit 1: u and u_n, even EV only), else by 8-byte
+  // cp.async of every lane.  The bulk copies of one element -- issued at different times -- all arrive on
+  // the warp's mbarrier, whose phase completes when each has announced its bytes and delivered them.
+  const bool bulk_f = (bulk & 1) != 0, bulk_u = (bulk & 2) != 0;
+  __shared__ uint64_t bars[8];
+  uint64_t* bar = &bars[w];
+  uint32_t phase = 0;
+  if (bulk && lane == 0) {
+    mbar_init(bar, (bulk_f ? 1 : 0) + (bulk_u ? (stage ? 2 : 1) : 0));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncwarp();
+  auto fetch = [&](double* dst, const double* src, int count, bool by_bulk) {
+    if (by_bulk) {
+      if (lane == 0) {
+        mbar_arrive_expect_tx(bar, (uint32_t)count * 8u);
+        bulk_g2s(dst, src, (uint32_t)count * 8u, bar);
+      }
+    } else {
+      for (int i = lane; i < count; i += 32) cp_async8(dst + i, src + i);
+    }
   };
   int64_t e = (int64_t)blockIdx.x * (blockDim.x >> 5) + w;
   if (e < n) {
-    fetch(su, u + (size_t)e * EV, EV);
-    if (stage) fetch(sn, un + (size_t)e * EV, EV);
-    fetch(sfs, fs + (size_t)e * FB, FB);
+    fetch(su, u + (size_t)e * EV, EV, bulk_u);
+    if (stage) fetch(sn, un + (size_t)e * EV, EV, bulk_u);
+    fetch(sfs, fs + (size_t)e * FB, FB, bulk_f);
   }
   cp_async_commit();
   for (; e < n; e += nw) {
     const int64_t e_next = e + nw;
     cp_async_wait_all();
+    if (bulk) {
+      while (!mbar_try_wait(bar, phase)) {
+      }
+      phase ^= 1;
+    }
     __syncwarp();
     double acc[KN];
 #pragma unroll
@@ -177,8 +205,9 @@ __global__ void __launch_bounds__(256, 2) k_fr_rhs(Geo g, const uint64_t* __rest
       const int i = lane + 32 * k;
       acc[k] = (stage && (EV % 32 == 0 || i < EV)) ? ca * sn[i] + cb * su[i] : 0.0;
     }
-    if (stage && e_next < n) {  // (a lane overwrites only the entries of u_n that it has just read)
-      fetch(sn, un + (size_t)e_next * EV, EV);
+    if (stage && e_next < n) {  // (a lane overwrites only the entries of u_n that it has just read;
+      if (bulk_u) __syncwarp();  //  the copy engine overwrites all of them: every lane has to be done)
+      fetch(sn, un + (size_t)e_next * EV, EV, bulk_u);
       cp_async_commit();
     }
     const int level = key_level(keys[e]);
@@ -199,7 +228,7 @@ __global__ void __launch_bounds__(256, 2) k_fr_rhs(Geo g, const uint64_t* __rest
       }
       __syncwarp();
       if (a == DIM - 1 && e_next < n) {  // u is dead: bring in the next element's
-        fetch(su, u + (size_t)e_next * EV, EV);
+        fetch(su, u + (size_t)e_next * EV, EV, bulk_u);
         cp_async_commit();
       }
       const double* fsm = sfs + 2 * a * E;  // common flux on the - face: [v][nt]
@@ -223,7 +252,7 @@ __global__ void __launch_bounds__(256, 2) k_fr_rhs(Geo g, const uint64_t* __rest
     }
     __syncwarp();
     if (e_next < n) {  // the flux blocks are dead
-      fetch(sfs, fs + (size_t)e_next * FB, FB);
+      fetch(sfs, fs + (size_t)e_next * FB, FB, bulk_f);
       cp_async_commit();
     }
     double* dst = R + (size_t)e * EV;
@@ -481,7 +510,7 @@ template <int DIM, int P1>
 __global__ void __launch_bounds__(256) k_fr_rhs_big(Geo g, const uint64_t* __restrict__ keys, const DevScalars* s,
                                                     const double* u, const double* fs, double* R,
                                                     double w0, double w1, double w2, const double* un, double ca,
-                                                    double cb, double dt, double* uf_out) {
+                                                    double cb, double dt, double* uf_out, int /*bulk: unused*/) {
   using S = FrShape<DIM, P1>;
   constexpr int NF = Dim<DIM>::NF, NV = S::NV, N = S::N, Nf = S::Nf, EV = S::EV;
   constexpr int E = NV * Nf;
@@ -716,16 +745,20 @@ static int launch_fr_rhs_t(Tree* t, const double* d_u, const double* d_fs, doubl
     return LT_OK;
   }
   int warps = 8;
-  const size_t per_warp = (size_t)S::PER_WARP * sizeof(double);
+  const size_t per_warp = (size_t)S::PER_WARP_EVEN * sizeof(double);
   while (warps > 1 && warps * per_warp > 96 * 1024) warps >>= 1;
   const size_t smem = warps * per_warp;
+  // which inputs the copy engine may fetch (16-byte multiples at 16-byte aligned addresses): bit 0 the flux
+  // blocks, bit 1 u and u_n
+  const auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };
+  const int bulk = (al16(d_fs) ? 1 : 0) | ((S::EV % 2 == 0 && al16(d_u) && (d_un == nullptr || al16(d_un))) ? 2 : 0);
   auto fn = fr_rhs_kernel<DIM, P1, S::REG>::get();
   LT_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int per_sm = 0;
   LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, warps * 32, smem));
   if (per_sm < 1) per_sm = 1;
   fn<<<t->num_sms * per_sm, warps * 32, smem, t->stream>>>(t->g, t->keys[t->cur], t->d_s, d_u, d_fs, d_R, w0, w1,
-                                                            w2, d_un, ca, cb, dt, d_uf_out);
+                                                            w2, d_un, ca, cb, dt, d_uf_out, bulk);
   return LT_OK;
 }
 
