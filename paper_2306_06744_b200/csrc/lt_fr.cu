@@ -505,6 +505,152 @@ __global__ void __launch_bounds__(256, 2) k_fr_rhs_p3(const uint64_t* __restrict
   }
 }
 
+
+// 3-D p = 2 -- the order of the paper's own 3-D runs (Table 5) -- register-resident like
+// k_fr_rhs_p3: lane i < 27 owns solution point i = x + 3 (y + 3 z) with all five variables, so the point
+// fluxes need no shared memory; a line along axis a is the three lanes base + j * 3^a, whose fluxes are
+// exchanged by warp shuffles (lanes 27-31 shuffle along and store nothing).  Only the six flux blocks
+// (2160 bytes, one cp.async.bulk when BULK) go through shared memory; u and u_n of the warp's next element
+// are loaded into registers when the tail of the current one begins.
+template <bool BULK>
+__global__ void __launch_bounds__(256, 2) k_fr_rhs_p2(const uint64_t* __restrict__ keys, const DevScalars* s,
+                                                      const double* u, const double* fs, double* R, double w0,
+                                                      double w1, double w2, const double* un, double ca, double cb,
+                                                      double dt, double* uf_out) {
+  constexpr int DIM = 3, P1 = 3, NV = 5, N = 27, Nf = 9, EV = 135, E = NV * Nf, FB = 6 * E;
+  constexpr int CP = P1 + 2, CT = P1 * CP;
+  constexpr unsigned FULL = 0xffffffffu;
+  extern __shared__ __align__(128) double sm_p2[];  // [warps]: f*[FB]
+  __shared__ double sc[CT + 2 * P1];  // D'[i][0..2] | g_L'(z_i) | g_R'(z_i) per row, then l(-1), l(+1)
+  __shared__ uint64_t bars[8];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  double* sfs = sm_p2 + (size_t)w * FB;
+  uint64_t* bar = &bars[w];
+  uint32_t phase = 0;
+  if (BULK && lane == 0) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  auto fetch_fluxes = [&](int64_t el) {
+    if (BULK) {
+      if (lane == 0) {
+        mbar_arrive_expect_tx(bar, FB * 8);
+        bulk_g2s(sfs, fs + (size_t)el * FB, FB * 8, bar);
+      }
+    } else {
+      for (int i = lane; i < FB; i += 32) cp_async8(sfs + i, fs + (size_t)el * FB + i);
+    }
+  };
+  {
+    const FrConst& c = c_fr[P1 - 1];
+    for (int t = threadIdx.x; t < CT + 2 * P1; t += blockDim.x) {
+      if (t < CT) {
+        const int i = t / CP, j = t - i * CP;
+        sc[t] = j < P1 ? c.Dp[i][j] : (j == P1 ? c.gl[i] : c.gr[i]);
+      } else {
+        const int j = t - CT;
+        sc[t] = j < P1 ? c.lm[j] : c.lp[j - P1];
+      }
+    }
+  }
+  __syncthreads();
+  const bool live = lane < N;
+  const int pi = live ? lane : 0;  // (the idle lanes mirror point 0)
+  const int cx = pi % 3, cy = (pi / 3) % 3, cz = pi / 9;
+  const int64_t n = s->n;
+  const int64_t nw = (int64_t)gridDim.x * (blockDim.x >> 5);
+  const bool stage = un != nullptr;
+  int64_t e = (int64_t)blockIdx.x * (blockDim.x >> 5) + w;
+  double nu[NV], nn[NV];  // u and u_n of the element about to be processed
+  if (e < n) {
+    fetch_fluxes(e);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+      nu[v] = __ldcs(u + (size_t)e * EV + v * N + pi);
+      nn[v] = stage ? __ldcs(un + (size_t)e * EV + v * N + pi) : 0.0;
+    }
+  }
+  cp_async_commit();
+  for (; e < n; e += nw) {
+    const int64_t e_next = e + nw;
+    double uo[NV], acc[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+      uo[v] = nu[v];
+      acc[v] = stage ? ca * nn[v] + cb * nu[v] : 0.0;
+    }
+    if (BULK) {
+      while (!mbar_try_wait(bar, phase)) {
+      }
+      phase ^= 1;
+    } else {
+      cp_async_wait_all();
+      __syncwarp();
+    }
+    const int level = key_level(keys[e]);
+    const double inv2l = (double)(1ull << level);
+    const double wgt = stage ? cb * dt : 1.0;
+#pragma unroll
+    for (int a = 0; a < DIM; ++a) {
+      const double scale = wgt * 2.0 * inv2l / (a == 0 ? w0 : (a == 1 ? w1 : w2));  // (cb dt) 2 / dx
+      double F[NV];
+      euler_flux<DIM>(a, uo, F);
+      const int stride = a == 0 ? 1 : (a == 1 ? 3 : 9);
+      const int idx = a == 0 ? cx : (a == 1 ? cy : cz);
+      const int base = pi - idx * stride;
+      const int nt = a == 0 ? cy + 3 * cz : (a == 1 ? cx + 3 * cz : cx + 3 * cy);  // lower tangential axis fastest
+      const double* row = sc + idx * CP;
+      const double* fsm = sfs + 2 * a * E;  // common flux on the - face: [v][nt]
+      const double* fsp = fsm + E;          // and on the + face
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        double d = row[P1] * fsm[v * Nf + nt];
+        d += row[P1 + 1] * fsp[v * Nf + nt];
+#pragma unroll
+        for (int j = 0; j < P1; ++j) d += row[j] * __shfl_sync(FULL, F[v], base + j * stride);
+        acc[v] -= scale * d;
+      }
+    }
+    __syncwarp();
+    if (e_next < n) {  // the flux blocks are dead: the next element's; its u and u_n go to registers
+      fetch_fluxes(e_next);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        nu[v] = __ldcs(u + (size_t)e_next * EV + v * N + pi);
+        nn[v] = stage ? __ldcs(un + (size_t)e_next * EV + v * N + pi) : 0.0;
+      }
+    }
+    cp_async_commit();
+    if (live) {
+      double* dst = R + (size_t)e * EV;
+#pragma unroll
+      for (int v = 0; v < NV; ++v) __stcs(dst + v * N + pi, acc[v]);
+    }
+    if (uf_out != nullptr) {
+      // Alg. 8 step 1 for the next stage: u_out at the face points; the lane at position 0 of its line
+      // forms the trace on the - face, the one at position 1 the trace on the + face
+      double* fd = uf_out + (size_t)e * FB;
+      const double* lm = sc + CT;
+      const double* lp = lm + P1;
+#pragma unroll
+      for (int a = 0; a < DIM; ++a) {
+        const int stride = a == 0 ? 1 : (a == 1 ? 3 : 9);
+        const int idx = a == 0 ? cx : (a == 1 ? cy : cz);
+        const int base = pi - idx * stride;
+        const int nt = a == 0 ? cy + 3 * cz : (a == 1 ? cx + 3 * cz : cx + 3 * cy);
+        const double* cf = idx == 0 ? lm : lp;
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+          double t = 0.0;
+#pragma unroll
+          for (int j = 0; j < P1; ++j) t += cf[j] * __shfl_sync(FULL, acc[v], base + j * stride);
+          if (live && idx < 2) __stcs(fd + (2 * a + idx) * E + v * Nf + nt, t);
+        }
+      }
+    }
+  }
+}
+
 // The same for larger blocks (3-D, p >= 4): right-hand side accumulated in shared memory, synchronous loads.
 template <int DIM, int P1>
 __global__ void __launch_bounds__(256) k_fr_rhs_big(Geo g, const uint64_t* __restrict__ keys, const DevScalars* s,
@@ -741,6 +887,22 @@ static int launch_fr_rhs_t(Tree* t, const double* d_u, const double* d_fs, doubl
                                                                          w1, w2, d_un, ca, cb, dt, d_uf_out);
     else
       k_fr_rhs_p3<false><<<t->num_sms * per_sm3, 256, smem3, t->stream>>>(t->keys[t->cur], t->d_s, d_u, d_fs, d_R, w0,
+                                                                          w1, w2, d_un, ca, cb, dt, d_uf_out);
+    return LT_OK;
+  }
+  if (DIM == 3 && P1 == 3) {
+    const size_t smem2 = (size_t)8 * 6 * S::NV * S::Nf * sizeof(double);
+    static int per_sm2 = 0;
+    if (per_sm2 == 0) {
+      int q = 0;
+      LT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&q, k_fr_rhs_p2<true>, 256, smem2));
+      per_sm2 = q < 1 ? 1 : q;
+    }
+    if ((reinterpret_cast<uintptr_t>(d_fs) & 15) == 0)  // cp.async.bulk needs 16-byte aligned addresses
+      k_fr_rhs_p2<true><<<t->num_sms * per_sm2, 256, smem2, t->stream>>>(t->keys[t->cur], t->d_s, d_u, d_fs, d_R, w0,
+                                                                         w1, w2, d_un, ca, cb, dt, d_uf_out);
+    else
+      k_fr_rhs_p2<false><<<t->num_sms * per_sm2, 256, smem2, t->stream>>>(t->keys[t->cur], t->d_s, d_u, d_fs, d_R, w0,
                                                                           w1, w2, d_un, ca, cb, dt, d_uf_out);
     return LT_OK;
   }
